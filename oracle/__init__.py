@@ -1,0 +1,231 @@
+"""CPU oracle (TEST INFRASTRUCTURE, NOT PRODUCT) — ctypes access to oracle/metad_oracle.c.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  It never imports the CUDA binding, and the CUDA binding never imports it.
+All arithmetic is in metad_oracle.c (fp64, -ffp-contract=off); this file only marshals numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "metad_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+                               "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+_lib = None
+_P = ctypes.c_void_p
+_I = ctypes.c_int
+_D = ctypes.c_double
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        L.orc_num_threads.restype = _I
+        L.orc_set_threads.argtypes = [_I]
+        L.orc_box_check.restype = _I
+        L.orc_box_check.argtypes = [_P, _D, _P]
+        L.orc_delta.argtypes = [_P, _P, _P, _P]
+        for f in (L.orc_neighbors_brute, L.orc_neighbors_images, L.orc_neighbors_cells):
+            f.restype = _I
+            f.argtypes = [_I, _P, _P, _D, _I, _P, _P]
+        L.orc_switch.restype = _D
+        L.orc_switch.argtypes = [_D, _I, _I, _P]
+        L.orc_cv_coord.restype = _D
+        L.orc_cv_coord.argtypes = [_I, _P, _P, _P, _P, _I, _P, _D, _I, _I, _D, _P]
+        L.orc_q6_atoms.argtypes = [_I, _P, _P, _P, _P, _I, _P]
+        L.orc_q6_grad.argtypes = [_I, _P, _P, _P, _P, _I, _P, _P, _P]
+        L.orc_y6.argtypes = [_P, _P]
+        L.orc_q6_atoms_ylm.argtypes = [_I, _P, _P, _P, _P, _I, _P, _P]
+        L.orc_cv_rgyr.restype = _D
+        L.orc_cv_rgyr.argtypes = [_I, _P, _P, _P, _P, _P]
+        L.orc_cv_contacts.restype = _D
+        L.orc_cv_contacts.argtypes = [_I, _I, _P, _P, _I, _I, _D, _P, _P, _P]
+        L.orc_bias.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P]
+        L.orc_wt_height.restype = _D
+        L.orc_wt_height.argtypes = [_D, _D, _D, _D]
+        L.orc_grid_add.argtypes = [_I, _I, _P, _P, _I, _I, _P, _P, _P, _P]
+        L.orc_grid_eval.restype = _I
+        L.orc_grid_eval.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P]
+        L.orc_apply_forces.argtypes = [_I, _I, _P, _P, _D, _P]
+        _lib = L
+    return _lib
+
+
+def _f(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data
+
+
+def num_threads():
+    return lib().orc_num_threads()
+
+
+def set_threads(n):
+    lib().orc_set_threads(int(n))
+
+
+def box_check(box, rc):
+    w = np.zeros(3)
+    rcode = lib().orc_box_check(_p(_f(box)), float(rc), _p(w))
+    return rcode, w
+
+
+def delta(box, ri, rj):
+    d = np.zeros(3)
+    box, ri, rj = _f(box), _f(ri), _f(rj)
+    lib().orc_delta(_p(box), _p(ri), _p(rj), _p(d))
+    return d
+
+
+def neighbors(pos, box, rc, maxn, method="cells"):
+    """Returns (count[N] int32, list[N,maxn] int32 row-major ascending j, max_count)."""
+    pos, box = _f(pos), _f(box)
+    N = len(pos)
+    count = np.zeros(N, dtype=np.int32)
+    lst = np.full((N, maxn), -1, dtype=np.int32)
+    fn = {"cells": lib().orc_neighbors_cells, "brute": lib().orc_neighbors_brute,
+          "images": lib().orc_neighbors_images}[method]
+    mx = fn(N, _p(pos), _p(box), float(rc), int(maxn), _p(count), _p(lst))
+    if mx < 0:
+        raise ValueError("invalid box / cutoff")
+    return count, lst, mx
+
+
+def switch(x, n, m):
+    d = ctypes.c_double(0.0)
+    v = lib().orc_switch(float(x), int(n), int(m), ctypes.addressof(d))
+    return v, d.value
+
+
+def make_flags(N, group_a, group_b):
+    """bit0 = in A, bit1 = in B; None = all atoms (reading C)."""
+    if group_a is None and group_b is None:
+        return None
+    fl = np.zeros(N, dtype=np.uint8)
+    if group_a is None:
+        fl |= 1
+    else:
+        fl[np.asarray(group_a)] |= 1
+    if group_b is None:
+        fl |= 2
+    else:
+        fl[np.asarray(group_b)] |= 2
+    return fl
+
+
+def cv_coord(pos, box, count, lst, r0, n, m, scale, flags=None, want_grad=True):
+    pos, box = _f(pos), _f(box)
+    N = len(pos)
+    grad = np.zeros((N, 3)) if want_grad else None
+    s = lib().orc_cv_coord(N, _p(pos), _p(box), _p(count), _p(lst), lst.shape[1], _p(flags),
+                           float(r0), int(n), int(m), float(scale), _p(grad))
+    return s, grad
+
+
+def q6_atoms(pos, box, count, lst):
+    pos, box = _f(pos), _f(box)
+    q = np.zeros(len(pos))
+    lib().orc_q6_atoms(len(pos), _p(pos), _p(box), _p(count), _p(lst), lst.shape[1], _p(q))
+    return q
+
+
+def q6_grad(pos, box, count, lst, q6, w):
+    pos, box, q6, w = _f(pos), _f(box), _f(q6), _f(w)
+    g = np.zeros((len(pos), 3))
+    lib().orc_q6_grad(len(pos), _p(pos), _p(box), _p(count), _p(lst), lst.shape[1], _p(q6), _p(w), _p(g))
+    return g
+
+
+def y6(u):
+    u = _f(u)
+    y = np.zeros(14)
+    lib().orc_y6(_p(u), _p(y))
+    return y[0::2] + 1j * y[1::2]
+
+
+def q6_atoms_ylm(pos, box, count, lst):
+    pos, box = _f(pos), _f(box)
+    q = np.zeros(len(pos))
+    y = np.zeros((len(pos), 14))
+    lib().orc_q6_atoms_ylm(len(pos), _p(pos), _p(box), _p(count), _p(lst), lst.shape[1], _p(q), _p(y))
+    return q, y[:, 0::2] + 1j * y[:, 1::2]
+
+
+def cv_rgyr(pos, box, chain, mass=None, want_grad=True):
+    pos, box, chain = _f(pos), _f(box), _i(chain)
+    mass = None if mass is None else _f(mass)
+    g = np.zeros((len(chain), 3)) if want_grad else None
+    rg = lib().orc_cv_rgyr(len(chain), _p(chain), _p(mass), _p(pos), _p(box), _p(g))
+    return rg, g
+
+
+def cv_contacts(pos, box, pairs, pair_r0, n, m, scale, want_grad=True):
+    pos, box, pairs, pair_r0 = _f(pos), _f(box), _i(pairs), _f(pair_r0)
+    g = np.zeros((len(pos), 3)) if want_grad else None
+    q = lib().orc_cv_contacts(len(pos), len(pairs), _p(pairs), _p(pair_r0), int(n), int(m), float(scale),
+                              _p(pos), _p(box), _p(g))
+    return q, g
+
+
+def bias(centers, heights, sigma, s):
+    centers, heights, sigma, s = _f(centers), _f(heights), _f(sigma), _f(np.atleast_1d(s))
+    D = len(sigma)
+    H = len(heights)
+    centers = centers.reshape(H, D)
+    V = ctypes.c_double(0.0)
+    dV = np.zeros(D)
+    lib().orc_bias(D, H, _p(centers), _p(heights), _p(sigma), _p(s), ctypes.addressof(V), _p(dV))
+    return V.value, dV
+
+
+def wt_height(w0, V, kT, gamma):
+    return lib().orc_wt_height(float(w0), float(V), float(kT), float(gamma))
+
+
+def grid_add(table, lo, hi, centers, heights, sigma, k0=0, k1=None):
+    """table: float64 [4,n0,n1], modified in place."""
+    lo, hi, centers, heights, sigma = _f(lo), _f(hi), _f(centers), _f(heights), _f(sigma)
+    if k1 is None:
+        k1 = len(heights)
+    assert table.dtype == np.float64 and table.flags.c_contiguous and table.shape[0] == 4
+    lib().orc_grid_add(table.shape[1], table.shape[2], _p(lo), _p(hi), int(k0), int(k1), _p(centers),
+                       _p(heights), _p(sigma), _p(table))
+    return table
+
+
+def grid_eval(table, lo, hi, s):
+    lo, hi, s = _f(lo), _f(hi), _f(s)
+    V = ctypes.c_double(0.0)
+    dV = np.zeros(2)
+    out = lib().orc_grid_eval(table.shape[1], table.shape[2], _p(lo), _p(hi), _p(table), _p(s),
+                              ctypes.addressof(V), _p(dV))
+    return out, V.value, dV
+
+
+def apply_forces(F, dVds, grads, force_scale=1.0):
+    """F (N,3) float64 modified in place; grads (D,N,3)."""
+    grads, dVds = _f(grads), _f(np.atleast_1d(dVds))
+    assert F.dtype == np.float64 and F.flags.c_contiguous
+    lib().orc_apply_forces(len(F), len(dVds), _p(dVds), _p(grads), float(force_scale), _p(F))
+    return F
