@@ -1,0 +1,162 @@
+/* metad.h — C ABI of the B200-native per-step metadynamics hot path (GPU-MetaD, arxiv 2510.06873).
+ *
+ * One context = one simulated system on one GPU.  Per MD step the caller issues, in this order
+ * (DESIGN.md §3 reading U; "end-to-end ... entirely implemented on GPUs"):
+ *
+ *     metad_build_neighbors -> metad_eval_cv -> metad_bias -> metad_apply_forces -> metad_deposit
+ *
+ * or metad_run(), which captures those five in a CUDA graph and replays it n times with zero host
+ * round trips.  Every hot-path call only ENQUEUES kernels on the context's stream and returns;
+ * nothing synchronises or copies to the host except the calls marked [sync].
+ *
+ * Pointers: "d_" = device pointer owned by the caller (never freed / reallocated by the library),
+ * "h_" = host pointer.  Plain pointers without a prefix in metad_params are HOST pointers read
+ * (copied) during metad_create only.  All scratch memory is allocated in metad_create.
+ *
+ * Precision: params.precision = 64 -> positions / forces are double[N][3]; 32 -> float[N][3]
+ * ("fp32 pair math with fp64 reductions", BASELINE.json configs[4]).  CV values, V, dV/ds, hills,
+ * grid and all reductions are double in both modes.
+ *
+ * Box: 9 doubles on the HOST, rows a=(ax,0,0), b=(bx,by,0), c=(cx,cy,cz) (lower-triangular;
+ * orthorhombic = diagonal).  Positions must lie in the primary cell (fractional coords in [0,1),
+ * up to rounding).  Requires rc < half of every perpendicular box width (else METAD_ERR_BOX).
+ *
+ * Return value: 0 (METAD_OK) or a metad_error.  Device-side conditions (neighbour-list overflow,
+ * hill-array overflow, grid out of range, non-finite CV) never abort: they set sticky bits read by
+ * metad_status(), and the kernels continue with defined behaviour (excess neighbours / hills are
+ * dropped, out-of-grid points fall back to the exact hill sum).
+ */
+#ifndef METAD_B200_H
+#define METAD_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct metad_ctx metad_ctx;
+
+enum metad_error { METAD_OK = 0, METAD_ERR_ARG = 1, METAD_ERR_BOX = 2, METAD_ERR_STATE = 3,
+                   METAD_ERR_CUDA = 4, METAD_ERR_NOMEM = 5 };
+
+enum metad_dev_bits { METAD_DEV_NEIGH_OVERFLOW = 1, METAD_DEV_HILL_OVERFLOW = 2,
+                      METAD_DEV_GRID_RANGE = 4, METAD_DEV_NONFINITE = 8 };
+
+enum metad_cv_kind {
+    METAD_CV_COORD = 0,    /* s = scale * sum_{i in A} sum_{j in B, j!=i, r<rc} sw(r_ij/r0),
+                              sw(x) = (1-x^n)/(1-x^m)           (BASELINE.json configs[0],[2]) */
+    METAD_CV_Q6_MEAN = 1,  /* s = scale * sum_i q6(i), Steinhardt q6 over hard-cutoff neighbours
+                              (BASELINE.json configs[3]; reading E); scale = 1/N for the mean   */
+    METAD_CV_Q6_SOLID = 2, /* s = scale * sum_i 1/(1+exp(-(q6(i)-q_thresh)/q_width))
+                              (BASELINE.json configs[4]; reading F)                                        */
+    METAD_CV_RGYR = 3,     /* radius of gyration of an ordered chain, unwrapped by sequential minimum
+                              image (BASELINE.json configs[1]; reading G)                                  */
+    METAD_CV_CONTACTS = 4  /* s = scale * sum_p sw(r_p / r0_p), n, m as given (configs[1]; reading H)      */
+};
+
+typedef struct {
+    int kind;                       /* metad_cv_kind */
+    int n, m;                       /* switching exponents (COORD, CONTACTS) */
+    double r0;                      /* switching length (COORD) */
+    double scale;                   /* normalisation, see metad_cv_kind */
+    const int *group_a; int n_a;    /* COORD: host index lists; NULL = all atoms */
+    const int *group_b; int n_b;
+    const int *pairs;               /* CONTACTS: host int[2*npairs] */
+    const double *pair_r0;          /* CONTACTS: host double[npairs] */
+    int npairs;
+    const int *chain; int nchain;   /* RGYR: host ordered atom indices */
+    const double *mass;             /* RGYR: host double[nchain] or NULL (equal masses) */
+    double q_thresh, q_width;       /* Q6_SOLID */
+} metad_cv_desc;
+
+#define METAD_MAX_CV 4
+
+typedef struct {
+    int natoms;
+    int precision;                  /* 32 or 64: dtype of pos / F and of the pair arithmetic */
+    int max_neigh;                  /* neighbour-list capacity per atom */
+    int ncv;                        /* 1..METAD_MAX_CV */
+    metad_cv_desc cv[METAD_MAX_CV];
+    double sigma[METAD_MAX_CV];     /* Gaussian width per CV dimension */
+    double w0;                      /* initial hill height (PAPER.md:37 W_k) */
+    double kT;                      /* k_B T in the hill energy unit */
+    double bias_factor;             /* gamma; <= 1 -> plain metadynamics (reading I) */
+    int max_hills;                  /* hill-array capacity */
+    int stride;                     /* deposit every `stride` steps; 0 = never ("periodically") */
+    int grid_n[2];                  /* grid_n[0] == 0 -> exact hill sum; else ncv must be 2 (reading M) */
+    double grid_lo[2], grid_hi[2];
+    double force_scale;             /* F += -force_scale * dV/dr (unit conversion; reading N) */
+} metad_params;
+
+/* Creates a context on the current CUDA device; `cuda_stream` is a cudaStream_t (NULL = default
+ * stream) on which every later call is enqueued.  [sync] */
+int metad_create(metad_ctx **out, const metad_params *params, void *cuda_stream);
+int metad_destroy(metad_ctx *ctx);
+
+/* a1 (BASELINE.json north_star "build the neighbour list"; reading O, P): bins atoms into cells,
+ * counting-sorts them, and builds the full neighbour list (all j != i with minimum-image
+ * r_ij < rc, strict).  Snapshots the positions: later calls of this step use them.
+ * d_pos: [N][3] in params.precision.  box: host.  Errors: METAD_ERR_BOX, METAD_ERR_ARG. */
+int metad_build_neighbors(metad_ctx *ctx, const void *d_pos, const double *h_box, double rc);
+
+/* a2-a4: evaluates all CVs; d_cv: double[ncv] (device, caller-owned). */
+int metad_eval_cv(metad_ctx *ctx, double *d_cv);
+
+/* a5: V(s) = sum_k w_k prod_d exp(-(s_d-c_kd)^2/(2 sigma_d^2)) and dV/ds_d at
+ * the point d_cv[ncv] over the hills deposited so far (through the grid if enabled).
+ * d_V: double[1], d_dVds: double[ncv]. */
+int metad_bias(metad_ctx *ctx, const double *d_cv, double *d_V, double *d_dVds);
+
+/* a6: F_i += -force_scale * sum_d d_dVds[d] * d s_d / d r_i for the CVs evaluated
+ * by the last metad_eval_cv.  Gather form, deterministic, no float atomics.
+ * d_F: [N][3] in params.precision, read-modify-write. */
+int metad_apply_forces(metad_ctx *ctx, const double *d_dVds, void *d_F);
+
+/* a7 ("periodically depositing"; PAPER.md:43 well-tempered; readings I, J, U):
+ * advances the device step counter; if (step % stride == 0) appends the hill
+ * (d_cv, w0 * exp(-V/((gamma-1) kT))) and, in grid mode, adds it to the table. */
+int metad_deposit(metad_ctx *ctx, const double *d_cv, const double *d_V);
+
+/* The five calls above for nsteps steps as one CUDA graph replayed nsteps times (fixed d_pos:
+ * positions are an input of this library, the MD integrator is out of scope).  Results of the last
+ * step are in the context (metad_get_state). */
+int metad_run(metad_ctx *ctx, const void *d_pos, const double *h_box, double rc, void *d_F, int nsteps);
+
+/* One step with HOST buffers (end-to-end path): copies h_pos -> device, h_F -> device, runs the
+ * five stages, copies F, cv[ncv] and V back.  [sync] */
+int metad_step_host(metad_ctx *ctx, const void *h_pos, const double *h_box, double rc, void *h_F,
+                    double *h_cv, double *h_V);
+
+/* [sync] ORs the sticky device bits into *bits (and clears nothing). */
+int metad_status(metad_ctx *ctx, unsigned *bits);
+
+/* [sync] last step's cv[ncv], V, dVds[ncv], step counter, hill count (any pointer may be NULL). */
+int metad_get_state(metad_ctx *ctx, double *h_cv, double *h_V, double *h_dVds, int *h_step, int *h_nhills);
+
+/* Neighbour list in ORIGINAL atom indices: d_count int[N], d_list int[N][max_neigh] row-major
+ * (unused slots = -1, order within a row unspecified).  Enqueued, not synchronised. */
+int metad_get_neighbors(metad_ctx *ctx, int *d_count, int *d_list);
+
+/* Per-atom q6 of the last metad_eval_cv in original atom order (d_q6: [N] in params.precision). */
+int metad_get_q6(metad_ctx *ctx, void *d_q6);
+
+/* Hills: centers [count][ncv] row-major, heights [count].  on_device: pointers are device (1) or
+ * host (0).  set_hills replaces all hills (and rebuilds the grid table).  [sync] */
+int metad_set_hills(metad_ctx *ctx, const double *centers, const double *heights, int count, int on_device);
+int metad_get_hills(metad_ctx *ctx, double *centers, double *heights, int capacity, int *count, int on_device);
+
+/* Grid table [4][n0][n1] = V, dV/ds0, dV/ds1, d2V/ds0ds1 at the nodes; copied to d_table. */
+int metad_get_grid(metad_ctx *ctx, double *d_table);
+
+/* Resets the step counter (hills stay). */
+int metad_reset_steps(metad_ctx *ctx);
+
+/* Number of kernels the library has launched on this context so far (graph replays included). */
+long long metad_launch_count(metad_ctx *ctx);
+
+const char *metad_version(void);
+const char *metad_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

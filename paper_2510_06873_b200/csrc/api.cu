@@ -1,0 +1,410 @@
+// api.cu — the C ABI of include/metad.h: context, argument checks, CUDA-graph step loop.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <algorithm>
+#include <vector>
+#include "common.cuh"
+
+static thread_local char g_err[512] = "";
+void metad_set_error(const char *msg) { snprintf(g_err, sizeof(g_err), "%s", msg ? msg : ""); }
+extern "C" const char *metad_last_error(void) { return g_err; }
+extern "C" const char *metad_version(void) { return "metad-b200 0.1 (sm_100a)"; }
+
+
+#define FAIL(code, msg) do { metad_set_error(msg); return code; } while (0)
+
+template <typename X>
+static cudaError_t dev_alloc(X **p, size_t n) { return cudaMalloc((void **)p, sizeof(X) * (n ? n : 1)); }
+
+static int upload_ints(int **dst, const int *src, size_t n) {
+    CUDA_TRY(dev_alloc(dst, n));
+    CUDA_TRY(cudaMemcpy(*dst, src, sizeof(int) * n, cudaMemcpyHostToDevice));
+    return METAD_OK;
+}
+static int upload_doubles(double **dst, const double *src, size_t n) {
+    CUDA_TRY(dev_alloc(dst, n));
+    CUDA_TRY(cudaMemcpy(*dst, src, sizeof(double) * n, cudaMemcpyHostToDevice));
+    return METAD_OK;
+}
+
+extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_stream) {
+    if (!out || !p) FAIL(METAD_ERR_ARG, "null argument");
+    if (p->natoms <= 0) FAIL(METAD_ERR_ARG, "natoms must be positive");
+    if (p->precision != 32 && p->precision != 64) FAIL(METAD_ERR_ARG, "precision must be 32 or 64");
+    if (p->ncv < 1 || p->ncv > METAD_MAX_CV) FAIL(METAD_ERR_ARG, "ncv out of range");
+    if (p->max_neigh < 1 || p->max_hills < 1) FAIL(METAD_ERR_ARG, "max_neigh / max_hills must be positive");
+    for (int d = 0; d < p->ncv; ++d)
+        if (!(p->sigma[d] > 0.0)) FAIL(METAD_ERR_ARG, "sigma must be positive");
+    if (p->grid_n[0] != 0 && (p->ncv != 2 || p->grid_n[0] < 2 || p->grid_n[1] < 2 ||
+                              !(p->grid_hi[0] > p->grid_lo[0]) || !(p->grid_hi[1] > p->grid_lo[1])))
+        FAIL(METAD_ERR_ARG, "grid needs ncv == 2, n >= 2 and hi > lo");
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0)
+        FAIL(METAD_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
+
+    metad_ctx *c = new metad_ctx();
+    memset(c, 0, sizeof(*c));
+    c->p = *p;
+    c->N = p->natoms; c->prec = p->precision; c->maxn = p->max_neigh; c->D = p->ncv;
+    if (c->p.force_scale == 0.0) c->p.force_scale = 1.0;
+    c->stream = (cudaStream_t)cuda_stream;
+    if (!c->stream) CUDA_TRY(cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking));
+    c->q6_mean_dim = c->q6_solid_dim = c->coord_dim = -1;
+    const int N = c->N;
+    const size_t tsz = c->prec == 32 ? sizeof(float) : sizeof(double);
+
+    // ---- CV descriptors
+    std::vector<unsigned char> flags;
+    for (int d = 0; d < c->D; ++d) {
+        const metad_cv_desc &s = p->cv[d];
+        CvDev &v = c->cv[d];
+        v.kind = s.kind; v.n = s.n; v.m = s.m; v.r0 = s.r0; v.scale = s.scale;
+        v.q_thresh = s.q_thresh; v.q_width = s.q_width;
+        switch (s.kind) {
+        case METAD_CV_COORD: {
+            if (c->coord_dim >= 0) FAIL(METAD_ERR_ARG, "only one COORD CV per context");
+            if (!(s.r0 > 0.0) || s.n < 1 || s.m <= s.n) FAIL(METAD_ERR_ARG, "COORD needs r0 > 0, 0 < n < m");
+            c->coord_dim = d; c->has_coord = true;
+            v.use_groups = s.group_a || s.group_b;
+            if (v.use_groups) {
+                flags.assign(N, 0);
+                if (s.group_a) { for (int k = 0; k < s.n_a; ++k) { int i = s.group_a[k]; if (i < 0 || i >= N) FAIL(METAD_ERR_ARG, "group index"); flags[i] |= 1; } }
+                else for (int i = 0; i < N; ++i) flags[i] |= 1;
+                if (s.group_b) { for (int k = 0; k < s.n_b; ++k) { int i = s.group_b[k]; if (i < 0 || i >= N) FAIL(METAD_ERR_ARG, "group index"); flags[i] |= 2; } }
+                else for (int i = 0; i < N; ++i) flags[i] |= 2;
+            }
+            break;
+        }
+        case METAD_CV_Q6_MEAN:
+            if (c->q6_mean_dim >= 0) FAIL(METAD_ERR_ARG, "only one Q6_MEAN CV per context");
+            c->q6_mean_dim = d; c->has_q6 = true; break;
+        case METAD_CV_Q6_SOLID:
+            if (c->q6_solid_dim >= 0) FAIL(METAD_ERR_ARG, "only one Q6_SOLID CV per context");
+            if (!(s.q_width > 0.0)) FAIL(METAD_ERR_ARG, "q_width must be positive");
+            c->q6_solid_dim = d; c->has_q6 = true; break;
+        case METAD_CV_RGYR: {
+            if (!s.chain || s.nchain < 1) FAIL(METAD_ERR_ARG, "RGYR needs a chain");
+            for (int k = 0; k < s.nchain; ++k) if (s.chain[k] < 0 || s.chain[k] >= N) FAIL(METAD_ERR_ARG, "chain index");
+            v.nchain = s.nchain;
+            if (upload_ints(&v.d_chain, s.chain, s.nchain)) return METAD_ERR_CUDA;
+            if (s.mass && upload_doubles(&v.d_mass, s.mass, s.nchain)) return METAD_ERR_CUDA;
+            CUDA_TRY(dev_alloc(&v.d_unwrapped, 3 * (size_t)s.nchain + 8));
+            break;
+        }
+        case METAD_CV_CONTACTS: {
+            if (!s.pairs || !s.pair_r0 || s.npairs < 1 || s.n < 1 || s.m <= s.n) FAIL(METAD_ERR_ARG, "CONTACTS needs pairs, r0, 0 < n < m");
+            v.npairs = s.npairs;
+            std::vector<std::pair<int, int>> inc;   // (atom, pair)
+            for (int q = 0; q < s.npairs; ++q) {
+                int a = s.pairs[2 * q], b = s.pairs[2 * q + 1];
+                if (a < 0 || a >= N || b < 0 || b >= N || a == b) FAIL(METAD_ERR_ARG, "pair index");
+                inc.push_back({ a, q }); inc.push_back({ b, q });
+            }
+            std::sort(inc.begin(), inc.end());
+            std::vector<int> atoms, off, prs;
+            for (size_t t = 0; t < inc.size(); ++t) {
+                if (t == 0 || inc[t].first != inc[t - 1].first) { atoms.push_back(inc[t].first); off.push_back((int)t); }
+                prs.push_back(inc[t].second);
+            }
+            off.push_back((int)inc.size());
+            v.ncatoms = (int)atoms.size();
+            if (upload_ints(&v.d_pairs, s.pairs, 2 * (size_t)s.npairs) || upload_doubles(&v.d_pair_r0, s.pair_r0, s.npairs) ||
+                upload_ints(&v.d_catoms, atoms.data(), atoms.size()) || upload_ints(&v.d_csr_off, off.data(), off.size()) ||
+                upload_ints(&v.d_csr_pair, prs.data(), prs.size()))
+                return METAD_ERR_CUDA;
+            break;
+        }
+        default: FAIL(METAD_ERR_ARG, "unknown CV kind");
+        }
+    }
+
+    // ---- buffers (everything the hot path needs; nothing is allocated later)
+    c->cell_cap = std::max(4 * N, 4096);
+    c->nblocks_atoms = div_up(N, 128) + 1;
+    int max_pair_blocks = 1;
+    for (int d = 0; d < c->D; ++d) max_pair_blocks = std::max(max_pair_blocks, div_up(c->cv[d].npairs, 256) + 1);
+    CUDA_TRY(dev_alloc(&c->d_cell_count, (size_t)c->cell_cap + 1));
+    CUDA_TRY(cudaMemset(c->d_cell_count, 0, sizeof(int) * ((size_t)c->cell_cap + 1)));
+    CUDA_TRY(dev_alloc(&c->d_cell_start, (size_t)c->cell_cap + 1));
+    CUDA_TRY(dev_alloc(&c->d_block_sums, (size_t)c->cell_cap / 1024 + 8));
+    CUDA_TRY(dev_alloc(&c->d_cell_of, N));
+    CUDA_TRY(dev_alloc(&c->d_slot, N));
+    CUDA_TRY(dev_alloc(&c->d_perm, N));
+    CUDA_TRY(dev_alloc(&c->d_scell, N));
+    CUDA_TRY(cudaMalloc(&c->d_spos, 4 * tsz * (size_t)N));
+    CUDA_TRY(dev_alloc(&c->d_nl_count, N));
+    CUDA_TRY(dev_alloc(&c->d_nl, (size_t)c->maxn * N));
+    if (!flags.empty()) {
+        CUDA_TRY(dev_alloc(&c->d_flags, N));
+        CUDA_TRY(cudaMemcpy(c->d_flags, flags.data(), N, cudaMemcpyHostToDevice));
+    }
+    if (c->has_q6) CUDA_TRY(cudaMalloc(&c->d_rec, METAD_NREC * tsz * (size_t)N));
+    CUDA_TRY(dev_alloc(&c->d_partials, 3 * (size_t)c->nblocks_atoms + max_pair_blocks));
+    CUDA_TRY(dev_alloc(&c->d_tickets, 16));
+    CUDA_TRY(cudaMemset(c->d_tickets, 0, sizeof(unsigned) * 16));
+    CUDA_TRY(dev_alloc(&c->d_centers, (size_t)c->D * p->max_hills));
+    CUDA_TRY(dev_alloc(&c->d_heights, p->max_hills));
+    CUDA_TRY(dev_alloc(&c->d_nhills, 1));
+    CUDA_TRY(dev_alloc(&c->d_step, 1));
+    CUDA_TRY(dev_alloc(&c->d_sticky, 1));
+    CUDA_TRY(cudaMemset(c->d_nhills, 0, sizeof(int)));
+    CUDA_TRY(cudaMemset(c->d_step, 0, sizeof(int)));
+    CUDA_TRY(cudaMemset(c->d_sticky, 0, sizeof(unsigned)));
+    CUDA_TRY(dev_alloc(&c->d_cv, METAD_MAX_CV));
+    CUDA_TRY(dev_alloc(&c->d_V, 1));
+    CUDA_TRY(dev_alloc(&c->d_dVds, METAD_MAX_CV));
+    CUDA_TRY(cudaMemset(c->d_cv, 0, sizeof(double) * METAD_MAX_CV));
+    CUDA_TRY(cudaMemset(c->d_V, 0, sizeof(double)));
+    CUDA_TRY(cudaMemset(c->d_dVds, 0, sizeof(double) * METAD_MAX_CV));
+    CUDA_TRY(dev_alloc(&c->d_bias_partials, 592 * (1 + METAD_MAX_CV)));
+    c->grid_on = p->grid_n[0] != 0;
+    if (c->grid_on) {
+        size_t nn = 4 * (size_t)p->grid_n[0] * p->grid_n[1];
+        CUDA_TRY(dev_alloc(&c->d_table, nn));
+        CUDA_TRY(cudaMemset(c->d_table, 0, sizeof(double) * nn));
+    }
+    CUDA_TRY(cudaMalloc(&c->d_pos_stage, 3 * tsz * (size_t)N));
+    CUDA_TRY(cudaMalloc(&c->d_F_stage, 3 * tsz * (size_t)N));
+    CUDA_TRY(dev_alloc(&c->d_aux, 4));
+    int aux0[4] = { 0, -1, 0, 0 };
+    CUDA_TRY(cudaMemcpy(c->d_aux, aux0, sizeof(aux0), cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaDeviceSynchronize());
+    *out = c;
+    return METAD_OK;
+}
+
+extern "C" int metad_destroy(metad_ctx *c) {
+    if (!c) return METAD_OK;
+    cudaStreamSynchronize(c->stream);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
+                     c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
+                     c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux };
+    for (void *q : ptrs) if (q) cudaFree(q);
+    for (int d = 0; d < c->D; ++d) {
+        CvDev &v = c->cv[d];
+        void *q2[] = { v.d_pairs, v.d_pair_r0, v.d_csr_off, v.d_csr_pair, v.d_catoms, v.d_chain, v.d_mass, v.d_unwrapped };
+        for (void *q : q2) if (q) cudaFree(q);
+    }
+    delete c;
+    return METAD_OK;
+}
+
+// host-side geometry: box checks (reading O) and the cell grid
+static int setup_geometry(metad_ctx *c, const double *box, double rc) {
+    if (!box) FAIL(METAD_ERR_ARG, "null box");
+    if (box[1] != 0.0 || box[2] != 0.0 || box[5] != 0.0) FAIL(METAD_ERR_BOX, "box must be lower-triangular (rows a,b,c)");
+    if (!(box[0] > 0.0) || !(box[4] > 0.0) || !(box[8] > 0.0)) FAIL(METAD_ERR_BOX, "box diagonal must be positive");
+    if (!(rc > 0.0)) FAIL(METAD_ERR_ARG, "rc must be positive");
+    const double ax = box[0], bx = box[3], by = box[4], cx = box[6], cy = box[7], cz = box[8];
+    const double vol = ax * by * cz;
+    // perpendicular widths: V / |b x c|, V / |c x a|, V / |a x b|
+    const double bxc[3] = { by * cz, -bx * cz, bx * cy - by * cx };
+    const double cxa[3] = { 0.0, cz * ax, -cy * ax };
+    double w[3];
+    w[0] = vol / sqrt(bxc[0] * bxc[0] + bxc[1] * bxc[1] + bxc[2] * bxc[2]);
+    w[1] = vol / sqrt(cxa[1] * cxa[1] + cxa[2] * cxa[2]);
+    w[2] = cz;
+    for (int d = 0; d < 3; ++d)
+        if (!(rc < 0.5 * w[d])) FAIL(METAD_ERR_BOX, "rc must be smaller than half of every perpendicular box width");
+    CellGrid g;
+    double shrink = 1.0;
+    for (;;) {
+        long long tot = 1;
+        for (int d = 0; d < 3; ++d) {
+            int n = (int)floor(w[d] / (rc * 1.000001 * shrink));
+            g.nc[d] = n < 1 ? 1 : n;
+            tot *= g.nc[d];
+        }
+        if (tot <= c->cell_cap) { g.ncell = (int)tot; break; }
+        shrink *= 1.26;   // cells larger than rc are still valid; keeps ncell within the fixed allocation
+    }
+    g.inv[0] = 1.0 / ax; g.inv[1] = 1.0 / by; g.inv[2] = 1.0 / cz;
+    g.inv[3] = g.inv[4] = g.inv[5] = 0.0;
+    g.cx = cx; g.cy = cy; g.bx = bx;
+    c->grid = g;
+    BoxD b = { ax, bx, by, cx, cy, cz, 0.5 * ax, 0.5 * by, 0.5 * cz };
+    c->boxd = b;
+    c->rc = rc; c->rc2 = rc * rc;
+    return METAD_OK;
+}
+
+extern "C" int metad_build_neighbors(metad_ctx *c, const void *d_pos, const double *h_box, double rc) {
+    if (!c || !d_pos) FAIL(METAD_ERR_ARG, "null argument");
+    int r = setup_geometry(c, h_box, rc);
+    if (r) return r;
+    c->d_pos_last = d_pos;
+    r = nb_build(c, d_pos);
+    if (r == METAD_OK) c->have_neighbors = true;
+    return r;
+}
+
+extern "C" int metad_eval_cv(metad_ctx *c, double *d_cv) {
+    if (!c || !d_cv) FAIL(METAD_ERR_ARG, "null argument");
+    if (!c->have_neighbors) FAIL(METAD_ERR_STATE, "metad_build_neighbors has not been called");
+    return cv_eval_all(c, d_cv);
+}
+
+extern "C" int metad_bias(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds) {
+    if (!c || !d_cv || !d_V || !d_dVds) FAIL(METAD_ERR_ARG, "null argument");
+    return bias_eval(c, d_cv, d_V, d_dVds);
+}
+
+extern "C" int metad_apply_forces(metad_ctx *c, const double *d_dVds, void *d_F) {
+    if (!c || !d_dVds || !d_F) FAIL(METAD_ERR_ARG, "null argument");
+    if (!c->have_neighbors) FAIL(METAD_ERR_STATE, "metad_build_neighbors has not been called");
+    return cv_forces_all(c, d_dVds, d_F);
+}
+
+extern "C" int metad_deposit(metad_ctx *c, const double *d_cv, const double *d_V) {
+    if (!c || !d_cv || !d_V) FAIL(METAD_ERR_ARG, "null argument");
+    return bias_deposit(c, d_cv, d_V);
+}
+
+static int enqueue_step(metad_ctx *c, const void *d_pos, const double *box, double rc, void *d_F) {
+    int r;
+    if ((r = metad_build_neighbors(c, d_pos, box, rc))) return r;
+    if ((r = metad_eval_cv(c, c->d_cv))) return r;
+    if ((r = metad_bias(c, c->d_cv, c->d_V, c->d_dVds))) return r;
+    if ((r = metad_apply_forces(c, c->d_dVds, d_F))) return r;
+    return metad_deposit(c, c->d_cv, c->d_V);
+}
+
+extern "C" int metad_run(metad_ctx *c, const void *d_pos, const double *h_box, double rc, void *d_F, int nsteps) {
+    if (!c || !d_pos || !d_F || !h_box || nsteps < 0) FAIL(METAD_ERR_ARG, "bad argument");
+    bool same = c->graph_exec && c->graph_pos == d_pos && c->graph_F == d_F && c->graph_rc == rc &&
+                memcmp(c->graph_box, h_box, sizeof(double) * 9) == 0;
+    if (!same) {
+        if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+        int r = setup_geometry(c, h_box, rc);     // argument errors surface before the capture starts
+        if (r) return r;
+        long long before = c->launches;
+        cudaGraph_t graph;
+        CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+        r = enqueue_step(c, d_pos, h_box, rc, d_F);
+        cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+        if (r) { if (e == cudaSuccess) cudaGraphDestroy(graph); return r; }
+        CUDA_TRY(e);
+        CUDA_TRY(cudaGraphInstantiate(&c->graph_exec, graph, 0));
+        cudaGraphDestroy(graph);
+        c->launches_per_step = (int)(c->launches - before);
+        c->launches = before;                      // capture enqueued nothing
+        c->graph_pos = d_pos; c->graph_F = d_F; c->graph_rc = rc;
+        memcpy(c->graph_box, h_box, sizeof(double) * 9);
+    }
+    for (int s = 0; s < nsteps; ++s) CUDA_TRY(cudaGraphLaunch(c->graph_exec, c->stream));
+    c->launches += (long long)c->launches_per_step * nsteps;
+    return METAD_OK;
+}
+
+extern "C" int metad_step_host(metad_ctx *c, const void *h_pos, const double *h_box, double rc, void *h_F,
+                               double *h_cv, double *h_V) {
+    if (!c || !h_pos || !h_F || !h_box) FAIL(METAD_ERR_ARG, "null argument");
+    const size_t bytes = 3 * (size_t)c->N * (c->prec == 32 ? sizeof(float) : sizeof(double));
+    CUDA_TRY(cudaMemcpyAsync(c->d_pos_stage, h_pos, bytes, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(c->d_F_stage, h_F, bytes, cudaMemcpyHostToDevice, c->stream));
+    int r = metad_run(c, c->d_pos_stage, h_box, rc, c->d_F_stage, 1);
+    if (r) return r;
+    CUDA_TRY(cudaMemcpyAsync(h_F, c->d_F_stage, bytes, cudaMemcpyDeviceToHost, c->stream));
+    if (h_cv) CUDA_TRY(cudaMemcpyAsync(h_cv, c->d_cv, sizeof(double) * c->D, cudaMemcpyDeviceToHost, c->stream));
+    if (h_V) CUDA_TRY(cudaMemcpyAsync(h_V, c->d_V, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return METAD_OK;
+}
+
+extern "C" int metad_status(metad_ctx *c, unsigned *bits) {
+    if (!c || !bits) FAIL(METAD_ERR_ARG, "null argument");
+    unsigned b = 0;
+    CUDA_TRY(cudaMemcpyAsync(&b, c->d_sticky, sizeof(unsigned), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    *bits |= b;
+    return METAD_OK;
+}
+
+extern "C" int metad_get_state(metad_ctx *c, double *h_cv, double *h_V, double *h_dVds, int *h_step, int *h_nhills) {
+    if (!c) FAIL(METAD_ERR_ARG, "null argument");
+    if (h_cv) CUDA_TRY(cudaMemcpyAsync(h_cv, c->d_cv, sizeof(double) * c->D, cudaMemcpyDeviceToHost, c->stream));
+    if (h_V) CUDA_TRY(cudaMemcpyAsync(h_V, c->d_V, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    if (h_dVds) CUDA_TRY(cudaMemcpyAsync(h_dVds, c->d_dVds, sizeof(double) * c->D, cudaMemcpyDeviceToHost, c->stream));
+    if (h_step) CUDA_TRY(cudaMemcpyAsync(h_step, c->d_step, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    if (h_nhills) CUDA_TRY(cudaMemcpyAsync(h_nhills, c->d_nhills, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return METAD_OK;
+}
+
+extern "C" int metad_get_neighbors(metad_ctx *c, int *d_count, int *d_list) {
+    if (!c || !d_count || !d_list) FAIL(METAD_ERR_ARG, "null argument");
+    if (!c->have_neighbors) FAIL(METAD_ERR_STATE, "metad_build_neighbors has not been called");
+    return nb_export(c, d_count, d_list);
+}
+
+extern "C" int metad_get_q6(metad_ctx *c, void *d_q6) {
+    if (!c || !d_q6) FAIL(METAD_ERR_ARG, "null argument");
+    return q6_export(c, d_q6);
+}
+
+extern "C" int metad_set_hills(metad_ctx *c, const double *centers, const double *heights, int count, int on_device) {
+    if (!c || count < 0 || (count > 0 && (!centers || !heights))) FAIL(METAD_ERR_ARG, "bad argument");
+    if (count > c->p.max_hills) FAIL(METAD_ERR_ARG, "count exceeds max_hills");
+    int r;
+    if (on_device || count == 0) {
+        r = bias_set_hills_dev(c, centers, heights, count);
+    } else {
+        double *dc = nullptr, *dh = nullptr;
+        CUDA_TRY(dev_alloc(&dc, (size_t)count * c->D));
+        CUDA_TRY(dev_alloc(&dh, count));
+        CUDA_TRY(cudaMemcpyAsync(dc, centers, sizeof(double) * (size_t)count * c->D, cudaMemcpyHostToDevice, c->stream));
+        CUDA_TRY(cudaMemcpyAsync(dh, heights, sizeof(double) * count, cudaMemcpyHostToDevice, c->stream));
+        r = bias_set_hills_dev(c, dc, dh, count);
+        cudaStreamSynchronize(c->stream);
+        cudaFree(dc); cudaFree(dh);
+    }
+    if (r) return r;
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return METAD_OK;
+}
+
+extern "C" int metad_get_hills(metad_ctx *c, double *centers, double *heights, int capacity, int *count, int on_device) {
+    if (!c) FAIL(METAD_ERR_ARG, "null argument");
+    int H = 0;
+    CUDA_TRY(cudaMemcpyAsync(&H, c->d_nhills, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    if (count) *count = H;
+    if (!centers || !heights || capacity <= 0) return METAD_OK;
+    int n = H < capacity ? H : capacity;
+    if (on_device) {
+        int r = bias_get_hills_dev(c, centers, heights, capacity);
+        if (r) return r;
+    } else {
+        double *dc = nullptr, *dh = nullptr;
+        CUDA_TRY(dev_alloc(&dc, (size_t)capacity * c->D));
+        CUDA_TRY(dev_alloc(&dh, capacity));
+        int r = bias_get_hills_dev(c, dc, dh, capacity);
+        if (r) return r;
+        CUDA_TRY(cudaMemcpyAsync(centers, dc, sizeof(double) * (size_t)n * c->D, cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(cudaMemcpyAsync(heights, dh, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+        cudaStreamSynchronize(c->stream);
+        cudaFree(dc); cudaFree(dh);
+    }
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return METAD_OK;
+}
+
+extern "C" int metad_get_grid(metad_ctx *c, double *d_table) {
+    if (!c || !d_table) FAIL(METAD_ERR_ARG, "null argument");
+    if (!c->grid_on) FAIL(METAD_ERR_STATE, "grid not enabled");
+    size_t nn = 4 * (size_t)c->p.grid_n[0] * c->p.grid_n[1];
+    CUDA_TRY(cudaMemcpyAsync(d_table, c->d_table, sizeof(double) * nn, cudaMemcpyDeviceToDevice, c->stream));
+    return METAD_OK;
+}
+
+extern "C" int metad_reset_steps(metad_ctx *c) {
+    if (!c) FAIL(METAD_ERR_ARG, "null argument");
+    CUDA_TRY(cudaMemsetAsync(c->d_step, 0, sizeof(int), c->stream));
+    return METAD_OK;
+}
+
+extern "C" long long metad_launch_count(metad_ctx *c) { return c ? c->launches : 0; }

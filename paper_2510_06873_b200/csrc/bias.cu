@@ -1,0 +1,301 @@
+// bias.cu — a5 hill sum, a5g grid-tabulated bias (bicubic Hermite), a7 on-device deposition.
+// V_b(s) = sum_tau w_tau exp(-(s - s_tau)^2 / (2 sigma^2)); well-tempered heights per
+// PAPER.md:43 / ref. [16] (reading I).  Everything fp64; hill count and step counter live on the device
+// so that the whole step can sit inside a CUDA graph.
+#include "common.cuh"
+
+#define BIAS_THREADS 256
+#define BIAS_MAX_BLOCKS 592   // 4 x 148 SMs
+
+struct BiasParams {
+    int D, max_hills;
+    double sigma[METAD_MAX_CV];
+    double inv_sigma[METAD_MAX_CV];
+};
+
+struct GridParams {
+    int n0, n1;
+    double lo[2], hi[2], h[2], inv_h[2];
+};
+
+// device scalars, one int array:  [0] = grid miss flag of this step, [1] = index of the hill
+// deposited in this step (-1: none)
+#define AUX_GRID_MISS 0
+#define AUX_DEP_INDEX 1
+
+// ------------------------------------------------------------------------------------------------
+// exact hill sum at one point: blocks stride over the hill array, fixed-order reduction.
+__global__ void __launch_bounds__(BIAS_THREADS)
+k_bias_sum(BiasParams bp, const double *__restrict__ centers, const double *__restrict__ heights,
+           const int *__restrict__ nhills, const double *__restrict__ cv, double *__restrict__ partials,
+           unsigned int *__restrict__ ticket, double *__restrict__ V, double *__restrict__ dVds,
+           const int *__restrict__ aux, int grid_on) {
+    __shared__ double red[(1 + METAD_MAX_CV) * 32];
+    if (grid_on && aux[AUX_GRID_MISS] == 0) return;   // the grid lookup already produced V, dVds
+    const int H = *nhills;
+    double s[METAD_MAX_CV];
+#pragma unroll
+    for (int d = 0; d < METAD_MAX_CV; ++d) s[d] = d < bp.D ? cv[d] : 0.0;
+    double acc[1 + METAD_MAX_CV];
+#pragma unroll
+    for (int d = 0; d <= METAD_MAX_CV; ++d) acc[d] = 0.0;
+    for (int k = blockIdx.x * BIAS_THREADS + threadIdx.x; k < H; k += gridDim.x * BIAS_THREADS) {
+        double e = 0.0, t[METAD_MAX_CV];
+#pragma unroll
+        for (int d = 0; d < METAD_MAX_CV; ++d) {
+            if (d < bp.D) {
+                t[d] = (s[d] - centers[(size_t)d * bp.max_hills + k]) * bp.inv_sigma[d];
+                e += t[d] * t[d];
+            }
+        }
+        double g = heights[k] * exp(-0.5 * e);
+        acc[0] += g;
+#pragma unroll
+        for (int d = 0; d < METAD_MAX_CV; ++d)
+            if (d < bp.D) acc[1 + d] -= g * t[d] * bp.inv_sigma[d];
+    }
+    block_reduce<1 + METAD_MAX_CV>(acc, red);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int d = 0; d <= METAD_MAX_CV; ++d) partials[blockIdx.x * (1 + METAD_MAX_CV) + d] = acc[d];
+    }
+    if (last_block_ticket(ticket)) {
+        double t[1 + METAD_MAX_CV];
+#pragma unroll
+        for (int d = 0; d <= METAD_MAX_CV; ++d) t[d] = 0.0;
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) {
+#pragma unroll
+            for (int d = 0; d <= METAD_MAX_CV; ++d) t[d] += partials[b * (1 + METAD_MAX_CV) + d];
+        }
+        block_reduce<1 + METAD_MAX_CV>(t, red);
+        if (threadIdx.x == 0) {
+            *V = t[0];
+            for (int d = 0; d < bp.D; ++d) dVds[d] = t[1 + d];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// grid lookup: bicubic Hermite on node values V, V_0, V_1, V_01 (reading M)
+__device__ __forceinline__ void hermite(double t, double *h, double *dh) {
+    double t2 = t * t, t3 = t2 * t;
+    h[0] = 2 * t3 - 3 * t2 + 1; h[1] = -2 * t3 + 3 * t2; h[2] = t3 - 2 * t2 + t; h[3] = t3 - t2;
+    dh[0] = 6 * t2 - 6 * t; dh[1] = -6 * t2 + 6 * t; dh[2] = 3 * t2 - 4 * t + 1; dh[3] = 3 * t2 - 2 * t;
+}
+
+__global__ void k_bias_grid(GridParams gp, const double *__restrict__ table, const double *__restrict__ cv,
+                            double *__restrict__ V, double *__restrict__ dVds, int *__restrict__ aux,
+                            unsigned int *__restrict__ sticky) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double s0 = cv[0], s1 = cv[1];
+    if (!(s0 >= gp.lo[0]) || !(s0 <= gp.hi[0]) || !(s1 >= gp.lo[1]) || !(s1 <= gp.hi[1])) {
+        aux[AUX_GRID_MISS] = 1;
+        atomicOr(sticky, (unsigned)METAD_DEV_GRID_RANGE);
+        return;
+    }
+    aux[AUX_GRID_MISS] = 0;
+    double fx = (s0 - gp.lo[0]) * gp.inv_h[0], fy = (s1 - gp.lo[1]) * gp.inv_h[1];
+    int i = min((int)floor(fx), gp.n0 - 2), j = min((int)floor(fy), gp.n1 - 2);
+    double hx[4], dhx[4], hy[4], dhy[4];
+    hermite(fx - i, hx, dhx);
+    hermite(fy - j, hy, dhy);
+    size_t plane = (size_t)gp.n0 * gp.n1;
+    double v = 0.0, vx = 0.0, vy = 0.0;
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            size_t o = (size_t)(i + a) * gp.n1 + (j + b);
+            double f = table[o], f0 = table[plane + o] * gp.h[0], f1 = table[2 * plane + o] * gp.h[1],
+                   f01 = table[3 * plane + o] * gp.h[0] * gp.h[1];
+            v += f * hx[a] * hy[b] + f0 * hx[2 + a] * hy[b] + f1 * hx[a] * hy[2 + b] + f01 * hx[2 + a] * hy[2 + b];
+            vx += f * dhx[a] * hy[b] + f0 * dhx[2 + a] * hy[b] + f1 * dhx[a] * hy[2 + b] + f01 * dhx[2 + a] * hy[2 + b];
+            vy += f * hx[a] * dhy[b] + f0 * hx[2 + a] * dhy[b] + f1 * hx[a] * dhy[2 + b] + f01 * hx[2 + a] * dhy[2 + b];
+        }
+    *V = v; dVds[0] = vx * gp.inv_h[0]; dVds[1] = vy * gp.inv_h[1];
+}
+
+// table build: 16x16 node tile per block; hills staged through shared memory in chunks, the two
+// 1-D Gaussian factors computed once per (hill, row) / (hill, column) of the tile (separable form).
+#define GT 16
+#define GCH 64
+__global__ void __launch_bounds__(GT * GT)
+k_grid_accumulate(GridParams gp, BiasParams bp, const double *__restrict__ centers, const double *__restrict__ heights,
+                  int k0, const int *__restrict__ nhills_dev, int k1_host, double *__restrict__ table) {
+    __shared__ double ex[GCH][GT], gx[GCH][GT], ey[GCH][GT], gy[GCH][GT];
+    const int k1 = nhills_dev ? *nhills_dev : k1_host;
+    const int tx = threadIdx.x % GT, ty = threadIdx.x / GT;
+    const int i = blockIdx.x * GT + ty, j = blockIdx.y * GT + tx;   // node (i along s0, j along s1)
+    double v = 0.0, v0 = 0.0, v1 = 0.0, v01 = 0.0;
+    for (int base = k0; base < k1; base += GCH) {
+        int nh = min(GCH, k1 - base);
+        __syncthreads();
+        // 2*GCH*GT factor evaluations spread over the 256 threads
+        for (int q = threadIdx.x; q < 2 * GCH * GT; q += GT * GT) {
+            int which = q / (GCH * GT), r = q % (GCH * GT), h = r / GT, t = r % GT;
+            if (h < nh) {
+                int k = base + h;
+                if (which == 0) {
+                    double x = gp.lo[0] + (blockIdx.x * GT + t) * gp.h[0];
+                    double a = (x - centers[k]) * bp.inv_sigma[0];
+                    ex[h][t] = heights[k] * exp(-0.5 * a * a);
+                    gx[h][t] = -a * bp.inv_sigma[0];
+                } else {
+                    double y = gp.lo[1] + (blockIdx.y * GT + t) * gp.h[1];
+                    double b = (y - centers[(size_t)bp.max_hills + k]) * bp.inv_sigma[1];
+                    ey[h][t] = exp(-0.5 * b * b);
+                    gy[h][t] = -b * bp.inv_sigma[1];
+                }
+            }
+        }
+        __syncthreads();
+        for (int h = 0; h < nh; ++h) {
+            double g = ex[h][ty] * ey[h][tx];
+            double ga = gx[h][ty], gb = gy[h][tx];
+            v += g; v0 += g * ga; v1 += g * gb; v01 += g * ga * gb;
+        }
+    }
+    if (i < gp.n0 && j < gp.n1) {
+        size_t plane = (size_t)gp.n0 * gp.n1, o = (size_t)i * gp.n1 + j;
+        table[o] += v; table[plane + o] += v0; table[2 * plane + o] += v1; table[3 * plane + o] += v01;
+    }
+}
+
+// per-step: add the hill deposited in this step (if any) to every node
+__global__ void k_grid_add_last(GridParams gp, BiasParams bp, const double *__restrict__ centers,
+                                const double *__restrict__ heights, const int *__restrict__ aux,
+                                double *__restrict__ table) {
+    const int k = aux[AUX_DEP_INDEX];
+    if (k < 0) return;
+    int o = blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= gp.n0 * gp.n1) return;
+    int i = o / gp.n1, j = o % gp.n1;
+    double a = (gp.lo[0] + i * gp.h[0] - centers[k]) * bp.inv_sigma[0];
+    double b = (gp.lo[1] + j * gp.h[1] - centers[(size_t)bp.max_hills + k]) * bp.inv_sigma[1];
+    double g = heights[k] * exp(-0.5 * (a * a + b * b));
+    double ga = -a * bp.inv_sigma[0], gb = -b * bp.inv_sigma[1];
+    size_t plane = (size_t)gp.n0 * gp.n1;
+    table[o] += g; table[plane + o] += g * ga; table[2 * plane + o] += g * gb; table[3 * plane + o] += g * ga * gb;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a7: deposition (readings I, J, U).  One thread.
+__global__ void k_deposit(BiasParams bp, int stride, double w0, double kT, double gamma, const double *__restrict__ cv,
+                          const double *__restrict__ V, double *__restrict__ centers, double *__restrict__ heights,
+                          int *__restrict__ nhills, int *__restrict__ step, int *__restrict__ aux,
+                          unsigned int *__restrict__ sticky) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    int st = *step + 1;
+    *step = st;
+    aux[AUX_DEP_INDEX] = -1;
+    if (stride <= 0 || st % stride != 0) return;
+    int H = *nhills;
+    if (H >= bp.max_hills) { atomicOr(sticky, (unsigned)METAD_DEV_HILL_OVERFLOW); return; }
+    double h = gamma > 1.0 ? w0 * exp(-(*V) / ((gamma - 1.0) * kT)) : w0;
+    for (int d = 0; d < bp.D; ++d) centers[(size_t)d * bp.max_hills + H] = cv[d];
+    heights[H] = h;
+    *nhills = H + 1;
+    aux[AUX_DEP_INDEX] = H;
+}
+
+__global__ void k_hills_import(int D, int max_hills, int count, const double *__restrict__ rowmajor,
+                               const double *__restrict__ h_in, double *__restrict__ centers,
+                               double *__restrict__ heights, int *__restrict__ nhills) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k == 0) *nhills = count;
+    if (k >= count) return;
+    for (int d = 0; d < D; ++d) centers[(size_t)d * max_hills + k] = rowmajor[(size_t)k * D + d];
+    heights[k] = h_in[k];
+}
+
+__global__ void k_hills_export(int D, int max_hills, int capacity, const double *__restrict__ centers,
+                               const double *__restrict__ heights, const int *__restrict__ nhills,
+                               double *__restrict__ rowmajor, double *__restrict__ h_out) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= *nhills || k >= capacity) return;
+    for (int d = 0; d < D; ++d) rowmajor[(size_t)k * D + d] = centers[(size_t)d * max_hills + k];
+    h_out[k] = heights[k];
+}
+
+// ------------------------------------------------------------------------------------------------
+static BiasParams make_bp(const metad_ctx *c) {
+    BiasParams bp;
+    bp.D = c->D; bp.max_hills = c->p.max_hills;
+    for (int d = 0; d < METAD_MAX_CV; ++d) {
+        bp.sigma[d] = d < c->D ? c->p.sigma[d] : 1.0;
+        bp.inv_sigma[d] = 1.0 / bp.sigma[d];
+    }
+    return bp;
+}
+static GridParams make_gp(const metad_ctx *c) {
+    GridParams gp;
+    gp.n0 = c->p.grid_n[0]; gp.n1 = c->p.grid_n[1];
+    for (int d = 0; d < 2; ++d) {
+        gp.lo[d] = c->p.grid_lo[d]; gp.hi[d] = c->p.grid_hi[d];
+        int n = d == 0 ? gp.n0 : gp.n1;
+        gp.h[d] = n > 1 ? (gp.hi[d] - gp.lo[d]) / (n - 1) : 1.0;
+        gp.inv_h[d] = 1.0 / gp.h[d];
+    }
+    return gp;
+}
+
+
+int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds) {
+    BiasParams bp = make_bp(c);
+    if (c->grid_on) {
+        k_bias_grid<<<1, 32, 0, c->stream>>>(make_gp(c), c->d_table, d_cv, d_V, d_dVds, ctx_aux(c), c->d_sticky);
+        c->launches++;
+    }
+    int nb = div_up(c->p.max_hills, BIAS_THREADS * 4);
+    if (nb > BIAS_MAX_BLOCKS) nb = BIAS_MAX_BLOCKS;
+    if (nb < 1) nb = 1;
+    k_bias_sum<<<nb, BIAS_THREADS, 0, c->stream>>>(bp, c->d_centers, c->d_heights, c->d_nhills, d_cv, c->d_bias_partials,
+                                                  c->d_tickets + 8, d_V, d_dVds, ctx_aux(c), c->grid_on);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+int bias_deposit(metad_ctx *c, const double *d_cv, const double *d_V) {
+    BiasParams bp = make_bp(c);
+    k_deposit<<<1, 32, 0, c->stream>>>(bp, c->p.stride, c->p.w0, c->p.kT, c->p.bias_factor, d_cv, d_V, c->d_centers,
+                                       c->d_heights, c->d_nhills, c->d_step, ctx_aux(c), c->d_sticky);
+    c->launches++;
+    if (c->grid_on) {
+        int nn = c->p.grid_n[0] * c->p.grid_n[1];
+        k_grid_add_last<<<div_up(nn, 256), 256, 0, c->stream>>>(make_gp(c), bp, c->d_centers, c->d_heights, ctx_aux(c),
+                                                                c->d_table);
+        c->launches++;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+int bias_grid_rebuild(metad_ctx *c) {
+    if (!c->grid_on) return METAD_OK;
+    GridParams gp = make_gp(c);
+    CUDA_TRY(cudaMemsetAsync(c->d_table, 0, sizeof(double) * 4 * (size_t)gp.n0 * gp.n1, c->stream));
+    dim3 g(div_up(gp.n0, GT), div_up(gp.n1, GT));
+    k_grid_accumulate<<<g, GT * GT, 0, c->stream>>>(gp, make_bp(c), c->d_centers, c->d_heights, 0, c->d_nhills, 0,
+                                                    c->d_table);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+int bias_set_hills_dev(metad_ctx *c, const double *d_rowmajor, const double *d_heights, int count) {
+    k_hills_import<<<div_up(count > 0 ? count : 1, 256), 256, 0, c->stream>>>(c->D, c->p.max_hills, count, d_rowmajor,
+                                                                            d_heights, c->d_centers, c->d_heights,
+                                                                            c->d_nhills);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return bias_grid_rebuild(c);
+}
+
+int bias_get_hills_dev(metad_ctx *c, double *d_rowmajor, double *d_heights, int capacity) {
+    k_hills_export<<<div_up(c->p.max_hills, 256), 256, 0, c->stream>>>(c->D, c->p.max_hills, capacity, c->d_centers,
+                                                                     c->d_heights, c->d_nhills, d_rowmajor, d_heights);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}

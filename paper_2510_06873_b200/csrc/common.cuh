@@ -1,0 +1,184 @@
+// common.cuh — shared device helpers and the context of the B200 metadynamics library.
+// (CUDA path only; shares nothing with oracle/.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/metad.h"
+
+#define METAD_NREC 16  // per-atom Q6 record: 13 normalised q6m components + f'(q6) + q6 + pad
+
+// ------------------------------------------------------------------------------------------------
+// Periodic box for the pair arithmetic in precision T.  Lattice rows a=(ax,0,0), b=(bx,by,0),
+// c=(cx,cy,cz).  For T=float every component is split hi+lo so that a lattice shift applied to an
+// (exact) fp32 coordinate difference stays accurate to ~1 ulp of the result.
+template <typename T>
+struct PBox {
+    T ax, bx, by, cx, cy, cz;        // hi parts (the whole value for T=double)
+    T lax, lbx, lby, lcx, lcy, lcz;  // lo parts (0 for T=double)
+    T hx, hy, hz;                    // half box: 0.5*ax, 0.5*by, 0.5*cz
+};
+
+struct BoxD {                        // fp64 box, used by the canonical neighbour predicate
+    double ax, bx, by, cx, cy, cz, hx, hy, hz;
+};
+
+struct CellGrid {
+    int nc[3];                       // cells along a, b, c
+    int ncell;
+    double inv[6];                   // fractional transform: s_c = z*i0; s_b = (y - s_c*cy)*i1; ...
+    double cx, cy, bx;               // tilt terms for cartesian -> fractional
+};
+
+template <typename T> struct Vec4;
+template <> struct Vec4<float> { typedef float4 type; };
+template <> struct Vec4<double> { typedef double4 type; };
+
+template <typename T>
+__device__ __forceinline__ typename Vec4<T>::type ld4(const typename Vec4<T>::type *p) { return *p; }
+
+// Minimum-image displacement (reading O order: z against c, y against b, x against a).
+template <typename T>
+__device__ __forceinline__ void min_image(const PBox<T> &b, T &dx, T &dy, T &dz) {
+    T sz = dz > b.hz ? T(-1) : (dz < -b.hz ? T(1) : T(0));
+    dx += sz * b.cx; dy += sz * b.cy; dz += sz * b.cz;
+    dx += sz * b.lcx; dy += sz * b.lcy; dz += sz * b.lcz;
+    T sy = dy > b.hy ? T(-1) : (dy < -b.hy ? T(1) : T(0));
+    dx += sy * b.bx; dy += sy * b.by;
+    dx += sy * b.lbx; dy += sy * b.lby;
+    T sx = dx > b.hx ? T(-1) : (dx < -b.hx ? T(1) : T(0));
+    dx += sx * b.ax;
+    dx += sx * b.lax;
+}
+
+// The canonical fp64 predicate arithmetic (reading O): identical operation order and rounding to
+// the definition — no FMA contraction in r^2.
+__device__ __forceinline__ double r2_canonical(const BoxD &b, double dx, double dy, double dz) {
+    if (dz > b.hz) { dx -= b.cx; dy -= b.cy; dz -= b.cz; }
+    else if (dz < -b.hz) { dx += b.cx; dy += b.cy; dz += b.cz; }
+    if (dy > b.hy) { dx -= b.bx; dy -= b.by; }
+    else if (dy < -b.hy) { dx += b.bx; dy += b.by; }
+    if (dx > b.hx) { dx -= b.ax; }
+    else if (dx < -b.hx) { dx += b.ax; }
+    return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+}
+
+// ------------------------------------------------------------------------------------------------
+// Deterministic block reduction of K doubles per thread (fixed tree: shuffle inside the warp, then
+// warp 0 sums the per-warp partials in warp order).
+template <int K>
+__device__ __forceinline__ void block_reduce(double (&v)[K], double *smem /* >= K*32 doubles */) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_down_sync(0xffffffffu, v[k], o);
+    }
+    __syncthreads();
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) smem[k * 32 + wid] = v[k];
+    }
+    __syncthreads();
+    if (wid == 0) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            double x = lane < nw ? smem[k * 32 + lane] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+            v[k] = x;  // valid in thread 0
+        }
+    }
+}
+
+// "Last block finishes" pattern: every block writes its partials, the last one to arrive (atomic
+// ticket) sums them in block order -> deterministic, one launch.  Returns true in the last block.
+__device__ __forceinline__ bool last_block_ticket(unsigned int *ticket) {
+    __shared__ bool is_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int t = atomicAdd(ticket, 1u);
+        is_last = (t == gridDim.x - 1);
+        if (is_last) *ticket = 0u;  // re-arm for the next launch
+    }
+    __syncthreads();
+    if (is_last) __threadfence();
+    return is_last;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Host-side context
+struct CvDev {                      // device copies of one CV descriptor
+    int kind, n, m;
+    double r0, scale, q_thresh, q_width;
+    int npairs, nchain;
+    int *d_pairs; double *d_pair_r0;      // CONTACTS
+    int *d_csr_off, *d_csr_pair;          // CONTACTS: per touched atom incident pairs (gather form)
+    int *d_catoms; int ncatoms;           //           the touched atoms
+    int *d_chain; double *d_mass;         // RGYR
+    double *d_unwrapped;                  // RGYR scratch: [nchain*3] + com[3] + rg
+    bool use_groups;
+};
+
+struct metad_ctx {
+    metad_params p;
+    cudaStream_t stream;
+    int N, prec, maxn, D;
+    // neighbour / cell state
+    CellGrid grid;
+    BoxD boxd;
+    double rc, rc2;
+    bool have_neighbors;
+    int cell_cap;
+    int *d_cell_count, *d_cell_start, *d_block_sums;
+    int *d_cell_of, *d_slot, *d_perm, *d_scell;
+    unsigned char *d_flags;               // per original atom: bit0 in A, bit1 in B (COORD)
+    void *d_spos;                         // Vec4<T>[N], cell-sorted
+    int *d_nl_count, *d_nl;               // sorted space; nl[k*N + s]
+    // CV state
+    CvDev cv[METAD_MAX_CV];
+    bool has_q6, has_coord;
+    int q6_mean_dim, q6_solid_dim, coord_dim;
+    void *d_rec;                          // T[N][METAD_NREC]
+    double *d_partials;                   // block partial sums
+    unsigned int *d_tickets;
+    int nblocks_atoms;
+    // bias state (all device)
+    double *d_centers;                    // SoA [D][max_hills]
+    double *d_heights;
+    int *d_nhills, *d_step;
+    unsigned int *d_sticky;
+    double *d_cv, *d_V, *d_dVds;          // internal state of the last step
+    double *d_bias_partials;
+    double *d_table;                      // grid [4][n0][n1]
+    int grid_on;
+    // host-path staging
+    void *d_pos_stage, *d_F_stage;
+    void *h_pin; size_t h_pin_bytes;
+    // graph
+    cudaGraphExec_t graph_exec;
+    const void *graph_pos; void *graph_F; double graph_rc; double graph_box[9];
+    long long launches; int launches_per_step;
+    const void *d_pos_last;               // positions snapshot pointer of the last build (chain CVs read it)
+    int *d_aux;                           // device scalars: grid-miss flag, index of the hill deposited this step
+};
+
+static inline const void *ctx_last_pos(const metad_ctx *c) { return c->d_pos_last; }
+static inline int *ctx_aux(const metad_ctx *c) { return c->d_aux; }
+
+void metad_set_error(const char *msg);
+#define CUDA_TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { metad_set_error(cudaGetErrorString(e_)); return METAD_ERR_CUDA; } } while (0)
+
+static inline int div_up(long long a, int b) { return (int)((a + b - 1) / b); }
+
+// stage entry points implemented in the .cu files (host functions that enqueue kernels)
+int nb_build(metad_ctx *c, const void *d_pos);
+int nb_export(metad_ctx *c, int *d_count, int *d_list);
+int cv_eval_all(metad_ctx *c, double *d_cv);
+int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F);
+int q6_export(metad_ctx *c, void *d_q6);
+int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds);
+int bias_deposit(metad_ctx *c, const double *d_cv, const double *d_V);
+int bias_grid_rebuild(metad_ctx *c);
+int bias_set_hills_dev(metad_ctx *c, const double *d_centers_rowmajor, const double *d_heights, int count);
+int bias_get_hills_dev(metad_ctx *c, double *d_centers_rowmajor, double *d_heights, int capacity);

@@ -1,0 +1,334 @@
+// cv.cu — a2/a3 CV evaluation and a6 gather-form forces for the neighbour-list CVs
+// (coordination number, Steinhardt Q6 mean, solid-like count).  Thread per (cell-sorted) atom;
+// pair arithmetic in T, every reduction in fp64 with a fixed order (deterministic).
+#include "common.cuh"
+#include "cv_q6.cuh"
+
+template <typename T> PBox<T> ctx_pbox(const metad_ctx *c);
+
+#define CV_THREADS 128
+
+// ------------------------------------------------------------------------------------------------
+// switching function sw(x) = (1-x^n)/(1-x^m) and d sw/dx (reading A).  m == 2n -> 1/(1+x^n).
+template <typename T>
+__device__ __forceinline__ T ipow(T x, int n) {
+    T r = T(1);
+    for (int k = 0; k < n; ++k) r *= x;
+    return r;
+}
+template <typename T>
+__device__ __forceinline__ T switch_fn(T x, int n, int m, T &dsw) {
+    if (m == 2 * n) {
+        T xn1 = ipow(x, n - 1), xn = xn1 * x;
+        T inv = T(1) / (T(1) + xn);
+        dsw = -T(n) * xn1 * inv * inv;
+        return inv;
+    }
+    T e = x - T(1);
+    if (fabs((double)e) < 1e-6) {
+        T s0 = T(n) / T(m), s1 = T(n) * T(n - m) / (T(2) * T(m));
+        dsw = s1;
+        return s0 + s1 * e;
+    }
+    T xn1 = ipow(x, n - 1), xm1 = ipow(x, m - 1);
+    T num = T(1) - xn1 * x, den = T(1) - xm1 * x;
+    T f = num / den;
+    dsw = (-T(n) * xn1 * den + num * T(m) * xm1) / (den * den);
+    return f;
+}
+
+// ------------------------------------------------------------------------------------------------
+// coordination number
+template <typename T>
+__global__ void __launch_bounds__(CV_THREADS)
+k_coord_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
+           const int *__restrict__ nl, PBox<T> pb, T inv_r0, int n, int m, double scale,
+           double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
+           unsigned int *__restrict__ sticky) {
+    __shared__ double red[32];
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    T acc = T(0);
+    if (s < N) {
+        typename Vec4<T>::type pi = spos[s];
+        if (((int)pi.w) & 1) {
+            int cnt = nl_count[s];
+            for (int k = 0; k < cnt; ++k) {
+                int j = nl[(size_t)k * N + s];
+                typename Vec4<T>::type pj = spos[j];
+                if (!(((int)pj.w) & 2)) continue;
+                T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+                min_image(pb, dx, dy, dz);
+                T r = sqrt(dx * dx + dy * dy + dz * dz), dsw;
+                acc += switch_fn<T>(r * inv_r0, n, m, dsw);
+            }
+        }
+    }
+    double v[1] = { (double)acc };
+    block_reduce<1>(v, red);
+    if (threadIdx.x == 0) partials[blockIdx.x] = v[0];
+    if (last_block_ticket(ticket)) {
+        double t[1] = { 0.0 };
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) t[0] += partials[b];
+        block_reduce<1>(t, red);
+        if (threadIdx.x == 0) {
+            double r = scale * t[0];
+            *cv_out = r;
+            if (!isfinite(r)) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
+        }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(CV_THREADS)
+k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
+              const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, T inv_r0, int n, int m,
+              double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    typename Vec4<T>::type pi = spos[s];
+    const int fi = (int)pi.w;
+    T ax = T(0), ay = T(0), az = T(0);
+    int cnt = nl_count[s];
+    for (int k = 0; k < cnt; ++k) {
+        int j = nl[(size_t)k * N + s];
+        typename Vec4<T>::type pj = spos[j];
+        const int fj = (int)pj.w;
+        int mult = ((fi & 1) && (fj & 2)) + ((fi & 2) && (fj & 1));
+        if (!mult) continue;
+        T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+        min_image(pb, dx, dy, dz);
+        T r = sqrt(dx * dx + dy * dy + dz * dz), dsw;
+        switch_fn<T>(r * inv_r0, n, m, dsw);
+        T g = T(mult) * dsw * inv_r0 / r;
+        ax += g * dx; ay += g * dy; az += g * dz;
+    }
+    // ds/dr_k = scale * sum g * (-d)  ->  F_k += -fs*dVds*ds/dr_k = +fs*scale*dVds * sum g*d
+    const double a = coef * dVds[0];
+    const int i = perm[s];
+    F[3 * i] += (T)(a * (double)ax);
+    F[3 * i + 1] += (T)(a * (double)ay);
+    F[3 * i + 2] += (T)(a * (double)az);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Q6 pass 1: per-atom q6m accumulation -> record + block partials of (sum q6, sum f(q6))
+template <typename T>
+__global__ void __launch_bounds__(CV_THREADS)
+k_q6_pass1(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
+           const int *__restrict__ nl, PBox<T> pb, T q_thresh, T inv_width, T *__restrict__ rec,
+           double scale_mean, double scale_solid, int dim_mean, int dim_solid,
+           double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
+           unsigned int *__restrict__ sticky) {
+    __shared__ double red[64];
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    double v[2] = { 0.0, 0.0 };
+    if (s < N) {
+        typename Vec4<T>::type pi = spos[s];
+        T A[13];
+#pragma unroll
+        for (int k = 0; k < 13; ++k) A[k] = T(0);
+        int cnt = nl_count[s];
+        for (int k = 0; k < cnt; ++k) {
+            int j = nl[(size_t)k * N + s];
+            typename Vec4<T>::type pj = spos[j];
+            T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+            min_image(pb, dx, dy, dz);
+            T rinv = T(1) / sqrt(dx * dx + dy * dy + dz * dz);
+            Y6<T> y;
+            y6_eval<T>(dx * rinv, dy * rinv, dz * rinv, y);
+            A[0] += y.E[0];
+#pragma unroll
+            for (int m = 1; m <= 6; ++m) {
+                A[2 * m - 1] += y.E[m] * y.c[m];
+                A[2 * m] += y.E[m] * y.s[m];
+            }
+        }
+        T S = T(0);
+#pragma unroll
+        for (int k = 0; k < 13; ++k) S += A[k] * A[k];
+        T q6 = T(0), fsw = T(0), dfsw = T(0), norm = T(0);
+        if (cnt > 0 && S > T(0)) {
+            T rs = sqrt(S);
+            q6 = rs / T(cnt);
+            norm = T(1) / (T(cnt) * rs);
+        }
+        {
+            T f = T(1) / (T(1) + exp(-(q6 - q_thresh) * inv_width));
+            fsw = f;
+            dfsw = f * (T(1) - f) * inv_width;
+        }
+        // record: B_m = conj(A_m)/(n sqrt(S)); [13] = f'(q6); [14] = q6
+        T out[METAD_NREC];
+        out[0] = A[0] * norm;
+#pragma unroll
+        for (int m = 1; m <= 6; ++m) { out[2 * m - 1] = A[2 * m - 1] * norm; out[2 * m] = -A[2 * m] * norm; }
+        out[13] = dfsw; out[14] = q6; out[15] = T(0);
+        typename Vec4<T>::type *r4 = reinterpret_cast<typename Vec4<T>::type *>(rec + (size_t)s * METAD_NREC);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            typename Vec4<T>::type w;
+            w.x = out[4 * q]; w.y = out[4 * q + 1]; w.z = out[4 * q + 2]; w.w = out[4 * q + 3];
+            r4[q] = w;
+        }
+        v[0] = (double)q6; v[1] = (double)fsw;
+    }
+    block_reduce<2>(v, red);
+    if (threadIdx.x == 0) { partials[2 * blockIdx.x] = v[0]; partials[2 * blockIdx.x + 1] = v[1]; }
+    if (last_block_ticket(ticket)) {
+        double t[2] = { 0.0, 0.0 };
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) { t[0] += partials[2 * b]; t[1] += partials[2 * b + 1]; }
+        block_reduce<2>(t, red);
+        if (threadIdx.x == 0) {
+            double a = scale_mean * t[0], b = scale_solid * t[1];
+            if (dim_mean >= 0) cv_out[dim_mean] = a;
+            if (dim_solid >= 0) cv_out[dim_solid] = b;
+            if (!isfinite(a) || !isfinite(b)) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
+        }
+    }
+}
+
+// Q6 pass 2 (gather form, reading E):  F_k += fs * sum_{j in N(k)} grad_d [ (g_k B(k) + g_j B(j)) . y ](d_kj),
+// g_i = alpha + beta f'(q6_i), alpha = dVds[mean]*scale_mean, beta = dVds[solid]*scale_solid.
+template <typename T>
+__global__ void __launch_bounds__(CV_THREADS)
+k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
+           const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, const T *__restrict__ rec,
+           double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
+           const double *__restrict__ dVds, T *__restrict__ F) {
+    typedef typename Vec4<T>::type V4;
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    const T alpha = dim_mean >= 0 ? (T)(dVds[dim_mean] * scale_mean) : T(0);
+    const T beta = dim_solid >= 0 ? (T)(dVds[dim_solid] * scale_solid) : T(0);
+    V4 pi = spos[s];
+    T Bk[13];
+    {
+        const V4 *r4 = reinterpret_cast<const V4 *>(rec + (size_t)s * METAD_NREC);
+        V4 a = r4[0], b = r4[1], c = r4[2], d = r4[3];
+        T gk = alpha + beta * d.y;
+        Bk[0] = gk * a.x; Bk[1] = gk * a.y; Bk[2] = gk * a.z; Bk[3] = gk * a.w;
+        Bk[4] = gk * b.x; Bk[5] = gk * b.y; Bk[6] = gk * b.z; Bk[7] = gk * b.w;
+        Bk[8] = gk * c.x; Bk[9] = gk * c.y; Bk[10] = gk * c.z; Bk[11] = gk * c.w;
+        Bk[12] = gk * d.x;
+    }
+    T ax = T(0), ay = T(0), az = T(0);
+    int cnt = nl_count[s];
+    for (int k = 0; k < cnt; ++k) {
+        int j = nl[(size_t)k * N + s];
+        V4 pj = spos[j];
+        const V4 *r4 = reinterpret_cast<const V4 *>(rec + (size_t)j * METAD_NREC);
+        V4 a = r4[0], b = r4[1], c = r4[2], d = r4[3];
+        T gj = alpha + beta * d.y;
+        T bb[13];
+        bb[0] = Bk[0] + gj * a.x; bb[1] = Bk[1] + gj * a.y; bb[2] = Bk[2] + gj * a.z; bb[3] = Bk[3] + gj * a.w;
+        bb[4] = Bk[4] + gj * b.x; bb[5] = Bk[5] + gj * b.y; bb[6] = Bk[6] + gj * b.z; bb[7] = Bk[7] + gj * b.w;
+        bb[8] = Bk[8] + gj * c.x; bb[9] = Bk[9] + gj * c.y; bb[10] = Bk[10] + gj * c.z; bb[11] = Bk[11] + gj * c.w;
+        bb[12] = Bk[12] + gj * d.x;
+        T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+        min_image(pb, dx, dy, dz);
+        T rinv = T(1) / sqrt(dx * dx + dy * dy + dz * dz);
+        T ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
+        Y6<T> y;
+        y6_eval<T>(ux, uy, uz, y);
+        T gx, gy, gz;
+        y6_grad<T>(y, bb, gx, gy, gz);
+        T gu = gx * ux + gy * uy + gz * uz;     // project onto the tangent plane, divide by r
+        ax += (gx - gu * ux) * rinv;
+        ay += (gy - gu * uy) * rinv;
+        az += (gz - gu * uz) * rinv;
+    }
+    const int i = perm[s];
+    F[3 * i] += (T)(force_scale * (double)ax);
+    F[3 * i + 1] += (T)(force_scale * (double)ay);
+    F[3 * i + 2] += (T)(force_scale * (double)az);
+}
+
+template <typename T>
+__global__ void k_q6_export(int N, const int *__restrict__ perm, const T *__restrict__ rec, T *__restrict__ q6) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < N) q6[perm[s]] = rec[(size_t)s * METAD_NREC + 14];
+}
+
+// ------------------------------------------------------------------------------------------------
+int chain_eval(metad_ctx *c, int dim, const void *d_pos_unused, double *d_cv);          // cv_chain.cu
+int chain_forces(metad_ctx *c, const double *d_dVds, void *d_F);                         // cv_chain.cu
+
+template <typename T>
+static int cv_eval_t(metad_ctx *c, double *d_cv) {
+    typedef typename Vec4<T>::type V4;
+    const int N = c->N, nb = div_up(N, CV_THREADS);
+    PBox<T> pb = ctx_pbox<T>(c);
+    if (c->has_coord) {
+        const CvDev &d = c->cv[c->coord_dim];
+        k_coord_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb,
+                                                       (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials,
+                                                       c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky);
+        c->launches++;
+    }
+    if (c->has_q6) {
+        double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
+        double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
+        double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
+        double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
+        k_q6_pass1<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, (T)qt,
+                                                       (T)(1.0 / qw), (T *)c->d_rec, sm, ss, c->q6_mean_dim,
+                                                       c->q6_solid_dim, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
+                                                       d_cv, c->d_sticky);
+        c->launches++;
+    }
+    return METAD_OK;
+}
+
+int cv_eval_all(metad_ctx *c, double *d_cv) {
+    int rcode = c->prec == 32 ? cv_eval_t<float>(c, d_cv) : cv_eval_t<double>(c, d_cv);
+    if (rcode) return rcode;
+    for (int d = 0; d < c->D; ++d)
+        if (c->cv[d].kind == METAD_CV_RGYR || c->cv[d].kind == METAD_CV_CONTACTS) {
+            rcode = chain_eval(c, d, nullptr, d_cv);
+            if (rcode) return rcode;
+        }
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+template <typename T>
+static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
+    typedef typename Vec4<T>::type V4;
+    const int N = c->N, nb = div_up(N, CV_THREADS);
+    PBox<T> pb = ctx_pbox<T>(c);
+    if (c->has_coord) {
+        const CvDev &d = c->cv[c->coord_dim];
+        k_coord_force<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
+                                                          pb, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
+                                                          d_dVds + c->coord_dim, (T *)d_F);
+        c->launches++;
+    }
+    if (c->has_q6) {
+        double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
+        double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
+        k_q6_force<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb,
+                                                       (const T *)c->d_rec, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
+                                                       c->p.force_scale, d_dVds, (T *)d_F);
+        c->launches++;
+    }
+    return METAD_OK;
+}
+
+int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F) {
+    int rcode = c->prec == 32 ? cv_forces_t<float>(c, d_dVds, d_F) : cv_forces_t<double>(c, d_dVds, d_F);
+    if (rcode) return rcode;
+    rcode = chain_forces(c, d_dVds, d_F);
+    if (rcode) return rcode;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+int q6_export(metad_ctx *c, void *d_q6) {
+    if (!c->has_q6) return METAD_ERR_STATE;
+    int nb = div_up(c->N, 256);
+    if (c->prec == 32) k_q6_export<float><<<nb, 256, 0, c->stream>>>(c->N, c->d_perm, (const float *)c->d_rec, (float *)d_q6);
+    else k_q6_export<double><<<nb, 256, 0, c->stream>>>(c->N, c->d_perm, (const double *)c->d_rec, (double *)d_q6);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}

@@ -1,0 +1,244 @@
+// cv_chain.cu — a4: radius of gyration of an ordered chain and native-contact fraction
+// (BASELINE.json configs[1]; readings G, H).  Tiny kernels: ~1,000 atoms / ~5,000 pairs, all fp64,
+// positions read from the caller's array in its own dtype.
+#include "common.cuh"
+
+#define RG_THREADS 1024
+
+struct RgScratch { double com[3]; double M; double rg; };   // stored after the unwrapped coords
+
+__device__ __forceinline__ void min_image_d(const BoxD &b, double &dx, double &dy, double &dz) {
+    if (dz > b.hz) { dx -= b.cx; dy -= b.cy; dz -= b.cz; }
+    else if (dz < -b.hz) { dx += b.cx; dy += b.cy; dz += b.cz; }
+    if (dy > b.hy) { dx -= b.bx; dy -= b.by; }
+    else if (dy < -b.hy) { dx += b.bx; dy += b.by; }
+    if (dx > b.hx) { dx -= b.ax; }
+    else if (dx < -b.hx) { dx += b.ax; }
+}
+
+// single block: unwrap by a block-wide prefix sum of minimum-image bond vectors, then COM and Rg.
+template <typename T>
+__global__ void __launch_bounds__(RG_THREADS)
+k_rgyr(int nchain, const int *__restrict__ chain, const double *__restrict__ mass, const T *__restrict__ pos,
+       BoxD bd, double *__restrict__ unwrapped, double *__restrict__ cv_out, unsigned int *__restrict__ sticky) {
+    __shared__ double wsum[3][32];
+    __shared__ double carry[3];
+    __shared__ double red[4 * 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (threadIdx.x < 3) carry[threadIdx.x] = 0.0;
+    __syncthreads();
+    for (int base = 0; base < nchain; base += RG_THREADS) {
+        int k = base + threadIdx.x;
+        double v[3] = { 0.0, 0.0, 0.0 };
+        if (k < nchain) {
+            int i = chain[k];
+            if (k == 0) {
+                v[0] = (double)pos[3 * i]; v[1] = (double)pos[3 * i + 1]; v[2] = (double)pos[3 * i + 2];
+            } else {
+                int p = chain[k - 1];
+                v[0] = (double)pos[3 * i] - (double)pos[3 * p];
+                v[1] = (double)pos[3 * i + 1] - (double)pos[3 * p + 1];
+                v[2] = (double)pos[3 * i + 2] - (double)pos[3 * p + 2];
+                min_image_d(bd, v[0], v[1], v[2]);
+            }
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                double t = __shfl_up_sync(0xffffffffu, v[a], o);
+                if (lane >= o) v[a] += t;
+            }
+            if (lane == 31) wsum[a][wid] = v[a];
+        }
+        __syncthreads();
+        if (wid == 0) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                double w = wsum[a][lane], inc = w;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    double t = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += t;
+                }
+                wsum[a][lane] = inc - w;
+            }
+        }
+        __syncthreads();
+        double tot[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            v[a] += wsum[a][wid] + carry[a];
+            if (k < nchain) unwrapped[3 * k + a] = v[a];
+            tot[a] = v[a];
+        }
+        __syncthreads();
+        if (threadIdx.x == RG_THREADS - 1) { carry[0] = tot[0]; carry[1] = tot[1]; carry[2] = tot[2]; }
+        __syncthreads();
+    }
+    // centre of mass
+    double s[4] = { 0.0, 0.0, 0.0, 0.0 };
+    for (int k = threadIdx.x; k < nchain; k += RG_THREADS) {
+        double mk = mass ? mass[k] : 1.0;
+        s[0] += mk * unwrapped[3 * k]; s[1] += mk * unwrapped[3 * k + 1]; s[2] += mk * unwrapped[3 * k + 2];
+        s[3] += mk;
+    }
+    block_reduce<4>(s, red);
+    __shared__ double com[4];
+    if (threadIdx.x == 0) { com[0] = s[0] / s[3]; com[1] = s[1] / s[3]; com[2] = s[2] / s[3]; com[3] = s[3]; }
+    __syncthreads();
+    double q[1] = { 0.0 };
+    for (int k = threadIdx.x; k < nchain; k += RG_THREADS) {
+        double mk = mass ? mass[k] : 1.0;
+        double x = unwrapped[3 * k] - com[0], y = unwrapped[3 * k + 1] - com[1], z = unwrapped[3 * k + 2] - com[2];
+        q[0] += mk * (x * x + y * y + z * z);
+    }
+    block_reduce<1>(q, red);
+    if (threadIdx.x == 0) {
+        double rg = sqrt(q[0] / com[3]);
+        RgScratch *sc = reinterpret_cast<RgScratch *>(unwrapped + 3 * (size_t)nchain);
+        sc->com[0] = com[0]; sc->com[1] = com[1]; sc->com[2] = com[2]; sc->M = com[3]; sc->rg = rg;
+        *cv_out = rg;
+        if (!isfinite(rg)) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
+    }
+}
+
+template <typename T>
+__global__ void k_rgyr_force(int nchain, const int *__restrict__ chain, const double *__restrict__ mass,
+                             const double *__restrict__ unwrapped, double force_scale,
+                             const double *__restrict__ dVds, T *__restrict__ F) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nchain) return;
+    const RgScratch *sc = reinterpret_cast<const RgScratch *>(unwrapped + 3 * (size_t)nchain);
+    if (!(sc->rg > 0.0)) return;
+    double mk = mass ? mass[k] : 1.0;
+    double a = -force_scale * dVds[0] * mk / (sc->M * sc->rg);
+    int i = chain[k];
+    F[3 * i] += (T)(a * (unwrapped[3 * k] - sc->com[0]));
+    F[3 * i + 1] += (T)(a * (unwrapped[3 * k + 1] - sc->com[1]));
+    F[3 * i + 2] += (T)(a * (unwrapped[3 * k + 2] - sc->com[2]));
+}
+
+__device__ __forceinline__ double switch_d(double x, int n, int m, double &dsw) {
+    double xn1 = 1.0;
+    for (int k = 0; k < n - 1; ++k) xn1 *= x;
+    if (m == 2 * n) {
+        double inv = 1.0 / (1.0 + xn1 * x);
+        dsw = -(double)n * xn1 * inv * inv;
+        return inv;
+    }
+    double e = x - 1.0;
+    if (fabs(e) < 1e-6) {
+        dsw = (double)n * (double)(n - m) / (2.0 * (double)m);
+        return (double)n / (double)m + dsw * e;
+    }
+    double xm1 = 1.0;
+    for (int k = 0; k < m - 1; ++k) xm1 *= x;
+    double num = 1.0 - xn1 * x, den = 1.0 - xm1 * x;
+    dsw = (-(double)n * xn1 * den + num * (double)m * xm1) / (den * den);
+    return num / den;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_contacts_cv(int npairs, const int *__restrict__ pairs, const double *__restrict__ pair_r0, int n, int m,
+              double scale, const T *__restrict__ pos, BoxD bd, double *__restrict__ partials,
+              unsigned int *__restrict__ ticket, double *__restrict__ cv_out, unsigned int *__restrict__ sticky) {
+    __shared__ double red[32];
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    double v[1] = { 0.0 };
+    if (p < npairs) {
+        int i = pairs[2 * p], j = pairs[2 * p + 1];
+        double dx = (double)pos[3 * j] - (double)pos[3 * i], dy = (double)pos[3 * j + 1] - (double)pos[3 * i + 1],
+               dz = (double)pos[3 * j + 2] - (double)pos[3 * i + 2];
+        min_image_d(bd, dx, dy, dz);
+        double dsw;
+        v[0] = switch_d(sqrt(dx * dx + dy * dy + dz * dz) / pair_r0[p], n, m, dsw);
+    }
+    block_reduce<1>(v, red);
+    if (threadIdx.x == 0) partials[blockIdx.x] = v[0];
+    if (last_block_ticket(ticket)) {
+        double t[1] = { 0.0 };
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) t[0] += partials[b];
+        block_reduce<1>(t, red);
+        if (threadIdx.x == 0) {
+            double r = scale * t[0];
+            *cv_out = r;
+            if (!isfinite(r)) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
+        }
+    }
+}
+
+// gather form: one thread per atom that appears in any pair; csr lists its incident pairs.
+template <typename T>
+__global__ void k_contacts_force(int natoms_touched, const int *__restrict__ atoms, const int *__restrict__ csr_off,
+                                 const int *__restrict__ csr_pair, const int *__restrict__ pairs,
+                                 const double *__restrict__ pair_r0, int n, int m, double coef /* fs*scale */,
+                                 const T *__restrict__ pos, BoxD bd, const double *__restrict__ dVds,
+                                 T *__restrict__ F) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= natoms_touched) return;
+    int a = atoms[t];
+    double ax = 0.0, ay = 0.0, az = 0.0;
+    for (int q = csr_off[t]; q < csr_off[t + 1]; ++q) {
+        int p = csr_pair[q];
+        int o = pairs[2 * p] == a ? pairs[2 * p + 1] : pairs[2 * p];
+        double dx = (double)pos[3 * o] - (double)pos[3 * a], dy = (double)pos[3 * o + 1] - (double)pos[3 * a + 1],
+               dz = (double)pos[3 * o + 2] - (double)pos[3 * a + 2];
+        min_image_d(bd, dx, dy, dz);
+        double r = sqrt(dx * dx + dy * dy + dz * dz), dsw;
+        switch_d(r / pair_r0[p], n, m, dsw);
+        double g = dsw / (pair_r0[p] * r);
+        ax += g * dx; ay += g * dy; az += g * dz;
+    }
+    // dQ/dr_a = scale * sum g * (-d_a)  ->  F_a += +fs*scale*dVds * sum g*d_a
+    double c = coef * dVds[0];
+    F[3 * a] += (T)(c * ax);
+    F[3 * a + 1] += (T)(c * ay);
+    F[3 * a + 2] += (T)(c * az);
+}
+
+
+template <typename T>
+static int chain_eval_t(metad_ctx *c, int dim, double *d_cv) {
+    CvDev &d = c->cv[dim];
+    const T *pos = (const T *)ctx_last_pos(c);
+    if (d.kind == METAD_CV_RGYR) {
+        k_rgyr<T><<<1, RG_THREADS, 0, c->stream>>>(d.nchain, d.d_chain, d.d_mass, pos, c->boxd, d.d_unwrapped, d_cv + dim,
+                                                   c->d_sticky);
+    } else {
+        int nb = div_up(d.npairs, 256);
+        k_contacts_cv<T><<<nb, 256, 0, c->stream>>>(d.npairs, d.d_pairs, d.d_pair_r0, d.n, d.m, d.scale, pos, c->boxd,
+                                                    c->d_partials + 3 * (size_t)c->nblocks_atoms, c->d_tickets + 2 + dim,
+                                                    d_cv + dim, c->d_sticky);
+    }
+    c->launches++;
+    return METAD_OK;
+}
+
+int chain_eval(metad_ctx *c, int dim, const void *, double *d_cv) {
+    return c->prec == 32 ? chain_eval_t<float>(c, dim, d_cv) : chain_eval_t<double>(c, dim, d_cv);
+}
+
+template <typename T>
+static int chain_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
+    const T *pos = (const T *)ctx_last_pos(c);
+    for (int dim = 0; dim < c->D; ++dim) {
+        CvDev &d = c->cv[dim];
+        if (d.kind == METAD_CV_RGYR) {
+            k_rgyr_force<T><<<div_up(d.nchain, 128), 128, 0, c->stream>>>(d.nchain, d.d_chain, d.d_mass, d.d_unwrapped,
+                                                                        c->p.force_scale, d_dVds + dim, (T *)d_F);
+            c->launches++;
+        } else if (d.kind == METAD_CV_CONTACTS) {
+            k_contacts_force<T><<<div_up(d.ncatoms, 128), 128, 0, c->stream>>>(
+                d.ncatoms, d.d_catoms, d.d_csr_off, d.d_csr_pair, d.d_pairs, d.d_pair_r0, d.n, d.m,
+                c->p.force_scale * d.scale, pos, c->boxd, d_dVds + dim, (T *)d_F);
+            c->launches++;
+        }
+    }
+    return METAD_OK;
+}
+
+int chain_forces(metad_ctx *c, const double *d_dVds, void *d_F) {
+    return c->prec == 32 ? chain_forces_t<float>(c, d_dVds, d_F) : chain_forces_t<double>(c, d_dVds, d_F);
+}

@@ -1,0 +1,270 @@
+// neighbor.cu — a1: cell-list neighbour build (BASELINE.json north_star).
+//   k_bin            cell index per atom + histogram (int atomics give the in-cell slot)
+//   k_scan_sums/k_scan_apply   exclusive scan of the histogram over cells (two launches)
+//   k_scatter        counting-sort scatter of atom indices
+//   k_cell_sort_gather  orders each cell by original index (run-to-run determinism, reading P) and
+//                    gathers positions into the cell-sorted Vec4 array (x, y, z, group flags)
+//   k_build_list     per-atom candidate scan of the 27 neighbouring cells; canonical predicate
+// Everything downstream works in "sorted space" (indices into the cell-sorted arrays), so that the
+// gathers of the CV and force passes touch neighbouring memory.
+#include "common.cuh"
+
+#define SCAN_THREADS 512
+#define SCAN_ITEMS 4
+#define SCAN_TILE (SCAN_THREADS * SCAN_ITEMS)
+
+template <typename T>
+__global__ void k_bin(int N, const T *__restrict__ pos, CellGrid g, int *__restrict__ cell_of,
+                      int *__restrict__ slot, int *__restrict__ cell_count) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    double x = (double)pos[3 * i], y = (double)pos[3 * i + 1], z = (double)pos[3 * i + 2];
+    double sc = z * g.inv[2];
+    double sb = (y - sc * g.cy) * g.inv[1];
+    double sa = (x - sb * g.bx - sc * g.cx) * g.inv[0];
+    sa -= floor(sa); sb -= floor(sb); sc -= floor(sc);
+    int ia = min(max((int)(sa * g.nc[0]), 0), g.nc[0] - 1);
+    int ib = min(max((int)(sb * g.nc[1]), 0), g.nc[1] - 1);
+    int ic = min(max((int)(sc * g.nc[2]), 0), g.nc[2] - 1);
+    int c = (ic * g.nc[1] + ib) * g.nc[0] + ia;
+    cell_of[i] = c;
+    slot[i] = atomicAdd(&cell_count[c], 1);
+}
+
+__global__ void k_scan_sums(int ncell, const int *__restrict__ cell_count, int *__restrict__ block_sums) {
+    __shared__ int ws[32];
+    int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+    int s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) s += (base + k < ncell) ? cell_count[base + k] : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        int v = threadIdx.x < SCAN_THREADS / 32 ? ws[threadIdx.x] : 0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) block_sums[blockIdx.x] = v;
+    }
+}
+
+// exclusive scan; also zeroes the histogram for the next step and writes cell_start[ncell] = N
+__global__ void k_scan_apply(int ncell, int N, int *__restrict__ cell_count, const int *__restrict__ block_sums,
+                             int *__restrict__ cell_start) {
+    __shared__ int ws[32];
+    __shared__ int s_prefix;
+    // prefix of the preceding blocks' sums
+    int pre = 0;
+    for (int b = threadIdx.x; b < (int)blockIdx.x; b += blockDim.x) pre += block_sums[b];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) pre += __shfl_down_sync(0xffffffffu, pre, o);
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = pre;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        int v = threadIdx.x < SCAN_THREADS / 32 ? ws[threadIdx.x] : 0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) s_prefix = v;
+    }
+    __syncthreads();
+    int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+    int v[SCAN_ITEMS], tsum = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        v[k] = (base + k < ncell) ? cell_count[base + k] : 0;
+        tsum += v[k];
+    }
+    // inclusive warp scan of thread sums
+    int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int inc = tsum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    __syncthreads();
+    if (lane == 31) ws[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        int w = lane < SCAN_THREADS / 32 ? ws[lane] : 0;
+        int winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, winc, o);
+            if (lane >= o) winc += t;
+        }
+        ws[lane] = winc - w;  // exclusive warp offsets
+    }
+    __syncthreads();
+    int run = s_prefix + ws[wid] + (inc - tsum);
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        if (base + k < ncell) {
+            cell_start[base + k] = run;
+            cell_count[base + k] = 0;
+            run += v[k];
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) cell_start[ncell] = N;
+}
+
+__global__ void k_scatter(int N, const int *__restrict__ cell_of, const int *__restrict__ slot,
+                          const int *__restrict__ cell_start, int *__restrict__ perm) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    perm[cell_start[cell_of[i]] + slot[i]] = i;
+}
+
+template <typename T>
+__global__ void k_cell_sort_gather(int ncell, const int *__restrict__ cell_start, int *__restrict__ perm,
+                                   const T *__restrict__ pos, const unsigned char *__restrict__ flags,
+                                   typename Vec4<T>::type *__restrict__ spos, int *__restrict__ scell) {
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncell) return;
+    int b = cell_start[c], e = cell_start[c + 1];
+    for (int a = b + 1; a < e; ++a) {  // insertion sort by original index
+        int key = perm[a], q = a - 1;
+        while (q >= b && perm[q] > key) { perm[q + 1] = perm[q]; --q; }
+        perm[q + 1] = key;
+    }
+    for (int a = b; a < e; ++a) {
+        int i = perm[a];
+        typename Vec4<T>::type v;
+        v.x = pos[3 * i]; v.y = pos[3 * i + 1]; v.z = pos[3 * i + 2];
+        int fl = flags ? (int)flags[i] : 3;
+        v.w = (T)fl;
+        spos[a] = v;
+        scell[a] = c;
+    }
+}
+
+template <typename T>
+__device__ __forceinline__ bool pair_in_range(const PBox<T> &pb, const BoxD &bd, T rc2T, double rc2,
+                                              const typename Vec4<T>::type &pi,
+                                              const typename Vec4<T>::type &pj);
+
+template <>
+__device__ __forceinline__ bool pair_in_range<double>(const PBox<double> &, const BoxD &bd, double, double rc2,
+                                                      const double4 &pi, const double4 &pj) {
+    return r2_canonical(bd, pj.x - pi.x, pj.y - pi.y, pj.z - pi.z) < rc2;
+}
+
+// fp32: fast test; any pair within a relative band of 1e-5 of rc^2 is re-decided with the canonical
+// fp64 arithmetic on the (exactly representable) fp32 coordinates, so the sets are identical to the
+// fp64 definition (reading O).
+template <>
+__device__ __forceinline__ bool pair_in_range<float>(const PBox<float> &pb, const BoxD &bd, float rc2T, double rc2,
+                                                     const float4 &pi, const float4 &pj) {
+    float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+    min_image(pb, dx, dy, dz);
+    float r2 = dx * dx + dy * dy + dz * dz;
+    bool in = r2 < rc2T;
+    if (fabsf(r2 - rc2T) <= 1e-5f * rc2T)
+        in = r2_canonical(bd, (double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y,
+                          (double)pj.z - (double)pi.z) < rc2;
+    return in;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128)
+k_build_list(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ scell,
+             const int *__restrict__ cell_start, CellGrid g, PBox<T> pb, BoxD bd, T rc2T, double rc2, int maxn,
+             int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    typename Vec4<T>::type pi = spos[s];
+    int c = scell[s];
+    int ia = c % g.nc[0], t = c / g.nc[0];
+    int ib = t % g.nc[1], ic = t / g.nc[1];
+    // offsets visited along a direction: all distinct cells among {-1,0,+1}
+    int za0 = g.nc[0] >= 3 ? -1 : 0, za1 = g.nc[0] >= 2 ? 1 : 0;
+    int zb0 = g.nc[1] >= 3 ? -1 : 0, zb1 = g.nc[1] >= 2 ? 1 : 0;
+    int zc0 = g.nc[2] >= 3 ? -1 : 0, zc1 = g.nc[2] >= 2 ? 1 : 0;
+    int cnt = 0;
+    for (int oc = zc0; oc <= zc1; ++oc) {
+        int jc = ic + oc; jc += jc < 0 ? g.nc[2] : 0; jc -= jc >= g.nc[2] ? g.nc[2] : 0;
+        for (int ob = zb0; ob <= zb1; ++ob) {
+            int jb = ib + ob; jb += jb < 0 ? g.nc[1] : 0; jb -= jb >= g.nc[1] ? g.nc[1] : 0;
+            int rowbase = (jc * g.nc[1] + jb) * g.nc[0];
+            for (int oa = za0; oa <= za1; ++oa) {
+                int ja = ia + oa; ja += ja < 0 ? g.nc[0] : 0; ja -= ja >= g.nc[0] ? g.nc[0] : 0;
+                int cb = cell_start[rowbase + ja], ce = cell_start[rowbase + ja + 1];
+                for (int j = cb; j < ce; ++j) {
+                    typename Vec4<T>::type pj = spos[j];
+                    if (j != s && pair_in_range<T>(pb, bd, rc2T, rc2, pi, pj)) {
+                        if (cnt < maxn) nl[(size_t)cnt * N + s] = j;
+                        ++cnt;
+                    }
+                }
+            }
+        }
+    }
+    if (cnt > maxn) { atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW); cnt = maxn; }
+    nl_count[s] = cnt;
+}
+
+__global__ void k_export_list(int N, int maxn, const int *__restrict__ perm, const int *__restrict__ nl_count,
+                              const int *__restrict__ nl, int *__restrict__ out_count, int *__restrict__ out_list) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    int i = perm[s], cnt = nl_count[s];
+    out_count[i] = cnt;
+    for (int k = 0; k < maxn; ++k) out_list[(size_t)i * maxn + k] = k < cnt ? perm[nl[(size_t)k * N + s]] : -1;
+}
+
+template <typename T>
+static PBox<T> make_pbox(const BoxD &b);
+template <>
+PBox<double> make_pbox<double>(const BoxD &b) {
+    PBox<double> p = { b.ax, b.bx, b.by, b.cx, b.cy, b.cz, 0, 0, 0, 0, 0, 0, b.hx, b.hy, b.hz };
+    return p;
+}
+template <>
+PBox<float> make_pbox<float>(const BoxD &b) {
+    PBox<float> p;
+    const double v[6] = { b.ax, b.bx, b.by, b.cx, b.cy, b.cz };
+    float hi[6], lo[6];
+    for (int k = 0; k < 6; ++k) { hi[k] = (float)v[k]; lo[k] = (float)(v[k] - (double)hi[k]); }
+    p.ax = hi[0]; p.bx = hi[1]; p.by = hi[2]; p.cx = hi[3]; p.cy = hi[4]; p.cz = hi[5];
+    p.lax = lo[0]; p.lbx = lo[1]; p.lby = lo[2]; p.lcx = lo[3]; p.lcy = lo[4]; p.lcz = lo[5];
+    p.hx = (float)b.hx; p.hy = (float)b.hy; p.hz = (float)b.hz;
+    return p;
+}
+template <typename T> PBox<T> ctx_pbox(const metad_ctx *c) { return make_pbox<T>(c->boxd); }
+template PBox<float> ctx_pbox<float>(const metad_ctx *);
+template PBox<double> ctx_pbox<double>(const metad_ctx *);
+
+template <typename T>
+static int nb_build_t(metad_ctx *c, const void *d_pos) {
+    typedef typename Vec4<T>::type V4;
+    const int N = c->N, ncell = c->grid.ncell;
+    cudaStream_t st = c->stream;
+    const int nsb = div_up(ncell, SCAN_TILE);
+    k_bin<T><<<div_up(N, 256), 256, 0, st>>>(N, (const T *)d_pos, c->grid, c->d_cell_of, c->d_slot, c->d_cell_count);
+    k_scan_sums<<<nsb, SCAN_THREADS, 0, st>>>(ncell, c->d_cell_count, c->d_block_sums);
+    k_scan_apply<<<nsb, SCAN_THREADS, 0, st>>>(ncell, N, c->d_cell_count, c->d_block_sums, c->d_cell_start);
+    k_scatter<<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_of, c->d_slot, c->d_cell_start, c->d_perm);
+    k_cell_sort_gather<T><<<div_up(ncell, 128), 128, 0, st>>>(ncell, c->d_cell_start, c->d_perm, (const T *)d_pos,
+                                                             c->has_coord && c->cv[c->coord_dim].use_groups ? c->d_flags : nullptr,
+                                                             (V4 *)c->d_spos, c->d_scell);
+    PBox<T> pb = make_pbox<T>(c->boxd);
+    k_build_list<T><<<div_up(N, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start, c->grid, pb,
+                                                   c->boxd, (T)c->rc2, c->rc2, c->maxn, c->d_nl_count, c->d_nl,
+                                                   c->d_sticky);
+    c->launches += 6;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+int nb_build(metad_ctx *c, const void *d_pos) {
+    return c->prec == 32 ? nb_build_t<float>(c, d_pos) : nb_build_t<double>(c, d_pos);
+}
+
+int nb_export(metad_ctx *c, int *d_count, int *d_list) {
+    k_export_list<<<div_up(c->N, 128), 128, 0, c->stream>>>(c->N, c->maxn, c->d_perm, c->d_nl_count, c->d_nl, d_count,
+                                                            d_list);
+    c->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}

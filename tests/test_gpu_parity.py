@@ -1,0 +1,276 @@
+"""-m gpu: CUDA path (through the C ABI) against the oracle, element by element, on seeded inputs.
+Tolerances are BASELINE.json north_star's: bit-exact neighbour sets, CV / V / dVds 1e-6 relative,
+forces 1e-5 * max|F| absolute (stage-wise, reading S)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2510_06873_b200.inputs import CVSpec, Workload, configs, hill_walk, wrap  # noqa: E402
+
+from gpu_util import (TOL_CV, TOL_F, assert_stagewise, make_hills, positions_for, rel, sorted_rows_fast,  # noqa: E402
+                      stagewise)
+
+
+def _small(name):
+    if name == "c0":
+        return configs.config0()
+    if name == "c0'":
+        return configs.config0(shifted=True)
+    return configs.small(name)
+
+
+@pytest.mark.parametrize("name", ["c0", "c0'", "c1", "c2", "c3", "c4"])
+def test_stagewise_parity_small(name):
+    w = _small(name)
+    r = stagewise(w)
+    assert_stagewise(r)
+    if "q6" in r:
+        tol = 2e-6 if w.precision == 32 else 1e-12
+        assert np.abs(r["q6"] - r["q6_ref"]).max() <= tol
+
+
+def test_c3_fp32_pair_math_meets_the_same_tolerances():
+    w = _small("c3")
+    r = stagewise(w, precision=32)
+    assert_stagewise(r)
+    assert np.abs(r["q6"] - r["q6_ref"]).max() <= 2e-6
+
+
+@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("boxname", ["cubic3cells", "two_cells", "hex120", "hex60", "triclinic"])
+def test_neighbor_sets_bit_exact_on_awkward_boxes(boxname, prec):
+    import oracle
+    import torch
+    from paper_2510_06873_b200.metad import MetaD
+    boxes = {
+        "cubic3cells": (np.array([10.0, 0, 0, 0, 10.0, 0, 0, 0, 10.0]), 3.2),
+        "two_cells": (np.array([9.0, 0, 0, 0, 11.0, 0, 0, 0, 30.0]), 4.4),      # 2 x 2 x 6 cells
+        "hex120": (np.array([24.0, 0, 0, -12.0, 12.0 * np.sqrt(3.0), 0, 0, 0, 19.0]), 4.0),
+        "hex60": (np.array([24.0, 0, 0, 12.0, 12.0 * np.sqrt(3.0), 0, 0, 0, 19.0]), 4.0),
+        "triclinic": (np.array([21.0, 0, 0, 5.0, 20.0, 0, -4.5, 7.0, 23.0]), 3.5),
+    }
+    box, rc = boxes[boxname]
+    rng = np.random.default_rng(17)
+    n = 3000
+    pos = wrap(rng.random((n, 3)) @ box.reshape(3, 3), box)
+    # plant borderline pairs: partner at distance rc*(1 +- tiny) so that the fp32 guard band is exercised
+    for k in range(0, 200, 2):
+        u = rng.standard_normal(3)
+        u /= np.linalg.norm(u)
+        pos[k + 1] = pos[k] + u * rc * (1.0 + (rng.random() - 0.5) * 4e-7)
+    pos = wrap(pos, box)
+    w = Workload(name=boxname, pos=pos, box=box, rc=rc, max_neigh=200, cvs=[CVSpec(kind=0, r0=1.0, scale=1.0)],
+                 sigma=[0.1], n_hills=4, precision=prec)
+    p = positions_for(w, prec)
+    cref, lref, mx = oracle.neighbors(p.astype(np.float64), box, rc, 200, "brute")
+    assert mx <= 200
+    md = MetaD(w, precision=prec)
+    dpos = torch.tensor(p, device="cuda")
+    torch.cuda.synchronize()
+    md.build_neighbors(dpos)
+    cnt, lst = md.neighbors()
+    assert md.status() == 0
+    assert np.array_equal(cnt, cref)
+    assert np.array_equal(sorted_rows_fast(cnt, lst), sorted_rows_fast(cref, lref))
+
+
+def test_deposition_replay_matches_oracle_heights():
+    """Reading K pin on the GPU side: replaying a scripted centre path through metad_bias +
+    metad_deposit reproduces the oracle's well-tempered heights to 1e-9 relative."""
+    import torch
+    from oracle.reference import replay_heights
+    from paper_2510_06873_b200.metad import MetaD
+    w = _small("c1")
+    w.stride = 1
+    H = 300
+    centers = hill_walk(3, [8.0, 0.9], w.sigma, H, step_frac=0.3)
+    href = replay_heights(centers, w.sigma, w.w0, w.kT, w.bias_factor)
+    md = MetaD(w, max_hills=H + 4)
+    with torch.cuda.stream(md.stream):
+        dc = torch.tensor(centers, device="cuda")
+    md.synchronize()
+    for k in range(H):
+        md.bias(cv=dc[k])
+        md.deposit(cv=dc[k])
+    c, h = md.get_hills()
+    assert len(h) == H and np.array_equal(c, centers)
+    assert rel(h, href) <= 1e-9
+    assert md.state()["step"] == H
+
+
+def test_graph_run_end_to_end_and_determinism():
+    """metad_run (CUDA graph, deposition every `stride` steps) against the oracle's step loop, and
+    bit-identical results when repeated (reading P)."""
+    import torch
+    from oracle.reference import OracleMetaD
+    from paper_2510_06873_b200.metad import MetaD
+    w = _small("c3")
+    w.stride = 2
+    nsteps = 7
+    o = OracleMetaD(w)
+    Fo = np.zeros((w.natoms, 3))
+    for _ in range(nsteps):
+        s_ref, V_ref, dV_ref = o.run_step(w.pos, Fo)
+    results = []
+    for rep in range(2):
+        md = MetaD(w, max_hills=64)
+        with torch.cuda.stream(md.stream):
+            dpos = torch.tensor(w.pos, device="cuda")
+            F = torch.zeros((w.natoms, 3), device="cuda", dtype=torch.float64)
+        md.synchronize()
+        md.run(dpos, F, nsteps)
+        st = md.state()
+        c, h = md.get_hills()
+        results.append((F.cpu().numpy(), st, c, h))
+        assert md.status() == 0
+    F, st, c, h = results[0]
+    assert st["step"] == nsteps and st["nhills"] == nsteps // 2 == len(o.heights)
+    assert rel(st["cv"], s_ref) <= TOL_CV
+    assert rel(c, o.centers) <= TOL_CV
+    # end-to-end V differs from the stage-wise bound by |ds * dVds / V| (reading S)
+    bound = TOL_CV + abs((st["cv"][0] - s_ref[0]) * dV_ref[0] / max(abs(V_ref), 1e-300)) + 1e-9
+    assert rel(st["V"], V_ref) <= 10 * bound
+    assert np.abs(F - Fo).max() <= 10 * TOL_F * np.abs(Fo).max()
+    # determinism
+    assert np.array_equal(results[0][0], results[1][0])
+    assert np.array_equal(results[0][3], results[1][3])
+    assert results[0][1]["V"] == results[1][1]["V"]
+
+
+def test_ten_fixed_position_steps_are_bit_identical_config0():
+    """BASELINE.json configs[0]: evaluate V, dV/ds and forces for 10 steps with fixed positions."""
+    import torch
+    from paper_2510_06873_b200.metad import MetaD
+    w = configs.config0(shifted=True)
+    md = MetaD(w)
+    md.set_hills(w.hill_centers, w.hill_heights)
+    dpos = torch.tensor(w.pos, device="cuda")
+    torch.cuda.synchronize()
+    outs = []
+    for _ in range(10):
+        F = torch.zeros((w.natoms, 3), device="cuda", dtype=torch.float64)
+        torch.cuda.synchronize()
+        md.run(dpos, F, 1)
+        st = md.state()
+        outs.append((st["cv"].copy(), st["V"], st["dVds"].copy(), F.cpu().numpy()))
+    for k in range(1, 10):
+        assert np.array_equal(outs[k][0], outs[0][0]) and outs[k][1] == outs[0][1]
+        assert np.array_equal(outs[k][2], outs[0][2]) and np.array_equal(outs[k][3], outs[0][3])
+    assert md.state()["nhills"] == 200          # stride 0: nothing deposited
+
+
+def test_grid_bias_matches_oracle_grid():
+    """Reading M: the grid path is compared with the ORACLE'S grid path (same nodes, same interpolant)."""
+    import torch
+    from oracle.reference import OracleMetaD
+    from paper_2510_06873_b200.metad import MetaD
+    w = _small("c4")
+    pos = positions_for(w, 32)
+    o = OracleMetaD(w)
+    o.build_neighbors(pos.astype(np.float64))
+    s_ref = o.eval_cv(want_grad=False)
+    sig = np.asarray(w.sigma)
+    centers, heights = make_hills(w, s_ref)
+    lo, hi = s_ref - 40 * sig, s_ref + 40 * sig
+    o.enable_grid(w.grid_n, lo, hi)
+    o.set_hills(centers, heights)
+    md = MetaD(w, precision=32, grid=(w.grid_n, lo, hi), max_hills=len(heights) + 8)
+    md.set_hills(centers, heights)
+    tab = md.grid_table()
+    scale = np.abs(o.grid["table"]).reshape(4, -1).max(1)[:, None, None]
+    assert np.abs(tab - o.grid["table"]).max() / 1.0 <= 1e-9 * scale.max()
+    assert (np.abs(tab - o.grid["table"]) / scale).max() <= 1e-10
+    rng = np.random.default_rng(0)
+    for k in range(20):
+        s = s_ref + (rng.random(2) - 0.5) * 20 * sig
+        V_ref, dV_ref = o.bias(s)
+        with torch.cuda.stream(md.stream):
+            ds = torch.tensor(s, device="cuda")
+        V, dV = md.bias(cv=ds)
+        md.synchronize()
+        assert rel(V.cpu().numpy(), V_ref) <= TOL_CV
+        assert np.abs(dV.cpu().numpy() - dV_ref).max() <= TOL_CV * np.abs(dV_ref).max() + 1e-300
+    assert md.status() == 0
+    # outside the table: exact sum + sticky bit
+    s = s_ref + np.array([50.0, 0.0]) * sig
+    with torch.cuda.stream(md.stream):
+        ds = torch.tensor(s, device="cuda")
+    V, dV = md.bias(cv=ds)
+    md.synchronize()
+    V_ref, dV_ref = o.bias(s, use_grid=False)
+    assert rel(V.cpu().numpy(), V_ref) <= TOL_CV
+    assert md.status() & 4
+    # deposition adds the new hill to the table
+    w2 = _small("c4")
+    w2.stride = 1
+    o2 = OracleMetaD(w2)
+    o2.enable_grid(w2.grid_n, lo, hi)
+    o2.set_hills(centers, heights)
+    md2 = MetaD(w2, precision=32, grid=(w2.grid_n, lo, hi), max_hills=len(heights) + 8)
+    md2.set_hills(centers, heights)
+    s = s_ref + np.array([0.4, -0.7]) * sig
+    V0, _ = o2.bias(s)
+    o2.deposit(s, V0)
+    with torch.cuda.stream(md2.stream):
+        ds = torch.tensor(s, device="cuda")
+    md2.bias(cv=ds)
+    md2.deposit(cv=ds)
+    tab2 = md2.grid_table()
+    assert (np.abs(tab2 - o2.grid["table"]) / scale).max() <= 1e-10
+    c, h = md2.get_hills()
+    assert rel(h[-1], o2.heights[-1]) <= 1e-9
+
+
+def test_step_host_round_trip():
+    import torch
+    from paper_2510_06873_b200.metad import MetaD
+    w = _small("c2")
+    r = stagewise(w)
+    md = MetaD(w, max_hills=len(r["heights"]) + 8)
+    md.set_hills(r["centers"], r["heights"])
+    pos_h = torch.tensor(w.pos).pin_memory()
+    F_h = torch.ones((w.natoms, 3), dtype=torch.float64).pin_memory()
+    cv, V = md.step_host(pos_h, F_h)
+    assert rel(cv, r["s_ref"]) <= TOL_CV
+    Fref = 1.0 + r["o"].forces(r["o"].bias(r["s_ref"], use_grid=False)[1])
+    assert np.abs(F_h.numpy() - Fref).max() <= 10 * TOL_F * np.abs(Fref - 1.0).max() + 1e-12
+
+
+def test_errors_and_sticky_bits():
+    import torch
+    from paper_2510_06873_b200 import metad
+    from paper_2510_06873_b200.metad import MetaD, MetadError
+    w = configs.config0()
+    md = MetaD(w)
+    dpos = torch.tensor(w.pos, device="cuda")
+    torch.cuda.synchronize()
+    with pytest.raises(MetadError) as e:
+        md.build_neighbors(dpos, rc=10.0)                     # rc == half the box
+    assert e.value.code == metad.ERR_BOX
+    with pytest.raises(MetadError) as e:
+        md.build_neighbors(dpos, box=np.array([20.0, 1, 0, 0, 20, 0, 0, 0, 20]))
+    assert e.value.code == metad.ERR_BOX
+    md2 = MetaD(w)
+    with pytest.raises(MetadError) as e:
+        md2.eval_cv()                                         # no neighbour list yet
+    assert e.value.code == metad.ERR_STATE
+    # neighbour overflow: capacity 16 < ~56 neighbours -> sticky bit, counts clipped
+    w.max_neigh = 16
+    md3 = MetaD(w)
+    md3.build_neighbors(dpos)
+    cnt, lst = md3.neighbors()
+    assert md3.status() & metad.DEV_NEIGH_OVERFLOW and cnt.max() == 16
+    # hill overflow
+    w4 = configs.config0()
+    w4.stride = 1
+    md4 = MetaD(w4, max_hills=3)
+    F = torch.zeros((w4.natoms, 3), device="cuda", dtype=torch.float64)
+    torch.cuda.synchronize()
+    md4.run(dpos, F, 5)
+    assert md4.status() & metad.DEV_HILL_OVERFLOW and md4.state()["nhills"] == 3
+    # empty hill set: V = 0, forces untouched
+    md5 = MetaD(configs.config0())
+    md5.run(dpos, F.zero_(), 1)
+    st = md5.state()
+    assert st["V"] == 0.0 and float(F.abs().max().cpu()) == 0.0
