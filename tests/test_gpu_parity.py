@@ -52,10 +52,11 @@ def test_neighbor_sets_bit_exact_on_awkward_boxes(boxname, prec):
     }
     box, rc = boxes[boxname]
     rng = np.random.default_rng(17)
-    n = 3000
+    vol = box[0] * box[4] * box[8]
+    n = max(int(0.15 * vol), 64)
     pos = wrap(rng.random((n, 3)) @ box.reshape(3, 3), box)
     # plant borderline pairs: partner at distance rc*(1 +- tiny) so that the fp32 guard band is exercised
-    for k in range(0, 200, 2):
+    for k in range(0, 2 * (n // 8), 2):
         u = rng.standard_normal(3)
         u /= np.linalg.norm(u)
         pos[k + 1] = pos[k] + u * rc * (1.0 + (rng.random() - 0.5) * 4e-7)
