@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py — headline benchmark of the B200 metadynamics hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config c3] [--precision 32|64]
+
+A "step" = one pass of the whole hot path (neighbour build -> CVs -> bias -> forces -> deposit) over
+one synthetic system.  Default workload: BASELINE.json configs[3] (1,024,000-atom GaN-shaped Q6 step,
+10,000 well-tempered hills), the configuration the metric "atom-steps/s at 1M atoms" is quoted on.
+Prints ONE JSON line (rank 0).  Multi-GPU: the path does not shard ("replicas only");
+--gpus N runs N independent replicas, one process per GPU, weak scaling, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "CV+bias+force atom-steps/s at 1M atoms"
+UNIT = "atom-steps/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c3", choices=["c0", "c1", "c2", "c3", "c4"])
+    ap.add_argument("--precision", type=int, default=0, help="0 = the workload's own (c3: 32 for the headline)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fast-setup", action="store_true",
+                    help="profiling runs only: seeded hill heights instead of the well-tempered replay, no e2e leg")
+    ap.add_argument("--stage-times", action="store_true", default=True)
+    return ap.parse_args()
+
+
+def workload(name):
+    from paper_2510_06873_b200.inputs import configs
+    return configs.BUILDERS[name]()
+
+
+def describe(w, precision):
+    kinds = {0: "coordination", 1: "Q6 mean", 2: "Q6 solid-like count", 3: "radius of gyration", 4: "native contacts"}
+    return {"workload": f"BASELINE.json configs[{w.name[1]}] ({w.name})", "atoms": int(w.natoms),
+            "cvs": [kinds[c.kind] for c in w.cvs], "hills": int(w.n_hills), "rc": w.rc,
+            "pair_precision": f"fp{precision}", "stride": int(w.stride),
+            "l2": "per-step working set (neighbour list + q6 records + positions + forces) exceeds the 126 MB L2; no flush"}
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------ oracle arm
+def oracle_sample(name):
+    """A bounded sample of the workload for the CPU oracle (same recipe, fewer atoms)."""
+    from paper_2510_06873_b200.inputs import configs
+    if name == "c3":
+        return configs.config3(cells=(30, 30, 16), sphere_r=18.0, n_hills=10000), "c3 recipe at 30x30x16 cells (57,600 atoms), 10,000 hills"
+    if name == "c4":
+        return configs.config4(cells=(30, 30, 16), sphere_r=18.0, n_hills=20000, grid=(0, 0)), "c4 recipe at 57,600 atoms, 20,000 hills, exact sum"
+    w = configs.BUILDERS[name]()
+    return w, f"{name} at full size"
+
+
+def oracle_time_steps(w, nsteps):
+    """Times the oracle as it stands (never tuned) on the host cores: full steps incl. neighbour build."""
+    import oracle
+    from oracle.reference import OracleMetaD
+    from paper_2510_06873_b200.inputs import hill_walk, seeded_heights
+    o = OracleMetaD(w)
+    o.build_neighbors(w.pos)
+    s0 = o.eval_cv(want_grad=False)
+    if w.hill_centers is not None:
+        o.set_hills(w.hill_centers, w.hill_heights)
+    else:
+        o.set_hills(hill_walk(5, s0, w.sigma, w.n_hills), seeded_heights(5, w.n_hills, w.w0))
+    F = np.zeros((w.natoms, 3))
+    times = []
+    for _ in range(nsteps):
+        t = time.perf_counter()
+        o.run_step(w.pos, F)
+        times.append(time.perf_counter() - t)
+    return times, oracle.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w, desc = oracle_sample(args.config)
+    steps = max(1, min(args.steps, 5))
+    warm = 1 if args.warmup > 0 else 0
+    times, cores = oracle_time_steps(w, warm + steps)
+    times = times[warm:]
+    total = sum(times)
+    value = w.natoms * len(times) / total
+    full = workload(args.config) if args.config in ("c0", "c1", "c2") else None
+    cfg = describe(w if full is None else full, 64)
+    if args.config in ("c3", "c4"):
+        cfg["workload"] = f"BASELINE.json configs[{args.config[1]}] ({args.config})"
+    cfg["sample"] = desc
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": len(times),
+            "warmup": warm, "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------ our arm
+def prepare_hills(w, md_cls, precision, dpos, torch):
+    """Hill centres = seeded walk around the structure's own CV (reading K); heights by replaying the
+    well-tempered rule through the library's own bias+deposit kernels (stride-1 helper context)."""
+    from paper_2510_06873_b200.inputs import hill_walk
+    import copy
+    if w.hill_centers is not None:
+        return np.asarray(w.hill_centers), np.asarray(w.hill_heights)
+    probe = md_cls(w, precision=precision, max_hills=8)
+    probe.build_neighbors(dpos)
+    probe.eval_cv()
+    probe.synchronize()
+    s0 = probe.cv.cpu().numpy()
+    probe.close()
+    centers = hill_walk(5, s0, w.sigma, w.n_hills)
+    w1 = copy.copy(w)
+    w1.stride = 1
+    w1.cvs = w.cvs
+    rep = md_cls(w1, precision=precision, max_hills=w.n_hills + 8)
+    with torch.cuda.stream(rep.stream):
+        dc = torch.tensor(centers, device="cuda")
+    rep.synchronize()
+    for k in range(w.n_hills):
+        rep.bias(cv=dc[k])
+        rep.deposit(cv=dc[k])
+    c, h = rep.get_hills()
+    rep.close()
+    return c, h
+
+
+ALGO_BYTES = {
+    # algorithmic (compulsory) bytes per atom of the dominant kernel k_q6_force, DESIGN.md §6:
+    #   neighbour indices 4*nb + count 4, own position 4*T4, own + gathered-once q6 records 16*T,
+    #   perm 4, force read+write 2*3*T           (nb = mean neighbours, T = bytes per scalar)
+    "q6_force": lambda nb, T: 4 * nb + 4 + 4 * T + 16 * T + 4 + 6 * T,
+}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2510_06873_b200.metad import MetaD
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl ours needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    w = workload(args.config)
+    precision = args.precision or (32 if args.config in ("c3", "c4") else w.precision)
+    tdt = torch.float32 if precision == 32 else torch.float64
+    pos = w.pos.astype(np.float32 if precision == 32 else np.float64)
+    dpos = torch.tensor(pos, device="cuda")
+    torch.cuda.synchronize()
+    if args.fast_setup:
+        from paper_2510_06873_b200.inputs import hill_walk, seeded_heights
+        centers, heights = hill_walk(5, np.full(w.ncv, 0.23), w.sigma, w.n_hills), seeded_heights(5, w.n_hills, w.w0)
+    else:
+        centers, heights = prepare_hills(w, MetaD, precision, dpos, torch)
+
+    grid = None
+    if w.grid_n[0]:
+        sig = np.asarray(w.sigma)
+        grid = (w.grid_n, centers[0] - 120 * sig, centers[0] + 120 * sig)      # reading M
+    md = MetaD(w, precision=precision, max_hills=w.n_hills + args.steps + args.warmup + 4096, grid=grid)
+    md.set_hills(centers, heights)
+    with torch.cuda.stream(md.stream):
+        F = torch.zeros((w.natoms, 3), device="cuda", dtype=tdt)
+    md.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timed region: K graph replays
+    md.run(dpos, F, args.warmup)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = md.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(md.stream)
+    md.run(dpos, F, args.steps)
+    e1.record(md.stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = md.launch_count() - l0
+    # ---- per-stage CUDA-event times (same stream, explicit five calls), inside the same clock-sampled window
+    stage_names = ["build_neighbors", "eval_cv", "bias", "apply_forces", "deposit"]
+    acc = np.zeros(5)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
+    reps = max(3, min(args.steps, 20))
+    for it in range(reps + 2):
+        evs[0].record(md.stream)
+        md.build_neighbors(dpos); evs[1].record(md.stream)
+        md.eval_cv(); evs[2].record(md.stream)
+        md.bias(); evs[3].record(md.stream)
+        md.apply_forces(F); evs[4].record(md.stream)
+        md.deposit(); evs[5].record(md.stream)
+        md.synchronize()
+        if it >= 2:
+            acc += np.array([evs[k].elapsed_time(evs[k + 1]) for k in range(5)])
+    stage_ms = acc / reps
+    clocks = sampler.stop() if rank == 0 else None
+    status = md.status()
+    state = md.state()
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    pos_h = torch.tensor(pos).pin_memory()
+    F_h = torch.zeros((w.natoms, 3), dtype=tdt).pin_memory()
+    for _ in range(min(args.warmup, 3)):
+        md.step_host(pos_h, F_h)
+    barrier()
+    ke = 1 if args.fast_setup else max(3, min(args.steps, 20))
+    t0 = time.perf_counter()
+    for _ in range(ke):
+        md.step_host(pos_h, F_h)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+
+    t_ms = torch.tensor([ms, e2e_s * 1e3], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    ms_max, e2e_ms_max = [float(x) for x in t_ms.cpu()]
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = world * w.natoms * args.steps / (ms_max * 1e-3)
+    e2e_value = world * w.natoms * ke / (e2e_ms_max * 1e-3)
+    tb = 4 if precision == 32 else 8
+    peaks = {}
+    pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(pk):
+        peaks = json.load(open(pk))
+    hbm_peak, peak_src = (peaks["hbm_gbs"], "measured (MEASURED_PEAKS.json hbm_gbs)") if "hbm_gbs" in peaks else (6650.0, "fallback (B200_PROFILING.md)")
+    roof = None
+    if any(c.kind in (1, 2) for c in w.cvs):
+        cnt, _ = md.neighbors()
+        nb = float(cnt.mean())
+        bytes_launch = ALGO_BYTES["q6_force"](nb, tb) * w.natoms
+        dur = stage_ms[3] * 1e-3
+        ach = bytes_launch / dur / 1e9
+        roof = {"kernel": "k_q6_force (stage apply_forces)", "bound": "hbm", "achieved": ach, "peak": hbm_peak,
+                "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": bytes_launch, "kernel_ms": float(stage_ms[3]), "mean_neighbours": nb}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if precision == 32 else "f64", "data": "synthetic", "config": describe(w, precision),
+            "clocks": clocks, "gpu_launches": int(launches),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(2 * pos_h.numel() * tb),
+                    "d2h_bytes_per_step": int(F_h.numel() * tb + 8 * (w.ncv + 1)), "ms_per_step": e2e_ms_max / ke},
+            "roofline": roof,
+            "stages_ms": {n: float(v) for n, v in zip(stage_names, stage_ms)},
+            "state": {"cv": [float(x) for x in state["cv"]], "V": float(state["V"]), "nhills": state["nhills"],
+                      "sticky": status}}
+    if not args.no_cpu_baseline and world == 1:
+        ws, desc = oracle_sample(args.config)
+        times, cores = oracle_time_steps(ws, 2)
+        line["cpu_baseline"] = {"value": ws.natoms / times[-1], "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": desc, "s_per_step": times[-1]}
+    else:
+        line["cpu_baseline"] = None
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
