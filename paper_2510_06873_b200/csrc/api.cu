@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <vector>
 #include "common.cuh"
+#include "tile.cuh"
 
 static thread_local char g_err[512] = "";
 void metad_set_error(const char *msg) { snprintf(g_err, sizeof(g_err), "%s", msg ? msg : ""); }
@@ -44,6 +45,7 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0)
         FAIL(METAD_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
 
+    if (tiled_init()) return METAD_ERR_CUDA;
     metad_ctx *c = new metad_ctx();
     memset(c, 0, sizeof(*c));
     c->p = *p;
@@ -229,7 +231,34 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
     BoxD b = { ax, bx, by, cx, cy, cz, 0.5 * ax, 0.5 * by, 0.5 * cz };
     c->boxd = b;
     c->rc = rc; c->rc2 = rc * rc;
+    // shared-memory tiled fast path: fp32, neighbour-list CVs = Q6 only, >= 3 cells per direction
+    c->tiled = 0;
+    const char *env = getenv("METAD_NO_TILES");
+    if (c->prec == 32 && c->has_q6 && !c->has_coord && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && !(env && env[0] == '1')) {
+        const double rho = (double)c->N / g.ncell, margin = 1.3;
+        const int cap = 1216;
+        double best = 1e30; int bt[3] = { 0, 0, 0 };
+        for (int ty = 1; ty <= 4; ++ty) for (int tz = 1; tz <= 4; ++tz) for (int tx = 1; tx <= TILE_TXMAX; ++tx) {
+            if (tx > g.nc[0] - 2 || ty > g.nc[1] - 2 || tz > g.nc[2] - 2) continue;
+            double own = rho * tx * ty * tz, halo = rho * (tx + 2) * (ty + 2) * (tz + 2);
+            if (halo * margin > cap || own > TILE_THREADS) continue;
+            double score = halo / own + (own < 128 ? 2.0 : 0.0);   // halo ratio; keep the block busy
+            if (score < best) { best = score; bt[0] = tx; bt[1] = ty; bt[2] = tz; }
+        }
+        if (bt[0] > 0) { c->tiled = 1; c->tile_T[0] = bt[0]; c->tile_T[1] = bt[1]; c->tile_T[2] = bt[2]; c->tile_cap = cap; }
+    }
     return METAD_OK;
+}
+
+TileGeom tile_geom(const metad_ctx *c) {
+    TileGeom t;
+    t.Tx = c->tile_T[0]; t.Ty = c->tile_T[1]; t.Tz = c->tile_T[2];
+    t.nc0 = c->grid.nc[0]; t.nc1 = c->grid.nc[1]; t.nc2 = c->grid.nc[2];
+    t.ntx = (t.nc0 + t.Tx - 1) / t.Tx; t.nty = (t.nc1 + t.Ty - 1) / t.Ty; t.ntz = (t.nc2 + t.Tz - 1) / t.Tz;
+    t.cap = c->tile_cap;
+    t.ax = c->boxd.ax; t.bx = c->boxd.bx; t.by = c->boxd.by; t.cx = c->boxd.cx; t.cy = c->boxd.cy; t.cz = c->boxd.cz;
+    t.wa = t.wb = t.wc = 0.0;
+    return t;
 }
 
 extern "C" int metad_build_neighbors(metad_ctx *c, const void *d_pos, const double *h_box, double rc) {

@@ -161,6 +161,8 @@ struct metad_ctx {
     long long launches; int launches_per_step;
     const void *d_pos_last;               // positions snapshot pointer of the last build (chain CVs read it)
     int *d_aux;                           // device scalars: grid-miss flag, index of the hill deposited this step
+    // shared-memory tiled fast path (fp32, Q6): tile.cuh / tiled.cu
+    int tiled; int tile_T[3]; int tile_cap;
 };
 
 static inline const void *ctx_last_pos(const metad_ctx *c) { return c->d_pos_last; }
@@ -182,3 +184,8 @@ int bias_deposit(metad_ctx *c, const double *d_cv, const double *d_V);
 int bias_grid_rebuild(metad_ctx *c);
 int bias_set_hills_dev(metad_ctx *c, const double *d_centers_rowmajor, const double *d_heights, int count);
 int bias_get_hills_dev(metad_ctx *c, double *d_centers_rowmajor, double *d_heights, int capacity);
+int tiled_init();
+int tiled_build(metad_ctx *c);
+int tiled_q6_pass1(metad_ctx *c, double *d_cv);
+int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F);
+int tiled_export(metad_ctx *c, int *d_count, int *d_list);

@@ -265,7 +265,10 @@ static int cv_eval_t(metad_ctx *c, double *d_cv) {
                                                        c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky);
         c->launches++;
     }
-    if (c->has_q6) {
+    if (c->has_q6 && c->tiled) {
+        int r = tiled_q6_pass1(c, d_cv);
+        if (r) return r;
+    } else if (c->has_q6) {
         double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
         double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
         double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
@@ -303,7 +306,10 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
                                                           d_dVds + c->coord_dim, (T *)d_F);
         c->launches++;
     }
-    if (c->has_q6) {
+    if (c->has_q6 && c->tiled) {
+        int r = tiled_q6_force(c, d_dVds, d_F);
+        if (r) return r;
+    } else if (c->has_q6) {
         double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
         double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
         k_q6_force<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb,

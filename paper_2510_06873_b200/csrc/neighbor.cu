@@ -248,6 +248,10 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     k_cell_sort_gather<T><<<div_up(ncell, 128), 128, 0, st>>>(ncell, c->d_cell_start, c->d_perm, (const T *)d_pos,
                                                              c->has_coord && c->cv[c->coord_dim].use_groups ? c->d_flags : nullptr,
                                                              (V4 *)c->d_spos, c->d_scell);
+    if (c->tiled && sizeof(T) == 4) {
+        c->launches += 5;
+        return tiled_build(c);
+    }
     PBox<T> pb = make_pbox<T>(c->boxd);
     k_build_list<T><<<div_up(N, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start, c->grid, pb,
                                                    c->boxd, (T)c->rc2, c->rc2, c->maxn, c->d_nl_count, c->d_nl,
@@ -262,6 +266,7 @@ int nb_build(metad_ctx *c, const void *d_pos) {
 }
 
 int nb_export(metad_ctx *c, int *d_count, int *d_list) {
+    if (c->tiled) return tiled_export(c, d_count, d_list);
     k_export_list<<<div_up(c->N, 128), 128, 0, c->stream>>>(c->N, c->maxn, c->d_perm, c->d_nl_count, c->d_nl, d_count,
                                                             d_list);
     c->launches += 1;

@@ -1,0 +1,204 @@
+// tile.cuh — shared-memory tiling of the cell grid (fp32 fast path).
+//
+// A thread block owns a tile of Tx x Ty x Tz cells.  Its halo = the tile grown by one cell in
+// every direction = (Ty+2)(Tz+2) "rows", each row a run of Tx+2 cells that is contiguous in the
+// cell-sorted atom order (up to a periodic split into <= 3 pieces A|B|C with lattice shift -a|0|+a).
+// The halo atoms are numbered 0..total-1 in (row, piece, atom) order: the LOCAL index.  Neighbour
+// lists of the tiled path store local indices (uint16), so that the CV and force kernels gather
+// positions and q6 records straight from shared memory.
+//
+// Positions are staged in tile-local coordinates  p - origin (+ lattice shift for periodic images):
+// for atoms of the primary cell the subtraction is exact in fp32 (origin is the point of the tile's
+// coordinate range nearest to 0, on a 2^-6 grid), periodic images are formed in fp64 and rounded
+// once.  No per-pair minimum image is needed afterwards.
+#pragma once
+#include "common.cuh"
+
+#define TILE_THREADS 256
+#define TILE_MAXROWS 36          // (Ty+2)(Tz+2), Ty,Tz <= 4
+#define TILE_TXMAX 30
+#define TILE_NSEG (3 * TILE_MAXROWS)
+#define TILE_MAXOWN 16           // Ty*Tz
+
+struct TileGeom {
+    int Tx, Ty, Tz;              // tile size in cells
+    int ntx, nty, ntz;           // tiles per direction
+    int nc0, nc1, nc2;           // cells per direction
+    int cap;                     // halo capacity (atoms) of the shared-memory staging area
+    double ax, bx, by, cx, cy, cz;   // lattice rows
+    double wa, wb, wc;           // cell edge vectors are a/nc0, b/nc1, c/nc2 (used for the tile's coordinate range)
+};
+
+struct TileTables {
+    int seg_g[TILE_NSEG];        // global (sorted-space) index of the segment's first atom
+    int seg_len[TILE_NSEG];
+    int seg_off[TILE_NSEG + 1];  // local index of the segment's first atom
+    double seg_k[TILE_NSEG][3];  // lattice shift - origin (fp64), used for periodic images
+    unsigned char seg_wrapped[TILE_NSEG];
+    int hcell[TILE_MAXROWS][TILE_TXMAX + 3];   // local index where halo cell (row, lx) starts; [Txe+2] = row end
+    short hpiece[TILE_MAXROWS][TILE_TXMAX + 3];
+    int own_g[TILE_MAXOWN];      // global index of the first own atom of own-row q
+    int own_l[TILE_MAXOWN];      // local index of the same atom
+    int own_off[TILE_MAXOWN + 1];
+    int own_row[TILE_MAXOWN];    // halo row id of own-row q
+    float origin[3];
+    int x0, y0, z0, Txe, Tye, Tze, nrows, nown, total, staged;
+};
+
+__device__ __forceinline__ int tile_row_id(const TileTables &t, int hy, int hz) {   // hy,hz in [-1, T*e]
+    return (hz + 1) * (t.Tye + 2) + (hy + 1);
+}
+
+// Builds the tables (all threads of the block must call it).  cell_start: exclusive scan over cells.
+__device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restrict__ cell_start, TileTables &t) {
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        int b = blockIdx.x;
+        int tx = b % g.ntx; b /= g.ntx;
+        int ty = b % g.nty, tz = b / g.nty;
+        t.x0 = tx * g.Tx; t.y0 = ty * g.Ty; t.z0 = tz * g.Tz;
+        t.Txe = min(g.Tx, g.nc0 - t.x0); t.Tye = min(g.Ty, g.nc1 - t.y0); t.Tze = min(g.Tz, g.nc2 - t.z0);
+        t.nrows = (t.Tye + 2) * (t.Tze + 2);
+        // coordinate range of the halo'd tile (8 corners of the parallelepiped), origin = point nearest to 0
+        double lo[3] = { 1e300, 1e300, 1e300 }, hi[3] = { -1e300, -1e300, -1e300 };
+        for (int c = 0; c < 8; ++c) {
+            double fa = (double)(t.x0 - 1 + ((c & 1) ? t.Txe + 2 : 0)) / g.nc0;
+            double fb = (double)(t.y0 - 1 + ((c & 2) ? t.Tye + 2 : 0)) / g.nc1;
+            double fc = (double)(t.z0 - 1 + ((c & 4) ? t.Tze + 2 : 0)) / g.nc2;
+            double p[3] = { fa * g.ax + fb * g.bx + fc * g.cx, fb * g.by + fc * g.cy, fc * g.cz };
+            for (int a = 0; a < 3; ++a) { lo[a] = fmin(lo[a], p[a]); hi[a] = fmax(hi[a], p[a]); }
+        }
+        for (int a = 0; a < 3; ++a) {
+            double o = lo[a] > 0.0 ? lo[a] : (hi[a] < 0.0 ? hi[a] : 0.0);
+            t.origin[a] = (float)(trunc(o * 64.0) * (1.0 / 64.0));   // toward zero, on a 2^-6 grid
+        }
+    }
+    __syncthreads();
+    const int Txe = t.Txe, Tye = t.Tye;
+    if (tid < t.nrows) {
+        const int r = tid;
+        const int hy = r % (Tye + 2) - 1, hz = r / (Tye + 2) - 1;
+        const int ly = t.y0 + hy, lz = t.z0 + hz;
+        const int wy = ly < 0 ? -1 : (ly >= g.nc1 ? 1 : 0), wz = lz < 0 ? -1 : (lz >= g.nc2 ? 1 : 0);
+        const int jy = ly - wy * g.nc1, jz = lz - wz * g.nc2;
+        const int rowbase = (jz * g.nc1 + jy) * g.nc0;
+        const int xa = t.x0 - 1, xb = t.x0 + Txe;
+        for (int p = 0; p < 3; ++p) {
+            int ls = p == 0 ? xa : (p == 1 ? max(xa, 0) : max(xa, g.nc0));
+            int le = p == 0 ? min(xb, -1) : (p == 1 ? min(xb, g.nc0 - 1) : xb);
+            const int wx = p - 1;
+            int s = 3 * r + p;
+            if (ls <= le) {
+                int gs = cell_start[rowbase + ls - wx * g.nc0], ge = cell_start[rowbase + le - wx * g.nc0 + 1];
+                t.seg_g[s] = gs; t.seg_len[s] = ge - gs;
+            } else {
+                t.seg_g[s] = 0; t.seg_len[s] = 0;
+            }
+            t.seg_wrapped[s] = (wx | wy | wz) != 0;
+            t.seg_k[s][0] = wx * g.ax + wy * g.bx + wz * g.cx - (double)t.origin[0];
+            t.seg_k[s][1] = wy * g.by + wz * g.cy - (double)t.origin[1];
+            t.seg_k[s][2] = wz * g.cz - (double)t.origin[2];
+        }
+        for (int lx = xa; lx <= xb; ++lx) {          // halo cell starts relative to their segment
+            int p = lx < 0 ? 0 : (lx >= g.nc0 ? 2 : 1);
+            int cs = cell_start[rowbase + lx - (p - 1) * g.nc0];
+            t.hcell[r][lx - xa] = cs - t.seg_g[3 * r + p];
+            t.hpiece[r][lx - xa] = (short)p;
+        }
+    }
+    for (int s = 3 * t.nrows + tid; s < TILE_NSEG; s += blockDim.x) t.seg_len[s] = 0;
+    __syncthreads();
+    if (tid < 32) {                                   // exclusive scan of seg_len (<= 108 entries) by warp 0
+        int base = tid * 4, v[4], sum = 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { v[k] = (base + k < TILE_NSEG) ? t.seg_len[base + k] : 0; sum += v[k]; }
+        int inc = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, inc, o); if (tid >= o) inc += u; }
+        int run = inc - sum;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { if (base + k < TILE_NSEG) t.seg_off[base + k] = run; run += v[k]; }
+        if (tid == 31) { t.seg_off[TILE_NSEG] = inc; t.total = inc; t.staged = inc <= g.cap; }
+    }
+    __syncthreads();
+    if (tid < t.nrows) {
+        const int r = tid;
+        for (int i = 0; i <= Txe + 1; ++i) t.hcell[r][i] += t.seg_off[3 * r + t.hpiece[r][i]];
+        t.hcell[r][Txe + 2] = t.seg_off[3 * r + 3];   // end of the row = start of the next row's piece A
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int n = 0, q = 0;
+        for (int oz = 0; oz < t.Tze; ++oz)
+            for (int oy = 0; oy < Tye; ++oy, ++q) {
+                int r = tile_row_id(t, oy, oz);
+                int l0 = t.hcell[r][1], l1 = t.hcell[r][Txe + 1];
+                t.own_row[q] = r; t.own_l[q] = l0;
+                t.own_g[q] = t.seg_g[3 * r + 1] + (l0 - t.seg_off[3 * r + 1]);
+                t.own_off[q] = n; n += l1 - l0;
+            }
+        t.own_off[q] = n; t.nown = n;
+        for (int qq = q + 1; qq <= TILE_MAXOWN; ++qq) t.own_off[qq] = n;
+    }
+    __syncthreads();
+}
+
+// local index -> segment (binary search over seg_off; used by the unstaged slow path and the export)
+__device__ __forceinline__ int tile_seg_of(const TileTables &t, int li) {
+    int lo = 0, hi = 3 * t.nrows;        // seg_off[lo] <= li < seg_off[hi]
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (t.seg_off[mid] <= li) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+__device__ __forceinline__ int tile_global_of(const TileTables &t, int li) {
+    int s = tile_seg_of(t, li);
+    return t.seg_g[s] + (li - t.seg_off[s]);
+}
+
+// tile-local position of a halo atom: (x, y, z, as_float(global sorted index))
+__device__ __forceinline__ float4 tile_transform(const TileTables &t, int seg, float4 p, int gidx) {
+    float4 o;
+    if (t.seg_wrapped[seg]) {
+        o.x = (float)((double)p.x + t.seg_k[seg][0]);
+        o.y = (float)((double)p.y + t.seg_k[seg][1]);
+        o.z = (float)((double)p.z + t.seg_k[seg][2]);
+    } else {
+        o.x = p.x - t.origin[0]; o.y = p.y - t.origin[1]; o.z = p.z - t.origin[2];
+    }
+    o.w = __int_as_float(gidx);
+    return o;
+}
+
+// Stages all halo positions into pos_s (warp per segment, coalesced).  No-op if the halo does not fit.
+__device__ __forceinline__ void tile_stage_pos(const TileTables &t, const float4 *__restrict__ spos, float4 *pos_s) {
+    if (!t.staged) return;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int s = wid; s < 3 * t.nrows; s += nw) {
+        const int len = t.seg_len[s], g0 = t.seg_g[s], l0 = t.seg_off[s];
+        for (int i = lane; i < len; i += 32) pos_s[l0 + i] = tile_transform(t, s, spos[g0 + i], g0 + i);
+    }
+}
+
+// position accessor that also works when the tile was not staged (slow path, global memory)
+__device__ __forceinline__ float4 tile_pos(const TileTables &t, const float4 *__restrict__ spos, const float4 *pos_s, int li) {
+    if (t.staged) return pos_s[li];
+    int s = tile_seg_of(t, li);
+    int gi = t.seg_g[s] + (li - t.seg_off[s]);
+    return tile_transform(t, s, spos[gi], gi);
+}
+
+// own atom number a (0..nown-1) -> own-row q
+__device__ __forceinline__ int tile_own_row(const TileTables &t, int a) {
+    int q = 0;
+#pragma unroll 1
+    while (a >= t.own_off[q + 1]) ++q;
+    return q;
+}
+
+// sliced neighbour-list layout: 32 consecutive atoms share a [maxn][32] slab (coalesced for
+// thread-per-atom consumers, compact in memory)
+__device__ __forceinline__ size_t nl_slot(int s, int k, int maxn) {
+    return ((size_t)(s >> 5) * maxn + k) * 32 + (s & 31);
+}

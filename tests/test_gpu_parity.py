@@ -37,9 +37,9 @@ def test_c3_fp32_pair_math_meets_the_same_tolerances():
     assert np.abs(r["q6"] - r["q6_ref"]).max() <= 2e-6
 
 
-@pytest.mark.parametrize("prec", [64, 32])
+@pytest.mark.parametrize("prec,kind", [(64, 0), (32, 0), (32, 1)])      # (32, Q6) takes the shared-memory tiled path
 @pytest.mark.parametrize("boxname", ["cubic3cells", "two_cells", "hex120", "hex60", "triclinic"])
-def test_neighbor_sets_bit_exact_on_awkward_boxes(boxname, prec):
+def test_neighbor_sets_bit_exact_on_awkward_boxes(boxname, prec, kind):
     import oracle
     import torch
     from paper_2510_06873_b200.metad import MetaD
@@ -61,7 +61,7 @@ def test_neighbor_sets_bit_exact_on_awkward_boxes(boxname, prec):
         u /= np.linalg.norm(u)
         pos[k + 1] = pos[k] + u * rc * (1.0 + (rng.random() - 0.5) * 4e-7)
     pos = wrap(pos, box)
-    w = Workload(name=boxname, pos=pos, box=box, rc=rc, max_neigh=200, cvs=[CVSpec(kind=0, r0=1.0, scale=1.0)],
+    w = Workload(name=boxname, pos=pos, box=box, rc=rc, max_neigh=200, cvs=[CVSpec(kind=kind, r0=1.0, scale=1.0)],
                  sigma=[0.1], n_hills=4, precision=prec)
     p = positions_for(w, prec)
     cref, lref, mx = oracle.neighbors(p.astype(np.float64), box, rc, 200, "brute")
