@@ -234,7 +234,8 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
     // shared-memory tiled fast path: fp32, neighbour-list CVs = Q6 only, >= 3 cells per direction
     c->tiled = 0;
     const char *env = getenv("METAD_NO_TILES");
-    if (c->prec == 32 && c->has_q6 && !c->has_coord && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && !(env && env[0] == '1')) {
+    if (c->prec == 32 && c->has_q6 && !c->has_coord && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32 &&
+        !(env && env[0] == '1')) {
         const double rho = (double)c->N / g.ncell, margin = 1.3;
         const int cap = 1216;
         double best = 1e30; int bt[3] = { 0, 0, 0 };
@@ -242,6 +243,8 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
             if (tx > g.nc[0] - 2 || ty > g.nc[1] - 2 || tz > g.nc[2] - 2) continue;
             double own = rho * tx * ty * tz, halo = rho * (tx + 2) * (ty + 2) * (tz + 2);
             if (halo * margin > cap || own > TILE_THREADS) continue;
+            long long ntl = (long long)((g.nc[0] + tx - 1) / tx) * ((g.nc[1] + ty - 1) / ty) * ((g.nc[2] + tz - 1) / tz);
+            if (ntl > c->nblocks_atoms) continue;     // per-tile partials live in the per-block scratch
             double score = halo / own + (own < 128 ? 2.0 : 0.0);   // halo ratio; keep the block busy
             if (score < best) { best = score; bt[0] = tx; bt[1] = ty; bt[2] = tz; }
         }

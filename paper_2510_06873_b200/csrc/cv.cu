@@ -243,6 +243,89 @@ k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
     F[3 * i + 2] += (T)(force_scale * (double)az);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Q6 pass 2 for the tiled fp32 path.  Neighbour entries are (global sorted index | lattice-shift
+// code << 27) in the sliced layout written by k_tile_build.  Per pair: one 128-bit load of the
+// neighbour position and two 256-bit loads (LDG.E.256, sm_100) of its 64-byte q6 record — half the
+// L1 requests of four 128-bit loads, which is what bounds this gather (profiles/r1a_ncu_top3.md).
+// Pairs across a periodic boundary (code != 13, a few %) form d in fp64 from the exact inputs.
+#define NLG_IDX_MASK ((1 << 27) - 1)
+__device__ __forceinline__ void ldg256(const float *p, float4 &a, float4 &b) {
+    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w)
+                 : "l"(p));
+}
+
+__global__ void __launch_bounds__(CV_THREADS)
+k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
+             const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, const float *__restrict__ rec,
+             double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
+             const double *__restrict__ dVds, float *__restrict__ F) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    const float alpha = dim_mean >= 0 ? (float)(dVds[dim_mean] * scale_mean) : 0.f;
+    const float beta = dim_solid >= 0 ? (float)(dVds[dim_solid] * scale_solid) : 0.f;
+    const float4 pi = spos[s];
+    float Bk[13];
+    {
+        float4 a4, b4, c4, d4;
+        ldg256(rec + (size_t)s * METAD_NREC, a4, b4);
+        ldg256(rec + (size_t)s * METAD_NREC + 8, c4, d4);
+        const float gk = alpha + beta * d4.y;
+        Bk[0] = gk * a4.x; Bk[1] = gk * a4.y; Bk[2] = gk * a4.z; Bk[3] = gk * a4.w;
+        Bk[4] = gk * b4.x; Bk[5] = gk * b4.y; Bk[6] = gk * b4.z; Bk[7] = gk * b4.w;
+        Bk[8] = gk * c4.x; Bk[9] = gk * c4.y; Bk[10] = gk * c4.z; Bk[11] = gk * c4.w;
+        Bk[12] = gk * d4.x;
+    }
+    const int *in = nl + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
+    const int cnt = nl_count[s];
+    float fx = 0.f, fy = 0.f, fz = 0.f;
+    for (int k = 0; k < cnt; ++k) {
+        const int e = in[k * 32];
+        const int j = e & NLG_IDX_MASK, code = (unsigned)e >> 27;
+        const float4 pj = spos[j];
+        float4 a4, b4, c4, d4;
+        ldg256(rec + (size_t)j * METAD_NREC, a4, b4);
+        ldg256(rec + (size_t)j * METAD_NREC + 8, c4, d4);
+        float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+        if (code != 13) {
+            const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
+            dx = (float)(((double)pj.x - (double)pi.x) + (wx * bd.ax + wy * bd.bx + wz * bd.cx));
+            dy = (float)(((double)pj.y - (double)pi.y) + (wy * bd.by + wz * bd.cy));
+            dz = (float)(((double)pj.z - (double)pi.z) + (wz * bd.cz));
+        }
+        const float gw = alpha + beta * d4.y;
+        float bb[13];
+        bb[0] = Bk[0] + gw * a4.x; bb[1] = Bk[1] + gw * a4.y; bb[2] = Bk[2] + gw * a4.z; bb[3] = Bk[3] + gw * a4.w;
+        bb[4] = Bk[4] + gw * b4.x; bb[5] = Bk[5] + gw * b4.y; bb[6] = Bk[6] + gw * b4.z; bb[7] = Bk[7] + gw * b4.w;
+        bb[8] = Bk[8] + gw * c4.x; bb[9] = Bk[9] + gw * c4.y; bb[10] = Bk[10] + gw * c4.z; bb[11] = Bk[11] + gw * c4.w;
+        bb[12] = Bk[12] + gw * d4.x;
+        const float rinv = rsqrtf(dx * dx + dy * dy + dz * dz);
+        const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
+        Y6<float> y;
+        y6_eval<float>(ux, uy, uz, y);
+        float gx, gy, gz;
+        y6_grad<float>(y, bb, gx, gy, gz);
+        const float gu = gx * ux + gy * uy + gz * uz;
+        fx += (gx - gu * ux) * rinv; fy += (gy - gu * uy) * rinv; fz += (gz - gu * uz) * rinv;
+    }
+    const int i = perm[s];
+    F[3 * i] += (float)(force_scale * (double)fx);
+    F[3 * i + 1] += (float)(force_scale * (double)fy);
+    F[3 * i + 2] += (float)(force_scale * (double)fz);
+}
+
+int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
+    double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
+    double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
+    k_q6_force_g<<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+        c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm,
+        ss, c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
 template <typename T>
 __global__ void k_q6_export(int N, const int *__restrict__ perm, const T *__restrict__ rec, T *__restrict__ q6) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;

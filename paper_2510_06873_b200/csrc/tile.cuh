@@ -35,7 +35,9 @@ struct TileTables {
     int seg_off[TILE_NSEG + 1];  // local index of the segment's first atom
     double seg_k[TILE_NSEG][3];  // lattice shift - origin (fp64), used for periodic images
     unsigned char seg_wrapped[TILE_NSEG];
+    unsigned char seg_code[TILE_NSEG];  // lattice-shift code (wx+1) + 3(wy+1) + 9(wz+1); 13 = no shift
     int hcell[TILE_MAXROWS][TILE_TXMAX + 3];   // local index where halo cell (row, lx) starts; [Txe+2] = row end
+    int hend[TILE_MAXROWS][TILE_TXMAX + 3];    // scratch of the setup: cell_start[cell + 1]
     short hpiece[TILE_MAXROWS][TILE_TXMAX + 3];
     int own_g[TILE_MAXOWN];      // global index of the first own atom of own-row q
     int own_l[TILE_MAXOWN];      // local index of the same atom
@@ -50,21 +52,37 @@ __device__ __forceinline__ int tile_row_id(const TileTables &t, int hy, int hz) 
 }
 
 // Builds the tables (all threads of the block must call it).  cell_start: exclusive scan over cells.
+// Four barrier-separated phases; every global load (two per halo cell) is issued in phase 1 by a
+// different thread, so the block pays the L2 latency once.
 __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restrict__ cell_start, TileTables &t) {
     const int tid = threadIdx.x;
+    int b = blockIdx.x;
+    const int tx = b % g.ntx; b /= g.ntx;
+    const int ty = b % g.nty, tz = b / g.nty;
+    const int x0 = tx * g.Tx, y0 = ty * g.Ty, z0 = tz * g.Tz;
+    const int Txe = min(g.Tx, g.nc0 - x0), Tye = min(g.Ty, g.nc1 - y0), Tze = min(g.Tz, g.nc2 - z0);
+    const int nrows = (Tye + 2) * (Tze + 2), ncol = Txe + 2;
+    const int xa = x0 - 1;
+    // ---- phase 1: cell_start of every halo cell (both ends); thread 0 also fixes the tile origin
+    for (int i = tid; i < nrows * ncol; i += blockDim.x) {
+        const int r = i / ncol, c = i - r * ncol;
+        const int hy = r % (Tye + 2) - 1, hz = r / (Tye + 2) - 1;
+        const int ly = y0 + hy, lz = z0 + hz, lx = xa + c;
+        const int jy = ly < 0 ? ly + g.nc1 : (ly >= g.nc1 ? ly - g.nc1 : ly);
+        const int jz = lz < 0 ? lz + g.nc2 : (lz >= g.nc2 ? lz - g.nc2 : lz);
+        const int jx = lx < 0 ? lx + g.nc0 : (lx >= g.nc0 ? lx - g.nc0 : lx);
+        const int id = (jz * g.nc1 + jy) * g.nc0 + jx;
+        t.hcell[r][c] = cell_start[id];
+        t.hend[r][c] = cell_start[id + 1];
+    }
     if (tid == 0) {
-        int b = blockIdx.x;
-        int tx = b % g.ntx; b /= g.ntx;
-        int ty = b % g.nty, tz = b / g.nty;
-        t.x0 = tx * g.Tx; t.y0 = ty * g.Ty; t.z0 = tz * g.Tz;
-        t.Txe = min(g.Tx, g.nc0 - t.x0); t.Tye = min(g.Ty, g.nc1 - t.y0); t.Tze = min(g.Tz, g.nc2 - t.z0);
-        t.nrows = (t.Tye + 2) * (t.Tze + 2);
+        t.x0 = x0; t.y0 = y0; t.z0 = z0; t.Txe = Txe; t.Tye = Tye; t.Tze = Tze; t.nrows = nrows;
         // coordinate range of the halo'd tile (8 corners of the parallelepiped), origin = point nearest to 0
         double lo[3] = { 1e300, 1e300, 1e300 }, hi[3] = { -1e300, -1e300, -1e300 };
         for (int c = 0; c < 8; ++c) {
-            double fa = (double)(t.x0 - 1 + ((c & 1) ? t.Txe + 2 : 0)) / g.nc0;
-            double fb = (double)(t.y0 - 1 + ((c & 2) ? t.Tye + 2 : 0)) / g.nc1;
-            double fc = (double)(t.z0 - 1 + ((c & 4) ? t.Tze + 2 : 0)) / g.nc2;
+            double fa = (double)(x0 - 1 + ((c & 1) ? Txe + 2 : 0)) / g.nc0;
+            double fb = (double)(y0 - 1 + ((c & 2) ? Tye + 2 : 0)) / g.nc1;
+            double fc = (double)(z0 - 1 + ((c & 4) ? Tze + 2 : 0)) / g.nc2;
             double p[3] = { fa * g.ax + fb * g.bx + fc * g.cx, fb * g.by + fc * g.cy, fc * g.cz };
             for (int a = 0; a < 3; ++a) { lo[a] = fmin(lo[a], p[a]); hi[a] = fmax(hi[a], p[a]); }
         }
@@ -73,42 +91,37 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
             t.origin[a] = (float)(trunc(o * 64.0) * (1.0 / 64.0));   // toward zero, on a 2^-6 grid
         }
     }
+    for (int s = 3 * nrows + tid; s < TILE_NSEG; s += blockDim.x) t.seg_len[s] = 0;
     __syncthreads();
-    const int Txe = t.Txe, Tye = t.Tye;
-    if (tid < t.nrows) {
+    // ---- phase 2: the <= 3 segments of every row, halo-cell starts relative to their segment
+    if (tid < nrows) {
         const int r = tid;
         const int hy = r % (Tye + 2) - 1, hz = r / (Tye + 2) - 1;
-        const int ly = t.y0 + hy, lz = t.z0 + hz;
+        const int ly = y0 + hy, lz = z0 + hz;
         const int wy = ly < 0 ? -1 : (ly >= g.nc1 ? 1 : 0), wz = lz < 0 ? -1 : (lz >= g.nc2 ? 1 : 0);
-        const int jy = ly - wy * g.nc1, jz = lz - wz * g.nc2;
-        const int rowbase = (jz * g.nc1 + jy) * g.nc0;
-        const int xa = t.x0 - 1, xb = t.x0 + Txe;
+        const int xb = x0 + Txe;
+        int segg[3];
         for (int p = 0; p < 3; ++p) {
-            int ls = p == 0 ? xa : (p == 1 ? max(xa, 0) : max(xa, g.nc0));
-            int le = p == 0 ? min(xb, -1) : (p == 1 ? min(xb, g.nc0 - 1) : xb);
-            const int wx = p - 1;
-            int s = 3 * r + p;
-            if (ls <= le) {
-                int gs = cell_start[rowbase + ls - wx * g.nc0], ge = cell_start[rowbase + le - wx * g.nc0 + 1];
-                t.seg_g[s] = gs; t.seg_len[s] = ge - gs;
-            } else {
-                t.seg_g[s] = 0; t.seg_len[s] = 0;
-            }
+            const int ls = p == 0 ? xa : (p == 1 ? max(xa, 0) : max(xa, g.nc0));
+            const int le = p == 0 ? min(xb, -1) : (p == 1 ? min(xb, g.nc0 - 1) : xb);
+            const int wx = p - 1, s = 3 * r + p;
+            if (ls <= le) { segg[p] = t.hcell[r][ls - xa]; t.seg_g[s] = segg[p]; t.seg_len[s] = t.hend[r][le - xa] - segg[p]; }
+            else { segg[p] = 0; t.seg_g[s] = 0; t.seg_len[s] = 0; }
             t.seg_wrapped[s] = (wx | wy | wz) != 0;
+            t.seg_code[s] = (unsigned char)((wx + 1) + 3 * (wy + 1) + 9 * (wz + 1));
             t.seg_k[s][0] = wx * g.ax + wy * g.bx + wz * g.cx - (double)t.origin[0];
             t.seg_k[s][1] = wy * g.by + wz * g.cy - (double)t.origin[1];
             t.seg_k[s][2] = wz * g.cz - (double)t.origin[2];
         }
-        for (int lx = xa; lx <= xb; ++lx) {          // halo cell starts relative to their segment
-            int p = lx < 0 ? 0 : (lx >= g.nc0 ? 2 : 1);
-            int cs = cell_start[rowbase + lx - (p - 1) * g.nc0];
-            t.hcell[r][lx - xa] = cs - t.seg_g[3 * r + p];
-            t.hpiece[r][lx - xa] = (short)p;
+        for (int c = 0; c < ncol; ++c) {
+            const int lx = xa + c, p = lx < 0 ? 0 : (lx >= g.nc0 ? 2 : 1);
+            t.hcell[r][c] -= segg[p];
+            t.hpiece[r][c] = (short)p;
         }
     }
-    for (int s = 3 * t.nrows + tid; s < TILE_NSEG; s += blockDim.x) t.seg_len[s] = 0;
     __syncthreads();
-    if (tid < 32) {                                   // exclusive scan of seg_len (<= 108 entries) by warp 0
+    // ---- phase 3: exclusive scan of seg_len (<= 108 entries) by warp 0
+    if (tid < 32) {
         int base = tid * 4, v[4], sum = 0;
 #pragma unroll
         for (int k = 0; k < 4; ++k) { v[k] = (base + k < TILE_NSEG) ? t.seg_len[base + k] : 0; sum += v[k]; }
@@ -121,17 +134,18 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
         if (tid == 31) { t.seg_off[TILE_NSEG] = inc; t.total = inc; t.staged = inc <= g.cap; }
     }
     __syncthreads();
-    if (tid < t.nrows) {
+    // ---- phase 4: local halo-cell starts; own rows
+    if (tid < nrows) {
         const int r = tid;
-        for (int i = 0; i <= Txe + 1; ++i) t.hcell[r][i] += t.seg_off[3 * r + t.hpiece[r][i]];
-        t.hcell[r][Txe + 2] = t.seg_off[3 * r + 3];   // end of the row = start of the next row's piece A
+        for (int c = 0; c < ncol; ++c) t.hcell[r][c] += t.seg_off[3 * r + t.hpiece[r][c]];
+        t.hcell[r][ncol] = t.seg_off[3 * r + 3];      // end of the row = start of the next row's piece A
     }
     __syncthreads();
     if (tid == 0) {
         int n = 0, q = 0;
-        for (int oz = 0; oz < t.Tze; ++oz)
+        for (int oz = 0; oz < Tze; ++oz)
             for (int oy = 0; oy < Tye; ++oy, ++q) {
-                int r = tile_row_id(t, oy, oz);
+                int r = (oz + 1) * (Tye + 2) + (oy + 1);
                 int l0 = t.hcell[r][1], l1 = t.hcell[r][Txe + 1];
                 t.own_row[q] = r; t.own_l[q] = l0;
                 t.own_g[q] = t.seg_g[3 * r + 1] + (l0 - t.seg_off[3 * r + 1]);
@@ -157,7 +171,12 @@ __device__ __forceinline__ int tile_global_of(const TileTables &t, int li) {
     return t.seg_g[s] + (li - t.seg_off[s]);
 }
 
-// tile-local position of a halo atom: (x, y, z, as_float(global sorted index))
+// neighbour-list entry of the tiled path: global sorted index | lattice-shift code << 27
+#define NL_IDX_BITS 27
+#define NL_IDX_MASK ((1 << NL_IDX_BITS) - 1)
+#define NL_CODE_NONE 13
+
+// tile-local position of a halo atom: (x, y, z, as_float(global sorted index | shift code << 27))
 __device__ __forceinline__ float4 tile_transform(const TileTables &t, int seg, float4 p, int gidx) {
     float4 o;
     if (t.seg_wrapped[seg]) {
@@ -167,7 +186,7 @@ __device__ __forceinline__ float4 tile_transform(const TileTables &t, int seg, f
     } else {
         o.x = p.x - t.origin[0]; o.y = p.y - t.origin[1]; o.z = p.z - t.origin[2];
     }
-    o.w = __int_as_float(gidx);
+    o.w = __int_as_float(gidx | ((int)t.seg_code[seg] << NL_IDX_BITS));
     return o;
 }
 
