@@ -160,6 +160,23 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------------------------------ multi-process plumbing
+def max_over_ranks(values, device="cuda"):
+    """Element-wise max over all ranks of a list of floats (device-timed durations): the whole job is
+    as slow as its slowest replica.  Works with NCCL (cuda tensors) and gloo (cpu tensors)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), device=device, dtype=torch.float64)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.cpu()]
+
+
+def job_throughput(world, atoms_per_replica, steps, ms_max):
+    """Replicas only: N independent copies of the workload, value = all atoms x steps / slowest time."""
+    return world * atoms_per_replica * steps / (ms_max * 1e-3)
+
+
 # ------------------------------------------------------------------------------------------ our arm
 def prepare_hills(w, md_cls, precision, dpos, torch):
     """Hill centres = seeded walk around the structure's own CV (reading K); heights by replaying the
@@ -190,12 +207,20 @@ def prepare_hills(w, md_cls, precision, dpos, torch):
     return c, h
 
 
-ALGO_BYTES = {
-    # algorithmic (compulsory) bytes per atom of the dominant kernel k_q6_force, DESIGN.md §6:
-    #   neighbour indices 4*nb + count 4, own position 4*T4, own + gathered-once q6 records 16*T,
-    #   perm 4, force read+write 2*3*T           (nb = mean neighbours, T = bytes per scalar)
-    "q6_force": lambda nb, T: 4 * nb + 4 + 4 * T + 16 * T + 4 + 6 * T,
-}
+# Algorithmic (compulsory) work per atom, DESIGN.md §6.  nb = mean neighbours, T = bytes per scalar.
+def algo_q6_force_bytes(nb, T):
+    # neighbour entries 4*nb + count 4, own position 4*T, q6 records 16*T (each read once), perm 4, force read+write 6*T
+    return 4 * nb + 4 + 4 * T + 16 * T + 4 + 6 * T
+
+
+def algo_build_flops(nb, cand=113.0):
+    # candidate scan: 3 sub + (1 mul + 2 fma = 5 flop) + 1 compare = 9 flop per candidate (27 cells x 4.2 atoms = 113);
+    # fused Q6 pass 1 per neighbour: r2 5, rsqrt 1, unit vector 3, E polynomials 20, (x+iy)^m recurrence 30, 13 fma = 26 -> 85
+    return 9.0 * cand + 85.0 * nb
+
+
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # nominal FMA peak from the guide's unit counts and clocks
+ISSUE_PEAK_GINST = 148 * 4 * 1.965                      # warp instructions / ns
 
 
 def run_ours(args):
@@ -270,6 +295,17 @@ def run_ours(args):
         if it >= 2:
             acc += np.array([evs[k].elapsed_time(evs[k + 1]) for k in range(5)])
     stage_ms = acc / reps
+    sort_ms = list_ms = None
+    try:
+        md.set_timing(True)
+        ts = []
+        for it in range(5):
+            md.build_neighbors(dpos)
+            ts.append(md.get_timing())
+        md.set_timing(False)
+        sort_ms, list_ms = float(np.median([t[0] for t in ts[1:]])), float(np.median([t[1] for t in ts[1:]]))
+    except Exception:
+        pass
     clocks = sampler.stop() if rank == 0 else None
     status = md.status()
     state = md.state()
@@ -287,40 +323,56 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
 
-    t_ms = torch.tensor([ms, e2e_s * 1e3], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-    ms_max, e2e_ms_max = [float(x) for x in t_ms.cpu()]
+    ms_max, e2e_ms_max = max_over_ranks([ms, e2e_s * 1e3])
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    value = world * w.natoms * args.steps / (ms_max * 1e-3)
-    e2e_value = world * w.natoms * ke / (e2e_ms_max * 1e-3)
+    value = job_throughput(world, w.natoms, args.steps, ms_max)
+    e2e_value = job_throughput(world, w.natoms, ke, e2e_ms_max)
     tb = 4 if precision == 32 else 8
     peaks = {}
     pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(pk):
         peaks = json.load(open(pk))
     hbm_peak, peak_src = (peaks["hbm_gbs"], "measured (MEASURED_PEAKS.json hbm_gbs)") if "hbm_gbs" in peaks else (6650.0, "fallback (B200_PROFILING.md)")
-    roof = None
+    roof, roof_all = None, []
+    traffic = {}
+    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(f"{args.config}_fp{precision}", {})
     if any(c.kind in (1, 2) for c in w.cvs):
         cnt, _ = md.neighbors()
         nb = float(cnt.mean())
-        bytes_launch = ALGO_BYTES["q6_force"](nb, tb) * w.natoms
-        dur = stage_ms[3] * 1e-3
-        ach = bytes_launch / dur / 1e9
-        roof = {"kernel": "k_q6_force (stage apply_forces)", "bound": "hbm", "achieved": ach, "peak": hbm_peak,
-                "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": bytes_launch, "kernel_ms": float(stage_ms[3]), "mean_neighbours": nb}
+        # a6: the gather-form force kernel against the HBM roofline (north_star: "HBM GB/s ... for the force pass")
+        bytes_launch = algo_q6_force_bytes(nb, tb) * w.natoms
+        ach = bytes_launch / (stage_ms[3] * 1e-3) / 1e9
+        kname = "k_q6_force_g" if precision == 32 else "k_q6_force<double>"
+        r_force = {"kernel": f"{kname} (stage apply_forces)", "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s",
+                   "frac": ach / hbm_peak, "traffic": traffic.get("force_dram_bytes"), "peak_source": peak_src,
+                   "algorithmic_bytes_per_launch": bytes_launch, "kernel_ms": float(stage_ms[3]), "mean_neighbours": nb}
+        roof_all.append(r_force)
+        roof = r_force
+        if precision == 32 and list_ms is not None:
+            # a1+a3: candidate scan fused with Q6 pass 1 — plain FP32 ALU / issue bound (no tensor-core work on this path)
+            fl = algo_build_flops(nb) * w.natoms
+            ach_tf = fl / (list_ms * 1e-3) / 1e12
+            r_build = {"kernel": "k_tile_build<Q6> (list phase of build_neighbors)", "bound": "alu", "achieved": ach_tf,
+                       "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach_tf / FP32_PEAK_TFLOPS,
+                       "traffic": traffic.get("build_dram_bytes"),
+                       "peak_source": "nominal FP32 FMA peak: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md §7)",
+                       "algorithmic_flops_per_launch": fl, "kernel_ms": float(list_ms), "sort_phase_ms": float(sort_ms)}
+            roof_all.append(r_build)
+            if list_ms > stage_ms[3]:
+                roof = r_build                     # the dominant kernel of the step
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if precision == 32 else "f64", "data": "synthetic", "config": describe(w, precision),
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(2 * pos_h.numel() * tb),
                     "d2h_bytes_per_step": int(F_h.numel() * tb + 8 * (w.ncv + 1)), "ms_per_step": e2e_ms_max / ke},
-            "roofline": roof,
+            "roofline": roof, "roofline_kernels": roof_all,
             "stages_ms": {n: float(v) for n, v in zip(stage_names, stage_ms)},
             "state": {"cv": [float(x) for x in state["cv"]], "V": float(state["V"]), "nhills": state["nhills"],
                       "sticky": status}}

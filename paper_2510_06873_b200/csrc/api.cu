@@ -172,6 +172,7 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     CUDA_TRY(dev_alloc(&c->d_aux, 4));
     int aux0[4] = { 0, -1, 0, 0 };
     CUDA_TRY(cudaMemcpy(c->d_aux, aux0, sizeof(aux0), cudaMemcpyHostToDevice));
+    for (int k = 0; k < 3; ++k) CUDA_TRY(cudaEventCreate(&c->ev[k]));
     CUDA_TRY(cudaDeviceSynchronize());
     *out = c;
     return METAD_OK;
@@ -181,6 +182,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     if (!c) return METAD_OK;
     cudaStreamSynchronize(c->stream);
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    for (int k = 0; k < 3; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
@@ -316,7 +318,9 @@ extern "C" int metad_run(metad_ctx *c, const void *d_pos, const double *h_box, d
         long long before = c->launches;
         cudaGraph_t graph;
         CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+        c->capturing = 1;
         r = enqueue_step(c, d_pos, h_box, rc, d_F);
+        c->capturing = 0;
         cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
         if (r) { if (e == cudaSuccess) cudaGraphDestroy(graph); return r; }
         CUDA_TRY(e);
@@ -436,6 +440,21 @@ extern "C" int metad_get_grid(metad_ctx *c, double *d_table) {
 extern "C" int metad_reset_steps(metad_ctx *c) {
     if (!c) FAIL(METAD_ERR_ARG, "null argument");
     CUDA_TRY(cudaMemsetAsync(c->d_step, 0, sizeof(int), c->stream));
+    return METAD_OK;
+}
+
+extern "C" int metad_set_timing(metad_ctx *c, int enabled) {
+    if (!c) FAIL(METAD_ERR_ARG, "null argument");
+    c->timing = enabled != 0;
+    return METAD_OK;
+}
+
+extern "C" int metad_get_timing(metad_ctx *c, float *ms_sort, float *ms_list) {
+    if (!c || !ms_sort || !ms_list) FAIL(METAD_ERR_ARG, "null argument");
+    if (!c->timing) FAIL(METAD_ERR_STATE, "timing is not enabled");
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    CUDA_TRY(cudaEventElapsedTime(ms_sort, c->ev[0], c->ev[1]));
+    CUDA_TRY(cudaEventElapsedTime(ms_list, c->ev[1], c->ev[2]));
     return METAD_OK;
 }
 

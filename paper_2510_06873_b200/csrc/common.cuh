@@ -163,6 +163,7 @@ struct metad_ctx {
     int *d_aux;                           // device scalars: grid-miss flag, index of the hill deposited this step
     // shared-memory tiled fast path (fp32, Q6): tile.cuh / tiled.cu
     int tiled; int tile_T[3]; int tile_cap;
+    int timing; int capturing; cudaEvent_t ev[3];
 };
 
 static inline const void *ctx_last_pos(const metad_ctx *c) { return c->d_pos_last; }

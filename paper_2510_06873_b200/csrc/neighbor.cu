@@ -241,6 +241,8 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     const int N = c->N, ncell = c->grid.ncell;
     cudaStream_t st = c->stream;
     const int nsb = div_up(ncell, SCAN_TILE);
+    const bool tm = c->timing && !c->capturing;
+    if (tm) cudaEventRecord(c->ev[0], st);
     k_bin<T><<<div_up(N, 256), 256, 0, st>>>(N, (const T *)d_pos, c->grid, c->d_cell_of, c->d_slot, c->d_cell_count);
     k_scan_sums<<<nsb, SCAN_THREADS, 0, st>>>(ncell, c->d_cell_count, c->d_block_sums);
     k_scan_apply<<<nsb, SCAN_THREADS, 0, st>>>(ncell, N, c->d_cell_count, c->d_block_sums, c->d_cell_start);
@@ -248,14 +250,18 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     k_cell_sort_gather<T><<<div_up(ncell, 128), 128, 0, st>>>(ncell, c->d_cell_start, c->d_perm, (const T *)d_pos,
                                                              c->has_coord && c->cv[c->coord_dim].use_groups ? c->d_flags : nullptr,
                                                              (V4 *)c->d_spos, c->d_scell);
+    if (tm) cudaEventRecord(c->ev[1], st);
     if (c->tiled && sizeof(T) == 4) {
         c->launches += 5;
-        return tiled_build(c);
+        int r = tiled_build(c);
+        if (tm) cudaEventRecord(c->ev[2], st);
+        return r;
     }
     PBox<T> pb = make_pbox<T>(c->boxd);
     k_build_list<T><<<div_up(N, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start, c->grid, pb,
                                                    c->boxd, (T)c->rc2, c->rc2, c->maxn, c->d_nl_count, c->d_nl,
                                                    c->d_sticky);
+    if (tm) cudaEventRecord(c->ev[2], st);
     c->launches += 6;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

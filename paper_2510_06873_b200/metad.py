@@ -42,7 +42,7 @@ class Params(ctypes.Structure):
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
            "metad_apply_forces", "metad_deposit", "metad_run", "metad_step_host", "metad_status",
            "metad_get_state", "metad_get_neighbors", "metad_get_q6", "metad_set_hills", "metad_get_hills",
-           "metad_get_grid", "metad_reset_steps", "metad_launch_count", "metad_version", "metad_last_error"]
+           "metad_get_grid", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
 
 _lib = None
 
@@ -73,6 +73,8 @@ def load():
     L.metad_get_hills.argtypes = [_P, _P, _P, _I, _P, _I]
     L.metad_get_grid.argtypes = [_P, _P]
     L.metad_reset_steps.argtypes = [_P]
+    L.metad_set_timing.argtypes = [_P, _I]
+    L.metad_get_timing.argtypes = [_P, _P, _P]
     L.metad_launch_count.argtypes = [_P]
     L.metad_launch_count.restype = ctypes.c_longlong
     L.metad_version.restype = ctypes.c_char_p
@@ -261,6 +263,14 @@ class MetaD:
 
     def reset_steps(self):
         _check(load().metad_reset_steps(self._h))
+
+    def set_timing(self, on=True):
+        _check(load().metad_set_timing(self._h, int(bool(on))))
+
+    def get_timing(self):
+        a, b = ctypes.c_float(0), ctypes.c_float(0)
+        _check(load().metad_get_timing(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
 
     def launch_count(self):
         return int(load().metad_launch_count(self._h))
