@@ -39,7 +39,8 @@ enum metad_error { METAD_OK = 0, METAD_ERR_ARG = 1, METAD_ERR_BOX = 2, METAD_ERR
                    METAD_ERR_CUDA = 4, METAD_ERR_NOMEM = 5 };
 
 enum metad_dev_bits { METAD_DEV_NEIGH_OVERFLOW = 1, METAD_DEV_HILL_OVERFLOW = 2,
-                      METAD_DEV_GRID_RANGE = 4, METAD_DEV_NONFINITE = 8 };
+                      METAD_DEV_GRID_RANGE = 4, METAD_DEV_NONFINITE = 8,
+                      METAD_DEV_POS_RANGE = 16 /* a position lies outside the primary cell */ };
 
 enum metad_cv_kind {
     METAD_CV_COORD = 0,    /* s = scale * sum_{i in A} sum_{j in B, j!=i, r<rc} sw(r_ij/r0),

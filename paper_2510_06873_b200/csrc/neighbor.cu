@@ -15,17 +15,21 @@
 
 template <typename T>
 __global__ void k_bin(int N, const T *__restrict__ pos, CellGrid g, int *__restrict__ cell_of,
-                      int *__restrict__ slot, int *__restrict__ cell_count) {
+                      int *__restrict__ slot, int *__restrict__ cell_count, unsigned int *__restrict__ sticky) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     double x = (double)pos[3 * i], y = (double)pos[3 * i + 1], z = (double)pos[3 * i + 2];
     double sc = z * g.inv[2];
     double sb = (y - sc * g.cy) * g.inv[1];
     double sa = (x - sb * g.bx - sc * g.cx) * g.inv[0];
-    sa -= floor(sa); sb -= floor(sb); sc -= floor(sc);
-    int ia = min(max((int)(sa * g.nc[0]), 0), g.nc[0] - 1);
-    int ib = min(max((int)(sb * g.nc[1]), 0), g.nc[1] - 1);
-    int ic = min(max((int)(sc * g.nc[2]), 0), g.nc[2] - 1);
+    // Positions must lie in the primary cell (include/metad.h).  A coordinate that rounds to the far face (fractional
+    // 1.0 + eps, e.g. after fp32 rounding) is CLAMPED into the boundary cell, not wrapped: its cartesian coordinates are
+    // next to that cell's atoms, which is what the lattice-shift logic of the tiled path relies on.
+    if (fabs(sa - 0.5) > 0.5001 || fabs(sb - 0.5) > 0.5001 || fabs(sc - 0.5) > 0.5001)
+        atomicOr(sticky, (unsigned)METAD_DEV_POS_RANGE);
+    int ia = min(max((int)floor(sa * g.nc[0]), 0), g.nc[0] - 1);
+    int ib = min(max((int)floor(sb * g.nc[1]), 0), g.nc[1] - 1);
+    int ic = min(max((int)floor(sc * g.nc[2]), 0), g.nc[2] - 1);
     int c = (ic * g.nc[1] + ib) * g.nc[0] + ia;
     cell_of[i] = c;
     slot[i] = atomicAdd(&cell_count[c], 1);
@@ -243,7 +247,8 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     const int nsb = div_up(ncell, SCAN_TILE);
     const bool tm = c->timing && !c->capturing;
     if (tm) cudaEventRecord(c->ev[0], st);
-    k_bin<T><<<div_up(N, 256), 256, 0, st>>>(N, (const T *)d_pos, c->grid, c->d_cell_of, c->d_slot, c->d_cell_count);
+    k_bin<T><<<div_up(N, 256), 256, 0, st>>>(N, (const T *)d_pos, c->grid, c->d_cell_of, c->d_slot, c->d_cell_count,
+                                             c->d_sticky);
     k_scan_sums<<<nsb, SCAN_THREADS, 0, st>>>(ncell, c->d_cell_count, c->d_block_sums);
     k_scan_apply<<<nsb, SCAN_THREADS, 0, st>>>(ncell, N, c->d_cell_count, c->d_block_sums, c->d_cell_start);
     k_scatter<<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_of, c->d_slot, c->d_cell_start, c->d_perm);

@@ -275,3 +275,35 @@ def test_errors_and_sticky_bits():
     md5.run(dpos, F.zero_(), 1)
     st = md5.state()
     assert st["V"] == 0.0 and float(F.abs().max().cpu()) == 0.0
+
+
+def test_positions_that_round_onto_the_far_box_face_fp32_tiled():
+    """Regression (found at 4.096 M atoms): a coordinate in [0, L) can round to fractional 1.0 in fp32.  Such atoms are
+    clamped into the boundary cell; neighbour sets must still be bit-exact on the tiled path."""
+    import oracle
+    import torch
+    from paper_2510_06873_b200.metad import MetaD
+    w = _small("c3")
+    B = w.box.reshape(3, 3)
+    rng = np.random.default_rng(3)
+    pos = w.pos.copy()
+    idx = rng.choice(w.natoms, 60, replace=False)
+    frac = np.linalg.solve(B.T, pos[idx].T).T
+    for k, i in enumerate(idx):
+        frac[k, k % 3] = 1.0 - 1e-10          # wrapped in fp64, == 1.0 (or just above) after fp32 rounding
+    pos[idx] = frac @ B
+    p32 = pos.astype(np.float32)
+    cref, lref, mx = oracle.neighbors(p32.astype(np.float64), w.box, w.rc, w.max_neigh, "brute")
+    assert mx <= w.max_neigh
+    md = MetaD(w, precision=32)
+    dpos = torch.tensor(p32, device="cuda")
+    torch.cuda.synchronize()
+    md.build_neighbors(dpos)
+    cnt, lst = md.neighbors()
+    assert md.status() == 0
+    assert np.array_equal(cnt, cref)
+    assert np.array_equal(sorted_rows_fast(cnt, lst), sorted_rows_fast(cref, lref))
+    md.eval_cv()
+    md.synchronize()
+    q_ref = oracle.q6_atoms(p32.astype(np.float64), w.box, cref, lref)
+    assert np.abs(md.q6() - q_ref).max() <= 5e-6
