@@ -164,6 +164,8 @@ struct metad_ctx {
     // shared-memory tiled fast path (fp32, Q6): tile.cuh / tiled.cu
     int tiled; int tile_T[3]; int tile_cap;
     int timing; int capturing; cudaEvent_t ev[3];
+    float *d_q6;                          // tiled path: per-atom q6 (sorted order)
+    double *d_cvq6;                       // tiled path: [Q6 mean, solid count] finished by k_tile_build
 };
 
 static inline const void *ctx_last_pos(const metad_ctx *c) { return c->d_pos_last; }

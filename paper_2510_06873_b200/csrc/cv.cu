@@ -256,6 +256,7 @@ __device__ __forceinline__ void ldg256(const float *p, float4 &a, float4 &b) {
                  : "l"(p));
 }
 
+template <bool SOLID>
 __global__ void __launch_bounds__(CV_THREADS)
 k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
              const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, const float *__restrict__ rec,
@@ -271,7 +272,7 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         float4 a4, b4, c4, d4;
         ldg256(rec + (size_t)s * METAD_NREC, a4, b4);
         ldg256(rec + (size_t)s * METAD_NREC + 8, c4, d4);
-        const float gk = alpha + beta * d4.y;
+        const float gk = SOLID ? alpha + beta * d4.y : alpha;
         Bk[0] = gk * a4.x; Bk[1] = gk * a4.y; Bk[2] = gk * a4.z; Bk[3] = gk * a4.w;
         Bk[4] = gk * b4.x; Bk[5] = gk * b4.y; Bk[6] = gk * b4.z; Bk[7] = gk * b4.w;
         Bk[8] = gk * c4.x; Bk[9] = gk * c4.y; Bk[10] = gk * c4.z; Bk[11] = gk * c4.w;
@@ -283,10 +284,11 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
     for (int k = 0; k < cnt; ++k) {
         const int e = in[k * 32];
         const int j = e & NLG_IDX_MASK, code = (unsigned)e >> 27;
-        const float4 pj = spos[j];
-        float4 a4, b4, c4, d4;
+        float4 a4, b4, c4, d4, pj;
         ldg256(rec + (size_t)j * METAD_NREC, a4, b4);
         ldg256(rec + (size_t)j * METAD_NREC + 8, c4, d4);
+        if (SOLID) pj = spos[j];
+        else { pj.x = d4.y; pj.y = d4.z; pj.z = d4.w; }     // Q6-mean-only records carry the position
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         if (code != 13) {
             const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
@@ -294,7 +296,7 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
             dy = (float)(((double)pj.y - (double)pi.y) + (wy * bd.by + wz * bd.cy));
             dz = (float)(((double)pj.z - (double)pi.z) + (wz * bd.cz));
         }
-        const float gw = alpha + beta * d4.y;
+        const float gw = SOLID ? alpha + beta * d4.y : alpha;
         float bb[13];
         bb[0] = Bk[0] + gw * a4.x; bb[1] = Bk[1] + gw * a4.y; bb[2] = Bk[2] + gw * a4.z; bb[3] = Bk[3] + gw * a4.w;
         bb[4] = Bk[4] + gw * b4.x; bb[5] = Bk[5] + gw * b4.y; bb[6] = Bk[6] + gw * b4.z; bb[7] = Bk[7] + gw * b4.w;
@@ -318,9 +320,14 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
 int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
     double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
-    k_q6_force_g<<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
-        c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm,
-        ss, c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F);
+    if (c->q6_solid_dim >= 0)
+        k_q6_force_g<true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+            c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm,
+            ss, c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F);
+    else
+        k_q6_force_g<false><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+            c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm,
+            ss, c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -330,6 +337,11 @@ template <typename T>
 __global__ void k_q6_export(int N, const int *__restrict__ perm, const T *__restrict__ rec, T *__restrict__ q6) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s < N) q6[perm[s]] = rec[(size_t)s * METAD_NREC + 14];
+}
+
+__global__ void k_q6_export_arr(int N, const int *__restrict__ perm, const float *__restrict__ q6s, float *__restrict__ q6) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < N) q6[perm[s]] = q6s[s];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -415,6 +427,12 @@ int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F) {
 int q6_export(metad_ctx *c, void *d_q6) {
     if (!c->has_q6) return METAD_ERR_STATE;
     int nb = div_up(c->N, 256);
+    if (c->tiled) {
+        k_q6_export_arr<<<nb, 256, 0, c->stream>>>(c->N, c->d_perm, c->d_q6, (float *)d_q6);
+        c->launches++;
+        CUDA_TRY(cudaGetLastError());
+        return METAD_OK;
+    }
     if (c->prec == 32) k_q6_export<float><<<nb, 256, 0, c->stream>>>(c->N, c->d_perm, (const float *)c->d_rec, (float *)d_q6);
     else k_q6_export<double><<<nb, 256, 0, c->stream>>>(c->N, c->d_perm, (const double *)c->d_rec, (double *)d_q6);
     c->launches++;

@@ -12,7 +12,7 @@
 #include "tile.cuh"
 
 typedef unsigned short nl16_t;   // local halo index (shared-memory candidate list only)
-#define LIST_CAP 40            // per-thread candidate slots in shared memory (maxn <= 32 on this path)
+#define LIST_CAP 64            // per-thread candidate slots in shared memory (maxn <= 32 on this path + one run of slack)
 
 template <bool STAGED>
 __device__ __forceinline__ float4 hpos(const TileTables &t, const float4 *__restrict__ spos, const float4 *pos_s, int li) {
@@ -28,7 +28,8 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
                                            const float4 *pos_s, nl16_t *list_s, const int *__restrict__ scell,
                                            const BoxD &bd, float rc2f, double rc2, int maxn, int *__restrict__ nl_count,
                                            int *__restrict__ nl, unsigned int *__restrict__ sticky, float q_thresh,
-                                           float inv_width, float *__restrict__ rec, double (&v)[2]) {
+                                           float inv_width, float *__restrict__ rec, float *__restrict__ q6_out, bool solid,
+                                           double (&v)[2]) {
     const float rc2_hi = rc2f * (1.f + 1e-5f), rc2_lo = rc2f * (1.f - 1e-5f);
     nl16_t *myl = list_s + threadIdx.x;
     for (int a = threadIdx.x; a < t.nown; a += blockDim.x) {
@@ -38,24 +39,35 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
         const float4 pi = hpos<STAGED>(t, spos, pos_s, li);
         const int ic = scell[s] % g.nc0 - t.x0 + 1;          // halo-cell column of the own atom
         const int r0 = t.own_row[q], rstride = t.Tye + 2;
-        int cnt = 0;
+        // candidate list written through 32-bit shared-memory addresses (generic 64-bit pointer bumps cost 4 extra
+        // instructions per candidate): slot k of this thread lives at w0 + k * STRIDE
+        const unsigned STRIDE = TILE_THREADS * (unsigned)sizeof(nl16_t);
+        const unsigned w0 = (unsigned)__cvta_generic_to_shared(myl);
+        unsigned wp = w0;
+        const unsigned wend = w0 + (LIST_CAP - 1) * STRIDE;
+        bool ovf = false;
 #pragma unroll 1
         for (int dz = -1; dz <= 1; ++dz) {
 #pragma unroll 1
             for (int dy = -1; dy <= 1; ++dy) {
                 const int r = r0 + dz * rstride + dy;
-                const int lo = t.hcell[r][ic - 1], hi = t.hcell[r][ic + 2];
+                const int lo = t.hcell[r][ic - 1];
+                int hi = t.hcell[r][ic + 2];
+                // capacity is checked once per run, so the inner loop is: load, 6 flop, store, compare, bump
+                const int room = (int)((wend - wp) / STRIDE);
+                if (hi - lo > room) { ovf = true; hi = lo + room; }
 #pragma unroll 4
                 for (int lj = lo; lj < hi; ++lj) {
                     const float4 pj = hpos<STAGED>(t, spos, pos_s, lj);
                     const float dx = pj.x - pi.x, dy2 = pj.y - pi.y, dz2 = pj.z - pi.z;
                     const float r2 = dx * dx + dy2 * dy2 + dz2 * dz2;
-                    myl[cnt * TILE_THREADS] = (nl16_t)lj;
-                    cnt = min(cnt + (r2 < rc2_hi ? 1 : 0), LIST_CAP - 1);
+                    asm volatile("st.shared.u16 [%0], %1;" ::"r"(wp), "h"((unsigned short)lj));
+                    wp += (r2 < rc2_hi) ? STRIDE : 0u;
                 }
             }
         }
-        if (cnt >= LIST_CAP - 1) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
+        const int cnt = (int)((wp - w0) / STRIDE);
+        if (ovf) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
         // exact decision on the short list; neighbour-list write; fused q6m accumulation
         int *out = nl + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
         float A[13];
@@ -101,7 +113,13 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
             r4[0] = make_float4(A[0] * norm, A[1] * norm, -A[2] * norm, A[3] * norm);
             r4[1] = make_float4(-A[4] * norm, A[5] * norm, -A[6] * norm, A[7] * norm);
             r4[2] = make_float4(-A[8] * norm, A[9] * norm, -A[10] * norm, A[11] * norm);
-            r4[3] = make_float4(-A[12] * norm, f * (1.f - f) * inv_width, q6, 0.f);
+            if (solid) {
+                r4[3] = make_float4(-A[12] * norm, f * (1.f - f) * inv_width, q6, 0.f);
+            } else {                                          // Q6 mean only: the record carries the atom's own (global,
+                const float4 gp = spos[s];                    // exact fp32) position, so the force pass needs no second gather
+                r4[3] = make_float4(-A[12] * norm, gp.x, gp.y, gp.z);
+            }
+            q6_out[s] = q6;
             v[0] += (double)q6; v[1] += (double)f;
         }
     }
@@ -112,7 +130,9 @@ __global__ void __launch_bounds__(TILE_THREADS, 3)
 k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict__ scell,
              const int *__restrict__ cell_start, BoxD bd, float rc2f, double rc2, int maxn,
              int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
-             float q_thresh, float inv_width, float *__restrict__ rec, double *__restrict__ partials) {
+             float q_thresh, float inv_width, float *__restrict__ rec, float *__restrict__ q6_out, int solid,
+             double *__restrict__ partials, unsigned int *__restrict__ ticket, double scale_mean, double scale_solid,
+             double *__restrict__ cv_q6 /* [2]: Q6 mean, solid count */) {
     extern __shared__ float4 dyn_smem[];
     __shared__ TileTables t;
     __shared__ double red[64];
@@ -126,30 +146,31 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
         if (threadIdx.x == 0) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
     } else if (t.staged) {
         build_body<true, WITH_Q6>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
-                                  inv_width, rec, v);
+                                  inv_width, rec, q6_out, solid != 0, v);
     } else {
         build_body<false, WITH_Q6>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
-                                   inv_width, rec, v);
+                                   inv_width, rec, q6_out, solid != 0, v);
     }
     if (WITH_Q6) {
         block_reduce<2>(v, red);
         if (threadIdx.x == 0) { partials[2 * blockIdx.x] = v[0]; partials[2 * blockIdx.x + 1] = v[1]; }
+        if (last_block_ticket(ticket)) {                      // fixed-order sum of the per-tile partials
+            double u[2] = { 0.0, 0.0 };
+            for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) { u[0] += partials[2 * b]; u[1] += partials[2 * b + 1]; }
+            block_reduce<2>(u, red);
+            if (threadIdx.x == 0) {
+                cv_q6[0] = scale_mean * u[0]; cv_q6[1] = scale_solid * u[1];
+                if (!isfinite(cv_q6[0]) || !isfinite(cv_q6[1])) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
+            }
+        }
     }
 }
 
-// fixed-order sum of the per-tile partials (one block)
-__global__ void __launch_bounds__(256)
-k_q6_finish(int nparts, const double *__restrict__ partials, double scale_mean, double scale_solid, int dim_mean,
-            int dim_solid, double *__restrict__ cv_out, unsigned int *__restrict__ sticky) {
-    __shared__ double red[64];
-    double u[2] = { 0.0, 0.0 };
-    for (int b = threadIdx.x; b < nparts; b += blockDim.x) { u[0] += partials[2 * b]; u[1] += partials[2 * b + 1]; }
-    block_reduce<2>(u, red);
+// a3 on the tiled path: the sums were finished by the last block of k_tile_build; hand them to the caller
+__global__ void k_q6_publish(const double *__restrict__ cv_q6, int dim_mean, int dim_solid, double *__restrict__ cv_out) {
     if (threadIdx.x == 0) {
-        double a = scale_mean * u[0], b = scale_solid * u[1];
-        if (dim_mean >= 0) cv_out[dim_mean] = a;
-        if (dim_solid >= 0) cv_out[dim_solid] = b;
-        if (!isfinite(a) || !isfinite(b)) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
+        if (dim_mean >= 0) cv_out[dim_mean] = cv_q6[0];
+        if (dim_solid >= 0) cv_out[dim_solid] = cv_q6[1];
     }
 }
 
@@ -187,25 +208,22 @@ int tiled_build(metad_ctx *c) {
     if (c->has_q6)
         k_tile_build<true><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
-            c->d_nl_count, c->d_nl, c->d_sticky, (float)qt, (float)(1.0 / qw), (float *)c->d_rec,
-            c->d_partials + c->nblocks_atoms);
+            c->d_nl_count, c->d_nl, c->d_sticky, (float)qt, (float)(1.0 / qw), (float *)c->d_rec, c->d_q6,
+            c->q6_solid_dim >= 0 ? 1 : 0, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
+            c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0, c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0,
+            c->d_cvq6);
     else
         k_tile_build<false><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
-            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr);
+            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, nullptr, nullptr, 0.0, 0.0, nullptr);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
 }
 
-// the q6m accumulation already ran inside k_tile_build: only the fixed-order sum of the partials is left
+// the q6m accumulation and its reduction already ran inside k_tile_build
 int tiled_q6_pass1(metad_ctx *c, double *d_cv) {
-    TileGeom g = tile_geom(c);
-    int nt = g.ntx * g.nty * g.ntz;
-    double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
-    double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
-    k_q6_finish<<<1, 256, 0, c->stream>>>(nt, c->d_partials + c->nblocks_atoms, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
-                                         d_cv, c->d_sticky);
+    k_q6_publish<<<1, 32, 0, c->stream>>>(c->d_cvq6, c->q6_mean_dim, c->q6_solid_dim, d_cv);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
