@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmetad_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-         "-Xcompiler", "-fPIC", "--fmad=true"]
+         "-Xcompiler", "-fPIC", "--fmad=true"] + os.environ.get("METAD_NVCC_FLAGS", "").split()
 
 
 def sources():

@@ -256,8 +256,11 @@ __device__ __forceinline__ void ldg256(const float *p, float4 &a, float4 &b) {
                  : "l"(p));
 }
 
+#ifndef Q6F_MINB
+#define Q6F_MINB 9
+#endif
 template <bool SOLID>
-__global__ void __launch_bounds__(CV_THREADS)
+__global__ void __launch_bounds__(CV_THREADS, Q6F_MINB)
 k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
              const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, const float *__restrict__ rec,
              double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,

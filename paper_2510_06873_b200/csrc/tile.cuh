@@ -33,12 +33,9 @@ struct TileTables {
     int seg_g[TILE_NSEG];        // global (sorted-space) index of the segment's first atom
     int seg_len[TILE_NSEG];
     int seg_off[TILE_NSEG + 1];  // local index of the segment's first atom
-    double seg_k[TILE_NSEG][3];  // lattice shift - origin (fp64), used for periodic images
     unsigned char seg_wrapped[TILE_NSEG];
     unsigned char seg_code[TILE_NSEG];  // lattice-shift code (wx+1) + 3(wy+1) + 9(wz+1); 13 = no shift
-    int hcell[TILE_MAXROWS][TILE_TXMAX + 3];   // local index where halo cell (row, lx) starts; [Txe+2] = row end
-    int hend[TILE_MAXROWS][TILE_TXMAX + 3];    // scratch of the setup: cell_start[cell + 1]
-    short hpiece[TILE_MAXROWS][TILE_TXMAX + 3];
+    unsigned short hcell[TILE_MAXROWS][TILE_TXMAX + 3];   // local index where halo cell (row, lx) starts; [Txe+2] = row end
     int own_g[TILE_MAXOWN];      // global index of the first own atom of own-row q
     int own_l[TILE_MAXOWN];      // local index of the same atom
     int own_off[TILE_MAXOWN + 1];
@@ -54,7 +51,13 @@ __device__ __forceinline__ int tile_row_id(const TileTables &t, int hy, int hz) 
 // Builds the tables (all threads of the block must call it).  cell_start: exclusive scan over cells.
 // Four barrier-separated phases; every global load (two per halo cell) is issued in phase 1 by a
 // different thread, so the block pays the L2 latency once.
-__device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restrict__ cell_start, TileTables &t) {
+// scratch: >= TILE_SCRATCH_BYTES of shared memory that is free during the setup (the position staging area)
+struct TileScratch {
+    int hbeg[TILE_MAXROWS][TILE_TXMAX + 3];    // cell_start[cell]
+    int hend[TILE_MAXROWS][TILE_TXMAX + 3];    // cell_start[cell + 1]
+};
+#define TILE_SCRATCH_BYTES sizeof(TileScratch)
+__device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restrict__ cell_start, TileTables &t, TileScratch &w) {
     const int tid = threadIdx.x;
     int b = blockIdx.x;
     const int tx = b % g.ntx; b /= g.ntx;
@@ -72,8 +75,8 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
         const int jz = lz < 0 ? lz + g.nc2 : (lz >= g.nc2 ? lz - g.nc2 : lz);
         const int jx = lx < 0 ? lx + g.nc0 : (lx >= g.nc0 ? lx - g.nc0 : lx);
         const int id = (jz * g.nc1 + jy) * g.nc0 + jx;
-        t.hcell[r][c] = cell_start[id];
-        t.hend[r][c] = cell_start[id + 1];
+        w.hbeg[r][c] = cell_start[id];
+        w.hend[r][c] = cell_start[id + 1];
     }
     if (tid == 0) {
         t.x0 = x0; t.y0 = y0; t.z0 = z0; t.Txe = Txe; t.Tye = Tye; t.Tze = Tze; t.nrows = nrows;
@@ -105,18 +108,14 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
             const int ls = p == 0 ? xa : (p == 1 ? max(xa, 0) : max(xa, g.nc0));
             const int le = p == 0 ? min(xb, -1) : (p == 1 ? min(xb, g.nc0 - 1) : xb);
             const int wx = p - 1, s = 3 * r + p;
-            if (ls <= le) { segg[p] = t.hcell[r][ls - xa]; t.seg_g[s] = segg[p]; t.seg_len[s] = t.hend[r][le - xa] - segg[p]; }
+            if (ls <= le) { segg[p] = w.hbeg[r][ls - xa]; t.seg_g[s] = segg[p]; t.seg_len[s] = w.hend[r][le - xa] - segg[p]; }
             else { segg[p] = 0; t.seg_g[s] = 0; t.seg_len[s] = 0; }
             t.seg_wrapped[s] = (wx | wy | wz) != 0;
             t.seg_code[s] = (unsigned char)((wx + 1) + 3 * (wy + 1) + 9 * (wz + 1));
-            t.seg_k[s][0] = wx * g.ax + wy * g.bx + wz * g.cx - (double)t.origin[0];
-            t.seg_k[s][1] = wy * g.by + wz * g.cy - (double)t.origin[1];
-            t.seg_k[s][2] = wz * g.cz - (double)t.origin[2];
         }
         for (int c = 0; c < ncol; ++c) {
             const int lx = xa + c, p = lx < 0 ? 0 : (lx >= g.nc0 ? 2 : 1);
-            t.hcell[r][c] -= segg[p];
-            t.hpiece[r][c] = (short)p;
+            w.hbeg[r][c] = (w.hbeg[r][c] - segg[p]) | (p << 28);     // start relative to its segment | piece
         }
     }
     __syncthreads();
@@ -137,8 +136,11 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
     // ---- phase 4: local halo-cell starts; own rows
     if (tid < nrows) {
         const int r = tid;
-        for (int c = 0; c < ncol; ++c) t.hcell[r][c] += t.seg_off[3 * r + t.hpiece[r][c]];
-        t.hcell[r][ncol] = t.seg_off[3 * r + 3];      // end of the row = start of the next row's piece A
+        for (int c = 0; c < ncol; ++c) {
+            const int v = w.hbeg[r][c];
+            t.hcell[r][c] = (unsigned short)((v & 0xfffffff) + t.seg_off[3 * r + (v >> 28)]);
+        }
+        t.hcell[r][ncol] = (unsigned short)t.seg_off[3 * r + 3];      // end of the row = start of the next row's piece A
     }
     __syncthreads();
     if (tid == 0) {
@@ -177,12 +179,14 @@ __device__ __forceinline__ int tile_global_of(const TileTables &t, int li) {
 #define NL_CODE_NONE 13
 
 // tile-local position of a halo atom: (x, y, z, as_float(global sorted index | shift code << 27))
-__device__ __forceinline__ float4 tile_transform(const TileTables &t, int seg, float4 p, int gidx) {
+__device__ __forceinline__ float4 tile_transform(const TileGeom &g, const TileTables &t, int seg, float4 p, int gidx) {
     float4 o;
-    if (t.seg_wrapped[seg]) {
-        o.x = (float)((double)p.x + t.seg_k[seg][0]);
-        o.y = (float)((double)p.y + t.seg_k[seg][1]);
-        o.z = (float)((double)p.z + t.seg_k[seg][2]);
+    if (t.seg_wrapped[seg]) {                  // periodic image: lattice shift - origin added in fp64, rounded once
+        const int code = t.seg_code[seg];
+        const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
+        o.x = (float)((double)p.x + (wx * g.ax + wy * g.bx + wz * g.cx - (double)t.origin[0]));
+        o.y = (float)((double)p.y + (wy * g.by + wz * g.cy - (double)t.origin[1]));
+        o.z = (float)((double)p.z + (wz * g.cz - (double)t.origin[2]));
     } else {
         o.x = p.x - t.origin[0]; o.y = p.y - t.origin[1]; o.z = p.z - t.origin[2];
     }
@@ -191,21 +195,21 @@ __device__ __forceinline__ float4 tile_transform(const TileTables &t, int seg, f
 }
 
 // Stages all halo positions into pos_s (warp per segment, coalesced).  No-op if the halo does not fit.
-__device__ __forceinline__ void tile_stage_pos(const TileTables &t, const float4 *__restrict__ spos, float4 *pos_s) {
+__device__ __forceinline__ void tile_stage_pos(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos, float4 *pos_s) {
     if (!t.staged) return;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     for (int s = wid; s < 3 * t.nrows; s += nw) {
         const int len = t.seg_len[s], g0 = t.seg_g[s], l0 = t.seg_off[s];
-        for (int i = lane; i < len; i += 32) pos_s[l0 + i] = tile_transform(t, s, spos[g0 + i], g0 + i);
+        for (int i = lane; i < len; i += 32) pos_s[l0 + i] = tile_transform(g, t, s, spos[g0 + i], g0 + i);
     }
 }
 
 // position accessor that also works when the tile was not staged (slow path, global memory)
-__device__ __forceinline__ float4 tile_pos(const TileTables &t, const float4 *__restrict__ spos, const float4 *pos_s, int li) {
+__device__ __forceinline__ float4 tile_pos(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos, const float4 *pos_s, int li) {
     if (t.staged) return pos_s[li];
     int s = tile_seg_of(t, li);
     int gi = t.seg_g[s] + (li - t.seg_off[s]);
-    return tile_transform(t, s, spos[gi], gi);
+    return tile_transform(g, t, s, spos[gi], gi);
 }
 
 // own atom number a (0..nown-1) -> own-row q

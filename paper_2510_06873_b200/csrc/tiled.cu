@@ -7,19 +7,20 @@
 //                     the neighbour list and — fused — accumulates the atom's 13 q6m components.
 //   k_q6_finish       fixed-order sum of the per-tile partials -> Q6 / solid-like CVs
 //   k_q6_force_g      gather-form forces: per pair two 256-bit loads of the neighbour's q6 record
+#include <algorithm>
 #include "common.cuh"
 #include "cv_q6.cuh"
 #include "tile.cuh"
 
 typedef unsigned short nl16_t;   // local halo index (shared-memory candidate list only)
-#define LIST_CAP 64            // per-thread candidate slots in shared memory (maxn <= 32 on this path + one run of slack)
+#define LIST_CAP 40            // per-thread candidate slots in shared memory (maxn <= 32 on this path + band + self)
 
 template <bool STAGED>
-__device__ __forceinline__ float4 hpos(const TileTables &t, const float4 *__restrict__ spos, const float4 *pos_s, int li) {
+__device__ __forceinline__ float4 hpos(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos, const float4 *pos_s, int li) {
     if (STAGED) return pos_s[li];
     int s = tile_seg_of(t, li);
     int gi = t.seg_g[s] + (li - t.seg_off[s]);
-    return tile_transform(t, s, spos[gi], gi);
+    return tile_transform(g, t, s, spos[gi], gi);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -36,7 +37,7 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
         const int q = tile_own_row(t, a);
         const int o = a - t.own_off[q];
         const int li = t.own_l[q] + o, s = t.own_g[q] + o;
-        const float4 pi = hpos<STAGED>(t, spos, pos_s, li);
+        const float4 pi = hpos<STAGED>(g, t, spos, pos_s, li);
         const int ic = scell[s] % g.nc0 - t.x0 + 1;          // halo-cell column of the own atom
         const int r0 = t.own_row[q], rstride = t.Tye + 2;
         // candidate list written through 32-bit shared-memory addresses (generic 64-bit pointer bumps cost 4 extra
@@ -51,18 +52,23 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
 #pragma unroll 1
             for (int dy = -1; dy <= 1; ++dy) {
                 const int r = r0 + dz * rstride + dy;
-                const int lo = t.hcell[r][ic - 1];
-                int hi = t.hcell[r][ic + 2];
-                // capacity is checked once per run, so the inner loop is: load, 6 flop, store, compare, bump
-                const int room = (int)((wend - wp) / STRIDE);
-                if (hi - lo > room) { ovf = true; hi = lo + room; }
+                int lo = t.hcell[r][ic - 1];
+                const int hi = t.hcell[r][ic + 2];
+                while (lo < hi) {
+                    // every candidate is stored unconditionally and the slot kept only if it passes (load, 6 flop, store,
+                    // compare, bump): one free slot is needed, capacity is checked once per stretch
+                    const int room = (int)((wend - wp) / STRIDE);
+                    if (room <= 0) { ovf = true; break; }
+                    const int h2 = min(hi, lo + room);
 #pragma unroll 4
-                for (int lj = lo; lj < hi; ++lj) {
-                    const float4 pj = hpos<STAGED>(t, spos, pos_s, lj);
-                    const float dx = pj.x - pi.x, dy2 = pj.y - pi.y, dz2 = pj.z - pi.z;
-                    const float r2 = dx * dx + dy2 * dy2 + dz2 * dz2;
-                    asm volatile("st.shared.u16 [%0], %1;" ::"r"(wp), "h"((unsigned short)lj));
-                    wp += (r2 < rc2_hi) ? STRIDE : 0u;
+                    for (int lj = lo; lj < h2; ++lj) {
+                        const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj);
+                        const float dx = pj.x - pi.x, dy2 = pj.y - pi.y, dz2 = pj.z - pi.z;
+                        const float r2 = dx * dx + dy2 * dy2 + dz2 * dz2;
+                        asm volatile("st.shared.u16 [%0], %1;" ::"r"(wp), "h"((unsigned short)lj));
+                        wp += (r2 < rc2_hi) ? STRIDE : 0u;
+                    }
+                    lo = h2;
                 }
             }
         }
@@ -77,7 +83,7 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
         for (int k = 0; k < cnt; ++k) {
             const int lj = myl[k * TILE_THREADS];
             if (lj == li) continue;
-            const float4 pj = hpos<STAGED>(t, spos, pos_s, lj);
+            const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj);
             const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
             const float r2 = dx * dx + dy * dy + dz * dz;
             bool in = r2 < rc2f;
@@ -126,7 +132,10 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
 }
 
 template <bool WITH_Q6>
-__global__ void __launch_bounds__(TILE_THREADS, 3)
+#ifndef TB_MINB
+#define TB_MINB 5
+#endif
+__global__ void __launch_bounds__(TILE_THREADS, TB_MINB)
 k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict__ scell,
              const int *__restrict__ cell_start, BoxD bd, float rc2f, double rc2, int maxn,
              int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
@@ -138,8 +147,8 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
     __shared__ double red[64];
     float4 *pos_s = dyn_smem;
     nl16_t *list_s = reinterpret_cast<nl16_t *>(dyn_smem + g.cap);
-    tile_setup(g, cell_start, t);
-    tile_stage_pos(t, spos, pos_s);
+    tile_setup(g, cell_start, t, *reinterpret_cast<TileScratch *>(dyn_smem));   // scratch = the (still unused) staging area
+    tile_stage_pos(g, t, spos, pos_s);
     __syncthreads();
     double v[2] = { 0.0, 0.0 };
     if (t.total > 65535) {
@@ -189,7 +198,9 @@ __global__ void k_tile_export(int N, int maxn, const int *__restrict__ perm, con
 // host side
 TileGeom tile_geom(const metad_ctx *c);        // api.cu
 
-static size_t smem_build(const TileGeom &g) { return sizeof(float4) * (size_t)g.cap + sizeof(nl16_t) * LIST_CAP * TILE_THREADS; }
+static size_t smem_build(const TileGeom &g) {
+    return std::max(sizeof(float4) * (size_t)g.cap, (size_t)TILE_SCRATCH_BYTES) + sizeof(nl16_t) * LIST_CAP * TILE_THREADS;
+}
 
 int tiled_init() {
     static bool done = false;
