@@ -49,24 +49,29 @@ __device__ __forceinline__ int tile_row_id(const TileTables &t, int hy, int hz) 
 }
 
 // Builds the tables (all threads of the block must call it).  cell_start: exclusive scan over cells.
-// Four barrier-separated phases; every global load (two per halo cell) is issued in phase 1 by a
-// different thread, so the block pays the L2 latency once.
+// Four barrier-separated phases, none with a serial loop: every global load (two per halo cell) is issued in phase 1
+// by a different thread, so the block pays the L2 latency once; the tile origin is worked out by 8 lanes in parallel.
+// Tiles partition each direction evenly (tile k covers cells [k nc / nt, (k+1) nc / nt)), so no sliver tiles.
 // scratch: >= TILE_SCRATCH_BYTES of shared memory that is free during the setup (the position staging area)
 struct TileScratch {
     int hbeg[TILE_MAXROWS][TILE_TXMAX + 3];    // cell_start[cell]
     int hend[TILE_MAXROWS][TILE_TXMAX + 3];    // cell_start[cell + 1]
+    int hrel[TILE_MAXROWS][TILE_TXMAX + 3];    // start of the halo cell relative to its segment | piece << 28
 };
 #define TILE_SCRATCH_BYTES sizeof(TileScratch)
+__device__ __forceinline__ int tile_cut(int k, int nc, int nt) { return (int)(((long long)k * nc) / nt); }
+
 __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restrict__ cell_start, TileTables &t, TileScratch &w) {
     const int tid = threadIdx.x;
     int b = blockIdx.x;
     const int tx = b % g.ntx; b /= g.ntx;
     const int ty = b % g.nty, tz = b / g.nty;
-    const int x0 = tx * g.Tx, y0 = ty * g.Ty, z0 = tz * g.Tz;
-    const int Txe = min(g.Tx, g.nc0 - x0), Tye = min(g.Ty, g.nc1 - y0), Tze = min(g.Tz, g.nc2 - z0);
+    const int x0 = tile_cut(tx, g.nc0, g.ntx), y0 = tile_cut(ty, g.nc1, g.nty), z0 = tile_cut(tz, g.nc2, g.ntz);
+    const int Txe = tile_cut(tx + 1, g.nc0, g.ntx) - x0, Tye = tile_cut(ty + 1, g.nc1, g.nty) - y0,
+              Tze = tile_cut(tz + 1, g.nc2, g.ntz) - z0;
     const int nrows = (Tye + 2) * (Tze + 2), ncol = Txe + 2;
-    const int xa = x0 - 1;
-    // ---- phase 1: cell_start of every halo cell (both ends); thread 0 also fixes the tile origin
+    const int xa = x0 - 1, xb = x0 + Txe;
+    // ---- phase 1: cell_start of every halo cell (both ends); warp 7 fixes the tile origin
     for (int i = tid; i < nrows * ncol; i += blockDim.x) {
         const int r = i / ncol, c = i - r * ncol;
         const int hy = r % (Tye + 2) - 1, hz = r / (Tye + 2) - 1;
@@ -78,45 +83,48 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
         w.hbeg[r][c] = cell_start[id];
         w.hend[r][c] = cell_start[id + 1];
     }
-    if (tid == 0) {
-        t.x0 = x0; t.y0 = y0; t.z0 = z0; t.Txe = Txe; t.Tye = Tye; t.Tze = Tze; t.nrows = nrows;
-        // coordinate range of the halo'd tile (8 corners of the parallelepiped), origin = point nearest to 0
-        double lo[3] = { 1e300, 1e300, 1e300 }, hi[3] = { -1e300, -1e300, -1e300 };
-        for (int c = 0; c < 8; ++c) {
-            double fa = (double)(x0 - 1 + ((c & 1) ? Txe + 2 : 0)) / g.nc0;
-            double fb = (double)(y0 - 1 + ((c & 2) ? Tye + 2 : 0)) / g.nc1;
-            double fc = (double)(z0 - 1 + ((c & 4) ? Tze + 2 : 0)) / g.nc2;
-            double p[3] = { fa * g.ax + fb * g.bx + fc * g.cx, fb * g.by + fc * g.cy, fc * g.cz };
-            for (int a = 0; a < 3; ++a) { lo[a] = fmin(lo[a], p[a]); hi[a] = fmax(hi[a], p[a]); }
-        }
+    if (tid == 0) { t.x0 = x0; t.y0 = y0; t.z0 = z0; t.Txe = Txe; t.Tye = Tye; t.Tze = Tze; t.nrows = nrows; }
+    if (tid >= blockDim.x - 32) {
+        // coordinate range of the halo'd tile (8 corners of the parallelepiped, one per lane), origin = point nearest to 0
+        const int c = tid & 7;
+        const double fa = (double)(x0 - 1 + ((c & 1) ? Txe + 2 : 0)) / g.nc0;
+        const double fb = (double)(y0 - 1 + ((c & 2) ? Tye + 2 : 0)) / g.nc1;
+        const double fc = (double)(z0 - 1 + ((c & 4) ? Tze + 2 : 0)) / g.nc2;
+        double lo[3] = { fa * g.ax + fb * g.bx + fc * g.cx, fb * g.by + fc * g.cy, fc * g.cz }, hi[3];
+#pragma unroll
         for (int a = 0; a < 3; ++a) {
-            double o = lo[a] > 0.0 ? lo[a] : (hi[a] < 0.0 ? hi[a] : 0.0);
-            t.origin[a] = (float)(trunc(o * 64.0) * (1.0 / 64.0));   // toward zero, on a 2^-6 grid
+            hi[a] = lo[a];
+#pragma unroll
+            for (int o = 1; o < 8; o <<= 1) {
+                lo[a] = fmin(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+                hi[a] = fmax(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+            }
+            const double o = lo[a] > 0.0 ? lo[a] : (hi[a] < 0.0 ? hi[a] : 0.0);
+            if ((tid & 31) == 0) t.origin[a] = (float)(trunc(o * 64.0) * (1.0 / 64.0));   // toward zero, on a 2^-6 grid
         }
     }
     for (int s = 3 * nrows + tid; s < TILE_NSEG; s += blockDim.x) t.seg_len[s] = 0;
     __syncthreads();
-    // ---- phase 2: the <= 3 segments of every row, halo-cell starts relative to their segment
-    if (tid < nrows) {
-        const int r = tid;
+    // ---- phase 2: the <= 3 segments of every row (thread per segment); halo-cell starts relative to their segment
+    //      (thread per halo cell).  Piece p of a row covers halo columns [ls, le]: p = 0 left of x = 0 (shift -a),
+    //      p = 1 inside the box, p = 2 right of x = nc0 - 1 (shift +a).
+    if (tid < 3 * nrows) {
+        const int r = tid / 3, p = tid - 3 * r;
         const int hy = r % (Tye + 2) - 1, hz = r / (Tye + 2) - 1;
         const int ly = y0 + hy, lz = z0 + hz;
-        const int wy = ly < 0 ? -1 : (ly >= g.nc1 ? 1 : 0), wz = lz < 0 ? -1 : (lz >= g.nc2 ? 1 : 0);
-        const int xb = x0 + Txe;
-        int segg[3];
-        for (int p = 0; p < 3; ++p) {
-            const int ls = p == 0 ? xa : (p == 1 ? max(xa, 0) : max(xa, g.nc0));
-            const int le = p == 0 ? min(xb, -1) : (p == 1 ? min(xb, g.nc0 - 1) : xb);
-            const int wx = p - 1, s = 3 * r + p;
-            if (ls <= le) { segg[p] = w.hbeg[r][ls - xa]; t.seg_g[s] = segg[p]; t.seg_len[s] = w.hend[r][le - xa] - segg[p]; }
-            else { segg[p] = 0; t.seg_g[s] = 0; t.seg_len[s] = 0; }
-            t.seg_wrapped[s] = (wx | wy | wz) != 0;
-            t.seg_code[s] = (unsigned char)((wx + 1) + 3 * (wy + 1) + 9 * (wz + 1));
-        }
-        for (int c = 0; c < ncol; ++c) {
-            const int lx = xa + c, p = lx < 0 ? 0 : (lx >= g.nc0 ? 2 : 1);
-            w.hbeg[r][c] = (w.hbeg[r][c] - segg[p]) | (p << 28);     // start relative to its segment | piece
-        }
+        const int wy = ly < 0 ? -1 : (ly >= g.nc1 ? 1 : 0), wz = lz < 0 ? -1 : (lz >= g.nc2 ? 1 : 0), wx = p - 1;
+        const int ls = p == 0 ? xa : (p == 1 ? max(xa, 0) : max(xa, g.nc0));
+        const int le = p == 0 ? min(xb, -1) : (p == 1 ? min(xb, g.nc0 - 1) : xb);
+        if (ls <= le) { const int sg = w.hbeg[r][ls - xa]; t.seg_g[tid] = sg; t.seg_len[tid] = w.hend[r][le - xa] - sg; }
+        else { t.seg_g[tid] = 0; t.seg_len[tid] = 0; }
+        t.seg_wrapped[tid] = (wx | wy | wz) != 0;
+        t.seg_code[tid] = (unsigned char)((wx + 1) + 3 * (wy + 1) + 9 * (wz + 1));
+    }
+    for (int i = tid; i < nrows * ncol; i += blockDim.x) {
+        const int r = i / ncol, c = i - r * ncol;
+        const int lx = xa + c, p = lx < 0 ? 0 : (lx >= g.nc0 ? 2 : 1);
+        const int ls = p == 0 ? xa : (p == 1 ? max(xa, 0) : max(xa, g.nc0));
+        w.hrel[r][c] = (w.hbeg[r][c] - w.hbeg[r][ls - xa]) | (p << 28);
     }
     __syncthreads();
     // ---- phase 3: exclusive scan of seg_len (<= 108 entries) by warp 0
@@ -133,28 +141,38 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
         if (tid == 31) { t.seg_off[TILE_NSEG] = inc; t.total = inc; t.staged = inc <= g.cap; }
     }
     __syncthreads();
-    // ---- phase 4: local halo-cell starts; own rows
-    if (tid < nrows) {
-        const int r = tid;
-        for (int c = 0; c < ncol; ++c) {
-            const int v = w.hbeg[r][c];
+    // ---- phase 4: local halo-cell starts (thread per halo cell); own rows (last warp, lane per own row)
+    for (int i = tid; i < nrows * (ncol + 1); i += blockDim.x) {
+        const int r = i / (ncol + 1), c = i - r * (ncol + 1);
+        if (c < ncol) {
+            const int v = w.hrel[r][c];
             t.hcell[r][c] = (unsigned short)((v & 0xfffffff) + t.seg_off[3 * r + (v >> 28)]);
+        } else {
+            t.hcell[r][ncol] = (unsigned short)t.seg_off[3 * r + 3];      // end of the row = start of the next row's piece A
         }
-        t.hcell[r][ncol] = (unsigned short)t.seg_off[3 * r + 3];      // end of the row = start of the next row's piece A
     }
-    __syncthreads();
-    if (tid == 0) {
-        int n = 0, q = 0;
-        for (int oz = 0; oz < Tze; ++oz)
-            for (int oy = 0; oy < Tye; ++oy, ++q) {
-                int r = (oz + 1) * (Tye + 2) + (oy + 1);
-                int l0 = t.hcell[r][1], l1 = t.hcell[r][Txe + 1];
-                t.own_row[q] = r; t.own_l[q] = l0;
-                t.own_g[q] = t.seg_g[3 * r + 1] + (l0 - t.seg_off[3 * r + 1]);
-                t.own_off[q] = n; n += l1 - l0;
-            }
-        t.own_off[q] = n; t.nown = n;
-        for (int qq = q + 1; qq <= TILE_MAXOWN; ++qq) t.own_off[qq] = n;
+    if (tid >= blockDim.x - 32) {
+        const int q = tid & 31, nq = Tye * Tze;
+        int len = 0, l0 = 0, r = 0;
+        if (q < nq) {
+            const int oz = q / Tye, oy = q - oz * Tye;
+            r = (oz + 1) * (Tye + 2) + (oy + 1);
+            // column 1 (cell x0) always lies in piece 1; column Txe + 1 (cell x0 + Txe) in piece 1 or, at the box end, 2
+            const int v1 = w.hrel[r][Txe + 1];
+            l0 = (w.hrel[r][1] & 0xfffffff) + t.seg_off[3 * r + 1];
+            len = (v1 & 0xfffffff) + t.seg_off[3 * r + (v1 >> 28)] - l0;
+        }
+        int inc = len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int u = __shfl_up_sync(0xffffffffu, inc, o); if (q >= o) inc += u; }
+        if (q < nq) {
+            t.own_row[q] = r; t.own_l[q] = l0;
+            t.own_g[q] = t.seg_g[3 * r + 1] + (l0 - t.seg_off[3 * r + 1]);
+            t.own_off[q] = inc - len;
+        }
+        const int n = __shfl_sync(0xffffffffu, inc, 31);
+        if (q >= nq && q <= TILE_MAXOWN) t.own_off[q] = n;
+        if (q == 0) t.nown = n;
     }
     __syncthreads();
 }
