@@ -131,7 +131,7 @@ struct metad_ctx {
     bool have_neighbors;
     int cell_cap;
     int *d_cell_count, *d_cell_start, *d_block_sums;
-    int *d_cell_of, *d_slot, *d_perm, *d_scell;
+    int *d_cell_of, *d_slot, *d_perm, *d_perm_raw, *d_scell;   // perm_raw: counting-sort output before the in-cell ordering
     unsigned char *d_flags;               // per original atom: bit0 in A, bit1 in B (COORD)
     void *d_spos;                         // Vec4<T>[N], cell-sorted
     int *d_nl_count, *d_nl;               // sorted space; nl[k*N + s]

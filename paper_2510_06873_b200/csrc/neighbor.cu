@@ -2,8 +2,8 @@
 //   k_bin            cell index per atom + histogram (int atomics give the in-cell slot)
 //   k_scan_sums/k_scan_apply   exclusive scan of the histogram over cells (two launches)
 //   k_scatter        counting-sort scatter of atom indices
-//   k_cell_sort_gather  orders each cell by original index (run-to-run determinism, reading P) and
-//                    gathers positions into the cell-sorted Vec4 array (x, y, z, group flags)
+//   k_cell_sort_gather  thread per atom: rank by original index inside the cell (run-to-run determinism,
+//                    reading P), gathers positions into the cell-sorted Vec4 array (x, y, z, group flags)
 //   k_build_list     per-atom candidate scan of the 27 neighbouring cells; canonical predicate
 // Everything downstream works in "sorted space" (indices into the cell-sorted arrays), so that the
 // gathers of the CV and force passes touch neighbouring memory.
@@ -120,27 +120,27 @@ __global__ void k_scatter(int N, const int *__restrict__ cell_of, const int *__r
     perm[cell_start[cell_of[i]] + slot[i]] = i;
 }
 
+// Thread per sorted slot: the atom in slot a finds its rank by original index among the atoms of its cell (a handful,
+// read from the unsorted permutation through L1) and moves itself to that place: in-cell order = original index, so the
+// float summation order downstream is run-to-run deterministic (reading P) no matter how the atomics of k_bin fell.
 template <typename T>
-__global__ void k_cell_sort_gather(int ncell, const int *__restrict__ cell_start, int *__restrict__ perm,
+__global__ void k_cell_sort_gather(int N, const int *__restrict__ cell_start, const int *__restrict__ cell_of,
+                                   const int *__restrict__ perm_in, int *__restrict__ perm,
                                    const T *__restrict__ pos, const unsigned char *__restrict__ flags,
                                    typename Vec4<T>::type *__restrict__ spos, int *__restrict__ scell) {
-    int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= ncell) return;
-    int b = cell_start[c], e = cell_start[c + 1];
-    for (int a = b + 1; a < e; ++a) {  // insertion sort by original index
-        int key = perm[a], q = a - 1;
-        while (q >= b && perm[q] > key) { perm[q + 1] = perm[q]; --q; }
-        perm[q + 1] = key;
-    }
-    for (int a = b; a < e; ++a) {
-        int i = perm[a];
-        typename Vec4<T>::type v;
-        v.x = pos[3 * i]; v.y = pos[3 * i + 1]; v.z = pos[3 * i + 2];
-        int fl = flags ? (int)flags[i] : 3;
-        v.w = (T)fl;
-        spos[a] = v;
-        scell[a] = c;
-    }
+    int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= N) return;
+    const int i = perm_in[a], c = cell_of[i];
+    const int b = cell_start[c], e = cell_start[c + 1];
+    int rank = 0;
+    for (int q = b; q < e; ++q) rank += perm_in[q] < i;
+    typename Vec4<T>::type v;
+    v.x = pos[3 * i]; v.y = pos[3 * i + 1]; v.z = pos[3 * i + 2];
+    v.w = (T)(flags ? (int)flags[i] : 3);
+    const int d = b + rank;
+    perm[d] = i;
+    spos[d] = v;
+    scell[d] = c;
 }
 
 template <typename T>
@@ -251,8 +251,8 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
                                              c->d_sticky);
     k_scan_sums<<<nsb, SCAN_THREADS, 0, st>>>(ncell, c->d_cell_count, c->d_block_sums);
     k_scan_apply<<<nsb, SCAN_THREADS, 0, st>>>(ncell, N, c->d_cell_count, c->d_block_sums, c->d_cell_start);
-    k_scatter<<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_of, c->d_slot, c->d_cell_start, c->d_perm);
-    k_cell_sort_gather<T><<<div_up(ncell, 128), 128, 0, st>>>(ncell, c->d_cell_start, c->d_perm, (const T *)d_pos,
+    k_scatter<<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_of, c->d_slot, c->d_cell_start, c->d_perm_raw);
+    k_cell_sort_gather<T><<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_start, c->d_cell_of, c->d_perm_raw, c->d_perm, (const T *)d_pos,
                                                              c->has_coord && c->cv[c->coord_dim].use_groups ? c->d_flags : nullptr,
                                                              (V4 *)c->d_spos, c->d_scell);
     if (tm) cudaEventRecord(c->ev[1], st);
