@@ -61,6 +61,16 @@ def lib():
         L.orc_grid_eval.restype = _I
         L.orc_grid_eval.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P]
         L.orc_apply_forces.argtypes = [_I, _I, _P, _P, _D, _P]
+        L.orc_cv_torsion.restype = _D
+        L.orc_cv_torsion.argtypes = [_P, _P, _P, _P]
+        L.orc_pdiff.restype = _D
+        L.orc_pdiff.argtypes = [_D, _D, _D]
+        L.orc_wrap.restype = _D
+        L.orc_wrap.argtypes = [_D, _D, _D]
+        L.orc_bias_periodic.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P, _P]
+        L.orc_grid_add_p.argtypes = [_I, _I, _P, _P, _P, _I, _I, _P, _P, _P, _P]
+        L.orc_grid_eval_p.restype = _I
+        L.orc_grid_eval_p.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P, _P]
         _lib = L
     return _lib
 
@@ -229,3 +239,49 @@ def apply_forces(F, dVds, grads, force_scale=1.0):
     assert F.dtype == np.float64 and F.flags.c_contiguous
     lib().orc_apply_forces(len(F), len(dVds), _p(dVds), _p(grads), float(force_scale), _p(F))
     return F
+
+
+# ---- NEXT-1: torsion CV, periodic bias (readings V, W, X)
+def cv_torsion(pos, box, idx, want_grad=True):
+    """phi in (-pi, pi] of atoms idx[0..3]; grad (4,3) = d phi / d r of those four atoms."""
+    pos, box, idx = _f(pos), _f(box), _i(idx)
+    g = np.zeros((4, 3)) if want_grad else None
+    phi = lib().orc_cv_torsion(_p(idx), _p(pos), _p(box), _p(g))
+    return phi, g
+
+
+def pdiff(x, c, period):
+    return lib().orc_pdiff(float(x), float(c), float(period))
+
+
+def wrap(x, lo, period):
+    return lib().orc_wrap(float(x), float(lo), float(period))
+
+
+def bias_periodic(centers, heights, sigma, period, s):
+    centers, heights, sigma, period, s = _f(centers), _f(heights), _f(sigma), _f(period), _f(np.atleast_1d(s))
+    D, H = len(sigma), len(heights)
+    centers = centers.reshape(H, D)
+    V = ctypes.c_double(0.0)
+    dV = np.zeros(D)
+    lib().orc_bias_periodic(D, H, _p(centers), _p(heights), _p(sigma), _p(period), _p(s), ctypes.addressof(V), _p(dV))
+    return V.value, dV
+
+
+def grid_add_p(table, lo, hi, periodic, centers, heights, sigma, k0=0, k1=None):
+    lo, hi, centers, heights, sigma, periodic = _f(lo), _f(hi), _f(centers), _f(heights), _f(sigma), _i(periodic)
+    if k1 is None:
+        k1 = len(heights)
+    assert table.dtype == np.float64 and table.flags.c_contiguous and table.shape[0] == 4
+    lib().orc_grid_add_p(table.shape[1], table.shape[2], _p(lo), _p(hi), _p(periodic), int(k0), int(k1), _p(centers),
+                         _p(heights), _p(sigma), _p(table))
+    return table
+
+
+def grid_eval_p(table, lo, hi, periodic, s):
+    lo, hi, s, periodic = _f(lo), _f(hi), _f(s), _i(periodic)
+    V = ctypes.c_double(0.0)
+    dV = np.zeros(2)
+    out = lib().orc_grid_eval_p(table.shape[1], table.shape[2], _p(lo), _p(hi), _p(periodic), _p(table), _p(s),
+                                ctypes.addressof(V), _p(dV))
+    return out, V.value, dV

@@ -572,3 +572,157 @@ void orc_apply_forces(int N, int D, const double *dVds, const double *grads, dou
         F[t] += -force_scale * acc;
     }
 }
+
+/* =============================================================================================
+ * NEXT-1: the paper's first workload — backbone torsions Phi, Psi of alanine
+ * dipeptide as CVs, sigma = 0.35 rad, W = 1.2 kJ/mol — needs a torsion CV and a
+ * bias that is periodic in the CV.  The paper gives neither formula; readings V, W, X of DESIGN.md.
+ * ============================================================================================= */
+
+/* Torsion (dihedral) angle of atoms i-j-k-l ("Phi(C-N-Ca-C) and Psi(N-Ca-C-N)";
+ * reading V): IUPAC convention, bond vectors by minimum image,
+ *     b1 = r_j - r_i, b2 = r_k - r_j, b3 = r_l - r_k,  n1 = b1 x b2,  n2 = b2 x b3,
+ *     phi = atan2( |b2| b1.n2 , n1.n2 )  in (-pi, pi];   cis = 0, trans = pi.
+ * Gradient (grad[4][3], may be NULL), written with F = -b1, G = -b2, H = b3, A = F x G = n1,
+ * B = H x G = -n2 (the textbook form of Blondel & Karplus):
+ *     dphi/dr_i = -|G|/A^2 A,   dphi/dr_l = +|G|/B^2 B,
+ *     dphi/dr_j = +|G|/A^2 A + (F.G)/(A^2 |G|) A - (H.G)/(B^2 |G|) B,
+ *     dphi/dr_k = -|G|/B^2 B - (F.G)/(A^2 |G|) A + (H.G)/(B^2 |G|) B.                            */
+static void cross3(const double *a, const double *b, double *c) {
+    c[0] = a[1] * b[2] - a[2] * b[1]; c[1] = a[2] * b[0] - a[0] * b[2]; c[2] = a[0] * b[1] - a[1] * b[0];
+}
+static double dot3(const double *a, const double *b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+
+double orc_cv_torsion(const int *idx, const double *pos, const double *box, double *grad) {
+    double b1[3], b2[3], b3[3], n1[3], n2[3];
+    orc_delta(box, pos + 3 * idx[0], pos + 3 * idx[1], b1);
+    orc_delta(box, pos + 3 * idx[1], pos + 3 * idx[2], b2);
+    orc_delta(box, pos + 3 * idx[2], pos + 3 * idx[3], b3);
+    cross3(b1, b2, n1);
+    cross3(b2, b3, n2);
+    double lb2 = sqrt(dot3(b2, b2));
+    double phi = atan2(lb2 * dot3(b1, n2), dot3(n1, n2));
+    if (grad) {
+        double F[3], G[3], H[3], A[3], B[3];
+        for (int a = 0; a < 3; ++a) { F[a] = -b1[a]; G[a] = -b2[a]; H[a] = b3[a]; }
+        cross3(F, G, A);
+        cross3(H, G, B);
+        double A2 = dot3(A, A), B2 = dot3(B, B), lG = sqrt(dot3(G, G));
+        double FG = dot3(F, G), HG = dot3(H, G);
+        for (int a = 0; a < 3; ++a) {
+            double gi = -lG / A2 * A[a];
+            double gl = lG / B2 * B[a];
+            double gj = lG / A2 * A[a] + FG / (A2 * lG) * A[a] - HG / (B2 * lG) * B[a];
+            double gk = -lG / B2 * B[a] - FG / (A2 * lG) * A[a] + HG / (B2 * lG) * B[a];
+            grad[a] = gi; grad[3 + a] = gj; grad[6 + a] = gk; grad[9 + a] = gl;
+        }
+    }
+    return phi;
+}
+
+/* Periodic difference (reading W): x - c brought to the nearest periodic image, in [-P/2, P/2];
+ * P <= 0 means the dimension is not periodic. */
+double orc_pdiff(double x, double c, double P) {
+    double d = x - c;
+    if (P > 0.0) d -= P * rint(d / P);
+    return d;
+}
+
+/* Wraps x into [lo, lo + P). */
+double orc_wrap(double x, double lo, double P) {
+    double y = x - P * floor((x - lo) / P);
+    if (y >= lo + P) y -= P;
+    if (y < lo) y += P;
+    return y;
+}
+
+/* Hill sum with periodic CV dimensions (PAPER.md:81 with (s - s_tau) read as the nearest-image
+ * difference, reading W): one image per hill, no sum over images (the next image of a
+ * sigma = 0.35 rad hill is below e^-40 at the discontinuity).  period[d] <= 0: not periodic.     */
+void orc_bias_periodic(int D, int H, const double *centers, const double *heights, const double *sigma,
+                       const double *period, const double *s, double *V, double *dVds) {
+    double v = 0.0, dv[8];
+    for (int d = 0; d < D; ++d) dv[d] = 0.0;
+    for (int k = 0; k < H; ++k) {
+        double e = 0.0, t[8];
+        for (int d = 0; d < D; ++d) {
+            t[d] = orc_pdiff(s[d], centers[(size_t)k * D + d], period[d]) / sigma[d];
+            e += t[d] * t[d];
+        }
+        double g = heights[k] * exp(-0.5 * e);
+        v += g;
+        for (int d = 0; d < D; ++d) dv[d] += -g * t[d] / sigma[d];
+    }
+    *V = v;
+    for (int d = 0; d < D; ++d) dVds[d] = dv[d];
+}
+
+/* Grid-tabulated 2-D bias with periodic dimensions (reading X): a periodic dimension d has n_d
+ * nodes at lo_d + i * P_d / n_d (P_d = hi_d - lo_d; node n_d coincides with node 0), a
+ * non-periodic one n_d nodes at lo_d + i (hi_d - lo_d)/(n_d - 1) as in orc_grid_add.  Node data
+ * and interpolant as in reading M; a periodic dimension has no "outside".                        */
+static double grid_h(int n, double lo, double hi, int periodic) { return periodic ? (hi - lo) / n : (hi - lo) / (n - 1); }
+
+void orc_grid_add_p(int n0, int n1, const double *lo, const double *hi, const int *periodic, int k0, int k1,
+                    const double *centers /*[H][2]*/, const double *heights, const double *sigma,
+                    double *table) {
+    double h0 = grid_h(n0, lo[0], hi[0], periodic[0]), h1 = grid_h(n1, lo[1], hi[1], periodic[1]);
+    double P0 = periodic[0] ? hi[0] - lo[0] : 0.0, P1 = periodic[1] ? hi[1] - lo[1] : 0.0;
+    size_t plane = (size_t)n0 * n1;
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < n0; ++i) {
+        double x = lo[0] + i * h0;
+        for (int j = 0; j < n1; ++j) {
+            double y = lo[1] + j * h1;
+            double v = 0.0, v0 = 0.0, v1 = 0.0, v01 = 0.0;
+            for (int k = k0; k < k1; ++k) {
+                double a = orc_pdiff(x, centers[2 * k], P0) / sigma[0], b = orc_pdiff(y, centers[2 * k + 1], P1) / sigma[1];
+                double g = heights[k] * exp(-0.5 * (a * a + b * b));
+                double ga = -a / sigma[0], gb = -b / sigma[1];
+                v += g; v0 += g * ga; v1 += g * gb; v01 += g * ga * gb;
+            }
+            size_t o = (size_t)i * n1 + j;
+            table[o] += v; table[plane + o] += v0; table[2 * plane + o] += v1; table[3 * plane + o] += v01;
+        }
+    }
+}
+
+int orc_grid_eval_p(int n0, int n1, const double *lo, const double *hi, const int *periodic, const double *table,
+                    const double *s, double *V, double *dVds) {
+    int n[2] = { n0, n1 }, i0[2], i1[2];
+    double h[2], t[2];
+    for (int d = 0; d < 2; ++d) {
+        h[d] = grid_h(n[d], lo[d], hi[d], periodic[d]);
+        if (periodic[d]) {
+            double x = orc_wrap(s[d], lo[d], hi[d] - lo[d]);
+            double f = (x - lo[d]) / h[d];
+            int i = (int)floor(f);
+            if (i > n[d] - 1) i = n[d] - 1;
+            if (i < 0) i = 0;
+            t[d] = f - i; i0[d] = i; i1[d] = (i + 1) % n[d];
+        } else {
+            if (!(s[d] >= lo[d]) || !(s[d] <= hi[d])) return 1;
+            double f = (s[d] - lo[d]) / h[d];
+            int i = (int)floor(f);
+            if (i > n[d] - 2) i = n[d] - 2;
+            t[d] = f - i; i0[d] = i; i1[d] = i + 1;
+        }
+    }
+    double hx[4], dhx[4], hy[4], dhy[4];
+    hermite(t[0], hx, dhx); hermite(t[1], hy, dhy);
+    size_t plane = (size_t)n0 * n1;
+    double v = 0.0, vx = 0.0, vy = 0.0;
+    for (int a = 0; a < 2; ++a)
+    for (int b = 0; b < 2; ++b) {
+        size_t o = (size_t)(a ? i1[0] : i0[0]) * n1 + (b ? i1[1] : i0[1]);
+        double f = table[o], f0 = table[plane + o] * h[0], f1 = table[2 * plane + o] * h[1],
+               f01 = table[3 * plane + o] * h[0] * h[1];
+        double wx = hx[a], wxs = hx[2 + a], wy = hy[b], wys = hy[2 + b];
+        double dwx = dhx[a], dwxs = dhx[2 + a], dwy = dhy[b], dwys = dhy[2 + b];
+        v  += f * wx * wy + f0 * wxs * wy + f1 * wx * wys + f01 * wxs * wys;
+        vx += f * dwx * wy + f0 * dwxs * wy + f1 * dwx * wys + f01 * dwxs * wys;
+        vy += f * wx * dwy + f0 * wxs * dwy + f1 * wx * dwys + f01 * wxs * dwys;
+    }
+    *V = v; dVds[0] = vx / h[0]; dVds[1] = vy / h[1];
+    return 0;
+}

@@ -7,11 +7,11 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import (apply_forces, bias, cv_contacts, cv_coord, cv_rgyr, grid_add, grid_eval, make_flags,
-               neighbors, q6_atoms, q6_grad, wt_height)
+from . import (apply_forces, bias, bias_periodic, cv_contacts, cv_coord, cv_rgyr, cv_torsion, grid_add, grid_add_p,
+               grid_eval, grid_eval_p, make_flags, neighbors, q6_atoms, q6_grad, wt_height)
 
 # CV kinds — restated (not imported) so the oracle depends on nothing of the product.
-COORD, Q6_MEAN, Q6_SOLID, RGYR, CONTACTS = 0, 1, 2, 3, 4
+COORD, Q6_MEAN, Q6_SOLID, RGYR, CONTACTS, TORSION = 0, 1, 2, 3, 4, 5
 
 
 def logistic(q, q0, width):
@@ -32,6 +32,9 @@ class OracleMetaD:
         self.step = 0
         self.method = neighbor_method
         self.grid = None
+        per = getattr(w, "period", None)
+        self.period = np.zeros(self.D) if per is None else np.asarray(per, dtype=np.float64)   # reading W
+        self.periodic = bool(np.any(self.period > 0))
 
     # -- a1
     def build_neighbors(self, pos):
@@ -70,6 +73,12 @@ class OracleMetaD:
                     np.add.at(g, np.asarray(cv.chain), gc)
             elif cv.kind == CONTACTS:
                 s[d], g = cv_contacts(pos, box, cv.pairs, cv.pair_r0, cv.n, cv.m, cv.scale, want_grad)
+            elif cv.kind == TORSION:
+                s[d], g4 = cv_torsion(pos, box, cv.atoms, want_grad)
+                g = None
+                if want_grad:
+                    g = np.zeros((self.N, 3))
+                    np.add.at(g, np.asarray(cv.atoms), g4)
             else:
                 raise ValueError(cv.kind)
             if want_grad:
@@ -83,22 +92,36 @@ class OracleMetaD:
         self.heights = np.array(heights, dtype=np.float64)
         if self.grid is not None:
             self.grid["table"][:] = 0.0
-            grid_add(self.grid["table"], self.grid["lo"], self.grid["hi"], self.centers, self.heights, self.sigma)
+            self._grid_add(0, len(self.heights))
 
     def enable_grid(self, n, lo, hi):
         self.grid = {"lo": np.asarray(lo, float), "hi": np.asarray(hi, float),
                      "table": np.zeros((4, n[0], n[1]))}
         if len(self.heights):
-            grid_add(self.grid["table"], lo, hi, self.centers, self.heights, self.sigma)
+            self._grid_add(0, len(self.heights))
+
+    def _grid_add(self, k0, k1):
+        g = self.grid
+        if self.periodic:
+            grid_add_p(g["table"], g["lo"], g["hi"], (self.period > 0).astype(np.int32), self.centers, self.heights,
+                       self.sigma, k0, k1)
+        else:
+            grid_add(g["table"], g["lo"], g["hi"], self.centers, self.heights, self.sigma, k0, k1)
 
     def bias(self, s, use_grid=None):
         use_grid = (self.grid is not None) if use_grid is None else use_grid
         if use_grid:
-            out, V, dV = grid_eval(self.grid["table"], self.grid["lo"], self.grid["hi"], s)
+            if self.periodic:
+                out, V, dV = grid_eval_p(self.grid["table"], self.grid["lo"], self.grid["hi"],
+                                         (self.period > 0).astype(np.int32), s)
+            else:
+                out, V, dV = grid_eval(self.grid["table"], self.grid["lo"], self.grid["hi"], s)
             if out == 0:
                 return V, dV
         if len(self.heights) == 0:
             return 0.0, np.zeros(self.D)
+        if self.periodic:
+            return bias_periodic(self.centers, self.heights, self.sigma, self.period, s)
         return bias(self.centers, self.heights, self.sigma, s)
 
     # -- a6
@@ -117,8 +140,7 @@ class OracleMetaD:
             self.heights = np.append(self.heights, h)
             if self.grid is not None:
                 k = len(self.heights)
-                grid_add(self.grid["table"], self.grid["lo"], self.grid["hi"], self.centers, self.heights,
-                         self.sigma, k - 1, k)
+                self._grid_add(k - 1, k)
             return h
         return None
 

@@ -23,7 +23,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = os.path.join(_HERE, "libmetad_inputs.so")
 
 # CV kinds (mirrors include/metad.h; plain integers, no arithmetic)
-CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS = 0, 1, 2, 3, 4
+CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION = 0, 1, 2, 3, 4, 5
 
 
 def build_native(force: bool = False) -> str:
@@ -95,6 +95,7 @@ class CVSpec:
     chain: Optional[np.ndarray] = None     # ordered int32      (RGYR)
     q_thresh: float = 0.35
     q_width: float = 0.05
+    atoms: Optional[np.ndarray] = None     # 4 int32 indices i-j-k-l (TORSION)
 
 
 @dataclass
@@ -115,6 +116,7 @@ class Workload:
     hill_centers: Optional[np.ndarray] = None   # (H, D) when the config fixes them (c0)
     hill_heights: Optional[np.ndarray] = None
     grid_n: tuple = (0, 0)
+    period: Optional[list] = None               # per CV dimension; 0 = not periodic (torsions: 2 pi)
     species: Optional[np.ndarray] = None
     extra: dict = field(default_factory=dict)
 
@@ -154,3 +156,18 @@ def seeded_heights(seed, n_hills, w0=1.0):
     """Synthetic hill heights in (0.05*w0, w0] for stage-wise tests that do not replay deposition."""
     rng = np.random.default_rng(seed + 77)
     return w0 * (0.05 + 0.95 * rng.random(n_hills))
+
+
+def hill_walk_periodic(seed, s0, sigma, n_hills, period, lo, step_frac=0.5):
+    """Scripted CV path on a periodic domain: seeded random walk with per-dimension step
+    step_frac*sigma_d, wrapped into [lo_d, lo_d + period_d).  Random-number bookkeeping only."""
+    rng = np.random.default_rng(seed)
+    s0 = np.atleast_1d(np.asarray(s0, dtype=np.float64))
+    sigma = np.atleast_1d(np.asarray(sigma, dtype=np.float64))
+    period = np.atleast_1d(np.asarray(period, dtype=np.float64))
+    lo = np.atleast_1d(np.asarray(lo, dtype=np.float64))
+    steps = rng.standard_normal((n_hills, len(s0))) * (step_frac * sigma)
+    path = s0 + np.concatenate([np.zeros((1, len(s0))), np.cumsum(steps[:-1], axis=0)])
+    out = lo + np.mod(path - lo, period)
+    out[out >= lo + period] = np.broadcast_to(lo, out.shape)[out >= lo + period]
+    return out

@@ -6,8 +6,8 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import (BASE_SEED, CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CVSpec, Workload,
-               rsa, wrap)
+from . import (BASE_SEED, CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CVSpec, Workload,
+               hill_walk_periodic, rsa, wrap)
 
 
 def _cubic(L):
@@ -192,6 +192,28 @@ def config4(seed=BASE_SEED + 4, cells=(160, 160, 40), sphere_r=50.0, n_hills=100
                     species=species)
 
 
+# ----------------------------------------------------------------------------------------- t0
+def config_t0(seed=BASE_SEED + 10, natoms=22, n_hills=20000, grid=(256, 256), n_solvent=0):
+    """Alanine-dipeptide-shaped torsion workload (Phi(C-N-Ca-C), Psi(N-Ca-C-N), sigma = 0.35 rad,
+    W = 1.2 kJ/mol, plain metadynamics; reading Y): a 22-atom chain (seeded self-avoiding walk, 1.5 A bonds,
+    2.2 A exclusion) centred in a cubic box L = 30 A (optionally plus uniform solvent atoms); Phi = atoms 4-6-8-14,
+    Psi = 6-8-14-16 (the usual 0-based backbone indices of the 22-atom molecule); hill centres = seeded walk on the
+    torus [-pi, pi)^2 started at the structure's own (Phi, Psi) (reading K), seeded heights; 256 x 256 periodic grid."""
+    rng = np.random.default_rng(seed)
+    L = 30.0
+    box = _cubic(L)
+    chain = _chain_walk(rng, natoms, 1.5, 2.2, np.full(3, 0.5 * L))
+    solvent = rng.random((n_solvent, 3)) * L
+    pos = wrap(np.concatenate([chain, solvent]), box)
+    cvs = [CVSpec(kind=CV_TORSION, atoms=np.array([4, 6, 8, 14], dtype=np.int32)),
+           CVSpec(kind=CV_TORSION, atoms=np.array([6, 8, 14, 16], dtype=np.int32))]
+    sigma = [0.35, 0.35]
+    P = 2.0 * np.pi
+    return Workload(name="t0", pos=pos, box=box, rc=6.0, max_neigh=64, cvs=cvs, sigma=sigma, n_hills=n_hills, w0=1.2,
+                    bias_factor=1.0, stride=10, precision=64, grid_n=tuple(grid), period=[P, P],
+                    extra={"period_lo": [-np.pi, -np.pi]})
+
+
 def small(name):
     """Scaled-down variants with the same structure, for the CPU suite and quick GPU parity."""
     if name == "c1":
@@ -206,7 +228,9 @@ def small(name):
         return w
     if name == "c0":
         return config0()
+    if name == "t0":
+        return config_t0(n_hills=500, grid=(48, 40))
     raise KeyError(name)
 
 
-BUILDERS = {"c0": config0, "c1": config1, "c2": config2, "c3": config3, "c4": config4}
+BUILDERS = {"c0": config0, "c1": config1, "c2": config2, "c3": config3, "c4": config4, "t0": config_t0}

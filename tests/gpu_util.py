@@ -3,7 +3,7 @@ oracle on the same seeded workload and return both sides' results."""
 import numpy as np
 
 from oracle.reference import OracleMetaD
-from paper_2510_06873_b200.inputs import hill_walk, seeded_heights
+from paper_2510_06873_b200.inputs import hill_walk, hill_walk_periodic, seeded_heights
 
 TOL_CV = 1e-6       # BASELINE.json north_star: "CV, V and dV/ds within 1e-6 relative"
 TOL_F = 1e-5        # "per-atom bias forces within 1e-5 * max|F| absolute"
@@ -38,7 +38,10 @@ def sorted_rows_fast(cnt, lst):
 def make_hills(w, s_ref, seed=5):
     if w.hill_centers is not None:
         return np.asarray(w.hill_centers, float), np.asarray(w.hill_heights, float)
-    c = hill_walk(seed, s_ref, w.sigma, w.n_hills)
+    if getattr(w, "period", None):
+        c = hill_walk_periodic(seed, s_ref, w.sigma, w.n_hills, w.period, w.extra["period_lo"])
+    else:
+        c = hill_walk(seed, s_ref, w.sigma, w.n_hills)
     return c, seeded_heights(seed, w.n_hills, w.w0)
 
 
