@@ -51,7 +51,10 @@ enum metad_cv_kind {
                               (BASELINE.json configs[4]; reading F)                                        */
     METAD_CV_RGYR = 3,     /* radius of gyration of an ordered chain, unwrapped by sequential minimum
                               image (BASELINE.json configs[1]; reading G)                                  */
-    METAD_CV_CONTACTS = 4  /* s = scale * sum_p sw(r_p / r0_p), n, m as given (configs[1]; reading H)      */
+    METAD_CV_CONTACTS = 4, /* s = scale * sum_p sw(r_p / r0_p), n, m as given (configs[1]; reading H)      */
+    METAD_CV_TORSION = 5   /* dihedral angle of atoms torsion[0..3] in (-pi, pi], IUPAC sign, minimum-image bonds
+                              ("Phi(C-N-Ca-C) and Psi(N-Ca-C-N) serve as the CVs"; reading V).
+                              Normally used with params.period = 2 pi for that dimension                  */
 };
 
 typedef struct {
@@ -67,6 +70,7 @@ typedef struct {
     const int *chain; int nchain;   /* RGYR: host ordered atom indices */
     const double *mass;             /* RGYR: host double[nchain] or NULL (equal masses) */
     double q_thresh, q_width;       /* Q6_SOLID */
+    int torsion[4];                 /* TORSION: atom indices i, j, k, l */
 } metad_cv_desc;
 
 #define METAD_MAX_CV 4
@@ -86,6 +90,10 @@ typedef struct {
     int grid_n[2];                  /* grid_n[0] == 0 -> exact hill sum; else ncv must be 2 (reading M) */
     double grid_lo[2], grid_hi[2];
     double force_scale;             /* F += -force_scale * dV/dr (unit conversion; reading N) */
+    double period[METAD_MAX_CV];    /* > 0: the CV dimension is periodic with this period (PAPER.md:37 torsions: 2 pi);
+                                       (s - s_tau) in PAPER.md:81 is then the nearest-image difference (reading W).
+                                       With a grid, a periodic dimension needs grid_hi - grid_lo == period and has
+                                       grid_n nodes at lo + i * period / grid_n, no "outside" (reading X).  0: not periodic */
 } metad_params;
 
 /* Creates a context on the current CUDA device; `cuda_stream` is a cudaStream_t (NULL = default

@@ -36,8 +36,13 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     if (p->precision != 32 && p->precision != 64) FAIL(METAD_ERR_ARG, "precision must be 32 or 64");
     if (p->ncv < 1 || p->ncv > METAD_MAX_CV) FAIL(METAD_ERR_ARG, "ncv out of range");
     if (p->max_neigh < 1 || p->max_hills < 1) FAIL(METAD_ERR_ARG, "max_neigh / max_hills must be positive");
-    for (int d = 0; d < p->ncv; ++d)
+    for (int d = 0; d < p->ncv; ++d) {
         if (!(p->sigma[d] > 0.0)) FAIL(METAD_ERR_ARG, "sigma must be positive");
+        if (!(p->period[d] >= 0.0)) FAIL(METAD_ERR_ARG, "period must be >= 0");
+        if (p->grid_n[0] != 0 && d < 2 && p->period[d] > 0.0 &&
+            fabs((p->grid_hi[d] - p->grid_lo[d]) - p->period[d]) > 1e-12 * p->period[d])
+            FAIL(METAD_ERR_ARG, "a periodic grid dimension needs grid_hi - grid_lo == period");
+    }
     if (p->grid_n[0] != 0 && (p->ncv != 2 || p->grid_n[0] < 2 || p->grid_n[1] < 2 ||
                               !(p->grid_hi[0] > p->grid_lo[0]) || !(p->grid_hi[1] > p->grid_lo[1])))
         FAIL(METAD_ERR_ARG, "grid needs ncv == 2, n >= 2 and hi > lo");
@@ -118,10 +123,29 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
                 return METAD_ERR_CUDA;
             break;
         }
+        case METAD_CV_TORSION: {
+            for (int k = 0; k < 4; ++k) {
+                if (s.torsion[k] < 0 || s.torsion[k] >= N) FAIL(METAD_ERR_ARG, "torsion index");
+                for (int q = 0; q < k; ++q) if (s.torsion[q] == s.torsion[k]) FAIL(METAD_ERR_ARG, "torsion atoms must be distinct");
+                v.tors[k] = s.torsion[k];
+            }
+            c->has_torsion = true;
+            break;
+        }
         default: FAIL(METAD_ERR_ARG, "unknown CV kind");
         }
     }
 
+    if (c->has_torsion) {
+        std::vector<int> ta;
+        for (int d = 0; d < c->D; ++d)
+            if (c->cv[d].kind == METAD_CV_TORSION) for (int k = 0; k < 4; ++k) ta.push_back(c->cv[d].tors[k]);
+        std::sort(ta.begin(), ta.end());
+        ta.erase(std::unique(ta.begin(), ta.end()), ta.end());
+        c->ntors_atoms = (int)ta.size();
+        if (upload_ints(&c->d_tors_atoms, ta.data(), ta.size())) return METAD_ERR_CUDA;
+        CUDA_TRY(dev_alloc(&c->d_tors_grad, 12 * METAD_MAX_CV));
+    }
     // ---- buffers (everything the hot path needs; nothing is allocated later)
     c->cell_cap = std::max(4 * N, 4096);
     c->nblocks_atoms = div_up(N, 128) + 1;
@@ -191,7 +215,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];

@@ -11,12 +11,21 @@ struct BiasParams {
     int D, max_hills;
     double sigma[METAD_MAX_CV];
     double inv_sigma[METAD_MAX_CV];
+    double period[METAD_MAX_CV];     // 0: not periodic (reading W)
 };
 
 struct GridParams {
     int n0, n1;
     double lo[2], hi[2], h[2], inv_h[2];
+    double period[2];                // > 0: periodic dimension, n nodes at lo + i * period / n (reading X)
 };
+
+// s - c brought to the nearest periodic image (reading W); P = 0: plain difference
+__device__ __forceinline__ double pdiff(double s, double c, double P) {
+    double d = s - c;
+    if (P > 0.0) d -= P * rint(d / P);
+    return d;
+}
 
 // device scalars, one int array:  [0] = grid miss flag of this step, [1] = index of the hill
 // deposited in this step (-1: none)
@@ -44,7 +53,7 @@ k_bias_sum(BiasParams bp, const double *__restrict__ centers, const double *__re
 #pragma unroll
         for (int d = 0; d < METAD_MAX_CV; ++d) {
             if (d < bp.D) {
-                t[d] = (s[d] - centers[(size_t)d * bp.max_hills + k]) * bp.inv_sigma[d];
+                t[d] = pdiff(s[d], centers[(size_t)d * bp.max_hills + k], bp.period[d]) * bp.inv_sigma[d];
                 e += t[d] * t[d];
             }
         }
@@ -87,25 +96,43 @@ __global__ void k_bias_grid(GridParams gp, const double *__restrict__ table, con
                             double *__restrict__ V, double *__restrict__ dVds, int *__restrict__ aux,
                             unsigned int *__restrict__ sticky) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    double s0 = cv[0], s1 = cv[1];
-    if (!(s0 >= gp.lo[0]) || !(s0 <= gp.hi[0]) || !(s1 >= gp.lo[1]) || !(s1 <= gp.hi[1])) {
+    double sv[2] = { cv[0], cv[1] };
+    const int nn[2] = { gp.n0, gp.n1 };
+    int i0[2], i1[2];
+    double tt[2];
+    bool miss = false;
+#pragma unroll
+    for (int d = 0; d < 2; ++d) {
+        if (gp.period[d] > 0.0) {            // periodic: wrap into [lo, lo + P); node n coincides with node 0
+            double x = sv[d] - gp.period[d] * floor((sv[d] - gp.lo[d]) / gp.period[d]);
+            if (x >= gp.lo[d] + gp.period[d]) x -= gp.period[d];
+            if (x < gp.lo[d]) x += gp.period[d];
+            const double f = (x - gp.lo[d]) * gp.inv_h[d];
+            const int i = max(min((int)floor(f), nn[d] - 1), 0);
+            tt[d] = f - i; i0[d] = i; i1[d] = i + 1 == nn[d] ? 0 : i + 1;
+        } else {
+            if (!(sv[d] >= gp.lo[d]) || !(sv[d] <= gp.hi[d])) miss = true;
+            const double f = (sv[d] - gp.lo[d]) * gp.inv_h[d];
+            const int i = max(min((int)floor(f), nn[d] - 2), 0);
+            tt[d] = f - i; i0[d] = i; i1[d] = i + 1;
+        }
+    }
+    if (miss || !isfinite(sv[0]) || !isfinite(sv[1])) {
         aux[AUX_GRID_MISS] = 1;
         atomicOr(sticky, (unsigned)METAD_DEV_GRID_RANGE);
         return;
     }
     aux[AUX_GRID_MISS] = 0;
-    double fx = (s0 - gp.lo[0]) * gp.inv_h[0], fy = (s1 - gp.lo[1]) * gp.inv_h[1];
-    int i = min((int)floor(fx), gp.n0 - 2), j = min((int)floor(fy), gp.n1 - 2);
     double hx[4], dhx[4], hy[4], dhy[4];
-    hermite(fx - i, hx, dhx);
-    hermite(fy - j, hy, dhy);
+    hermite(tt[0], hx, dhx);
+    hermite(tt[1], hy, dhy);
     size_t plane = (size_t)gp.n0 * gp.n1;
     double v = 0.0, vx = 0.0, vy = 0.0;
 #pragma unroll
     for (int a = 0; a < 2; ++a)
 #pragma unroll
         for (int b = 0; b < 2; ++b) {
-            size_t o = (size_t)(i + a) * gp.n1 + (j + b);
+            size_t o = (size_t)(a ? i1[0] : i0[0]) * gp.n1 + (b ? i1[1] : i0[1]);
             double f = table[o], f0 = table[plane + o] * gp.h[0], f1 = table[2 * plane + o] * gp.h[1],
                    f01 = table[3 * plane + o] * gp.h[0] * gp.h[1];
             v += f * hx[a] * hy[b] + f0 * hx[2 + a] * hy[b] + f1 * hx[a] * hy[2 + b] + f01 * hx[2 + a] * hy[2 + b];
@@ -137,12 +164,12 @@ k_grid_accumulate(GridParams gp, BiasParams bp, const double *__restrict__ cente
                 int k = base + h;
                 if (which == 0) {
                     double x = gp.lo[0] + (blockIdx.x * GT + t) * gp.h[0];
-                    double a = (x - centers[k]) * bp.inv_sigma[0];
+                    double a = pdiff(x, centers[k], gp.period[0]) * bp.inv_sigma[0];
                     ex[h][t] = heights[k] * exp(-0.5 * a * a);
                     gx[h][t] = -a * bp.inv_sigma[0];
                 } else {
                     double y = gp.lo[1] + (blockIdx.y * GT + t) * gp.h[1];
-                    double b = (y - centers[(size_t)bp.max_hills + k]) * bp.inv_sigma[1];
+                    double b = pdiff(y, centers[(size_t)bp.max_hills + k], gp.period[1]) * bp.inv_sigma[1];
                     ey[h][t] = exp(-0.5 * b * b);
                     gy[h][t] = -b * bp.inv_sigma[1];
                 }
@@ -170,8 +197,8 @@ __global__ void k_grid_add_last(GridParams gp, BiasParams bp, const double *__re
     int o = blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= gp.n0 * gp.n1) return;
     int i = o / gp.n1, j = o % gp.n1;
-    double a = (gp.lo[0] + i * gp.h[0] - centers[k]) * bp.inv_sigma[0];
-    double b = (gp.lo[1] + j * gp.h[1] - centers[(size_t)bp.max_hills + k]) * bp.inv_sigma[1];
+    double a = pdiff(gp.lo[0] + i * gp.h[0], centers[k], gp.period[0]) * bp.inv_sigma[0];
+    double b = pdiff(gp.lo[1] + j * gp.h[1], centers[(size_t)bp.max_hills + k], gp.period[1]) * bp.inv_sigma[1];
     double g = heights[k] * exp(-0.5 * (a * a + b * b));
     double ga = -a * bp.inv_sigma[0], gb = -b * bp.inv_sigma[1];
     size_t plane = (size_t)gp.n0 * gp.n1;
@@ -224,6 +251,7 @@ static BiasParams make_bp(const metad_ctx *c) {
     for (int d = 0; d < METAD_MAX_CV; ++d) {
         bp.sigma[d] = d < c->D ? c->p.sigma[d] : 1.0;
         bp.inv_sigma[d] = 1.0 / bp.sigma[d];
+        bp.period[d] = d < c->D ? c->p.period[d] : 0.0;
     }
     return bp;
 }
@@ -233,7 +261,8 @@ static GridParams make_gp(const metad_ctx *c) {
     for (int d = 0; d < 2; ++d) {
         gp.lo[d] = c->p.grid_lo[d]; gp.hi[d] = c->p.grid_hi[d];
         int n = d == 0 ? gp.n0 : gp.n1;
-        gp.h[d] = n > 1 ? (gp.hi[d] - gp.lo[d]) / (n - 1) : 1.0;
+        gp.period[d] = c->p.period[d];
+        gp.h[d] = gp.period[d] > 0.0 ? (gp.hi[d] - gp.lo[d]) / n : (n > 1 ? (gp.hi[d] - gp.lo[d]) / (n - 1) : 1.0);
         gp.inv_h[d] = 1.0 / gp.h[d];
     }
     return gp;

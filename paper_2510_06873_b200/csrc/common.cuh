@@ -118,6 +118,7 @@ struct CvDev {                      // device copies of one CV descriptor
     int *d_chain; double *d_mass;         // RGYR
     double *d_unwrapped;                  // RGYR scratch: [nchain*3] + com[3] + rg
     bool use_groups;
+    int tors[4];                          // TORSION
 };
 
 struct metad_ctx {
@@ -137,7 +138,9 @@ struct metad_ctx {
     int *d_nl_count, *d_nl;               // sorted space; nl[k*N + s]
     // CV state
     CvDev cv[METAD_MAX_CV];
-    bool has_q6, has_coord;
+    bool has_q6, has_coord, has_torsion;
+    double *d_tors_grad;                  // TORSION: [D][12] d phi / d r of the four atoms, written by the CV kernel
+    int *d_tors_atoms; int ntors_atoms;   //          unique touched atoms (gather-form force kernel: thread per atom)
     int q6_mean_dim, q6_solid_dim, coord_dim;
     void *d_rec;                          // T[N][METAD_NREC]
     double *d_partials;                   // block partial sums
@@ -182,6 +185,8 @@ int nb_export(metad_ctx *c, int *d_count, int *d_list);
 int cv_eval_all(metad_ctx *c, double *d_cv);
 int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F);
 int q6_export(metad_ctx *c, void *d_q6);
+int torsion_eval_all(metad_ctx *c, double *d_cv);
+int torsion_forces(metad_ctx *c, const double *d_dVds, void *d_F);
 int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds);
 int bias_deposit(metad_ctx *c, const double *d_cv, const double *d_V);
 int bias_grid_rebuild(metad_ctx *c);

@@ -388,6 +388,8 @@ int cv_eval_all(metad_ctx *c, double *d_cv) {
             rcode = chain_eval(c, d, nullptr, d_cv);
             if (rcode) return rcode;
         }
+    rcode = torsion_eval_all(c, d_cv);
+    if (rcode) return rcode;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
 }
@@ -422,6 +424,8 @@ int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F) {
     int rcode = c->prec == 32 ? cv_forces_t<float>(c, d_dVds, d_F) : cv_forces_t<double>(c, d_dVds, d_F);
     if (rcode) return rcode;
     rcode = chain_forces(c, d_dVds, d_F);
+    if (rcode) return rcode;
+    rcode = torsion_forces(c, d_dVds, d_F);
     if (rcode) return rcode;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

@@ -2,6 +2,7 @@
 // (BASELINE.json configs[1]; readings G, H).  Tiny kernels: ~1,000 atoms / ~5,000 pairs, all fp64,
 // positions read from the caller's array in its own dtype.
 #include "common.cuh"
+#include "cv_torsion.cuh"
 
 #define RG_THREADS 1024
 
@@ -241,4 +242,80 @@ static int chain_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
 
 int chain_forces(metad_ctx *c, const double *d_dVds, void *d_F) {
     return c->prec == 32 ? chain_forces_t<float>(c, d_dVds, d_F) : chain_forces_t<double>(c, d_dVds, d_F);
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-1: torsion CVs (reading V).  One thread per torsion dimension evaluates the angle and
+// keeps the gradient of its four atoms; the force kernel is gather form (thread per touched atom, fixed
+// summation order over dimensions and slots, no atomics).
+struct TorsTable { int kind[METAD_MAX_CV]; int idx[METAD_MAX_CV][4]; };
+
+template <typename T>
+__global__ void k_torsions_cv(int D, TorsTable tt, const T *__restrict__ pos, BoxD bd, double *__restrict__ grad,
+                              double *__restrict__ cv_out, unsigned int *__restrict__ sticky) {
+    const int d = threadIdx.x;
+    if (d >= D || tt.kind[d] != METAD_CV_TORSION) return;
+    double r[4][3], b[3][3];
+    for (int k = 0; k < 4; ++k)
+        for (int a = 0; a < 3; ++a) r[k][a] = (double)pos[3 * (size_t)tt.idx[d][k] + a];
+    for (int k = 0; k < 3; ++k) {
+        b[k][0] = r[k + 1][0] - r[k][0]; b[k][1] = r[k + 1][1] - r[k][1]; b[k][2] = r[k + 1][2] - r[k][2];
+        min_image_d(bd, b[k][0], b[k][1], b[k][2]);
+    }
+    double g[12];
+    const double phi = torsion_eval(b[0], b[1], b[2], g);
+    for (int k = 0; k < 12; ++k) grad[12 * d + k] = g[k];
+    cv_out[d] = phi;
+    if (!isfinite(phi)) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
+}
+
+template <typename T>
+__global__ void k_torsions_force(int D, TorsTable tt, int natoms_touched, const int *__restrict__ atoms,
+                                 const double *__restrict__ grad, double force_scale, const double *__restrict__ dVds,
+                                 T *__restrict__ F) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= natoms_touched) return;
+    const int a = atoms[t];
+    double f[3] = { 0.0, 0.0, 0.0 };
+    for (int d = 0; d < D; ++d) {
+        if (tt.kind[d] != METAD_CV_TORSION) continue;
+        const double w = dVds[d];
+        for (int k = 0; k < 4; ++k)
+            if (tt.idx[d][k] == a) { f[0] += w * grad[12 * d + 3 * k]; f[1] += w * grad[12 * d + 3 * k + 1]; f[2] += w * grad[12 * d + 3 * k + 2]; }
+    }
+    F[3 * (size_t)a] += (T)(-force_scale * f[0]);
+    F[3 * (size_t)a + 1] += (T)(-force_scale * f[1]);
+    F[3 * (size_t)a + 2] += (T)(-force_scale * f[2]);
+}
+
+static TorsTable tors_table(const metad_ctx *c) {
+    TorsTable tt;
+    for (int d = 0; d < METAD_MAX_CV; ++d) {
+        tt.kind[d] = d < c->D ? c->cv[d].kind : -1;
+        for (int k = 0; k < 4; ++k) tt.idx[d][k] = d < c->D ? c->cv[d].tors[k] : 0;
+    }
+    return tt;
+}
+
+int torsion_eval_all(metad_ctx *c, double *d_cv) {
+    if (!c->has_torsion) return METAD_OK;
+    if (c->prec == 32)
+        k_torsions_cv<float><<<1, 32, 0, c->stream>>>(c->D, tors_table(c), (const float *)ctx_last_pos(c), c->boxd, c->d_tors_grad, d_cv, c->d_sticky);
+    else
+        k_torsions_cv<double><<<1, 32, 0, c->stream>>>(c->D, tors_table(c), (const double *)ctx_last_pos(c), c->boxd, c->d_tors_grad, d_cv, c->d_sticky);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+int torsion_forces(metad_ctx *c, const double *d_dVds, void *d_F) {
+    if (!c->has_torsion) return METAD_OK;
+    if (c->prec == 32)
+        k_torsions_force<float><<<1, 32, 0, c->stream>>>(c->D, tors_table(c), c->ntors_atoms, c->d_tors_atoms, c->d_tors_grad, c->p.force_scale, d_dVds, (float *)d_F);
+    else
+        k_torsions_force<double><<<1, 32, 0, c->stream>>>(c->D, tors_table(c), c->ntors_atoms, c->d_tors_atoms, c->d_tors_grad, c->p.force_scale, d_dVds, (double *)d_F);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
 }

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmetad_b200.so")
 MAX_CV = 4
 OK, ERR_ARG, ERR_BOX, ERR_STATE, ERR_CUDA, ERR_NOMEM = range(6)
 DEV_NEIGH_OVERFLOW, DEV_HILL_OVERFLOW, DEV_GRID_RANGE, DEV_NONFINITE, DEV_POS_RANGE = 1, 2, 4, 8, 16
-CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS = range(5)
+CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION = range(6)
 
 _P = ctypes.c_void_p
 _I = ctypes.c_int
@@ -29,14 +29,14 @@ class CvDesc(ctypes.Structure):
                 ("group_a", _P), ("n_a", _I), ("group_b", _P), ("n_b", _I),
                 ("pairs", _P), ("pair_r0", _P), ("npairs", _I),
                 ("chain", _P), ("nchain", _I), ("mass", _P),
-                ("q_thresh", _D), ("q_width", _D)]
+                ("q_thresh", _D), ("q_width", _D), ("torsion", _I * 4)]
 
 
 class Params(ctypes.Structure):
     _fields_ = [("natoms", _I), ("precision", _I), ("max_neigh", _I), ("ncv", _I),
                 ("cv", CvDesc * MAX_CV), ("sigma", _D * MAX_CV), ("w0", _D), ("kT", _D),
                 ("bias_factor", _D), ("max_hills", _I), ("stride", _I), ("grid_n", _I * 2),
-                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D)]
+                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV)]
 
 
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
@@ -135,7 +135,12 @@ class MetaD:
                 b = np.ascontiguousarray(cv.pair_r0, dtype=np.float64)
                 self._keep += [a, b]
                 c.pairs, c.pair_r0, c.npairs = a.ctypes.data, b.ctypes.data, len(b)
+            if getattr(cv, "atoms", None) is not None:
+                for k in range(4):
+                    c.torsion[k] = int(cv.atoms[k])
             p.sigma[d] = float(w.sigma[d])
+            per = getattr(w, "period", None)
+            p.period[d] = float(per[d]) if per else 0.0
         p.w0, p.kT, p.bias_factor = float(w.w0), float(w.kT), float(w.bias_factor)
         self.max_hills = int(max_hills if max_hills is not None else max(w.n_hills + 1024, 1024))
         p.max_hills, p.stride = self.max_hills, int(w.stride)
