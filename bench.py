@@ -35,7 +35,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="c3", choices=["c0", "c1", "c2", "c3", "c4"])
+    ap.add_argument("--config", default="c3", choices=["c0", "c1", "c2", "c3", "c4", "t0"])
     ap.add_argument("--precision", type=int, default=0, help="0 = the workload's own (c3: 32 for the headline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fast-setup", action="store_true",
@@ -50,8 +50,10 @@ def workload(name):
 
 
 def describe(w, precision):
-    kinds = {0: "coordination", 1: "Q6 mean", 2: "Q6 solid-like count", 3: "radius of gyration", 4: "native contacts"}
-    return {"workload": f"BASELINE.json configs[{w.name[1]}] ({w.name})", "atoms": int(w.natoms),
+    kinds = {0: "coordination", 1: "Q6 mean", 2: "Q6 solid-like count", 3: "radius of gyration", 4: "native contacts", 5: "torsion"}
+    wl = ("PAPER.md:37 alanine-dipeptide-shaped torsion workload (t0, SURVEY.md §8(f) NEXT-1)" if w.name == "t0"
+          else f"BASELINE.json configs[{w.name[1]}] ({w.name})")
+    return {"workload": wl, "atoms": int(w.natoms),
             "cvs": [kinds[c.kind] for c in w.cvs], "hills": int(w.n_hills), "rc": w.rc,
             "pair_precision": f"fp{precision}", "stride": int(w.stride),
             "l2": "per-step working set (neighbour list + q6 records + positions + forces) exceeds the 126 MB L2; no flush"}
@@ -118,12 +120,15 @@ def oracle_time_steps(w, nsteps):
     """Times the oracle as it stands (never tuned) on the host cores: full steps incl. neighbour build."""
     import oracle
     from oracle.reference import OracleMetaD
-    from paper_2510_06873_b200.inputs import hill_walk, seeded_heights
+    from paper_2510_06873_b200.inputs import hill_walk, hill_walk_periodic, seeded_heights
     o = OracleMetaD(w)
     o.build_neighbors(w.pos)
     s0 = o.eval_cv(want_grad=False)
     if w.hill_centers is not None:
         o.set_hills(w.hill_centers, w.hill_heights)
+    elif w.period:
+        o.set_hills(hill_walk_periodic(5, s0, w.sigma, w.n_hills, w.period, w.extra["period_lo"]),
+                    seeded_heights(5, w.n_hills, w.w0))
     else:
         o.set_hills(hill_walk(5, s0, w.sigma, w.n_hills), seeded_heights(5, w.n_hills, w.w0))
     F = np.zeros((w.natoms, 3))
@@ -181,7 +186,7 @@ def job_throughput(world, atoms_per_replica, steps, ms_max):
 def prepare_hills(w, md_cls, precision, dpos, torch):
     """Hill centres = seeded walk around the structure's own CV (reading K); heights by replaying the
     well-tempered rule through the library's own bias+deposit kernels (stride-1 helper context)."""
-    from paper_2510_06873_b200.inputs import hill_walk
+    from paper_2510_06873_b200.inputs import hill_walk, hill_walk_periodic
     import copy
     if w.hill_centers is not None:
         return np.asarray(w.hill_centers), np.asarray(w.hill_heights)
@@ -191,7 +196,10 @@ def prepare_hills(w, md_cls, precision, dpos, torch):
     probe.synchronize()
     s0 = probe.cv.cpu().numpy()
     probe.close()
-    centers = hill_walk(5, s0, w.sigma, w.n_hills)
+    if w.period:
+        centers = hill_walk_periodic(5, s0, w.sigma, w.n_hills, w.period, w.extra["period_lo"])
+    else:
+        centers = hill_walk(5, s0, w.sigma, w.n_hills)
     w1 = copy.copy(w)
     w1.stride = 1
     w1.cvs = w.cvs
@@ -245,12 +253,20 @@ def run_ours(args):
     torch.cuda.synchronize()
     if args.fast_setup:
         from paper_2510_06873_b200.inputs import hill_walk, seeded_heights
-        centers, heights = hill_walk(5, np.full(w.ncv, 0.23), w.sigma, w.n_hills), seeded_heights(5, w.n_hills, w.w0)
+        if w.period:
+            from paper_2510_06873_b200.inputs import hill_walk_periodic
+            centers = hill_walk_periodic(5, np.zeros(w.ncv), w.sigma, w.n_hills, w.period, w.extra["period_lo"])
+        else:
+            centers = hill_walk(5, np.full(w.ncv, 0.23), w.sigma, w.n_hills)
+        heights = seeded_heights(5, w.n_hills, w.w0)
     else:
         centers, heights = prepare_hills(w, MetaD, precision, dpos, torch)
 
     grid = None
-    if w.grid_n[0]:
+    if w.grid_n[0] and w.period:
+        lo = np.asarray(w.extra["period_lo"], dtype=np.float64)
+        grid = (w.grid_n, lo, lo + np.asarray(w.period))                        # reading X: one period
+    elif w.grid_n[0]:
         sig = np.asarray(w.sigma)
         grid = (w.grid_n, centers[0] - 120 * sig, centers[0] + 120 * sig)      # reading M
     md = MetaD(w, precision=precision, max_hills=w.n_hills + args.steps + args.warmup + 4096, grid=grid)

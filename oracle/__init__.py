@@ -69,6 +69,7 @@ def lib():
         L.orc_wrap.argtypes = [_D, _D, _D]
         L.orc_bias_periodic.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P, _P]
         L.orc_grid_add_p.argtypes = [_I, _I, _P, _P, _P, _I, _I, _P, _P, _P, _P]
+        L.orc_reweight.argtypes = [_I, _I, _P, _I, _P, _P, _P, _P, _D, _P, _P, _P, _P, _P]
         L.orc_grid_eval_p.restype = _I
         L.orc_grid_eval_p.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P, _P]
         _lib = L
@@ -285,3 +286,21 @@ def grid_eval_p(table, lo, hi, periodic, s):
     out = lib().orc_grid_eval_p(table.shape[1], table.shape[2], _p(lo), _p(hi), _p(periodic), _p(table), _p(s),
                                 ctypes.addressof(V), _p(dV))
     return out, V.value, dV
+
+
+# ---- NEXT-2: free-energy reconstruction by reweighting (reading Z)
+def reweight(traj, centers, heights, sigma, period, kT, nbins, lo, hi):
+    """Returns (P, F), each (nb0, nb1) (nb1 = 1 for a 1-D CV)."""
+    sigma = _f(np.atleast_1d(sigma))
+    D = len(sigma)
+    traj = _f(traj).reshape(-1, D)
+    heights = _f(heights)
+    centers = _f(centers).reshape(len(heights), D)
+    period = _f(np.zeros(D) if period is None else np.atleast_1d(period))
+    nb = _i(list(np.atleast_1d(nbins)) + [1] * (2 - D))
+    lo2, hi2 = _f(list(np.atleast_1d(lo)) + [0.0] * (2 - D)), _f(list(np.atleast_1d(hi)) + [1.0] * (2 - D))
+    P = np.zeros((int(nb[0]), int(nb[1])))
+    F = np.zeros_like(P)
+    lib().orc_reweight(D, len(traj), _p(traj), len(heights), _p(centers), _p(heights), _p(sigma), _p(period), float(kT),
+                       _p(nb), _p(lo2), _p(hi2), _p(P), _p(F))
+    return P, F

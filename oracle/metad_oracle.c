@@ -726,3 +726,45 @@ int orc_grid_eval_p(int n0, int n1, const double *lo, const double *hi, const in
     *V = v; dVds[0] = vx / h[0]; dVds[1] = vy / h[1];
     return 0;
 }
+
+/* =============================================================================================
+ * NEXT-2: free-energy reconstruction by reweighting:
+ *     P_unbias(s) = < delta[s - s(R)] e^{beta V_b(s)} >_{U_b} / < e^{beta V_b(s)} >_{U_b},
+ *     F(s) = -(1/beta) log P_unbias(s),
+ * the averages running over the frames of the biased trajectory, V_b the (final) bias potential.
+ * Reading Z: the delta function is a histogram on uniform bins (bin b of dimension d covers
+ * [lo_d + b h_d, lo_d + (b+1) h_d), h_d = (hi_d - lo_d)/nb_d; a periodic dimension is wrapped into
+ * [lo_d, hi_d) first); P is the bin average divided by the bin volume; frames outside the range of
+ * a non-periodic dimension count in the denominator only; empty bins give F = +inf.
+ * traj [T][D] row-major, D = 1 or 2 (nb[1] = 1, lo/hi[1] ignored for D = 1); P, F [nb0][nb1].       */
+void orc_reweight(int D, int T, const double *traj, int H, const double *centers, const double *heights,
+                  const double *sigma, const double *period, double kT, const int *nb, const double *lo,
+                  const double *hi, double *P, double *F) {
+    int n0 = nb[0], n1 = D > 1 ? nb[1] : 1;
+    double vol = 1.0;
+    for (int d = 0; d < D; ++d) vol *= (hi[d] - lo[d]) / nb[d];
+    for (int b = 0; b < n0 * n1; ++b) P[b] = 0.0;
+    double den = 0.0;
+    for (int t = 0; t < T; ++t) {
+        const double *s = traj + (size_t)t * D;
+        double V, dV[8];
+        orc_bias_periodic(D, H, centers, heights, sigma, period, s, &V, dV);
+        double w = exp(V / kT);
+        den += w;
+        int idx[2] = { 0, 0 }, inside = 1;
+        for (int d = 0; d < D; ++d) {
+            double x = s[d];
+            if (period[d] > 0.0) x = orc_wrap(x, lo[d], period[d]);
+            double f = (x - lo[d]) / ((hi[d] - lo[d]) / nb[d]);
+            int b = (int)floor(f);
+            if (period[d] > 0.0 && b >= nb[d]) b = nb[d] - 1;
+            if (b < 0 || b >= nb[d] || !(x >= lo[d])) inside = 0;
+            idx[d] = b;
+        }
+        if (inside) P[(size_t)idx[0] * n1 + idx[1]] += w;
+    }
+    for (int b = 0; b < n0 * n1; ++b) {
+        P[b] = P[b] / (den * vol);
+        F[b] = P[b] > 0.0 ? -kT * log(P[b]) : INFINITY;
+    }
+}
