@@ -156,6 +156,21 @@ int metad_get_hills(metad_ctx *ctx, double *centers, double *heights, int capaci
 /* Grid table [4][n0][n1] = V, dV/ds0, dV/ds1, d2V/ds0ds1 at the nodes; copied to d_table. */
 int metad_get_grid(metad_ctx *ctx, double *d_table);
 
+/* NEXT-2 — batched bias: V_b at npoints CV points (d_points: double[npoints][ncv], d_V: double[npoints]) by the exact
+ * hill sum over the hills deposited so far (periodic dimensions by nearest image).  Enqueued. */
+int metad_bias_batch(metad_ctx *ctx, const double *d_points, int npoints, double *d_V);
+
+/* NEXT-2 — free-energy reconstruction by reweighting:
+ *     P(s) = < delta[s - s(R)] e^{V_b(s)/kT} > / < e^{V_b(s)/kT} >,   F(s) = -kT log P(s),
+ * averages over the nframes CV frames d_traj (double[nframes][ncv], ncv = 1 or 2) of a biased run, V_b = the current
+ * hills.  The delta is a histogram (reading Z): h_nbins[d] uniform bins on [h_lo[d], h_hi[d]) (periodic
+ * dimensions are wrapped first and need hi - lo == period); frames outside a non-periodic range count in the
+ * denominator only.  d_P, d_F: double[nbins0 * nbins1] row-major (nbins1 = 1 if ncv = 1); empty bins: P = 0, F = +inf.
+ * Weights are accumulated as 2^-40 fixed point relative to the largest one (integer atomics: bit-identical from run to
+ * run).  Not a per-step call: allocates and frees its scratch (V per frame, bins).  [sync] */
+int metad_reweight(metad_ctx *ctx, const double *d_traj, int nframes, const int *h_nbins, const double *h_lo,
+                   const double *h_hi, double *d_P, double *d_F);
+
 /* Resets the step counter (hills stay). */
 int metad_reset_steps(metad_ctx *ctx);
 

@@ -466,6 +466,26 @@ extern "C" int metad_get_grid(metad_ctx *c, double *d_table) {
     return METAD_OK;
 }
 
+extern "C" int metad_bias_batch(metad_ctx *c, const double *d_points, int npoints, double *d_V) {
+    if (!c || npoints < 0 || (npoints > 0 && (!d_points || !d_V))) FAIL(METAD_ERR_ARG, "bad argument");
+    return bias_batch(c, d_points, npoints, d_V);
+}
+
+extern "C" int metad_reweight(metad_ctx *c, const double *d_traj, int nframes, const int *h_nbins, const double *h_lo,
+                              const double *h_hi, double *d_P, double *d_F) {
+    if (!c || nframes < 0 || (nframes > 0 && !d_traj) || !h_nbins || !h_lo || !h_hi || !d_P || !d_F)
+        FAIL(METAD_ERR_ARG, "bad argument");
+    if (c->D > 2) FAIL(METAD_ERR_ARG, "reweighting histograms 1 or 2 CV dimensions");
+    if (!(c->p.kT > 0.0)) FAIL(METAD_ERR_ARG, "kT must be positive");
+    for (int d = 0; d < c->D; ++d) {
+        if (h_nbins[d] < 1 || !(h_hi[d] > h_lo[d])) FAIL(METAD_ERR_ARG, "bins need n >= 1 and hi > lo");
+        if (c->p.period[d] > 0.0 && fabs((h_hi[d] - h_lo[d]) - c->p.period[d]) > 1e-12 * c->p.period[d])
+            FAIL(METAD_ERR_ARG, "a periodic dimension needs hi - lo == period");
+    }
+    if ((long long)h_nbins[0] * (c->D > 1 ? h_nbins[1] : 1) > (1ll << 26)) FAIL(METAD_ERR_ARG, "too many bins");
+    return reweight_run(c, d_traj, nframes, h_nbins, h_lo, h_hi, d_P, d_F);
+}
+
 extern "C" int metad_reset_steps(metad_ctx *c) {
     if (!c) FAIL(METAD_ERR_ARG, "null argument");
     CUDA_TRY(cudaMemsetAsync(c->d_step, 0, sizeof(int), c->stream));

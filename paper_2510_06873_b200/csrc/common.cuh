@@ -192,6 +192,9 @@ int bias_deposit(metad_ctx *c, const double *d_cv, const double *d_V);
 int bias_grid_rebuild(metad_ctx *c);
 int bias_set_hills_dev(metad_ctx *c, const double *d_centers_rowmajor, const double *d_heights, int count);
 int bias_get_hills_dev(metad_ctx *c, double *d_centers_rowmajor, double *d_heights, int capacity);
+int bias_batch(metad_ctx *c, const double *d_points, int T, double *d_V);
+int reweight_run(metad_ctx *c, const double *d_traj, int T, const int *nbins, const double *lo, const double *hi,
+                 double *d_P, double *d_F);
 int tiled_init();
 int tiled_build(metad_ctx *c);
 int tiled_q6_pass1(metad_ctx *c, double *d_cv);

@@ -42,7 +42,7 @@ class Params(ctypes.Structure):
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
            "metad_apply_forces", "metad_deposit", "metad_run", "metad_step_host", "metad_status",
            "metad_get_state", "metad_get_neighbors", "metad_get_q6", "metad_set_hills", "metad_get_hills",
-           "metad_get_grid", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
+           "metad_get_grid", "metad_bias_batch", "metad_reweight", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
 
 _lib = None
 
@@ -73,6 +73,8 @@ def load():
     L.metad_get_hills.argtypes = [_P, _P, _P, _I, _P, _I]
     L.metad_get_grid.argtypes = [_P, _P]
     L.metad_reset_steps.argtypes = [_P]
+    L.metad_bias_batch.argtypes = [_P, _P, _I, _P]
+    L.metad_reweight.argtypes = [_P, _P, _I, _P, _P, _P, _P, _P]
     L.metad_set_timing.argtypes = [_P, _I]
     L.metad_get_timing.argtypes = [_P, _P, _P]
     L.metad_launch_count.argtypes = [_P]
@@ -265,6 +267,28 @@ class MetaD:
         _check(load().metad_get_grid(self._h, _ptr(t)))
         self.synchronize()
         return t.cpu().numpy()
+
+    def bias_batch(self, points):
+        """V_b at many CV points (torch float64 CUDA tensor [T, ncv]) -> tensor [T]."""
+        torch = self.torch
+        T = int(points.shape[0])
+        with torch.cuda.stream(self.stream):
+            V = torch.empty(T, dtype=torch.float64, device="cuda")
+        _check(load().metad_bias_batch(self._h, _ptr(points), T, _ptr(V)))
+        return V
+
+    def reweight(self, traj, nbins, lo, hi):
+        """(P, F) on the bins, numpy arrays of shape (nb0, nb1)."""
+        torch = self.torch
+        T = int(traj.shape[0])
+        nb = (ctypes.c_int * 2)(int(nbins[0]), int(nbins[1]) if self.D > 1 else 1)
+        lo2 = (ctypes.c_double * 2)(float(lo[0]), float(lo[1]) if self.D > 1 else 0.0)
+        hi2 = (ctypes.c_double * 2)(float(hi[0]), float(hi[1]) if self.D > 1 else 1.0)
+        with torch.cuda.stream(self.stream):
+            P = torch.empty((nb[0], nb[1]), dtype=torch.float64, device="cuda")
+            F = torch.empty((nb[0], nb[1]), dtype=torch.float64, device="cuda")
+        _check(load().metad_reweight(self._h, _ptr(traj), T, nb, lo2, hi2, _ptr(P), _ptr(F)))
+        return P.cpu().numpy(), F.cpu().numpy()
 
     def reset_steps(self):
         _check(load().metad_reset_steps(self._h))

@@ -1,0 +1,98 @@
+"""-m gpu: NEXT-2 — batched bias and reweighting of the CUDA path against the oracle."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle  # noqa: E402
+from paper_2510_06873_b200.inputs import configs, hill_walk, hill_walk_periodic, seeded_heights  # noqa: E402
+
+from gpu_util import TOL_CV, rel  # noqa: E402
+
+P2 = 2.0 * np.pi
+
+
+def _ctx(w, centers, heights):
+    from paper_2510_06873_b200.metad import MetaD
+    md = MetaD(w, max_hills=len(heights) + 8)
+    md.set_hills(centers, heights)
+    return md
+
+
+def test_bias_batch_matches_oracle_point_by_point():
+    import torch
+    for name in ("t0", "c0'", "c4"):
+        w = configs.config0(shifted=True) if name == "c0'" else configs.small(name)
+        rng = np.random.default_rng(11)
+        if w.period:
+            c = hill_walk_periodic(5, np.zeros(2), w.sigma, 700, w.period, w.extra["period_lo"])
+            pts = rng.uniform(-4.0, 4.0, (3001, 2))
+        elif name == "c4":
+            c = hill_walk(5, [0.23, 400.0], w.sigma, 700)
+            pts = c[rng.integers(0, 700, 3001)] + rng.standard_normal((3001, 2)) * np.asarray(w.sigma)
+        else:
+            c = np.asarray(w.hill_centers)
+            pts = rng.uniform(4.5, 13.5, (3001, 1))
+        h = seeded_heights(5, len(c), w.w0)
+        md = _ctx(w, c, h)
+        with torch.cuda.stream(md.stream):
+            dp = torch.tensor(pts, device="cuda")
+        V = md.bias_batch(dp)
+        md.synchronize()
+        V = V.cpu().numpy()
+        per = w.period if w.period else np.zeros(w.ncv)
+        ref = np.array([oracle.bias_periodic(c, h, w.sigma, per, s)[0] for s in pts])
+        big = ref > 1e-12 * ref.max()
+        assert big.sum() > 100
+        assert np.abs(V[big] - ref[big]).max() / 1.0 <= TOL_CV * ref.max()
+        assert (np.abs(V[big] - ref[big]) / ref[big]).max() <= TOL_CV
+        assert md.status() == 0
+
+
+@pytest.mark.parametrize("name", ["t0", "c0'"])
+def test_reweight_matches_oracle(name):
+    import torch
+    w = configs.config0(shifted=True) if name == "c0'" else configs.small(name)
+    rng = np.random.default_rng(12)
+    T = 20011
+    if name == "t0":
+        c = hill_walk_periodic(5, np.zeros(2), w.sigma, 400, w.period, w.extra["period_lo"])
+        traj = hill_walk_periodic(6, np.zeros(2), [1.0, 1.0], T, w.period, w.extra["period_lo"], step_frac=0.3)
+        traj = traj + rng.integers(-1, 2, traj.shape) * P2            # unwrapped frames must be wrapped by the library
+        nb, lo, hi = [36, 30], [-np.pi, -np.pi], [np.pi, np.pi]
+        h = seeded_heights(5, len(c), w.w0)
+    else:
+        c = np.asarray(w.hill_centers)
+        traj = rng.uniform(4.0, 14.0, (T, 1))                          # some frames outside the histogram range
+        nb, lo, hi = [64], [5.0], [13.0]
+        h = 3.0 * seeded_heights(5, len(c), w.w0)
+    md = _ctx(w, c, h)
+    with torch.cuda.stream(md.stream):
+        dt = torch.tensor(traj, device="cuda")
+    md.synchronize()
+    P, F = md.reweight(dt, nb, lo, hi)
+    P_ref, F_ref = oracle.reweight(traj, c, h, w.sigma, w.period, w.kT, nb, lo, hi)
+    assert P.shape == P_ref.shape
+    # weights are 2^-40 fixed point relative to the largest one: absolute bound on P, relative where P is resolved
+    assert np.abs(P - P_ref).max() <= 1e-9 * P_ref.max()
+    ok = P_ref > 1e-5 * P_ref.max()
+    assert ok.sum() > 10
+    assert (np.abs(P[ok] - P_ref[ok]) / P_ref[ok]).max() <= TOL_CV
+    assert np.abs(F[ok] - F_ref[ok]).max() <= TOL_CV * w.kT * 10
+    assert np.array_equal(np.isinf(F), P == 0.0)
+    # run-to-run bit-identical (integer atomics)
+    Pb, Fb = md.reweight(dt, nb, lo, hi)
+    assert np.array_equal(P, Pb) and np.array_equal(F, Fb)
+    assert md.status() == 0
+
+
+def test_reweight_argument_errors():
+    import torch
+    from paper_2510_06873_b200.metad import MetadError
+    w = configs.small("t0")
+    md = _ctx(w, np.zeros((1, 2)), np.ones(1))
+    dt = torch.zeros((4, 2), device="cuda", dtype=torch.float64)
+    with pytest.raises(MetadError):
+        md.reweight(dt, [8, 8], [-np.pi, -np.pi], [np.pi, 3.0])        # span != period
+    with pytest.raises(MetadError):
+        md.reweight(dt, [0, 8], [-np.pi, -np.pi], [np.pi, np.pi])
