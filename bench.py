@@ -392,6 +392,26 @@ def run_ours(args):
             "stages_ms": {n: float(v) for n, v in zip(stage_names, stage_ms)},
             "state": {"cv": [float(x) for x in state["cv"]], "V": float(state["V"]), "nhills": state["nhills"],
                       "sticky": status}}
+    if w.period and w.ncv == 2:
+        # NEXT-2: reweighting of a synthetic 2^20-frame CV trajectory against the workload's hills
+        from paper_2510_06873_b200.inputs import hill_walk_periodic
+        T = 1 << 20
+        traj = hill_walk_periodic(9, np.zeros(2), [1.0, 1.0], T, w.period, w.extra["period_lo"], step_frac=0.3)
+        with torch.cuda.stream(md.stream):
+            dt = torch.tensor(traj, device="cuda")
+        md.synchronize()
+        lo = np.asarray(w.extra["period_lo"]); hi = lo + np.asarray(w.period)
+        md.reweight(dt, (128, 128), lo, hi)
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record(md.stream)
+        Pm, Fm = md.reweight(dt, (128, 128), lo, hi)
+        r1.record(md.stream)
+        torch.cuda.synchronize()
+        rms = r0.elapsed_time(r1)
+        nh = md.state()["nhills"]
+        line["reweight"] = {"frames": T, "hills": int(nh), "bins": [128, 128], "ms": rms,
+                            "gaussian_evals_per_s": T * nh / (rms * 1e-3), "dtype": "f64",
+                            "fes_span_kT": float((Fm[np.isfinite(Fm)].max() - Fm.min()) / w.kT)}
     if not args.no_cpu_baseline and world == 1:
         ws, desc = oracle_sample(args.config)
         times, cores = oracle_time_steps(ws, 2)

@@ -173,6 +173,7 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
         CUDA_TRY(dev_alloc(&c->d_cvq6, 2));
     }
     CUDA_TRY(dev_alloc(&c->d_partials, 3 * (size_t)c->nblocks_atoms + max_pair_blocks));
+    if (c->has_coord && N <= METAD_WARP_PER_ATOM_MAX) CUDA_TRY(dev_alloc(&c->d_partials_warp, (size_t)N / 4 + 2));
     CUDA_TRY(dev_alloc(&c->d_tickets, 16));
     CUDA_TRY(cudaMemset(c->d_tickets, 0, sizeof(unsigned) * 16));
     CUDA_TRY(dev_alloc(&c->d_centers, (size_t)c->D * p->max_hills));
@@ -215,7 +216,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];

@@ -5,6 +5,10 @@
 #include <stdint.h>
 #include "../../include/metad.h"
 
+// generic (non-tiled) kernels switch from one thread to one warp per atom below this size: a system this small cannot
+// fill 148 SMs with one thread per atom (BASELINE.json configs[0]-[2] are latency-bound otherwise)
+#define METAD_WARP_PER_ATOM_MAX 32768
+
 #define METAD_NREC 16  // per-atom Q6 record: 13 normalised q6m components + f'(q6) + q6 + pad
 
 // ------------------------------------------------------------------------------------------------
@@ -144,6 +148,7 @@ struct metad_ctx {
     int q6_mean_dim, q6_solid_dim, coord_dim;
     void *d_rec;                          // T[N][METAD_NREC]
     double *d_partials;                   // block partial sums
+    double *d_partials_warp;              // block partial sums of the warp-per-atom coordination kernel (N/4 blocks)
     unsigned int *d_tickets;
     int nblocks_atoms;
     // bias state (all device)

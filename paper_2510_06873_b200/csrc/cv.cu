@@ -110,6 +110,86 @@ k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int 
     F[3 * i + 2] += (T)(a * (double)az);
 }
 
+// Warp-per-atom variants for small systems (N <= METAD_WARP_PER_ATOM_MAX): the lanes share an atom's neighbours, a fixed
+// shuffle tree sums the lane partials (deterministic).  Same arithmetic per pair as the thread-per-atom kernels.
+template <typename T>
+__global__ void __launch_bounds__(CV_THREADS)
+k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
+                const int *__restrict__ nl, PBox<T> pb, T inv_r0, int n, int m, double scale,
+                double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
+                unsigned int *__restrict__ sticky) {
+    __shared__ double red[32];
+    const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    T acc = T(0);
+    if (s < N) {
+        typename Vec4<T>::type pi = spos[s];
+        if (((int)pi.w) & 1) {
+            const int cnt = nl_count[s];
+            for (int k = lane; k < cnt; k += 32) {
+                const int j = nl[(size_t)k * N + s];
+                typename Vec4<T>::type pj = spos[j];
+                if (!(((int)pj.w) & 2)) continue;
+                T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+                min_image(pb, dx, dy, dz);
+                T r = sqrt(dx * dx + dy * dy + dz * dz), dsw;
+                acc += switch_fn<T>(r * inv_r0, n, m, dsw);
+            }
+        }
+    }
+    double v[1] = { (double)acc };
+    block_reduce<1>(v, red);
+    if (threadIdx.x == 0) partials[blockIdx.x] = v[0];
+    if (last_block_ticket(ticket)) {
+        double t[1] = { 0.0 };
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) t[0] += partials[b];
+        block_reduce<1>(t, red);
+        if (threadIdx.x == 0) {
+            double r = scale * t[0];
+            *cv_out = r;
+            if (!isfinite(r)) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
+        }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(CV_THREADS)
+k_coord_force_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
+                   const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, T inv_r0, int n, int m,
+                   double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F) {
+    const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (s >= N) return;
+    typename Vec4<T>::type pi = spos[s];
+    const int fi = (int)pi.w;
+    T ax = T(0), ay = T(0), az = T(0);
+    const int cnt = nl_count[s];
+    for (int k = lane; k < cnt; k += 32) {
+        const int j = nl[(size_t)k * N + s];
+        typename Vec4<T>::type pj = spos[j];
+        const int fj = (int)pj.w;
+        const int mult = ((fi & 1) && (fj & 2)) + ((fi & 2) && (fj & 1));
+        if (!mult) continue;
+        T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+        min_image(pb, dx, dy, dz);
+        T r = sqrt(dx * dx + dy * dy + dz * dz), dsw;
+        switch_fn<T>(r * inv_r0, n, m, dsw);
+        T g = T(mult) * dsw * inv_r0 / r;
+        ax += g * dx; ay += g * dy; az += g * dz;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        ax += __shfl_down_sync(0xffffffffu, ax, o);
+        ay += __shfl_down_sync(0xffffffffu, ay, o);
+        az += __shfl_down_sync(0xffffffffu, az, o);
+    }
+    if (lane == 0) {
+        const double a = coef * dVds[0];
+        const int i = perm[s];
+        F[3 * i] += (T)(a * (double)ax);
+        F[3 * i + 1] += (T)(a * (double)ay);
+        F[3 * i + 2] += (T)(a * (double)az);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // Q6 pass 1: per-atom q6m accumulation -> record + block partials of (sum q6, sum f(q6))
 template <typename T>
@@ -358,6 +438,11 @@ static int cv_eval_t(metad_ctx *c, double *d_cv) {
     PBox<T> pb = ctx_pbox<T>(c);
     if (c->has_coord) {
         const CvDev &d = c->cv[c->coord_dim];
+        if (N <= METAD_WARP_PER_ATOM_MAX)
+            k_coord_cv_warp<T><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials_warp,
+                c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky);
+        else
         k_coord_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb,
                                                        (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials,
                                                        c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky);
@@ -401,6 +486,11 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
     PBox<T> pb = ctx_pbox<T>(c);
     if (c->has_coord) {
         const CvDev &d = c->cv[c->coord_dim];
+        if (N <= METAD_WARP_PER_ATOM_MAX)
+            k_coord_force_warp<T><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, (T)(1.0 / d.r0), d.n, d.m,
+                c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F);
+        else
         k_coord_force<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
                                                           pb, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
                                                           d_dVds + c->coord_dim, (T *)d_F);

@@ -208,6 +208,58 @@ k_build_list(int N, const typename Vec4<T>::type *__restrict__ spos, const int *
     nl_count[s] = cnt;
 }
 
+// Warp per atom (systems too small to fill the GPU with one thread per atom: BASELINE.json configs[0]-[2]): the lanes
+// share the candidates of each run of cells, a ballot keeps the accepted ones in candidate order (deterministic list).
+// A row's three cells are one contiguous run of the cell-sorted order unless the row wraps in x.
+template <typename T>
+__global__ void __launch_bounds__(128)
+k_build_list_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ scell,
+                  const int *__restrict__ cell_start, CellGrid g, PBox<T> pb, BoxD bd, T rc2T, double rc2, int maxn,
+                  int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky) {
+    const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (s >= N) return;
+    const typename Vec4<T>::type pi = spos[s];
+    const int c = scell[s];
+    const int ia = c % g.nc[0], t = c / g.nc[0];
+    const int ib = t % g.nc[1], ic = t / g.nc[1];
+    const int zb0 = g.nc[1] >= 3 ? -1 : 0, zb1 = g.nc[1] >= 2 ? 1 : 0;
+    const int zc0 = g.nc[2] >= 3 ? -1 : 0, zc1 = g.nc[2] >= 2 ? 1 : 0;
+    // runs along x: [first cell, last cell] pairs, in the visiting order of the thread-per-atom kernel (-1, 0, +1)
+    int ra[3], rb[3], nr = 0;
+    if (g.nc[0] >= 3) {
+        if (ia == 0) { ra[nr] = g.nc[0] - 1; rb[nr++] = g.nc[0] - 1; ra[nr] = 0; rb[nr++] = 1; }
+        else if (ia == g.nc[0] - 1) { ra[nr] = ia - 1; rb[nr++] = ia; ra[nr] = 0; rb[nr++] = 0; }
+        else { ra[nr] = ia - 1; rb[nr++] = ia + 1; }
+    } else if (g.nc[0] == 2) { ra[nr] = ia; rb[nr++] = ia; ra[nr] = 1 - ia; rb[nr++] = 1 - ia; }
+    else { ra[nr] = 0; rb[nr++] = 0; }
+    int cnt = 0;
+    for (int oc = zc0; oc <= zc1; ++oc) {
+        int jc = ic + oc; jc += jc < 0 ? g.nc[2] : 0; jc -= jc >= g.nc[2] ? g.nc[2] : 0;
+        for (int ob = zb0; ob <= zb1; ++ob) {
+            int jb = ib + ob; jb += jb < 0 ? g.nc[1] : 0; jb -= jb >= g.nc[1] ? g.nc[1] : 0;
+            const int rowbase = (jc * g.nc[1] + jb) * g.nc[0];
+            for (int r = 0; r < nr; ++r) {
+                const int cb = cell_start[rowbase + ra[r]], ce = cell_start[rowbase + rb[r] + 1];
+                for (int j0 = cb; j0 < ce; j0 += 32) {
+                    const int j = j0 + lane;
+                    bool hit = false;
+                    if (j < ce && j != s) hit = pair_in_range<T>(pb, bd, rc2T, rc2, pi, spos[j]);
+                    const unsigned m = __ballot_sync(0xffffffffu, hit);
+                    if (hit) {
+                        const int k = cnt + __popc(m & ((1u << lane) - 1u));
+                        if (k < maxn) nl[(size_t)k * N + s] = j;
+                    }
+                    cnt += __popc(m);
+                }
+            }
+        }
+    }
+    if (lane == 0) {
+        if (cnt > maxn) { atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW); cnt = maxn; }
+        nl_count[s] = cnt;
+    }
+}
+
 __global__ void k_export_list(int N, int maxn, const int *__restrict__ perm, const int *__restrict__ nl_count,
                               const int *__restrict__ nl, int *__restrict__ out_count, int *__restrict__ out_list) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -263,6 +315,11 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
         return r;
     }
     PBox<T> pb = make_pbox<T>(c->boxd);
+    if (N <= METAD_WARP_PER_ATOM_MAX)
+        k_build_list_warp<T><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start,
+                                                                             c->grid, pb, c->boxd, (T)c->rc2, c->rc2, c->maxn,
+                                                                             c->d_nl_count, c->d_nl, c->d_sticky);
+    else
     k_build_list<T><<<div_up(N, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start, c->grid, pb,
                                                    c->boxd, (T)c->rc2, c->rc2, c->maxn, c->d_nl_count, c->d_nl,
                                                    c->d_sticky);
