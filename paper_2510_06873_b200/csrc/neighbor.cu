@@ -211,13 +211,17 @@ k_build_list(int N, const typename Vec4<T>::type *__restrict__ spos, const int *
 // Warp per atom (systems too small to fill the GPU with one thread per atom: BASELINE.json configs[0]-[2]): the lanes
 // share the candidates of each run of cells, a ballot keeps the accepted ones in candidate order (deterministic list).
 // A row's three cells are one contiguous run of the cell-sorted order unless the row wraps in x.
-template <typename T>
+template <typename T, int G>
 __global__ void __launch_bounds__(128)
 k_build_list_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ scell,
                   const int *__restrict__ cell_start, CellGrid g, PBox<T> pb, BoxD bd, T rc2T, double rc2, int maxn,
                   int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky) {
-    const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    // G lanes per atom (G = 32: one warp per atom; G = 8: four atoms per warp, each group votes under its own mask)
+    const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = gt / G, lane = gt % G;
     if (s >= N) return;
+    const unsigned gmask = G == 32 ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
+    const int gshift = (threadIdx.x & 31) / G * G;
     const typename Vec4<T>::type pi = spos[s];
     const int c = scell[s];
     const int ia = c % g.nc[0], t = c / g.nc[0];
@@ -240,11 +244,11 @@ k_build_list_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const 
             const int rowbase = (jc * g.nc[1] + jb) * g.nc[0];
             for (int r = 0; r < nr; ++r) {
                 const int cb = cell_start[rowbase + ra[r]], ce = cell_start[rowbase + rb[r] + 1];
-                for (int j0 = cb; j0 < ce; j0 += 32) {
+                for (int j0 = cb; j0 < ce; j0 += G) {
                     const int j = j0 + lane;
                     bool hit = false;
                     if (j < ce && j != s) hit = pair_in_range<T>(pb, bd, rc2T, rc2, pi, spos[j]);
-                    const unsigned m = __ballot_sync(0xffffffffu, hit);
+                    const unsigned m = (__ballot_sync(gmask, hit) & gmask) >> gshift;
                     if (hit) {
                         const int k = cnt + __popc(m & ((1u << lane) - 1u));
                         if (k < maxn) nl[(size_t)k * N + s] = j;
@@ -316,9 +320,13 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     }
     PBox<T> pb = make_pbox<T>(c->boxd);
     if (N <= METAD_WARP_PER_ATOM_MAX)
-        k_build_list_warp<T><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start,
-                                                                             c->grid, pb, c->boxd, (T)c->rc2, c->rc2, c->maxn,
-                                                                             c->d_nl_count, c->d_nl, c->d_sticky);
+        k_build_list_warp<T, 32><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start,
+                                                                                 c->grid, pb, c->boxd, (T)c->rc2, c->rc2, c->maxn,
+                                                                                 c->d_nl_count, c->d_nl, c->d_sticky);
+    else if (N <= 8 * METAD_WARP_PER_ATOM_MAX)
+        k_build_list_warp<T, 8><<<div_up((long long)N * 8, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start,
+                                                                               c->grid, pb, c->boxd, (T)c->rc2, c->rc2, c->maxn,
+                                                                               c->d_nl_count, c->d_nl, c->d_sticky);
     else
     k_build_list<T><<<div_up(N, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start, c->grid, pb,
                                                    c->boxd, (T)c->rc2, c->rc2, c->maxn, c->d_nl_count, c->d_nl,
