@@ -203,6 +203,8 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     int aux0[4] = { 0, -1, 0, 0 };
     CUDA_TRY(cudaMemcpy(c->d_aux, aux0, sizeof(aux0), cudaMemcpyHostToDevice));
     for (int k = 0; k < 3; ++k) CUDA_TRY(cudaEventCreate(&c->ev[k]));
+    CUDA_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
     CUDA_TRY(cudaDeviceSynchronize());
     *out = c;
     return METAD_OK;
@@ -213,6 +215,8 @@ extern "C" int metad_destroy(metad_ctx *c) {
     cudaStreamSynchronize(c->stream);
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     for (int k = 0; k < 3; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+    if (c->ev_copy) cudaEventDestroy(c->ev_copy);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
@@ -370,10 +374,18 @@ extern "C" int metad_step_host(metad_ctx *c, const void *h_pos, const double *h_
                                double *h_cv, double *h_V) {
     if (!c || !h_pos || !h_F || !h_box) FAIL(METAD_ERR_ARG, "null argument");
     const size_t bytes = 3 * (size_t)c->N * (c->prec == 32 ? sizeof(float) : sizeof(double));
+    // positions first; the caller's forces travel on a second stream while the neighbour build, the CVs and the bias
+    // run (they are not needed before apply_forces)
     CUDA_TRY(cudaMemcpyAsync(c->d_pos_stage, h_pos, bytes, cudaMemcpyHostToDevice, c->stream));
-    CUDA_TRY(cudaMemcpyAsync(c->d_F_stage, h_F, bytes, cudaMemcpyHostToDevice, c->stream));
-    int r = metad_run(c, c->d_pos_stage, h_box, rc, c->d_F_stage, 1);
-    if (r) return r;
+    CUDA_TRY(cudaMemcpyAsync(c->d_F_stage, h_F, bytes, cudaMemcpyHostToDevice, c->copy_stream));
+    CUDA_TRY(cudaEventRecord(c->ev_copy, c->copy_stream));
+    int r;
+    if ((r = metad_build_neighbors(c, c->d_pos_stage, h_box, rc))) return r;
+    if ((r = metad_eval_cv(c, c->d_cv))) return r;
+    if ((r = metad_bias(c, c->d_cv, c->d_V, c->d_dVds))) return r;
+    CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_copy, 0));
+    if ((r = metad_apply_forces(c, c->d_dVds, c->d_F_stage))) return r;
+    if ((r = metad_deposit(c, c->d_cv, c->d_V))) return r;
     CUDA_TRY(cudaMemcpyAsync(h_F, c->d_F_stage, bytes, cudaMemcpyDeviceToHost, c->stream));
     if (h_cv) CUDA_TRY(cudaMemcpyAsync(h_cv, c->d_cv, sizeof(double) * c->D, cudaMemcpyDeviceToHost, c->stream));
     if (h_V) CUDA_TRY(cudaMemcpyAsync(h_V, c->d_V, sizeof(double), cudaMemcpyDeviceToHost, c->stream));

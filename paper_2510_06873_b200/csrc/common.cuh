@@ -172,6 +172,7 @@ struct metad_ctx {
     // shared-memory tiled fast path (fp32, Q6): tile.cuh / tiled.cu
     int tiled; int tile_T[3]; int tile_cap;
     int timing; int capturing; cudaEvent_t ev[3];
+    cudaStream_t copy_stream; cudaEvent_t ev_copy;   // metad_step_host: the force upload overlaps the first three stages
     float *d_q6;                          // tiled path: per-atom q6 (sorted order)
     double *d_cvq6;                       // tiled path: [Q6 mean, solid count] finished by k_tile_build
 };

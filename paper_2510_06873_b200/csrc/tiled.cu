@@ -24,6 +24,125 @@ __device__ __forceinline__ float4 hpos(const TileGeom &g, const TileTables &t, c
 }
 
 // ------------------------------------------------------------------------------------------------
+// Candidate scan of own atom a into list column `col`: every halo atom of the 3 x 3 row-runs around the atom's cell with
+// r^2 < rc^2 (1 + 1e-5) (tile-local coordinates, no per-pair minimum image).  Returns the number of candidates kept.
+template <bool STAGED>
+__device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos,
+                                         const float4 *pos_s, nl16_t *list_s, const int *__restrict__ scell, int a, int col,
+                                         float rc2_hi, bool &ovf) {
+    const int q = tile_own_row(t, a);
+    const int o = a - t.own_off[q];
+    const int li = t.own_l[q] + o, s = t.own_g[q] + o;
+    const float4 pi = hpos<STAGED>(g, t, spos, pos_s, li);
+    const int ic = scell[s] % g.nc0 - t.x0 + 1;          // halo-cell column of the own atom
+    const int r0 = t.own_row[q], rstride = t.Tye + 2;
+    // candidate list written through 32-bit shared-memory addresses (generic 64-bit pointer bumps cost 4 extra
+    // instructions per candidate): slot k of this column lives at w0 + k * STRIDE
+    const unsigned STRIDE = TILE_THREADS * (unsigned)sizeof(nl16_t);
+    const unsigned w0 = (unsigned)__cvta_generic_to_shared(list_s + col);
+    unsigned wp = w0;
+    const unsigned wend = w0 + (LIST_CAP - 1) * STRIDE;
+#pragma unroll 1
+    for (int dz = -1; dz <= 1; ++dz) {
+#pragma unroll 1
+        for (int dy = -1; dy <= 1; ++dy) {
+            const int r = r0 + dz * rstride + dy;
+            int lo = t.hcell[r][ic - 1];
+            const int hi = t.hcell[r][ic + 2];
+            while (lo < hi) {
+                // every candidate is stored unconditionally and the slot kept only if it passes (load, 6 flop, store,
+                // compare, bump): one free slot is needed, capacity is checked once per stretch
+                const int room = (int)((wend - wp) / STRIDE);
+                if (room <= 0) { ovf = true; break; }
+                const int h2 = min(hi, lo + room);
+#pragma unroll 4
+                for (int lj = lo; lj < h2; ++lj) {
+                    const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj);
+                    const float dx = pj.x - pi.x, dy2 = pj.y - pi.y, dz2 = pj.z - pi.z;
+                    const float r2 = dx * dx + dy2 * dy2 + dz2 * dz2;
+                    asm volatile("st.shared.u16 [%0], %1;" ::"r"(wp), "h"((unsigned short)lj));
+                    wp += (r2 < rc2_hi) ? STRIDE : 0u;
+                }
+                lo = h2;
+            }
+        }
+    }
+    return (int)((wp - w0) / STRIDE);
+}
+
+// Exact decision on the short list of own atom a (list column `col`, cnt candidates), neighbour-list write, fused q6m
+// accumulation and the atom's q6 record.  Returns q6.
+template <bool STAGED, bool WITH_Q6>
+__device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos,
+                                             const float4 *pos_s, const nl16_t *list_s, int a, int col, int cnt, bool ovf,
+                                             const BoxD &bd, float rc2f, float rc2_lo, double rc2, int maxn,
+                                             int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
+                                             float q_thresh, float inv_width, float *__restrict__ rec,
+                                             float *__restrict__ q6_out, bool solid) {
+    const int q = tile_own_row(t, a);
+    const int o = a - t.own_off[q];
+    const int li = t.own_l[q] + o, s = t.own_g[q] + o;
+    const float4 pi = hpos<STAGED>(g, t, spos, pos_s, li);
+    const nl16_t *myl = list_s + col;
+    if (ovf) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
+    int *out = nl + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
+    float A[13];
+#pragma unroll
+    for (int k = 0; k < 13; ++k) A[k] = 0.f;
+    int n = 0;
+    for (int k = 0; k < cnt; ++k) {
+        const int lj = myl[k * TILE_THREADS];
+        if (lj == li) continue;
+        const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj);
+        const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+        const float r2 = dx * dx + dy * dy + dz * dz;
+        bool in = r2 < rc2f;
+        if (r2 >= rc2_lo) {                                // borderline: canonical fp64 predicate on the inputs
+            const float4 gi = spos[s], gj = spos[__float_as_int(pj.w) & NL_IDX_MASK];
+            in = r2_canonical(bd, (double)gj.x - (double)gi.x, (double)gj.y - (double)gi.y,
+                              (double)gj.z - (double)gi.z) < rc2;
+        }
+        if (!in) continue;
+        if (n < maxn) {
+            out[n * 32] = __float_as_int(pj.w);
+            if (WITH_Q6) {
+                const float rinv = rsqrtf(r2);
+                Y6<float> y;
+                y6_eval<float>(dx * rinv, dy * rinv, dz * rinv, y);
+                A[0] += y.E[0];
+#pragma unroll
+                for (int m = 1; m <= 6; ++m) { A[2 * m - 1] += y.E[m] * y.c[m]; A[2 * m] += y.E[m] * y.s[m]; }
+            }
+        }
+        ++n;
+    }
+    if (n > maxn) { atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW); n = maxn; }
+    nl_count[s] = n;
+    float q6 = 0.f;
+    if (WITH_Q6) {
+        float S = 0.f;
+#pragma unroll
+        for (int k = 0; k < 13; ++k) S += A[k] * A[k];
+        float norm = 0.f;
+        if (n > 0 && S > 0.f) { float rs = sqrtf(S); q6 = rs / (float)n; norm = 1.f / ((float)n * rs); }
+        float4 *r4 = reinterpret_cast<float4 *>(rec + (size_t)s * METAD_NREC);
+        r4[0] = make_float4(A[0] * norm, A[1] * norm, -A[2] * norm, A[3] * norm);
+        r4[1] = make_float4(-A[4] * norm, A[5] * norm, -A[6] * norm, A[7] * norm);
+        r4[2] = make_float4(-A[8] * norm, A[9] * norm, -A[10] * norm, A[11] * norm);
+        if (solid) {
+            const float f = 1.f / (1.f + expf(-(q6 - q_thresh) * inv_width));
+            r4[3] = make_float4(-A[12] * norm, f * (1.f - f) * inv_width, q6, 0.f);
+        } else {                                          // Q6 mean only: the record carries the atom's own (global,
+            const float4 gp = spos[s];                    // exact fp32) position, so the force pass needs no second gather
+            r4[3] = make_float4(-A[12] * norm, gp.x, gp.y, gp.z);
+        }
+        q6_out[s] = q6;
+    }
+    return q6;
+}
+
+// One thread per own atom: scan, then the exact pass.  (Re-dealing the atoms to the threads by candidate count between the
+// two passes, so that the lanes of a warp run equal trip counts, was measured and dropped: profiles/r1h_rejected.md.)
 template <bool STAGED, bool WITH_Q6>
 __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos,
                                            const float4 *pos_s, nl16_t *list_s, const int *__restrict__ scell,
@@ -32,101 +151,15 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
                                            float inv_width, float *__restrict__ rec, float *__restrict__ q6_out, bool solid,
                                            double (&v)[2]) {
     const float rc2_hi = rc2f * (1.f + 1e-5f), rc2_lo = rc2f * (1.f - 1e-5f);
-    nl16_t *myl = list_s + threadIdx.x;
-    for (int a = threadIdx.x; a < t.nown; a += blockDim.x) {
-        const int q = tile_own_row(t, a);
-        const int o = a - t.own_off[q];
-        const int li = t.own_l[q] + o, s = t.own_g[q] + o;
-        const float4 pi = hpos<STAGED>(g, t, spos, pos_s, li);
-        const int ic = scell[s] % g.nc0 - t.x0 + 1;          // halo-cell column of the own atom
-        const int r0 = t.own_row[q], rstride = t.Tye + 2;
-        // candidate list written through 32-bit shared-memory addresses (generic 64-bit pointer bumps cost 4 extra
-        // instructions per candidate): slot k of this thread lives at w0 + k * STRIDE
-        const unsigned STRIDE = TILE_THREADS * (unsigned)sizeof(nl16_t);
-        const unsigned w0 = (unsigned)__cvta_generic_to_shared(myl);
-        unsigned wp = w0;
-        const unsigned wend = w0 + (LIST_CAP - 1) * STRIDE;
+    const int tid = threadIdx.x;
+    for (int a = tid; a < t.nown; a += blockDim.x) {
         bool ovf = false;
-#pragma unroll 1
-        for (int dz = -1; dz <= 1; ++dz) {
-#pragma unroll 1
-            for (int dy = -1; dy <= 1; ++dy) {
-                const int r = r0 + dz * rstride + dy;
-                int lo = t.hcell[r][ic - 1];
-                const int hi = t.hcell[r][ic + 2];
-                while (lo < hi) {
-                    // every candidate is stored unconditionally and the slot kept only if it passes (load, 6 flop, store,
-                    // compare, bump): one free slot is needed, capacity is checked once per stretch
-                    const int room = (int)((wend - wp) / STRIDE);
-                    if (room <= 0) { ovf = true; break; }
-                    const int h2 = min(hi, lo + room);
-#pragma unroll 4
-                    for (int lj = lo; lj < h2; ++lj) {
-                        const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj);
-                        const float dx = pj.x - pi.x, dy2 = pj.y - pi.y, dz2 = pj.z - pi.z;
-                        const float r2 = dx * dx + dy2 * dy2 + dz2 * dz2;
-                        asm volatile("st.shared.u16 [%0], %1;" ::"r"(wp), "h"((unsigned short)lj));
-                        wp += (r2 < rc2_hi) ? STRIDE : 0u;
-                    }
-                    lo = h2;
-                }
-            }
-        }
-        const int cnt = (int)((wp - w0) / STRIDE);
-        if (ovf) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
-        // exact decision on the short list; neighbour-list write; fused q6m accumulation
-        int *out = nl + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
-        float A[13];
-#pragma unroll
-        for (int k = 0; k < 13; ++k) A[k] = 0.f;
-        int n = 0;
-        for (int k = 0; k < cnt; ++k) {
-            const int lj = myl[k * TILE_THREADS];
-            if (lj == li) continue;
-            const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj);
-            const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-            const float r2 = dx * dx + dy * dy + dz * dz;
-            bool in = r2 < rc2f;
-            if (r2 >= rc2_lo) {                                // borderline: canonical fp64 predicate on the inputs
-                const float4 gi = spos[s], gj = spos[__float_as_int(pj.w) & NL_IDX_MASK];
-                in = r2_canonical(bd, (double)gj.x - (double)gi.x, (double)gj.y - (double)gi.y,
-                                  (double)gj.z - (double)gi.z) < rc2;
-            }
-            if (!in) continue;
-            if (n < maxn) {
-                out[n * 32] = __float_as_int(pj.w);
-                if (WITH_Q6) {
-                    const float rinv = rsqrtf(r2);
-                    Y6<float> y;
-                    y6_eval<float>(dx * rinv, dy * rinv, dz * rinv, y);
-                    A[0] += y.E[0];
-#pragma unroll
-                    for (int m = 1; m <= 6; ++m) { A[2 * m - 1] += y.E[m] * y.c[m]; A[2 * m] += y.E[m] * y.s[m]; }
-                }
-            }
-            ++n;
-        }
-        if (n > maxn) { atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW); n = maxn; }
-        nl_count[s] = n;
+        const int cnt = scan_atom<STAGED>(g, t, spos, pos_s, list_s, scell, a, tid, rc2_hi, ovf);
+        const float q6 = finish_atom<STAGED, WITH_Q6>(g, t, spos, pos_s, list_s, a, tid, cnt, ovf, bd, rc2f, rc2_lo, rc2, maxn,
+                                                      nl_count, nl, sticky, q_thresh, inv_width, rec, q6_out, solid);
         if (WITH_Q6) {
-            float S = 0.f;
-#pragma unroll
-            for (int k = 0; k < 13; ++k) S += A[k] * A[k];
-            float q6 = 0.f, norm = 0.f;
-            if (n > 0 && S > 0.f) { float rs = sqrtf(S); q6 = rs / (float)n; norm = 1.f / ((float)n * rs); }
-            const float f = 1.f / (1.f + expf(-(q6 - q_thresh) * inv_width));
-            float4 *r4 = reinterpret_cast<float4 *>(rec + (size_t)s * METAD_NREC);
-            r4[0] = make_float4(A[0] * norm, A[1] * norm, -A[2] * norm, A[3] * norm);
-            r4[1] = make_float4(-A[4] * norm, A[5] * norm, -A[6] * norm, A[7] * norm);
-            r4[2] = make_float4(-A[8] * norm, A[9] * norm, -A[10] * norm, A[11] * norm);
-            if (solid) {
-                r4[3] = make_float4(-A[12] * norm, f * (1.f - f) * inv_width, q6, 0.f);
-            } else {                                          // Q6 mean only: the record carries the atom's own (global,
-                const float4 gp = spos[s];                    // exact fp32) position, so the force pass needs no second gather
-                r4[3] = make_float4(-A[12] * norm, gp.x, gp.y, gp.z);
-            }
-            q6_out[s] = q6;
-            v[0] += (double)q6; v[1] += (double)f;
+            v[0] += (double)q6;
+            v[1] += (double)(1.f / (1.f + expf(-(q6 - q_thresh) * inv_width)));
         }
     }
 }
