@@ -70,6 +70,8 @@ def lib():
         L.orc_bias_periodic.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P, _P]
         L.orc_grid_add_p.argtypes = [_I, _I, _P, _P, _P, _I, _I, _P, _P, _P, _P]
         L.orc_reweight.argtypes = [_I, _I, _P, _I, _P, _P, _P, _P, _D, _P, _P, _P, _P, _P]
+        L.orc_cv_mindist.restype = _D
+        L.orc_cv_mindist.argtypes = [_I, _P, _P, _P, _P, _I, _P, _D, _P, _P]
         L.orc_grid_eval_p.restype = _I
         L.orc_grid_eval_p.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P, _P]
         _lib = L
@@ -304,3 +306,14 @@ def reweight(traj, centers, heights, sigma, period, kT, nbins, lo, hi):
     lib().orc_reweight(D, len(traj), _p(traj), len(heights), _p(centers), _p(heights), _p(sigma), _p(period), float(kT),
                        _p(nb), _p(lo2), _p(hi2), _p(P), _p(F))
     return P, F
+
+
+# ---- NEXT-2b: distance to the nearest atom of a group (reading AA)
+def cv_mindist(pos, box, count, lst, rc, flags=None, want_grad=True):
+    """Returns (s, grad (N,3) or None, (i, j) of the nearest pair or (-1, -1))."""
+    pos, box = _f(pos), _f(box)
+    N = len(pos)
+    grad = np.zeros((N, 3)) if want_grad else None
+    pair = np.zeros(2, dtype=np.int32)
+    s = lib().orc_cv_mindist(N, _p(pos), _p(box), _p(count), _p(lst), lst.shape[1], _p(flags), float(rc), _p(grad), _p(pair))
+    return s, grad, (int(pair[0]), int(pair[1]))

@@ -768,3 +768,39 @@ void orc_reweight(int D, int T, const double *traj, int H, const double *centers
         F[b] = P[b] > 0.0 ? -kT * log(P[b]) : INFINITY;
     }
 }
+
+/* =============================================================================================
+ * NEXT-2b: the paper's second workload biases "the distance between a surface
+ * oxygen atom and its nearest hydrogen atom".  Reading AA: s = min over i in A,
+ * j in B, j != i, r_ij < rc of the minimum-image distance r_ij (A = the surface oxygen(s), B = the
+ * hydrogens); the paper obtains forces by automatic differentiation, and the
+ * derivative of a minimum is the derivative of its arg-min: d s/d r_j = d/r, d s/d r_i = -d/r for
+ * the nearest pair (i, j), zero for every other atom.  Ties: the pair with the smallest (i, j) in
+ * lexicographic order.  No pair within rc: s = rc, zero gradient.  The neighbour list (r < rc)
+ * restricts the search exactly as in orc_cv_coord.  pair_out[2] (may be NULL) receives (i, j) or (-1,-1). */
+double orc_cv_mindist(int N, const double *pos, const double *box, const int *count, const int *list,
+                      int maxn, const unsigned char *flags, double rc, double *grad, int *pair_out) {
+    double best = INFINITY, bd[3] = { 0, 0, 0 };
+    int bi = -1, bj = -1;
+    if (grad) memset(grad, 0, sizeof(double) * 3 * (size_t)N);
+    for (int i = 0; i < N; ++i) {
+        if (flags && !(flags[i] & 1)) continue;
+        int c = count[i] < maxn ? count[i] : maxn;
+        for (int k = 0; k < c; ++k) {
+            int j = list[(size_t)i * maxn + k];
+            if (flags && !(flags[j] & 2)) continue;
+            double d[3];
+            orc_delta(box, pos + 3 * i, pos + 3 * j, d);
+            double r2 = r2_of(d);
+            if (r2 < best || (r2 == best && (i < bi || (i == bi && j < bj)))) {
+                best = r2; bi = i; bj = j; bd[0] = d[0]; bd[1] = d[1]; bd[2] = d[2];
+            }
+        }
+    }
+    if (pair_out) { pair_out[0] = bi; pair_out[1] = bj; }
+    if (bi < 0) return rc;
+    double r = sqrt(best);
+    if (grad)
+        for (int a = 0; a < 3; ++a) { grad[3 * bj + a] += bd[a] / r; grad[3 * bi + a] -= bd[a] / r; }
+    return r;
+}

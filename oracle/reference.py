@@ -7,11 +7,11 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import (apply_forces, bias, bias_periodic, cv_contacts, cv_coord, cv_rgyr, cv_torsion, grid_add, grid_add_p,
+from . import (apply_forces, bias, bias_periodic, cv_contacts, cv_coord, cv_mindist, cv_rgyr, cv_torsion, grid_add, grid_add_p,
                grid_eval, grid_eval_p, make_flags, neighbors, q6_atoms, q6_grad, wt_height)
 
 # CV kinds — restated (not imported) so the oracle depends on nothing of the product.
-COORD, Q6_MEAN, Q6_SOLID, RGYR, CONTACTS, TORSION = 0, 1, 2, 3, 4, 5
+COORD, Q6_MEAN, Q6_SOLID, RGYR, CONTACTS, TORSION, MINDIST = 0, 1, 2, 3, 4, 5, 6
 
 
 def logistic(q, q0, width):
@@ -73,6 +73,9 @@ class OracleMetaD:
                     np.add.at(g, np.asarray(cv.chain), gc)
             elif cv.kind == CONTACTS:
                 s[d], g = cv_contacts(pos, box, cv.pairs, cv.pair_r0, cv.n, cv.m, cv.scale, want_grad)
+            elif cv.kind == MINDIST:
+                fl = make_flags(self.N, cv.group_a, cv.group_b)
+                s[d], g, self.min_pair = cv_mindist(pos, box, self.count, self.list, w.rc, fl, want_grad)
             elif cv.kind == TORSION:
                 s[d], g4 = cv_torsion(pos, box, cv.atoms, want_grad)
                 g = None
