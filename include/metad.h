@@ -52,6 +52,11 @@ enum metad_cv_kind {
     METAD_CV_RGYR = 3,     /* radius of gyration of an ordered chain, unwrapped by sequential minimum
                               image (BASELINE.json configs[1]; reading G)                                  */
     METAD_CV_CONTACTS = 4, /* s = scale * sum_p sw(r_p / r0_p), n, m as given (configs[1]; reading H)      */
+    METAD_CV_MINDIST = 6,  /* s = min over i in A, j in B, j != i, r_ij < rc of the minimum-image distance; forces act on the
+                              nearest pair only (the derivative of a minimum is that of its arg-min, which is what automatic
+                              differentiation returns); nobody within rc: s = rc, no force
+                              ("distance between a surface oxygen atom and its nearest hydrogen atom"; reading AA).
+                              Groups as for COORD; at most one COORD or MINDIST CV per context                              */
     METAD_CV_TORSION = 5   /* dihedral angle of atoms torsion[0..3] in (-pi, pi], IUPAC sign, minimum-image bonds
                               ("Phi(C-N-Ca-C) and Psi(N-Ca-C-N) serve as the CVs"; reading V).
                               Normally used with params.period = 2 pi for that dimension                  */
@@ -62,7 +67,7 @@ typedef struct {
     int n, m;                       /* switching exponents (COORD, CONTACTS) */
     double r0;                      /* switching length (COORD) */
     double scale;                   /* normalisation, see metad_cv_kind */
-    const int *group_a; int n_a;    /* COORD: host index lists; NULL = all atoms */
+    const int *group_a; int n_a;    /* COORD, MINDIST: host index lists; NULL = all atoms */
     const int *group_b; int n_b;
     const int *pairs;               /* CONTACTS: host int[2*npairs] */
     const double *pair_r0;          /* CONTACTS: host double[npairs] */

@@ -58,7 +58,7 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     if (c->p.force_scale == 0.0) c->p.force_scale = 1.0;
     c->stream = (cudaStream_t)cuda_stream;
     if (!c->stream) CUDA_TRY(cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking));
-    c->q6_mean_dim = c->q6_solid_dim = c->coord_dim = -1;
+    c->q6_mean_dim = c->q6_solid_dim = c->coord_dim = c->mindist_dim = -1;
     const int N = c->N;
     const size_t tsz = c->prec == 32 ? sizeof(float) : sizeof(double);
 
@@ -70,10 +70,15 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
         v.kind = s.kind; v.n = s.n; v.m = s.m; v.r0 = s.r0; v.scale = s.scale;
         v.q_thresh = s.q_thresh; v.q_width = s.q_width;
         switch (s.kind) {
-        case METAD_CV_COORD: {
-            if (c->coord_dim >= 0) FAIL(METAD_ERR_ARG, "only one COORD CV per context");
-            if (!(s.r0 > 0.0) || s.n < 1 || s.m <= s.n) FAIL(METAD_ERR_ARG, "COORD needs r0 > 0, 0 < n < m");
-            c->coord_dim = d; c->has_coord = true;
+        case METAD_CV_COORD:
+        case METAD_CV_MINDIST: {
+            if (c->coord_dim >= 0 || c->mindist_dim >= 0) FAIL(METAD_ERR_ARG, "only one COORD or MINDIST CV per context");
+            if (s.kind == METAD_CV_COORD) {
+                if (!(s.r0 > 0.0) || s.n < 1 || s.m <= s.n) FAIL(METAD_ERR_ARG, "COORD needs r0 > 0, 0 < n < m");
+                c->coord_dim = d; c->has_coord = true;
+            } else {
+                c->mindist_dim = d; c->has_mindist = true;
+            }
             v.use_groups = s.group_a || s.group_b;
             if (v.use_groups) {
                 flags.assign(N, 0);
@@ -136,6 +141,7 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
         }
     }
 
+    if (c->has_mindist) CUDA_TRY(dev_alloc(&c->d_mind, 8));
     if (c->has_torsion) {
         std::vector<int> ta;
         for (int d = 0; d < c->D; ++d)
@@ -220,7 +226,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
@@ -270,7 +276,7 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
     // shared-memory tiled fast path: fp32, neighbour-list CVs = Q6 only, >= 3 cells per direction
     c->tiled = 0;
     const char *env = getenv("METAD_NO_TILES");
-    if (c->prec == 32 && c->has_q6 && !c->has_coord && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32 &&
+    if (c->prec == 32 && c->has_q6 && !c->has_coord && !c->has_mindist && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32 &&
         !(env && env[0] == '1')) {
         const double rho = (double)c->N / g.ncell, margin = 1.3;
         const int cap = 1216;

@@ -428,6 +428,129 @@ __global__ void k_q6_export_arr(int N, const int *__restrict__ perm, const float
 }
 
 // ------------------------------------------------------------------------------------------------
+// Distance to the nearest atom of a group (reading AA): arg-min over the neighbour list of (r^2, i, j) in
+// ORIGINAL indices (ties -> smallest pair), block partials + last-block pass.  The result record feeds the force kernel.
+struct MinKey { double r2; long long ij; };
+__device__ __forceinline__ bool min_less(double r2a, long long ija, double r2b, long long ijb) {
+    return r2a < r2b || (r2a == r2b && ija < ijb);
+}
+__device__ __forceinline__ void min_warp(double &r2, long long &ij, int &sj, int &si) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double r2o = __shfl_down_sync(0xffffffffu, r2, o);
+        const long long ijo = __shfl_down_sync(0xffffffffu, ij, o);
+        const int sjo = __shfl_down_sync(0xffffffffu, sj, o), sio = __shfl_down_sync(0xffffffffu, si, o);
+        if (min_less(r2o, ijo, r2, ij)) { r2 = r2o; ij = ijo; sj = sjo; si = sio; }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(CV_THREADS)
+k_mindist_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
+             const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, double rc,
+             double *__restrict__ part_r2, long long *__restrict__ part_ij, int *__restrict__ part_s /* [2*nblocks] */,
+             unsigned int *__restrict__ ticket, double *__restrict__ rec /* [r, dx, dy, dz, (i, j) as two ints] */,
+             double *__restrict__ cv_out) {
+    __shared__ double s_r2[32];
+    __shared__ long long s_ij[32];
+    __shared__ int s_sj[32], s_si[32];
+    const int s = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double r2 = 1e300; long long ij = 0x7fffffffffffffffll; int sj = -1, si = -1;
+    if (s < N) {
+        const typename Vec4<T>::type pi = spos[s];
+        if (((int)pi.w) & 1) {
+            const int cnt = nl_count[s];
+            const long long io = perm[s];
+            for (int k = 0; k < cnt; ++k) {
+                const int j = nl[(size_t)k * N + s];
+                const typename Vec4<T>::type pj = spos[j];
+                if (!(((int)pj.w) & 2)) continue;
+                T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+                min_image(pb, dx, dy, dz);
+                const double q = (double)(dx * dx + dy * dy + dz * dz);
+                const long long key = (io << 32) | (long long)perm[j];
+                if (min_less(q, key, r2, ij)) { r2 = q; ij = key; sj = j; si = s; }
+            }
+        }
+    }
+    min_warp(r2, ij, sj, si);
+    if (lane == 0) { s_r2[wid] = r2; s_ij[wid] = ij; s_sj[wid] = sj; s_si[wid] = si; }
+    __syncthreads();
+    if (wid == 0) {
+        const int nw = blockDim.x >> 5;
+        r2 = lane < nw ? s_r2[lane] : 1e300; ij = lane < nw ? s_ij[lane] : 0x7fffffffffffffffll;
+        sj = lane < nw ? s_sj[lane] : -1; si = lane < nw ? s_si[lane] : -1;
+        min_warp(r2, ij, sj, si);
+        if (lane == 0) { part_r2[blockIdx.x] = r2; part_ij[blockIdx.x] = ij; part_s[2 * blockIdx.x] = si; part_s[2 * blockIdx.x + 1] = sj; }
+    }
+    if (last_block_ticket(ticket)) {
+        r2 = 1e300; ij = 0x7fffffffffffffffll; sj = -1; si = -1;
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x)
+            if (min_less(part_r2[b], part_ij[b], r2, ij)) { r2 = part_r2[b]; ij = part_ij[b]; si = part_s[2 * b]; sj = part_s[2 * b + 1]; }
+        min_warp(r2, ij, sj, si);
+        if (lane == 0) { s_r2[wid] = r2; s_ij[wid] = ij; s_sj[wid] = sj; s_si[wid] = si; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < (int)(blockDim.x >> 5); ++w)
+                if (min_less(s_r2[w], s_ij[w], r2, ij)) { r2 = s_r2[w]; ij = s_ij[w]; sj = s_sj[w]; si = s_si[w]; }
+            int *pair = reinterpret_cast<int *>(rec + 4);
+            if (sj < 0) {                                   // nobody within rc: s = rc, no force
+                rec[0] = rc; rec[1] = rec[2] = rec[3] = 0.0; pair[0] = pair[1] = -1;
+                *cv_out = rc;
+            } else {
+                const typename Vec4<T>::type pi = spos[si], pj = spos[sj];
+                T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+                min_image(pb, dx, dy, dz);
+                const double r = sqrt((double)dx * (double)dx + (double)dy * (double)dy + (double)dz * (double)dz);
+                rec[0] = r; rec[1] = (double)dx; rec[2] = (double)dy; rec[3] = (double)dz;
+                pair[0] = (int)(ij >> 32); pair[1] = (int)(ij & 0xffffffffll);
+                *cv_out = r;
+            }
+        }
+    }
+}
+
+template <typename T>
+__global__ void k_mindist_force(const double *__restrict__ rec, double force_scale, const double *__restrict__ dVds,
+                                T *__restrict__ F) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int *pair = reinterpret_cast<const int *>(rec + 4);
+    if (pair[0] < 0) return;
+    // d s/d r_j = d/r, d s/d r_i = -d/r  ->  F_j += -fs dVds d/r, F_i += +fs dVds d/r
+    const double a = force_scale * dVds[0] / rec[0];
+    for (int k = 0; k < 3; ++k) {
+        F[3 * (size_t)pair[0] + k] += (T)(a * rec[1 + k]);
+        F[3 * (size_t)pair[1] + k] += (T)(-a * rec[1 + k]);
+    }
+}
+
+template <typename T>
+static int mindist_eval_t(metad_ctx *c, double *d_cv) {
+    typedef typename Vec4<T>::type V4;
+    const int nb = div_up(c->N, CV_THREADS);
+    double *pr = c->d_partials;
+    long long *pk = reinterpret_cast<long long *>(c->d_partials + c->nblocks_atoms);
+    int *ps = reinterpret_cast<int *>(c->d_partials + 2 * (size_t)c->nblocks_atoms);
+    k_mindist_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(c->N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, ctx_pbox<T>(c),
+                                                     c->rc, pr, pk, ps, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+int mindist_eval(metad_ctx *c, double *d_cv) {
+    if (!c->has_mindist) return METAD_OK;
+    return c->prec == 32 ? mindist_eval_t<float>(c, d_cv) : mindist_eval_t<double>(c, d_cv);
+}
+int mindist_forces(metad_ctx *c, const double *d_dVds, void *d_F) {
+    if (!c->has_mindist) return METAD_OK;
+    if (c->prec == 32) k_mindist_force<float><<<1, 32, 0, c->stream>>>(c->d_mind, c->p.force_scale, d_dVds + c->mindist_dim, (float *)d_F);
+    else k_mindist_force<double><<<1, 32, 0, c->stream>>>(c->d_mind, c->p.force_scale, d_dVds + c->mindist_dim, (double *)d_F);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
 int chain_eval(metad_ctx *c, int dim, const void *d_pos_unused, double *d_cv);          // cv_chain.cu
 int chain_forces(metad_ctx *c, const double *d_dVds, void *d_F);                         // cv_chain.cu
 
@@ -475,6 +598,8 @@ int cv_eval_all(metad_ctx *c, double *d_cv) {
         }
     rcode = torsion_eval_all(c, d_cv);
     if (rcode) return rcode;
+    rcode = mindist_eval(c, d_cv);
+    if (rcode) return rcode;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
 }
@@ -516,6 +641,8 @@ int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F) {
     rcode = chain_forces(c, d_dVds, d_F);
     if (rcode) return rcode;
     rcode = torsion_forces(c, d_dVds, d_F);
+    if (rcode) return rcode;
+    rcode = mindist_forces(c, d_dVds, d_F);
     if (rcode) return rcode;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

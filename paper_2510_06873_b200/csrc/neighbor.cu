@@ -309,7 +309,7 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     k_scan_apply<<<nsb, SCAN_THREADS, 0, st>>>(ncell, N, c->d_cell_count, c->d_block_sums, c->d_cell_start);
     k_scatter<<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_of, c->d_slot, c->d_cell_start, c->d_perm_raw);
     k_cell_sort_gather<T><<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_start, c->d_cell_of, c->d_perm_raw, c->d_perm, (const T *)d_pos,
-                                                             c->has_coord && c->cv[c->coord_dim].use_groups ? c->d_flags : nullptr,
+                                                             c->d_flags,   /* NULL unless a COORD / MINDIST CV has groups */
                                                              (V4 *)c->d_spos, c->d_scell);
     if (tm) cudaEventRecord(c->ev[1], st);
     if (c->tiled && sizeof(T) == 4) {

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmetad_b200.so")
 MAX_CV = 4
 OK, ERR_ARG, ERR_BOX, ERR_STATE, ERR_CUDA, ERR_NOMEM = range(6)
 DEV_NEIGH_OVERFLOW, DEV_HILL_OVERFLOW, DEV_GRID_RANGE, DEV_NONFINITE, DEV_POS_RANGE = 1, 2, 4, 8, 16
-CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION = range(6)
+CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CV_MINDIST = range(7)
 
 _P = ctypes.c_void_p
 _I = ctypes.c_int
