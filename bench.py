@@ -56,7 +56,10 @@ def describe(w, precision):
     return {"workload": wl, "atoms": int(w.natoms),
             "cvs": [kinds[c.kind] for c in w.cvs], "hills": int(w.n_hills), "rc": w.rc,
             "pair_precision": f"fp{precision}", "stride": int(w.stride),
-            "l2": "per-step working set (neighbour list + q6 records + positions + forces) exceeds the 126 MB L2; no flush"}
+            "l2": ("per-step working set (neighbour list + q6 records + positions + forces) exceeds the 126 MB L2; no flush"
+                   if w.natoms * (4 * w.max_neigh + 64 + 16 + 24 + 16) > 126e6 else
+                   "working set fits the 126 MB L2 and is not flushed: this workload is bound by the latency of its ~10 "
+                   "dependent kernel launches per step, not by memory")}
 
 
 # ------------------------------------------------------------------------------------------ clocks
