@@ -72,6 +72,8 @@ def lib():
         L.orc_reweight.argtypes = [_I, _I, _P, _I, _P, _P, _P, _P, _D, _P, _P, _P, _P, _P]
         L.orc_cv_mindist.restype = _D
         L.orc_cv_mindist.argtypes = [_I, _P, _P, _P, _P, _I, _P, _D, _P, _P]
+        L.orc_cv_lattice.restype = _D
+        L.orc_cv_lattice.argtypes = [_P, _I, _P]
         L.orc_grid_eval_p.restype = _I
         L.orc_grid_eval_p.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P, _P]
         _lib = L
@@ -317,3 +319,12 @@ def cv_mindist(pos, box, count, lst, rc, flags=None, want_grad=True):
     pair = np.zeros(2, dtype=np.int32)
     s = lib().orc_cv_mindist(N, _p(pos), _p(box), _p(count), _p(lst), lst.shape[1], _p(flags), float(rc), _p(grad), _p(pair))
     return s, grad, (int(pair[0]), int(pair[1]))
+
+
+# ---- NEXT-3: lattice-parameter CV (reading AB)
+def cv_lattice(box, axis):
+    """Returns (|h_axis|, d s / d box as (3,3))."""
+    box = _f(box)
+    g = np.zeros(9)
+    s = lib().orc_cv_lattice(_p(box), int(axis), _p(g))
+    return s, g.reshape(3, 3)

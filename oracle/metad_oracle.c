@@ -804,3 +804,20 @@ double orc_cv_mindist(int N, const double *pos, const double *box, const int *co
         for (int a = 0; a < 3; ++a) { grad[3 * bj + a] += bd[a] / r; grad[3 * bi + a] -= bd[a] / r; }
     return r;
 }
+
+/* =============================================================================================
+ * NEXT-3: "We selected the coordination number (C.N.) and the triaxial lattice
+ * parameters as CVs and ran NPT simulation".  Reading AB: the lattice parameter of
+ * axis k is the length of box row k, s = |h_k| (a, b, c of the supercell); it does not depend on
+ * the atomic positions, its gradient is taken with respect to the box matrix:
+ * d s/d h_k = h_k/|h_k| (row k of grad9, other rows zero).  The bias then acts on the cell:
+ * F_h = -force_scale * sum_d dV/ds_d * d s_d/d h (what an NPT integrator adds to its box force).   */
+double orc_cv_lattice(const double *box, int axis, double *grad9) {
+    const double *h = box + 3 * axis;
+    double s = sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
+    if (grad9) {
+        for (int k = 0; k < 9; ++k) grad9[k] = 0.0;
+        for (int a = 0; a < 3; ++a) grad9[3 * axis + a] = h[a] / s;
+    }
+    return s;
+}

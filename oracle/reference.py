@@ -7,11 +7,11 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import (apply_forces, bias, bias_periodic, cv_contacts, cv_coord, cv_mindist, cv_rgyr, cv_torsion, grid_add, grid_add_p,
+from . import (apply_forces, bias, bias_periodic, cv_contacts, cv_coord, cv_lattice, cv_mindist, cv_rgyr, cv_torsion, grid_add, grid_add_p,
                grid_eval, grid_eval_p, make_flags, neighbors, q6_atoms, q6_grad, wt_height)
 
 # CV kinds — restated (not imported) so the oracle depends on nothing of the product.
-COORD, Q6_MEAN, Q6_SOLID, RGYR, CONTACTS, TORSION, MINDIST = 0, 1, 2, 3, 4, 5, 6
+COORD, Q6_MEAN, Q6_SOLID, RGYR, CONTACTS, TORSION, MINDIST, LATTICE = 0, 1, 2, 3, 4, 5, 6, 7
 
 
 def logistic(q, q0, width):
@@ -49,6 +49,7 @@ class OracleMetaD:
         s = np.zeros(self.D)
         grads = np.zeros((self.D, self.N, 3)) if want_grad else None
         q6 = None
+        box_grads = np.zeros((self.D, 3, 3))          # d s_d / d box (lattice CVs only; reading AB)
         for d, cv in enumerate(w.cvs):
             if cv.kind == COORD:
                 fl = make_flags(self.N, cv.group_a, cv.group_b)
@@ -73,6 +74,9 @@ class OracleMetaD:
                     np.add.at(g, np.asarray(cv.chain), gc)
             elif cv.kind == CONTACTS:
                 s[d], g = cv_contacts(pos, box, cv.pairs, cv.pair_r0, cv.n, cv.m, cv.scale, want_grad)
+            elif cv.kind == LATTICE:
+                s[d], box_grads[d] = cv_lattice(box, cv.n)
+                g = np.zeros((self.N, 3)) if want_grad else None
             elif cv.kind == MINDIST:
                 fl = make_flags(self.N, cv.group_a, cv.group_b)
                 s[d], g, self.min_pair = cv_mindist(pos, box, self.count, self.list, w.rc, fl, want_grad)
@@ -87,6 +91,7 @@ class OracleMetaD:
             if want_grad:
                 grads[d] = g
         self.s, self.grads = s, grads
+        self.box_grads = box_grads
         return s
 
     # -- a5 / a5g
@@ -132,6 +137,10 @@ class OracleMetaD:
         if F is None:
             F = np.zeros((self.N, 3))
         return apply_forces(F, dVds, self.grads, force_scale)
+
+    def box_force(self, dVds, force_scale=1.0):
+        """F_h = -force_scale * sum_d dVds_d * d s_d / d h  (reading AB)."""
+        return -force_scale * np.tensordot(np.atleast_1d(dVds), self.box_grads, axes=1)
 
     # -- a7 (readings I, J, U): every `stride` steps append (s, w0*exp(-V/((gamma-1)kT)))
     def deposit(self, s, V):

@@ -23,7 +23,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = os.path.join(_HERE, "libmetad_inputs.so")
 
 # CV kinds (mirrors include/metad.h; plain integers, no arithmetic)
-CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CV_MINDIST = 0, 1, 2, 3, 4, 5, 6
+CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CV_MINDIST, CV_LATTICE = 0, 1, 2, 3, 4, 5, 6, 7
 
 
 def build_native(force: bool = False) -> str:
