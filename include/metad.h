@@ -57,6 +57,8 @@ enum metad_cv_kind {
                               differentiation returns); nobody within rc: s = rc, no force
                               ("distance between a surface oxygen atom and its nearest hydrogen atom"; reading AA).
                               Groups as for COORD; at most one COORD or MINDIST CV per context                              */
+    METAD_CV_LATTICE = 7,  /* s = |h_k|, the length of box row k = cv.n in {0, 1, 2} ("the triaxial lattice parameters as
+                              CVs"; reading AB).  No atomic forces: the bias acts on the cell, see metad_get_box_force          */
     METAD_CV_TORSION = 5   /* dihedral angle of atoms torsion[0..3] in (-pi, pi], IUPAC sign, minimum-image bonds
                               ("Phi(C-N-Ca-C) and Psi(N-Ca-C-N) serve as the CVs"; reading V).
                               Normally used with params.period = 2 pi for that dimension                  */
@@ -175,6 +177,11 @@ int metad_bias_batch(metad_ctx *ctx, const double *d_points, int npoints, double
  * run).  Not a per-step call: allocates and frees its scratch (V per frame, bins).  [sync] */
 int metad_reweight(metad_ctx *ctx, const double *d_traj, int nframes, const int *h_nbins, const double *h_lo,
                    const double *h_hi, double *d_P, double *d_F);
+
+/* Bias force on the cell for NPT integrators (reading AB): F_h[3][3] = -force_scale * sum_d dVds[d] * d s_d/d h
+ * of the last metad_apply_forces, h = the box rows; non-zero only for METAD_CV_LATTICE dimensions.  Copied to d_out9
+ * (device double[9]); enqueued, not synchronised. */
+int metad_get_box_force(metad_ctx *ctx, double *d_out9);
 
 /* Resets the step counter (hills stay). */
 int metad_reset_steps(metad_ctx *ctx);

@@ -128,6 +128,10 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
                 return METAD_ERR_CUDA;
             break;
         }
+        case METAD_CV_LATTICE:
+            if (s.n < 0 || s.n > 2) FAIL(METAD_ERR_ARG, "LATTICE needs an axis n in {0, 1, 2}");
+            c->has_lattice = true;
+            break;
         case METAD_CV_TORSION: {
             for (int k = 0; k < 4; ++k) {
                 if (s.torsion[k] < 0 || s.torsion[k] >= N) FAIL(METAD_ERR_ARG, "torsion index");
@@ -142,6 +146,8 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     }
 
     if (c->has_mindist) CUDA_TRY(dev_alloc(&c->d_mind, 8));
+    CUDA_TRY(dev_alloc(&c->d_box_force, 9));
+    CUDA_TRY(cudaMemset(c->d_box_force, 0, sizeof(double) * 9));
     if (c->has_torsion) {
         std::vector<int> ta;
         for (int d = 0; d < c->D; ++d)
@@ -226,7 +232,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
@@ -503,6 +509,12 @@ extern "C" int metad_reweight(metad_ctx *c, const double *d_traj, int nframes, c
     }
     if ((long long)h_nbins[0] * (c->D > 1 ? h_nbins[1] : 1) > (1ll << 26)) FAIL(METAD_ERR_ARG, "too many bins");
     return reweight_run(c, d_traj, nframes, h_nbins, h_lo, h_hi, d_P, d_F);
+}
+
+extern "C" int metad_get_box_force(metad_ctx *c, double *d_out9) {
+    if (!c || !d_out9) FAIL(METAD_ERR_ARG, "null argument");
+    CUDA_TRY(cudaMemcpyAsync(d_out9, c->d_box_force, sizeof(double) * 9, cudaMemcpyDeviceToDevice, c->stream));
+    return METAD_OK;
 }
 
 extern "C" int metad_reset_steps(metad_ctx *c) {

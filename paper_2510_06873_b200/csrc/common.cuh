@@ -142,7 +142,8 @@ struct metad_ctx {
     int *d_nl_count, *d_nl;               // sorted space; nl[k*N + s]
     // CV state
     CvDev cv[METAD_MAX_CV];
-    bool has_q6, has_coord, has_torsion, has_mindist;
+    bool has_q6, has_coord, has_torsion, has_mindist, has_lattice;
+    double *d_box_force;                  // LATTICE: [9] bias force on the box rows, written by apply_forces
     int mindist_dim;
     double *d_mind;                       // MINDIST: [r, dx, dy, dz] of the nearest pair + its two original indices (as int pair)
     double *d_tors_grad;                  // TORSION: [D][12] d phi / d r of the four atoms, written by the CV kernel
@@ -193,6 +194,8 @@ int nb_export(metad_ctx *c, int *d_count, int *d_list);
 int cv_eval_all(metad_ctx *c, double *d_cv);
 int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F);
 int q6_export(metad_ctx *c, void *d_q6);
+int lattice_eval(metad_ctx *c, double *d_cv);
+int lattice_forces(metad_ctx *c, const double *d_dVds);
 int mindist_eval(metad_ctx *c, double *d_cv);
 int mindist_forces(metad_ctx *c, const double *d_dVds, void *d_F);
 int torsion_eval_all(metad_ctx *c, double *d_cv);

@@ -600,6 +600,8 @@ int cv_eval_all(metad_ctx *c, double *d_cv) {
     if (rcode) return rcode;
     rcode = mindist_eval(c, d_cv);
     if (rcode) return rcode;
+    rcode = lattice_eval(c, d_cv);
+    if (rcode) return rcode;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
 }
@@ -643,6 +645,8 @@ int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F) {
     rcode = torsion_forces(c, d_dVds, d_F);
     if (rcode) return rcode;
     rcode = mindist_forces(c, d_dVds, d_F);
+    if (rcode) return rcode;
+    rcode = lattice_forces(c, d_dVds);
     if (rcode) return rcode;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

@@ -319,3 +319,54 @@ int torsion_forces(metad_ctx *c, const double *d_dVds, void *d_F) {
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
 }
+
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-3: lattice-parameter CVs (reading AB): s = |h_k|; the bias force acts on the box rows.
+struct LatTable { int kind[METAD_MAX_CV]; int axis[METAD_MAX_CV]; double h[9]; };
+
+__global__ void k_lattice_cv(int D, LatTable lt, double *__restrict__ cv_out) {
+    const int d = threadIdx.x;
+    if (d >= D || lt.kind[d] != METAD_CV_LATTICE) return;
+    const double *h = lt.h + 3 * lt.axis[d];
+    cv_out[d] = sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
+}
+
+__global__ void k_lattice_force(int D, LatTable lt, double force_scale, const double *__restrict__ dVds,
+                                double *__restrict__ fbox) {
+    const int e = threadIdx.x;              // box element (row, component)
+    if (e >= 9) return;
+    const int row = e / 3;
+    double f = 0.0;
+    for (int d = 0; d < D; ++d) {
+        if (lt.kind[d] != METAD_CV_LATTICE || lt.axis[d] != row) continue;
+        const double *h = lt.h + 3 * row;
+        f += dVds[d] * h[e - 3 * row] / sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
+    }
+    fbox[e] = -force_scale * f;
+}
+
+static LatTable lat_table(const metad_ctx *c) {
+    LatTable lt;
+    for (int d = 0; d < METAD_MAX_CV; ++d) { lt.kind[d] = d < c->D ? c->cv[d].kind : -1; lt.axis[d] = d < c->D ? c->cv[d].n : 0; }
+    const BoxD &b = c->boxd;
+    const double h[9] = { b.ax, 0.0, 0.0, b.bx, b.by, 0.0, b.cx, b.cy, b.cz };
+    for (int k = 0; k < 9; ++k) lt.h[k] = h[k];
+    return lt;
+}
+
+int lattice_eval(metad_ctx *c, double *d_cv) {
+    if (!c->has_lattice) return METAD_OK;
+    k_lattice_cv<<<1, 32, 0, c->stream>>>(c->D, lat_table(c), d_cv);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+int lattice_forces(metad_ctx *c, const double *d_dVds) {
+    if (!c->has_lattice) return METAD_OK;
+    k_lattice_force<<<1, 32, 0, c->stream>>>(c->D, lat_table(c), c->p.force_scale, d_dVds, c->d_box_force);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmetad_b200.so")
 MAX_CV = 4
 OK, ERR_ARG, ERR_BOX, ERR_STATE, ERR_CUDA, ERR_NOMEM = range(6)
 DEV_NEIGH_OVERFLOW, DEV_HILL_OVERFLOW, DEV_GRID_RANGE, DEV_NONFINITE, DEV_POS_RANGE = 1, 2, 4, 8, 16
-CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CV_MINDIST = range(7)
+CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CV_MINDIST, CV_LATTICE = range(8)
 
 _P = ctypes.c_void_p
 _I = ctypes.c_int
@@ -42,7 +42,7 @@ class Params(ctypes.Structure):
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
            "metad_apply_forces", "metad_deposit", "metad_run", "metad_step_host", "metad_status",
            "metad_get_state", "metad_get_neighbors", "metad_get_q6", "metad_set_hills", "metad_get_hills",
-           "metad_get_grid", "metad_bias_batch", "metad_reweight", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
+           "metad_get_grid", "metad_get_box_force", "metad_bias_batch", "metad_reweight", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
 
 _lib = None
 
@@ -73,6 +73,7 @@ def load():
     L.metad_get_hills.argtypes = [_P, _P, _P, _I, _P, _I]
     L.metad_get_grid.argtypes = [_P, _P]
     L.metad_reset_steps.argtypes = [_P]
+    L.metad_get_box_force.argtypes = [_P, _P]
     L.metad_bias_batch.argtypes = [_P, _P, _I, _P]
     L.metad_reweight.argtypes = [_P, _P, _I, _P, _P, _P, _P, _P]
     L.metad_set_timing.argtypes = [_P, _I]
@@ -267,6 +268,13 @@ class MetaD:
         _check(load().metad_get_grid(self._h, _ptr(t)))
         self.synchronize()
         return t.cpu().numpy()
+
+    def box_force(self):
+        """Bias force on the box rows (3,3) of the last apply_forces (lattice-parameter CVs)."""
+        t = self.torch.empty(9, dtype=self.torch.float64, device="cuda")
+        _check(load().metad_get_box_force(self._h, _ptr(t)))
+        self.synchronize()
+        return t.cpu().numpy().reshape(3, 3)
 
     def bias_batch(self, points):
         """V_b at many CV points (torch float64 CUDA tensor [T, ncv]) -> tensor [T]."""

@@ -1,0 +1,64 @@
+"""-m gpu: the CV set of the paper's GaN workload — coordination number + the three lattice parameters (
+reading AB) — CUDA path against the oracle, including the bias force on the cell."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2510_06873_b200.inputs import CV_COORD, CV_LATTICE, CVSpec, configs  # noqa: E402
+
+from gpu_util import assert_stagewise, stagewise  # noqa: E402
+
+
+def _workload():
+    w = configs.small("c3")                     # GaN-shaped: wurtzite nucleus in random liquid, triclinic (hexagonal) box
+    w.cvs = [CVSpec(kind=CV_COORD, r0=2.4, n=6, m=12, scale=1.0 / w.natoms),
+             CVSpec(kind=CV_LATTICE, n=0), CVSpec(kind=CV_LATTICE, n=1), CVSpec(kind=CV_LATTICE, n=2)]
+    w.sigma = [0.05, 0.1, 0.1, 0.15]
+    w.n_hills = 200
+    w.precision = 64
+    return w
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_coordination_plus_lattice_parameters(precision):
+    w = _workload()
+    r = stagewise(w, precision=precision)
+    assert_stagewise(r)
+    B = w.box.reshape(3, 3)
+    assert np.allclose(r["s"][1:], np.linalg.norm(B, axis=1), rtol=1e-14)
+    fb = r["md"].box_force()
+    fb_ref = r["o"].box_force(r["dV_ref"])
+    assert np.abs(fb_ref).max() > 0
+    assert np.abs(fb - fb_ref).max() <= 1e-12 * np.abs(fb_ref).max()
+    # the lattice dimensions put no force on the atoms: F equals the coordination-number term alone
+    F_cn = -r["dV_ref"][0] * r["o"].grads[0]
+    assert np.abs(r["F_ref"] - F_cn).max() <= 1e-15 * np.abs(F_cn).max()
+
+
+def test_lattice_only_context_and_bad_axis():
+    import torch
+    from paper_2510_06873_b200.metad import MetaD, MetadError
+    w = _workload()
+    w.cvs = w.cvs[1:]
+    w.sigma = w.sigma[1:]
+    md = MetaD(w)
+    dpos = torch.tensor(w.pos, device="cuda")
+    F = torch.zeros((w.natoms, 3), device="cuda", dtype=torch.float64)
+    torch.cuda.synchronize()
+    s0 = np.linalg.norm(w.box.reshape(3, 3), axis=1)
+    md.set_hills(np.array([s0 + [0.05, -0.02, 0.1]]), np.array([2.0]))
+    md.run(dpos, F, 1)
+    st = md.state()
+    assert np.allclose(st["cv"], s0, rtol=1e-14) and not F.cpu().numpy().any()
+    d = s0 - (s0 + [0.05, -0.02, 0.1])
+    V = 2.0 * np.exp(-0.5 * np.sum((d / np.asarray(w.sigma)) ** 2))
+    assert abs(st["V"] - V) <= 1e-12 * V
+    fb = md.box_force()
+    ref = np.zeros((3, 3))
+    for k in range(3):
+        ref[k] = -(-V * d[k] / w.sigma[k] ** 2) * w.box.reshape(3, 3)[k] / s0[k]
+    assert np.abs(fb - ref).max() <= 1e-12 * np.abs(ref).max()
+    w.cvs[0].n = 3
+    with pytest.raises(MetadError):
+        MetaD(w)
