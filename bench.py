@@ -35,7 +35,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="c3", choices=["c0", "c1", "c2", "c3", "c4", "t0"])
+    ap.add_argument("--config", default="c3", choices=["c0", "c1", "c2", "c3", "c4", "t0", "g0"])
     ap.add_argument("--precision", type=int, default=0, help="0 = the workload's own (c3: 32 for the headline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fast-setup", action="store_true",
@@ -50,9 +50,10 @@ def workload(name):
 
 
 def describe(w, precision):
-    kinds = {0: "coordination", 1: "Q6 mean", 2: "Q6 solid-like count", 3: "radius of gyration", 4: "native contacts", 5: "torsion"}
-    wl = ("PAPER.md:37 alanine-dipeptide-shaped torsion workload (t0, SURVEY.md §8(f) NEXT-1)" if w.name == "t0"
-          else f"BASELINE.json configs[{w.name[1]}] ({w.name})")
+    kinds = {0: "coordination", 1: "Q6 mean", 2: "Q6 solid-like count", 3: "radius of gyration", 4: "native contacts", 5: "torsion", 6: "distance to nearest", 7: "lattice parameter"}
+    wl = {"t0": "PAPER.md:37 alanine-dipeptide-shaped torsion workload (t0, SURVEY.md §8(f) NEXT-1)",
+          "g0": "PAPER.md:51 GaN CV set (coordination number + 3 lattice parameters) on the configs[3] structure (g0)"
+          }.get(w.name, f"BASELINE.json configs[{w.name[1]}] ({w.name})")
     return {"workload": wl, "atoms": int(w.natoms),
             "cvs": [kinds[c.kind] for c in w.cvs], "hills": int(w.n_hills), "rc": w.rc,
             "pair_precision": f"fp{precision}", "stride": int(w.stride),
@@ -115,6 +116,8 @@ def oracle_sample(name):
         return configs.config3(cells=(30, 30, 16), sphere_r=18.0, n_hills=10000), "c3 recipe at 30x30x16 cells (57,600 atoms), 10,000 hills"
     if name == "c4":
         return configs.config4(cells=(30, 30, 16), sphere_r=18.0, n_hills=20000, grid=(0, 0)), "c4 recipe at 57,600 atoms, 20,000 hills, exact sum"
+    if name == "g0":
+        return configs.config_g0(cells=(30, 30, 16), sphere_r=18.0, n_hills=10000), "g0 recipe at 30x30x16 cells (57,600 atoms), 10,000 hills"
     w = configs.BUILDERS[name]()
     return w, f"{name} at full size"
 
@@ -249,7 +252,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     w = workload(args.config)
-    precision = args.precision or (32 if args.config in ("c3", "c4") else w.precision)
+    precision = args.precision or (32 if args.config in ("c3", "c4", "g0") else w.precision)
     tdt = torch.float32 if precision == 32 else torch.float64
     pos = w.pos.astype(np.float32 if precision == 32 else np.float64)
     dpos = torch.tensor(pos, device="cuda")

@@ -146,6 +146,7 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     }
 
     if (c->has_mindist) CUDA_TRY(dev_alloc(&c->d_mind, 8));
+    CUDA_TRY(dev_alloc(&c->d_cvq6, 2));
     CUDA_TRY(dev_alloc(&c->d_box_force, 9));
     CUDA_TRY(cudaMemset(c->d_box_force, 0, sizeof(double) * 9));
     if (c->has_torsion) {
@@ -182,7 +183,6 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     if (c->has_q6) {
         CUDA_TRY(cudaMalloc(&c->d_rec, METAD_NREC * tsz * (size_t)N));
         CUDA_TRY(dev_alloc(&c->d_q6, N));
-        CUDA_TRY(dev_alloc(&c->d_cvq6, 2));
     }
     CUDA_TRY(dev_alloc(&c->d_partials, 3 * (size_t)c->nblocks_atoms + max_pair_blocks));
     if (c->has_coord && N <= METAD_WARP_PER_ATOM_MAX) CUDA_TRY(dev_alloc(&c->d_partials_warp, (size_t)N / 4 + 2));
@@ -279,10 +279,13 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
     BoxD b = { ax, bx, by, cx, cy, cz, 0.5 * ax, 0.5 * by, 0.5 * cz };
     c->boxd = b;
     c->rc = rc; c->rc2 = rc * rc;
-    // shared-memory tiled fast path: fp32, neighbour-list CVs = Q6 only, >= 3 cells per direction
+    // shared-memory tiled fast path: fp32, neighbour-list CVs = Q6 only or an ungrouped coordination number only,
+    // >= 3 cells per direction
     c->tiled = 0;
     const char *env = getenv("METAD_NO_TILES");
-    if (c->prec == 32 && c->has_q6 && !c->has_coord && !c->has_mindist && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32 &&
+    const bool q6_only = c->has_q6 && !c->has_coord;
+    const bool coord_only = c->has_coord && !c->has_q6 && !c->cv[c->coord_dim].use_groups;
+    if (c->prec == 32 && (q6_only || coord_only) && !c->has_mindist && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32 &&
         !(env && env[0] == '1')) {
         const double rho = (double)c->N / g.ncell, margin = 1.3;
         const int cap = 1216;

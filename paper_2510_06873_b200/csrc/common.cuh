@@ -212,4 +212,5 @@ int tiled_init();
 int tiled_build(metad_ctx *c);
 int tiled_q6_pass1(metad_ctx *c, double *d_cv);
 int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F);
+int tiled_coord_force(metad_ctx *c, const double *d_dVds, void *d_F);
 int tiled_export(metad_ctx *c, int *d_count, int *d_list);

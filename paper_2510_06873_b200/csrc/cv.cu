@@ -3,39 +3,11 @@
 // pair arithmetic in T, every reduction in fp64 with a fixed order (deterministic).
 #include "common.cuh"
 #include "cv_q6.cuh"
+#include "cv_switch.cuh"
 
 template <typename T> PBox<T> ctx_pbox(const metad_ctx *c);
 
 #define CV_THREADS 128
-
-// ------------------------------------------------------------------------------------------------
-// switching function sw(x) = (1-x^n)/(1-x^m) and d sw/dx (reading A).  m == 2n -> 1/(1+x^n).
-template <typename T>
-__device__ __forceinline__ T ipow(T x, int n) {
-    T r = T(1);
-    for (int k = 0; k < n; ++k) r *= x;
-    return r;
-}
-template <typename T>
-__device__ __forceinline__ T switch_fn(T x, int n, int m, T &dsw) {
-    if (m == 2 * n) {
-        T xn1 = ipow(x, n - 1), xn = xn1 * x;
-        T inv = T(1) / (T(1) + xn);
-        dsw = -T(n) * xn1 * inv * inv;
-        return inv;
-    }
-    T e = x - T(1);
-    if (fabs((double)e) < 1e-6) {
-        T s0 = T(n) / T(m), s1 = T(n) * T(n - m) / (T(2) * T(m));
-        dsw = s1;
-        return s0 + s1 * e;
-    }
-    T xn1 = ipow(x, n - 1), xm1 = ipow(x, m - 1);
-    T num = T(1) - xn1 * x, den = T(1) - xm1 * x;
-    T f = num / den;
-    dsw = (-T(n) * xn1 * den + num * T(m) * xm1) / (den * den);
-    return f;
-}
 
 // ------------------------------------------------------------------------------------------------
 // coordination number
@@ -400,6 +372,52 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
     F[3 * i + 2] += (float)(force_scale * (double)fz);
 }
 
+// Coordination-number forces on the tiled fp32 path (ungrouped: every ordered pair counts, i.e. each pair twice in
+// d s/d r_k): thread per atom, gather form over the sliced list; per pair one 128-bit position load.
+__global__ void __launch_bounds__(CV_THREADS)
+k_coord_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
+                const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, float inv_r0, int n, int m,
+                double coef /* force_scale * scale */, const double *__restrict__ dVds, float *__restrict__ F) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    const float4 pi = spos[s];
+    const int *in = nl + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
+    const int cnt = nl_count[s];
+    float ax = 0.f, ay = 0.f, az = 0.f;
+    for (int k = 0; k < cnt; ++k) {
+        const int e = in[k * 32];
+        const int j = e & NLG_IDX_MASK, code = (unsigned)e >> 27;
+        const float4 pj = spos[j];
+        float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+        if (code != 13) {
+            const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
+            dx = (float)(((double)pj.x - (double)pi.x) + (wx * bd.ax + wy * bd.bx + wz * bd.cx));
+            dy = (float)(((double)pj.y - (double)pi.y) + (wy * bd.by + wz * bd.cy));
+            dz = (float)(((double)pj.z - (double)pi.z) + (wz * bd.cz));
+        }
+        const float r2 = dx * dx + dy * dy + dz * dz, rinv = rsqrtf(r2);
+        float dsw;
+        switch_fn<float>(r2 * rinv * inv_r0, n, m, dsw);
+        const float g = 2.f * dsw * inv_r0 * rinv;
+        ax += g * dx; ay += g * dy; az += g * dz;
+    }
+    const double a = coef * dVds[0];
+    const int i = perm[s];
+    F[3 * i] += (float)(a * (double)ax);
+    F[3 * i + 1] += (float)(a * (double)ay);
+    F[3 * i + 2] += (float)(a * (double)az);
+}
+
+int tiled_coord_force(metad_ctx *c, const double *d_dVds, void *d_F) {
+    const CvDev &d = c->cv[c->coord_dim];
+    k_coord_force_g<<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+        c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (float)(1.0 / d.r0), d.n, d.m,
+        c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
 int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
     double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
@@ -559,7 +577,10 @@ static int cv_eval_t(metad_ctx *c, double *d_cv) {
     typedef typename Vec4<T>::type V4;
     const int N = c->N, nb = div_up(N, CV_THREADS);
     PBox<T> pb = ctx_pbox<T>(c);
-    if (c->has_coord) {
+    if (c->has_coord && c->tiled) {                          // the sum ran inside k_tile_build<2>
+        int r = tiled_q6_pass1(c, d_cv);
+        if (r) return r;
+    } else if (c->has_coord) {
         const CvDev &d = c->cv[c->coord_dim];
         if (N <= METAD_WARP_PER_ATOM_MAX)
             k_coord_cv_warp<T><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
@@ -611,7 +632,10 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
     typedef typename Vec4<T>::type V4;
     const int N = c->N, nb = div_up(N, CV_THREADS);
     PBox<T> pb = ctx_pbox<T>(c);
-    if (c->has_coord) {
+    if (c->has_coord && c->tiled) {
+        int r = tiled_coord_force(c, d_dVds, d_F);
+        if (r) return r;
+    } else if (c->has_coord) {
         const CvDev &d = c->cv[c->coord_dim];
         if (N <= METAD_WARP_PER_ATOM_MAX)
             k_coord_force_warp<T><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(

@@ -10,6 +10,7 @@
 #include <algorithm>
 #include "common.cuh"
 #include "cv_q6.cuh"
+#include "cv_switch.cuh"
 #include "tile.cuh"
 
 typedef unsigned short nl16_t;   // local halo index (shared-memory candidate list only)
@@ -72,13 +73,15 @@ __device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t,
 
 // Exact decision on the short list of own atom a (list column `col`, cnt candidates), neighbour-list write, fused q6m
 // accumulation and the atom's q6 record.  Returns q6.
-template <bool STAGED, bool WITH_Q6>
+template <bool STAGED, int MODE>
 __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos,
                                              const float4 *pos_s, const nl16_t *list_s, int a, int col, int cnt, bool ovf,
                                              const BoxD &bd, float rc2f, float rc2_lo, double rc2, int maxn,
                                              int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
                                              float q_thresh, float inv_width, float *__restrict__ rec,
-                                             float *__restrict__ q6_out, bool solid) {
+                                             float *__restrict__ q6_out, bool solid, int sw_n, int sw_m) {
+    const bool WITH_Q6 = MODE == 1;
+    float csum = 0.f;                                      // MODE 2: sum of sw(r / r0) over the neighbours (q_thresh = 1 / r0)
     const int q = tile_own_row(t, a);
     const int o = a - t.own_off[q];
     const int li = t.own_l[q] + o, s = t.own_g[q] + o;
@@ -105,6 +108,7 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
         if (!in) continue;
         if (n < maxn) {
             out[n * 32] = __float_as_int(pj.w);
+            if (MODE == 2) { float dsw; csum += switch_fn<float>(sqrtf(r2) * q_thresh, sw_n, sw_m, dsw); }
             if (WITH_Q6) {
                 const float rinv = rsqrtf(r2);
                 Y6<float> y;
@@ -138,33 +142,31 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
         }
         q6_out[s] = q6;
     }
-    return q6;
+    return MODE == 2 ? csum : q6;
 }
 
 // One thread per own atom: scan, then the exact pass.  (Re-dealing the atoms to the threads by candidate count between the
 // two passes, so that the lanes of a warp run equal trip counts, was measured and dropped: profiles/r1h_rejected.md.)
-template <bool STAGED, bool WITH_Q6>
+template <bool STAGED, int MODE>
 __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos,
                                            const float4 *pos_s, nl16_t *list_s, const int *__restrict__ scell,
                                            const BoxD &bd, float rc2f, double rc2, int maxn, int *__restrict__ nl_count,
                                            int *__restrict__ nl, unsigned int *__restrict__ sticky, float q_thresh,
                                            float inv_width, float *__restrict__ rec, float *__restrict__ q6_out, bool solid,
-                                           double (&v)[2]) {
+                                           int sw_n, int sw_m, double (&v)[2]) {
     const float rc2_hi = rc2f * (1.f + 1e-5f), rc2_lo = rc2f * (1.f - 1e-5f);
     const int tid = threadIdx.x;
     for (int a = tid; a < t.nown; a += blockDim.x) {
         bool ovf = false;
         const int cnt = scan_atom<STAGED>(g, t, spos, pos_s, list_s, scell, a, tid, rc2_hi, ovf);
-        const float q6 = finish_atom<STAGED, WITH_Q6>(g, t, spos, pos_s, list_s, a, tid, cnt, ovf, bd, rc2f, rc2_lo, rc2, maxn,
-                                                      nl_count, nl, sticky, q_thresh, inv_width, rec, q6_out, solid);
-        if (WITH_Q6) {
-            v[0] += (double)q6;
-            v[1] += (double)(1.f / (1.f + expf(-(q6 - q_thresh) * inv_width)));
-        }
+        const float q6 = finish_atom<STAGED, MODE>(g, t, spos, pos_s, list_s, a, tid, cnt, ovf, bd, rc2f, rc2_lo, rc2, maxn,
+                                                   nl_count, nl, sticky, q_thresh, inv_width, rec, q6_out, solid, sw_n, sw_m);
+        if (MODE != 0) v[0] += (double)q6;
+        if (MODE == 1) v[1] += (double)(1.f / (1.f + expf(-(q6 - q_thresh) * inv_width)));
     }
 }
 
-template <bool WITH_Q6>
+template <int MODE>   // 0: list only, 1: + Q6 pass 1, 2: + coordination sum (ungrouped COORD, q_thresh = 1 / r0)
 #ifndef TB_MINB
 #define TB_MINB 5
 #endif
@@ -173,7 +175,7 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
              const int *__restrict__ cell_start, BoxD bd, float rc2f, double rc2, int maxn,
              int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
              float q_thresh, float inv_width, float *__restrict__ rec, float *__restrict__ q6_out, int solid,
-             double *__restrict__ partials, unsigned int *__restrict__ ticket, double scale_mean, double scale_solid,
+             int sw_n, int sw_m, double *__restrict__ partials, unsigned int *__restrict__ ticket, double scale_mean, double scale_solid,
              double *__restrict__ cv_q6 /* [2]: Q6 mean, solid count */) {
     extern __shared__ float4 dyn_smem[];
     __shared__ TileTables t;
@@ -187,13 +189,13 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
     if (t.total > 65535) {
         if (threadIdx.x == 0) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
     } else if (t.staged) {
-        build_body<true, WITH_Q6>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
-                                  inv_width, rec, q6_out, solid != 0, v);
+        build_body<true, MODE>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
+                                  inv_width, rec, q6_out, solid != 0, sw_n, sw_m, v);
     } else {
-        build_body<false, WITH_Q6>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
-                                   inv_width, rec, q6_out, solid != 0, v);
+        build_body<false, MODE>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
+                                   inv_width, rec, q6_out, solid != 0, sw_n, sw_m, v);
     }
-    if (WITH_Q6) {
+    if (MODE != 0) {
         block_reduce<2>(v, red);
         if (threadIdx.x == 0) { partials[2 * blockIdx.x] = v[0]; partials[2 * blockIdx.x + 1] = v[1]; }
         if (last_block_ticket(ticket)) {                      // fixed-order sum of the per-tile partials
@@ -238,8 +240,9 @@ static size_t smem_build(const TileGeom &g) {
 int tiled_init() {
     static bool done = false;
     if (done) return METAD_OK;
-    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
     done = true;
     return METAD_OK;
 }
@@ -250,16 +253,22 @@ int tiled_build(metad_ctx *c) {
     double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
     double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
     if (c->has_q6)
-        k_tile_build<true><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
+        k_tile_build<1><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
             c->d_nl_count, c->d_nl, c->d_sticky, (float)qt, (float)(1.0 / qw), (float *)c->d_rec, c->d_q6,
-            c->q6_solid_dim >= 0 ? 1 : 0, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
+            c->q6_solid_dim >= 0 ? 1 : 0, 0, 0, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
             c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0, c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0,
             c->d_cvq6);
-    else
-        k_tile_build<false><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
+    else if (c->has_coord) {                                  // ungrouped coordination number: the sum of sw rides on the exact pass
+        const CvDev &d = c->cv[c->coord_dim];
+        k_tile_build<2><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
-            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, nullptr, nullptr, 0.0, 0.0, nullptr);
+            c->d_nl_count, c->d_nl, c->d_sticky, (float)(1.0 / d.r0), 1.f, nullptr, nullptr, 0, d.n, d.m,
+            c->d_partials + c->nblocks_atoms, c->d_tickets + 1, d.scale, 0.0, c->d_cvq6);
+    } else
+        k_tile_build<0><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
+            g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
+            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, 0, 0, nullptr, nullptr, 0.0, 0.0, nullptr);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -267,7 +276,8 @@ int tiled_build(metad_ctx *c) {
 
 // the q6m accumulation and its reduction already ran inside k_tile_build
 int tiled_q6_pass1(metad_ctx *c, double *d_cv) {
-    k_q6_publish<<<1, 32, 0, c->stream>>>(c->d_cvq6, c->q6_mean_dim, c->q6_solid_dim, d_cv);
+    if (c->has_q6) k_q6_publish<<<1, 32, 0, c->stream>>>(c->d_cvq6, c->q6_mean_dim, c->q6_solid_dim, d_cv);
+    else k_q6_publish<<<1, 32, 0, c->stream>>>(c->d_cvq6, c->coord_dim, -1, d_cv);          // tiled coordination number
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

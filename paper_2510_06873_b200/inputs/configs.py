@@ -6,7 +6,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import (BASE_SEED, CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CVSpec, Workload,
+from . import (BASE_SEED, CV_LATTICE, CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CVSpec, Workload,
                hill_walk_periodic, rsa, wrap)
 
 
@@ -214,6 +214,20 @@ def config_t0(seed=BASE_SEED + 10, natoms=22, n_hills=20000, grid=(256, 256), n_
                     extra={"period_lo": [-np.pi, -np.pi]})
 
 
+# ----------------------------------------------------------------------------------------- g0
+def config_g0(seed=BASE_SEED + 3, cells=(80, 80, 40), sphere_r=30.0, n_hills=10000):
+    """The CV set of the paper's own GaN runs ("the coordination number (C.N.) and the triaxial lattice
+    parameters as CVs") on the GaN-shaped structure of BASELINE.json configs[3] (same seed, same atoms): 4-D CV =
+    mean coordination number (r0 = 2.4 A between the first and second wurtzite shells, n = 6, m = 12, rc = 3.6 A) and
+    the lengths of the three box rows; well-tempered, bias factor 20; widths (0.02, 0.1, 0.1, 0.1)."""
+    w = config3(seed=seed, cells=cells, sphere_r=sphere_r, n_hills=n_hills)
+    w.name = "g0"
+    w.cvs = [CVSpec(kind=CV_COORD, r0=2.4, n=6, m=12, scale=1.0 / w.natoms),
+             CVSpec(kind=CV_LATTICE, n=0), CVSpec(kind=CV_LATTICE, n=1), CVSpec(kind=CV_LATTICE, n=2)]
+    w.sigma = [0.02, 0.1, 0.1, 0.1]
+    return w
+
+
 def small(name):
     """Scaled-down variants with the same structure, for the CPU suite and quick GPU parity."""
     if name == "c1":
@@ -230,7 +244,9 @@ def small(name):
         return config0()
     if name == "t0":
         return config_t0(n_hills=500, grid=(48, 40))
+    if name == "g0":
+        return config_g0(cells=(12, 12, 8), sphere_r=9.0, n_hills=400)
     raise KeyError(name)
 
 
-BUILDERS = {"c0": config0, "c1": config1, "c2": config2, "c3": config3, "c4": config4, "t0": config_t0}
+BUILDERS = {"c0": config0, "c1": config1, "c2": config2, "c3": config3, "c4": config4, "t0": config_t0, "g0": config_g0}
