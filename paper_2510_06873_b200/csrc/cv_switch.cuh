@@ -5,8 +5,12 @@
 // switching function sw(x) = (1-x^n)/(1-x^m) and d sw/dx (reading A).  m == 2n -> 1/(1+x^n).
 template <typename T>
 __device__ __forceinline__ T ipow(T x, int n) {
-    T r = T(1);
-    for (int k = 0; k < n; ++k) r *= x;
+    T r = T(1);                                   // square and multiply: log2(n) steps instead of n
+    while (n > 0) {
+        if (n & 1) r *= x;
+        x *= x;
+        n >>= 1;
+    }
     return r;
 }
 template <typename T>
