@@ -337,7 +337,7 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
     const int cnt = nl_count[s];
     float fx = 0.f, fy = 0.f, fz = 0.f;
     for (int k = 0; k < cnt; ++k) {
-        const int e = in[k * 32];
+        const int e = __ldcs(in + k * 32);            // streamed once: do not displace positions / records in L2
         const int j = e & NLG_IDX_MASK, code = (unsigned)e >> 27;
         float4 a4, b4, c4, d4, pj;
         ldg256(rec + (size_t)j * METAD_NREC, a4, b4);
@@ -385,7 +385,7 @@ k_coord_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__r
     const int cnt = nl_count[s];
     float ax = 0.f, ay = 0.f, az = 0.f;
     for (int k = 0; k < cnt; ++k) {
-        const int e = in[k * 32];
+        const int e = __ldcs(in + k * 32);            // streamed once: do not displace positions / records in L2
         const int j = e & NLG_IDX_MASK, code = (unsigned)e >> 27;
         const float4 pj = spos[j];
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;

@@ -107,7 +107,7 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
         }
         if (!in) continue;
         if (n < maxn) {
-            out[n * 32] = __float_as_int(pj.w);
+            __stcs(out + n * 32, __float_as_int(pj.w));     // streaming store: the list is read once, by the force pass
             if (MODE == 2) { float dsw; csum += switch_fn<float>(sqrtf(r2) * q_thresh, sw_n, sw_m, dsw); }
             if (WITH_Q6) {
                 const float rinv = rsqrtf(r2);
