@@ -38,3 +38,19 @@ def test_config4_full_size():
     r = stagewise(w)                      # fp32 pair math, exact hill sum (grid parity: test_gpu_parity)
     assert_stagewise(r)
     assert np.abs(r["q6"] - r["q6_ref"]).max() <= 2e-6
+
+
+def test_gan_cv_set_full_size_fp32_tiled():
+    """PAPER.md:51 CV set (coordination number + a, b, c) at 1,024,000 atoms in the configuration bench.py --config g0
+    times: fp32 pair math on the tiled path (coordination sum fused into the list build)."""
+    w = configs.config_g0()
+    r = stagewise(w, precision=32)
+    assert_stagewise(r)
+    fb, fb_ref = r["md"].box_force(), r["o"].box_force(r["dV_ref"])
+    assert np.abs(fb - fb_ref).max() <= 1e-12 * np.abs(fb_ref).max()
+
+
+def test_torsion_workload_full_size():
+    """PAPER.md:37 workload in the configuration bench.py --config t0 times (20,000 hills, periodic)."""
+    r = stagewise(configs.config_t0())
+    assert_stagewise(r)
