@@ -287,19 +287,30 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
     const bool coord_only = c->has_coord && !c->has_q6 && !c->cv[c->coord_dim].use_groups;
     if (c->prec == 32 && (q6_only || coord_only) && !c->has_mindist && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32 &&
         !(env && env[0] == '1')) {
-        const double rho = (double)c->N / g.ncell, margin = 1.3;
+        // the rc-wide cells are subdivided along x (the direction of the contiguous row runs): an atom then scans
+        // 2 xsub + 1 sub-cells per row (2.5 / 2.25 cell widths for xsub = 2 / 4) instead of 3 cells
+        int xsub = 2;
+        const char *xs = getenv("METAD_XSUB");
+        if (xs && xs[0] >= '1' && xs[0] <= '4') xsub = xs[0] - '0';
+        while (xsub > 1 && (long long)g.ncell * xsub > c->cell_cap) --xsub;
+        CellGrid gs = g;
+        gs.nc[0] *= xsub; gs.ncell *= xsub;
+        const double rho = (double)c->N / gs.ncell, margin = 1.3;
         const int cap = 1216;
         double best = 1e30; int bt[3] = { 0, 0, 0 };
         for (int ty = 1; ty <= 4; ++ty) for (int tz = 1; tz <= 4; ++tz) for (int tx = 1; tx <= TILE_TXMAX; ++tx) {
-            if (tx > g.nc[0] - 2 || ty > g.nc[1] - 2 || tz > g.nc[2] - 2) continue;
-            double own = rho * tx * ty * tz, halo = rho * (tx + 2) * (ty + 2) * (tz + 2);
+            if (tx > gs.nc[0] - 2 * xsub || ty > gs.nc[1] - 2 || tz > gs.nc[2] - 2) continue;
+            double own = rho * tx * ty * tz, halo = rho * (tx + 2 * xsub) * (ty + 2) * (tz + 2);
             if (halo * margin > cap || own > TILE_THREADS) continue;
-            long long ntl = (long long)((g.nc[0] + tx - 1) / tx) * ((g.nc[1] + ty - 1) / ty) * ((g.nc[2] + tz - 1) / tz);
+            long long ntl = (long long)((gs.nc[0] + tx - 1) / tx) * ((gs.nc[1] + ty - 1) / ty) * ((gs.nc[2] + tz - 1) / tz);
             if (ntl > c->nblocks_atoms) continue;     // per-tile partials live in the per-block scratch
             double score = halo / own + (own < 128 ? 2.0 : 0.0);   // halo ratio; keep the block busy
             if (score < best) { best = score; bt[0] = tx; bt[1] = ty; bt[2] = tz; }
         }
-        if (bt[0] > 0) { c->tiled = 1; c->tile_T[0] = bt[0]; c->tile_T[1] = bt[1]; c->tile_T[2] = bt[2]; c->tile_cap = cap; }
+        if (bt[0] > 0) {
+            c->tiled = 1; c->tile_T[0] = bt[0]; c->tile_T[1] = bt[1]; c->tile_T[2] = bt[2]; c->tile_cap = cap; c->tile_hx = xsub;
+            c->grid = gs;
+        }
     }
     return METAD_OK;
 }
@@ -309,7 +320,7 @@ TileGeom tile_geom(const metad_ctx *c) {
     t.Tx = c->tile_T[0]; t.Ty = c->tile_T[1]; t.Tz = c->tile_T[2];
     t.nc0 = c->grid.nc[0]; t.nc1 = c->grid.nc[1]; t.nc2 = c->grid.nc[2];
     t.ntx = (t.nc0 + t.Tx - 1) / t.Tx; t.nty = (t.nc1 + t.Ty - 1) / t.Ty; t.ntz = (t.nc2 + t.Tz - 1) / t.Tz;
-    t.cap = c->tile_cap;
+    t.cap = c->tile_cap; t.hx = c->tile_hx;
     t.ax = c->boxd.ax; t.bx = c->boxd.bx; t.by = c->boxd.by; t.cx = c->boxd.cx; t.cy = c->boxd.cy; t.cz = c->boxd.cz;
     t.wa = t.wb = t.wc = 0.0;
     return t;

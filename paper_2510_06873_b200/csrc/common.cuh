@@ -173,7 +173,7 @@ struct metad_ctx {
     const void *d_pos_last;               // positions snapshot pointer of the last build (chain CVs read it)
     int *d_aux;                           // device scalars: grid-miss flag, index of the hill deposited this step
     // shared-memory tiled fast path (fp32, Q6): tile.cuh / tiled.cu
-    int tiled; int tile_T[3]; int tile_cap;
+    int tiled; int tile_T[3]; int tile_cap; int tile_hx;
     int timing; int capturing; cudaEvent_t ev[3];
     cudaStream_t copy_stream; cudaEvent_t ev_copy;   // metad_step_host: the force upload overlaps the first three stages
     float *d_q6;                          // tiled path: per-atom q6 (sorted order)

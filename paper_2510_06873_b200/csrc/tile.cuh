@@ -17,11 +17,13 @@
 #define TILE_THREADS 256
 #define TILE_MAXROWS 36          // (Ty+2)(Tz+2), Ty,Tz <= 4
 #define TILE_TXMAX 30
+#define TILE_HXMAX 4
 #define TILE_NSEG (3 * TILE_MAXROWS)
 #define TILE_MAXOWN 16           // Ty*Tz
 
 struct TileGeom {
     int Tx, Ty, Tz;              // tile size in cells
+    int hx;                      // halo width along x in cells (= the x-subdivision of the rc-wide cells, api.cu)
     int ntx, nty, ntz;           // tiles per direction
     int nc0, nc1, nc2;           // cells per direction
     int cap;                     // halo capacity (atoms) of the shared-memory staging area
@@ -35,7 +37,7 @@ struct TileTables {
     int seg_off[TILE_NSEG + 1];  // local index of the segment's first atom
     unsigned char seg_wrapped[TILE_NSEG];
     unsigned char seg_code[TILE_NSEG];  // lattice-shift code (wx+1) + 3(wy+1) + 9(wz+1); 13 = no shift
-    unsigned short hcell[TILE_MAXROWS][TILE_TXMAX + 3];   // local index where halo cell (row, lx) starts; [Txe+2] = row end
+    unsigned short hcell[TILE_MAXROWS][TILE_TXMAX + 2 * TILE_HXMAX + 1];   // local index where halo cell (row, lx) starts; [Txe+2] = row end
     int own_g[TILE_MAXOWN];      // global index of the first own atom of own-row q
     int own_l[TILE_MAXOWN];      // local index of the same atom
     int own_off[TILE_MAXOWN + 1];
@@ -54,9 +56,9 @@ __device__ __forceinline__ int tile_row_id(const TileTables &t, int hy, int hz) 
 // Tiles partition each direction evenly (tile k covers cells [k nc / nt, (k+1) nc / nt)), so no sliver tiles.
 // scratch: >= TILE_SCRATCH_BYTES of shared memory that is free during the setup (the position staging area)
 struct TileScratch {
-    int hbeg[TILE_MAXROWS][TILE_TXMAX + 3];    // cell_start[cell]
-    int hend[TILE_MAXROWS][TILE_TXMAX + 3];    // cell_start[cell + 1]
-    int hrel[TILE_MAXROWS][TILE_TXMAX + 3];    // start of the halo cell relative to its segment | piece << 28
+    int hbeg[TILE_MAXROWS][TILE_TXMAX + 2 * TILE_HXMAX + 1];    // cell_start[cell]
+    int hend[TILE_MAXROWS][TILE_TXMAX + 2 * TILE_HXMAX + 1];    // cell_start[cell + 1]
+    int hrel[TILE_MAXROWS][TILE_TXMAX + 2 * TILE_HXMAX + 1];    // start of the halo cell relative to its segment | piece << 28
 };
 #define TILE_SCRATCH_BYTES sizeof(TileScratch)
 __device__ __forceinline__ int tile_cut(int k, int nc, int nt) { return (int)(((long long)k * nc) / nt); }
@@ -69,8 +71,9 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
     const int x0 = tile_cut(tx, g.nc0, g.ntx), y0 = tile_cut(ty, g.nc1, g.nty), z0 = tile_cut(tz, g.nc2, g.ntz);
     const int Txe = tile_cut(tx + 1, g.nc0, g.ntx) - x0, Tye = tile_cut(ty + 1, g.nc1, g.nty) - y0,
               Tze = tile_cut(tz + 1, g.nc2, g.ntz) - z0;
-    const int nrows = (Tye + 2) * (Tze + 2), ncol = Txe + 2;
-    const int xa = x0 - 1, xb = x0 + Txe;
+    const int hx = g.hx;
+    const int nrows = (Tye + 2) * (Tze + 2), ncol = Txe + 2 * hx;
+    const int xa = x0 - hx, xb = x0 + Txe + hx - 1;
     // ---- phase 1: cell_start of every halo cell (both ends); warp 7 fixes the tile origin
     for (int i = tid; i < nrows * ncol; i += blockDim.x) {
         const int r = i / ncol, c = i - r * ncol;
@@ -87,7 +90,7 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
     if (tid >= blockDim.x - 32) {
         // coordinate range of the halo'd tile (8 corners of the parallelepiped, one per lane), origin = point nearest to 0
         const int c = tid & 7;
-        const double fa = (double)(x0 - 1 + ((c & 1) ? Txe + 2 : 0)) / g.nc0;
+        const double fa = (double)(x0 - hx + ((c & 1) ? Txe + 2 * hx : 0)) / g.nc0;
         const double fb = (double)(y0 - 1 + ((c & 2) ? Tye + 2 : 0)) / g.nc1;
         const double fc = (double)(z0 - 1 + ((c & 4) ? Tze + 2 : 0)) / g.nc2;
         double lo[3] = { fa * g.ax + fb * g.bx + fc * g.cx, fb * g.by + fc * g.cy, fc * g.cz }, hi[3];
@@ -157,9 +160,9 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
         if (q < nq) {
             const int oz = q / Tye, oy = q - oz * Tye;
             r = (oz + 1) * (Tye + 2) + (oy + 1);
-            // column 1 (cell x0) always lies in piece 1; column Txe + 1 (cell x0 + Txe) in piece 1 or, at the box end, 2
-            const int v1 = w.hrel[r][Txe + 1];
-            l0 = (w.hrel[r][1] & 0xfffffff) + t.seg_off[3 * r + 1];
+            // column hx (cell x0) always lies in piece 1; column Txe + hx (cell x0 + Txe) in piece 1 or, at the box end, 2
+            const int v1 = w.hrel[r][Txe + hx];
+            l0 = (w.hrel[r][hx] & 0xfffffff) + t.seg_off[3 * r + 1];
             len = (v1 & 0xfffffff) + t.seg_off[3 * r + (v1 >> 28)] - l0;
         }
         int inc = len;

@@ -35,7 +35,7 @@ __device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t,
     const int o = a - t.own_off[q];
     const int li = t.own_l[q] + o, s = t.own_g[q] + o;
     const float4 pi = hpos<STAGED>(g, t, spos, pos_s, li);
-    const int ic = scell[s] % g.nc0 - t.x0 + 1;          // halo-cell column of the own atom
+    const int ic = scell[s] % g.nc0 - t.x0 + g.hx;       // halo-cell column of the own atom
     const int r0 = t.own_row[q], rstride = t.Tye + 2;
     // candidate list written through 32-bit shared-memory addresses (generic 64-bit pointer bumps cost 4 extra
     // instructions per candidate): slot k of this column lives at w0 + k * STRIDE
@@ -48,8 +48,8 @@ __device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t,
 #pragma unroll 1
         for (int dy = -1; dy <= 1; ++dy) {
             const int r = r0 + dz * rstride + dy;
-            int lo = t.hcell[r][ic - 1];
-            const int hi = t.hcell[r][ic + 2];
+            int lo = t.hcell[r][ic - g.hx];
+            const int hi = t.hcell[r][ic + g.hx + 1];
             while (lo < hi) {
                 // every candidate is stored unconditionally and the slot kept only if it passes (load, 6 flop, store,
                 // compare, bump): one free slot is needed, capacity is checked once per stretch
