@@ -62,7 +62,9 @@ __device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t,
                     const float dx = pj.x - pi.x, dy2 = pj.y - pi.y, dz2 = pj.z - pi.z;
                     const float r2 = dx * dx + dy2 * dy2 + dz2 * dz2;
                     asm volatile("st.shared.u16 [%0], %1;" ::"r"(wp), "h"((unsigned short)lj));
-                    wp += (r2 < rc2_hi) ? STRIDE : 0u;
+                    // keep the slot iff the candidate passes: one predicated add (the compiler's select form costs 3)
+                    asm volatile("{ .reg .pred p; setp.lt.f32 p, %1, %2; @p add.u32 %0, %0, %3; }"
+                                 : "+r"(wp) : "f"(r2), "f"(rc2_hi), "r"(STRIDE));
                 }
                 lo = h2;
             }
