@@ -227,8 +227,8 @@ def algo_q6_force_bytes(nb, T):
     return 4 * nb + 4 + 4 * T + 16 * T + 4 + 6 * T
 
 
-def algo_build_flops(nb, cand=113.0):
-    # candidate scan: 3 sub + (1 mul + 2 fma = 5 flop) + 1 compare = 9 flop per candidate (27 cells x 4.2 atoms = 113);
+def algo_build_flops(nb, cand=94.5):
+    # candidate scan: 3 sub + (1 mul + 2 fma = 5 flop) + 1 compare = 9 flop per candidate (9 rows x 2.5 cells x 4.2 atoms = 94.5);
     # fused Q6 pass 1 per neighbour: r2 5, rsqrt 1, unit vector 3, E polynomials 20, (x+iy)^m recurrence 30, 13 fma = 26 -> 85
     return 9.0 * cand + 85.0 * nb
 
