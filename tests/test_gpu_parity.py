@@ -307,3 +307,30 @@ def test_positions_that_round_onto_the_far_box_face_fp32_tiled():
     md.synchronize()
     q_ref = oracle.q6_atoms(p32.astype(np.float64), w.box, cref, lref)
     assert np.abs(md.q6() - q_ref).max() <= 5e-6
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_isolated_atoms_and_empty_cells(precision):
+    """Degenerate cases of the Q6 path: atoms with no neighbour at all (q6 = 0, zero gradient, reading E), atoms with a single
+    neighbour (q6 = 1), and a box that is mostly vacuum (empty cells, empty tiles) — generic fp64 and tiled fp32 paths."""
+    from paper_2510_06873_b200.inputs import CV_Q6_MEAN
+    rng = np.random.default_rng(21)
+    L = 64.0
+    box = np.array([L, 0, 0, 0, L, 0, 0, 0, L], dtype=np.float64)
+    blob = 8.0 + rng.random((1500, 3)) * 18.0                       # dense-ish droplet in one corner: ~0.26 atoms / A^3 -> thin it
+    keep = [0]
+    for i in range(1, len(blob)):                                    # minimum separation 2.0 A
+        if np.min(np.linalg.norm(blob[keep] - blob[i], axis=1)) > 2.0:
+            keep.append(i)
+    blob = blob[keep]
+    lone = np.array([[50.0, 50.0, 50.0], [40.0, 10.0, 55.0], [5.0, 60.0, 33.0]])          # no neighbour within rc
+    pair = np.array([[52.0, 20.0, 20.0], [52.0, 20.0, 22.5]])                              # one neighbour each
+    pos = np.concatenate([blob, lone, pair])
+    w = Workload(name="iso", pos=pos, box=box, rc=3.6, max_neigh=32,
+                 cvs=[CVSpec(kind=CV_Q6_MEAN, scale=1.0 / len(pos))], sigma=[0.01], n_hills=50, precision=precision)
+    r = stagewise(w, precision=precision)
+    assert_stagewise(r)
+    nb = len(blob)
+    assert np.all(r["cnt"][nb:nb + 3] == 0) and np.all(r["cnt"][nb + 3:] == 1)
+    assert np.all(r["q6"][nb:nb + 3] == 0.0) and np.allclose(r["q6"][nb + 3:], 1.0, atol=2e-6)
+    assert np.all(r["F"][nb:nb + 3] == 0.0) and np.all(np.isfinite(r["F"]))
