@@ -170,18 +170,19 @@ k_contacts_cv(int npairs, const int *__restrict__ pairs, const double *__restric
     }
 }
 
-// gather form: one thread per atom that appears in any pair; csr lists its incident pairs.
+// gather form: one WARP per atom that appears in any pair; csr lists its incident pairs, the lanes share them and a
+// fixed shuffle tree sums the lane partials (deterministic; ~1,000 atoms with ~10 pairs each are pure latency otherwise).
 template <typename T>
 __global__ void k_contacts_force(int natoms_touched, const int *__restrict__ atoms, const int *__restrict__ csr_off,
                                  const int *__restrict__ csr_pair, const int *__restrict__ pairs,
                                  const double *__restrict__ pair_r0, int n, int m, double coef /* fs*scale */,
                                  const T *__restrict__ pos, BoxD bd, const double *__restrict__ dVds,
                                  T *__restrict__ F) {
-    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (t >= natoms_touched) return;
     int a = atoms[t];
     double ax = 0.0, ay = 0.0, az = 0.0;
-    for (int q = csr_off[t]; q < csr_off[t + 1]; ++q) {
+    for (int q = csr_off[t] + lane; q < csr_off[t + 1]; q += 32) {
         int p = csr_pair[q];
         int o = pairs[2 * p] == a ? pairs[2 * p + 1] : pairs[2 * p];
         double dx = (double)pos[3 * o] - (double)pos[3 * a], dy = (double)pos[3 * o + 1] - (double)pos[3 * a + 1],
@@ -192,6 +193,13 @@ __global__ void k_contacts_force(int natoms_touched, const int *__restrict__ ato
         double g = dsw / (pair_r0[p] * r);
         ax += g * dx; ay += g * dy; az += g * dz;
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        ax += __shfl_down_sync(0xffffffffu, ax, o);
+        ay += __shfl_down_sync(0xffffffffu, ay, o);
+        az += __shfl_down_sync(0xffffffffu, az, o);
+    }
+    if (lane != 0) return;
     // dQ/dr_a = scale * sum g * (-d_a)  ->  F_a += +fs*scale*dVds * sum g*d_a
     double c = coef * dVds[0];
     F[3 * a] += (T)(c * ax);
@@ -231,7 +239,7 @@ static int chain_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
                                                                         c->p.force_scale, d_dVds + dim, (T *)d_F);
             c->launches++;
         } else if (d.kind == METAD_CV_CONTACTS) {
-            k_contacts_force<T><<<div_up(d.ncatoms, 128), 128, 0, c->stream>>>(
+            k_contacts_force<T><<<div_up((long long)d.ncatoms * 32, 128), 128, 0, c->stream>>>(
                 d.ncatoms, d.d_catoms, d.d_csr_off, d.d_csr_pair, d.d_pairs, d.d_pair_r0, d.n, d.m,
                 c->p.force_scale * d.scale, pos, c->boxd, d_dVds + dim, (T *)d_F);
             c->launches++;
