@@ -1,12 +1,13 @@
-// tiled.cu — fp32 fast path of a1 (neighbour list) fused with a3 (Q6 pass 1), and a6 (Q6 forces),
+// tiled.cu — fp32 fast path of a1 (neighbour list) fused with a3 (Q6 pass 1) or a2 (ungrouped coordination sum)
 // on shared-memory tiles of the cell grid (tile.cuh).  One block per tile; one thread per own atom.
-//   k_tile_build<Q6>  candidate scan from shared memory with no per-pair minimum image: every
+//   k_tile_build<MODE> candidate scan from shared memory with no per-pair minimum image: every
 //                     candidate with r^2 < rc^2(1+1e-5) goes to a per-thread list in shared memory;
 //                     a second loop over that short list takes the exact decision (pairs within the
 //                     1e-5 band are re-decided with the canonical fp64 predicate, reading O), writes
-//                     the neighbour list and — fused — accumulates the atom's 13 q6m components.
-//   k_q6_finish       fixed-order sum of the per-tile partials -> Q6 / solid-like CVs
-//   k_q6_force_g      gather-form forces: per pair two 256-bit loads of the neighbour's q6 record
+//                     the neighbour list and — fused — accumulates the atom's 13 q6m components (MODE 1) or its
+//                     sum of switching functions (MODE 2); MODE 0 builds the list only.
+//   k_q6_publish      hands the sums finished by the last block of k_tile_build to the caller (Q6 / solid-like / C.N.)
+// (the force kernels of this path, k_q6_force_g and k_coord_force_g, live in cv.cu)
 #include <algorithm>
 #include "common.cuh"
 #include "cv_q6.cuh"
