@@ -74,6 +74,9 @@ def lib():
         L.orc_cv_mindist.argtypes = [_I, _P, _P, _P, _P, _I, _P, _D, _P, _P]
         L.orc_cv_lattice.restype = _D
         L.orc_cv_lattice.argtypes = [_P, _I, _P]
+        L.orc_cv_coord_strain.argtypes = [_I, _P, _P, _P, _P, _I, _P, _D, _I, _I, _D, _P]
+        L.orc_q6_strain.argtypes = [_I, _P, _P, _P, _P, _I, _P, _P, _P]
+        L.orc_cv_lattice_strain.argtypes = [_P, _I, _P]
         L.orc_grid_eval_p.restype = _I
         L.orc_grid_eval_p.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P, _P]
         _lib = L
@@ -328,3 +331,26 @@ def cv_lattice(box, axis):
     g = np.zeros(9)
     s = lib().orc_cv_lattice(_p(box), int(axis), _p(g))
     return s, g.reshape(3, 3)
+
+
+# ---- NEXT-3b: strain derivatives d s / d eps (3,3) for the bias virial (PAPER.md:51 NPT; reading AD)
+def cv_coord_strain(pos, box, count, lst, r0, n, m, scale, flags=None):
+    pos, box = _f(pos), _f(box)
+    out = np.zeros(9)
+    lib().orc_cv_coord_strain(len(pos), _p(pos), _p(box), _p(count), _p(lst), lst.shape[1], _p(flags), float(r0), int(n), int(m),
+                              float(scale), _p(out))
+    return out.reshape(3, 3)
+
+
+def q6_strain(pos, box, count, lst, q6, w):
+    pos, box, q6, w = _f(pos), _f(box), _f(q6), _f(w)
+    out = np.zeros(9)
+    lib().orc_q6_strain(len(pos), _p(pos), _p(box), _p(count), _p(lst), lst.shape[1], _p(q6), _p(w), _p(out))
+    return out.reshape(3, 3)
+
+
+def cv_lattice_strain(box, axis):
+    box = _f(box)
+    out = np.zeros(9)
+    lib().orc_cv_lattice_strain(_p(box), int(axis), _p(out))
+    return out.reshape(3, 3)

@@ -821,3 +821,79 @@ double orc_cv_lattice(const double *box, int axis, double *grad9) {
     }
     return s;
 }
+
+/* =============================================================================================
+ * NEXT-3b: bias virial for NPT runs ("ran NPT simulation at 300K and 50 GPa" with the
+ * coordination number and the lattice parameters as CVs).  Reading AD: under a homogeneous strain
+ * eps (r -> r + eps r, box rows h_k -> h_k + eps h_k) every pair vector changes as d -> d + eps d,
+ * so for a CV that is a function of the pair vectors
+ *     d s / d eps_ab = sum over ordered pairs (d s / d d_ij)_a (d_ij)_b ,
+ * and the bias virial is W_ab = - sum_d dV/ds_d * d s_d / d eps_ab (energy units; its contribution
+ * to the pressure tensor is W / volume).  The functions below return d s / d eps (3x3, row-major).  */
+
+/* coordination number: d s/d d_ij = scale * sw'(r/r0)/(r0 r) d_ij for every ordered pair (i in A, j in B). */
+void orc_cv_coord_strain(int N, const double *pos, const double *box, const int *count, const int *list,
+                         int maxn, const unsigned char *flags, double r0, int n, int m, double scale,
+                         double *dsde /*[9]*/) {
+    for (int k = 0; k < 9; ++k) dsde[k] = 0.0;
+    for (int i = 0; i < N; ++i) {
+        if (flags && !(flags[i] & 1)) continue;
+        int c = count[i] < maxn ? count[i] : maxn;
+        for (int k = 0; k < c; ++k) {
+            int j = list[(size_t)i * maxn + k];
+            if (flags && !(flags[j] & 2)) continue;
+            double d[3];
+            orc_delta(box, pos + 3 * i, pos + 3 * j, d);
+            double r = sqrt(r2_of(d));
+            double dsw;
+            orc_switch(r / r0, n, m, &dsw);
+            double g = scale * dsw / (r0 * r);
+            for (int a = 0; a < 3; ++a)
+                for (int b = 0; b < 3; ++b) dsde[3 * a + b] += g * d[a] * d[b];
+        }
+    }
+}
+
+/* E = sum_i w_i q6(i): the per-pair derivative dE/d d_ij is the vector t of orc_q6_grad (same formula). */
+void orc_q6_strain(int N, const double *pos, const double *box, const int *count, const int *list,
+                   int maxn, const double *q6, const double *w, double *dsde /*[9]*/) {
+    for (int k = 0; k < 9; ++k) dsde[k] = 0.0;
+    double (*uu)[3] = (double (*)[3])malloc(sizeof(double) * 3 * (maxn > 0 ? maxn : 1));
+    double *rr = (double *)malloc(sizeof(double) * (maxn > 0 ? maxn : 1));
+    for (int i = 0; i < N; ++i) {
+        int c = count[i] < maxn ? count[i] : maxn;
+        if (c == 0 || !(q6[i] > 0.0) || w[i] == 0.0) continue;
+        for (int k = 0; k < c; ++k) {
+            int j = list[(size_t)i * maxn + k];
+            double d[3];
+            orc_delta(box, pos + 3 * i, pos + 3 * j, d);
+            double r = sqrt(r2_of(d));
+            rr[k] = r;
+            uu[k][0] = d[0] / r; uu[k][1] = d[1] / r; uu[k][2] = d[2] / r;
+        }
+        double pref = w[i] / (2.0 * (double)c * (double)c * q6[i]);
+        for (int j = 0; j < c; ++j) {
+            double g[3] = { 0.0, 0.0, 0.0 };
+            for (int k = 0; k < c; ++k) {
+                if (k == j) continue;
+                double x = uu[j][0] * uu[k][0] + uu[j][1] * uu[k][1] + uu[j][2] * uu[k][2];
+                double dp = 2.0 * dP6(x);
+                g[0] += dp * uu[k][0]; g[1] += dp * uu[k][1]; g[2] += dp * uu[k][2];
+            }
+            double gu = g[0] * uu[j][0] + g[1] * uu[j][1] + g[2] * uu[j][2];
+            for (int a = 0; a < 3; ++a) {
+                double t = pref * (g[a] - gu * uu[j][a]) / rr[j];
+                for (int b = 0; b < 3; ++b) dsde[3 * a + b] += t * rr[j] * uu[j][b];
+            }
+        }
+    }
+    free(uu); free(rr);
+}
+
+/* lattice parameter s = |h_k|: h_k -> h_k + eps h_k  =>  d s/d eps_ab = h_a h_b / |h_k|. */
+void orc_cv_lattice_strain(const double *box, int axis, double *dsde /*[9]*/) {
+    const double *h = box + 3 * axis;
+    double s = sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) dsde[3 * a + b] = h[a] * h[b] / s;
+}

@@ -7,7 +7,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import (apply_forces, bias, bias_periodic, cv_contacts, cv_coord, cv_lattice, cv_mindist, cv_rgyr, cv_torsion, grid_add, grid_add_p,
+from . import (cv_coord_strain, cv_lattice_strain, q6_strain, apply_forces, bias, bias_periodic, cv_contacts, cv_coord, cv_lattice, cv_mindist, cv_rgyr, cv_torsion, grid_add, grid_add_p,
                grid_eval, grid_eval_p, make_flags, neighbors, q6_atoms, q6_grad, wt_height)
 
 # CV kinds — restated (not imported) so the oracle depends on nothing of the product.
@@ -141,6 +141,27 @@ class OracleMetaD:
     def box_force(self, dVds, force_scale=1.0):
         """F_h = -force_scale * sum_d dVds_d * d s_d / d h  (reading AB)."""
         return -force_scale * np.tensordot(np.atleast_1d(dVds), self.box_grads, axes=1)
+
+    def strain_derivatives(self):
+        """d s_d / d eps (D, 3, 3) of the CVs of the last eval_cv (reading AD); NaN for CV kinds without one here."""
+        w, pos, box = self.w, self.pos, self.w.box
+        out = np.full((self.D, 3, 3), np.nan)
+        for d, cv in enumerate(w.cvs):
+            if cv.kind == COORD:
+                fl = make_flags(self.N, cv.group_a, cv.group_b)
+                out[d] = cv_coord_strain(pos, box, self.count, self.list, cv.r0, cv.n, cv.m, cv.scale, fl)
+            elif cv.kind == Q6_MEAN:
+                out[d] = q6_strain(pos, box, self.count, self.list, self.q6, np.full(self.N, cv.scale))
+            elif cv.kind == Q6_SOLID:
+                _, df = logistic(self.q6, cv.q_thresh, cv.q_width)
+                out[d] = q6_strain(pos, box, self.count, self.list, self.q6, cv.scale * df)
+            elif cv.kind == LATTICE:
+                out[d] = cv_lattice_strain(box, cv.n)
+        return out
+
+    def virial(self, dVds, force_scale=1.0):
+        """W = -force_scale * sum_d dVds_d * d s_d / d eps (reading AD)."""
+        return -force_scale * np.tensordot(np.atleast_1d(dVds), self.strain_derivatives(), axes=1)
 
     # -- a7 (readings I, J, U): every `stride` steps append (s, w0*exp(-V/((gamma-1)kT)))
     def deposit(self, s, V):
