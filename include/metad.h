@@ -101,6 +101,9 @@ typedef struct {
                                        (s - s_tau) in PAPER.md:81 is then the nearest-image difference (reading W).
                                        With a grid, a periodic dimension needs grid_hi - grid_lo == period and has
                                        grid_n nodes at lo + i * period / grid_n, no "outside" (reading X).  0: not periodic */
+    int want_virial;                /* != 0: metad_apply_forces also computes the bias virial (metad_get_virial) for NPT runs
+                                       (reading AD).  Supported for COORD, Q6_MEAN, Q6_SOLID and LATTICE
+                                       dimensions; any other CV kind in the context -> METAD_ERR_ARG at create */
 } metad_params;
 
 /* Creates a context on the current CUDA device; `cuda_stream` is a cudaStream_t (NULL = default
@@ -182,6 +185,11 @@ int metad_reweight(metad_ctx *ctx, const double *d_traj, int nframes, const int 
  * of the last metad_apply_forces, h = the box rows; non-zero only for METAD_CV_LATTICE dimensions.  Copied to d_out9
  * (device double[9]); enqueued, not synchronised. */
 int metad_get_box_force(metad_ctx *ctx, double *d_out9);
+
+/* Bias virial of the last metad_apply_forces (needs params.want_virial): W[3][3] = -force_scale * sum_d dVds[d] * d s_d/d eps,
+ * eps = homogeneous strain of positions and box (PAPER.md:51 NPT; reading AD); energy units, its contribution to the pressure
+ * tensor is W / volume.  Copied to d_out9 (device double[9], row-major); enqueued, not synchronised. */
+int metad_get_virial(metad_ctx *ctx, double *d_out9);
 
 /* Resets the step counter (hills stay). */
 int metad_reset_steps(metad_ctx *ctx);

@@ -146,6 +146,16 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     }
 
     if (c->has_mindist) CUDA_TRY(dev_alloc(&c->d_mind, 8));
+    if (p->want_virial) {
+        for (int d = 0; d < c->D; ++d) {
+            const int k = c->cv[d].kind;
+            if (k != METAD_CV_COORD && k != METAD_CV_Q6_MEAN && k != METAD_CV_Q6_SOLID && k != METAD_CV_LATTICE)
+                FAIL(METAD_ERR_ARG, "want_virial supports COORD, Q6_MEAN, Q6_SOLID and LATTICE dimensions only");
+        }
+        CUDA_TRY(dev_alloc(&c->d_virial, 9));
+        CUDA_TRY(cudaMemset(c->d_virial, 0, sizeof(double) * 9));
+        CUDA_TRY(dev_alloc(&c->d_vir_partials, 9 * ((size_t)div_up(N, 128) + 1)));
+    }
     CUDA_TRY(dev_alloc(&c->d_cvq6, 2));
     CUDA_TRY(dev_alloc(&c->d_box_force, 9));
     CUDA_TRY(cudaMemset(c->d_box_force, 0, sizeof(double) * 9));
@@ -232,7 +242,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
@@ -528,6 +538,13 @@ extern "C" int metad_reweight(metad_ctx *c, const double *d_traj, int nframes, c
 extern "C" int metad_get_box_force(metad_ctx *c, double *d_out9) {
     if (!c || !d_out9) FAIL(METAD_ERR_ARG, "null argument");
     CUDA_TRY(cudaMemcpyAsync(d_out9, c->d_box_force, sizeof(double) * 9, cudaMemcpyDeviceToDevice, c->stream));
+    return METAD_OK;
+}
+
+extern "C" int metad_get_virial(metad_ctx *c, double *d_out9) {
+    if (!c || !d_out9) FAIL(METAD_ERR_ARG, "null argument");
+    if (!c->p.want_virial) FAIL(METAD_ERR_STATE, "params.want_virial was not set");
+    CUDA_TRY(cudaMemcpyAsync(d_out9, c->d_virial, sizeof(double) * 9, cudaMemcpyDeviceToDevice, c->stream));
     return METAD_OK;
 }
 

@@ -110,6 +110,33 @@ __device__ __forceinline__ bool last_block_ticket(unsigned int *ticket) {
     return is_last;
 }
 
+// Bias virial (NEXT-3b, reading AD): every thread of the block hands in its 9 partial sums of G_a d_b over the pairs
+// it visited; fixed-order block reduction, per-block partials, the last block adds coef * dv * sum to out9.
+struct VirArgs { double *partials; unsigned int *ticket; double *out9; };
+__device__ __forceinline__ void virial_finish(double (&w)[9], double *smem /* >= 9*32 doubles */, const VirArgs &va,
+                                              double coef, const double *dv /* device scalar or NULL */) {
+    block_reduce<9>(w, smem);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < 9; ++k) va.partials[(size_t)blockIdx.x * 9 + k] = w[k];
+    }
+    if (last_block_ticket(va.ticket)) {
+        double t[9];
+#pragma unroll
+        for (int k = 0; k < 9; ++k) t[k] = 0.0;
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) {
+#pragma unroll
+            for (int k = 0; k < 9; ++k) t[k] += va.partials[(size_t)b * 9 + k];
+        }
+        block_reduce<9>(t, smem);
+        if (threadIdx.x == 0) {
+            const double f = coef * (dv ? dv[0] : 1.0);
+#pragma unroll
+            for (int k = 0; k < 9; ++k) va.out9[k] += f * t[k];
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // Host-side context
 struct CvDev {                      // device copies of one CV descriptor
@@ -143,6 +170,7 @@ struct metad_ctx {
     // CV state
     CvDev cv[METAD_MAX_CV];
     bool has_q6, has_coord, has_torsion, has_mindist, has_lattice;
+    double *d_virial, *d_vir_partials;    // want_virial: [9] bias virial of the last apply_forces; per-block partials
     double *d_box_force;                  // LATTICE: [9] bias force on the box rows, written by apply_forces
     int mindist_dim;
     double *d_mind;                       // MINDIST: [r, dx, dy, dz] of the nearest pair + its two original indices (as int pair)

@@ -50,17 +50,25 @@ k_coord_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
     }
 }
 
-template <typename T>
+// VIRIAL: the same pass also sums g d_a d_b over the visited pairs (every unordered pair is visited from both ends, hence
+// the factor 1/2): W = -1/2 force_scale scale dV/ds sum_k sum_j g d d^T (reading AD).
+template <typename T, bool VIRIAL>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
               const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, T inv_r0, int n, int m,
-              double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F) {
+              double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F, VirArgs va) {
+    __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
     int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
+    if (!VIRIAL && s >= N) return;
+    const bool act = s < N;
+    if (!act) s = N - 1;                       // idle thread of the virial instance: valid addresses, zero trip count
+    T wv[9];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) wv[q] = T(0);
     typename Vec4<T>::type pi = spos[s];
     const int fi = (int)pi.w;
     T ax = T(0), ay = T(0), az = T(0);
-    int cnt = nl_count[s];
+    int cnt = act ? nl_count[s] : 0;
     for (int k = 0; k < cnt; ++k) {
         int j = nl[(size_t)k * N + s];
         typename Vec4<T>::type pj = spos[j];
@@ -73,13 +81,27 @@ k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int 
         switch_fn<T>(r * inv_r0, n, m, dsw);
         T g = T(mult) * dsw * inv_r0 / r;
         ax += g * dx; ay += g * dy; az += g * dz;
+        if (VIRIAL) {
+            const T gx = g * dx, gy = g * dy, gz = g * dz;
+            wv[0] += gx * dx; wv[1] += gx * dy; wv[2] += gx * dz;
+            wv[3] += gy * dx; wv[4] += gy * dy; wv[5] += gy * dz;
+            wv[6] += gz * dx; wv[7] += gz * dy; wv[8] += gz * dz;
+        }
     }
     // ds/dr_k = scale * sum g * (-d)  ->  F_k += -fs*dVds*ds/dr_k = +fs*scale*dVds * sum g*d
-    const double a = coef * dVds[0];
-    const int i = perm[s];
-    F[3 * i] += (T)(a * (double)ax);
-    F[3 * i + 1] += (T)(a * (double)ay);
-    F[3 * i + 2] += (T)(a * (double)az);
+    if (act) {
+        const double a = coef * dVds[0];
+        const int i = perm[s];
+        F[3 * i] += (T)(a * (double)ax);
+        F[3 * i + 1] += (T)(a * (double)ay);
+        F[3 * i + 2] += (T)(a * (double)az);
+    }
+    if (VIRIAL) {
+        double w[9];
+#pragma unroll
+        for (int q = 0; q < 9; ++q) w[q] = (double)wv[q];
+        virial_finish(w, vsm, va, -0.5 * coef, dVds);
+    }
 }
 
 // Warp-per-atom variants for small systems (N <= METAD_WARP_PER_ATOM_MAX): the lanes share an atom's neighbours, a fixed
@@ -241,15 +263,21 @@ k_q6_pass1(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
 
 // Q6 pass 2 (gather form, reading E):  F_k += fs * sum_{j in N(k)} grad_d [ (g_k B(k) + g_j B(j)) . y ](d_kj),
 // g_i = alpha + beta f'(q6_i), alpha = dVds[mean]*scale_mean, beta = dVds[solid]*scale_solid.
-template <typename T>
+template <typename T, bool VIRIAL>
 __global__ void __launch_bounds__(CV_THREADS)
 k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
            const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, const T *__restrict__ rec,
            double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
-           const double *__restrict__ dVds, T *__restrict__ F) {
+           const double *__restrict__ dVds, T *__restrict__ F, VirArgs va) {
     typedef typename Vec4<T>::type V4;
+    __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
     int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
+    if (!VIRIAL && s >= N) return;
+    const bool act = s < N;
+    if (!act) s = N - 1;
+    T wv[9];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) wv[q] = T(0);
     const T alpha = dim_mean >= 0 ? (T)(dVds[dim_mean] * scale_mean) : T(0);
     const T beta = dim_solid >= 0 ? (T)(dVds[dim_solid] * scale_solid) : T(0);
     V4 pi = spos[s];
@@ -264,7 +292,7 @@ k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
         Bk[12] = gk * d.x;
     }
     T ax = T(0), ay = T(0), az = T(0);
-    int cnt = nl_count[s];
+    int cnt = act ? nl_count[s] : 0;
     for (int k = 0; k < cnt; ++k) {
         int j = nl[(size_t)k * N + s];
         V4 pj = spos[j];
@@ -285,14 +313,26 @@ k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
         T gx, gy, gz;
         y6_grad<T>(y, bb, gx, gy, gz);
         T gu = gx * ux + gy * uy + gz * uz;     // project onto the tangent plane, divide by r
-        ax += (gx - gu * ux) * rinv;
-        ay += (gy - gu * uy) * rinv;
-        az += (gz - gu * uz) * rinv;
+        const T tx = (gx - gu * ux) * rinv, ty = (gy - gu * uy) * rinv, tz = (gz - gu * uz) * rinv;
+        ax += tx; ay += ty; az += tz;
+        if (VIRIAL) {
+            wv[0] += tx * dx; wv[1] += tx * dy; wv[2] += tx * dz;
+            wv[3] += ty * dx; wv[4] += ty * dy; wv[5] += ty * dz;
+            wv[6] += tz * dx; wv[7] += tz * dy; wv[8] += tz * dz;
+        }
     }
-    const int i = perm[s];
-    F[3 * i] += (T)(force_scale * (double)ax);
-    F[3 * i + 1] += (T)(force_scale * (double)ay);
-    F[3 * i + 2] += (T)(force_scale * (double)az);
+    if (act) {
+        const int i = perm[s];
+        F[3 * i] += (T)(force_scale * (double)ax);
+        F[3 * i + 1] += (T)(force_scale * (double)ay);
+        F[3 * i + 2] += (T)(force_scale * (double)az);
+    }
+    if (VIRIAL) {                               // alpha, beta already carry dV/ds: W = -1/2 force_scale sum t d^T
+        double w[9];
+#pragma unroll
+        for (int q = 0; q < 9; ++q) w[q] = (double)wv[q];
+        virial_finish(w, vsm, va, -0.5 * force_scale, nullptr);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -311,14 +351,20 @@ __device__ __forceinline__ void ldg256(const float *p, float4 &a, float4 &b) {
 #ifndef Q6F_MINB
 #define Q6F_MINB 9
 #endif
-template <bool SOLID>
-__global__ void __launch_bounds__(CV_THREADS, Q6F_MINB)
+template <bool SOLID, bool VIRIAL>
+__global__ void __launch_bounds__(CV_THREADS, VIRIAL ? 4 : Q6F_MINB)
 k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
              const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, const float *__restrict__ rec,
              double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
-             const double *__restrict__ dVds, float *__restrict__ F) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
+             const double *__restrict__ dVds, float *__restrict__ F, VirArgs va) {
+    __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (!VIRIAL && s >= N) return;
+    const bool act = s < N;
+    if (!act) s = N - 1;                       // idle thread of the virial instance: valid addresses, zero trip count
+    float wv[9];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) wv[q] = 0.f;
     const float alpha = dim_mean >= 0 ? (float)(dVds[dim_mean] * scale_mean) : 0.f;
     const float beta = dim_solid >= 0 ? (float)(dVds[dim_solid] * scale_solid) : 0.f;
     const float4 pi = spos[s];
@@ -334,7 +380,7 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         Bk[12] = gk * d4.x;
     }
     const int *in = nl + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
-    const int cnt = nl_count[s];
+    const int cnt = act ? nl_count[s] : 0;
     float fx = 0.f, fy = 0.f, fz = 0.f;
     for (int k = 0; k < cnt; ++k) {
         const int e = __ldcs(in + k * 32);            // streamed once: do not displace positions / records in L2
@@ -364,25 +410,46 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         float gx, gy, gz;
         y6_grad<float>(y, bb, gx, gy, gz);
         const float gu = gx * ux + gy * uy + gz * uz;
-        fx += (gx - gu * ux) * rinv; fy += (gy - gu * uy) * rinv; fz += (gz - gu * uz) * rinv;
+        const float tx = (gx - gu * ux) * rinv, ty = (gy - gu * uy) * rinv, tz = (gz - gu * uz) * rinv;
+        fx += tx; fy += ty; fz += tz;
+        if (VIRIAL) {
+            wv[0] += tx * dx; wv[1] += tx * dy; wv[2] += tx * dz;
+            wv[3] += ty * dx; wv[4] += ty * dy; wv[5] += ty * dz;
+            wv[6] += tz * dx; wv[7] += tz * dy; wv[8] += tz * dz;
+        }
     }
-    const int i = perm[s];
-    F[3 * i] += (float)(force_scale * (double)fx);
-    F[3 * i + 1] += (float)(force_scale * (double)fy);
-    F[3 * i + 2] += (float)(force_scale * (double)fz);
+    if (act) {
+        const int i = perm[s];
+        F[3 * i] += (float)(force_scale * (double)fx);
+        F[3 * i + 1] += (float)(force_scale * (double)fy);
+        F[3 * i + 2] += (float)(force_scale * (double)fz);
+    }
+    if (VIRIAL) {                               // alpha, beta already carry dV/ds: W = -1/2 force_scale sum t d^T
+        double w[9];
+#pragma unroll
+        for (int q = 0; q < 9; ++q) w[q] = (double)wv[q];
+        virial_finish(w, vsm, va, -0.5 * force_scale, nullptr);
+    }
 }
 
 // Coordination-number forces on the tiled fp32 path (ungrouped: every ordered pair counts, i.e. each pair twice in
 // d s/d r_k): thread per atom, gather form over the sliced list; per pair one 128-bit position load.
+template <bool VIRIAL>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
                 const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, float inv_r0, int n, int m,
-                double coef /* force_scale * scale */, const double *__restrict__ dVds, float *__restrict__ F) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
+                double coef /* force_scale * scale */, const double *__restrict__ dVds, float *__restrict__ F, VirArgs va) {
+    __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (!VIRIAL && s >= N) return;
+    const bool act = s < N;
+    if (!act) s = N - 1;
+    float wv[9];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) wv[q] = 0.f;
     const float4 pi = spos[s];
     const int *in = nl + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
-    const int cnt = nl_count[s];
+    const int cnt = act ? nl_count[s] : 0;
     float ax = 0.f, ay = 0.f, az = 0.f;
     for (int k = 0; k < cnt; ++k) {
         const int e = __ldcs(in + k * 32);            // streamed once: do not displace positions / records in L2
@@ -400,19 +467,39 @@ k_coord_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__r
         switch_fn<float>(r2 * rinv * inv_r0, n, m, dsw);
         const float g = 2.f * dsw * inv_r0 * rinv;
         ax += g * dx; ay += g * dy; az += g * dz;
+        if (VIRIAL) {
+            const float gx = g * dx, gy = g * dy, gz = g * dz;
+            wv[0] += gx * dx; wv[1] += gx * dy; wv[2] += gx * dz;
+            wv[3] += gy * dx; wv[4] += gy * dy; wv[5] += gy * dz;
+            wv[6] += gz * dx; wv[7] += gz * dy; wv[8] += gz * dz;
+        }
     }
-    const double a = coef * dVds[0];
-    const int i = perm[s];
-    F[3 * i] += (float)(a * (double)ax);
-    F[3 * i + 1] += (float)(a * (double)ay);
-    F[3 * i + 2] += (float)(a * (double)az);
+    if (act) {
+        const double a = coef * dVds[0];
+        const int i = perm[s];
+        F[3 * i] += (float)(a * (double)ax);
+        F[3 * i + 1] += (float)(a * (double)ay);
+        F[3 * i + 2] += (float)(a * (double)az);
+    }
+    if (VIRIAL) {
+        double w[9];
+#pragma unroll
+        for (int q = 0; q < 9; ++q) w[q] = (double)wv[q];
+        virial_finish(w, vsm, va, -0.5 * coef, dVds);
+    }
 }
 
 int tiled_coord_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     const CvDev &d = c->cv[c->coord_dim];
-    k_coord_force_g<<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
-        c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (float)(1.0 / d.r0), d.n, d.m,
-        c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F);
+    const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
+    if (c->p.want_virial)
+        k_coord_force_g<true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+            c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (float)(1.0 / d.r0), d.n, d.m,
+            c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F, va);
+    else
+        k_coord_force_g<false><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+            c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (float)(1.0 / d.r0), d.n, d.m,
+            c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F, va);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -421,14 +508,14 @@ int tiled_coord_force(metad_ctx *c, const double *d_dVds, void *d_F) {
 int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
     double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
-    if (c->q6_solid_dim >= 0)
-        k_q6_force_g<true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
-            c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm,
-            ss, c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F);
-    else
-        k_q6_force_g<false><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
-            c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm,
-            ss, c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F);
+    const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
+#define Q6FG_LAUNCH(SOLID, VIR)                                                                                            \
+    k_q6_force_g<SOLID, VIR><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(                                      \
+        c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm, \
+        ss, c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va)
+    if (c->q6_solid_dim >= 0) { if (c->p.want_virial) Q6FG_LAUNCH(true, true); else Q6FG_LAUNCH(true, false); }
+    else { if (c->p.want_virial) Q6FG_LAUNCH(false, true); else Q6FG_LAUNCH(false, false); }
+#undef Q6FG_LAUNCH
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -637,14 +724,19 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
         if (r) return r;
     } else if (c->has_coord) {
         const CvDev &d = c->cv[c->coord_dim];
-        if (N <= METAD_WARP_PER_ATOM_MAX)
+        const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
+        if (c->p.want_virial)                                 // forces and virial in one thread-per-atom pass
+            k_coord_force<T, true><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
+                                                                    pb, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
+                                                                    d_dVds + c->coord_dim, (T *)d_F, va);
+        else if (N <= METAD_WARP_PER_ATOM_MAX)
             k_coord_force_warp<T><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
                 N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, (T)(1.0 / d.r0), d.n, d.m,
                 c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F);
         else
-        k_coord_force<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
-                                                          pb, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
-                                                          d_dVds + c->coord_dim, (T *)d_F);
+            k_coord_force<T, false><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
+                                                                     pb, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
+                                                                     d_dVds + c->coord_dim, (T *)d_F, va);
         c->launches++;
     }
     if (c->has_q6 && c->tiled) {
@@ -653,15 +745,22 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
     } else if (c->has_q6) {
         double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
         double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
-        k_q6_force<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb,
-                                                       (const T *)c->d_rec, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
-                                                       c->p.force_scale, d_dVds, (T *)d_F);
+        const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
+        if (c->p.want_virial)
+            k_q6_force<T, true><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb,
+                                                                 (const T *)c->d_rec, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
+                                                                 c->p.force_scale, d_dVds, (T *)d_F, va);
+        else
+            k_q6_force<T, false><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb,
+                                                                  (const T *)c->d_rec, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
+                                                                  c->p.force_scale, d_dVds, (T *)d_F, va);
         c->launches++;
     }
     return METAD_OK;
 }
 
 int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F) {
+    if (c->p.want_virial) CUDA_TRY(cudaMemsetAsync(c->d_virial, 0, sizeof(double) * 9, c->stream));
     int rcode = c->prec == 32 ? cv_forces_t<float>(c, d_dVds, d_F) : cv_forces_t<double>(c, d_dVds, d_F);
     if (rcode) return rcode;
     rcode = chain_forces(c, d_dVds, d_F);

@@ -341,10 +341,19 @@ __global__ void k_lattice_cv(int D, LatTable lt, double *__restrict__ cv_out) {
 }
 
 __global__ void k_lattice_force(int D, LatTable lt, double force_scale, const double *__restrict__ dVds,
-                                double *__restrict__ fbox) {
+                                double *__restrict__ fbox, double *__restrict__ virial /* NULL: not wanted */) {
     const int e = threadIdx.x;              // box element (row, component)
     if (e >= 9) return;
     const int row = e / 3;
+    if (virial) {                           // d|h_k|/d eps_ab = h_a h_b / |h_k| (reading AD); e = (a, b)
+        double w = 0.0;
+        for (int d = 0; d < D; ++d) {
+            if (lt.kind[d] != METAD_CV_LATTICE) continue;
+            const double *h = lt.h + 3 * lt.axis[d];
+            w += dVds[d] * h[e / 3] * h[e % 3] / sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
+        }
+        virial[e] += -force_scale * w;
+    }
     double f = 0.0;
     for (int d = 0; d < D; ++d) {
         if (lt.kind[d] != METAD_CV_LATTICE || lt.axis[d] != row) continue;
@@ -373,7 +382,8 @@ int lattice_eval(metad_ctx *c, double *d_cv) {
 
 int lattice_forces(metad_ctx *c, const double *d_dVds) {
     if (!c->has_lattice) return METAD_OK;
-    k_lattice_force<<<1, 32, 0, c->stream>>>(c->D, lat_table(c), c->p.force_scale, d_dVds, c->d_box_force);
+    k_lattice_force<<<1, 32, 0, c->stream>>>(c->D, lat_table(c), c->p.force_scale, d_dVds, c->d_box_force,
+                                            c->p.want_virial ? c->d_virial : nullptr);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

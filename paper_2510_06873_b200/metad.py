@@ -36,13 +36,13 @@ class Params(ctypes.Structure):
     _fields_ = [("natoms", _I), ("precision", _I), ("max_neigh", _I), ("ncv", _I),
                 ("cv", CvDesc * MAX_CV), ("sigma", _D * MAX_CV), ("w0", _D), ("kT", _D),
                 ("bias_factor", _D), ("max_hills", _I), ("stride", _I), ("grid_n", _I * 2),
-                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV)]
+                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("want_virial", _I)]
 
 
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
            "metad_apply_forces", "metad_deposit", "metad_run", "metad_step_host", "metad_status",
            "metad_get_state", "metad_get_neighbors", "metad_get_q6", "metad_set_hills", "metad_get_hills",
-           "metad_get_grid", "metad_get_box_force", "metad_bias_batch", "metad_reweight", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
+           "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
 
 _lib = None
 
@@ -74,6 +74,7 @@ def load():
     L.metad_get_grid.argtypes = [_P, _P]
     L.metad_reset_steps.argtypes = [_P]
     L.metad_get_box_force.argtypes = [_P, _P]
+    L.metad_get_virial.argtypes = [_P, _P]
     L.metad_bias_batch.argtypes = [_P, _P, _I, _P]
     L.metad_reweight.argtypes = [_P, _P, _I, _P, _P, _P, _P, _P]
     L.metad_set_timing.argtypes = [_P, _I]
@@ -106,7 +107,7 @@ class MetaD:
     fields); tensors passed to the methods are torch CUDA tensors (float64, or float32 for pos/F when
     precision == 32)."""
 
-    def __init__(self, workload, max_hills=None, precision=None, grid=None, force_scale=1.0, stream=None):
+    def __init__(self, workload, max_hills=None, precision=None, grid=None, force_scale=1.0, stream=None, want_virial=False):
         import torch
         self.torch = torch
         L = load()
@@ -156,6 +157,7 @@ class MetaD:
         else:
             self.grid_n = None
         p.force_scale = float(force_scale)
+        p.want_virial = 1 if want_virial else 0
         self._params = p
         h = _P()
         _check(L.metad_create(ctypes.byref(h), ctypes.byref(p), _P(self.stream.cuda_stream)))
@@ -273,6 +275,13 @@ class MetaD:
         """Bias force on the box rows (3,3) of the last apply_forces (lattice-parameter CVs)."""
         t = self.torch.empty(9, dtype=self.torch.float64, device="cuda")
         _check(load().metad_get_box_force(self._h, _ptr(t)))
+        self.synchronize()
+        return t.cpu().numpy().reshape(3, 3)
+
+    def virial(self):
+        """Bias virial W (3,3) of the last apply_forces (needs want_virial=True; PAPER.md:51 NPT, reading AD)."""
+        t = self.torch.empty(9, dtype=self.torch.float64, device="cuda")
+        _check(load().metad_get_virial(self._h, _ptr(t)))
         self.synchronize()
         return t.cpu().numpy().reshape(3, 3)
 

@@ -45,7 +45,7 @@ def make_hills(w, s_ref, seed=5):
     return c, seeded_heights(seed, w.n_hills, w.w0)
 
 
-def stagewise(w, precision=None, threads=None):
+def stagewise(w, precision=None, threads=None, want_virial=False):
     """Runs both sides stage by stage (reading S): the oracle's s feeds the GPU bias, the oracle's
     dV/ds feeds the GPU forces.  Returns a dict of reference / measured arrays."""
     import torch
@@ -60,7 +60,7 @@ def stagewise(w, precision=None, threads=None):
     V_ref, dV_ref = o.bias(s_ref, use_grid=False)
     F_ref = o.forces(dV_ref)
 
-    md = MetaD(w, precision=precision, max_hills=len(heights) + 16)
+    md = MetaD(w, precision=precision, max_hills=len(heights) + 16, want_virial=want_virial)
     tdt = torch.float32 if precision == 32 else torch.float64
     with torch.cuda.stream(md.stream):
         dpos = torch.tensor(pos, device="cuda", dtype=tdt)

@@ -1,0 +1,59 @@
+"""-m gpu: bias virial for NPT (reading AD) of the CUDA path against the oracle's strain derivatives."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2510_06873_b200.inputs import (CV_COORD, CV_LATTICE, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CVSpec,  # noqa: E402
+                                          configs)
+
+from gpu_util import assert_stagewise, stagewise  # noqa: E402
+
+
+def _check(w, precision, tol):
+    r = stagewise(w, precision=precision, want_virial=True)
+    assert_stagewise(r)
+    W = r["md"].virial()
+    W_ref = r["o"].virial(r["dV_ref"])
+    assert np.abs(W_ref).max() > 0
+    assert np.abs(W - W_ref).max() <= tol * np.abs(W_ref).max(), (W, W_ref)
+    assert np.abs(W - W.T).max() <= 10 * tol * np.abs(W_ref).max()          # rotation-invariant CVs: symmetric virial
+    return r, W
+
+
+@pytest.mark.parametrize("precision,tol", [(64, 1e-9), (32, 1e-5)])
+def test_virial_generic_path_four_cvs(precision, tol):
+    """Coordination number + Q6 mean + solid-like count + lattice parameter c in one context (generic kernels)."""
+    w = configs.small("c3")
+    N = w.natoms
+    w.cvs = [CVSpec(kind=CV_COORD, r0=2.4, n=6, m=12, scale=1.0 / N), CVSpec(kind=CV_Q6_MEAN, scale=1.0 / N),
+             CVSpec(kind=CV_Q6_SOLID, scale=1.0, q_thresh=0.25, q_width=0.05), CVSpec(kind=CV_LATTICE, n=2)]
+    w.sigma = [0.05, 0.005, 20.0, 0.2]
+    w.n_hills = 200
+    _check(w, precision, tol)
+
+
+@pytest.mark.parametrize("solid", [False, True])
+def test_virial_tiled_q6(solid):
+    w = configs.small("c4" if solid else "c3")                 # c4: Q6 mean + solid-like count; c3: Q6 mean only
+    r, W = _check(w, 32, 1e-5)
+    if not solid:
+        assert abs(np.trace(W)) <= 1e-4 * np.abs(W).max()      # Q6 is scale-invariant: traceless virial
+
+
+def test_virial_tiled_coordination_and_lattice():
+    w = configs.small("g0")                                    # PAPER.md:51 CV set: C.N. + a, b, c
+    r, W = _check(w, 32, 1e-5)
+    assert np.trace(W) != 0.0
+
+
+def test_virial_needs_the_flag_and_supported_cvs():
+    from paper_2510_06873_b200.metad import MetaD, MetadError
+    w = configs.small("c3")
+    md = MetaD(w)
+    with pytest.raises(MetadError):
+        md.virial()
+    w1 = configs.small("c1")
+    assert any(cv.kind == CV_RGYR for cv in w1.cvs)
+    with pytest.raises(MetadError):
+        MetaD(w1, want_virial=True)
