@@ -40,6 +40,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fast-setup", action="store_true",
                     help="profiling runs only: seeded hill heights instead of the well-tempered replay, no e2e leg")
+    ap.add_argument("--virial", action="store_true", help="also compute the bias virial every step (NPT; COORD / Q6 / LATTICE CVs)")
     ap.add_argument("--stage-times", action="store_true", default=True)
     return ap.parse_args()
 
@@ -56,7 +57,7 @@ def describe(w, precision):
           }.get(w.name, f"BASELINE.json configs[{w.name[1]}] ({w.name})")
     return {"workload": wl, "atoms": int(w.natoms),
             "cvs": [kinds[c.kind] for c in w.cvs], "hills": int(w.n_hills), "rc": w.rc,
-            "pair_precision": f"fp{precision}", "stride": int(w.stride),
+            "pair_precision": f"fp{precision}", "stride": int(w.stride), "virial": bool(getattr(w, "_virial", False)),
             "l2": ("per-step working set (neighbour list + q6 records + positions + forces) exceeds the 126 MB L2; no flush"
                    if w.natoms * (4 * w.max_neigh + 64 + 16 + 24 + 16) > 126e6 else
                    "working set fits the 126 MB L2 and is not flushed: this workload is bound by the latency of its ~10 "
@@ -252,6 +253,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     w = workload(args.config)
+    w._virial = bool(args.virial)
     precision = args.precision or (32 if args.config in ("c3", "c4", "g0") else w.precision)
     tdt = torch.float32 if precision == 32 else torch.float64
     pos = w.pos.astype(np.float32 if precision == 32 else np.float64)
@@ -275,7 +277,8 @@ def run_ours(args):
     elif w.grid_n[0]:
         sig = np.asarray(w.sigma)
         grid = (w.grid_n, centers[0] - 120 * sig, centers[0] + 120 * sig)      # reading M
-    md = MetaD(w, precision=precision, max_hills=w.n_hills + args.steps + args.warmup + 4096, grid=grid)
+    md = MetaD(w, precision=precision, max_hills=w.n_hills + args.steps + args.warmup + 4096, grid=grid,
+               want_virial=args.virial)
     md.set_hills(centers, heights)
     with torch.cuda.stream(md.stream):
         F = torch.zeros((w.natoms, 3), device="cuda", dtype=tdt)

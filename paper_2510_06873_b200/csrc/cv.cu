@@ -352,7 +352,7 @@ __device__ __forceinline__ void ldg256(const float *p, float4 &a, float4 &b) {
 #define Q6F_MINB 9
 #endif
 template <bool SOLID, bool VIRIAL>
-__global__ void __launch_bounds__(CV_THREADS, VIRIAL ? 4 : Q6F_MINB)
+__global__ void __launch_bounds__(CV_THREADS, VIRIAL ? 8 : Q6F_MINB)
 k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
              const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, const float *__restrict__ rec,
              double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
