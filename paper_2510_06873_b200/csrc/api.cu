@@ -382,7 +382,6 @@ extern "C" int metad_run(metad_ctx *c, const void *d_pos, const double *h_box, d
     bool same = c->graph_exec && c->graph_pos == d_pos && c->graph_F == d_F && c->graph_rc == rc &&
                 memcmp(c->graph_box, h_box, sizeof(double) * 9) == 0;
     if (!same) {
-        if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         int r = setup_geometry(c, h_box, rc);     // argument errors surface before the capture starts
         if (r) return r;
         long long before = c->launches;
@@ -394,7 +393,15 @@ extern "C" int metad_run(metad_ctx *c, const void *d_pos, const double *h_box, d
         cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
         if (r) { if (e == cudaSuccess) cudaGraphDestroy(graph); return r; }
         CUDA_TRY(e);
-        CUDA_TRY(cudaGraphInstantiate(&c->graph_exec, graph, 0));
+        // a changed box (NPT) or pointer changes kernel arguments and grid sizes, not the topology: update the
+        // instantiated graph in place when the driver allows it, re-instantiate otherwise
+        bool updated = false;
+        if (c->graph_exec) {
+            cudaGraphExecUpdateResultInfo info;
+            if (cudaGraphExecUpdate(c->graph_exec, graph, &info) == cudaSuccess) updated = true;
+            else { cudaGetLastError(); cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+        }
+        if (!updated) CUDA_TRY(cudaGraphInstantiate(&c->graph_exec, graph, 0));
         cudaGraphDestroy(graph);
         c->launches_per_step = (int)(c->launches - before);
         c->launches = before;                      // capture enqueued nothing
