@@ -77,6 +77,10 @@ def lib():
         L.orc_cv_coord_strain.argtypes = [_I, _P, _P, _P, _P, _I, _P, _D, _I, _I, _D, _P]
         L.orc_q6_strain.argtypes = [_I, _P, _P, _P, _P, _I, _P, _P, _P]
         L.orc_cv_lattice_strain.argtypes = [_P, _I, _P]
+        L.orc_cv_rgyr_strain.argtypes = [_I, _P, _P, _P, _P, _P]
+        L.orc_cv_contacts_strain.argtypes = [_I, _P, _P, _I, _I, _D, _P, _P, _P]
+        L.orc_cv_mindist_strain.argtypes = [_I, _P, _P, _P, _P, _I, _P, _D, _P]
+        L.orc_cv_torsion_strain.argtypes = [_P, _P, _P, _P]
         L.orc_grid_eval_p.restype = _I
         L.orc_grid_eval_p.argtypes = [_I, _I, _P, _P, _P, _P, _P, _P, _P]
         _lib = L
@@ -353,4 +357,33 @@ def cv_lattice_strain(box, axis):
     box = _f(box)
     out = np.zeros(9)
     lib().orc_cv_lattice_strain(_p(box), int(axis), _p(out))
+    return out.reshape(3, 3)
+
+
+def cv_rgyr_strain(pos, box, chain, mass=None):
+    pos, box, chain = _f(pos), _f(box), _i(chain)
+    mass = None if mass is None else _f(mass)
+    out = np.zeros(9)
+    lib().orc_cv_rgyr_strain(len(chain), _p(chain), _p(mass), _p(pos), _p(box), _p(out))
+    return out.reshape(3, 3)
+
+
+def cv_contacts_strain(pos, box, pairs, pair_r0, n, m, scale):
+    pos, box, pairs, pair_r0 = _f(pos), _f(box), _i(pairs), _f(pair_r0)
+    out = np.zeros(9)
+    lib().orc_cv_contacts_strain(len(pairs), _p(pairs), _p(pair_r0), int(n), int(m), float(scale), _p(pos), _p(box), _p(out))
+    return out.reshape(3, 3)
+
+
+def cv_mindist_strain(pos, box, count, lst, rc, flags=None):
+    pos, box = _f(pos), _f(box)
+    out = np.zeros(9)
+    lib().orc_cv_mindist_strain(len(pos), _p(pos), _p(box), _p(count), _p(lst), lst.shape[1], _p(flags), float(rc), _p(out))
+    return out.reshape(3, 3)
+
+
+def cv_torsion_strain(pos, box, idx):
+    pos, box, idx = _f(pos), _f(box), _i(idx)
+    out = np.zeros(9)
+    lib().orc_cv_torsion_strain(_p(idx), _p(pos), _p(box), _p(out))
     return out.reshape(3, 3)

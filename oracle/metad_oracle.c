@@ -897,3 +897,62 @@ void orc_cv_lattice_strain(const double *box, int axis, double *dsde /*[9]*/) {
     for (int a = 0; a < 3; ++a)
         for (int b = 0; b < 3; ++b) dsde[3 * a + b] = h[a] * h[b] / s;
 }
+
+/* Strain derivatives of the remaining CVs (reading AD), each a function of a few minimum-image vectors. */
+
+/* Rg^2 = sum m |u - com|^2 / M on the unwrapped chain; u - com scales with the strain:
+ * d Rg/d eps_ab = sum m (u - com)_a (u - com)_b / (M Rg). */
+void orc_cv_rgyr_strain(int nchain, const int *chain, const double *mass, const double *pos,
+                        const double *box, double *dsde) {
+    double *g = (double *)malloc(sizeof(double) * 3 * (size_t)nchain);
+    double rg = orc_cv_rgyr(nchain, chain, mass, pos, box, g);      /* g_k = m_k (u_k - com) / (M Rg) */
+    double M = 0.0;
+    for (int k = 0; k < nchain; ++k) M += mass ? mass[k] : 1.0;
+    for (int k = 0; k < 9; ++k) dsde[k] = 0.0;
+    for (int k = 0; k < nchain; ++k) {
+        double mk = mass ? mass[k] : 1.0;
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b)
+                dsde[3 * a + b] += rg > 0.0 ? g[3 * k + a] * (g[3 * k + b] * M * rg / mk) : 0.0;
+    }
+    free(g);
+}
+
+/* Qc = scale sum_p sw(r_p / r0_p):  d Qc/d eps = scale sum_p sw'/(r0_p r_p) d_p d_p^T. */
+void orc_cv_contacts_strain(int npairs, const int *pairs, const double *pair_r0, int n, int m, double scale,
+                            const double *pos, const double *box, double *dsde) {
+    for (int k = 0; k < 9; ++k) dsde[k] = 0.0;
+    for (int p = 0; p < npairs; ++p) {
+        double d[3];
+        orc_delta(box, pos + 3 * pairs[2 * p], pos + 3 * pairs[2 * p + 1], d);
+        double r = sqrt(r2_of(d)), dsw;
+        orc_switch(r / pair_r0[p], n, m, &dsw);
+        double g = scale * dsw / (pair_r0[p] * r);
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) dsde[3 * a + b] += g * d[a] * d[b];
+    }
+}
+
+/* s = |d| of the nearest pair: d s/d eps = d d^T / |d| (zero if nobody is within rc). */
+void orc_cv_mindist_strain(int N, const double *pos, const double *box, const int *count, const int *list,
+                           int maxn, const unsigned char *flags, double rc, double *dsde) {
+    int pair[2];
+    double s = orc_cv_mindist(N, pos, box, count, list, maxn, flags, rc, NULL, pair);
+    for (int k = 0; k < 9; ++k) dsde[k] = 0.0;
+    if (pair[0] < 0) return;
+    double d[3];
+    orc_delta(box, pos + 3 * pair[0], pos + 3 * pair[1], d);
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) dsde[3 * a + b] = d[a] * d[b] / s;
+}
+
+/* phi(b1, b2, b3): d phi/d eps = sum_k (d phi/d b_k) b_k^T with d phi/d b1 = -g_i, d phi/d b2 = -(g_i + g_j),
+ * d phi/d b3 = g_l (g = the atom gradients of orc_cv_torsion, b1 = r_j - r_i, ...). */
+void orc_cv_torsion_strain(const int *idx, const double *pos, const double *box, double *dsde) {
+    double g[12], b[3][3];
+    orc_cv_torsion(idx, pos, box, g);
+    for (int k = 0; k < 3; ++k) orc_delta(box, pos + 3 * idx[k], pos + 3 * idx[k + 1], b[k]);
+    for (int a = 0; a < 3; ++a)
+        for (int c = 0; c < 3; ++c)
+            dsde[3 * a + c] = -g[a] * b[0][c] - (g[a] + g[3 + a]) * b[1][c] + g[9 + a] * b[2][c];
+}

@@ -7,7 +7,8 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import (cv_coord_strain, cv_lattice_strain, q6_strain, apply_forces, bias, bias_periodic, cv_contacts, cv_coord, cv_lattice, cv_mindist, cv_rgyr, cv_torsion, grid_add, grid_add_p,
+from . import (cv_contacts_strain, cv_coord_strain, cv_lattice_strain, cv_mindist_strain, cv_rgyr_strain,
+               cv_torsion_strain, q6_strain, apply_forces, bias, bias_periodic, cv_contacts, cv_coord, cv_lattice, cv_mindist, cv_rgyr, cv_torsion, grid_add, grid_add_p,
                grid_eval, grid_eval_p, make_flags, neighbors, q6_atoms, q6_grad, wt_height)
 
 # CV kinds — restated (not imported) so the oracle depends on nothing of the product.
@@ -157,6 +158,14 @@ class OracleMetaD:
                 out[d] = q6_strain(pos, box, self.count, self.list, self.q6, cv.scale * df)
             elif cv.kind == LATTICE:
                 out[d] = cv_lattice_strain(box, cv.n)
+            elif cv.kind == RGYR:
+                out[d] = cv_rgyr_strain(pos, box, cv.chain)
+            elif cv.kind == CONTACTS:
+                out[d] = cv_contacts_strain(pos, box, cv.pairs, cv.pair_r0, cv.n, cv.m, cv.scale)
+            elif cv.kind == MINDIST:
+                out[d] = cv_mindist_strain(pos, box, self.count, self.list, w.rc, make_flags(self.N, cv.group_a, cv.group_b))
+            elif cv.kind == TORSION:
+                out[d] = cv_torsion_strain(pos, box, cv.atoms)
         return out
 
     def virial(self, dVds, force_scale=1.0):

@@ -71,3 +71,42 @@ def test_virial_of_a_single_pair_by_hand():
     ref = 2 * dsw / (2.0 * r) * np.outer(d, d)              # two ordered pairs
     got = oracle.cv_coord_strain(pos, box, cnt, lst, 2.0, 6, 12, 1.0)
     assert np.allclose(got, ref, rtol=1e-13)
+
+
+def _fd_strain(w, pos, box, ana, comps=((0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)), h=1e-6, tol=2e-6):
+    for a, b in comps:
+        eps = np.zeros((3, 3)); eps[a, b] = h
+        sp = _cv_values(w, *_deform(pos, box, eps))
+        sm = _cv_values(w, *_deform(pos, box, -eps))
+        fd = (sp - sm) / (2 * h)
+        fd = np.where(np.abs(fd) > np.pi / (4 * h), fd - np.sign(fd) * np.pi / h, fd)      # a torsion crossing +-pi
+        for d in range(len(ana)):
+            scale = max(np.abs(ana[d]).max(), 1e-12)
+            assert abs(fd[d] - ana[d][a, b]) < tol * scale + 1e-9, (d, a, b, fd[d], ana[d][a, b])
+
+
+def test_strain_derivatives_of_the_chain_torsion_and_nearest_distance_cvs():
+    # Rg + native contacts on the chain workload (molecule and contacts well inside the box)
+    w = configs.small("c1")
+    o = OracleMetaD(w); o.build_neighbors(w.pos); o.eval_cv(want_grad=False)
+    ana = o.strain_derivatives()
+    _fd_strain(w, w.pos, w.box, ana)
+    assert np.abs(ana[0] - ana[0].T).max() < 1e-12 and np.abs(ana[1] - ana[1].T).max() < 1e-12
+    assert abs(np.trace(ana[0]) - o.s[0]) < 1e-10 * o.s[0]                 # Rg is homogeneous of degree 1 (Euler)
+    # torsions: scale- and rotation-invariant -> symmetric, traceless
+    w = configs.small("t0")
+    o = OracleMetaD(w); o.build_neighbors(w.pos); o.eval_cv(want_grad=False)
+    ana = o.strain_derivatives()
+    _fd_strain(w, w.pos, w.box, ana)
+    for d in range(2):
+        assert np.abs(ana[d] - ana[d].T).max() < 1e-12 and abs(np.trace(ana[d])) < 1e-12
+    # nearest-neighbour distance: d d^T / |d|, trace = s
+    from paper_2510_06873_b200.inputs import CV_MINDIST
+    w = configs.small("c2")
+    cv = w.cvs[0]
+    w.cvs = [CVSpec(kind=CV_MINDIST, group_a=np.asarray(cv.group_a)[11:12], group_b=cv.group_b)]
+    w.sigma = [0.05]
+    o = OracleMetaD(w); o.build_neighbors(w.pos); o.eval_cv(want_grad=False)
+    ana = o.strain_derivatives()
+    _fd_strain(w, w.pos, w.box, ana)
+    assert abs(np.trace(ana[0]) - o.s[0]) < 1e-12
