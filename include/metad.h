@@ -102,8 +102,7 @@ typedef struct {
                                        With a grid, a periodic dimension needs grid_hi - grid_lo == period and has
                                        grid_n nodes at lo + i * period / grid_n, no "outside" (reading X).  0: not periodic */
     int want_virial;                /* != 0: metad_apply_forces also computes the bias virial (metad_get_virial) for NPT runs
-                                       (reading AD).  Supported for COORD, Q6_MEAN, Q6_SOLID and LATTICE
-                                       dimensions; any other CV kind in the context -> METAD_ERR_ARG at create */
+                                       (reading AD), for every CV kind */
 } metad_params;
 
 /* Creates a context on the current CUDA device; `cuda_stream` is a cudaStream_t (NULL = default

@@ -147,11 +147,6 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
 
     if (c->has_mindist) CUDA_TRY(dev_alloc(&c->d_mind, 8));
     if (p->want_virial) {
-        for (int d = 0; d < c->D; ++d) {
-            const int k = c->cv[d].kind;
-            if (k != METAD_CV_COORD && k != METAD_CV_Q6_MEAN && k != METAD_CV_Q6_SOLID && k != METAD_CV_LATTICE)
-                FAIL(METAD_ERR_ARG, "want_virial supports COORD, Q6_MEAN, Q6_SOLID and LATTICE dimensions only");
-        }
         CUDA_TRY(dev_alloc(&c->d_virial, 9));
         CUDA_TRY(cudaMemset(c->d_virial, 0, sizeof(double) * 9));
         CUDA_TRY(dev_alloc(&c->d_vir_partials, 9 * ((size_t)div_up(N, 128) + 1)));

@@ -222,6 +222,7 @@ int nb_export(metad_ctx *c, int *d_count, int *d_list);
 int cv_eval_all(metad_ctx *c, double *d_cv);
 int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F);
 int q6_export(metad_ctx *c, void *d_q6);
+int chain_virial(metad_ctx *c, const double *d_dVds);
 int lattice_eval(metad_ctx *c, double *d_cv);
 int lattice_forces(metad_ctx *c, const double *d_dVds);
 int mindist_eval(metad_ctx *c, double *d_cv);

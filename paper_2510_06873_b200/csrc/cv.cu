@@ -617,7 +617,7 @@ k_mindist_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *
 
 template <typename T>
 __global__ void k_mindist_force(const double *__restrict__ rec, double force_scale, const double *__restrict__ dVds,
-                                T *__restrict__ F) {
+                                T *__restrict__ F, double *__restrict__ virial /* NULL: not wanted */) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     const int *pair = reinterpret_cast<const int *>(rec + 4);
     if (pair[0] < 0) return;
@@ -627,6 +627,9 @@ __global__ void k_mindist_force(const double *__restrict__ rec, double force_sca
         F[3 * (size_t)pair[0] + k] += (T)(a * rec[1 + k]);
         F[3 * (size_t)pair[1] + k] += (T)(-a * rec[1 + k]);
     }
+    if (virial)                                  // d s/d eps = d d^T / |d| (reading AD)
+        for (int p = 0; p < 3; ++p)
+            for (int q = 0; q < 3; ++q) virial[3 * p + q] += -a * rec[1 + p] * rec[1 + q];
 }
 
 template <typename T>
@@ -648,8 +651,10 @@ int mindist_eval(metad_ctx *c, double *d_cv) {
 }
 int mindist_forces(metad_ctx *c, const double *d_dVds, void *d_F) {
     if (!c->has_mindist) return METAD_OK;
-    if (c->prec == 32) k_mindist_force<float><<<1, 32, 0, c->stream>>>(c->d_mind, c->p.force_scale, d_dVds + c->mindist_dim, (float *)d_F);
-    else k_mindist_force<double><<<1, 32, 0, c->stream>>>(c->d_mind, c->p.force_scale, d_dVds + c->mindist_dim, (double *)d_F);
+    if (c->prec == 32) k_mindist_force<float><<<1, 32, 0, c->stream>>>(c->d_mind, c->p.force_scale, d_dVds + c->mindist_dim, (float *)d_F,
+                                                                   c->p.want_virial ? c->d_virial : nullptr);
+    else k_mindist_force<double><<<1, 32, 0, c->stream>>>(c->d_mind, c->p.force_scale, d_dVds + c->mindist_dim, (double *)d_F,
+                                                         c->p.want_virial ? c->d_virial : nullptr);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -770,6 +775,8 @@ int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F) {
     rcode = mindist_forces(c, d_dVds, d_F);
     if (rcode) return rcode;
     rcode = lattice_forces(c, d_dVds);
+    if (rcode) return rcode;
+    rcode = chain_virial(c, d_dVds);
     if (rcode) return rcode;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

@@ -388,3 +388,109 @@ int lattice_forces(metad_ctx *c, const double *d_dVds) {
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
 }
+
+
+// ------------------------------------------------------------------------------------------------
+// Bias virial of the chain / torsion CVs (reading AD), only launched with params.want_virial.  One block each; the
+// sums are short (<= a few thousand terms) and taken in a fixed order.
+__global__ void __launch_bounds__(256)
+k_rgyr_virial(int nchain, const double *__restrict__ mass, const double *__restrict__ unwrapped, double force_scale,
+              const double *__restrict__ dVds, double *__restrict__ virial) {
+    __shared__ double red[9 * 32];
+    const RgScratch *sc = reinterpret_cast<const RgScratch *>(unwrapped + 3 * (size_t)nchain);
+    double w[9];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) w[q] = 0.0;
+    for (int k = threadIdx.x; k < nchain; k += blockDim.x) {
+        const double mk = mass ? mass[k] : 1.0;
+        const double u[3] = { unwrapped[3 * k] - sc->com[0], unwrapped[3 * k + 1] - sc->com[1], unwrapped[3 * k + 2] - sc->com[2] };
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) w[3 * a + b] += mk * u[a] * u[b];
+    }
+    block_reduce<9>(w, red);
+    if (threadIdx.x == 0 && sc->rg > 0.0) {
+        const double f = -force_scale * dVds[0] / (sc->M * sc->rg);      // d Rg/d eps = sum m u u^T / (M Rg)
+        for (int q = 0; q < 9; ++q) virial[q] += f * w[q];
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_contacts_virial(int npairs, const int *__restrict__ pairs, const double *__restrict__ pair_r0, int n, int m,
+                  double coef /* force_scale * scale */, const T *__restrict__ pos, BoxD bd, const double *__restrict__ dVds,
+                  double *__restrict__ virial) {
+    __shared__ double red[9 * 32];
+    double w[9];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) w[q] = 0.0;
+    for (int p = threadIdx.x; p < npairs; p += blockDim.x) {
+        const int i = pairs[2 * p], j = pairs[2 * p + 1];
+        double d[3] = { (double)pos[3 * j] - (double)pos[3 * i], (double)pos[3 * j + 1] - (double)pos[3 * i + 1],
+                        (double)pos[3 * j + 2] - (double)pos[3 * i + 2] };
+        min_image_d(bd, d[0], d[1], d[2]);
+        const double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        double dsw;
+        switch_d(r / pair_r0[p], n, m, dsw);
+        const double g = dsw / (pair_r0[p] * r);
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int b = 0; b < 3; ++b) w[3 * a + b] += g * d[a] * d[b];
+    }
+    block_reduce<9>(w, red);
+    if (threadIdx.x == 0) {
+        const double f = -coef * dVds[0];
+        for (int q = 0; q < 9; ++q) virial[q] += f * w[q];
+    }
+}
+
+// d phi/d eps = sum_k (d phi/d b_k) b_k^T,  d phi/d b1 = -g_i, d phi/d b2 = -(g_i + g_j), d phi/d b3 = g_l
+template <typename T>
+__global__ void k_torsions_virial(int D, TorsTable tt, const T *__restrict__ pos, BoxD bd, const double *__restrict__ grad,
+                                  double force_scale, const double *__restrict__ dVds, double *__restrict__ virial) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    for (int d = 0; d < D; ++d) {
+        if (tt.kind[d] != METAD_CV_TORSION) continue;
+        double b[3][3];
+        for (int k = 0; k < 3; ++k) {
+            for (int a = 0; a < 3; ++a)
+                b[k][a] = (double)pos[3 * (size_t)tt.idx[d][k + 1] + a] - (double)pos[3 * (size_t)tt.idx[d][k] + a];
+            min_image_d(bd, b[k][0], b[k][1], b[k][2]);
+        }
+        const double *g = grad + 12 * d;
+        const double f = -force_scale * dVds[d];
+        for (int a = 0; a < 3; ++a)
+            for (int c = 0; c < 3; ++c)
+                virial[3 * a + c] += f * (-g[a] * b[0][c] - (g[a] + g[3 + a]) * b[1][c] + g[9 + a] * b[2][c]);
+    }
+}
+
+template <typename T>
+static int chain_virial_t(metad_ctx *c, const double *d_dVds) {
+    const T *pos = (const T *)ctx_last_pos(c);
+    for (int dim = 0; dim < c->D; ++dim) {
+        CvDev &d = c->cv[dim];
+        if (d.kind == METAD_CV_RGYR) {
+            k_rgyr_virial<<<1, 256, 0, c->stream>>>(d.nchain, d.d_mass, d.d_unwrapped, c->p.force_scale, d_dVds + dim, c->d_virial);
+            c->launches++;
+        } else if (d.kind == METAD_CV_CONTACTS) {
+            k_contacts_virial<T><<<1, 256, 0, c->stream>>>(d.npairs, d.d_pairs, d.d_pair_r0, d.n, d.m, c->p.force_scale * d.scale,
+                                                           pos, c->boxd, d_dVds + dim, c->d_virial);
+            c->launches++;
+        }
+    }
+    if (c->has_torsion) {
+        k_torsions_virial<T><<<1, 32, 0, c->stream>>>(c->D, tors_table(c), pos, c->boxd, c->d_tors_grad, c->p.force_scale, d_dVds,
+                                                      c->d_virial);
+        c->launches++;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+int chain_virial(metad_ctx *c, const double *d_dVds) {
+    if (!c->p.want_virial) return METAD_OK;
+    return c->prec == 32 ? chain_virial_t<float>(c, d_dVds) : chain_virial_t<double>(c, d_dVds);
+}

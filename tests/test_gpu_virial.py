@@ -47,13 +47,28 @@ def test_virial_tiled_coordination_and_lattice():
     assert np.trace(W) != 0.0
 
 
-def test_virial_needs_the_flag_and_supported_cvs():
+@pytest.mark.parametrize("name,precision,tol", [("c1", 64, 1e-9), ("c1", 32, 1e-5), ("t0", 64, 1e-9), ("c2", 64, 1e-9)])
+def test_virial_chain_torsion_and_grouped_coordination(name, precision, tol):
+    """Rg + native contacts (c1), two torsions (t0, traceless), grouped coordination number on the warp-per-atom sizes (c2)."""
+    w = configs.small(name)
+    r, W = _check(w, precision, tol)
+    if name == "t0":
+        assert abs(np.trace(W)) <= 1e-9 * np.abs(W).max()
+
+
+def test_virial_nearest_distance():
+    from paper_2510_06873_b200.inputs import CV_MINDIST
+    w = configs.small("c2")
+    cv = w.cvs[0]
+    w.cvs = [CVSpec(kind=CV_MINDIST, group_a=np.asarray(cv.group_a)[11:12], group_b=cv.group_b)]
+    w.sigma = [0.05]
+    w.n_hills = 100
+    _check(w, 64, 1e-9)
+
+
+def test_virial_needs_the_flag():
     from paper_2510_06873_b200.metad import MetaD, MetadError
     w = configs.small("c3")
     md = MetaD(w)
     with pytest.raises(MetadError):
         md.virial()
-    w1 = configs.small("c1")
-    assert any(cv.kind == CV_RGYR for cv in w1.cvs)
-    with pytest.raises(MetadError):
-        MetaD(w1, want_virial=True)
