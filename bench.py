@@ -58,6 +58,7 @@ def describe(w, precision):
     return {"workload": wl, "atoms": int(w.natoms),
             "cvs": [kinds[c.kind] for c in w.cvs], "hills": int(w.n_hills), "rc": w.rc,
             "pair_precision": f"fp{precision}", "stride": int(w.stride), "virial": bool(getattr(w, "_virial", False)),
+            "neighbour_build": ("skipped (lazy_neighbors: no CV of this workload reads the list)" if w.name == "t0" else "every step"),
             "l2": ("per-step working set (neighbour list + q6 records + positions + forces) exceeds the 126 MB L2; no flush"
                    if w.natoms * (4 * w.max_neigh + 64 + 16 + 24 + 16) > 126e6 else
                    "working set fits the 126 MB L2 and is not flushed: this workload is bound by the latency of its ~10 "
@@ -278,7 +279,7 @@ def run_ours(args):
         sig = np.asarray(w.sigma)
         grid = (w.grid_n, centers[0] - 120 * sig, centers[0] + 120 * sig)      # reading M
     md = MetaD(w, precision=precision, max_hills=w.n_hills + args.steps + args.warmup + 4096, grid=grid,
-               want_virial=args.virial)
+               want_virial=args.virial, lazy_neighbors=(args.config == "t0"))
     md.set_hills(centers, heights)
     with torch.cuda.stream(md.stream):
         F = torch.zeros((w.natoms, 3), device="cuda", dtype=tdt)

@@ -101,6 +101,9 @@ typedef struct {
                                        (s - s_tau) in PAPER.md:81 is then the nearest-image difference (reading W).
                                        With a grid, a periodic dimension needs grid_hi - grid_lo == period and has
                                        grid_n nodes at lo + i * period / grid_n, no "outside" (reading X).  0: not periodic */
+    int lazy_neighbors;             /* != 0: metad_build_neighbors only snapshots the positions when no CV of the context reads the
+                                       neighbour list (torsion / Rg / contacts / lattice CVs): a 22-atom torsion step is pure
+                                       launch latency and the list build is half of its launches.  0 (default): always built */
     int want_virial;                /* != 0: metad_apply_forces also computes the bias virial (metad_get_virial) for NPT runs
                                        (reading AD), for every CV kind */
 } metad_params;

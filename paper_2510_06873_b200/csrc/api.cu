@@ -336,8 +336,12 @@ extern "C" int metad_build_neighbors(metad_ctx *c, const void *d_pos, const doub
     int r = setup_geometry(c, h_box, rc);
     if (r) return r;
     c->d_pos_last = d_pos;
+    if (c->p.lazy_neighbors && !c->has_q6 && !c->has_coord && !c->has_mindist) {   // no CV reads the list
+        c->have_neighbors = true; c->list_built = false;
+        return METAD_OK;
+    }
     r = nb_build(c, d_pos);
-    if (r == METAD_OK) c->have_neighbors = true;
+    if (r == METAD_OK) { c->have_neighbors = true; c->list_built = true; }
     return r;
 }
 
@@ -454,6 +458,7 @@ extern "C" int metad_get_state(metad_ctx *c, double *h_cv, double *h_V, double *
 extern "C" int metad_get_neighbors(metad_ctx *c, int *d_count, int *d_list) {
     if (!c || !d_count || !d_list) FAIL(METAD_ERR_ARG, "null argument");
     if (!c->have_neighbors) FAIL(METAD_ERR_STATE, "metad_build_neighbors has not been called");
+    if (!c->list_built) FAIL(METAD_ERR_STATE, "lazy_neighbors: no CV reads the list, it was not built");
     return nb_export(c, d_count, d_list);
 }
 
@@ -559,12 +564,14 @@ extern "C" int metad_reset_steps(metad_ctx *c) {
 extern "C" int metad_set_timing(metad_ctx *c, int enabled) {
     if (!c) FAIL(METAD_ERR_ARG, "null argument");
     c->timing = enabled != 0;
+    c->timing_recorded = 0;
     return METAD_OK;
 }
 
 extern "C" int metad_get_timing(metad_ctx *c, float *ms_sort, float *ms_list) {
     if (!c || !ms_sort || !ms_list) FAIL(METAD_ERR_ARG, "null argument");
     if (!c->timing) FAIL(METAD_ERR_STATE, "timing is not enabled");
+    if (!c->timing_recorded) FAIL(METAD_ERR_STATE, "no neighbour build has been timed yet");
     CUDA_TRY(cudaStreamSynchronize(c->stream));
     CUDA_TRY(cudaEventElapsedTime(ms_sort, c->ev[0], c->ev[1]));
     CUDA_TRY(cudaEventElapsedTime(ms_list, c->ev[1], c->ev[2]));

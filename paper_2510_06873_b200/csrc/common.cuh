@@ -160,7 +160,7 @@ struct metad_ctx {
     CellGrid grid;
     BoxD boxd;
     double rc, rc2;
-    bool have_neighbors;
+    bool have_neighbors, list_built;
     int cell_cap;
     int *d_cell_count, *d_cell_start, *d_block_sums;
     int *d_cell_of, *d_slot, *d_perm, *d_perm_raw, *d_scell;   // perm_raw: counting-sort output before the in-cell ordering
@@ -202,7 +202,7 @@ struct metad_ctx {
     int *d_aux;                           // device scalars: grid-miss flag, index of the hill deposited this step
     // shared-memory tiled fast path (fp32, Q6): tile.cuh / tiled.cu
     int tiled; int tile_T[3]; int tile_cap; int tile_hx;
-    int timing; int capturing; cudaEvent_t ev[3];
+    int timing; int capturing; int timing_recorded; cudaEvent_t ev[3];
     cudaStream_t copy_stream; cudaEvent_t ev_copy;   // metad_step_host: the force upload overlaps the first three stages
     float *d_q6;                          // tiled path: per-atom q6 (sorted order)
     double *d_cvq6;                       // tiled path: [Q6 mean, solid count] finished by k_tile_build
@@ -212,7 +212,7 @@ static inline const void *ctx_last_pos(const metad_ctx *c) { return c->d_pos_las
 static inline int *ctx_aux(const metad_ctx *c) { return c->d_aux; }
 
 void metad_set_error(const char *msg);
-#define CUDA_TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { metad_set_error(cudaGetErrorString(e_)); return METAD_ERR_CUDA; } } while (0)
+#define CUDA_TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { metad_set_error(cudaGetErrorString(e_)); (void)cudaGetLastError(); return METAD_ERR_CUDA; } } while (0)
 
 static inline int div_up(long long a, int b) { return (int)((a + b - 1) / b); }
 

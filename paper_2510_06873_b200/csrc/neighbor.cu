@@ -302,7 +302,7 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     cudaStream_t st = c->stream;
     const int nsb = div_up(ncell, SCAN_TILE);
     const bool tm = c->timing && !c->capturing;
-    if (tm) cudaEventRecord(c->ev[0], st);
+    if (tm) { cudaEventRecord(c->ev[0], st); c->timing_recorded = 1; }
     k_bin<T><<<div_up(N, 256), 256, 0, st>>>(N, (const T *)d_pos, c->grid, c->d_cell_of, c->d_slot, c->d_cell_count,
                                              c->d_sticky);
     k_scan_sums<<<nsb, SCAN_THREADS, 0, st>>>(ncell, c->d_cell_count, c->d_block_sums);

@@ -36,7 +36,7 @@ class Params(ctypes.Structure):
     _fields_ = [("natoms", _I), ("precision", _I), ("max_neigh", _I), ("ncv", _I),
                 ("cv", CvDesc * MAX_CV), ("sigma", _D * MAX_CV), ("w0", _D), ("kT", _D),
                 ("bias_factor", _D), ("max_hills", _I), ("stride", _I), ("grid_n", _I * 2),
-                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("want_virial", _I)]
+                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("lazy_neighbors", _I), ("want_virial", _I)]
 
 
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
@@ -107,7 +107,7 @@ class MetaD:
     fields); tensors passed to the methods are torch CUDA tensors (float64, or float32 for pos/F when
     precision == 32)."""
 
-    def __init__(self, workload, max_hills=None, precision=None, grid=None, force_scale=1.0, stream=None, want_virial=False):
+    def __init__(self, workload, max_hills=None, precision=None, grid=None, force_scale=1.0, stream=None, want_virial=False, lazy_neighbors=False):
         import torch
         self.torch = torch
         L = load()
@@ -158,6 +158,7 @@ class MetaD:
             self.grid_n = None
         p.force_scale = float(force_scale)
         p.want_virial = 1 if want_virial else 0
+        p.lazy_neighbors = 1 if lazy_neighbors else 0
         self._params = p
         h = _P()
         _check(L.metad_create(ctypes.byref(h), ctypes.byref(p), _P(self.stream.cuda_stream)))

@@ -157,3 +157,34 @@ def test_create_rejects_bad_torsion_and_period_arguments():
     w = configs.small("t0")
     with pytest.raises(MetadError):
         MetaD(w, grid=(w.grid_n, LO, HI + 0.1))      # grid span != period
+
+
+def test_lazy_neighbors_skips_the_unused_list_and_changes_nothing_else():
+    import torch
+    from paper_2510_06873_b200.metad import MetaD, MetadError
+    w = configs.small("t0")
+    centers = hill_walk_periodic(5, np.zeros(2), w.sigma, 80, w.period, w.extra["period_lo"])
+    heights = seeded_heights(5, 80, w.w0)
+    out = []
+    for lazy in (False, True):
+        md = MetaD(w, max_hills=128, lazy_neighbors=lazy)
+        md.set_hills(centers, heights)
+        with torch.cuda.stream(md.stream):
+            dpos = torch.tensor(w.pos, device="cuda")
+            F = torch.zeros((w.natoms, 3), device="cuda", dtype=torch.float64)
+        md.synchronize()
+        l0 = md.launch_count()
+        md.run(dpos, F, 4)
+        st = md.state()
+        out.append((st["cv"].copy(), st["V"], F.cpu().numpy(), (md.launch_count() - l0) // 4))
+        if lazy:
+            with pytest.raises(MetadError):
+                md.neighbors()
+    assert np.array_equal(out[0][0], out[1][0]) and out[0][1] == out[1][1] and np.array_equal(out[0][2], out[1][2])
+    assert out[1][3] == out[0][3] - 6                       # the six kernels of the list build are gone
+    # a context whose CVs read the list builds it regardless of the flag
+    w3 = configs.small("c3")
+    md = MetaD(w3, lazy_neighbors=True)
+    md.build_neighbors(torch.tensor(w3.pos, device="cuda"))
+    cnt, _ = md.neighbors()
+    assert cnt.sum() > 0
