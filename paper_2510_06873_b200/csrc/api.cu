@@ -367,8 +367,19 @@ extern "C" int metad_deposit(metad_ctx *c, const double *d_cv, const double *d_V
     return bias_deposit(c, d_cv, d_V);
 }
 
+static bool fused_torsion_ok(const metad_ctx *c) {
+    if (!c->p.lazy_neighbors || c->p.want_virial || c->ntors_atoms > 256) return false;
+    for (int d = 0; d < c->D; ++d) if (c->cv[d].kind != METAD_CV_TORSION) return false;
+    return c->D <= 2 || !c->grid_on;
+}
+
 static int enqueue_step(metad_ctx *c, const void *d_pos, const double *box, double rc, void *d_F) {
     int r;
+    if (fused_torsion_ok(c)) {                    // torsion-only context: the whole step is one kernel (bias.cu)
+        if ((r = setup_geometry(c, box, rc))) return r;
+        c->d_pos_last = d_pos; c->have_neighbors = true; c->list_built = false;
+        return bias_fused_torsion_step(c, d_pos, d_F);
+    }
     if ((r = metad_build_neighbors(c, d_pos, box, rc))) return r;
     if ((r = metad_eval_cv(c, c->d_cv))) return r;
     if ((r = metad_bias(c, c->d_cv, c->d_V, c->d_dVds))) return r;
@@ -422,12 +433,17 @@ extern "C" int metad_step_host(metad_ctx *c, const void *h_pos, const double *h_
     CUDA_TRY(cudaMemcpyAsync(c->d_F_stage, h_F, bytes, cudaMemcpyHostToDevice, c->copy_stream));
     CUDA_TRY(cudaEventRecord(c->ev_copy, c->copy_stream));
     int r;
-    if ((r = metad_build_neighbors(c, c->d_pos_stage, h_box, rc))) return r;
-    if ((r = metad_eval_cv(c, c->d_cv))) return r;
-    if ((r = metad_bias(c, c->d_cv, c->d_V, c->d_dVds))) return r;
-    CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_copy, 0));
-    if ((r = metad_apply_forces(c, c->d_dVds, c->d_F_stage))) return r;
-    if ((r = metad_deposit(c, c->d_cv, c->d_V))) return r;
+    if (fused_torsion_ok(c)) {
+        CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_copy, 0));
+        if ((r = enqueue_step(c, c->d_pos_stage, h_box, rc, c->d_F_stage))) return r;
+    } else {
+        if ((r = metad_build_neighbors(c, c->d_pos_stage, h_box, rc))) return r;
+        if ((r = metad_eval_cv(c, c->d_cv))) return r;
+        if ((r = metad_bias(c, c->d_cv, c->d_V, c->d_dVds))) return r;
+        CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_copy, 0));
+        if ((r = metad_apply_forces(c, c->d_dVds, c->d_F_stage))) return r;
+        if ((r = metad_deposit(c, c->d_cv, c->d_V))) return r;
+    }
     CUDA_TRY(cudaMemcpyAsync(h_F, c->d_F_stage, bytes, cudaMemcpyDeviceToHost, c->stream));
     if (h_cv) CUDA_TRY(cudaMemcpyAsync(h_cv, c->d_cv, sizeof(double) * c->D, cudaMemcpyDeviceToHost, c->stream));
     if (h_V) CUDA_TRY(cudaMemcpyAsync(h_V, c->d_V, sizeof(double), cudaMemcpyDeviceToHost, c->stream));

@@ -3,6 +3,7 @@
 // PAPER.md:43 / ref. [16] (reading I).  Everything fp64; hill count and step counter live on the device
 // so that the whole step can sit inside a CUDA graph.
 #include "common.cuh"
+#include "cv_torsion.cuh"
 
 #define BIAS_THREADS 256
 #define BIAS_MAX_BLOCKS 592   // 4 x 148 SMs
@@ -92,11 +93,10 @@ __device__ __forceinline__ void hermite(double t, double *h, double *dh) {
     dh[0] = 6 * t2 - 6 * t; dh[1] = -6 * t2 + 6 * t; dh[2] = 3 * t2 - 4 * t + 1; dh[3] = 3 * t2 - 2 * t;
 }
 
-__global__ void k_bias_grid(GridParams gp, const double *__restrict__ table, const double *__restrict__ cv,
-                            double *__restrict__ V, double *__restrict__ dVds, int *__restrict__ aux,
-                            unsigned int *__restrict__ sticky) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    double sv[2] = { cv[0], cv[1] };
+// bicubic Hermite lookup at (s0, s1); returns true if the point is outside a non-periodic range (no result then)
+__device__ __forceinline__ bool grid_lookup(const GridParams &gp, const double *__restrict__ table, double s0, double s1,
+                                            double &V, double &dV0, double &dV1) {
+    const double sv[2] = { s0, s1 };
     const int nn[2] = { gp.n0, gp.n1 };
     int i0[2], i1[2];
     double tt[2];
@@ -117,12 +117,7 @@ __global__ void k_bias_grid(GridParams gp, const double *__restrict__ table, con
             tt[d] = f - i; i0[d] = i; i1[d] = i + 1;
         }
     }
-    if (miss || !isfinite(sv[0]) || !isfinite(sv[1])) {
-        aux[AUX_GRID_MISS] = 1;
-        atomicOr(sticky, (unsigned)METAD_DEV_GRID_RANGE);
-        return;
-    }
-    aux[AUX_GRID_MISS] = 0;
+    if (miss || !isfinite(sv[0]) || !isfinite(sv[1])) return true;
     double hx[4], dhx[4], hy[4], dhy[4];
     hermite(tt[0], hx, dhx);
     hermite(tt[1], hy, dhy);
@@ -139,7 +134,22 @@ __global__ void k_bias_grid(GridParams gp, const double *__restrict__ table, con
             vx += f * dhx[a] * hy[b] + f0 * dhx[2 + a] * hy[b] + f1 * dhx[a] * hy[2 + b] + f01 * dhx[2 + a] * hy[2 + b];
             vy += f * hx[a] * dhy[b] + f0 * hx[2 + a] * dhy[b] + f1 * hx[a] * dhy[2 + b] + f01 * hx[2 + a] * dhy[2 + b];
         }
-    *V = v; dVds[0] = vx * gp.inv_h[0]; dVds[1] = vy * gp.inv_h[1];
+    V = v; dV0 = vx * gp.inv_h[0]; dV1 = vy * gp.inv_h[1];
+    return false;
+}
+
+__global__ void k_bias_grid(GridParams gp, const double *__restrict__ table, const double *__restrict__ cv,
+                            double *__restrict__ V, double *__restrict__ dVds, int *__restrict__ aux,
+                            unsigned int *__restrict__ sticky) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double v, d0, d1;
+    if (grid_lookup(gp, table, cv[0], cv[1], v, d0, d1)) {
+        aux[AUX_GRID_MISS] = 1;
+        atomicOr(sticky, (unsigned)METAD_DEV_GRID_RANGE);
+        return;
+    }
+    aux[AUX_GRID_MISS] = 0;
+    *V = v; dVds[0] = d0; dVds[1] = d1;
 }
 
 // table build: 16x16 node tile per block; hills staged through shared memory in chunks, the two
@@ -223,6 +233,103 @@ __global__ void k_deposit(BiasParams bp, int stride, double w0, double kT, doubl
     heights[H] = h;
     *nhills = H + 1;
     aux[AUX_DEP_INDEX] = H;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Fused step for torsion-only contexts (a 22-atom molecule, two torsions): CV evaluation, bias (grid
+// lookup, else the exact hill sum by the whole block in a fixed order), gather-form forces and deposition in ONE launch.
+// Such a step is nothing but launch latency (6 dependent launches of ~2.3 us otherwise).  Used by metad_run /
+// metad_step_host when params.lazy_neighbors is set and every CV is a torsion; the five stage calls stay available.
+struct FusedTors { int D; int idx[METAD_MAX_CV][4]; int natoms; };
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_fused_torsion_step(FusedTors ft, const int *__restrict__ tors_atoms, const T *__restrict__ pos, BoxD bd, BiasParams bp,
+                     GridParams gp, int grid_on, const double *__restrict__ table, double *__restrict__ centers,
+                     double *__restrict__ heights, int *__restrict__ nhills, int *__restrict__ step, int *__restrict__ aux,
+                     unsigned int *__restrict__ sticky, int stride, double w0, double kT, double gamma, double force_scale,
+                     double *__restrict__ cv_out, double *__restrict__ V_out, double *__restrict__ dVds_out,
+                     double *__restrict__ tors_grad, T *__restrict__ F) {
+    __shared__ double s_cv[METAD_MAX_CV], s_g[METAD_MAX_CV][12], s_V, s_dV[METAD_MAX_CV];
+    __shared__ int s_exact;
+    __shared__ double red[(1 + METAD_MAX_CV) * 32];
+    const int tid = threadIdx.x;
+    if (tid < ft.D) {                                            // a2t: one thread per torsion
+        double b[3][3];
+        for (int k = 0; k < 3; ++k) {
+            for (int a = 0; a < 3; ++a)
+                b[k][a] = (double)pos[3 * (size_t)ft.idx[tid][k + 1] + a] - (double)pos[3 * (size_t)ft.idx[tid][k] + a];
+            min_image_d(bd, b[k][0], b[k][1], b[k][2]);
+        }
+        double g[12];
+        const double phi = torsion_eval(b[0], b[1], b[2], g);
+        s_cv[tid] = phi; cv_out[tid] = phi;
+        for (int k = 0; k < 12; ++k) { s_g[tid][k] = g[k]; tors_grad[12 * tid + k] = g[k]; }
+        if (!isfinite(phi)) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
+    }
+    __syncthreads();
+    if (tid == 0) {                                              // a5g: table lookup
+        int exact = 1;
+        if (grid_on) {
+            double v, d0, d1;
+            if (grid_lookup(gp, table, s_cv[0], s_cv[1], v, d0, d1)) { aux[AUX_GRID_MISS] = 1; atomicOr(sticky, (unsigned)METAD_DEV_GRID_RANGE); }
+            else { aux[AUX_GRID_MISS] = 0; s_V = v; s_dV[0] = d0; s_dV[1] = d1; exact = 0; }
+        }
+        s_exact = exact;
+    }
+    __syncthreads();
+    if (s_exact) {                                               // a5: exact hill sum, thread-strided, fixed-order reduction
+        const int H = *nhills;
+        double acc[1 + METAD_MAX_CV];
+#pragma unroll
+        for (int d = 0; d <= METAD_MAX_CV; ++d) acc[d] = 0.0;
+        for (int k = tid; k < H; k += blockDim.x) {
+            double e = 0.0, t[METAD_MAX_CV];
+#pragma unroll
+            for (int d = 0; d < METAD_MAX_CV; ++d) {
+                if (d < bp.D) {
+                    t[d] = pdiff(s_cv[d], centers[(size_t)d * bp.max_hills + k], bp.period[d]) * bp.inv_sigma[d];
+                    e += t[d] * t[d];
+                }
+            }
+            const double g = heights[k] * exp(-0.5 * e);
+            acc[0] += g;
+#pragma unroll
+            for (int d = 0; d < METAD_MAX_CV; ++d)
+                if (d < bp.D) acc[1 + d] -= g * t[d] * bp.inv_sigma[d];
+        }
+        block_reduce<1 + METAD_MAX_CV>(acc, red);
+        if (tid == 0) { s_V = acc[0]; for (int d = 0; d < bp.D; ++d) s_dV[d] = acc[1 + d]; }
+        __syncthreads();
+    }
+    if (tid < ft.natoms) {                                       // a6: gather form, thread per touched atom
+        const int a = tors_atoms[tid];
+        double f[3] = { 0.0, 0.0, 0.0 };
+        for (int d = 0; d < ft.D; ++d)
+            for (int k = 0; k < 4; ++k)
+                if (ft.idx[d][k] == a) { f[0] += s_dV[d] * s_g[d][3 * k]; f[1] += s_dV[d] * s_g[d][3 * k + 1]; f[2] += s_dV[d] * s_g[d][3 * k + 2]; }
+        F[3 * (size_t)a] += (T)(-force_scale * f[0]);
+        F[3 * (size_t)a + 1] += (T)(-force_scale * f[1]);
+        F[3 * (size_t)a + 2] += (T)(-force_scale * f[2]);
+    }
+    if (tid == 0) {                                              // a7: deposition (readings I, J, U)
+        *V_out = s_V;
+        for (int d = 0; d < bp.D; ++d) dVds_out[d] = s_dV[d];
+        const int st = *step + 1;
+        *step = st;
+        aux[AUX_DEP_INDEX] = -1;
+        if (stride > 0 && st % stride == 0) {
+            const int H = *nhills;
+            if (H >= bp.max_hills) atomicOr(sticky, (unsigned)METAD_DEV_HILL_OVERFLOW);
+            else {
+                const double h = gamma > 1.0 ? w0 * exp(-s_V / ((gamma - 1.0) * kT)) : w0;
+                for (int d = 0; d < bp.D; ++d) centers[(size_t)d * bp.max_hills + H] = s_cv[d];
+                heights[H] = h;
+                *nhills = H + 1;
+                aux[AUX_DEP_INDEX] = H;
+            }
+        }
+    }
 }
 
 __global__ void k_hills_import(int D, int max_hills, int count, const double *__restrict__ rowmajor,
@@ -325,6 +432,33 @@ int bias_get_hills_dev(metad_ctx *c, double *d_rowmajor, double *d_heights, int 
     k_hills_export<<<div_up(c->p.max_hills, 256), 256, 0, c->stream>>>(c->D, c->p.max_hills, capacity, c->d_centers,
                                                                      c->d_heights, c->d_nhills, d_rowmajor, d_heights);
     c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
+
+// the whole step of a torsion-only context in one launch (+ the table update in grid mode)
+int bias_fused_torsion_step(metad_ctx *c, const void *d_pos, void *d_F) {
+    FusedTors ft;
+    ft.D = c->D; ft.natoms = c->ntors_atoms;
+    for (int d = 0; d < METAD_MAX_CV; ++d)
+        for (int k = 0; k < 4; ++k) ft.idx[d][k] = d < c->D ? c->cv[d].tors[k] : 0;
+    BiasParams bp = make_bp(c);
+    GridParams gp = make_gp(c);
+    if (c->prec == 32)
+        k_fused_torsion_step<float><<<1, 256, 0, c->stream>>>(ft, c->d_tors_atoms, (const float *)d_pos, c->boxd, bp, gp, c->grid_on,
+            c->d_table, c->d_centers, c->d_heights, c->d_nhills, c->d_step, ctx_aux(c), c->d_sticky, c->p.stride, c->p.w0, c->p.kT,
+            c->p.bias_factor, c->p.force_scale, c->d_cv, c->d_V, c->d_dVds, c->d_tors_grad, (float *)d_F);
+    else
+        k_fused_torsion_step<double><<<1, 256, 0, c->stream>>>(ft, c->d_tors_atoms, (const double *)d_pos, c->boxd, bp, gp, c->grid_on,
+            c->d_table, c->d_centers, c->d_heights, c->d_nhills, c->d_step, ctx_aux(c), c->d_sticky, c->p.stride, c->p.w0, c->p.kT,
+            c->p.bias_factor, c->p.force_scale, c->d_cv, c->d_V, c->d_dVds, c->d_tors_grad, (double *)d_F);
+    c->launches++;
+    if (c->grid_on) {
+        int nn = c->p.grid_n[0] * c->p.grid_n[1];
+        k_grid_add_last<<<div_up(nn, 256), 256, 0, c->stream>>>(gp, bp, c->d_centers, c->d_heights, ctx_aux(c), c->d_table);
+        c->launches++;
+    }
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
 }

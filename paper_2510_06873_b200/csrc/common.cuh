@@ -66,6 +66,16 @@ __device__ __forceinline__ double r2_canonical(const BoxD &b, double dx, double 
     return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
 }
 
+// fp64 minimum image in the order of reading O (chain / torsion CVs, fused small-molecule step)
+__device__ __forceinline__ void min_image_d(const BoxD &b, double &dx, double &dy, double &dz) {
+    if (dz > b.hz) { dx -= b.cx; dy -= b.cy; dz -= b.cz; }
+    else if (dz < -b.hz) { dx += b.cx; dy += b.cy; dz += b.cz; }
+    if (dy > b.hy) { dx -= b.bx; dy -= b.by; }
+    else if (dy < -b.hy) { dx += b.bx; dy += b.by; }
+    if (dx > b.hx) { dx -= b.ax; }
+    else if (dx < -b.hx) { dx += b.ax; }
+}
+
 // ------------------------------------------------------------------------------------------------
 // Deterministic block reduction of K doubles per thread (fixed tree: shuffle inside the warp, then
 // warp 0 sums the per-warp partials in warp order).
@@ -232,6 +242,7 @@ int torsion_forces(metad_ctx *c, const double *d_dVds, void *d_F);
 int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds);
 int bias_deposit(metad_ctx *c, const double *d_cv, const double *d_V);
 int bias_grid_rebuild(metad_ctx *c);
+int bias_fused_torsion_step(metad_ctx *c, const void *d_pos, void *d_F);
 int bias_set_hills_dev(metad_ctx *c, const double *d_centers_rowmajor, const double *d_heights, int count);
 int bias_get_hills_dev(metad_ctx *c, double *d_centers_rowmajor, double *d_heights, int capacity);
 int bias_batch(metad_ctx *c, const double *d_points, int T, double *d_V);

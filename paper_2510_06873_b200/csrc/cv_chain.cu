@@ -8,15 +8,6 @@
 
 struct RgScratch { double com[3]; double M; double rg; };   // stored after the unwrapped coords
 
-__device__ __forceinline__ void min_image_d(const BoxD &b, double &dx, double &dy, double &dz) {
-    if (dz > b.hz) { dx -= b.cx; dy -= b.cy; dz -= b.cz; }
-    else if (dz < -b.hz) { dx += b.cx; dy += b.cy; dz += b.cz; }
-    if (dy > b.hy) { dx -= b.bx; dy -= b.by; }
-    else if (dy < -b.hy) { dx += b.bx; dy += b.by; }
-    if (dx > b.hx) { dx -= b.ax; }
-    else if (dx < -b.hx) { dx += b.ax; }
-}
-
 // single block: unwrap by a block-wide prefix sum of minimum-image bond vectors, then COM and Rg.
 template <typename T>
 __global__ void __launch_bounds__(RG_THREADS)
