@@ -25,7 +25,7 @@ __global__ void k_bin(int N, const T *__restrict__ pos, CellGrid g, int *__restr
     // Positions must lie in the primary cell (include/metad.h).  A coordinate that rounds to the far face (fractional
     // 1.0 + eps, e.g. after fp32 rounding) is CLAMPED into the boundary cell, not wrapped: its cartesian coordinates are
     // next to that cell's atoms, which is what the lattice-shift logic of the tiled path relies on.
-    if (fabs(sa - 0.5) > 0.5001 || fabs(sb - 0.5) > 0.5001 || fabs(sc - 0.5) > 0.5001)
+    if (!(fabs(sa - 0.5) <= 0.5001) || !(fabs(sb - 0.5) <= 0.5001) || !(fabs(sc - 0.5) <= 0.5001))   // also catches NaN
         atomicOr(sticky, (unsigned)METAD_DEV_POS_RANGE);
     int ia = min(max((int)floor(sa * g.nc[0]), 0), g.nc[0] - 1);
     int ib = min(max((int)floor(sb * g.nc[1]), 0), g.nc[1] - 1);

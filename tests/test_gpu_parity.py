@@ -270,6 +270,12 @@ def test_errors_and_sticky_bits():
     torch.cuda.synchronize()
     md4.run(dpos, F, 5)
     assert md4.status() & metad.DEV_HILL_OVERFLOW and md4.state()["nhills"] == 3
+    # a position outside the primary cell, and a NaN position: POS_RANGE sticky bit, no crash
+    for bad in (np.array([25.0, 1.0, 1.0]), np.array([np.nan, 1.0, 1.0])):
+        p = w4.pos.copy(); p[7] = bad
+        md6 = MetaD(configs.config0())
+        md6.build_neighbors(torch.tensor(p, device="cuda"))
+        assert md6.status() & metad.DEV_POS_RANGE
     # empty hill set: V = 0, forces untouched
     md5 = MetaD(configs.config0())
     md5.run(dpos, F.zero_(), 1)
