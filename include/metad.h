@@ -40,7 +40,8 @@ enum metad_error { METAD_OK = 0, METAD_ERR_ARG = 1, METAD_ERR_BOX = 2, METAD_ERR
 
 enum metad_dev_bits { METAD_DEV_NEIGH_OVERFLOW = 1, METAD_DEV_HILL_OVERFLOW = 2,
                       METAD_DEV_GRID_RANGE = 4, METAD_DEV_NONFINITE = 8,
-                      METAD_DEV_POS_RANGE = 16 /* a position lies outside the primary cell */ };
+                      METAD_DEV_POS_RANGE = 16 /* a position lies outside the primary cell */,
+                      METAD_DEV_TRAJ_FULL = 32 /* the recorded CV trajectory is full, later frames are dropped */ };
 
 enum metad_cv_kind {
     METAD_CV_COORD = 0,    /* s = scale * sum_{i in A} sum_{j in B, j!=i, r<rc} sw(r_ij/r0),
@@ -101,6 +102,9 @@ typedef struct {
                                        (s - s_tau) in PAPER.md:81 is then the nearest-image difference (reading W).
                                        With a grid, a periodic dimension needs grid_hi - grid_lo == period and has
                                        grid_n nodes at lo + i * period / grid_n, no "outside" (reading X).  0: not periodic */
+    int traj_capacity;              /* > 0: every metad_deposit also appends the step's CV values to a device-resident trajectory
+                                       of this many frames ("GSTA" keeps the CV outputs aligned with the MD run;
+                                       PAPER.md:85-87 reweights them) — see metad_reweight_recorded.  Full: METAD_DEV_TRAJ_FULL */
     int lazy_neighbors;             /* != 0: metad_build_neighbors only snapshots the positions when no CV of the context reads the
                                        neighbour list (torsion / Rg / contacts / lattice CVs): a 22-atom torsion step is pure
                                        launch latency and the list build is half of its launches.  0 (default): always built */
@@ -193,7 +197,12 @@ int metad_get_box_force(metad_ctx *ctx, double *d_out9);
  * tensor is W / volume.  Copied to d_out9 (device double[9], row-major); enqueued, not synchronised. */
 int metad_get_virial(metad_ctx *ctx, double *d_out9);
 
-/* Resets the step counter (hills stay). */
+/* metad_reweight over the CV frames recorded on the device since the last metad_reset_steps (params.traj_capacity > 0):
+ * the frames never leave the GPU.  h_nframes (may be NULL) receives the number of frames used.  [sync] */
+int metad_reweight_recorded(metad_ctx *ctx, const int *h_nbins, const double *h_lo, const double *h_hi, double *d_P,
+                            double *d_F, int *h_nframes);
+
+/* Resets the step counter and the recorded trajectory (hills stay). */
 int metad_reset_steps(metad_ctx *ctx);
 
 /* Kernel-level timing for bench.py: when enabled, metad_build_neighbors records CUDA events around its

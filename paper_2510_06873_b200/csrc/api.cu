@@ -146,6 +146,8 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     }
 
     if (c->has_mindist) CUDA_TRY(dev_alloc(&c->d_mind, 8));
+    if (p->traj_capacity < 0) FAIL(METAD_ERR_ARG, "traj_capacity must be >= 0");
+    if (p->traj_capacity > 0) CUDA_TRY(dev_alloc(&c->d_traj, (size_t)p->traj_capacity * c->D));
     if (p->want_virial) {
         CUDA_TRY(dev_alloc(&c->d_virial, 9));
         CUDA_TRY(cudaMemset(c->d_virial, 0, sizeof(double) * 9));
@@ -237,7 +239,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
@@ -569,6 +571,18 @@ extern "C" int metad_get_virial(metad_ctx *c, double *d_out9) {
     if (!c->p.want_virial) FAIL(METAD_ERR_STATE, "params.want_virial was not set");
     CUDA_TRY(cudaMemcpyAsync(d_out9, c->d_virial, sizeof(double) * 9, cudaMemcpyDeviceToDevice, c->stream));
     return METAD_OK;
+}
+
+extern "C" int metad_reweight_recorded(metad_ctx *c, const int *h_nbins, const double *h_lo, const double *h_hi, double *d_P,
+                                       double *d_F, int *h_nframes) {
+    if (!c) FAIL(METAD_ERR_ARG, "null argument");
+    if (!c->d_traj) FAIL(METAD_ERR_STATE, "params.traj_capacity was 0: no trajectory is recorded");
+    int steps = 0;
+    CUDA_TRY(cudaMemcpyAsync(&steps, c->d_step, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    const int n = steps < c->p.traj_capacity ? steps : c->p.traj_capacity;
+    if (h_nframes) *h_nframes = n;
+    return metad_reweight(c, c->d_traj, n, h_nbins, h_lo, h_hi, d_P, d_F);
 }
 
 extern "C" int metad_reset_steps(metad_ctx *c) {

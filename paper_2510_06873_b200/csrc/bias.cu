@@ -220,10 +220,14 @@ __global__ void k_grid_add_last(GridParams gp, BiasParams bp, const double *__re
 __global__ void k_deposit(BiasParams bp, int stride, double w0, double kT, double gamma, const double *__restrict__ cv,
                           const double *__restrict__ V, double *__restrict__ centers, double *__restrict__ heights,
                           int *__restrict__ nhills, int *__restrict__ step, int *__restrict__ aux,
-                          unsigned int *__restrict__ sticky) {
+                          unsigned int *__restrict__ sticky, double *__restrict__ traj, int traj_cap) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     int st = *step + 1;
     *step = st;
+    if (traj) {                                   // device-resident CV trajectory (reweighting input)
+        if (st <= traj_cap) { for (int d = 0; d < bp.D; ++d) traj[(size_t)(st - 1) * bp.D + d] = cv[d]; }
+        else atomicOr(sticky, (unsigned)METAD_DEV_TRAJ_FULL);
+    }
     aux[AUX_DEP_INDEX] = -1;
     if (stride <= 0 || st % stride != 0) return;
     int H = *nhills;
@@ -249,7 +253,7 @@ k_fused_torsion_step(FusedTors ft, const int *__restrict__ tors_atoms, const T *
                      double *__restrict__ heights, int *__restrict__ nhills, int *__restrict__ step, int *__restrict__ aux,
                      unsigned int *__restrict__ sticky, int stride, double w0, double kT, double gamma, double force_scale,
                      double *__restrict__ cv_out, double *__restrict__ V_out, double *__restrict__ dVds_out,
-                     double *__restrict__ tors_grad, T *__restrict__ F) {
+                     double *__restrict__ tors_grad, T *__restrict__ F, double *__restrict__ traj, int traj_cap) {
     __shared__ double s_cv[METAD_MAX_CV], s_g[METAD_MAX_CV][12], s_V, s_dV[METAD_MAX_CV];
     __shared__ int s_exact;
     __shared__ double red[(1 + METAD_MAX_CV) * 32];
@@ -317,6 +321,10 @@ k_fused_torsion_step(FusedTors ft, const int *__restrict__ tors_atoms, const T *
         for (int d = 0; d < bp.D; ++d) dVds_out[d] = s_dV[d];
         const int st = *step + 1;
         *step = st;
+        if (traj) {
+            if (st <= traj_cap) { for (int d = 0; d < bp.D; ++d) traj[(size_t)(st - 1) * bp.D + d] = s_cv[d]; }
+            else atomicOr(sticky, (unsigned)METAD_DEV_TRAJ_FULL);
+        }
         aux[AUX_DEP_INDEX] = -1;
         if (stride > 0 && st % stride == 0) {
             const int H = *nhills;
@@ -395,7 +403,8 @@ int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds) {
 int bias_deposit(metad_ctx *c, const double *d_cv, const double *d_V) {
     BiasParams bp = make_bp(c);
     k_deposit<<<1, 32, 0, c->stream>>>(bp, c->p.stride, c->p.w0, c->p.kT, c->p.bias_factor, d_cv, d_V, c->d_centers,
-                                       c->d_heights, c->d_nhills, c->d_step, ctx_aux(c), c->d_sticky);
+                                       c->d_heights, c->d_nhills, c->d_step, ctx_aux(c), c->d_sticky, c->d_traj,
+                                       c->p.traj_capacity);
     c->launches++;
     if (c->grid_on) {
         int nn = c->p.grid_n[0] * c->p.grid_n[1];
@@ -448,11 +457,11 @@ int bias_fused_torsion_step(metad_ctx *c, const void *d_pos, void *d_F) {
     if (c->prec == 32)
         k_fused_torsion_step<float><<<1, 256, 0, c->stream>>>(ft, c->d_tors_atoms, (const float *)d_pos, c->boxd, bp, gp, c->grid_on,
             c->d_table, c->d_centers, c->d_heights, c->d_nhills, c->d_step, ctx_aux(c), c->d_sticky, c->p.stride, c->p.w0, c->p.kT,
-            c->p.bias_factor, c->p.force_scale, c->d_cv, c->d_V, c->d_dVds, c->d_tors_grad, (float *)d_F);
+            c->p.bias_factor, c->p.force_scale, c->d_cv, c->d_V, c->d_dVds, c->d_tors_grad, (float *)d_F, c->d_traj, c->p.traj_capacity);
     else
         k_fused_torsion_step<double><<<1, 256, 0, c->stream>>>(ft, c->d_tors_atoms, (const double *)d_pos, c->boxd, bp, gp, c->grid_on,
             c->d_table, c->d_centers, c->d_heights, c->d_nhills, c->d_step, ctx_aux(c), c->d_sticky, c->p.stride, c->p.w0, c->p.kT,
-            c->p.bias_factor, c->p.force_scale, c->d_cv, c->d_V, c->d_dVds, c->d_tors_grad, (double *)d_F);
+            c->p.bias_factor, c->p.force_scale, c->d_cv, c->d_V, c->d_dVds, c->d_tors_grad, (double *)d_F, c->d_traj, c->p.traj_capacity);
     c->launches++;
     if (c->grid_on) {
         int nn = c->p.grid_n[0] * c->p.grid_n[1];

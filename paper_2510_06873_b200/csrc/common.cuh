@@ -180,6 +180,7 @@ struct metad_ctx {
     // CV state
     CvDev cv[METAD_MAX_CV];
     bool has_q6, has_coord, has_torsion, has_mindist, has_lattice;
+    double *d_traj;                       // traj_capacity > 0: [capacity][D] CV frames, frame k = step k + 1 since the last reset
     double *d_virial, *d_vir_partials;    // want_virial: [9] bias virial of the last apply_forces; per-block partials
     double *d_box_force;                  // LATTICE: [9] bias force on the box rows, written by apply_forces
     int mindist_dim;

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmetad_b200.so")
 
 MAX_CV = 4
 OK, ERR_ARG, ERR_BOX, ERR_STATE, ERR_CUDA, ERR_NOMEM = range(6)
-DEV_NEIGH_OVERFLOW, DEV_HILL_OVERFLOW, DEV_GRID_RANGE, DEV_NONFINITE, DEV_POS_RANGE = 1, 2, 4, 8, 16
+DEV_NEIGH_OVERFLOW, DEV_HILL_OVERFLOW, DEV_GRID_RANGE, DEV_NONFINITE, DEV_POS_RANGE, DEV_TRAJ_FULL = 1, 2, 4, 8, 16, 32
 CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CV_MINDIST, CV_LATTICE = range(8)
 
 _P = ctypes.c_void_p
@@ -36,13 +36,13 @@ class Params(ctypes.Structure):
     _fields_ = [("natoms", _I), ("precision", _I), ("max_neigh", _I), ("ncv", _I),
                 ("cv", CvDesc * MAX_CV), ("sigma", _D * MAX_CV), ("w0", _D), ("kT", _D),
                 ("bias_factor", _D), ("max_hills", _I), ("stride", _I), ("grid_n", _I * 2),
-                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("lazy_neighbors", _I), ("want_virial", _I)]
+                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("traj_capacity", _I), ("lazy_neighbors", _I), ("want_virial", _I)]
 
 
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
            "metad_apply_forces", "metad_deposit", "metad_run", "metad_step_host", "metad_status",
            "metad_get_state", "metad_get_neighbors", "metad_get_q6", "metad_set_hills", "metad_get_hills",
-           "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
+           "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reweight_recorded", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
 
 _lib = None
 
@@ -77,6 +77,7 @@ def load():
     L.metad_get_virial.argtypes = [_P, _P]
     L.metad_bias_batch.argtypes = [_P, _P, _I, _P]
     L.metad_reweight.argtypes = [_P, _P, _I, _P, _P, _P, _P, _P]
+    L.metad_reweight_recorded.argtypes = [_P, _P, _P, _P, _P, _P, _P]
     L.metad_set_timing.argtypes = [_P, _I]
     L.metad_get_timing.argtypes = [_P, _P, _P]
     L.metad_launch_count.argtypes = [_P]
@@ -107,7 +108,7 @@ class MetaD:
     fields); tensors passed to the methods are torch CUDA tensors (float64, or float32 for pos/F when
     precision == 32)."""
 
-    def __init__(self, workload, max_hills=None, precision=None, grid=None, force_scale=1.0, stream=None, want_virial=False, lazy_neighbors=False):
+    def __init__(self, workload, max_hills=None, precision=None, grid=None, force_scale=1.0, stream=None, want_virial=False, lazy_neighbors=False, traj_capacity=0):
         import torch
         self.torch = torch
         L = load()
@@ -159,6 +160,7 @@ class MetaD:
         p.force_scale = float(force_scale)
         p.want_virial = 1 if want_virial else 0
         p.lazy_neighbors = 1 if lazy_neighbors else 0
+        p.traj_capacity = int(traj_capacity)
         self._params = p
         h = _P()
         _check(L.metad_create(ctypes.byref(h), ctypes.byref(p), _P(self.stream.cuda_stream)))
@@ -307,6 +309,19 @@ class MetaD:
             F = torch.empty((nb[0], nb[1]), dtype=torch.float64, device="cuda")
         _check(load().metad_reweight(self._h, _ptr(traj), T, nb, lo2, hi2, _ptr(P), _ptr(F)))
         return P.cpu().numpy(), F.cpu().numpy()
+
+    def reweight_recorded(self, nbins, lo, hi):
+        """(P, F, nframes) from the CV frames recorded on the device (needs traj_capacity > 0)."""
+        torch = self.torch
+        nb = (ctypes.c_int * 2)(int(nbins[0]), int(nbins[1]) if self.D > 1 else 1)
+        lo2 = (ctypes.c_double * 2)(float(lo[0]), float(lo[1]) if self.D > 1 else 0.0)
+        hi2 = (ctypes.c_double * 2)(float(hi[0]), float(hi[1]) if self.D > 1 else 1.0)
+        with torch.cuda.stream(self.stream):
+            P = torch.empty((nb[0], nb[1]), dtype=torch.float64, device="cuda")
+            F = torch.empty((nb[0], nb[1]), dtype=torch.float64, device="cuda")
+        n = ctypes.c_int(0)
+        _check(load().metad_reweight_recorded(self._h, nb, lo2, hi2, _ptr(P), _ptr(F), ctypes.byref(n)))
+        return P.cpu().numpy(), F.cpu().numpy(), n.value
 
     def reset_steps(self):
         _check(load().metad_reset_steps(self._h))

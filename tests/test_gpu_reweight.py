@@ -96,3 +96,44 @@ def test_reweight_argument_errors():
         md.reweight(dt, [8, 8], [-np.pi, -np.pi], [np.pi, 3.0])        # span != period
     with pytest.raises(MetadError):
         md.reweight(dt, [0, 8], [-np.pi, -np.pi], [np.pi, np.pi])
+
+
+@pytest.mark.parametrize("fused", [False, True])
+def test_recorded_trajectory_is_reweighted_on_the_device(fused):
+    """The CV frames of a run stay on the GPU (params.traj_capacity) and feed metad_reweight_recorded; the same frames,
+    read back step by step, go through the oracle."""
+    import torch
+    from paper_2510_06873_b200 import metad
+    from paper_2510_06873_b200.metad import MetaD
+    w = configs.small("t0")
+    w.stride = 3
+    rng = np.random.default_rng(31)
+    c = hill_walk_periodic(5, np.array([-1.4, -0.9]), w.sigma, 60, w.period, w.extra["period_lo"])
+    h = seeded_heights(5, 60, w.w0)
+    md = MetaD(w, max_hills=128, traj_capacity=40, lazy_neighbors=fused)
+    md.set_hills(c, h)
+    F = torch.zeros((w.natoms, 3), device="cuda", dtype=torch.float64)
+    frames = []
+    for k in range(25):
+        pos = w.pos + rng.standard_normal(w.pos.shape) * 0.08
+        dpos = torch.tensor(pos, device="cuda")
+        torch.cuda.synchronize()
+        md.run(dpos, F, 1)
+        frames.append(md.state()["cv"].copy())
+    frames = np.array(frames)
+    nb, lo, hi = [96, 80], [-np.pi, -np.pi], [np.pi, np.pi]
+    P, Fe, n = md.reweight_recorded(nb, lo, hi)
+    assert n == 25
+    cc, hh = md.get_hills()
+    assert len(hh) == 60 + 25 // 3
+    P_ref, F_ref = oracle.reweight(frames, cc, hh, w.sigma, w.period, w.kT, nb, lo, hi)
+    assert np.abs(P - P_ref).max() <= 1e-9 * P_ref.max()
+    ok = P_ref > 1e-5 * P_ref.max()
+    assert ok.sum() >= 1 and (np.abs(P[ok] - P_ref[ok]) / P_ref[ok]).max() <= TOL_CV
+    # capacity: frames beyond it are dropped and flagged
+    md.run(dpos, F, 20)
+    _, _, n2 = md.reweight_recorded(nb, lo, hi)
+    assert n2 == 40 and md.status() & metad.DEV_TRAJ_FULL
+    md.reset_steps()
+    md.run(dpos, F, 2)
+    assert md.reweight_recorded(nb, lo, hi)[2] == 2
