@@ -292,7 +292,7 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
     const char *env = getenv("METAD_NO_TILES");
     const bool q6_only = c->has_q6 && !c->has_coord;
     const bool coord_only = c->has_coord && !c->has_q6 && !c->cv[c->coord_dim].use_groups;
-    if (c->prec == 32 && (q6_only || coord_only) && !c->has_mindist && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32 &&
+    if (c->prec == 32 && (q6_only || coord_only) && !c->has_mindist && c->N < (1 << NL_IDX_BITS) && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32 &&
         !(env && env[0] == '1')) {
         // the rc-wide cells are subdivided along x (the direction of the contiguous row runs): an atom then scans
         // 2 xsub + 1 sub-cells per row (2.5 / 2.25 cell widths for xsub = 2 / 4) instead of 3 cells
