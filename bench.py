@@ -40,6 +40,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fast-setup", action="store_true",
                     help="profiling runs only: seeded hill heights instead of the well-tempered replay, no e2e leg")
+    ap.add_argument("--lazy", action="store_true", help="params.lazy_neighbors: skip the list build when no CV reads it (c1, t0)")
     ap.add_argument("--virial", action="store_true", help="also compute the bias virial every step (NPT; COORD / Q6 / LATTICE CVs)")
     ap.add_argument("--stage-times", action="store_true", default=True)
     return ap.parse_args()
@@ -58,7 +59,9 @@ def describe(w, precision):
     return {"workload": wl, "atoms": int(w.natoms),
             "cvs": [kinds[c.kind] for c in w.cvs], "hills": int(w.n_hills), "rc": w.rc,
             "pair_precision": f"fp{precision}", "stride": int(w.stride), "virial": bool(getattr(w, "_virial", False)),
-            "neighbour_build": ("skipped (lazy_neighbors: no CV of this workload reads the list)" if w.name == "t0" else "every step"),
+            "neighbour_build": ("skipped (lazy_neighbors: no CV of this workload reads the list)"
+                                if (w.name == "t0" or getattr(w, "_lazy", False)) and all(c.kind in (3, 4, 5, 7) for c in w.cvs)
+                                else "every step"),
             "l2": ("per-step working set (neighbour list + q6 records + positions + forces) exceeds the 126 MB L2; no flush"
                    if w.natoms * (4 * w.max_neigh + 64 + 16 + 24 + 16) > 126e6 else
                    "working set fits the 126 MB L2 and is not flushed: this workload is bound by the latency of its ~10 "
@@ -255,6 +258,7 @@ def run_ours(args):
 
     w = workload(args.config)
     w._virial = bool(args.virial)
+    w._lazy = bool(args.lazy)
     precision = args.precision or (32 if args.config in ("c3", "c4", "g0") else w.precision)
     tdt = torch.float32 if precision == 32 else torch.float64
     pos = w.pos.astype(np.float32 if precision == 32 else np.float64)
@@ -279,7 +283,7 @@ def run_ours(args):
         sig = np.asarray(w.sigma)
         grid = (w.grid_n, centers[0] - 120 * sig, centers[0] + 120 * sig)      # reading M
     md = MetaD(w, precision=precision, max_hills=w.n_hills + args.steps + args.warmup + 4096, grid=grid,
-               want_virial=args.virial, lazy_neighbors=(args.config == "t0"))
+               want_virial=args.virial, lazy_neighbors=(args.config == "t0" or args.lazy))
     md.set_hills(centers, heights)
     with torch.cuda.stream(md.stream):
         F = torch.zeros((w.natoms, 3), device="cuda", dtype=tdt)
