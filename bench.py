@@ -35,7 +35,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="c3", choices=["c0", "c1", "c2", "c3", "c4", "t0", "g0"])
+    ap.add_argument("--config", default="c3", choices=["c0", "c1", "c2", "c3", "c4", "t0", "g0", "r0"])
     ap.add_argument("--precision", type=int, default=0, help="0 = the workload's own (c3: 32 for the headline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fast-setup", action="store_true",
@@ -54,13 +54,14 @@ def workload(name):
 def describe(w, precision):
     kinds = {0: "coordination", 1: "Q6 mean", 2: "Q6 solid-like count", 3: "radius of gyration", 4: "native contacts", 5: "torsion", 6: "distance to nearest", 7: "lattice parameter"}
     wl = {"t0": "PAPER.md:37 alanine-dipeptide-shaped torsion workload (t0, SURVEY.md §8(f) NEXT-1)",
+          "r0": "PAPER.md:43 surface-O ... nearest-H distance, well-tempered, on the configs[2] slab + water structure (r0)",
           "g0": "PAPER.md:51 GaN CV set (coordination number + 3 lattice parameters) on the configs[3] structure (g0)"
           }.get(w.name, f"BASELINE.json configs[{w.name[1]}] ({w.name})")
     return {"workload": wl, "atoms": int(w.natoms),
             "cvs": [kinds[c.kind] for c in w.cvs], "hills": int(w.n_hills), "rc": w.rc,
             "pair_precision": f"fp{precision}", "stride": int(w.stride), "virial": bool(getattr(w, "_virial", False)),
             "neighbour_build": ("skipped (lazy_neighbors: no CV of this workload reads the list)"
-                                if (w.name == "t0" or getattr(w, "_lazy", False)) and all(c.kind in (3, 4, 5, 7) for c in w.cvs)
+                                if (w.name in ("t0", "r0") or getattr(w, "_lazy", False)) and all(c.kind in (3, 4, 5, 6, 7) for c in w.cvs)
                                 else "every step"),
             "l2": ("per-step working set (neighbour list + q6 records + positions + forces) exceeds the 126 MB L2; no flush"
                    if w.natoms * (4 * w.max_neigh + 64 + 16 + 24 + 16) > 126e6 else
@@ -283,7 +284,7 @@ def run_ours(args):
         sig = np.asarray(w.sigma)
         grid = (w.grid_n, centers[0] - 120 * sig, centers[0] + 120 * sig)      # reading M
     md = MetaD(w, precision=precision, max_hills=w.n_hills + args.steps + args.warmup + 4096, grid=grid,
-               want_virial=args.virial, lazy_neighbors=(args.config == "t0" or args.lazy))
+               want_virial=args.virial, lazy_neighbors=(args.config in ("t0", "r0") or args.lazy))
     md.set_hills(centers, heights)
     with torch.cuda.stream(md.stream):
         F = torch.zeros((w.natoms, 3), device="cuda", dtype=tdt)

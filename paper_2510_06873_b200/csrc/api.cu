@@ -78,6 +78,10 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
                 c->coord_dim = d; c->has_coord = true;
             } else {
                 c->mindist_dim = d; c->has_mindist = true;
+                if (s.group_a && s.group_b && s.n_a > 0 && s.n_b > 0) {      // list-free variant needs explicit groups
+                    v.n_ga = s.n_a; v.n_gb = s.n_b;
+                    if (upload_ints(&v.d_ga, s.group_a, s.n_a) || upload_ints(&v.d_gb, s.group_b, s.n_b)) return METAD_ERR_CUDA;
+                }
             }
             v.use_groups = s.group_a || s.group_b;
             if (v.use_groups) {
@@ -243,7 +247,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
-        void *q2[] = { v.d_pairs, v.d_pair_r0, v.d_csr_off, v.d_csr_pair, v.d_catoms, v.d_chain, v.d_mass, v.d_unwrapped };
+        void *q2[] = { v.d_pairs, v.d_pair_r0, v.d_csr_off, v.d_csr_pair, v.d_catoms, v.d_chain, v.d_mass, v.d_unwrapped, v.d_ga, v.d_gb };
         for (void *q : q2) if (q) cudaFree(q);
     }
     delete c;
@@ -338,7 +342,10 @@ extern "C" int metad_build_neighbors(metad_ctx *c, const void *d_pos, const doub
     int r = setup_geometry(c, h_box, rc);
     if (r) return r;
     c->d_pos_last = d_pos;
-    if (c->p.lazy_neighbors && !c->has_q6 && !c->has_coord && !c->has_mindist) {   // no CV reads the list
+    // no CV reads the list; a nearest-distance CV with a few explicit centres is scanned without one (k_mindist_brute)
+    const bool mind_brute = c->has_mindist && c->cv[c->mindist_dim].d_ga && c->cv[c->mindist_dim].n_ga <= 64 &&
+                            div_up(c->cv[c->mindist_dim].n_gb, 128) <= c->nblocks_atoms;
+    if (c->p.lazy_neighbors && !c->has_q6 && !c->has_coord && (!c->has_mindist || mind_brute)) {
         c->have_neighbors = true; c->list_built = false;
         return METAD_OK;
     }

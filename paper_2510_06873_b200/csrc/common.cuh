@@ -160,6 +160,7 @@ struct CvDev {                      // device copies of one CV descriptor
     double *d_unwrapped;                  // RGYR scratch: [nchain*3] + com[3] + rg
     bool use_groups;
     int tors[4];                          // TORSION
+    int *d_ga, *d_gb; int n_ga, n_gb;     // MINDIST: device copies of the group index lists (list-free variant)
 };
 
 struct metad_ctx {

@@ -632,6 +632,68 @@ __global__ void k_mindist_force(const double *__restrict__ rec, double force_sca
             for (int q = 0; q < 3; ++q) virial[3 * p + q] += -a * rec[1 + p] * rec[1 + q];
 }
 
+// List-free variant for a few centres (ONE surface oxygen against all hydrogens): thread per group-B atom
+// loops over the nA centres with the fp64 minimum image of reading O on the caller's positions; same arg-min reduction.
+// Chosen when params.lazy_neighbors is set and MINDIST is the only CV that would read the list.
+template <typename T>
+__global__ void __launch_bounds__(CV_THREADS)
+k_mindist_brute(int nA, const int *__restrict__ ga, int nB, const int *__restrict__ gb, const T *__restrict__ pos, BoxD bd,
+                double rc, double *__restrict__ part_r2, long long *__restrict__ part_ij, unsigned int *__restrict__ ticket,
+                double *__restrict__ rec, double *__restrict__ cv_out) {
+    __shared__ double s_r2[32];
+    __shared__ long long s_ij[32];
+    const int t = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double r2 = 1e300; long long ij = 0x7fffffffffffffffll; int u0 = -1, u1 = -1;     // u0/u1 unused payload of min_warp
+    const double rc2 = rc * rc;
+    if (t < nB) {
+        const int j = gb[t];
+        const double xj = (double)pos[3 * (size_t)j], yj = (double)pos[3 * (size_t)j + 1], zj = (double)pos[3 * (size_t)j + 2];
+        for (int a = 0; a < nA; ++a) {
+            const int i = ga[a];
+            if (i == j) continue;
+            const double q = r2_canonical(bd, xj - (double)pos[3 * (size_t)i], yj - (double)pos[3 * (size_t)i + 1],
+                                          zj - (double)pos[3 * (size_t)i + 2]);
+            const long long key = ((long long)i << 32) | (long long)j;
+            if (q < rc2 && min_less(q, key, r2, ij)) { r2 = q; ij = key; }
+        }
+    }
+    min_warp(r2, ij, u0, u1);
+    if (lane == 0) { s_r2[wid] = r2; s_ij[wid] = ij; }
+    __syncthreads();
+    if (wid == 0) {
+        const int nw = blockDim.x >> 5;
+        r2 = lane < nw ? s_r2[lane] : 1e300; ij = lane < nw ? s_ij[lane] : 0x7fffffffffffffffll;
+        min_warp(r2, ij, u0, u1);
+        if (lane == 0) { part_r2[blockIdx.x] = r2; part_ij[blockIdx.x] = ij; }
+    }
+    if (last_block_ticket(ticket)) {
+        r2 = 1e300; ij = 0x7fffffffffffffffll;
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x)
+            if (min_less(part_r2[b], part_ij[b], r2, ij)) { r2 = part_r2[b]; ij = part_ij[b]; }
+        min_warp(r2, ij, u0, u1);
+        if (lane == 0) { s_r2[wid] = r2; s_ij[wid] = ij; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < (int)(blockDim.x >> 5); ++w)
+                if (min_less(s_r2[w], s_ij[w], r2, ij)) { r2 = s_r2[w]; ij = s_ij[w]; }
+            int *pair = reinterpret_cast<int *>(rec + 4);
+            if (!(r2 < 1e299)) {
+                rec[0] = rc; rec[1] = rec[2] = rec[3] = 0.0; pair[0] = pair[1] = -1;
+                *cv_out = rc;
+            } else {
+                const int i = (int)(ij >> 32), j = (int)(ij & 0xffffffffll);
+                double dx = (double)pos[3 * (size_t)j] - (double)pos[3 * (size_t)i],
+                       dy = (double)pos[3 * (size_t)j + 1] - (double)pos[3 * (size_t)i + 1],
+                       dz = (double)pos[3 * (size_t)j + 2] - (double)pos[3 * (size_t)i + 2];
+                min_image_d(bd, dx, dy, dz);
+                const double r = sqrt(dx * dx + dy * dy + dz * dz);
+                rec[0] = r; rec[1] = dx; rec[2] = dy; rec[3] = dz; pair[0] = i; pair[1] = j;
+                *cv_out = r;
+            }
+        }
+    }
+}
+
 template <typename T>
 static int mindist_eval_t(metad_ctx *c, double *d_cv) {
     typedef typename Vec4<T>::type V4;
@@ -647,6 +709,21 @@ static int mindist_eval_t(metad_ctx *c, double *d_cv) {
 }
 int mindist_eval(metad_ctx *c, double *d_cv) {
     if (!c->has_mindist) return METAD_OK;
+    if (!c->list_built) {                                       // lazy_neighbors: list-free scan of the few centres
+        const CvDev &d = c->cv[c->mindist_dim];
+        const int nb = div_up(d.n_gb, CV_THREADS);
+        double *pr = c->d_partials;
+        long long *pk = reinterpret_cast<long long *>(c->d_partials + c->nblocks_atoms);
+        if (c->prec == 32)
+            k_mindist_brute<float><<<nb, CV_THREADS, 0, c->stream>>>(d.n_ga, d.d_ga, d.n_gb, d.d_gb, (const float *)ctx_last_pos(c), c->boxd,
+                                                                     c->rc, pr, pk, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim);
+        else
+            k_mindist_brute<double><<<nb, CV_THREADS, 0, c->stream>>>(d.n_ga, d.d_ga, d.n_gb, d.d_gb, (const double *)ctx_last_pos(c), c->boxd,
+                                                                      c->rc, pr, pk, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim);
+        c->launches++;
+        CUDA_TRY(cudaGetLastError());
+        return METAD_OK;
+    }
     return c->prec == 32 ? mindist_eval_t<float>(c, d_cv) : mindist_eval_t<double>(c, d_cv);
 }
 int mindist_forces(metad_ctx *c, const double *d_dVds, void *d_F) {

@@ -6,7 +6,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import (BASE_SEED, CV_LATTICE, CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CVSpec, Workload,
+from . import (BASE_SEED, CV_LATTICE, CV_MINDIST, CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CVSpec, Workload,
                hill_walk_periodic, rsa, wrap)
 
 
@@ -214,6 +214,25 @@ def config_t0(seed=BASE_SEED + 10, natoms=22, n_hills=20000, grid=(256, 256), n_
                     extra={"period_lo": [-np.pi, -np.pi]})
 
 
+# ----------------------------------------------------------------------------------------- r0
+def config_r0(seed=BASE_SEED + 2, ncell=40, n_water=20533, n_hills=20000):
+    """The CV of the paper's second workload ("the distance between a surface oxygen atom and its nearest
+    hydrogen atom", well-tempered metadynamics) on the slab + water structure of BASELINE.json configs[2] (same seed, same
+    atoms): 1-D CV = distance from ONE top-layer anion (the middle one of group A) to its nearest H within rc = 5 A (the
+    water layer starts 2 A above the slab, so 3 A does not always reach a hydrogen); bias factor 10, width 0.05 A,
+    20,000 hills."""
+    w = config2(seed=seed, ncell=ncell, n_water=n_water, n_hills=n_hills)
+    cv = w.cvs[0]
+    A = np.asarray(cv.group_a)
+    w.name = "r0"
+    w.cvs = [CVSpec(kind=CV_MINDIST, group_a=A[len(A) // 2:len(A) // 2 + 1], group_b=cv.group_b)]
+    w.sigma = [0.05]
+    w.bias_factor = 10.0
+    w.rc = 5.0
+    w.max_neigh = 128
+    return w
+
+
 # ----------------------------------------------------------------------------------------- g0
 def config_g0(seed=BASE_SEED + 3, cells=(80, 80, 40), sphere_r=30.0, n_hills=10000):
     """The CV set of the paper's own GaN runs ("the coordination number (C.N.) and the triaxial lattice
@@ -246,7 +265,9 @@ def small(name):
         return config_t0(n_hills=500, grid=(48, 40))
     if name == "g0":
         return config_g0(cells=(12, 12, 8), sphere_r=9.0, n_hills=400)
+    if name == "r0":
+        return config_r0(ncell=8, n_water=800, n_hills=500)
     raise KeyError(name)
 
 
-BUILDERS = {"c0": config0, "c1": config1, "c2": config2, "c3": config3, "c4": config4, "t0": config_t0, "g0": config_g0}
+BUILDERS = {"c0": config0, "c1": config1, "c2": config2, "c3": config3, "c4": config4, "t0": config_t0, "g0": config_g0, "r0": config_r0}

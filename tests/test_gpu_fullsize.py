@@ -54,3 +54,10 @@ def test_torsion_workload_full_size():
     """PAPER.md:37 workload in the configuration bench.py --config t0 times (20,000 hills, periodic)."""
     r = stagewise(configs.config_t0())
     assert_stagewise(r)
+
+
+def test_nearest_hydrogen_workload_full_size():
+    """PAPER.md:43 workload in the configuration bench.py --config r0 times (99,999 atoms, one surface oxygen)."""
+    r = stagewise(configs.config_r0())
+    assert_stagewise(r)
+    assert 0.5 < r["s_ref"][0] < 5.0
