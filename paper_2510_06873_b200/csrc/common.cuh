@@ -8,6 +8,8 @@
 // generic (non-tiled) kernels switch from one thread to one warp per atom below this size: a system this small cannot
 // fill 148 SMs with one thread per atom (BASELINE.json configs[0]-[2] are latency-bound otherwise)
 #define METAD_WARP_PER_ATOM_MAX 32768
+// below this size the neighbour stage is one brute-force kernel without cells (k_build_list_small)
+#define METAD_SMALL_N 1024
 
 #define METAD_NREC 16  // per-atom Q6 record: 13 normalised q6m components + f'(q6) + q6 + pad
 

@@ -264,6 +264,50 @@ k_build_list_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const 
     }
 }
 
+// Systems of at most METAD_SMALL_N atoms: no cells at all.  One warp per atom tests every other atom with the canonical
+// predicate (N^2 / 32 tests per lane), the ballot keeps ascending j; the kernel also writes the identity "sort" (spos = the
+// positions in their original order, perm = identity), so that the whole of a1 is ONE launch instead of six.
+template <typename T>
+__global__ void __launch_bounds__(128)
+k_build_list_small(int N, const T *__restrict__ pos, const unsigned char *__restrict__ flags,
+                   typename Vec4<T>::type *__restrict__ spos, int *__restrict__ perm, int *__restrict__ scell,
+                   PBox<T> pb, BoxD bd, T rc2T, double rc2, int maxn, int *__restrict__ nl_count, int *__restrict__ nl,
+                   CellGrid g, unsigned int *__restrict__ sticky) {
+    const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (s >= N) return;
+    typename Vec4<T>::type pi;
+    pi.x = pos[3 * s]; pi.y = pos[3 * s + 1]; pi.z = pos[3 * s + 2];
+    pi.w = (T)(flags ? (int)flags[s] : 3);
+    if (lane == 0) {
+        spos[s] = pi; perm[s] = s; scell[s] = 0;
+        // positions must lie in the primary cell (same check as k_bin)
+        const double sc = (double)pi.z * g.inv[2], sb = ((double)pi.y - sc * g.cy) * g.inv[1],
+                     sa = ((double)pi.x - sb * g.bx - sc * g.cx) * g.inv[0];
+        if (!(fabs(sa - 0.5) <= 0.5001) || !(fabs(sb - 0.5) <= 0.5001) || !(fabs(sc - 0.5) <= 0.5001))
+            atomicOr(sticky, (unsigned)METAD_DEV_POS_RANGE);
+    }
+    int cnt = 0;
+    for (int j0 = 0; j0 < N; j0 += 32) {
+        const int j = j0 + lane;
+        bool hit = false;
+        if (j < N && j != s) {
+            typename Vec4<T>::type pj;
+            pj.x = pos[3 * j]; pj.y = pos[3 * j + 1]; pj.z = pos[3 * j + 2]; pj.w = T(0);
+            hit = pair_in_range<T>(pb, bd, rc2T, rc2, pi, pj);
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, hit);
+        if (hit) {
+            const int k = cnt + __popc(m & ((1u << lane) - 1u));
+            if (k < maxn) nl[(size_t)k * N + s] = j;
+        }
+        cnt += __popc(m);
+    }
+    if (lane == 0) {
+        if (cnt > maxn) { atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW); cnt = maxn; }
+        nl_count[s] = cnt;
+    }
+}
+
 __global__ void k_export_list(int N, int maxn, const int *__restrict__ perm, const int *__restrict__ nl_count,
                               const int *__restrict__ nl, int *__restrict__ out_count, int *__restrict__ out_list) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -302,6 +346,16 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     cudaStream_t st = c->stream;
     const int nsb = div_up(ncell, SCAN_TILE);
     const bool tm = c->timing && !c->capturing;
+    if (N <= METAD_SMALL_N && !c->tiled) {                     // the whole neighbour stage in one launch
+        if (tm) { cudaEventRecord(c->ev[0], st); cudaEventRecord(c->ev[1], st); c->timing_recorded = 1; }
+        k_build_list_small<T><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const T *)d_pos, c->d_flags, (V4 *)c->d_spos, c->d_perm,
+                                                                             c->d_scell, make_pbox<T>(c->boxd), c->boxd, (T)c->rc2, c->rc2,
+                                                                             c->maxn, c->d_nl_count, c->d_nl, c->grid, c->d_sticky);
+        if (tm) cudaEventRecord(c->ev[2], st);
+        c->launches += 1;
+        CUDA_TRY(cudaGetLastError());
+        return METAD_OK;
+    }
     if (tm) { cudaEventRecord(c->ev[0], st); c->timing_recorded = 1; }
     k_bin<T><<<div_up(N, 256), 256, 0, st>>>(N, (const T *)d_pos, c->grid, c->d_cell_of, c->d_slot, c->d_cell_count,
                                              c->d_sticky);
