@@ -127,7 +127,7 @@ template <typename T>
 __global__ void k_cell_sort_gather(int N, const int *__restrict__ cell_start, const int *__restrict__ cell_of,
                                    const int *__restrict__ perm_in, int *__restrict__ perm,
                                    const T *__restrict__ pos, const unsigned char *__restrict__ flags,
-                                   typename Vec4<T>::type *__restrict__ spos, int *__restrict__ scell) {
+                                   typename Vec4<T>::type *__restrict__ spos, int *__restrict__ scell, int index_in_w) {
     int a = blockIdx.x * blockDim.x + threadIdx.x;
     if (a >= N) return;
     const int i = perm_in[a], c = cell_of[i];
@@ -138,6 +138,9 @@ __global__ void k_cell_sort_gather(int N, const int *__restrict__ cell_start, co
     v.x = pos[3 * i]; v.y = pos[3 * i + 1]; v.z = pos[3 * i + 2];
     v.w = (T)(flags ? (int)flags[i] : 3);
     const int d = b + rank;
+    // tiled fp32 contexts have no group flags: .w carries (sorted index | no-shift code << 27), the neighbour-list entry of
+    // this atom, so that interior tiles can be staged by raw bulk copies (tile.cuh)
+    if (index_in_w && sizeof(T) == 4) v.w = (T)__int_as_float(d | (13 << 27));
     perm[d] = i;
     spos[d] = v;
     scell[d] = c;
@@ -364,7 +367,7 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     k_scatter<<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_of, c->d_slot, c->d_cell_start, c->d_perm_raw);
     k_cell_sort_gather<T><<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_start, c->d_cell_of, c->d_perm_raw, c->d_perm, (const T *)d_pos,
                                                              c->d_flags,   /* NULL unless a COORD / MINDIST CV has groups */
-                                                             (V4 *)c->d_spos, c->d_scell);
+                                                             (V4 *)c->d_spos, c->d_scell, c->tiled ? 1 : 0);
     if (tm) cudaEventRecord(c->ev[1], st);
     if (c->tiled && sizeof(T) == 4) {
         c->launches += 5;

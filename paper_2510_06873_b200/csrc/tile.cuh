@@ -44,6 +44,7 @@ struct TileTables {
     int own_row[TILE_MAXOWN];    // halo row id of own-row q
     float origin[3];
     int x0, y0, z0, Txe, Tye, Tze, nrows, nown, total, staged;
+    int any_wrapped;             // some non-empty segment of the halo is a periodic image (boundary tile)
 };
 
 __device__ __forceinline__ int tile_row_id(const TileTables &t, int hy, int hz) {   // hy,hz in [-1, T*e]
@@ -86,7 +87,7 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
         w.hbeg[r][c] = cell_start[id];
         w.hend[r][c] = cell_start[id + 1];
     }
-    if (tid == 0) { t.x0 = x0; t.y0 = y0; t.z0 = z0; t.Txe = Txe; t.Tye = Tye; t.Tze = Tze; t.nrows = nrows; }
+    if (tid == 0) { t.x0 = x0; t.y0 = y0; t.z0 = z0; t.Txe = Txe; t.Tye = Tye; t.Tze = Tze; t.nrows = nrows; t.any_wrapped = 0; }
     if (tid >= blockDim.x - 32) {
         // coordinate range of the halo'd tile (8 corners of the parallelepiped, one per lane), origin = point nearest to 0
         const int c = tid & 7;
@@ -121,6 +122,7 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
         if (ls <= le) { const int sg = w.hbeg[r][ls - xa]; t.seg_g[tid] = sg; t.seg_len[tid] = w.hend[r][le - xa] - sg; }
         else { t.seg_g[tid] = 0; t.seg_len[tid] = 0; }
         t.seg_wrapped[tid] = (wx | wy | wz) != 0;
+        if ((wx | wy | wz) != 0 && ls <= le && t.seg_len[tid] > 0) t.any_wrapped = 1;      // benign race: every writer stores 1
         t.seg_code[tid] = (unsigned char)((wx + 1) + 3 * (wy + 1) + 9 * (wz + 1));
     }
     for (int i = tid; i < nrows * ncol; i += blockDim.x) {
@@ -222,6 +224,38 @@ __device__ __forceinline__ void tile_stage_pos(const TileGeom &g, const TileTabl
     for (int s = wid; s < 3 * t.nrows; s += nw) {
         const int len = t.seg_len[s], g0 = t.seg_g[s], l0 = t.seg_off[s];
         for (int i = lane; i < len; i += 32) pos_s[l0 + i] = tile_transform(g, t, s, spos[g0 + i], g0 + i);
+    }
+}
+
+// Interior tiles (no periodic image in the halo): every segment is a contiguous range of the cell-sorted float4 array whose
+// .w already holds (sorted index | no-shift code) (k_cell_sort_gather on tiled contexts), so the staging is a handful of TMA
+// bulk copies (cp.async.bulk, one per segment, completion on an mbarrier) of the RAW coordinates — differences of fp32
+// inputs inside the primary cell are exact, no origin is needed.  All threads of the block must call it; returns after the
+// data has landed.
+__device__ __forceinline__ void tile_stage_pos_tma(const TileTables &t, const float4 *__restrict__ spos, float4 *pos_s,
+                                                   unsigned long long *bar) {
+    const unsigned bar_a = (unsigned)__cvta_generic_to_shared(bar);
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_a));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // the set-up scratch lived where the copies will land
+    __syncthreads();
+    if (threadIdx.x == 0)
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_a), "r"((unsigned)t.total * 16u) : "memory");
+    if (threadIdx.x < 3 * t.nrows) {
+        const int len = t.seg_len[threadIdx.x];
+        if (len > 0) {
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(pos_s + t.seg_off[threadIdx.x]);
+            const float4 *src = spos + t.seg_g[threadIdx.x];
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(dst), "l"(src), "r"((unsigned)len * 16u), "r"(bar_a) : "memory");
+        }
+    }
+    unsigned done = 0;
+    while (!done) {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(done) : "r"(bar_a) : "memory");
     }
 }
 

@@ -14,6 +14,10 @@
 #include "cv_switch.cuh"
 #include "tile.cuh"
 
+#ifndef TB_TMA
+#define TB_TMA 1               // interior tiles are staged by TMA bulk copies (tile_stage_pos_tma); 0: plain loads everywhere
+#endif
+
 typedef unsigned short nl16_t;   // local halo index (shared-memory candidate list only)
 #define LIST_CAP 40            // per-thread candidate slots in shared memory (maxn <= 32 on this path + band + self)
 
@@ -186,6 +190,11 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
     float4 *pos_s = dyn_smem;
     nl16_t *list_s = reinterpret_cast<nl16_t *>(dyn_smem + g.cap);
     tile_setup(g, cell_start, t, *reinterpret_cast<TileScratch *>(dyn_smem));   // scratch = the (still unused) staging area
+#if TB_TMA
+    __shared__ unsigned long long stage_bar;
+    if (t.staged && !t.any_wrapped && t.total > 0) tile_stage_pos_tma(t, spos, pos_s, &stage_bar);   // block-uniform choice
+    else
+#endif
     tile_stage_pos(g, t, spos, pos_s);
     __syncthreads();
     double v[2] = { 0.0, 0.0 };
