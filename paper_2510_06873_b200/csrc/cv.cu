@@ -106,20 +106,21 @@ k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int 
 
 // Warp-per-atom variants for small systems (N <= METAD_WARP_PER_ATOM_MAX): the lanes share an atom's neighbours, a fixed
 // shuffle tree sums the lane partials (deterministic).  Same arithmetic per pair as the thread-per-atom kernels.
-template <typename T>
+template <typename T, int G>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
                 const int *__restrict__ nl, PBox<T> pb, T inv_r0, int n, int m, double scale,
                 double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
                 unsigned int *__restrict__ sticky) {
     __shared__ double red[32];
-    const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = gt / G, lane = gt % G;
     T acc = T(0);
     if (s < N) {
         typename Vec4<T>::type pi = spos[s];
         if (((int)pi.w) & 1) {
             const int cnt = nl_count[s];
-            for (int k = lane; k < cnt; k += 32) {
+            for (int k = lane; k < cnt; k += G) {
                 const int j = nl[(size_t)k * N + s];
                 typename Vec4<T>::type pj = spos[j];
                 if (!(((int)pj.w) & 2)) continue;
@@ -145,18 +146,20 @@ k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const in
     }
 }
 
-template <typename T>
+template <typename T, int G>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_force_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
                    const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, T inv_r0, int n, int m,
                    double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F) {
-    const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = gt / G, lane = gt % G;
     if (s >= N) return;
+    const unsigned gmask = G == 32 ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
     typename Vec4<T>::type pi = spos[s];
     const int fi = (int)pi.w;
     T ax = T(0), ay = T(0), az = T(0);
-    const int cnt = nl_count[s];
-    for (int k = lane; k < cnt; k += 32) {
+    const int cnt = (fi & 3) ? nl_count[s] : 0;             // an atom in neither group takes no force
+    for (int k = lane; k < cnt; k += G) {
         const int j = nl[(size_t)k * N + s];
         typename Vec4<T>::type pj = spos[j];
         const int fj = (int)pj.w;
@@ -170,12 +173,12 @@ k_coord_force_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const
         ax += g * dx; ay += g * dy; az += g * dz;
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        ax += __shfl_down_sync(0xffffffffu, ax, o);
-        ay += __shfl_down_sync(0xffffffffu, ay, o);
-        az += __shfl_down_sync(0xffffffffu, az, o);
+    for (int o = G / 2; o > 0; o >>= 1) {
+        ax += __shfl_down_sync(gmask, ax, o, G);
+        ay += __shfl_down_sync(gmask, ay, o, G);
+        az += __shfl_down_sync(gmask, az, o, G);
     }
-    if (lane == 0) {
+    if (lane == 0 && (fi & 3)) {
         const double a = coef * dVds[0];
         const int i = perm[s];
         F[3 * i] += (T)(a * (double)ax);
@@ -752,7 +755,7 @@ static int cv_eval_t(metad_ctx *c, double *d_cv) {
     } else if (c->has_coord) {
         const CvDev &d = c->cv[c->coord_dim];
         if (N <= METAD_WARP_PER_ATOM_MAX)
-            k_coord_cv_warp<T><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+            k_coord_cv_warp<T, 32><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
                 N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials_warp,
                 c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky);
         else
@@ -812,7 +815,11 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
                                                                     pb, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
                                                                     d_dVds + c->coord_dim, (T *)d_F, va);
         else if (N <= METAD_WARP_PER_ATOM_MAX)
-            k_coord_force_warp<T><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+            k_coord_force_warp<T, 32><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
+                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, (T)(1.0 / d.r0), d.n, d.m,
+                c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F);
+        else if (d.use_groups && N <= 8 * METAD_WARP_PER_ATOM_MAX)
+            k_coord_force_warp<T, 8><<<div_up((long long)N * 8, CV_THREADS), CV_THREADS, 0, c->stream>>>(
                 N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, (T)(1.0 / d.r0), d.n, d.m,
                 c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F);
         else
