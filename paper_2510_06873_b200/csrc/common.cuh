@@ -68,6 +68,20 @@ __device__ __forceinline__ double r2_canonical(const BoxD &b, double dx, double 
     return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
 }
 
+// The same arithmetic with the branch decisions taken once per run of cells instead of once per pair: inside a cell list
+// with >= 3 cells per direction the neighbouring cell (jc, jb, ja) of (ic, ib, ia) names ONE image of its atoms, the wrap
+// flags (wz, wy, wx) in {-1, 0, +1} of that cell are the branch outcomes of r2_canonical for every pair within rc (the
+// margins hz - rc, hy - rc, hx - rc are positive by the box check), and adding +-c, +-b, +-a or 0.0 in the same order
+// rounds identically.  Pairs farther than rc may land on another image than the canonical one; both are >= rc.
+// sz = wz (cx, cy, cz), sy = wy (bx, by), sx = wx ax.
+struct RunShift { double zx, zy, zz, yx, yy, xx; };
+__device__ __forceinline__ double r2_shifted(const RunShift &w, double dx, double dy, double dz) {
+    dx = __dadd_rn(dx, w.zx); dy = __dadd_rn(dy, w.zy); dz = __dadd_rn(dz, w.zz);
+    dx = __dadd_rn(dx, w.yx); dy = __dadd_rn(dy, w.yy);
+    dx = __dadd_rn(dx, w.xx);
+    return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+}
+
 // fp64 minimum image in the order of reading O (chain / torsion CVs, fused small-molecule step)
 __device__ __forceinline__ void min_image_d(const BoxD &b, double &dx, double &dy, double &dz) {
     if (dz > b.hz) { dx -= b.cx; dy -= b.cy; dz -= b.cz; }

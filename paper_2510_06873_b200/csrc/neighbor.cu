@@ -173,6 +173,15 @@ __device__ __forceinline__ bool pair_in_range<float>(const PBox<float> &pb, cons
     return in;
 }
 
+// fp64 contexts on a grid with >= 3 cells per direction take the per-run form of the predicate (common.cuh: r2_shifted)
+template <typename T>
+__device__ __forceinline__ bool pair_in_run(bool shifted, const RunShift &w, const PBox<T> &pb, const BoxD &bd, T rc2T, double rc2,
+                                            const typename Vec4<T>::type &pi, const typename Vec4<T>::type &pj) {
+    if (sizeof(T) == 8 && shifted)
+        return r2_shifted(w, (double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y, (double)pj.z - (double)pi.z) < rc2;
+    return pair_in_range<T>(pb, bd, rc2T, rc2, pi, pj);
+}
+
 template <typename T>
 __global__ void __launch_bounds__(128)
 k_build_list(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ scell,
@@ -189,17 +198,27 @@ k_build_list(int N, const typename Vec4<T>::type *__restrict__ spos, const int *
     int zb0 = g.nc[1] >= 3 ? -1 : 0, zb1 = g.nc[1] >= 2 ? 1 : 0;
     int zc0 = g.nc[2] >= 3 ? -1 : 0, zc1 = g.nc[2] >= 2 ? 1 : 0;
     int cnt = 0;
+    const bool shifted = sizeof(T) == 8 && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3;
+    RunShift w = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
     for (int oc = zc0; oc <= zc1; ++oc) {
-        int jc = ic + oc; jc += jc < 0 ? g.nc[2] : 0; jc -= jc >= g.nc[2] ? g.nc[2] : 0;
+        int jc = ic + oc;
+        const double wz = jc < 0 ? -1.0 : (jc >= g.nc[2] ? 1.0 : 0.0);
+        jc += jc < 0 ? g.nc[2] : 0; jc -= jc >= g.nc[2] ? g.nc[2] : 0;
+        w.zx = wz * bd.cx; w.zy = wz * bd.cy; w.zz = wz * bd.cz;
         for (int ob = zb0; ob <= zb1; ++ob) {
-            int jb = ib + ob; jb += jb < 0 ? g.nc[1] : 0; jb -= jb >= g.nc[1] ? g.nc[1] : 0;
+            int jb = ib + ob;
+            const double wy = jb < 0 ? -1.0 : (jb >= g.nc[1] ? 1.0 : 0.0);
+            jb += jb < 0 ? g.nc[1] : 0; jb -= jb >= g.nc[1] ? g.nc[1] : 0;
+            w.yx = wy * bd.bx; w.yy = wy * bd.by;
             int rowbase = (jc * g.nc[1] + jb) * g.nc[0];
             for (int oa = za0; oa <= za1; ++oa) {
-                int ja = ia + oa; ja += ja < 0 ? g.nc[0] : 0; ja -= ja >= g.nc[0] ? g.nc[0] : 0;
+                int ja = ia + oa;
+                w.xx = ja < 0 ? -bd.ax : (ja >= g.nc[0] ? bd.ax : 0.0);
+                ja += ja < 0 ? g.nc[0] : 0; ja -= ja >= g.nc[0] ? g.nc[0] : 0;
                 int cb = cell_start[rowbase + ja], ce = cell_start[rowbase + ja + 1];
                 for (int j = cb; j < ce; ++j) {
                     typename Vec4<T>::type pj = spos[j];
-                    if (j != s && pair_in_range<T>(pb, bd, rc2T, rc2, pi, pj)) {
+                    if (j != s && pair_in_run<T>(shifted, w, pb, bd, rc2T, rc2, pi, pj)) {
                         if (cnt < maxn) nl[(size_t)cnt * N + s] = j;
                         ++cnt;
                     }
@@ -233,24 +252,34 @@ k_build_list_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const 
     const int zc0 = g.nc[2] >= 3 ? -1 : 0, zc1 = g.nc[2] >= 2 ? 1 : 0;
     // runs along x: [first cell, last cell] pairs, in the visiting order of the thread-per-atom kernel (-1, 0, +1)
     int ra[3], rb[3], nr = 0;
+    double rsx[3] = { 0.0, 0.0, 0.0 };                     // lattice shift along a of each run (per-run predicate, fp64)
     if (g.nc[0] >= 3) {
-        if (ia == 0) { ra[nr] = g.nc[0] - 1; rb[nr++] = g.nc[0] - 1; ra[nr] = 0; rb[nr++] = 1; }
-        else if (ia == g.nc[0] - 1) { ra[nr] = ia - 1; rb[nr++] = ia; ra[nr] = 0; rb[nr++] = 0; }
+        if (ia == 0) { rsx[nr] = -bd.ax; ra[nr] = g.nc[0] - 1; rb[nr++] = g.nc[0] - 1; ra[nr] = 0; rb[nr++] = 1; }
+        else if (ia == g.nc[0] - 1) { ra[nr] = ia - 1; rb[nr++] = ia; rsx[nr] = bd.ax; ra[nr] = 0; rb[nr++] = 0; }
         else { ra[nr] = ia - 1; rb[nr++] = ia + 1; }
     } else if (g.nc[0] == 2) { ra[nr] = ia; rb[nr++] = ia; ra[nr] = 1 - ia; rb[nr++] = 1 - ia; }
     else { ra[nr] = 0; rb[nr++] = 0; }
     int cnt = 0;
+    const bool shifted = sizeof(T) == 8 && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3;
+    RunShift w = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
     for (int oc = zc0; oc <= zc1; ++oc) {
-        int jc = ic + oc; jc += jc < 0 ? g.nc[2] : 0; jc -= jc >= g.nc[2] ? g.nc[2] : 0;
+        int jc = ic + oc;
+        const double wz = jc < 0 ? -1.0 : (jc >= g.nc[2] ? 1.0 : 0.0);
+        jc += jc < 0 ? g.nc[2] : 0; jc -= jc >= g.nc[2] ? g.nc[2] : 0;
+        w.zx = wz * bd.cx; w.zy = wz * bd.cy; w.zz = wz * bd.cz;
         for (int ob = zb0; ob <= zb1; ++ob) {
-            int jb = ib + ob; jb += jb < 0 ? g.nc[1] : 0; jb -= jb >= g.nc[1] ? g.nc[1] : 0;
+            int jb = ib + ob;
+            const double wy = jb < 0 ? -1.0 : (jb >= g.nc[1] ? 1.0 : 0.0);
+            jb += jb < 0 ? g.nc[1] : 0; jb -= jb >= g.nc[1] ? g.nc[1] : 0;
+            w.yx = wy * bd.bx; w.yy = wy * bd.by;
             const int rowbase = (jc * g.nc[1] + jb) * g.nc[0];
             for (int r = 0; r < nr; ++r) {
                 const int cb = cell_start[rowbase + ra[r]], ce = cell_start[rowbase + rb[r] + 1];
+                w.xx = rsx[r];
                 for (int j0 = cb; j0 < ce; j0 += G) {
                     const int j = j0 + lane;
                     bool hit = false;
-                    if (j < ce && j != s) hit = pair_in_range<T>(pb, bd, rc2T, rc2, pi, spos[j]);
+                    if (j < ce && j != s) hit = pair_in_run<T>(shifted, w, pb, bd, rc2T, rc2, pi, spos[j]);
                     const unsigned m = (__ballot_sync(gmask, hit) & gmask) >> gshift;
                     if (hit) {
                         const int k = cnt + __popc(m & ((1u << lane) - 1u));
