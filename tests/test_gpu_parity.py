@@ -38,22 +38,26 @@ def test_c3_fp32_pair_math_meets_the_same_tolerances():
 
 
 @pytest.mark.parametrize("prec,kind", [(64, 0), (32, 0), (32, 1)])      # (32, Q6) takes the shared-memory tiled path
-@pytest.mark.parametrize("boxname", ["cubic3cells", "two_cells", "hex120", "hex60", "triclinic"])
+@pytest.mark.parametrize("boxname", ["cubic3cells", "cubic3dense", "two_cells", "hex120", "hex60", "triclinic"])
 def test_neighbor_sets_bit_exact_on_awkward_boxes(boxname, prec, kind):
     import oracle
     import torch
     from paper_2510_06873_b200.metad import MetaD
     boxes = {
         "cubic3cells": (np.array([10.0, 0, 0, 0, 10.0, 0, 0, 0, 10.0]), 3.2),
+        # exactly 3 x 3 x 3 cells with more than 1,024 atoms: the cell-list kernels (not the brute-force one-launch build),
+        # every neighbouring cell reached through a wrap in some direction (per-run lattice shifts of the fp64 build)
+        "cubic3dense": (np.array([12.6, 0, 0, 0, 12.6, 0, 0, 0, 12.6]), 3.9, 0.55),
         "two_cells": (np.array([9.0, 0, 0, 0, 11.0, 0, 0, 0, 30.0]), 4.4),      # 2 x 2 x 6 cells
         "hex120": (np.array([24.0, 0, 0, -12.0, 12.0 * np.sqrt(3.0), 0, 0, 0, 19.0]), 4.0),
         "hex60": (np.array([24.0, 0, 0, 12.0, 12.0 * np.sqrt(3.0), 0, 0, 0, 19.0]), 4.0),
         "triclinic": (np.array([21.0, 0, 0, 5.0, 20.0, 0, -4.5, 7.0, 23.0]), 3.5),
     }
-    box, rc = boxes[boxname]
+    box, rc = boxes[boxname][:2]
+    density = boxes[boxname][2] if len(boxes[boxname]) > 2 else 0.15
     rng = np.random.default_rng(17)
     vol = box[0] * box[4] * box[8]
-    n = max(int(0.15 * vol), 64)
+    n = max(int(density * vol), 64)
     pos = wrap(rng.random((n, 3)) @ box.reshape(3, 3), box)
     # plant borderline pairs: partner at distance rc*(1 +- tiny) so that the fp32 guard band is exercised
     for k in range(0, 2 * (n // 8), 2):
