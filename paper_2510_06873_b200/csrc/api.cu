@@ -307,8 +307,17 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
         CellGrid gs = g;
         gs.nc[0] *= xsub; gs.ncell *= xsub;
         const double rho = (double)c->N / gs.ncell, margin = 1.3;
-        const int cap = 1216;
+        int cap = 1216;
         double best = 1e30; int bt[3] = { 0, 0, 0 };
+        int ov[4] = { 0, 0, 0, 0 };
+        const char *te = getenv("METAD_TILE");               // experiment switch: "tx,ty,tz,cap" (tx in sub-cells)
+        if (te && sscanf(te, "%d,%d,%d,%d", &ov[0], &ov[1], &ov[2], &ov[3]) == 4 && ov[0] >= 1 && ov[0] <= TILE_TXMAX &&
+            ov[1] >= 1 && ov[1] <= 4 && ov[2] >= 1 && ov[2] <= 4 && ov[3] >= 64 && ov[3] <= 4096) {
+            bt[0] = ov[0]; bt[1] = ov[1]; bt[2] = ov[2]; cap = ov[3];
+        } else
+        // two passes: the smallest halo ratio, then among the shapes within 2 % of it the longest along x (rows are the
+        // contiguous runs of the staging copies and of the scan: 11 x 3 x 3 beats 8 x 4 x 3 by 1.8 % at c3)
+        for (int pass = 0; pass < 2; ++pass)
         for (int ty = 1; ty <= 4; ++ty) for (int tz = 1; tz <= 4; ++tz) for (int tx = 1; tx <= TILE_TXMAX; ++tx) {
             if (tx > gs.nc[0] - 2 * xsub || ty > gs.nc[1] - 2 || tz > gs.nc[2] - 2) continue;
             double own = rho * tx * ty * tz, halo = rho * (tx + 2 * xsub) * (ty + 2) * (tz + 2);
@@ -316,7 +325,8 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
             long long ntl = (long long)((gs.nc[0] + tx - 1) / tx) * ((gs.nc[1] + ty - 1) / ty) * ((gs.nc[2] + tz - 1) / tz);
             if (ntl > c->nblocks_atoms) continue;     // per-tile partials live in the per-block scratch
             double score = halo / own + (own < 128 ? 2.0 : 0.0);   // halo ratio; keep the block busy
-            if (score < best) { best = score; bt[0] = tx; bt[1] = ty; bt[2] = tz; }
+            if (pass == 0) { if (score < best) best = score; }
+            else if (score <= 1.02 * best && tx > bt[0]) { bt[0] = tx; bt[1] = ty; bt[2] = tz; }
         }
         if (bt[0] > 0) {
             c->tiled = 1; c->tile_T[0] = bt[0]; c->tile_T[1] = bt[1]; c->tile_T[2] = bt[2]; c->tile_cap = cap; c->tile_hx = xsub;
