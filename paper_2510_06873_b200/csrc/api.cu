@@ -341,7 +341,7 @@ TileGeom tile_geom(const metad_ctx *c) {
     t.Tx = c->tile_T[0]; t.Ty = c->tile_T[1]; t.Tz = c->tile_T[2];
     t.nc0 = c->grid.nc[0]; t.nc1 = c->grid.nc[1]; t.nc2 = c->grid.nc[2];
     t.ntx = (t.nc0 + t.Tx - 1) / t.Tx; t.nty = (t.nc1 + t.Ty - 1) / t.Ty; t.ntz = (t.nc2 + t.Tz - 1) / t.Tz;
-    t.cap = c->tile_cap; t.hx = c->tile_hx;
+    t.cap = c->tile_cap; t.hx = c->tile_hx; t.natoms = c->N;
     t.ax = c->boxd.ax; t.bx = c->boxd.bx; t.by = c->boxd.by; t.cx = c->boxd.cx; t.cy = c->boxd.cy; t.cz = c->boxd.cz;
     t.wa = t.wb = t.wc = 0.0;
     return t;

@@ -371,11 +371,12 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
     const float alpha = dim_mean >= 0 ? (float)(dVds[dim_mean] * scale_mean) : 0.f;
     const float beta = dim_solid >= 0 ? (float)(dVds[dim_solid] * scale_solid) : 0.f;
     const float4 pi = spos[s];
+    const float *__restrict__ recB = rec + (size_t)N * 8;
     float Bk[13];
     {
         float4 a4, b4, c4, d4;
-        ldg256(rec + (size_t)s * METAD_NREC, a4, b4);
-        ldg256(rec + (size_t)s * METAD_NREC + 8, c4, d4);
+        ldg256(rec + (size_t)s * 8, a4, b4);                 // split layout of the tiled path (tiled.cu: finish_atom)
+        ldg256(recB + (size_t)s * 8, c4, d4);
         const float gk = SOLID ? alpha + beta * d4.y : alpha;
         Bk[0] = gk * a4.x; Bk[1] = gk * a4.y; Bk[2] = gk * a4.z; Bk[3] = gk * a4.w;
         Bk[4] = gk * b4.x; Bk[5] = gk * b4.y; Bk[6] = gk * b4.z; Bk[7] = gk * b4.w;
@@ -389,8 +390,8 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         const int e = __ldcs(in + k * 32);            // streamed once: do not displace positions / records in L2
         const int j = e & NLG_IDX_MASK, code = (unsigned)e >> 27;
         float4 a4, b4, c4, d4, pj;
-        ldg256(rec + (size_t)j * METAD_NREC, a4, b4);
-        ldg256(rec + (size_t)j * METAD_NREC + 8, c4, d4);
+        ldg256(rec + (size_t)j * 8, a4, b4);
+        ldg256(recB + (size_t)j * 8, c4, d4);
         if (SOLID) pj = spos[j];
         else { pj.x = d4.y; pj.y = d4.z; pj.z = d4.w; }     // Q6-mean-only records carry the position
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;

@@ -27,6 +27,7 @@ struct TileGeom {
     int ntx, nty, ntz;           // tiles per direction
     int nc0, nc1, nc2;           // cells per direction
     int cap;                     // halo capacity (atoms) of the shared-memory staging area
+    int natoms;                  // N (the second halves of the q6 records start at rec + 8 N)
     double ax, bx, by, cx, cy, cz;   // lattice rows
     double wa, wb, wc;           // cell edge vectors are a/nc0, b/nc1, c/nc2 (used for the tile's coordinate range)
 };

@@ -175,16 +175,19 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
         for (int k = 0; k < 13; ++k) S += A[k] * A[k];
         float norm = 0.f;
         if (n > 0 && S > 0.f) { float rs = sqrtf(S); q6 = rs / (float)n; norm = 1.f / ((float)n * rs); }
-        float4 *r4 = reinterpret_cast<float4 *>(rec + (size_t)s * METAD_NREC);
+        // the two 32-byte halves of a record live in two arrays (a 128-byte line then holds four atoms per half: the
+        // lanes of the force pass, whose neighbours are near one another in the sorted order, touch fewer lines per load)
+        float4 *r4 = reinterpret_cast<float4 *>(rec + (size_t)s * 8);
+        float4 *r4b = reinterpret_cast<float4 *>(rec + (size_t)g.natoms * 8 + (size_t)s * 8) - 2;
         r4[0] = make_float4(A[0] * norm, A[1] * norm, -A[2] * norm, A[3] * norm);
         r4[1] = make_float4(-A[4] * norm, A[5] * norm, -A[6] * norm, A[7] * norm);
-        r4[2] = make_float4(-A[8] * norm, A[9] * norm, -A[10] * norm, A[11] * norm);
+        r4b[2] = make_float4(-A[8] * norm, A[9] * norm, -A[10] * norm, A[11] * norm);
         if (solid) {
             const float f = 1.f / (1.f + expf(-(q6 - q_thresh) * inv_width));
-            r4[3] = make_float4(-A[12] * norm, f * (1.f - f) * inv_width, q6, 0.f);
+            r4b[3] = make_float4(-A[12] * norm, f * (1.f - f) * inv_width, q6, 0.f);
         } else {                                          // Q6 mean only: the record carries the atom's own (global,
             const float4 gp = spos[s];                    // exact fp32) position, so the force pass needs no second gather
-            r4[3] = make_float4(-A[12] * norm, gp.x, gp.y, gp.z);
+            r4b[3] = make_float4(-A[12] * norm, gp.x, gp.y, gp.z);
         }
         q6_out[s] = q6;
     }
