@@ -193,7 +193,7 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     }
     if (c->has_q6) {
         CUDA_TRY(cudaMalloc(&c->d_rec, METAD_NREC * tsz * (size_t)N));
-        CUDA_TRY(dev_alloc(&c->d_q6, N));
+        CUDA_TRY(dev_alloc(&c->d_q6, 2 * (size_t)N));       // q6 per atom, then f'(q6) per atom (tiled path, solid-like count)
     }
     CUDA_TRY(dev_alloc(&c->d_partials, 3 * (size_t)c->nblocks_atoms + max_pair_blocks));
     if (c->has_coord && N <= METAD_WARP_PER_ATOM_MAX) CUDA_TRY(dev_alloc(&c->d_partials_warp, (size_t)N / 4 + 2));

@@ -232,7 +232,7 @@ struct metad_ctx {
     int tiled; int tile_T[3]; int tile_cap; int tile_hx;
     int timing; int capturing; int timing_recorded; cudaEvent_t ev[3];
     cudaStream_t copy_stream; cudaEvent_t ev_copy;   // metad_step_host: the force upload overlaps the first three stages
-    float *d_q6;                          // tiled path: per-atom q6 (sorted order)
+    float *d_q6;                          // tiled path: per-atom q6 (sorted order) [N], then f'(q6) [N]
     double *d_cvq6;                       // tiled path: [Q6 mean, solid count] finished by k_tile_build
 };
 

@@ -359,7 +359,7 @@ __global__ void __launch_bounds__(CV_THREADS, VIRIAL ? 8 : Q6F_MINB)
 k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
              const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, const float *__restrict__ rec,
              double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
-             const double *__restrict__ dVds, float *__restrict__ F, VirArgs va) {
+             const double *__restrict__ dVds, float *__restrict__ F, VirArgs va, const float *__restrict__ fprime) {
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (!VIRIAL && s >= N) return;
@@ -377,7 +377,7 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         float4 a4, b4, c4, d4;
         ldg256(rec + (size_t)s * 8, a4, b4);                 // split layout of the tiled path (tiled.cu: finish_atom)
         ldg256(recB + (size_t)s * 8, c4, d4);
-        const float gk = SOLID ? alpha + beta * d4.y : alpha;
+        const float gk = SOLID ? alpha + beta * fprime[s] : alpha;
         Bk[0] = gk * a4.x; Bk[1] = gk * a4.y; Bk[2] = gk * a4.z; Bk[3] = gk * a4.w;
         Bk[4] = gk * b4.x; Bk[5] = gk * b4.y; Bk[6] = gk * b4.z; Bk[7] = gk * b4.w;
         Bk[8] = gk * c4.x; Bk[9] = gk * c4.y; Bk[10] = gk * c4.z; Bk[11] = gk * c4.w;
@@ -392,8 +392,7 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         float4 a4, b4, c4, d4, pj;
         ldg256(rec + (size_t)j * 8, a4, b4);
         ldg256(recB + (size_t)j * 8, c4, d4);
-        if (SOLID) pj = spos[j];
-        else { pj.x = d4.y; pj.y = d4.z; pj.z = d4.w; }     // Q6-mean-only records carry the position
+        pj.x = d4.y; pj.y = d4.z; pj.z = d4.w;               // the record carries the position
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         if (code != 13) {
             const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
@@ -401,7 +400,7 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
             dy = (float)(((double)pj.y - (double)pi.y) + (wy * bd.by + wz * bd.cy));
             dz = (float)(((double)pj.z - (double)pi.z) + (wz * bd.cz));
         }
-        const float gw = SOLID ? alpha + beta * d4.y : alpha;
+        const float gw = SOLID ? alpha + beta * fprime[j] : alpha;   // 4-byte gather from a dense array: few lines per warp
         float bb[13];
         bb[0] = Bk[0] + gw * a4.x; bb[1] = Bk[1] + gw * a4.y; bb[2] = Bk[2] + gw * a4.z; bb[3] = Bk[3] + gw * a4.w;
         bb[4] = Bk[4] + gw * b4.x; bb[5] = Bk[5] + gw * b4.y; bb[6] = Bk[6] + gw * b4.z; bb[7] = Bk[7] + gw * b4.w;
@@ -516,7 +515,7 @@ int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
 #define Q6FG_LAUNCH(SOLID, VIR)                                                                                            \
     k_q6_force_g<SOLID, VIR><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(                                      \
         c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm, \
-        ss, c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va)
+        ss, c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va, c->d_q6 + c->N)
     if (c->q6_solid_dim >= 0) { if (c->p.want_virial) Q6FG_LAUNCH(true, true); else Q6FG_LAUNCH(true, false); }
     else { if (c->p.want_virial) Q6FG_LAUNCH(false, true); else Q6FG_LAUNCH(false, false); }
 #undef Q6FG_LAUNCH

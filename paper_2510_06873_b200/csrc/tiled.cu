@@ -182,12 +182,13 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
         r4[0] = make_float4(A[0] * norm, A[1] * norm, -A[2] * norm, A[3] * norm);
         r4[1] = make_float4(-A[4] * norm, A[5] * norm, -A[6] * norm, A[7] * norm);
         r4b[2] = make_float4(-A[8] * norm, A[9] * norm, -A[10] * norm, A[11] * norm);
-        if (solid) {
-            const float f = 1.f / (1.f + expf(-(q6 - q_thresh) * inv_width));
-            r4b[3] = make_float4(-A[12] * norm, f * (1.f - f) * inv_width, q6, 0.f);
-        } else {                                          // Q6 mean only: the record carries the atom's own (global,
-            const float4 gp = spos[s];                    // exact fp32) position, so the force pass needs no second gather
+        {                                                 // the record carries the atom's own (global, exact fp32)
+            const float4 gp = spos[s];                    // position, so the force pass needs no second 16-byte gather
             r4b[3] = make_float4(-A[12] * norm, gp.x, gp.y, gp.z);
+        }
+        if (solid) {                                      // f'(q6) of the solid-like count: a dense 4-byte array of its own
+            const float f = 1.f / (1.f + expf(-(q6 - q_thresh) * inv_width));
+            q6_out[(size_t)g.natoms + s] = f * (1.f - f) * inv_width;
         }
         q6_out[s] = q6;
     }
