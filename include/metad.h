@@ -29,6 +29,8 @@
 #ifndef METAD_B200_H
 #define METAD_B200_H
 
+#include <stddef.h>
+
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -150,6 +152,13 @@ int metad_run(metad_ctx *ctx, const void *d_pos, const double *h_box, double rc,
  * five stages, copies F, cv[ncv] and V back.  [sync] */
 int metad_step_host(metad_ctx *ctx, const void *h_pos, const double *h_box, double rc, void *h_F,
                     double *h_cv, double *h_V);
+
+/* Page-locked host memory for the buffers of metad_step_host (cudaHostAlloc, default flags; *ptr is owned by the caller
+ * until metad_host_free).  Any host pointer works with metad_step_host, but pageable memory is staged by the driver, and
+ * memory pinned after the fact has been measured at 12-19 GB/s host -> device on the test machine against 54 GB/s for
+ * these buffers.  bytes == 0 or ptr == NULL: METAD_ERR_ARG; allocation failure: METAD_ERR_CUDA. */
+int metad_host_alloc(void **ptr, size_t bytes);
+int metad_host_free(void *ptr);
 
 /* [sync] ORs the sticky device bits into *bits (and clears nothing). */
 int metad_status(metad_ctx *ctx, unsigned *bits);

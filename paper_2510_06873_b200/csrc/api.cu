@@ -381,6 +381,19 @@ extern "C" int metad_apply_forces(metad_ctx *c, const double *d_dVds, void *d_F)
     return cv_forces_all(c, d_dVds, d_F);
 }
 
+extern "C" int metad_host_alloc(void **ptr, size_t bytes) {
+    if (!ptr || bytes == 0) FAIL(METAD_ERR_ARG, "null pointer or zero size");
+    *ptr = nullptr;
+    CUDA_TRY(cudaHostAlloc(ptr, bytes, cudaHostAllocDefault));
+    return METAD_OK;
+}
+
+extern "C" int metad_host_free(void *ptr) {
+    if (!ptr) return METAD_OK;
+    CUDA_TRY(cudaFreeHost(ptr));
+    return METAD_OK;
+}
+
 extern "C" int metad_deposit(metad_ctx *c, const double *d_cv, const double *d_V) {
     if (!c || !d_cv || !d_V) FAIL(METAD_ERR_ARG, "null argument");
     return bias_deposit(c, d_cv, d_V);

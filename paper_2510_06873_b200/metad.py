@@ -40,7 +40,7 @@ class Params(ctypes.Structure):
 
 
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
-           "metad_apply_forces", "metad_deposit", "metad_run", "metad_step_host", "metad_status",
+           "metad_apply_forces", "metad_deposit", "metad_run", "metad_step_host", "metad_host_alloc", "metad_host_free", "metad_status",
            "metad_get_state", "metad_get_neighbors", "metad_get_q6", "metad_set_hills", "metad_get_hills",
            "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reweight_recorded", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
 
@@ -65,6 +65,8 @@ def load():
     L.metad_deposit.argtypes = [_P, _P, _P]
     L.metad_run.argtypes = [_P, _P, _P, _D, _P, _I]
     L.metad_step_host.argtypes = [_P, _P, _P, _D, _P, _P, _P]
+    L.metad_host_alloc.argtypes = [ctypes.POINTER(_P), ctypes.c_size_t]
+    L.metad_host_free.argtypes = [_P]
     L.metad_status.argtypes = [_P, _P]
     L.metad_get_state.argtypes = [_P, _P, _P, _P, _P, _P]
     L.metad_get_neighbors.argtypes = [_P, _P, _P]
@@ -101,6 +103,30 @@ def _check(code):
 
 def _ptr(t):
     return ctypes.c_void_p(t.data_ptr())
+
+
+class _PinnedBlock:
+    """Owner of one metad_host_alloc allocation (freed when the last array viewing it goes away)."""
+
+    def __init__(self, nbytes):
+        self.ptr = ctypes.c_void_p()
+        _check(load().metad_host_alloc(ctypes.byref(self.ptr), nbytes))
+        self.nbytes = nbytes
+
+    def __del__(self):
+        if getattr(self, "ptr", None) and self.ptr.value and _lib is not None:
+            _lib.metad_host_free(self.ptr)
+            self.ptr = ctypes.c_void_p()
+
+
+def pinned_array(shape, dtype):
+    """numpy array in page-locked host memory from metad_host_alloc: the buffers metad_step_host copies at full PCIe rate."""
+    dtype = np.dtype(dtype)
+    n = int(np.prod(shape))
+    blk = _PinnedBlock(max(n * dtype.itemsize, 1))
+    buf = (ctypes.c_char * blk.nbytes).from_address(blk.ptr.value)
+    buf._owner = blk                                   # keeps the allocation alive as long as the buffer is referenced
+    return np.frombuffer(buf, dtype=dtype, count=n).reshape(shape)
 
 
 class MetaD:

@@ -242,6 +242,31 @@ def test_step_host_round_trip():
     assert np.abs(F_h.numpy() - Fref).max() <= 10 * TOL_F * np.abs(Fref - 1.0).max() + 1e-12
 
 
+def test_step_host_with_the_library_page_locked_buffers():
+    """metad_host_alloc / metad_host_free through the binding: same numbers as with any other host pointer."""
+    import gc
+    from paper_2510_06873_b200.metad import MetaD, MetadError, load, pinned_array
+    import ctypes
+    w = _small("c2")
+    r = stagewise(w)
+    md = MetaD(w, max_hills=len(r["heights"]) + 8)
+    md.set_hills(r["centers"], r["heights"])
+    pos_h = pinned_array(w.pos.shape, np.float64)
+    pos_h[...] = w.pos
+    F_h = pinned_array((w.natoms, 3), np.float64)
+    F_h[...] = 1.0
+    cv, V = md.step_host(pos_h, F_h)
+    assert rel(cv, r["s_ref"]) <= TOL_CV
+    Fref = 1.0 + r["o"].forces(r["o"].bias(r["s_ref"], use_grid=False)[1])
+    assert np.abs(F_h - Fref).max() <= 10 * TOL_F * np.abs(Fref - 1.0).max() + 1e-12
+    del pos_h, F_h
+    gc.collect()
+    p = ctypes.c_void_p()
+    assert load().metad_host_alloc(ctypes.byref(p), 0) != 0          # zero size is an argument error
+    assert load().metad_host_alloc(None, 16) != 0
+    assert load().metad_host_free(None) == 0
+
+
 def test_errors_and_sticky_bits():
     import torch
     from paper_2510_06873_b200 import metad
