@@ -61,3 +61,34 @@ def test_nearest_hydrogen_workload_full_size():
     r = stagewise(configs.config_r0())
     assert_stagewise(r)
     assert 0.5 < r["s_ref"][0] < 5.0
+
+
+def test_config3_full_size_is_bit_identical_from_run_to_run():
+    """Reading P at the size and in the launch configuration bench.py times (fp32 pair math, tiled build with TMA-staged
+    interior tiles, CUDA-graph replay with deposition): two fresh contexts give the same bits in every force component,
+    every per-atom q6, the CV, V and the deposited hills."""
+    import torch
+    from paper_2510_06873_b200.inputs import seeded_heights
+    from paper_2510_06873_b200.metad import MetaD
+    w = configs.config3()
+    w.stride = 2
+    pos = w.pos.astype(np.float32)
+    centers = (0.23 + 0.002 * np.arange(50))[:, None]
+    heights = seeded_heights(11, 50, w.w0)
+    out = []
+    for rep in range(2):
+        md = MetaD(w, precision=32, max_hills=128)
+        md.set_hills(centers, heights)
+        with torch.cuda.stream(md.stream):
+            dpos = torch.tensor(pos, device="cuda")
+            F = torch.zeros((w.natoms, 3), device="cuda", dtype=torch.float32)
+        md.synchronize()
+        md.run(dpos, F, 5)
+        st = md.state()
+        c, h = md.get_hills()
+        assert md.status() == 0
+        out.append((F.cpu().numpy(), md.q6(), st["cv"].copy(), st["V"], c, h))
+        del md
+    assert np.abs(out[0][0]).max() > 0
+    for a, b in zip(out[0], out[1]):
+        assert np.array_equal(np.asarray(a), np.asarray(b))
