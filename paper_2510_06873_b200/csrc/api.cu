@@ -191,6 +191,8 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
         CUDA_TRY(dev_alloc(&c->d_flags, N));
         CUDA_TRY(cudaMemcpy(c->d_flags, flags.data(), N, cudaMemcpyHostToDevice));
     }
+    if (c->has_coord && !c->has_q6 && c->prec == 32 && !c->cv[c->coord_dim].use_groups)   // candidates for the tiled path
+        CUDA_TRY(dev_alloc(&c->d_cgrad, 4 * (size_t)N));
     if (c->has_q6) {
         CUDA_TRY(cudaMalloc(&c->d_rec, METAD_NREC * tsz * (size_t)N));
         CUDA_TRY(dev_alloc(&c->d_q6, 2 * (size_t)N));       // q6 per atom, then f'(q6) per atom (tiled path, solid-like count)
@@ -243,7 +245,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];

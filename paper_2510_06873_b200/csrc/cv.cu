@@ -492,10 +492,28 @@ k_coord_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__r
     }
 }
 
+// Coordination forces from the per-atom gradient that k_tile_build<2> accumulated on its exact pass (tiled.cu): the sum
+// over the neighbours does not depend on dV/ds, so the force stage is one scaled add per atom — no list walk, no gathers.
+__global__ void __launch_bounds__(256)
+k_coord_force_pre(int N, const float4 *__restrict__ cgrad, const int *__restrict__ perm, double coef /* force_scale * scale */,
+                  const double *__restrict__ dVds, float *__restrict__ F) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    const float4 gsum = cgrad[s];
+    const double a = coef * dVds[0];
+    const int i = perm[s];
+    F[3 * i] += (float)(a * (double)gsum.x);
+    F[3 * i + 1] += (float)(a * (double)gsum.y);
+    F[3 * i + 2] += (float)(a * (double)gsum.z);
+}
+
 int tiled_coord_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     const CvDev &d = c->cv[c->coord_dim];
     const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
-    if (c->p.want_virial)
+    if (!c->p.want_virial && c->d_cgrad)
+        k_coord_force_pre<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, (const float4 *)c->d_cgrad, c->d_perm,
+                                                                    c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F);
+    else if (c->p.want_virial)
         k_coord_force_g<true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
             c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (float)(1.0 / d.r0), d.n, d.m,
             c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F, va);

@@ -114,6 +114,7 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
                                              float *__restrict__ q6_out, bool solid, int sw_n, int sw_m) {
     const bool WITH_Q6 = MODE == 1;
     float csum = 0.f;                                      // MODE 2: sum of sw(r / r0) over the neighbours (q_thresh = 1 / r0)
+    float cgx = 0.f, cgy = 0.f, cgz = 0.f;                 // MODE 2: sum of 2 sw' d / (r0 r)
     const int q = tile_own_row(t, a);
     const int o = a - t.own_off[q];
     const int li = t.own_l[q] + o, s = t.own_g[q] + o;
@@ -145,7 +146,14 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
         if (!in) continue;
         if (n < maxn) {
             __stcs(out + n * 32, __float_as_int(pj.w));     // streaming store: the list is read once, by the force pass
-            if (MODE == 2) { float dsw; csum += switch_fn<float>(sqrtf(r2) * q_thresh, sw_n, sw_m, dsw); }
+            if (MODE == 2) {
+                // the per-atom gradient sum_j 2 sw'(r_ij) d_ij / (r0 r_ij) does not depend on dV/ds: accumulated here, the
+                // force stage only scales it (k_coord_force_pre) instead of walking the list again
+                float dsw;
+                csum += switch_fn<float>(sqrtf(r2) * q_thresh, sw_n, sw_m, dsw);
+                const float gpair = 2.f * dsw * q_thresh * rsqrtf(r2);
+                cgx += gpair * dx; cgy += gpair * dy; cgz += gpair * dz;
+            }
             if (WITH_Q6) {
                 const float rinv = rsqrtf(r2);
                 Y6<float> y;
@@ -192,6 +200,7 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
         }
         q6_out[s] = q6;
     }
+    if (MODE == 2 && rec) reinterpret_cast<float4 *>(rec)[s] = make_float4(cgx, cgy, cgz, 0.f);
     return MODE == 2 ? csum : q6;
 }
 
@@ -318,7 +327,7 @@ int tiled_build(metad_ctx *c) {
         const CvDev &d = c->cv[c->coord_dim];
         k_tile_build<2><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
-            c->d_nl_count, c->d_nl, c->d_sticky, (float)(1.0 / d.r0), 1.f, nullptr, nullptr, 0, d.n, d.m,
+            c->d_nl_count, c->d_nl, c->d_sticky, (float)(1.0 / d.r0), 1.f, c->d_cgrad, nullptr, 0, d.n, d.m,
             c->d_partials + c->nblocks_atoms, c->d_tickets + 1, d.scale, 0.0, c->d_cvq6);
     } else
         k_tile_build<0><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
