@@ -233,7 +233,8 @@ struct metad_ctx {
     int timing; int capturing; int timing_recorded; cudaEvent_t ev[3];
     cudaStream_t copy_stream; cudaEvent_t ev_copy;   // metad_step_host: the force upload overlaps the first three stages
     float *d_q6;                          // tiled path: per-atom q6 (sorted order) [N], then f'(q6) [N]
-    float *d_cgrad;                       // tiled coordination path: per-atom sum_j 2 sw' d / (r0 r) as float4 (sorted order)
+    float *d_cgrad;                       // tiled coordination path: per-atom sum_j 2 sw' d / (r0 r) as float4, ORIGINAL atom
+                                          // order (k_tile_build<2>), scaled and added to F by k_force_add
     double *d_cvq6;                       // tiled path: [Q6 mean, solid count] finished by k_tile_build
 };
 

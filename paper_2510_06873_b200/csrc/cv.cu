@@ -492,27 +492,27 @@ k_coord_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__r
     }
 }
 
-// Coordination forces from the per-atom gradient that k_tile_build<2> accumulated on its exact pass (tiled.cu): the sum
-// over the neighbours does not depend on dV/ds, so the force stage is one scaled add per atom — no list walk, no gathers.
+// Coalesced force update of the tiled coordination path: F[i] += a * v[i] for a float4 array v in ORIGINAL atom order, one
+// thread per force component (F is [N][3], 12-byte rows: consecutive threads touch consecutive floats of F).
+// v = the per-atom gradient sum_j 2 sw'(r_ij) d_ij / (r0 r_ij) that k_tile_build<2> accumulated on its exact pass (tiled.cu):
+// it does not depend on dV/ds, so the coordination force stage is this one scaled add per atom, no list walk, no gathers;
+// a = force_scale * scale * dV/ds.  (The same split for the Q6 forces — k_q6_force_g storing into a scratch array in original
+// order, this pass adding it — was measured and dropped: profiles/r1h_rejected.md.)
 __global__ void __launch_bounds__(256)
-k_coord_force_pre(int N, const float4 *__restrict__ cgrad, const int *__restrict__ perm, double coef /* force_scale * scale */,
-                  const double *__restrict__ dVds, float *__restrict__ F) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
-    const float4 gsum = cgrad[s];
+k_force_add(int N, const float *__restrict__ v4, double coef, const double *__restrict__ dVds, float *__restrict__ F) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= 3 * N) return;
+    const int i = t / 3, k = t - 3 * i;
     const double a = coef * dVds[0];
-    const int i = perm[s];
-    F[3 * i] += (float)(a * (double)gsum.x);
-    F[3 * i + 1] += (float)(a * (double)gsum.y);
-    F[3 * i + 2] += (float)(a * (double)gsum.z);
+    F[t] += (float)(a * (double)v4[4 * i + k]);
 }
 
 int tiled_coord_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     const CvDev &d = c->cv[c->coord_dim];
     const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
     if (!c->p.want_virial && c->d_cgrad)
-        k_coord_force_pre<<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, (const float4 *)c->d_cgrad, c->d_perm,
-                                                                    c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F);
+        k_force_add<<<div_up(3 * c->N, 256), 256, 0, c->stream>>>(c->N, c->d_cgrad, c->p.force_scale * d.scale,
+                                                                  d_dVds + c->coord_dim, (float *)d_F);
     else if (c->p.want_virial)
         k_coord_force_g<true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
             c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (float)(1.0 / d.r0), d.n, d.m,

@@ -111,7 +111,8 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
                                              const BoxD &bd, float rc2f, float rc2_lo, double rc2, int maxn,
                                              int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
                                              float q_thresh, float inv_width, float *__restrict__ rec,
-                                             float *__restrict__ q6_out, bool solid, int sw_n, int sw_m) {
+                                             float *__restrict__ q6_out, bool solid, int sw_n, int sw_m,
+                                             const int *__restrict__ perm) {
     const bool WITH_Q6 = MODE == 1;
     float csum = 0.f;                                      // MODE 2: sum of sw(r / r0) over the neighbours (q_thresh = 1 / r0)
     float cgx = 0.f, cgy = 0.f, cgz = 0.f;                 // MODE 2: sum of 2 sw' d / (r0 r)
@@ -149,9 +150,20 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
             if (MODE == 2) {
                 // the per-atom gradient sum_j 2 sw'(r_ij) d_ij / (r0 r_ij) does not depend on dV/ds: accumulated here, the
                 // force stage only scales it (k_coord_force_pre) instead of walking the list again
-                float dsw;
-                csum += switch_fn<float>(sqrtf(r2) * q_thresh, sw_n, sw_m, dsw);
-                const float gpair = 2.f * dsw * q_thresh * rsqrtf(r2);
+                float gpair;
+                if (sw_m == 2 * sw_n && !(sw_n & 1)) {
+                    // sw = 1 / (1 + x^n) with n even needs only x^2 = r^2 / r0^2 (no square roots):
+                    // 2 sw' / (r0 r) = -2 n (x^2)^(n/2 - 1) sw^2 / r0^2        (block-uniform branch; all five configs)
+                    const float x2 = r2 * q_thresh * q_thresh;
+                    const float xh = sw_n == 6 ? x2 * x2 : ipow(x2, sw_n / 2 - 1);
+                    const float sw = __fdividef(1.f, 1.f + xh * x2);
+                    csum += sw;
+                    gpair = (float)(-2 * sw_n) * xh * sw * sw * (q_thresh * q_thresh);
+                } else {
+                    float dsw;
+                    csum += switch_fn<float>(sqrtf(r2) * q_thresh, sw_n, sw_m, dsw);
+                    gpair = 2.f * dsw * q_thresh * rsqrtf(r2);
+                }
                 cgx += gpair * dx; cgy += gpair * dy; cgz += gpair * dz;
             }
             if (WITH_Q6) {
@@ -200,7 +212,9 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
         }
         q6_out[s] = q6;
     }
-    if (MODE == 2 && rec) reinterpret_cast<float4 *>(rec)[s] = make_float4(cgx, cgy, cgz, 0.f);
+    // ORIGINAL atom order (one scattered 16-byte store here, where the memory pipes idle): the force stage is then a
+    // coalesced pass over F (k_force_add)
+    if (MODE == 2 && rec) reinterpret_cast<float4 *>(rec)[perm[s]] = make_float4(cgx, cgy, cgz, 0.f);
     return MODE == 2 ? csum : q6;
 }
 
@@ -212,14 +226,14 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
                                            const BoxD &bd, float rc2f, double rc2, int maxn, int *__restrict__ nl_count,
                                            int *__restrict__ nl, unsigned int *__restrict__ sticky, float q_thresh,
                                            float inv_width, float *__restrict__ rec, float *__restrict__ q6_out, bool solid,
-                                           int sw_n, int sw_m, double (&v)[2]) {
+                                           int sw_n, int sw_m, const int *__restrict__ perm, double (&v)[2]) {
     const float rc2_hi = rc2f * (1.f + 1e-5f), rc2_lo = rc2f * (1.f - 1e-5f);
     const int tid = threadIdx.x;
     for (int a = tid; a < t.nown; a += blockDim.x) {
         bool ovf = false;
         const int cnt = scan_atom<STAGED>(g, t, spos, pos_s, list_s, scell, a, tid, rc2_hi, ovf);
         const float q6 = finish_atom<STAGED, MODE>(g, t, spos, pos_s, list_s, a, tid, cnt, ovf, bd, rc2f, rc2_lo, rc2, maxn,
-                                                   nl_count, nl, sticky, q_thresh, inv_width, rec, q6_out, solid, sw_n, sw_m);
+                                                   nl_count, nl, sticky, q_thresh, inv_width, rec, q6_out, solid, sw_n, sw_m, perm);
         if (MODE != 0) v[0] += (double)q6;
         if (MODE == 1) v[1] += (double)(1.f / (1.f + expf(-(q6 - q_thresh) * inv_width)));
     }
@@ -234,7 +248,7 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
              const int *__restrict__ cell_start, BoxD bd, float rc2f, double rc2, int maxn,
              int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
              float q_thresh, float inv_width, float *__restrict__ rec, float *__restrict__ q6_out, int solid,
-             int sw_n, int sw_m, double *__restrict__ partials, unsigned int *__restrict__ ticket, double scale_mean, double scale_solid,
+             int sw_n, int sw_m, const int *__restrict__ perm, double *__restrict__ partials, unsigned int *__restrict__ ticket, double scale_mean, double scale_solid,
              double *__restrict__ cv_q6 /* [2]: Q6 mean, solid count */) {
     extern __shared__ float4 dyn_smem[];
     __shared__ TileTables t;
@@ -254,10 +268,10 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
         if (threadIdx.x == 0) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
     } else if (t.staged) {
         build_body<true, MODE>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
-                                  inv_width, rec, q6_out, solid != 0, sw_n, sw_m, v);
+                                  inv_width, rec, q6_out, solid != 0, sw_n, sw_m, perm, v);
     } else {
         build_body<false, MODE>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
-                                   inv_width, rec, q6_out, solid != 0, sw_n, sw_m, v);
+                                   inv_width, rec, q6_out, solid != 0, sw_n, sw_m, perm, v);
     }
     if (MODE != 0) {
         block_reduce<2>(v, red);
@@ -320,19 +334,19 @@ int tiled_build(metad_ctx *c) {
         k_tile_build<1><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
             c->d_nl_count, c->d_nl, c->d_sticky, (float)qt, (float)(1.0 / qw), (float *)c->d_rec, c->d_q6,
-            c->q6_solid_dim >= 0 ? 1 : 0, 0, 0, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
+            c->q6_solid_dim >= 0 ? 1 : 0, 0, 0, c->d_perm, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
             c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0, c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0,
             c->d_cvq6);
     else if (c->has_coord) {                                  // ungrouped coordination number: the sum of sw rides on the exact pass
         const CvDev &d = c->cv[c->coord_dim];
         k_tile_build<2><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
-            c->d_nl_count, c->d_nl, c->d_sticky, (float)(1.0 / d.r0), 1.f, c->d_cgrad, nullptr, 0, d.n, d.m,
+            c->d_nl_count, c->d_nl, c->d_sticky, (float)(1.0 / d.r0), 1.f, c->d_cgrad, nullptr, 0, d.n, d.m, c->d_perm,
             c->d_partials + c->nblocks_atoms, c->d_tickets + 1, d.scale, 0.0, c->d_cvq6);
     } else
         k_tile_build<0><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
-            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, 0, 0, nullptr, nullptr, 0.0, 0.0, nullptr);
+            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, 0, 0, c->d_perm, nullptr, nullptr, 0.0, 0.0, nullptr);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
