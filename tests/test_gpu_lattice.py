@@ -36,6 +36,20 @@ def test_coordination_plus_lattice_parameters(precision):
     assert np.abs(r["F_ref"] - F_cn).max() <= 1e-15 * np.abs(F_cn).max()
 
 
+@pytest.mark.parametrize("n,m", [(6, 12), (8, 16), (4, 8), (2, 4), (5, 10), (6, 10)])
+def test_tiled_coordination_switching_exponents(n, m):
+    """The tiled fp32 coordination path (k_tile_build<2> + k_force_add) evaluates sw = 1 / (1 + x^n) for even n with m = 2n
+    from r^2 alone (n = 6 special-cased, other even n by square-and-multiply, n = 2 with exponent 0), odd n and m != 2n through
+    the general form with a square root (reading A): every branch against the oracle, CV and per-atom forces."""
+    w = _workload()
+    w.cvs = [CVSpec(kind=CV_COORD, r0=2.4, n=n, m=m, scale=1.0 / w.natoms)]
+    w.sigma = [0.05]
+    r = stagewise(w, precision=32)
+    assert_stagewise(r)
+    assert np.abs(r["F_ref"]).max() > 0
+    assert np.abs(r["F"].sum(axis=0)).max() <= 1e-3 * np.abs(r["F_ref"]).max()      # translation invariance (reading N), fp32 sums
+
+
 def test_lattice_only_context_and_bad_axis():
     import torch
     from paper_2510_06873_b200.metad import MetaD, MetadError
