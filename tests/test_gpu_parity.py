@@ -30,6 +30,18 @@ def test_stagewise_parity_small(name):
         assert np.abs(r["q6"] - r["q6_ref"]).max() <= tol
 
 
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("n,m", [(6, 10), (5, 9)])
+def test_grouped_coordination_general_exponents(precision, n, m):
+    """m != 2n takes the general branch of the switching function (reading A) on the generic (grouped, warp-per-atom) kernels;
+    in fp32 pair math it has to stay accurate for pairs near r0, where (1 - x^n) / (1 - x^m) is 0 / 0."""
+    w = _small("c2")
+    w.cvs[0].n, w.cvs[0].m = n, m
+    r = stagewise(w, precision=precision)
+    assert_stagewise(r)
+    assert np.abs(r["F_ref"]).max() > 0
+
+
 def test_c3_fp32_pair_math_meets_the_same_tolerances():
     w = _small("c3")
     r = stagewise(w, precision=32)
