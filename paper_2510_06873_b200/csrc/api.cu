@@ -186,7 +186,8 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     CUDA_TRY(dev_alloc(&c->d_scell, N));
     CUDA_TRY(cudaMalloc(&c->d_spos, 4 * tsz * (size_t)N));
     CUDA_TRY(dev_alloc(&c->d_nl_count, N));
-    CUDA_TRY(dev_alloc(&c->d_nl, (size_t)c->maxn * N));
+    // the tiled path stores the list in slabs of 32 atoms x maxn entries (tile.cuh: nl_slot): the last slab is a whole one
+    CUDA_TRY(dev_alloc(&c->d_nl, (size_t)c->maxn * (((size_t)N + 31) / 32 * 32)));
     if (!flags.empty()) {
         CUDA_TRY(dev_alloc(&c->d_flags, N));
         CUDA_TRY(cudaMemcpy(c->d_flags, flags.data(), N, cudaMemcpyHostToDevice));
