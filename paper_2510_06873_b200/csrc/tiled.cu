@@ -149,7 +149,7 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
             __stcs(out + n * 32, __float_as_int(pj.w));     // streaming store: the list is read once, by the force pass
             if (MODE == 2) {
                 // the per-atom gradient sum_j 2 sw'(r_ij) d_ij / (r0 r_ij) does not depend on dV/ds: accumulated here, the
-                // force stage only scales it (k_coord_force_pre) instead of walking the list again
+                // force stage only scales it (k_force_add, cv.cu) instead of walking the list again
                 float gpair;
                 if (sw_m == 2 * sw_n && !(sw_n & 1)) {
                     // sw = 1 / (1 + x^n) with n even needs only x^2 = r^2 / r0^2 (no square roots):
