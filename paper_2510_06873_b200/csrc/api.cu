@@ -415,11 +415,17 @@ static int enqueue_step(metad_ctx *c, const void *d_pos, const double *box, doub
         c->d_pos_last = d_pos; c->have_neighbors = true; c->list_built = false;
         return bias_fused_torsion_step(c, d_pos, d_F);
     }
-    if ((r = metad_build_neighbors(c, d_pos, box, rc))) return r;
-    if ((r = metad_eval_cv(c, c->d_cv))) return r;
-    if ((r = metad_bias(c, c->d_cv, c->d_V, c->d_dVds))) return r;
+    // without a grid the deposition rides on the hill sum (one launch less; same V, same order of effects: the forces of
+    // this step use the dV/ds of the hills deposited before it, reading U)
+    const bool fuse = !c->grid_on;
+    c->cv_direct = c->d_cv;
+    r = metad_build_neighbors(c, d_pos, box, rc);
+    if (!r) r = metad_eval_cv(c, c->d_cv);
+    c->cv_direct = nullptr;
+    if (r) return r;
+    if ((r = bias_eval(c, c->d_cv, c->d_V, c->d_dVds, fuse))) return r;
     if ((r = metad_apply_forces(c, c->d_dVds, d_F))) return r;
-    return metad_deposit(c, c->d_cv, c->d_V);
+    return fuse ? METAD_OK : metad_deposit(c, c->d_cv, c->d_V);
 }
 
 extern "C" int metad_run(metad_ctx *c, const void *d_pos, const double *h_box, double rc, void *d_F, int nsteps) {
@@ -472,12 +478,16 @@ extern "C" int metad_step_host(metad_ctx *c, const void *h_pos, const double *h_
         CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_copy, 0));
         if ((r = enqueue_step(c, c->d_pos_stage, h_box, rc, c->d_F_stage))) return r;
     } else {
-        if ((r = metad_build_neighbors(c, c->d_pos_stage, h_box, rc))) return r;
-        if ((r = metad_eval_cv(c, c->d_cv))) return r;
-        if ((r = metad_bias(c, c->d_cv, c->d_V, c->d_dVds))) return r;
+        const bool fuse = !c->grid_on;            // as in enqueue_step
+        c->cv_direct = c->d_cv;
+        r = metad_build_neighbors(c, c->d_pos_stage, h_box, rc);
+        if (!r) r = metad_eval_cv(c, c->d_cv);
+        c->cv_direct = nullptr;
+        if (r) return r;
+        if ((r = bias_eval(c, c->d_cv, c->d_V, c->d_dVds, fuse))) return r;
         CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_copy, 0));
         if ((r = metad_apply_forces(c, c->d_dVds, c->d_F_stage))) return r;
-        if ((r = metad_deposit(c, c->d_cv, c->d_V))) return r;
+        if (!fuse && (r = metad_deposit(c, c->d_cv, c->d_V))) return r;
     }
     CUDA_TRY(cudaMemcpyAsync(h_F, c->d_F_stage, bytes, cudaMemcpyDeviceToHost, c->stream));
     if (h_cv) CUDA_TRY(cudaMemcpyAsync(h_cv, c->d_cv, sizeof(double) * c->D, cudaMemcpyDeviceToHost, c->stream));

@@ -34,12 +34,46 @@ __device__ __forceinline__ double pdiff(double s, double c, double P) {
 #define AUX_DEP_INDEX 1
 
 // ------------------------------------------------------------------------------------------------
+// a7: deposition (readings I, J, U).  One thread.  V = the bias at cv from the hills deposited before this step.
+__device__ __forceinline__ void deposit_one(const BiasParams &bp, int stride, double w0, double kT, double gamma,
+                                            const double *cv, double V, double *centers, double *heights, int *nhills,
+                                            int *step, int *aux, unsigned int *sticky, double *traj, int traj_cap) {
+    int st = *step + 1;
+    *step = st;
+    if (traj) {                                   // device-resident CV trajectory (reweighting input)
+        if (st <= traj_cap) { for (int d = 0; d < bp.D; ++d) traj[(size_t)(st - 1) * bp.D + d] = cv[d]; }
+        else atomicOr(sticky, (unsigned)METAD_DEV_TRAJ_FULL);
+    }
+    aux[AUX_DEP_INDEX] = -1;
+    if (stride <= 0 || st % stride != 0) return;
+    int H = *nhills;
+    if (H >= bp.max_hills) { atomicOr(sticky, (unsigned)METAD_DEV_HILL_OVERFLOW); return; }
+    double h = gamma > 1.0 ? w0 * exp(-V / ((gamma - 1.0) * kT)) : w0;
+    for (int d = 0; d < bp.D; ++d) centers[(size_t)d * bp.max_hills + H] = cv[d];
+    heights[H] = h;
+    *nhills = H + 1;
+    aux[AUX_DEP_INDEX] = H;
+}
+
+__global__ void k_deposit(BiasParams bp, int stride, double w0, double kT, double gamma, const double *__restrict__ cv,
+                          const double *__restrict__ V, double *__restrict__ centers, double *__restrict__ heights,
+                          int *__restrict__ nhills, int *__restrict__ step, int *__restrict__ aux,
+                          unsigned int *__restrict__ sticky, double *__restrict__ traj, int traj_cap) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    deposit_one(bp, stride, w0, kT, gamma, cv, *V, centers, heights, nhills, step, aux, sticky, traj, traj_cap);
+}
+
+// deposition riding on the hill sum (metad_run / metad_step_host without a grid): the last block of k_bias_sum, which holds
+// V, deposits in the same launch — every other block has finished reading the hill arrays by then (ticket), the new hill
+// goes to slot H, which this launch never read
+struct DepArgs { int on, stride, traj_cap; double w0, kT, gamma; int *step; unsigned int *sticky; double *traj; };
+
+// ------------------------------------------------------------------------------------------------
 // exact hill sum at one point: blocks stride over the hill array, fixed-order reduction.
 __global__ void __launch_bounds__(BIAS_THREADS)
-k_bias_sum(BiasParams bp, const double *__restrict__ centers, const double *__restrict__ heights,
-           const int *__restrict__ nhills, const double *__restrict__ cv, double *__restrict__ partials,
-           unsigned int *__restrict__ ticket, double *__restrict__ V, double *__restrict__ dVds,
-           const int *__restrict__ aux, int grid_on) {
+k_bias_sum(BiasParams bp, double *centers, double *heights, int *nhills, const double *__restrict__ cv,
+           double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ V,
+           double *__restrict__ dVds, int *aux, int grid_on, DepArgs dep) {
     __shared__ double red[(1 + METAD_MAX_CV) * 32];
     if (grid_on && aux[AUX_GRID_MISS] == 0) return;   // the grid lookup already produced V, dVds
     const int H = *nhills;
@@ -81,6 +115,9 @@ k_bias_sum(BiasParams bp, const double *__restrict__ centers, const double *__re
         if (threadIdx.x == 0) {
             *V = t[0];
             for (int d = 0; d < bp.D; ++d) dVds[d] = t[1 + d];
+            if (dep.on)
+                deposit_one(bp, dep.stride, dep.w0, dep.kT, dep.gamma, cv, t[0], centers, heights, nhills, dep.step, aux,
+                            dep.sticky, dep.traj, dep.traj_cap);
         }
     }
 }
@@ -213,30 +250,6 @@ __global__ void k_grid_add_last(GridParams gp, BiasParams bp, const double *__re
     double ga = -a * bp.inv_sigma[0], gb = -b * bp.inv_sigma[1];
     size_t plane = (size_t)gp.n0 * gp.n1;
     table[o] += g; table[plane + o] += g * ga; table[2 * plane + o] += g * gb; table[3 * plane + o] += g * ga * gb;
-}
-
-// ------------------------------------------------------------------------------------------------
-// a7: deposition (readings I, J, U).  One thread.
-__global__ void k_deposit(BiasParams bp, int stride, double w0, double kT, double gamma, const double *__restrict__ cv,
-                          const double *__restrict__ V, double *__restrict__ centers, double *__restrict__ heights,
-                          int *__restrict__ nhills, int *__restrict__ step, int *__restrict__ aux,
-                          unsigned int *__restrict__ sticky, double *__restrict__ traj, int traj_cap) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    int st = *step + 1;
-    *step = st;
-    if (traj) {                                   // device-resident CV trajectory (reweighting input)
-        if (st <= traj_cap) { for (int d = 0; d < bp.D; ++d) traj[(size_t)(st - 1) * bp.D + d] = cv[d]; }
-        else atomicOr(sticky, (unsigned)METAD_DEV_TRAJ_FULL);
-    }
-    aux[AUX_DEP_INDEX] = -1;
-    if (stride <= 0 || st % stride != 0) return;
-    int H = *nhills;
-    if (H >= bp.max_hills) { atomicOr(sticky, (unsigned)METAD_DEV_HILL_OVERFLOW); return; }
-    double h = gamma > 1.0 ? w0 * exp(-(*V) / ((gamma - 1.0) * kT)) : w0;
-    for (int d = 0; d < bp.D; ++d) centers[(size_t)d * bp.max_hills + H] = cv[d];
-    heights[H] = h;
-    *nhills = H + 1;
-    aux[AUX_DEP_INDEX] = H;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -384,8 +397,13 @@ static GridParams make_gp(const metad_ctx *c) {
 }
 
 
-int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds) {
+int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds, bool with_deposit) {
     BiasParams bp = make_bp(c);
+    DepArgs dep = { 0, c->p.stride, c->p.traj_capacity, c->p.w0, c->p.kT, c->p.bias_factor, c->d_step, c->d_sticky, c->d_traj };
+    if (with_deposit) {
+        if (c->grid_on) return METAD_ERR_STATE;            // the table update follows the deposit: separate launches
+        dep.on = 1;
+    }
     if (c->grid_on) {
         k_bias_grid<<<1, 32, 0, c->stream>>>(make_gp(c), c->d_table, d_cv, d_V, d_dVds, ctx_aux(c), c->d_sticky);
         c->launches++;
@@ -394,7 +412,7 @@ int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds) {
     if (nb > BIAS_MAX_BLOCKS) nb = BIAS_MAX_BLOCKS;
     if (nb < 1) nb = 1;
     k_bias_sum<<<nb, BIAS_THREADS, 0, c->stream>>>(bp, c->d_centers, c->d_heights, c->d_nhills, d_cv, c->d_bias_partials,
-                                                  c->d_tickets + 8, d_V, d_dVds, ctx_aux(c), c->grid_on);
+                                                  c->d_tickets + 8, d_V, d_dVds, ctx_aux(c), c->grid_on, dep);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

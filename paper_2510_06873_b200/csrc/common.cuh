@@ -236,6 +236,8 @@ struct metad_ctx {
     float *d_cgrad;                       // tiled coordination path: per-atom sum_j 2 sw' d / (r0 r) as float4, ORIGINAL atom
                                           // order (k_tile_build<2>), scaled and added to F by k_force_add
     double *d_cvq6;                       // tiled path: [Q6 mean, solid count] finished by k_tile_build
+    double *cv_direct;                    // run paths (metad_run, metad_step_host): the context's CV vector, which the last block
+                                          // of k_tile_build fills itself (no k_q6_publish launch); NULL on the stage calls
 };
 
 static inline const void *ctx_last_pos(const metad_ctx *c) { return c->d_pos_last; }
@@ -259,7 +261,7 @@ int mindist_eval(metad_ctx *c, double *d_cv);
 int mindist_forces(metad_ctx *c, const double *d_dVds, void *d_F);
 int torsion_eval_all(metad_ctx *c, double *d_cv);
 int torsion_forces(metad_ctx *c, const double *d_dVds, void *d_F);
-int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds);
+int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds, bool with_deposit = false);
 int bias_deposit(metad_ctx *c, const double *d_cv, const double *d_V);
 int bias_grid_rebuild(metad_ctx *c);
 int bias_fused_torsion_step(metad_ctx *c, const void *d_pos, void *d_F);

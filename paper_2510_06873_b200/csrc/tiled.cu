@@ -249,7 +249,9 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
              int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
              float q_thresh, float inv_width, float *__restrict__ rec, float *__restrict__ q6_out, int solid,
              int sw_n, int sw_m, const int *__restrict__ perm, double *__restrict__ partials, unsigned int *__restrict__ ticket, double scale_mean, double scale_solid,
-             double *__restrict__ cv_q6 /* [2]: Q6 mean, solid count */) {
+             double *__restrict__ cv_q6 /* [2]: Q6 mean, solid count */,
+             double *__restrict__ cv_out /* the context's CV vector on the run paths (NULL: k_q6_publish hands the sums over) */,
+             int dim0, int dim1) {
     extern __shared__ float4 dyn_smem[];
     __shared__ TileTables t;
     __shared__ double red[64];
@@ -282,6 +284,10 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
             block_reduce<2>(u, red);
             if (threadIdx.x == 0) {
                 cv_q6[0] = scale_mean * u[0]; cv_q6[1] = scale_solid * u[1];
+                if (cv_out) {
+                    if (dim0 >= 0) cv_out[dim0] = cv_q6[0];
+                    if (dim1 >= 0) cv_out[dim1] = cv_q6[1];
+                }
                 if (!isfinite(cv_q6[0]) || !isfinite(cv_q6[1])) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
             }
         }
@@ -336,17 +342,17 @@ int tiled_build(metad_ctx *c) {
             c->d_nl_count, c->d_nl, c->d_sticky, (float)qt, (float)(1.0 / qw), (float *)c->d_rec, c->d_q6,
             c->q6_solid_dim >= 0 ? 1 : 0, 0, 0, c->d_perm, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
             c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0, c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0,
-            c->d_cvq6);
+            c->d_cvq6, c->cv_direct, c->q6_mean_dim, c->q6_solid_dim);
     else if (c->has_coord) {                                  // ungrouped coordination number: the sum of sw rides on the exact pass
         const CvDev &d = c->cv[c->coord_dim];
         k_tile_build<2><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
             c->d_nl_count, c->d_nl, c->d_sticky, (float)(1.0 / d.r0), 1.f, c->d_cgrad, nullptr, 0, d.n, d.m, c->d_perm,
-            c->d_partials + c->nblocks_atoms, c->d_tickets + 1, d.scale, 0.0, c->d_cvq6);
+            c->d_partials + c->nblocks_atoms, c->d_tickets + 1, d.scale, 0.0, c->d_cvq6, c->cv_direct, c->coord_dim, -1);
     } else
         k_tile_build<0><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
-            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, 0, 0, c->d_perm, nullptr, nullptr, 0.0, 0.0, nullptr);
+            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, 0, 0, c->d_perm, nullptr, nullptr, 0.0, 0.0, nullptr, nullptr, -1, -1);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -354,6 +360,7 @@ int tiled_build(metad_ctx *c) {
 
 // the q6m accumulation and its reduction already ran inside k_tile_build
 int tiled_q6_pass1(metad_ctx *c, double *d_cv) {
+    if (c->cv_direct && c->cv_direct == d_cv) return METAD_OK;      // the build kernel wrote these dimensions itself
     if (c->has_q6) k_q6_publish<<<1, 32, 0, c->stream>>>(c->d_cvq6, c->q6_mean_dim, c->q6_solid_dim, d_cv);
     else k_q6_publish<<<1, 32, 0, c->stream>>>(c->d_cvq6, c->coord_dim, -1, d_cv);          // tiled coordination number
     c->launches++;
