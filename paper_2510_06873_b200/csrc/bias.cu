@@ -408,7 +408,7 @@ int bias_eval(metad_ctx *c, const double *d_cv, double *d_V, double *d_dVds, boo
         k_bias_grid<<<1, 32, 0, c->stream>>>(make_gp(c), c->d_table, d_cv, d_V, d_dVds, ctx_aux(c), c->d_sticky);
         c->launches++;
     }
-    int nb = div_up(c->p.max_hills, BIAS_THREADS * 4);
+    int nb = div_up(c->p.max_hills, BIAS_THREADS);
     if (nb > BIAS_MAX_BLOCKS) nb = BIAS_MAX_BLOCKS;
     if (nb < 1) nb = 1;
     k_bias_sum<<<nb, BIAS_THREADS, 0, c->stream>>>(bp, c->d_centers, c->d_heights, c->d_nhills, d_cv, c->d_bias_partials,
