@@ -50,6 +50,35 @@ def test_tiled_coordination_switching_exponents(n, m):
     assert np.abs(r["F"].sum(axis=0)).max() <= 1e-3 * np.abs(r["F_ref"]).max()      # translation invariance (reading N), fp32 sums
 
 
+@pytest.mark.parametrize("drop", [0, 1, 2, 3])
+def test_tiled_coordination_force_update_unaligned_and_ragged(drop):
+    """k_force_add4 adds the per-atom gradient to F with 128-bit accesses, four atoms per thread; a ragged tail (N not a
+    multiple of 4, nor of the 32-atom list slabs) and a caller's F that is not 16-byte aligned (scalar k_force_add) must give
+    the same forces: both against the oracle, on top of a non-zero F."""
+    import torch
+    w = _workload()
+    n = w.natoms - drop
+    w.pos = np.ascontiguousarray(w.pos[:n])
+    assert w.natoms == n
+    w.cvs = [CVSpec(kind=CV_COORD, r0=2.4, n=6, m=12, scale=1.0 / n)]
+    w.sigma = [0.05]
+    r = stagewise(w, precision=32)
+    assert_stagewise(r)
+    md, fmax = r["md"], np.abs(r["F_ref"]).max()
+    dV_in = torch.tensor(r["dV_ref"], device="cuda", dtype=torch.float64)
+    for offset in (0, 1):                                    # offset 1 float: F is 4 bytes off a 16-byte boundary
+        with torch.cuda.stream(md.stream):
+            buf = torch.full((3 * n + 4,), 0.25, device="cuda", dtype=torch.float32)
+        F = buf[offset:offset + 3 * n].view(n, 3)
+        assert (F.data_ptr() % 16 == 0) == (offset == 0)
+        md.synchronize()
+        md.apply_forces(F, dVds=dV_in)
+        md.synchronize()
+        out = buf.cpu().numpy().astype(np.float64)
+        assert np.abs(out[offset:offset + 3 * n].reshape(n, 3) - 0.25 - r["F_ref"]).max() <= TOL_F * fmax + 2 ** -24
+        assert np.all(out[:offset] == 0.25) and np.all(out[offset + 3 * n:] == 0.25)      # nothing written outside F
+
+
 def test_lattice_only_context_and_bad_axis():
     import torch
     from paper_2510_06873_b200.metad import MetaD, MetadError
