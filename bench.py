@@ -62,6 +62,11 @@ def describe(w, precision):
             "pair_precision": f"fp{precision}", "stride": int(w.stride), "virial": bool(getattr(w, "_virial", False)),
             "neighbour_build": ("skipped (lazy_neighbors: no CV of this workload reads the list)"
                                 if (w.name in ("t0", "r0") or getattr(w, "_lazy", False)) and all(c.kind in (3, 4, 5, 6, 7) for c in w.cvs)
+                                else "every step, list-free (lazy_neighbors: the candidate scan accumulates the coordination sum and "
+                                     "the per-atom gradient and stores no list)"
+                                if getattr(w, "_lazy", False) and precision == 32 and not getattr(w, "_virial", False)
+                                and w.max_neigh <= 32 and any(c.kind == 0 and c.group_a is None and c.group_b is None for c in w.cvs)
+                                and not any(c.kind in (1, 2, 6) for c in w.cvs)
                                 else "every step"),
             "l2": ("per-step working set (neighbour list + q6 records + positions + forces) exceeds the 126 MB L2; no flush"
                    if w.natoms * (4 * w.max_neigh + 64 + 16 + 24 + 16) > 126e6 else
@@ -407,7 +412,7 @@ def run_ours(args):
             roof_all.append(r_build)
             if list_ms > stage_ms[3]:
                 roof = r_build                     # the dominant kernel of the step
-    elif (precision == 32 and list_ms is not None and not args.virial
+    elif (precision == 32 and list_ms is not None and not args.virial and not args.lazy
           and sum(c.kind == 0 and c.group_a is None and c.group_b is None for c in w.cvs) == 1
           and getattr(w, "max_neigh", 64) <= 32):
         # tiled coordination path (g0): the list build with the sum of sw and its per-atom gradient riding on the exact pass

@@ -109,7 +109,10 @@ typedef struct {
                                        PAPER.md:85-87 reweights them) — see metad_reweight_recorded.  Full: METAD_DEV_TRAJ_FULL */
     int lazy_neighbors;             /* != 0: metad_build_neighbors only snapshots the positions when no CV of the context reads the
                                        neighbour list (torsion / Rg / contacts / lattice CVs): a 22-atom torsion step is pure
-                                       launch latency and the list build is half of its launches.  0 (default): always built */
+                                       launch latency and the list build is half of its launches.  An ungrouped coordination
+                                       number in fp32 (tiled path, no virial) then runs list-free as well: the candidate scan
+                                       accumulates the sum and the per-atom gradient and stores no list.  metad_get_neighbors
+                                       returns METAD_ERR_STATE in both cases.  0 (default): always built */
     int want_virial;                /* != 0: metad_apply_forces also computes the bias virial (metad_get_virial) for NPT runs
                                        (reading AD), for every CV kind */
 } metad_params;

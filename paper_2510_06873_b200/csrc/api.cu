@@ -362,8 +362,9 @@ extern "C" int metad_build_neighbors(metad_ctx *c, const void *d_pos, const doub
         c->have_neighbors = true; c->list_built = false;
         return METAD_OK;
     }
+    c->list_skipped = 0;
     r = nb_build(c, d_pos);
-    if (r == METAD_OK) { c->have_neighbors = true; c->list_built = true; }
+    if (r == METAD_OK) { c->have_neighbors = true; c->list_built = !c->list_skipped; }
     return r;
 }
 
@@ -519,7 +520,7 @@ extern "C" int metad_get_state(metad_ctx *c, double *h_cv, double *h_V, double *
 extern "C" int metad_get_neighbors(metad_ctx *c, int *d_count, int *d_list) {
     if (!c || !d_count || !d_list) FAIL(METAD_ERR_ARG, "null argument");
     if (!c->have_neighbors) FAIL(METAD_ERR_STATE, "metad_build_neighbors has not been called");
-    if (!c->list_built) FAIL(METAD_ERR_STATE, "lazy_neighbors: no CV reads the list, it was not built");
+    if (!c->list_built) FAIL(METAD_ERR_STATE, "lazy_neighbors: nothing in this context reads the list, it was not built");
     return nb_export(c, d_count, d_list);
 }
 

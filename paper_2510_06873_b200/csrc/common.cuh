@@ -236,6 +236,7 @@ struct metad_ctx {
     float *d_cgrad;                       // tiled coordination path: per-atom sum_j 2 sw' d / (r0 r) as float4, ORIGINAL atom
                                           // order (k_tile_build<2>), scaled and added to F by k_force_add
     double *d_cvq6;                       // tiled path: [Q6 mean, solid count] finished by k_tile_build
+    int list_skipped;                     // the last tiled coordination build ran list-free (lazy_neighbors)
     double *cv_direct;                    // run paths (metad_run, metad_step_host): the context's CV vector, which the last block
                                           // of k_tile_build fills itself (no k_q6_publish launch); NULL on the stage calls
 };

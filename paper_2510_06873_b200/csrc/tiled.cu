@@ -146,7 +146,9 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
         }
         if (!in) continue;
         if (n < maxn) {
-            __stcs(out + n * 32, __float_as_int(pj.w));     // streaming store: the list is read once, by the force pass
+            // streaming store: the list is read once, by the force pass (MODE 2 with nl == NULL: list-free pass, the sum
+            // and the gradient below are all the step needs — params.lazy_neighbors)
+            if (MODE != 2 || nl) __stcs(out + n * 32, __float_as_int(pj.w));
             if (MODE == 2) {
                 // the per-atom gradient sum_j 2 sw'(r_ij) d_ij / (r0 r_ij) does not depend on dV/ds: accumulated here, the
                 // force stage only scales it (k_force_add, cv.cu) instead of walking the list again
@@ -187,7 +189,7 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
     for (int m = 1; m <= 6; ++m) upk2(AP[m - 1], A[2 * m - 1], A[2 * m]);
 #endif
     if (n > maxn) { atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW); n = maxn; }
-    nl_count[s] = n;
+    if (MODE != 2 || nl) nl_count[s] = n;
     float q6 = 0.f;
     if (WITH_Q6) {
         float S = 0.f;
@@ -345,9 +347,12 @@ int tiled_build(metad_ctx *c) {
             c->d_cvq6, c->cv_direct, c->q6_mean_dim, c->q6_solid_dim);
     else if (c->has_coord) {                                  // ungrouped coordination number: the sum of sw rides on the exact pass
         const CvDev &d = c->cv[c->coord_dim];
+        // lazy_neighbors: nothing downstream reads the list (the force stage scales the per-atom gradient; the virial would
+        // walk the list) — the pass runs list-free and metad_get_neighbors reports that there is no list
+        c->list_skipped = c->p.lazy_neighbors && !c->p.want_virial && c->d_cgrad;
         k_tile_build<2><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
-            c->d_nl_count, c->d_nl, c->d_sticky, (float)(1.0 / d.r0), 1.f, c->d_cgrad, nullptr, 0, d.n, d.m, c->d_perm,
+            c->d_nl_count, c->list_skipped ? nullptr : c->d_nl, c->d_sticky, (float)(1.0 / d.r0), 1.f, c->d_cgrad, nullptr, 0, d.n, d.m, c->d_perm,
             c->d_partials + c->nblocks_atoms, c->d_tickets + 1, d.scale, 0.0, c->d_cvq6, c->cv_direct, c->coord_dim, -1);
     } else
         k_tile_build<0><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(

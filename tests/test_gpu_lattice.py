@@ -79,6 +79,40 @@ def test_tiled_coordination_force_update_unaligned_and_ragged(drop):
         assert np.all(out[:offset] == 0.25) and np.all(out[offset + 3 * n:] == 0.25)      # nothing written outside F
 
 
+def test_lazy_neighbors_runs_the_tiled_coordination_pass_list_free():
+    """params.lazy_neighbors on the paper's GaN CV set: the fp32 tiled build accumulates the coordination sum and
+    the per-atom gradient and stores no list — same CV, V and forces bit for bit as with the list, metad_get_neighbors says so;
+    with the virial wanted the list is built regardless (its force kernel walks it)."""
+    import torch
+    from paper_2510_06873_b200.metad import MetaD, MetadError
+    w = _workload()
+    pos = np.ascontiguousarray(w.pos.astype(np.float32))
+    outs = []
+    for lazy, vir in ((False, False), (True, False), (True, True)):
+        md = MetaD(w, precision=32, max_hills=64, lazy_neighbors=lazy, want_virial=vir)
+        s0 = np.array([5.4, *np.linalg.norm(w.box.reshape(3, 3), axis=1)])
+        md.set_hills(np.array([s0 + [0.03, 0.05, -0.02, 0.04]]), np.array([1.5]))
+        with torch.cuda.stream(md.stream):
+            dpos = torch.tensor(pos, device="cuda")
+            F = torch.zeros((w.natoms, 3), device="cuda", dtype=torch.float32)
+        md.synchronize()
+        md.run(dpos, F, 3)
+        st = md.state()
+        assert md.status() == 0
+        outs.append((st["cv"].copy(), st["V"], F.cpu().numpy()))
+        if lazy and not vir:
+            with pytest.raises(MetadError):
+                md.neighbors()
+        else:
+            cnt, _ = md.neighbors()
+            assert cnt.sum() > 0
+    assert np.abs(outs[0][2]).max() > 0
+    for o in outs[1:]:
+        assert np.array_equal(o[0], outs[0][0]) and o[1] == outs[0][1]
+    assert np.array_equal(outs[1][2], outs[0][2])
+    assert np.abs(outs[2][2] - outs[0][2]).max() <= 1e-5 * np.abs(outs[0][2]).max()      # k_coord_force_g: other summation order
+
+
 def test_lattice_only_context_and_bad_axis():
     import torch
     from paper_2510_06873_b200.metad import MetaD, MetadError
