@@ -117,15 +117,21 @@ typedef struct {
                                        (reading AD), for every CV kind */
 } metad_params;
 
-/* Creates a context on the current CUDA device; `cuda_stream` is a cudaStream_t (NULL = default
- * stream) on which every later call is enqueued.  [sync] */
+/* Creates a context on the current CUDA device; `cuda_stream` is the cudaStream_t on which every later call is enqueued.
+ * NULL: the library creates a private NON-BLOCKING stream for the context (owned by it, destroyed by metad_destroy) — the
+ * legacy default stream cannot be captured into a CUDA graph, which metad_run needs.  Work of the caller on other streams
+ * (the legacy default stream included) is then NOT ordered with the library's kernels: order it with metad_synchronize()
+ * or any [sync] call before reading results, and finish writing d_pos / d_F before calling in.
+ * On failure nothing stays allocated.  [sync] */
 int metad_create(metad_ctx **out, const metad_params *params, void *cuda_stream);
 int metad_destroy(metad_ctx *ctx);
 
 /* a1 (BASELINE.json north_star "build the neighbour list"; reading O, P): bins atoms into cells,
  * counting-sorts them, and builds the full neighbour list (all j != i with minimum-image
- * r_ij < rc, strict).  Snapshots the positions: later calls of this step use them.
- * d_pos: [N][3] in params.precision.  box: host.  Errors: METAD_ERR_BOX, METAD_ERR_ARG. */
+ * r_ij < rc, strict).  d_pos: [N][3] in params.precision; the pointer is kept, not the data: the chain, torsion and
+ * nearest-distance CVs (and their forces / virial) read d_pos again in metad_eval_cv / metad_apply_forces, so the caller must
+ * leave d_pos unmodified until the metad_apply_forces of this step has completed (the neighbour-list CVs work on the
+ * cell-sorted copy made here).  box: host.  Errors: METAD_ERR_BOX, METAD_ERR_ARG. */
 int metad_build_neighbors(metad_ctx *ctx, const void *d_pos, const double *h_box, double rc);
 
 /* a2-a4: evaluates all CVs; d_cv: double[ncv] (device, caller-owned). */
@@ -194,8 +200,10 @@ int metad_bias_batch(metad_ctx *ctx, const double *d_points, int npoints, double
  * hills.  The delta is a histogram (reading Z): h_nbins[d] uniform bins on [h_lo[d], h_hi[d]) (periodic
  * dimensions are wrapped first and need hi - lo == period); frames outside a non-periodic range count in the
  * denominator only.  d_P, d_F: double[nbins0 * nbins1] row-major (nbins1 = 1 if ncv = 1); empty bins: P = 0, F = +inf.
- * Weights are accumulated as 2^-40 fixed point relative to the largest one (integer atomics: bit-identical from run to
- * run).  Not a per-step call: allocates and frees its scratch (V per frame, bins).  [sync] */
+ * Weights are accumulated per bin, relative to the largest weight of that bin, as 2^-64 fixed point in 128-bit integer
+ * sums (integer atomics: bit-identical from run to run; up to 2^63 frames per bin), and the bins are combined in log space:
+ * a bin any number of kT below the most probable one keeps full precision, and F is finite for every bin that holds a frame
+ * (P may underflow to 0 there).  Not a per-step call: allocates and frees its scratch (V and bin per frame, bins).  [sync] */
 int metad_reweight(metad_ctx *ctx, const double *d_traj, int nframes, const int *h_nbins, const double *h_lo,
                    const double *h_hi, double *d_P, double *d_F);
 
@@ -226,6 +234,23 @@ int metad_get_timing(metad_ctx *ctx, float *h_ms_sort, float *h_ms_list);
 
 /* Number of kernels the library has launched on this context so far (graph replays included). */
 long long metad_launch_count(metad_ctx *ctx);
+
+/* [sync] Waits for everything enqueued on the context's stream (the way to order a context created with cuda_stream ==
+ * NULL against the caller's own work). */
+int metad_synchronize(metad_ctx *ctx);
+
+/* Proof of the zero-host-copy step (BASELINE.json north_star: "a multi-step loop makes zero host round-trips"; PAPER.md:61 on
+ * GPU-CPU transfer overhead): node counts of the CUDA graph metad_run captured last.
+ * h_counts: int[8] = { nodes, kernel nodes, memcpy nodes, memset nodes, host nodes, other nodes,
+ *                      captures so far, in-place graph updates so far }.
+ * Errors: METAD_ERR_STATE before the first metad_run. */
+int metad_graph_info(metad_ctx *ctx, int *h_counts);
+
+/* Scalar-pipe roofline denominators: dependent-free FMA chains on every SM of the current device,
+ * timed with CUDA events, best of four launches after two warm-up launches.  kind 0: fp32 FFMA, 1: fp32 FFMA2 (packed pairs,
+ * sm_100), 2: fp64 DFMA.  *h_tflops: achieved TFLOP/s (an FMA = 2 flop); *h_ms (may be NULL): duration of that launch.
+ * Needs no context.  [sync] */
+int metad_fma_peak(int kind, double *h_tflops, double *h_ms);
 
 const char *metad_version(void);
 const char *metad_last_error(void);

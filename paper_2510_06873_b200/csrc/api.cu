@@ -30,6 +30,8 @@ static int upload_doubles(double **dst, const double *src, size_t n) {
     return METAD_OK;
 }
 
+static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream);
+
 extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_stream) {
     if (!out || !p) FAIL(METAD_ERR_ARG, "null argument");
     if (p->natoms <= 0) FAIL(METAD_ERR_ARG, "natoms must be positive");
@@ -53,11 +55,29 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     if (tiled_init()) return METAD_ERR_CUDA;
     metad_ctx *c = new metad_ctx();
     memset(c, 0, sizeof(*c));
+    // every failure below leaves through ONE path that frees whatever was allocated so far (metad_destroy works on a
+    // partially built context: all members start as zero)
+    const int r = create_impl(c, p, cuda_stream);
+    if (r != METAD_OK) {
+        char keep[sizeof(g_err)];
+        snprintf(keep, sizeof(keep), "%s", g_err);
+        metad_destroy(c);
+        metad_set_error(keep);
+        return r;
+    }
+    *out = c;
+    return METAD_OK;
+}
+
+static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
     c->p = *p;
     c->N = p->natoms; c->prec = p->precision; c->maxn = p->max_neigh; c->D = p->ncv;
     if (c->p.force_scale == 0.0) c->p.force_scale = 1.0;
     c->stream = (cudaStream_t)cuda_stream;
-    if (!c->stream) CUDA_TRY(cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking));
+    if (!c->stream) {                             // include/metad.h: NULL = a private non-blocking stream owned by the context
+        CUDA_TRY(cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking));
+        c->owns_stream = 1;
+    }
     c->q6_mean_dim = c->q6_solid_dim = c->coord_dim = c->mindist_dim = -1;
     const int N = c->N;
     const size_t tsz = c->prec == 32 ? sizeof(float) : sizeof(double);
@@ -231,28 +251,31 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     for (int k = 0; k < 3; ++k) CUDA_TRY(cudaEventCreate(&c->ev[k]));
     CUDA_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
     CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
+    CUDA_TRY(dev_alloc(&c->d_hill_stage, (size_t)(c->D + 1) * p->max_hills));
     CUDA_TRY(cudaDeviceSynchronize());
-    *out = c;
     return METAD_OK;
 }
 
 extern "C" int metad_destroy(metad_ctx *c) {
     if (!c) return METAD_OK;
-    cudaStreamSynchronize(c->stream);
+    if (c->stream) cudaStreamSynchronize(c->stream);
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->graph) cudaGraphDestroy(c->graph);
     for (int k = 0; k < 3; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     if (c->ev_copy) cudaEventDestroy(c->ev_copy);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
         void *q2[] = { v.d_pairs, v.d_pair_r0, v.d_csr_off, v.d_csr_pair, v.d_catoms, v.d_chain, v.d_mass, v.d_unwrapped, v.d_ga, v.d_gb };
         for (void *q : q2) if (q) cudaFree(q);
     }
+    if (c->owns_stream && c->stream) cudaStreamDestroy(c->stream);
+    (void)cudaGetLastError();
     delete c;
     return METAD_OK;
 }
@@ -296,28 +319,18 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
     // shared-memory tiled fast path: fp32, neighbour-list CVs = Q6 only or an ungrouped coordination number only,
     // >= 3 cells per direction
     c->tiled = 0;
-    const char *env = getenv("METAD_NO_TILES");
     const bool q6_only = c->has_q6 && !c->has_coord;
     const bool coord_only = c->has_coord && !c->has_q6 && !c->cv[c->coord_dim].use_groups;
-    if (c->prec == 32 && (q6_only || coord_only) && !c->has_mindist && c->N < (1 << NL_IDX_BITS) && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32 &&
-        !(env && env[0] == '1')) {
+    if (c->prec == 32 && (q6_only || coord_only) && !c->has_mindist && c->N < (1 << NL_IDX_BITS) && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32) {
         // the rc-wide cells are subdivided along x (the direction of the contiguous row runs): an atom then scans
         // 2 xsub + 1 sub-cells per row (2.5 / 2.25 cell widths for xsub = 2 / 4) instead of 3 cells
         int xsub = 2;
-        const char *xs = getenv("METAD_XSUB");
-        if (xs && xs[0] >= '1' && xs[0] <= '4') xsub = xs[0] - '0';
         while (xsub > 1 && (long long)g.ncell * xsub > c->cell_cap) --xsub;
         CellGrid gs = g;
         gs.nc[0] *= xsub; gs.ncell *= xsub;
         const double rho = (double)c->N / gs.ncell, margin = 1.3;
         int cap = 1216;
         double best = 1e30; int bt[3] = { 0, 0, 0 };
-        int ov[4] = { 0, 0, 0, 0 };
-        const char *te = getenv("METAD_TILE");               // experiment switch: "tx,ty,tz,cap" (tx in sub-cells)
-        if (te && sscanf(te, "%d,%d,%d,%d", &ov[0], &ov[1], &ov[2], &ov[3]) == 4 && ov[0] >= 1 && ov[0] <= TILE_TXMAX &&
-            ov[1] >= 1 && ov[1] <= 4 && ov[2] >= 1 && ov[2] <= 4 && ov[3] >= 64 && ov[3] <= 4096) {
-            bt[0] = ov[0]; bt[1] = ov[1]; bt[2] = ov[2]; cap = ov[3];
-        } else
         // two passes: the smallest halo ratio, then among the shapes within 2 % of it the longest along x (rows are the
         // contiguous runs of the staging copies and of the scan: 11 x 3 x 3 beats 8 x 4 x 3 by 1.8 % at c3)
         for (int pass = 0; pass < 2; ++pass)
@@ -454,7 +467,10 @@ extern "C" int metad_run(metad_ctx *c, const void *d_pos, const double *h_box, d
             else { cudaGetLastError(); cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         }
         if (!updated) CUDA_TRY(cudaGraphInstantiate(&c->graph_exec, graph, 0));
-        cudaGraphDestroy(graph);
+        if (c->graph) cudaGraphDestroy(c->graph);
+        c->graph = graph;                           // kept for metad_graph_info
+        c->graph_captures++;
+        c->graph_updates += updated ? 1 : 0;
         c->launches_per_step = (int)(c->launches - before);
         c->launches = before;                      // capture enqueued nothing
         c->graph_pos = d_pos; c->graph_F = d_F; c->graph_rc = rc;
@@ -536,14 +552,10 @@ extern "C" int metad_set_hills(metad_ctx *c, const double *centers, const double
     if (on_device || count == 0) {
         r = bias_set_hills_dev(c, centers, heights, count);
     } else {
-        double *dc = nullptr, *dh = nullptr;
-        CUDA_TRY(dev_alloc(&dc, (size_t)count * c->D));
-        CUDA_TRY(dev_alloc(&dh, count));
+        double *dc = c->d_hill_stage, *dh = c->d_hill_stage + (size_t)c->D * c->p.max_hills;   // staging from metad_create
         CUDA_TRY(cudaMemcpyAsync(dc, centers, sizeof(double) * (size_t)count * c->D, cudaMemcpyHostToDevice, c->stream));
         CUDA_TRY(cudaMemcpyAsync(dh, heights, sizeof(double) * count, cudaMemcpyHostToDevice, c->stream));
         r = bias_set_hills_dev(c, dc, dh, count);
-        cudaStreamSynchronize(c->stream);
-        cudaFree(dc); cudaFree(dh);
     }
     if (r) return r;
     CUDA_TRY(cudaStreamSynchronize(c->stream));
@@ -562,15 +574,11 @@ extern "C" int metad_get_hills(metad_ctx *c, double *centers, double *heights, i
         int r = bias_get_hills_dev(c, centers, heights, capacity);
         if (r) return r;
     } else {
-        double *dc = nullptr, *dh = nullptr;
-        CUDA_TRY(dev_alloc(&dc, (size_t)capacity * c->D));
-        CUDA_TRY(dev_alloc(&dh, capacity));
-        int r = bias_get_hills_dev(c, dc, dh, capacity);
+        double *dc = c->d_hill_stage, *dh = c->d_hill_stage + (size_t)c->D * c->p.max_hills;
+        int r = bias_get_hills_dev(c, dc, dh, std::min(capacity, c->p.max_hills));
         if (r) return r;
         CUDA_TRY(cudaMemcpyAsync(centers, dc, sizeof(double) * (size_t)n * c->D, cudaMemcpyDeviceToHost, c->stream));
         CUDA_TRY(cudaMemcpyAsync(heights, dh, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
-        cudaStreamSynchronize(c->stream);
-        cudaFree(dc); cudaFree(dh);
     }
     CUDA_TRY(cudaStreamSynchronize(c->stream));
     return METAD_OK;
@@ -653,3 +661,32 @@ extern "C" int metad_get_timing(metad_ctx *c, float *ms_sort, float *ms_list) {
 }
 
 extern "C" long long metad_launch_count(metad_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" int metad_synchronize(metad_ctx *c) {
+    if (!c) FAIL(METAD_ERR_ARG, "null argument");
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return METAD_OK;
+}
+
+extern "C" int metad_graph_info(metad_ctx *c, int *h_counts) {
+    if (!c || !h_counts) FAIL(METAD_ERR_ARG, "null argument");
+    if (!c->graph) FAIL(METAD_ERR_STATE, "metad_run has not captured a step yet");
+    size_t n = 0;
+    CUDA_TRY(cudaGraphGetNodes(c->graph, nullptr, &n));
+    std::vector<cudaGraphNode_t> nodes(n);
+    if (n) CUDA_TRY(cudaGraphGetNodes(c->graph, nodes.data(), &n));
+    int k[6] = { (int)n, 0, 0, 0, 0, 0 };
+    for (size_t i = 0; i < n; ++i) {
+        cudaGraphNodeType t;
+        CUDA_TRY(cudaGraphNodeGetType(nodes[i], &t));
+        if (t == cudaGraphNodeTypeKernel) k[1]++;
+        else if (t == cudaGraphNodeTypeMemcpy) k[2]++;
+        else if (t == cudaGraphNodeTypeMemset) k[3]++;
+        else if (t == cudaGraphNodeTypeHost) k[4]++;
+        else k[5]++;
+    }
+    memcpy(h_counts, k, sizeof(k));
+    h_counts[6] = c->graph_captures;
+    h_counts[7] = c->graph_updates;
+    return METAD_OK;
+}

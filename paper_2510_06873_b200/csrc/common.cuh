@@ -22,6 +22,7 @@ struct PBox {
     T ax, bx, by, cx, cy, cz;        // hi parts (the whole value for T=double)
     T lax, lbx, lby, lcx, lcy, lcz;  // lo parts (0 for T=double)
     T hx, hy, hz;                    // half box: 0.5*ax, 0.5*by, 0.5*cz
+    T band;                          // T=float: |r^2 - rc^2| <= band is re-decided in fp64 (neighbor.cu: pair_in_range); 0 for double
 };
 
 struct BoxD {                        // fp64 box, used by the canonical neighbour predicate
@@ -224,6 +225,10 @@ struct metad_ctx {
     void *h_pin; size_t h_pin_bytes;
     // graph
     cudaGraphExec_t graph_exec;
+    cudaGraph_t graph;                    // the captured step (kept for metad_graph_info)
+    int graph_captures, graph_updates;    // how often metad_run captured a step / updated the instantiated graph in place
+    int owns_stream;                      // metad_create made the stream (cuda_stream == NULL): destroyed with the context
+    double *d_hill_stage;                 // [(D + 1) * max_hills] staging of metad_set_hills / metad_get_hills with host pointers
     const void *graph_pos; void *graph_F; double graph_rc; double graph_box[9];
     long long launches; int launches_per_step;
     const void *d_pos_last;               // positions snapshot pointer of the last build (chain CVs read it)

@@ -351,9 +351,7 @@ __device__ __forceinline__ void ldg256(const float *p, float4 &a, float4 &b) {
                  : "l"(p));
 }
 
-#ifndef Q6F_MINB
-#define Q6F_MINB 9
-#endif
+#define Q6F_MINB 9             // resident blocks per SM of k_q6_force_g (56 registers)
 template <bool SOLID, bool VIRIAL>
 __global__ void __launch_bounds__(CV_THREADS, VIRIAL ? 8 : Q6F_MINB)
 k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,

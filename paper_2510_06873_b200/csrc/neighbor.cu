@@ -7,6 +7,7 @@
 //   k_build_list     per-atom candidate scan of the 27 neighbouring cells; canonical predicate
 // Everything downstream works in "sorted space" (indices into the cell-sorted arrays), so that the
 // gathers of the CV and force passes touch neighbouring memory.
+#include <math.h>
 #include "common.cuh"
 
 #define SCAN_THREADS 512
@@ -167,7 +168,7 @@ __device__ __forceinline__ bool pair_in_range<float>(const PBox<float> &pb, cons
     min_image(pb, dx, dy, dz);
     float r2 = dx * dx + dy * dy + dz * dz;
     bool in = r2 < rc2T;
-    if (fabsf(r2 - rc2T) <= 1e-5f * rc2T)
+    if (fabsf(r2 - rc2T) <= pb.band)
         in = r2_canonical(bd, (double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y,
                           (double)pj.z - (double)pi.z) < rc2;
     return in;
@@ -350,14 +351,14 @@ __global__ void k_export_list(int N, int maxn, const int *__restrict__ perm, con
 }
 
 template <typename T>
-static PBox<T> make_pbox(const BoxD &b);
+static PBox<T> make_pbox(const BoxD &b, double rc);
 template <>
-PBox<double> make_pbox<double>(const BoxD &b) {
-    PBox<double> p = { b.ax, b.bx, b.by, b.cx, b.cy, b.cz, 0, 0, 0, 0, 0, 0, b.hx, b.hy, b.hz };
+PBox<double> make_pbox<double>(const BoxD &b, double) {
+    PBox<double> p = { b.ax, b.bx, b.by, b.cx, b.cy, b.cz, 0, 0, 0, 0, 0, 0, b.hx, b.hy, b.hz, 0.0 };
     return p;
 }
 template <>
-PBox<float> make_pbox<float>(const BoxD &b) {
+PBox<float> make_pbox<float>(const BoxD &b, double rc) {
     PBox<float> p;
     const double v[6] = { b.ax, b.bx, b.by, b.cx, b.cy, b.cz };
     float hi[6], lo[6];
@@ -365,9 +366,17 @@ PBox<float> make_pbox<float>(const BoxD &b) {
     p.ax = hi[0]; p.bx = hi[1]; p.by = hi[2]; p.cx = hi[3]; p.cy = hi[4]; p.cz = hi[5];
     p.lax = lo[0]; p.lbx = lo[1]; p.lby = lo[2]; p.lcx = lo[3]; p.lcy = lo[4]; p.lcz = lo[5];
     p.hx = (float)b.hx; p.hy = (float)b.hy; p.hz = (float)b.hz;
+    // Recheck band of the fp32 fast test.  Inside the primary cell pj - pi is exact only while the two coordinates are within
+    // a factor 2 of one another; across a periodic face the raw difference is of the order of the box and is rounded at
+    // ulp_f32(L) / 2 per component before the (hi + lo) lattice shift restores the small vector, so r^2 carries up to
+    // 2 sum_c |d_c| ulp(L) / 2 <= sqrt(3) rc ulp(L) on top of the ~4 ulp(rc^2) of the three products.  The band must cover
+    // both: max(1e-5 rc^2, 4 rc ulp_f32(L)) with L the largest coordinate a position can take.
+    const double L = fmax(fabs(b.ax) + fabs(b.bx) + fabs(b.cx), fmax(fabs(b.by) + fabs(b.cy), fabs(b.cz)));
+    const double ulpL = ldexp(1.0, ilogb(fmax(L, 1e-30)) - 23);
+    p.band = (float)fmax(1e-5 * rc * rc, 4.0 * rc * ulpL);
     return p;
 }
-template <typename T> PBox<T> ctx_pbox(const metad_ctx *c) { return make_pbox<T>(c->boxd); }
+template <typename T> PBox<T> ctx_pbox(const metad_ctx *c) { return make_pbox<T>(c->boxd, c->rc); }
 template PBox<float> ctx_pbox<float>(const metad_ctx *);
 template PBox<double> ctx_pbox<double>(const metad_ctx *);
 
@@ -381,7 +390,7 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     if (N <= METAD_SMALL_N && !c->tiled) {                     // the whole neighbour stage in one launch
         if (tm) { cudaEventRecord(c->ev[0], st); cudaEventRecord(c->ev[1], st); c->timing_recorded = 1; }
         k_build_list_small<T><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const T *)d_pos, c->d_flags, (V4 *)c->d_spos, c->d_perm,
-                                                                             c->d_scell, make_pbox<T>(c->boxd), c->boxd, (T)c->rc2, c->rc2,
+                                                                             c->d_scell, make_pbox<T>(c->boxd, c->rc), c->boxd, (T)c->rc2, c->rc2,
                                                                              c->maxn, c->d_nl_count, c->d_nl, c->grid, c->d_sticky);
         if (tm) cudaEventRecord(c->ev[2], st);
         c->launches += 1;
@@ -404,7 +413,7 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
         if (tm) cudaEventRecord(c->ev[2], st);
         return r;
     }
-    PBox<T> pb = make_pbox<T>(c->boxd);
+    PBox<T> pb = make_pbox<T>(c->boxd, c->rc);
     if (N <= METAD_WARP_PER_ATOM_MAX)
         k_build_list_warp<T, 32><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start,
                                                                                  c->grid, pb, c->boxd, (T)c->rc2, c->rc2, c->maxn,

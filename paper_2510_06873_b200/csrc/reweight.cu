@@ -3,10 +3,11 @@
 // averages over the frames of the biased trajectory (reading Z: delta = uniform bins).
 //   k_bias_batch      V_b at T points: thread per point, the hill array streamed through shared memory
 //                     in tiles (the FP64 exp is the work: T x H evaluations, pure ALU, no HBM re-reads)
-//   k_vmax            max of V over the frames (order-independent)
-//   k_reweight_hist   w = e^{(V - Vmax)/kT} as 2^-40 fixed point, integer atomics into the bins: the
-//                     sums do not depend on the order of the atomics => run-to-run bit-identical
-//   k_reweight_finish P = bin / (total x bin volume), F = -kT log P (+inf for empty bins)
+//   k_reweight_binmax bin of every frame; largest V inside each bin (order-independent atomic max)
+//   k_reweight_hist   w = e^{(V - Vmax_bin)/kT} as 2^-64 fixed point summed into a 128-bit integer per bin: the
+//                     sums do not depend on the order of the atomics => run-to-run bit-identical, and a bin far
+//                     below the most probable one keeps the full resolution of its own sum
+//   k_reweight_finish bins combined in log space: P = W_b / (sum W x bin volume), F = -kT log P (+inf for empty bins)
 #include <math.h>
 #include <string.h>
 #include <algorithm>
@@ -61,39 +62,19 @@ __device__ __forceinline__ unsigned long long dkey(double x) {
     unsigned long long u = (unsigned long long)__double_as_longlong(x);
     return (u >> 63) ? ~u : (u | 0x8000000000000000ull);
 }
-__host__ __device__ inline double dkey_inv(unsigned long long k) {
+__device__ __forceinline__ double dkey_inv(unsigned long long k) {
     unsigned long long u = (k >> 63) ? (k & 0x7fffffffffffffffull) : ~k;
-#ifdef __CUDA_ARCH__
     return __longlong_as_double((long long)u);
-#else
-    double d; memcpy(&d, &u, sizeof(d)); return d;
-#endif
 }
 
-__global__ void k_vmax(int T, const double *__restrict__ V, unsigned long long *__restrict__ key) {
-    unsigned long long m = 0ull;
-    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < T; t += gridDim.x * blockDim.x) m = max(m, dkey(V[t]));
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_down_sync(0xffffffffu, m, o));
-    if ((threadIdx.x & 31) == 0) atomicMax(key, m);
-}
-
-#define RW_FIXED 1099511627776.0   // 2^40
-
-__global__ void k_reweight_hist(RwBins rb, int T, const double *__restrict__ traj, const double *__restrict__ V,
-                                const unsigned long long *__restrict__ vmax_key, double inv_kT,
-                                unsigned long long *__restrict__ hist /* [nb0*nb1] + total */) {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= T) return;
-    const double vmax = dkey_inv(*vmax_key);
-    const double w = exp((V[t] - vmax) * inv_kT);
-    const unsigned long long q = (unsigned long long)(w * RW_FIXED + 0.5);
+// bin of a frame (reading Z); nbins = the "outside" bin (frames beyond a non-periodic range: denominator only)
+__device__ __forceinline__ int rw_bin(const RwBins &rb, const double *__restrict__ s) {
     int idx[2] = { 0, 0 };
     bool inside = true;
 #pragma unroll
     for (int d = 0; d < 2; ++d) {
         if (d < rb.D) {
-            double x = traj[(size_t)t * rb.D + d];
+            double x = s[d];
             if (rb.period[d] > 0.0) {
                 x -= rb.period[d] * floor((x - rb.lo[d]) / rb.period[d]);
                 if (x >= rb.lo[d] + rb.period[d]) x -= rb.period[d];
@@ -105,20 +86,85 @@ __global__ void k_reweight_hist(RwBins rb, int T, const double *__restrict__ tra
             idx[d] = b;
         }
     }
-    const int nbins = rb.nb[0] * rb.nb[1];
-    atomicAdd(hist + nbins, q);
-    if (inside) atomicAdd(hist + (size_t)idx[0] * rb.nb[1] + idx[1], q);
+    return inside ? idx[0] * rb.nb[1] + idx[1] : rb.nb[0] * rb.nb[1];
 }
 
-__global__ void k_reweight_finish(RwBins rb, const unsigned long long *__restrict__ hist, double kT,
-                                  double *__restrict__ P, double *__restrict__ F) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+// Pass A: bin of every frame and the largest V inside each bin (atomic max on an order-preserving key).
+__global__ void k_reweight_binmax(RwBins rb, int T, const double *__restrict__ traj, const double *__restrict__ V,
+                                  int *__restrict__ bin_of, unsigned long long *__restrict__ vmax_key /* [nbins + 1] */) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= T) return;
+    const int b = rw_bin(rb, traj + (size_t)t * rb.D);
+    bin_of[t] = b;
+    atomicMax(vmax_key + b, dkey(V[t]));
+}
+
+// Pass B: the weight of a frame RELATIVE TO THE LARGEST ONE OF ITS OWN BIN, w = e^{(V - Vmax_bin)/kT} in (0, 1], as a 2^-64
+// fixed-point number summed into a 128-bit integer per bin (low word by atomicAdd, the carry into the high word): an
+// integer sum does not depend on the order of the atomics, so P and F are bit-identical from run to run; a bin holds up to
+// 2^63 frames, and a bin 60 kT (or 600 kT) below the most probable one keeps the full 64-bit resolution of its own sum —
+// nothing is quantised against the global maximum (the bins are combined in log space by k_reweight_finish).
+__global__ void k_reweight_hist(int T, const double *__restrict__ V, const int *__restrict__ bin_of,
+                                const unsigned long long *__restrict__ vmax_key, double inv_kT,
+                                unsigned long long *__restrict__ sum_lo, unsigned long long *__restrict__ sum_hi) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= T) return;
+    const int b = bin_of[t];
+    const double w = exp((V[t] - dkey_inv(vmax_key[b])) * inv_kT);           // <= 1, == 1 for the bin's top frame
+    const double x = w * 18446744073709551616.0;                              // * 2^64, exact scaling
+    if (x >= 18446744073709551616.0) { atomicAdd(sum_hi + b, 1ull); return; }
+    const unsigned long long q = (unsigned long long)x;                       // truncation: deterministic
+    const unsigned long long old = atomicAdd(sum_lo + b, q);
+    if (old + q < old) atomicAdd(sum_hi + b, 1ull);                           // carry
+}
+
+// log of the (unnormalised) weight of every bin, log W_b = log(sum_b) + Vmax_b / kT; the normalisation
+// log sum_b' W_b' (outside bin included) by a fixed-order log-sum-exp in one block; then
+//     P_b = W_b / (sum W vol),   F_b = -kT log P_b   (formed in log space: finite whenever the bin holds a frame).
+#define RW_FIN_THREADS 1024
+__global__ void __launch_bounds__(RW_FIN_THREADS)
+k_reweight_finish(RwBins rb, const unsigned long long *__restrict__ sum_lo, const unsigned long long *__restrict__ sum_hi,
+                  const unsigned long long *__restrict__ vmax_key, double kT, double *__restrict__ P, double *__restrict__ F) {
+    __shared__ double red[32];
+    __shared__ double s_top, s_logtot;
     const int nbins = rb.nb[0] * rb.nb[1];
-    if (b >= nbins) return;
-    const double tot = (double)hist[nbins];
-    const double p = tot > 0.0 ? (double)hist[b] / (tot * rb.vol) : 0.0;
-    P[b] = p;
-    F[b] = p > 0.0 ? -kT * log(p) : (double)INFINITY;
+    const double inv_kT = 1.0 / kT;
+    auto logw = [&](int b) -> double {
+        const double sum = (double)sum_hi[b] + (double)sum_lo[b] * (1.0 / 18446744073709551616.0);
+        return sum > 0.0 ? log(sum) + dkey_inv(vmax_key[b]) * inv_kT : -INFINITY;
+    };
+    // largest log W (fixed order)
+    double m = -INFINITY;
+    for (int b = threadIdx.x; b <= nbins; b += blockDim.x) m = fmax(m, logw(b));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_down_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = red[0];
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) t = fmax(t, red[w]);
+        s_top = t;
+    }
+    __syncthreads();
+    const double top = s_top;
+    double acc[1] = { 0.0 };
+    if (top > -INFINITY)
+        for (int b = threadIdx.x; b <= nbins; b += blockDim.x) { const double l = logw(b); if (l > -INFINITY) acc[0] += exp(l - top); }
+    block_reduce<1>(acc, red);
+    if (threadIdx.x == 0) s_logtot = top > -INFINITY ? top + log(acc[0]) : -INFINITY;
+    __syncthreads();
+    const double logtot = s_logtot, logvol = log(rb.vol);
+    for (int b = threadIdx.x; b < nbins; b += blockDim.x) {
+        const double l = logw(b);
+        if (l > -INFINITY) {
+            const double lp = l - logtot - logvol;
+            P[b] = exp(lp);
+            F[b] = -kT * lp;
+        } else {
+            P[b] = 0.0;
+            F[b] = (double)INFINITY;
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -155,22 +201,29 @@ int reweight_run(metad_ctx *c, const double *d_traj, int T, const int *nbins, co
         if (on) rb.vol *= (rb.hi[d] - rb.lo[d]) / rb.nb[d];
     }
     const int nb = rb.nb[0] * rb.nb[1];
+    // scratch of this call (not a per-step call): V per frame, bin per frame, per bin (+ the outside bin) the key of the
+    // largest V and the two words of the 128-bit weight sum
     double *d_V = nullptr;
-    unsigned long long *d_hist = nullptr;     // [nb] bins, [nb] total, [nb + 1] key of max V
-    CUDA_TRY(cudaMalloc((void **)&d_V, sizeof(double) * (size_t)(T > 0 ? T : 1)));
-    CUDA_TRY(cudaMalloc((void **)&d_hist, sizeof(unsigned long long) * ((size_t)nb + 2)));
-    CUDA_TRY(cudaMemsetAsync(d_hist, 0, sizeof(unsigned long long) * ((size_t)nb + 2), c->stream));
+    int *d_bin = nullptr;
+    unsigned long long *d_acc = nullptr;
+    const size_t nacc = 3 * ((size_t)nb + 1);
+    cudaError_t ea = cudaMalloc((void **)&d_V, sizeof(double) * (size_t)(T > 0 ? T : 1));
+    if (ea == cudaSuccess) ea = cudaMalloc((void **)&d_bin, sizeof(int) * (size_t)(T > 0 ? T : 1));
+    if (ea == cudaSuccess) ea = cudaMalloc((void **)&d_acc, sizeof(unsigned long long) * nacc);
+    if (ea != cudaSuccess) { cudaFree(d_V); cudaFree(d_bin); cudaFree(d_acc); CUDA_TRY(ea); }
+    unsigned long long *d_key = d_acc, *d_lo = d_acc + (nb + 1), *d_hi = d_acc + 2 * ((size_t)nb + 1);
+    cudaMemsetAsync(d_acc, 0, sizeof(unsigned long long) * nacc, c->stream);      // key 0 sorts below every double
     int r = bias_batch(c, d_traj, T, d_V);
     if (r == METAD_OK && T > 0) {
-        k_vmax<<<std::min(div_up(T, 256), 1024), 256, 0, c->stream>>>(T, d_V, d_hist + nb + 1);
-        k_reweight_hist<<<div_up(T, 256), 256, 0, c->stream>>>(rb, T, d_traj, d_V, d_hist + nb + 1, 1.0 / c->p.kT, d_hist);
+        k_reweight_binmax<<<div_up(T, 256), 256, 0, c->stream>>>(rb, T, d_traj, d_V, d_bin, d_key);
+        k_reweight_hist<<<div_up(T, 256), 256, 0, c->stream>>>(T, d_V, d_bin, d_key, 1.0 / c->p.kT, d_lo, d_hi);
         c->launches += 2;
     }
-    k_reweight_finish<<<div_up(nb, 256), 256, 0, c->stream>>>(rb, d_hist, c->p.kT, d_P, d_F);
+    k_reweight_finish<<<1, RW_FIN_THREADS, 0, c->stream>>>(rb, d_lo, d_hi, d_key, c->p.kT, d_P, d_F);
     c->launches++;
     cudaError_t e = cudaGetLastError();
     cudaStreamSynchronize(c->stream);
-    cudaFree(d_V); cudaFree(d_hist);
+    cudaFree(d_V); cudaFree(d_bin); cudaFree(d_acc);
     CUDA_TRY(e);
     return r;
 }

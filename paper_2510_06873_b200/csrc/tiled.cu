@@ -14,18 +14,12 @@
 #include "cv_switch.cuh"
 #include "tile.cuh"
 
-#ifndef TB_TMA
-#define TB_TMA 1               // interior tiles are staged by TMA bulk copies (tile_stage_pos_tma); 0: plain loads everywhere
-#endif
 
 typedef unsigned short nl16_t;   // local halo index (shared-memory candidate list only)
 #define LIST_CAP 40            // per-thread candidate slots in shared memory (maxn <= 32 on this path + band + self)
 
 // Packed fp32 pairs (sm_100 FADD2 / FMUL2 / FFMA2: one issue slot for two lanes of arithmetic; this kernel is bound by
 // instruction issue, not by the FMA pipe).  A scalar second operand is broadcast by the instruction itself.
-#ifndef TB_PACKED
-#define TB_PACKED 1
-#endif
 typedef unsigned long long f32x2_t;
 __device__ __forceinline__ f32x2_t pk2(float a, float b) { f32x2_t r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
 __device__ __forceinline__ void upk2(f32x2_t r, float &a, float &b) { asm("mov.b64 {%0,%1}, %2;" : "=f"(a), "=f"(b) : "l"(r)); }
@@ -60,9 +54,7 @@ __device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t,
     const unsigned w0 = (unsigned)__cvta_generic_to_shared(list_s + col);
     unsigned wp = w0;
     const unsigned wend = w0 + (LIST_CAP - 1) * STRIDE;
-#if TB_PACKED
     const f32x2_t npi_xy = pk2(-pi.x, -pi.y);
-#endif
 #pragma unroll 1
     for (int dz = -1; dz <= 1; ++dz) {
 #pragma unroll 1
@@ -79,7 +71,6 @@ __device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t,
 #pragma unroll 4
                 for (int lj = lo; lj < h2; ++lj) {
                     const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj);
-#if TB_PACKED
                     // (dx, dy) and their squares as one packed pair each: 5 issue slots instead of 6 per candidate (the
                     // rounding differs from the exact pass by an ulp: far inside the 1e-5 band of this prefilter)
                     const f32x2_t dxy = add2(pk2(pj.x, pj.y), npi_xy);
@@ -87,10 +78,6 @@ __device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t,
                     upk2(mul2(dxy, dxy), sx, sy);
                     const float dz2 = pj.z - pi.z;
                     const float r2 = fmaf(dz2, dz2, sx + sy);
-#else
-                    const float dx = pj.x - pi.x, dy2 = pj.y - pi.y, dz2 = pj.z - pi.z;
-                    const float r2 = dx * dx + dy2 * dy2 + dz2 * dz2;
-#endif
                     asm volatile("st.shared.u16 [%0], %1;" ::"r"(wp), "h"((unsigned short)lj));
                     // keep the slot iff the candidate passes: one predicated add (the compiler's select form costs 3)
                     asm volatile("{ .reg .pred p; setp.lt.f32 p, %1, %2; @p add.u32 %0, %0, %3; }"
@@ -126,11 +113,9 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
     float A[13];
 #pragma unroll
     for (int k = 0; k < 13; ++k) A[k] = 0.f;
-#if TB_PACKED
     f32x2_t AP[6];                                        // (A[2m-1], A[2m]), m = 1..6: one FFMA2 per m and neighbour
 #pragma unroll
     for (int k = 0; k < 6; ++k) AP[k] = 0ull;
-#endif
     int n = 0;
     for (int k = 0; k < cnt; ++k) {
         const int lj = myl[k * TILE_THREADS];
@@ -173,21 +158,14 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
                 Y6<float> y;
                 y6_eval<float>(dx * rinv, dy * rinv, dz * rinv, y);
                 A[0] += y.E[0];
-#if TB_PACKED
 #pragma unroll
                 for (int m = 1; m <= 6; ++m) AP[m - 1] = fma2(pk2(y.c[m], y.s[m]), pk2(y.E[m], y.E[m]), AP[m - 1]);
-#else
-#pragma unroll
-                for (int m = 1; m <= 6; ++m) { A[2 * m - 1] += y.E[m] * y.c[m]; A[2 * m] += y.E[m] * y.s[m]; }
-#endif
             }
         }
         ++n;
     }
-#if TB_PACKED
 #pragma unroll
     for (int m = 1; m <= 6; ++m) upk2(AP[m - 1], A[2 * m - 1], A[2 * m]);
-#endif
     if (n > maxn) { atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW); n = maxn; }
     if (MODE != 2 || nl) nl_count[s] = n;
     float q6 = 0.f;
@@ -242,10 +220,7 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
 }
 
 template <int MODE>   // 0: list only, 1: + Q6 pass 1, 2: + coordination sum (ungrouped COORD, q_thresh = 1 / r0)
-#ifndef TB_MINB
-#define TB_MINB 5
-#endif
-__global__ void __launch_bounds__(TILE_THREADS, TB_MINB)
+__global__ void __launch_bounds__(TILE_THREADS, 5)
 k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict__ scell,
              const int *__restrict__ cell_start, BoxD bd, float rc2f, double rc2, int maxn,
              int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
@@ -260,11 +235,9 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
     float4 *pos_s = dyn_smem;
     nl16_t *list_s = reinterpret_cast<nl16_t *>(dyn_smem + g.cap);
     tile_setup(g, cell_start, t, *reinterpret_cast<TileScratch *>(dyn_smem));   // scratch = the (still unused) staging area
-#if TB_TMA
     __shared__ unsigned long long stage_bar;
     if (t.staged && !t.any_wrapped && t.total > 0) tile_stage_pos_tma(t, spos, pos_s, &stage_bar);   // block-uniform choice
     else
-#endif
     tile_stage_pos(g, t, spos, pos_s);
     __syncthreads();
     double v[2] = { 0.0, 0.0 };
@@ -324,12 +297,11 @@ static size_t smem_build(const TileGeom &g) {
 }
 
 int tiled_init() {
-    static bool done = false;
-    if (done) return METAD_OK;
+    // per (device, function) attribute: set on every metad_create — no process-wide "done" flag, so contexts created from
+    // several threads or on several devices need no synchronisation
     CUDA_TRY(cudaFuncSetAttribute(k_tile_build<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
     CUDA_TRY(cudaFuncSetAttribute(k_tile_build<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
     CUDA_TRY(cudaFuncSetAttribute(k_tile_build<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-    done = true;
     return METAD_OK;
 }
 

@@ -42,7 +42,7 @@ class Params(ctypes.Structure):
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
            "metad_apply_forces", "metad_deposit", "metad_run", "metad_step_host", "metad_host_alloc", "metad_host_free", "metad_status",
            "metad_get_state", "metad_get_neighbors", "metad_get_q6", "metad_set_hills", "metad_get_hills",
-           "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reweight_recorded", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_version", "metad_last_error"]
+           "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reweight_recorded", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_synchronize", "metad_graph_info", "metad_fma_peak", "metad_version", "metad_last_error"]
 
 _lib = None
 
@@ -84,10 +84,20 @@ def load():
     L.metad_get_timing.argtypes = [_P, _P, _P]
     L.metad_launch_count.argtypes = [_P]
     L.metad_launch_count.restype = ctypes.c_longlong
+    L.metad_synchronize.argtypes = [_P]
+    L.metad_graph_info.argtypes = [_P, _P]
+    L.metad_fma_peak.argtypes = [_I, _P, _P]
     L.metad_version.restype = ctypes.c_char_p
     L.metad_last_error.restype = ctypes.c_char_p
     _lib = L
     return L
+
+
+def fma_peak(kind):
+    """Measured scalar-pipe FMA throughput of the current device in TFLOP/s (metad_fma_peak): kind 'f32', 'f32x2' or 'f64'."""
+    t, ms = ctypes.c_double(0), ctypes.c_double(0)
+    _check(load().metad_fma_peak({"f32": 0, "f32x2": 1, "f64": 2}[kind], ctypes.byref(t), ctypes.byref(ms)))
+    return t.value, ms.value
 
 
 class MetadError(RuntimeError):
@@ -362,3 +372,10 @@ class MetaD:
 
     def launch_count(self):
         return int(load().metad_launch_count(self._h))
+
+    def graph_info(self):
+        """Node counts of the captured step graph (metad_graph_info)."""
+        k = (ctypes.c_int * 8)()
+        _check(load().metad_graph_info(self._h, k))
+        names = ("nodes", "kernel", "memcpy", "memset", "host", "other", "captures", "updates")
+        return dict(zip(names, (int(x) for x in k)))

@@ -3,7 +3,7 @@ oracle on the same seeded workload and return both sides' results."""
 import numpy as np
 
 from oracle.reference import OracleMetaD
-from paper_2510_06873_b200.inputs import hill_walk, hill_walk_periodic, seeded_heights
+from paper_2510_06873_b200.inputs import hill_walk, hill_walk_periodic, seeded_heights  # noqa: F401
 
 TOL_CV = 1e-6       # BASELINE.json north_star: "CV, V and dV/ds within 1e-6 relative"
 TOL_F = 1e-5        # "per-atom bias forces within 1e-5 * max|F| absolute"
@@ -99,3 +99,115 @@ def assert_stagewise(r, tol_cv=TOL_CV, tol_f=TOL_F):
     assert rel(r["dV"], r["dV_ref"]) <= tol_cv, (r["dV"], r["dV_ref"])
     fmax = np.abs(r["F_ref"]).max()
     assert np.abs(r["F"] - r["F_ref"]).max() <= tol_f * fmax, (np.abs(r["F"] - r["F_ref"]).max(), fmax)
+
+
+def force_bound(F_ref, dV_gpu, dV_ref, grads, tol_f=TOL_F):
+    """End-to-end bound on |F_gpu - F_ref| when the two sides used their OWN dV/ds (reading S):
+    F = -sum_d dV/ds_d * ds_d/dr, so a difference delta(dV/ds_d) between the two chains moves every force component by at
+    most |delta(dV/ds_d)| * max|ds_d/dr|; on top of that the stage tolerance 1e-5 * max|F|."""
+    dd = np.abs(np.atleast_1d(dV_gpu) - np.atleast_1d(dV_ref))
+    gmax = np.array([np.abs(g).max() for g in grads])
+    return tol_f * np.abs(F_ref).max() + float(np.sum(dd * gmax))
+
+
+def chained_run(w, precision=None, nsteps=7, grid=None, lazy=False, hills=None, host=False, n_init_hills=40,
+                pos_of_step=None, box_of_step=None, seed=5):
+    """The library's RUN paths (metad_run = CUDA-graph replay, or metad_step_host with host=True) one step at a time, every
+    step checked stage-wise against the oracle fed with the CUDA path's OWN upstream values (reading S, no slack factor):
+
+        s_gpu            vs  oracle CV of the same positions                              1e-6 relative
+        V_gpu, dVds_gpu  vs  oracle bias of (the hills the library held BEFORE the step) at s_gpu    1e-6
+        F_gpu (one step) vs  oracle forces with dVds_gpu                                  1e-5 max|F|
+        deposited hill   ==  (s_gpu bit for bit, w0 exp(-V_gpu / ((gamma - 1) kT)) to 1e-12), earlier hills untouched
+
+    and, beside it, a FREE-RUNNING oracle loop (its own hills): CV 1e-6, hill count, and the accumulated forces within the
+    derived bound sum_steps force_bound().  Returns a dict (md, per-step states, launches per step)."""
+    import oracle as orc
+    import torch
+    from paper_2510_06873_b200.metad import MetaD, pinned_array
+    precision = w.precision if precision is None else precision
+    tdt = torch.float32 if precision == 32 else torch.float64
+    pos = positions_for(w, precision)
+    o, of = OracleMetaD(w), OracleMetaD(w)          # chained (hills reset from the library every step), free-running
+    if hills is None:
+        o.build_neighbors(pos.astype(np.float64))
+        s0 = o.eval_cv(want_grad=False)
+        if getattr(w, "period", None):
+            c0 = hill_walk_periodic(seed, s0, w.sigma, n_init_hills, w.period, w.extra["period_lo"])
+        else:
+            c0 = hill_walk(seed, s0, w.sigma, n_init_hills)
+        hills = (c0, seeded_heights(seed, n_init_hills, w.w0))
+    if grid is not None:
+        o.enable_grid(*grid)
+        of.enable_grid(*grid)
+    of.set_hills(*hills)
+    md = MetaD(w, precision=precision, max_hills=len(hills[1]) + nsteps + 8, grid=grid, lazy_neighbors=lazy)
+    md.set_hills(*hills)
+    with torch.cuda.stream(md.stream):
+        dpos = torch.tensor(pos, device="cuda", dtype=tdt)
+        F = torch.zeros((w.natoms, 3), device="cuda", dtype=tdt)
+    md.synchronize()
+    if host:
+        pos_h = pinned_array(pos.shape, pos.dtype)
+        F_h = pinned_array((w.natoms, 3), pos.dtype)
+    F_acc, Fo_acc, bound_acc = np.zeros((w.natoms, 3)), np.zeros((w.natoms, 3)), 0.0
+    states, per_step_launches = [], None
+    box0 = np.array(w.box, dtype=np.float64)
+    for k in range(nsteps):
+        box = box0 if box_of_step is None else np.asarray(box_of_step(k), dtype=np.float64)
+        p = pos if pos_of_step is None else np.ascontiguousarray(pos_of_step(k).astype(pos.dtype))
+        p64 = p.astype(np.float64)
+        o.w.box = box                                # o.w is of.w is w: the oracle reads the box from the workload
+        hc, hh = md.get_hills()
+        l0 = md.launch_count()
+        if host:
+            pos_h[...] = p
+            F_h[...] = 0
+            cv_h, V_h = md.step_host(pos_h, F_h, box=box)
+            Fg = np.array(F_h, dtype=np.float64)
+        else:
+            with torch.cuda.stream(md.stream):
+                dpos.copy_(torch.from_numpy(p))
+                F.zero_()
+            md.synchronize()
+            md.run(dpos, F, 1, box=box)
+            md.synchronize()
+            Fg = F.cpu().numpy().astype(np.float64)
+        per_step_launches = md.launch_count() - l0
+        st = md.state()
+        if host:
+            assert np.array_equal(cv_h, st["cv"]) and V_h == st["V"]
+        ac, ah = md.get_hills()
+        # ---- stage-wise, chained on the library's own values
+        o.set_hills(hc, hh)
+        o.build_neighbors(p64)
+        s_ref = o.eval_cv()
+        assert rel(st["cv"], s_ref) <= TOL_CV, (k, st["cv"], s_ref)
+        V_ref, dV_ref = o.bias(st["cv"])
+        assert abs(st["V"] - V_ref) <= TOL_CV * max(abs(V_ref), TINY), (k, st["V"], V_ref)
+        assert np.abs(st["dVds"] - dV_ref).max() <= TOL_CV * max(np.abs(dV_ref).max(), TINY), (k, st["dVds"], dV_ref)
+        F_ref = o.forces(st["dVds"])
+        ulp = 2.0 ** -24 * np.abs(F_ref).max() if precision == 32 else 0.0
+        assert np.abs(Fg - F_ref).max() <= TOL_F * np.abs(F_ref).max() + ulp, (k, np.abs(Fg - F_ref).max(), np.abs(F_ref).max())
+        due = w.stride > 0 and (k + 1) % w.stride == 0
+        assert st["step"] == k + 1 and len(ah) == len(hh) + int(due) == st["nhills"]
+        assert np.array_equal(ac[:len(hh)], hc) and np.array_equal(ah[:len(hh)], hh)
+        if due:
+            assert np.array_equal(ac[-1], st["cv"])
+            h_ref = orc.wt_height(w.w0, st["V"], w.kT, w.bias_factor)
+            assert abs(ah[-1] - h_ref) <= 1e-12 * h_ref, (k, ah[-1], h_ref)
+        # ---- free-running oracle loop beside it
+        Fo = np.zeros((w.natoms, 3))
+        s_f, V_f, dV_f = of.run_step(p64, Fo)
+        assert rel(st["cv"], s_f) <= TOL_CV
+        bound_acc += force_bound(Fo, st["dVds"], dV_f, of.grads)
+        F_acc += Fg
+        Fo_acc += Fo
+        states.append(dict(st, s_ref=s_ref, V_ref=V_ref, dV_ref=dV_ref, V_free=V_f, dV_free=dV_f))
+    assert md.status() == 0, md.status()
+    assert len(of.heights) == states[-1]["nhills"]
+    assert rel(md.get_hills()[0], of.centers) <= TOL_CV
+    assert np.abs(F_acc - Fo_acc).max() <= bound_acc, (np.abs(F_acc - Fo_acc).max(), bound_acc)
+    o.w.box = box0
+    return dict(md=md, states=states, launches_per_step=per_step_launches, F=F_acc, F_free=Fo_acc, oracle=of, dpos=dpos,
+                hills0=hills)

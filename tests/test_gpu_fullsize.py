@@ -40,6 +40,59 @@ def test_config4_full_size():
     assert np.abs(r["q6"] - r["q6_ref"]).max() <= 2e-6
 
 
+def test_config4_grid_leg_full_size():
+    """BASELINE.json configs[4]: "100,000 hills, also evaluated through a 512x512 grid-tabulated bias with bicubic
+    interpolation" at ITS size (readings K, M): the separable 16 x 16-node tile build over 100,000 hills against the oracle's
+    direct node sums (2.6e10 Gaussian terms on the host cores), 20 lookups, one deposit into the table.  The atoms play no
+    part in this leg, so the context sits on the small c4 structure; hill centres walk around the full-size structure's own CV
+    values (Q6 = 0.2315, solid-like count = 4.7e5)."""
+    import oracle as orc
+    import torch
+    from paper_2510_06873_b200.inputs import hill_walk, seeded_heights
+    from paper_2510_06873_b200.metad import MetaD
+    from gpu_util import TOL_CV, rel
+    w = configs.small("c4")
+    w.sigma = [0.005, 500.0]
+    w.stride = 1
+    n, sig = 100000, np.array([0.005, 500.0])
+    s0 = np.array([0.2315, 4.7e5])
+    centers, heights = hill_walk(5, s0, sig, n), seeded_heights(5, n, w.w0)
+    lo, hi = s0 - 120 * sig, s0 + 120 * sig
+    table = np.zeros((4, 512, 512))
+    orc.grid_add(table, lo, hi, centers, heights, sig)
+    md = MetaD(w, precision=32, grid=((512, 512), lo, hi), max_hills=n + 8)
+    md.set_hills(centers, heights)
+    tab = md.grid_table()
+    scale = np.abs(table).reshape(4, -1).max(1)[:, None, None]
+    assert scale.min() > 0
+    assert (np.abs(tab - table) / scale).max() <= 1e-10
+    rng = np.random.default_rng(1)
+    for k in range(20):
+        s = s0 + (rng.random(2) - 0.5) * 120 * sig
+        out, V_ref, dV_ref = orc.grid_eval(table, lo, hi, s)
+        assert out == 0
+        with torch.cuda.stream(md.stream):
+            ds = torch.tensor(s, device="cuda")
+        V, dV = md.bias(cv=ds)
+        md.synchronize()
+        assert rel(V.cpu().numpy(), V_ref) <= TOL_CV
+        assert np.abs(dV.cpu().numpy() - dV_ref).max() <= TOL_CV * np.abs(dV_ref).max()
+    assert md.status() == 0
+    # one deposition: the new hill (height by the well-tempered rule from the table's V) lands in the table
+    s = s0 + np.array([3.3, -7.1]) * sig
+    out, V0, _ = orc.grid_eval(table, lo, hi, s)
+    h_new = orc.wt_height(w.w0, V0, w.kT, w.bias_factor)
+    orc.grid_add(table, lo, hi, s[None, :], np.array([h_new]), sig)
+    with torch.cuda.stream(md.stream):
+        ds = torch.tensor(s, device="cuda")
+    md.bias(cv=ds)
+    md.deposit(cv=ds)
+    tab2 = md.grid_table()
+    assert (np.abs(tab2 - table) / scale).max() <= 1e-10
+    c, h = md.get_hills()
+    assert len(h) == n + 1 and rel(h[-1], h_new) <= 1e-9
+
+
 def test_gan_cv_set_full_size_fp32_tiled():
     """PAPER.md:51 CV set (coordination number + a, b, c) at 1,024,000 atoms in the configuration bench.py --config g0
     times: fp32 pair math on the tiled path (coordination sum fused into the list build)."""

@@ -7,7 +7,7 @@ pytestmark = pytest.mark.gpu
 
 from paper_2510_06873_b200.inputs import CV_COORD, CV_LATTICE, CVSpec, configs  # noqa: E402
 
-from gpu_util import TOL_CV, TOL_F, assert_stagewise, rel, stagewise  # noqa: E402
+from gpu_util import TOL_CV, TOL_F, assert_stagewise, chained_run, rel, stagewise  # noqa: E402
 
 
 def _workload():
@@ -143,30 +143,17 @@ def test_lattice_only_context_and_bad_axis():
 
 def test_changing_box_every_step_updates_the_graph():
     """NPT-like loop: positions and box are rescaled every step; metad_run must follow the new box (kernel
-    arguments, cell grid and tile counts change, the captured graph is updated in place) and match the oracle loop."""
-    import copy
-    import torch
-    from oracle.reference import OracleMetaD
-    from paper_2510_06873_b200.metad import MetaD
+    arguments, cell grid and tile counts change) and match the oracle loop step by step (gpu_util.chained_run)."""
     w = _workload()
     w.stride = 2
-    wo = copy.copy(w)
-    o = OracleMetaD(wo)
-    md = MetaD(w, max_hills=64)
-    F = torch.zeros((w.natoms, 3), device="cuda", dtype=torch.float64)
-    Fo = np.zeros((w.natoms, 3))
     frac = np.linalg.solve(w.box.reshape(3, 3).T, w.pos.T).T
-    for k, scale in enumerate([1.0, 1.004, 0.97, 1.08, 1.0801, 0.9]):      # 0.97 / 1.08 / 0.9 change the cell counts
-        box = w.box * scale
-        pos = frac @ box.reshape(3, 3)
-        wo.box = box
-        s_ref, V_ref, dV_ref = o.run_step(pos, Fo)
-        dpos = torch.tensor(pos, device="cuda")
-        torch.cuda.synchronize()
-        md.run(dpos, F, 1, box=box)
-        st = md.state()
-        assert rel(st["cv"], s_ref) <= TOL_CV, (k, st["cv"], s_ref)
-        assert rel(st["V"], V_ref) <= 1e-5 or abs(st["V"] - V_ref) < 1e-12
-    assert md.status() == 0
-    assert st["nhills"] == len(o.heights) == 3
-    assert np.abs(F.cpu().numpy() - Fo).max() <= 10 * TOL_F * np.abs(Fo).max()
+    box0 = w.box.copy()
+    scales = [1.0, 1.004, 0.97, 1.08, 1.0801, 0.9]      # 0.97 / 1.08 / 0.9 change the cell counts
+    # hills that cover the whole excursion of the lattice parameters (widths 0.1 A): a few wide-spread seeded centres
+    s0 = np.array([5.4, *np.linalg.norm(box0.reshape(3, 3), axis=1)])
+    rng = np.random.default_rng(8)
+    centers = s0 * (1.0 + 0.1 * (rng.random((30, 4)) - 0.5))
+    r = chained_run(w, nsteps=len(scales), hills=(centers, np.full(30, 1.0)),
+                    box_of_step=lambda k: box0 * scales[k], pos_of_step=lambda k: frac @ (box0 * scales[k]).reshape(3, 3))
+    assert r["states"][-1]["nhills"] == 30 + 3
+    assert np.array_equal(w.box, box0)

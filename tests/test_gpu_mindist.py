@@ -54,38 +54,17 @@ def test_nobody_within_rc_gives_rc_and_no_force():
 
 @pytest.mark.parametrize("precision", [64, 32])
 def test_list_free_variant_matches_the_list_based_one_and_the_oracle(precision):
-    """lazy_neighbors + a single centre: no neighbour list is built, group B is scanned directly (k_mindist_brute)."""
-    import torch
+    """lazy_neighbors + a single centre: no neighbour list is built, group B is scanned directly (k_mindist_brute).  Both
+    variants step by step against the oracle loop (gpu_util.chained_run)."""
+    from gpu_util import chained_run, positions_for, rel
     from oracle.reference import OracleMetaD
-    from paper_2510_06873_b200.metad import MetaD
-    from gpu_util import TOL_CV, TOL_F, positions_for, rel
     w = _workload(True)
     w.stride = 2
-    pos = positions_for(w, precision)
     o = OracleMetaD(w)
-    o.build_neighbors(pos.astype(np.float64))
+    o.build_neighbors(positions_for(w, precision).astype(np.float64))
     s0 = o.eval_cv(want_grad=False)
-    centers = s0 + np.linspace(0.02, 0.3, 40)[:, None]          # one-sided: a non-zero dV/ds at s0
-    heights = np.full(40, 1.0)
-    o.set_hills(centers, heights)
-    Fo = np.zeros((w.natoms, 3))
-    for _ in range(5):
-        s_ref, V_ref, dV_ref = o.run_step(pos.astype(np.float64), Fo)
-    outs = []
-    tdt = torch.float32 if precision == 32 else torch.float64
-    for lazy in (False, True):
-        md = MetaD(w, precision=precision, max_hills=64, lazy_neighbors=lazy)
-        md.set_hills(centers, heights)
-        with torch.cuda.stream(md.stream):
-            dpos = torch.tensor(pos, device="cuda")
-            F = torch.zeros((w.natoms, 3), device="cuda", dtype=tdt)
-        md.synchronize()
-        l0 = md.launch_count()
-        md.run(dpos, F, 5)
-        st = md.state()
-        outs.append((st, F.cpu().numpy().astype(np.float64), (md.launch_count() - l0) // 5))
-        assert md.status() == 0
-        assert rel(st["cv"], s_ref) <= TOL_CV and rel(st["V"], V_ref) <= 1e-5
-        assert np.abs(outs[-1][1] - Fo).max() <= 10 * TOL_F * np.abs(Fo).max()
-    assert outs[1][2] == outs[0][2] - 6                      # the six kernels of the list build are gone
-    assert rel(outs[1][0]["cv"], outs[0][0]["cv"]) <= 1e-7
+    hills = (s0 + np.linspace(0.02, 0.3, 40)[:, None], np.full(40, 1.0))     # one-sided: a non-zero dV/ds at s0
+    outs = [chained_run(w, precision=precision, nsteps=5, lazy=lazy, hills=hills) for lazy in (False, True)]
+    assert abs(outs[0]["states"][-1]["dVds"][0]) > 0
+    assert outs[1]["launches_per_step"] == outs[0]["launches_per_step"] - 6      # the six kernels of the list build are gone
+    assert rel(outs[1]["states"][-1]["cv"], outs[0]["states"][-1]["cv"]) <= 1e-7

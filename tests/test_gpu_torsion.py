@@ -7,7 +7,7 @@ pytestmark = pytest.mark.gpu
 
 from paper_2510_06873_b200.inputs import configs, hill_walk_periodic, seeded_heights  # noqa: E402
 
-from gpu_util import TOL_CV, TOL_F, assert_stagewise, make_hills, rel, stagewise  # noqa: E402
+from gpu_util import TOL_CV, TOL_F, assert_stagewise, chained_run, make_hills, rel, stagewise  # noqa: E402
 
 P = 2.0 * np.pi
 LO, HI = np.array([-np.pi, -np.pi]), np.array([np.pi, np.pi])
@@ -109,42 +109,16 @@ def test_periodic_grid_matches_oracle_periodic_grid():
 @pytest.mark.parametrize("fused", [False, True])
 @pytest.mark.parametrize("use_grid", [False, True])
 def test_graph_run_t0_matches_oracle_loop(use_grid, fused):
-    """metad_run (CUDA graph, plain metadynamics W = 1.2 kJ/mol, deposition every 2 steps) against the oracle loop."""
-    import torch
-    from oracle.reference import OracleMetaD
-    from paper_2510_06873_b200.metad import MetaD
+    """metad_run (CUDA graph, plain metadynamics W = 1.2 kJ/mol, deposition every 2 steps) against the oracle loop, step by
+    step (gpu_util.chained_run: stage-wise on the library's own values, and the free-running loop with the derived bound)."""
     w = configs.small("t0")
     w.stride = 2
     nsteps = 9
-    o = OracleMetaD(w)
-    o.build_neighbors(w.pos)
-    s0 = o.eval_cv(want_grad=False)
-    centers = hill_walk_periodic(5, s0, w.sigma, 60, w.period, w.extra["period_lo"])
-    heights = seeded_heights(5, 60, w.w0)
-    if use_grid:
-        o.enable_grid(w.grid_n, LO, HI)
-    o.set_hills(centers, heights)
-    Fo = np.zeros((w.natoms, 3))
-    for _ in range(nsteps):
-        s_ref, V_ref, dV_ref = o.run_step(w.pos, Fo)
-    md = MetaD(w, max_hills=128, grid=(w.grid_n, LO, HI) if use_grid else None, lazy_neighbors=fused)
-    md.set_hills(centers, heights)
-    with torch.cuda.stream(md.stream):
-        dpos = torch.tensor(w.pos, device="cuda")
-        F = torch.zeros((w.natoms, 3), device="cuda", dtype=torch.float64)
-    md.synchronize()
-    l0 = md.launch_count()
-    md.run(dpos, F, nsteps)
-    assert (md.launch_count() - l0 == nsteps * (2 if use_grid else 1)) == fused
-    st = md.state()
-    c, h = md.get_hills()
-    assert md.status() == 0
-    assert st["step"] == nsteps and st["nhills"] == 60 + nsteps // 2 == len(o.heights)
-    assert rel(st["cv"], s_ref) <= TOL_CV
-    assert rel(st["V"], V_ref) <= 10 * TOL_CV
+    r = chained_run(w, nsteps=nsteps, grid=(w.grid_n, LO, HI) if use_grid else None, lazy=fused, n_init_hills=60)
+    assert (r["launches_per_step"] == (2 if use_grid else 1)) == fused
+    c, h = r["md"].get_hills()
+    assert len(h) == 60 + nsteps // 2
     assert np.all(h[60:] == w.w0)                   # plain metadynamics: every deposited hill has height W
-    assert rel(c, o.centers) <= TOL_CV
-    assert np.abs(F.cpu().numpy() - Fo).max() <= 10 * TOL_F * np.abs(Fo).max()
 
 
 def test_create_rejects_bad_torsion_and_period_arguments():

@@ -144,3 +144,36 @@ def test_q6_gradient_fd_and_sum_zero():
         assert g[i, a] == pytest.approx(fd, rel=1e-6, abs=1e-8)
         checked += 1
     assert checked >= 20
+
+
+def test_solid_like_switching_is_the_logistic_of_reading_F(golden):
+    """oracle.reference.logistic (BASELINE.json configs[4]: "switching on per-atom q6, threshold 0.35, width 0.05";
+    SURVEY.md §8(c)-F): f(q0) = 1/2, f(q0 +- w) = 1/(1 + e^-+1), limits 0 and 1, monotone, symmetric about the threshold,
+    f' = df/dq by central differences and f'(q0) = 1/(4 w) — a shifted threshold, another width convention (w vs 2w), a
+    flipped sign or a different sigmoid each fail one of these."""
+    from oracle.reference import logistic
+    q0, w = 0.35, 0.05
+    f, df = logistic(np.array([q0, q0 + w, q0 - w]), q0, w)
+    assert f[0] == golden["solid_half"]
+    assert f[1] == pytest.approx(1.0 / (1.0 + np.exp(-1.0)), abs=1e-15) and f[1] == pytest.approx(golden["solid_plus_w"], abs=1e-12)
+    assert f[2] == pytest.approx(1.0 / (1.0 + np.exp(1.0)), abs=1e-15) and f[2] == pytest.approx(golden["solid_minus_w"], abs=1e-12)
+    assert df[0] == pytest.approx(1.0 / (4.0 * w), rel=1e-15)
+    lim, dlim = logistic(np.array([q0 - 40 * w, q0 + 40 * w, 0.0, 1.0]), q0, w)
+    assert lim[0] < 1e-17 and lim[1] == 1.0 and abs(dlim[0]) < 1e-15 and dlim[1] == 0.0
+    assert lim[2] == pytest.approx(1.0 / (1.0 + np.exp(7.0)), rel=1e-14)          # a liquid-like atom, q6 = 0
+    assert lim[3] == pytest.approx(1.0 / (1.0 + np.exp(-13.0)), rel=1e-14)       # q6 = 1 (one neighbour)
+    q = np.linspace(0.0, 1.0, 2001)
+    fq, dq = logistic(q, q0, w)
+    assert np.all(np.diff(fq) > 0) and np.all(dq > 0)
+    # point symmetry about (q0, 1/2) and the central-difference derivative
+    d = np.linspace(0.0, 0.3, 301)
+    fa, _ = logistic(q0 + d, q0, w)
+    fb, _ = logistic(q0 - d, q0, w)
+    assert np.abs(fa + fb - 1.0).max() < 1e-15
+    h = 1e-6
+    fp, _ = logistic(q + h, q0, w)
+    fm, _ = logistic(q - h, q0, w)
+    assert np.abs((fp - fm) / (2 * h) - dq).max() < 1e-8
+    # other parameters: the width really is the e-folding scale of the odds f/(1-f)
+    f2, _ = logistic(np.array([0.5, 0.6]), 0.5, 0.1)
+    assert f2[0] == 0.5 and f2[1] / (1 - f2[1]) == pytest.approx(np.e, rel=1e-14)
