@@ -384,8 +384,13 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
     const int *in = nl + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
     const int cnt = act ? nl_count[s] : 0;
     float fx = 0.f, fy = 0.f, fz = 0.f;
+    // the list entries are fetched two iterations ahead: an entry load (streamed from DRAM) followed by the dependent record
+    // gather was 40 % of the stall samples of this kernel (profiles/r1w_ncu.md)
+    int e0 = cnt > 0 ? __ldcs(in) : 0, e1 = cnt > 1 ? __ldcs(in + 32) : 0;
     for (int k = 0; k < cnt; ++k) {
-        const int e = __ldcs(in + k * 32);            // streamed once: do not displace positions / records in L2
+        const int e = e0;                              // streamed once: do not displace positions / records in L2
+        e0 = e1;
+        if (k + 2 < cnt) e1 = __ldcs(in + (k + 2) * 32);
         const int j = e & NLG_IDX_MASK, code = (unsigned)e >> 27;
         float4 a4, b4, c4, d4, pj;
         ldg256(rec + (size_t)j * 8, a4, b4);

@@ -63,7 +63,7 @@ struct TileScratch {
     int hrel[TILE_MAXROWS][TILE_TXMAX + 2 * TILE_HXMAX + 1];    // start of the halo cell relative to its segment | piece << 28
 };
 #define TILE_SCRATCH_BYTES sizeof(TileScratch)
-__device__ __forceinline__ int tile_cut(int k, int nc, int nt) { return (int)(((long long)k * nc) / nt); }
+__device__ __forceinline__ int tile_cut(int k, int nc, int nt) { return (int)(((unsigned)k * (unsigned)nc) / (unsigned)nt); }
 
 __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restrict__ cell_start, TileTables &t, TileScratch &w) {
     const int tid = threadIdx.x;
