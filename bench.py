@@ -43,6 +43,9 @@ def parse():
     ap.add_argument("--lazy", action="store_true", help="params.lazy_neighbors: skip the list build when no CV reads it (c1, t0)")
     ap.add_argument("--virial", action="store_true", help="also compute the bias virial every step (NPT; COORD / Q6 / LATTICE CVs)")
     ap.add_argument("--stage-times", action="store_true", default=True)
+    ap.add_argument("--peaks", action="store_true",
+                    help="only measure the scalar-pipe roofline denominators (FP32 / FP32x2 / FP64 FMA microbenchmark, "
+                         "metad_fma_peak) and print them as one JSON line")
     return ap.parse_args()
 
 
@@ -120,9 +123,11 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------ oracle arm
-def oracle_sample(name):
+def oracle_sample(name, full=False):
     """A bounded sample of the workload for the CPU oracle (same recipe, fewer atoms)."""
     from paper_2510_06873_b200.inputs import configs
+    if name == "c3" and full:
+        return configs.config3(), "none: the full BASELINE.json configs[3] workload (1,024,000 atoms, 10,000 hills), one step"
     if name == "c3":
         return configs.config3(cells=(30, 30, 16), sphere_r=18.0, n_hills=10000), "c3 recipe at 30x30x16 cells (57,600 atoms), 10,000 hills"
     if name == "c4":
@@ -250,8 +255,34 @@ def algo_coord_build_flops(nb, cand=94.5):
     return 9.0 * cand + 28.0 * nb
 
 
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # nominal FMA peak from the guide's unit counts and clocks
+FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # nominal FMA peak from the guide's unit counts and clocks
+FP64_NOMINAL_TFLOPS = FP32_NOMINAL_TFLOPS / 2            # B200: one FP64 FMA lane per two FP32 lanes
 ISSUE_PEAK_GINST = 148 * 4 * 1.965                      # warp instructions / ns
+
+
+def algo_q6_force_flops(nb):
+    # per pair: 13 fma for the combined record 26, d and r 9, rsqrt + unit vector 5, Y6m (E polynomials 20, recurrence 30),
+    # gradient (6 x 14 + 8) 92, tangent projection and 1/r 14, sum 3 -> ~199; per atom: own record 13, force update 9
+    return 199.0 * nb + 22.0
+
+
+def algo_grid_build_flops(nodes, hills):
+    # separable tile build (bias.cu: k_grid_accumulate): per node and hill g = ex ey, v += g, v0 += g ga, v1 += g gb,
+    # v01 += (g ga) gb = 9 flop; the 1-D factors (one exp per hill and tile row / column) add 2 x 16 exps per 256 node-hills
+    return 9.0 * nodes * hills
+
+
+def measure_peaks():
+    """Scalar-pipe roofline denominators, measured on this GPU right now."""
+    from paper_2510_06873_b200 import metad
+    out = {}
+    for kind in ("f32", "f32x2", "f64"):
+        tf, ms = metad.fma_peak(kind)
+        out[kind] = {"tflops": tf, "ms": ms}
+    out["nominal"] = {"f32": FP32_NOMINAL_TFLOPS, "f64": FP64_NOMINAL_TFLOPS}
+    out["how"] = ("metad_fma_peak: 8 dependent-free FMA chains per thread, 2,048 threads per SM on every SM, CUDA events, best of 4 "
+                  "launches after 2 warm-up launches")
+    return out
 
 
 def run_ours(args):
@@ -383,6 +414,10 @@ def run_ours(args):
     if os.path.exists(pk):
         peaks = json.load(open(pk))
     hbm_peak, peak_src = (peaks["hbm_gbs"], "measured (MEASURED_PEAKS.json hbm_gbs)") if "hbm_gbs" in peaks else (6650.0, "fallback (B200_PROFILING.md)")
+    fpk = measure_peaks()
+    f32_peak, f64_peak = fpk["f32"]["tflops"], fpk["f64"]["tflops"]
+    f32_src = f"measured: metad_fma_peak FP32 FFMA {f32_peak:.1f} TFLOP/s (nominal 148 x 128 x 2 x 1.965 GHz = {FP32_NOMINAL_TFLOPS:.1f})"
+    f64_src = f"measured: metad_fma_peak FP64 DFMA {f64_peak:.1f} TFLOP/s (nominal {FP64_NOMINAL_TFLOPS:.1f})"
     roof, roof_all = None, []
     traffic = {}
     tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
@@ -400,14 +435,27 @@ def run_ours(args):
                    "algorithmic_bytes_per_launch": bytes_launch, "kernel_ms": float(stage_ms[3]), "mean_neighbours": nb}
         roof_all.append(r_force)
         roof = r_force
+        # the same kernel against the scalar pipe it computes on (north_star: "FP32/FP64 pipe utilisation for the Q6 ... passes")
+        ffl = algo_q6_force_flops(nb) * w.natoms
+        pk_, src_ = (f32_peak, f32_src) if precision == 32 else (f64_peak, f64_src)
+        roof_all.append({"kernel": f"{kname} (stage apply_forces), scalar-pipe view", "bound": "alu",
+                         "achieved": ffl / (stage_ms[3] * 1e-3) / 1e12, "peak": pk_, "unit": "TFLOP/s",
+                         "frac": ffl / (stage_ms[3] * 1e-3) / 1e12 / pk_, "traffic": traffic.get("force_dram_bytes"),
+                         "peak_source": src_, "algorithmic_flops_per_launch": ffl, "kernel_ms": float(stage_ms[3])})
+        if precision == 64:
+            # generic fp64 path: list build and Q6 pass 1 are separate kernels (stage times), both on the FP64 pipe
+            p1 = (85.0 * nb) * w.natoms
+            roof_all.append({"kernel": "k_q6_pass1<double> (stage eval_cv)", "bound": "alu",
+                             "achieved": p1 / (stage_ms[1] * 1e-3) / 1e12, "peak": f64_peak, "unit": "TFLOP/s",
+                             "frac": p1 / (stage_ms[1] * 1e-3) / 1e12 / f64_peak, "traffic": None, "peak_source": f64_src,
+                             "algorithmic_flops_per_launch": p1, "kernel_ms": float(stage_ms[1])})
         if precision == 32 and list_ms is not None:
             # a1+a3: candidate scan fused with Q6 pass 1 — plain FP32 ALU / issue bound (no tensor-core work on this path)
             fl = algo_build_flops(nb) * w.natoms
             ach_tf = fl / (list_ms * 1e-3) / 1e12
             r_build = {"kernel": "k_tile_build<Q6> (list phase of build_neighbors)", "bound": "alu", "achieved": ach_tf,
-                       "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach_tf / FP32_PEAK_TFLOPS,
-                       "traffic": traffic.get("build_dram_bytes"),
-                       "peak_source": "nominal FP32 FMA peak: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md §7)",
+                       "peak": f32_peak, "unit": "TFLOP/s", "frac": ach_tf / f32_peak,
+                       "traffic": traffic.get("build_dram_bytes"), "peak_source": f32_src,
                        "algorithmic_flops_per_launch": fl, "kernel_ms": float(list_ms), "sort_phase_ms": float(sort_ms)}
             roof_all.append(r_build)
             if list_ms > stage_ms[3]:
@@ -422,19 +470,55 @@ def run_ours(args):
         fl = algo_coord_build_flops(nb) * w.natoms
         ach_tf = fl / (list_ms * 1e-3) / 1e12
         roof = {"kernel": "k_tile_build<coordination> (list phase of build_neighbors)", "bound": "alu", "achieved": ach_tf,
-                "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach_tf / FP32_PEAK_TFLOPS,
-                "traffic": traffic.get("build_dram_bytes"),
-                "peak_source": "nominal FP32 FMA peak: 148 SMs x 128 lanes x 2 x 1.965 GHz (DESIGN.md §7)",
+                "peak": f32_peak, "unit": "TFLOP/s", "frac": ach_tf / f32_peak,
+                "traffic": traffic.get("build_dram_bytes"), "peak_source": f32_src,
                 "algorithmic_flops_per_launch": fl, "kernel_ms": float(list_ms), "sort_phase_ms": float(sort_ms),
                 "mean_neighbours": nb}
         roof_all.append(roof)
+    lps = int(launches) // max(args.steps, 1)
+    if roof is None:
+        # c0-c2, t0, r0: a handful of dependent launches of a few microseconds each in one CUDA graph.  The dominant stage is
+        # reported against HBM with its compulsory bytes, and the line says what really bounds it: launch latency.
+        k = int(np.argmax(stage_ms))
+        nbm = 0.0
+        try:
+            cnt, _ = md.neighbors()
+            nbm = float(cnt.mean())
+        except Exception:
+            pass                                        # lazy_neighbors: no list in this context
+        by = w.natoms * ((3 * tb + 2 * 4 * tb + 4 * nbm + 8) if k == 0 else 3 * tb)
+        ach = by / (stage_ms[k] * 1e-3) / 1e9
+        roof = {"kernel": f"stage {stage_names[k]} (generic kernels)", "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s",
+                "frac": ach / hbm_peak, "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": by,
+                "kernel_ms": float(stage_ms[k]), "mean_neighbours": nbm, "launch_bound": True, "launches_per_step": lps,
+                "us_per_launch": 1e3 * ms_max / args.steps / max(lps, 1),
+                "note": "latency-bound: the step is a chain of dependent launches of 2-10 us each; neither HBM nor the ALUs are near a roof"}
+        roof_all.append(roof)
+    if grid is not None:
+        # a5g: time of the table build over all hills (metad_set_hills: separable 16 x 16-node tiles), FP64 pipe
+        g0_, g1_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        md.synchronize()
+        nh_now = md.state()["nhills"]
+        ch, hh = md.get_hills()
+        g0_.record(md.stream)
+        md.set_hills(ch, hh)
+        g1_.record(md.stream)
+        torch.cuda.synchronize()
+        gms = g0_.elapsed_time(g1_)
+        gfl = algo_grid_build_flops(grid[0][0] * grid[0][1], nh_now)
+        roof_all.append({"kernel": "k_grid_accumulate (metad_set_hills: whole-table build, not a per-step kernel)", "bound": "alu",
+                         "achieved": gfl / (gms * 1e-3) / 1e12, "peak": f64_peak, "unit": "TFLOP/s",
+                         "frac": gfl / (gms * 1e-3) / 1e12 / f64_peak, "traffic": None, "peak_source": f64_src,
+                         "algorithmic_flops_per_launch": gfl, "kernel_ms": float(gms), "hills": int(nh_now),
+                         "nodes": [int(grid[0][0]), int(grid[0][1])],
+                         "gaussian_terms_per_s": grid[0][0] * grid[0][1] * nh_now / (gms * 1e-3)})
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if precision == 32 else "f64", "data": "synthetic", "config": describe(w, precision),
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(pos_h.nbytes + F_h.nbytes),
                     "d2h_bytes_per_step": int(F_h.nbytes + 8 * (w.ncv + 1)), "ms_per_step": e2e_ms_max / ke},
-            "roofline": roof, "roofline_kernels": roof_all,
+            "roofline": roof, "roofline_kernels": roof_all, "peaks": fpk, "graph": md.graph_info(),
             "stages_ms": {n: float(v) for n, v in zip(stage_names, stage_ms)},
             "state": {"cv": [float(x) for x in state["cv"]], "V": float(state["V"]), "nhills": state["nhills"],
                       "sticky": status}}
@@ -459,8 +543,8 @@ def run_ours(args):
                             "gaussian_evals_per_s": T * nh / (rms * 1e-3), "dtype": "f64",
                             "fes_span_kT": float((Fm[np.isfinite(Fm)].max() - Fm.min()) / w.kT)}
     if not args.no_cpu_baseline and world == 1:
-        ws, desc = oracle_sample(args.config)
-        times, cores = oracle_time_steps(ws, 2)
+        ws, desc = oracle_sample(args.config, full=True)
+        times, cores = oracle_time_steps(ws, 1 if ws.natoms > 500000 else 2)
         line["cpu_baseline"] = {"value": ws.natoms / times[-1], "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": desc, "s_per_step": times[-1]}
     else:
@@ -470,8 +554,23 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_peaks(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --peaks needs a CUDA device")
+    sampler = ClockSampler(0)
+    sampler.start()
+    pk = measure_peaks()
+    for _ in range(3):                        # keep the SMs busy long enough for a few clock samples
+        measure_peaks()
+    print(json.dumps({"peaks": pk, "clocks": sampler.stop(), "gpu": torch.cuda.get_device_name(0)}), flush=True)
+
+
 def main():
     args = parse()
+    if args.peaks:
+        run_peaks(args)
+        return
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -43,7 +43,11 @@ enum metad_error { METAD_OK = 0, METAD_ERR_ARG = 1, METAD_ERR_BOX = 2, METAD_ERR
 enum metad_dev_bits { METAD_DEV_NEIGH_OVERFLOW = 1, METAD_DEV_HILL_OVERFLOW = 2,
                       METAD_DEV_GRID_RANGE = 4, METAD_DEV_NONFINITE = 8,
                       METAD_DEV_POS_RANGE = 16 /* a position lies outside the primary cell */,
-                      METAD_DEV_TRAJ_FULL = 32 /* the recorded CV trajectory is full, later frames are dropped */ };
+                      METAD_DEV_TRAJ_FULL = 32 /* the recorded CV trajectory is full, later frames are dropped */,
+                      METAD_DEV_BOX = 64 /* device-resident box (metad_*_dev calls): not lower-triangular / not positive, rc not
+                                            below half of every perpendicular width, or the box shrank so far that a cell of the
+                                            frozen cell grid is narrower than rc — neighbour sets of that step are not valid;
+                                            call metad_reset_box and repeat the step */ };
 
 enum metad_cv_kind {
     METAD_CV_COORD = 0,    /* s = scale * sum_{i in A} sum_{j in B, j!=i, r<rc} sw(r_ij/r0),
@@ -115,6 +119,9 @@ typedef struct {
                                        returns METAD_ERR_STATE in both cases.  0 (default): always built */
     int want_virial;                /* != 0: metad_apply_forces also computes the bias virial (metad_get_virial) for NPT runs
                                        (reading AD), for every CV kind */
+    double box_slack;               /* metad_*_dev calls: the cell grid is derived ONCE (first call / after metad_reset_box) with
+                                       cells at least rc (1 + box_slack) wide, so the device-resident box may shrink by that
+                                       fraction before METAD_DEV_BOX is raised; 0 = cells as small as rc allows */
 } metad_params;
 
 /* Creates a context on the current CUDA device; `cuda_stream` is the cudaStream_t on which every later call is enqueued.
@@ -156,6 +163,18 @@ int metad_deposit(metad_ctx *ctx, const double *d_cv, const double *d_V);
  * positions are an input of this library, the MD integrator is out of scope).  Results of the last
  * step are in the context (metad_get_state). */
 int metad_run(metad_ctx *ctx, const void *d_pos, const double *h_box, double rc, void *d_F, int nsteps);
+
+/* NEXT-3 ("ran NPT simulation at 300K and 50 GPa" with lattice parameters as CVs; PAPER.md:61 on the cost of
+ * GPU-CPU transfers) — the box lives in DEVICE memory (d_box: double[9], same convention as h_box) and may change every step
+ * without the host ever seeing it: a kernel derives the step's geometry from it, every other kernel reads that.  The cell
+ * grid and tiling are derived from the box ONCE ([sync]: one 72-byte read on the first call, or the first call after
+ * metad_reset_box) and then frozen, so metad_run_dev captures its CUDA graph once and replays it for every later box; a box
+ * that has become invalid for the frozen grid raises the sticky bit METAD_DEV_BOX instead of an error code.  The two calls
+ * otherwise behave like metad_build_neighbors / metad_run; stage calls that follow metad_build_neighbors_dev use its box. */
+int metad_build_neighbors_dev(metad_ctx *ctx, const void *d_pos, const double *d_box, double rc);
+int metad_run_dev(metad_ctx *ctx, const void *d_pos, const double *d_box, double rc, void *d_F, int nsteps);
+/* Forget the frozen cell grid (and the captured graph): the next *_dev call derives it again from the then current box. */
+int metad_reset_box(metad_ctx *ctx);
 
 /* One step with HOST buffers (end-to-end path): copies h_pos -> device, h_F -> device, runs the
  * five stages, copies F, cv[ncv] and V back.  [sync] */

@@ -252,6 +252,8 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
     CUDA_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
     CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
     CUDA_TRY(dev_alloc(&c->d_hill_stage, (size_t)(c->D + 1) * p->max_hills));
+    CUDA_TRY(dev_alloc(&c->d_geom, 1));
+    if (!(p->box_slack >= 0.0) || p->box_slack > 1.0) FAIL(METAD_ERR_ARG, "box_slack must be in [0, 1]");
     CUDA_TRY(cudaDeviceSynchronize());
     return METAD_OK;
 }
@@ -267,7 +269,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage, c->d_geom };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
@@ -281,7 +283,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
 }
 
 // host-side geometry: box checks (reading O) and the cell grid
-static int setup_geometry(metad_ctx *c, const double *box, double rc) {
+static int setup_geometry(metad_ctx *c, const double *box, double rc, double slack = 0.0) {
     if (!box) FAIL(METAD_ERR_ARG, "null box");
     if (box[1] != 0.0 || box[2] != 0.0 || box[5] != 0.0) FAIL(METAD_ERR_BOX, "box must be lower-triangular (rows a,b,c)");
     if (!(box[0] > 0.0) || !(box[4] > 0.0) || !(box[8] > 0.0)) FAIL(METAD_ERR_BOX, "box diagonal must be positive");
@@ -302,7 +304,7 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc) {
     for (;;) {
         long long tot = 1;
         for (int d = 0; d < 3; ++d) {
-            int n = (int)floor(w[d] / (rc * 1.000001 * shrink));
+            int n = (int)floor(w[d] / (rc * 1.000001 * (1.0 + slack) * shrink));
             g.nc[d] = n < 1 ? 1 : n;
             tot *= g.nc[d];
         }
@@ -363,9 +365,45 @@ TileGeom tile_geom(const metad_ctx *c) {
     return t;
 }
 
+static int build_neighbors_impl(metad_ctx *c, const void *d_pos, const double *h_box, double rc);
+
 extern "C" int metad_build_neighbors(metad_ctx *c, const void *d_pos, const double *h_box, double rc) {
     if (!c || !d_pos) FAIL(METAD_ERR_ARG, "null argument");
-    int r = setup_geometry(c, h_box, rc);
+    c->dg = nullptr;                               // host box: geometry travels in the kernel arguments
+    return build_neighbors_impl(c, d_pos, h_box, rc);
+}
+
+// device box: derive the cell grid once from the box as it is now (the only host read), then freeze it
+static int dev_geometry(metad_ctx *c, const double *d_box, double rc) {
+    if (!c->dev_geom_ready || c->rc != rc) {
+        double hb[9];
+        CUDA_TRY(cudaMemcpyAsync(hb, d_box, sizeof(hb), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(cudaStreamSynchronize(c->stream));
+        int r = setup_geometry(c, hb, rc, c->p.box_slack);
+        if (r) return r;
+        c->dev_geom_ready = 1;
+    }
+    return METAD_OK;
+}
+
+extern "C" int metad_build_neighbors_dev(metad_ctx *c, const void *d_pos, const double *d_box, double rc) {
+    if (!c || !d_pos || !d_box) FAIL(METAD_ERR_ARG, "null argument");
+    int r = dev_geometry(c, d_box, rc);
+    if (r) return r;
+    c->dg = c->d_geom; c->d_box_last = d_box;
+    if ((r = geom_update(c, d_box))) return r;
+    return build_neighbors_impl(c, d_pos, nullptr, rc);
+}
+
+extern "C" int metad_reset_box(metad_ctx *c) {
+    if (!c) FAIL(METAD_ERR_ARG, "null argument");
+    c->dev_geom_ready = 0;
+    if (c->graph_exec && c->graph_devbox) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    return METAD_OK;
+}
+
+static int build_neighbors_impl(metad_ctx *c, const void *d_pos, const double *h_box, double rc) {
+    int r = c->dg ? METAD_OK : setup_geometry(c, h_box, rc);     // device box: geometry frozen by metad_build_neighbors_dev
     if (r) return r;
     c->d_pos_last = d_pos;
     // no CV reads the list; a nearest-distance CV with a few explicit centres is scanned without one (k_mindist_brute)
@@ -422,10 +460,12 @@ static bool fused_torsion_ok(const metad_ctx *c) {
     return c->D <= 2 || !c->grid_on;
 }
 
-static int enqueue_step(metad_ctx *c, const void *d_pos, const double *box, double rc, void *d_F) {
+// d_box != NULL: the step reads its box from device memory (geometry frozen by dev_geometry before the capture)
+static int enqueue_step(metad_ctx *c, const void *d_pos, const double *box, double rc, void *d_F, const double *d_box = nullptr) {
     int r;
     if (fused_torsion_ok(c)) {                    // torsion-only context: the whole step is one kernel (bias.cu)
-        if ((r = setup_geometry(c, box, rc))) return r;
+        if (d_box) { c->dg = c->d_geom; c->d_box_last = d_box; if ((r = geom_update(c, d_box))) return r; }
+        else { c->dg = nullptr; if ((r = setup_geometry(c, box, rc))) return r; }
         c->d_pos_last = d_pos; c->have_neighbors = true; c->list_built = false;
         return bias_fused_torsion_step(c, d_pos, d_F);
     }
@@ -433,7 +473,13 @@ static int enqueue_step(metad_ctx *c, const void *d_pos, const double *box, doub
     // this step use the dV/ds of the hills deposited before it, reading U)
     const bool fuse = !c->grid_on;
     c->cv_direct = c->d_cv;
-    r = metad_build_neighbors(c, d_pos, box, rc);
+    if (d_box) {
+        c->dg = c->d_geom; c->d_box_last = d_box;
+        r = geom_update(c, d_box);
+        if (!r) r = build_neighbors_impl(c, d_pos, nullptr, rc);
+    } else {
+        r = metad_build_neighbors(c, d_pos, box, rc);
+    }
     if (!r) r = metad_eval_cv(c, c->d_cv);
     c->cv_direct = nullptr;
     if (r) return r;
@@ -442,18 +488,31 @@ static int enqueue_step(metad_ctx *c, const void *d_pos, const double *box, doub
     return fuse ? METAD_OK : metad_deposit(c, c->d_cv, c->d_V);
 }
 
+static int run_impl(metad_ctx *c, const void *d_pos, const double *h_box, const double *d_box, double rc, void *d_F, int nsteps);
+
 extern "C" int metad_run(metad_ctx *c, const void *d_pos, const double *h_box, double rc, void *d_F, int nsteps) {
     if (!c || !d_pos || !d_F || !h_box || nsteps < 0) FAIL(METAD_ERR_ARG, "bad argument");
+    return run_impl(c, d_pos, h_box, nullptr, rc, d_F, nsteps);
+}
+
+extern "C" int metad_run_dev(metad_ctx *c, const void *d_pos, const double *d_box, double rc, void *d_F, int nsteps) {
+    if (!c || !d_pos || !d_F || !d_box || nsteps < 0) FAIL(METAD_ERR_ARG, "bad argument");
+    return run_impl(c, d_pos, nullptr, d_box, rc, d_F, nsteps);
+}
+
+static int run_impl(metad_ctx *c, const void *d_pos, const double *h_box, const double *d_box, double rc, void *d_F, int nsteps) {
     bool same = c->graph_exec && c->graph_pos == d_pos && c->graph_F == d_F && c->graph_rc == rc &&
-                memcmp(c->graph_box, h_box, sizeof(double) * 9) == 0;
+                (d_box ? (c->graph_devbox && c->graph_dbox == d_box && c->dev_geom_ready)
+                       : (!c->graph_devbox && memcmp(c->graph_box, h_box, sizeof(double) * 9) == 0));
     if (!same) {
-        int r = setup_geometry(c, h_box, rc);     // argument errors surface before the capture starts
+        // argument errors surface before the capture starts; a device box is read ONCE here to derive the frozen cell grid
+        int r = d_box ? dev_geometry(c, d_box, rc) : setup_geometry(c, h_box, rc);
         if (r) return r;
         long long before = c->launches;
         cudaGraph_t graph;
         CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
         c->capturing = 1;
-        r = enqueue_step(c, d_pos, h_box, rc, d_F);
+        r = enqueue_step(c, d_pos, h_box, rc, d_F, d_box);
         c->capturing = 0;
         cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
         if (r) { if (e == cudaSuccess) cudaGraphDestroy(graph); return r; }
@@ -474,7 +533,8 @@ extern "C" int metad_run(metad_ctx *c, const void *d_pos, const double *h_box, d
         c->launches_per_step = (int)(c->launches - before);
         c->launches = before;                      // capture enqueued nothing
         c->graph_pos = d_pos; c->graph_F = d_F; c->graph_rc = rc;
-        memcpy(c->graph_box, h_box, sizeof(double) * 9);
+        c->graph_devbox = d_box != nullptr; c->graph_dbox = d_box;
+        if (h_box) memcpy(c->graph_box, h_box, sizeof(double) * 9);
     }
     for (int s = 0; s < nsteps; ++s) CUDA_TRY(cudaGraphLaunch(c->graph_exec, c->stream));
     c->launches += (long long)c->launches_per_step * nsteps;

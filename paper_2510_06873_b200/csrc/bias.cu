@@ -266,7 +266,8 @@ k_fused_torsion_step(FusedTors ft, const int *__restrict__ tors_atoms, const T *
                      double *__restrict__ heights, int *__restrict__ nhills, int *__restrict__ step, int *__restrict__ aux,
                      unsigned int *__restrict__ sticky, int stride, double w0, double kT, double gamma, double force_scale,
                      double *__restrict__ cv_out, double *__restrict__ V_out, double *__restrict__ dVds_out,
-                     double *__restrict__ tors_grad, T *__restrict__ F, double *__restrict__ traj, int traj_cap) {
+                     double *__restrict__ tors_grad, T *__restrict__ F, double *__restrict__ traj, int traj_cap, const DevGeom *__restrict__ dg) {
+    if (dg) bd = dg->bd;                          // device-resident box (NPT): metad_*_dev
     __shared__ double s_cv[METAD_MAX_CV], s_g[METAD_MAX_CV][12], s_V, s_dV[METAD_MAX_CV];
     __shared__ int s_exact;
     __shared__ double red[(1 + METAD_MAX_CV) * 32];
@@ -475,11 +476,11 @@ int bias_fused_torsion_step(metad_ctx *c, const void *d_pos, void *d_F) {
     if (c->prec == 32)
         k_fused_torsion_step<float><<<1, 256, 0, c->stream>>>(ft, c->d_tors_atoms, (const float *)d_pos, c->boxd, bp, gp, c->grid_on,
             c->d_table, c->d_centers, c->d_heights, c->d_nhills, c->d_step, ctx_aux(c), c->d_sticky, c->p.stride, c->p.w0, c->p.kT,
-            c->p.bias_factor, c->p.force_scale, c->d_cv, c->d_V, c->d_dVds, c->d_tors_grad, (float *)d_F, c->d_traj, c->p.traj_capacity);
+            c->p.bias_factor, c->p.force_scale, c->d_cv, c->d_V, c->d_dVds, c->d_tors_grad, (float *)d_F, c->d_traj, c->p.traj_capacity, c->dg);
     else
         k_fused_torsion_step<double><<<1, 256, 0, c->stream>>>(ft, c->d_tors_atoms, (const double *)d_pos, c->boxd, bp, gp, c->grid_on,
             c->d_table, c->d_centers, c->d_heights, c->d_nhills, c->d_step, ctx_aux(c), c->d_sticky, c->p.stride, c->p.w0, c->p.kT,
-            c->p.bias_factor, c->p.force_scale, c->d_cv, c->d_V, c->d_dVds, c->d_tors_grad, (double *)d_F, c->d_traj, c->p.traj_capacity);
+            c->p.bias_factor, c->p.force_scale, c->d_cv, c->d_V, c->d_dVds, c->d_tors_grad, (double *)d_F, c->d_traj, c->p.traj_capacity, c->dg);
     c->launches++;
     if (c->grid_on) {
         int nn = c->p.grid_n[0] * c->p.grid_n[1];

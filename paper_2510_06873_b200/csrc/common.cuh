@@ -36,6 +36,22 @@ struct CellGrid {
     double cx, cy, bx;               // tilt terms for cartesian -> fractional
 };
 
+// Device-resident geometry of the current step (metad_build_neighbors_dev / metad_run_dev: the box lives in device memory and
+// may change every step without the host seeing it — NPT).  k_geom_update derives it from the 9 box doubles;
+// every kernel takes a `const DevGeom *dg` that is NULL on the host-box paths (geometry in the kernel arguments, constant bank)
+// and overrides the by-value arguments otherwise.  The cell COUNTS stay those of the capture; the kernel checks that the cells
+// are still at least rc wide and sets METAD_DEV_BOX otherwise.
+struct DevGeom {
+    BoxD bd;
+    PBox<float> pbf;
+    PBox<double> pbd;
+    double inv[6], cx, cy, bx;       // CellGrid: cartesian -> fractional
+    double box[9];
+};
+template <typename T> __device__ __forceinline__ const PBox<T> &dg_pb(const DevGeom *dg);
+template <> __device__ __forceinline__ const PBox<float> &dg_pb<float>(const DevGeom *dg) { return dg->pbf; }
+template <> __device__ __forceinline__ const PBox<double> &dg_pb<double>(const DevGeom *dg) { return dg->pbd; }
+
 template <typename T> struct Vec4;
 template <> struct Vec4<float> { typedef float4 type; };
 template <> struct Vec4<double> { typedef double4 type; };
@@ -224,6 +240,12 @@ struct metad_ctx {
     void *d_pos_stage, *d_F_stage;
     void *h_pin; size_t h_pin_bytes;
     // graph
+    DevGeom *d_geom;                      // device-resident geometry (box in device memory), written by k_geom_update
+    const DevGeom *dg;                    // d_geom while the current step runs on a device box, else NULL
+    const double *d_box_last;             // device box of the last *_dev call
+    int dev_geom_ready;                   // the cell grid / tiling was derived for the device box (frozen until metad_reset_box)
+    int graph_devbox;                     // the captured graph reads the box from device memory
+    const double *graph_dbox;             //   ... from this pointer
     cudaGraphExec_t graph_exec;
     cudaGraph_t graph;                    // the captured step (kept for metad_graph_info)
     int graph_captures, graph_updates;    // how often metad_run captured a step / updated the instantiated graph in place
@@ -256,6 +278,7 @@ static inline int div_up(long long a, int b) { return (int)((a + b - 1) / b); }
 
 // stage entry points implemented in the .cu files (host functions that enqueue kernels)
 int nb_build(metad_ctx *c, const void *d_pos);
+int geom_update(metad_ctx *c, const double *d_box);
 int nb_export(metad_ctx *c, int *d_count, int *d_list);
 int cv_eval_all(metad_ctx *c, double *d_cv);
 int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F);

@@ -16,8 +16,9 @@ __global__ void __launch_bounds__(CV_THREADS)
 k_coord_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
            const int *__restrict__ nl, PBox<T> pb, T inv_r0, int n, int m, double scale,
            double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
-           unsigned int *__restrict__ sticky) {
+           unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
     __shared__ double red[32];
+    if (dg) pb = dg_pb<T>(dg);
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     T acc = T(0);
     if (s < N) {
@@ -56,8 +57,10 @@ template <typename T, bool VIRIAL>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
               const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, T inv_r0, int n, int m,
-              double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F, VirArgs va) {
+              double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F, VirArgs va,
+              const DevGeom *__restrict__ dg) {
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
+    if (dg) pb = dg_pb<T>(dg);
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (!VIRIAL && s >= N) return;
     const bool act = s < N;
@@ -111,8 +114,9 @@ __global__ void __launch_bounds__(CV_THREADS)
 k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
                 const int *__restrict__ nl, PBox<T> pb, T inv_r0, int n, int m, double scale,
                 double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
-                unsigned int *__restrict__ sticky) {
+                unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
     __shared__ double red[32];
+    if (dg) pb = dg_pb<T>(dg);
     const int gt = blockIdx.x * blockDim.x + threadIdx.x;
     const int s = gt / G, lane = gt % G;
     T acc = T(0);
@@ -150,10 +154,12 @@ template <typename T, int G>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_force_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
                    const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, T inv_r0, int n, int m,
-                   double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F) {
+                   double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F,
+                   const DevGeom *__restrict__ dg) {
     const int gt = blockIdx.x * blockDim.x + threadIdx.x;
     const int s = gt / G, lane = gt % G;
     if (s >= N) return;
+    if (dg) pb = dg_pb<T>(dg);
     const unsigned gmask = G == 32 ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
     typename Vec4<T>::type pi = spos[s];
     const int fi = (int)pi.w;
@@ -195,8 +201,9 @@ k_q6_pass1(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
            const int *__restrict__ nl, PBox<T> pb, T q_thresh, T inv_width, T *__restrict__ rec,
            double scale_mean, double scale_solid, int dim_mean, int dim_solid,
            double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
-           unsigned int *__restrict__ sticky) {
+           unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
     __shared__ double red[64];
+    if (dg) pb = dg_pb<T>(dg);
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     double v[2] = { 0.0, 0.0 };
     if (s < N) {
@@ -271,8 +278,9 @@ __global__ void __launch_bounds__(CV_THREADS)
 k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
            const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, const T *__restrict__ rec,
            double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
-           const double *__restrict__ dVds, T *__restrict__ F, VirArgs va) {
+           const double *__restrict__ dVds, T *__restrict__ F, VirArgs va, const DevGeom *__restrict__ dg) {
     typedef typename Vec4<T>::type V4;
+    if (dg) pb = dg_pb<T>(dg);
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (!VIRIAL && s >= N) return;
@@ -352,12 +360,14 @@ __device__ __forceinline__ void ldg256(const float *p, float4 &a, float4 &b) {
 }
 
 #define Q6F_MINB 9             // resident blocks per SM of k_q6_force_g (56 registers)
-template <bool SOLID, bool VIRIAL>
+template <bool SOLID, bool VIRIAL, bool DEVBOX>   // DEVBOX: box in device memory (metad_*_dev); the other instances never touch dg
 __global__ void __launch_bounds__(CV_THREADS, VIRIAL ? 8 : Q6F_MINB)
 k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
              const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, const float *__restrict__ rec,
              double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
-             const double *__restrict__ dVds, float *__restrict__ F, VirArgs va, const float *__restrict__ fprime) {
+             const double *__restrict__ dVds, float *__restrict__ F, VirArgs va, const float *__restrict__ fprime,
+             const DevGeom *__restrict__ dg_arg) {
+    const DevGeom *dg = DEVBOX ? dg_arg : nullptr;
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (!VIRIAL && s >= N) return;
@@ -399,9 +409,10 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         if (code != 13) {
             const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
-            dx = (float)(((double)pj.x - (double)pi.x) + (wx * bd.ax + wy * bd.bx + wz * bd.cx));
-            dy = (float)(((double)pj.y - (double)pi.y) + (wy * bd.by + wz * bd.cy));
-            dz = (float)(((double)pj.z - (double)pi.z) + (wz * bd.cz));
+            const BoxD &b = dg ? dg->bd : bd;                  // device-resident box (NPT): read at the rare point of use
+            dx = (float)(((double)pj.x - (double)pi.x) + (wx * b.ax + wy * b.bx + wz * b.cx));
+            dy = (float)(((double)pj.y - (double)pi.y) + (wy * b.by + wz * b.cy));
+            dz = (float)(((double)pj.z - (double)pi.z) + (wz * b.cz));
         }
         const float gw = SOLID ? alpha + beta * fprime[j] : alpha;   // 4-byte gather from a dense array: few lines per warp
         float bb[13];
@@ -444,7 +455,8 @@ template <bool VIRIAL>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
                 const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, float inv_r0, int n, int m,
-                double coef /* force_scale * scale */, const double *__restrict__ dVds, float *__restrict__ F, VirArgs va) {
+                double coef /* force_scale * scale */, const double *__restrict__ dVds, float *__restrict__ F, VirArgs va,
+                const DevGeom *__restrict__ dg) {
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (!VIRIAL && s >= N) return;
@@ -464,9 +476,10 @@ k_coord_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__r
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         if (code != 13) {
             const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
-            dx = (float)(((double)pj.x - (double)pi.x) + (wx * bd.ax + wy * bd.bx + wz * bd.cx));
-            dy = (float)(((double)pj.y - (double)pi.y) + (wy * bd.by + wz * bd.cy));
-            dz = (float)(((double)pj.z - (double)pi.z) + (wz * bd.cz));
+            const BoxD &b = dg ? dg->bd : bd;
+            dx = (float)(((double)pj.x - (double)pi.x) + (wx * b.ax + wy * b.bx + wz * b.cx));
+            dy = (float)(((double)pj.y - (double)pi.y) + (wy * b.by + wz * b.cy));
+            dz = (float)(((double)pj.z - (double)pi.z) + (wz * b.cz));
         }
         const float r2 = dx * dx + dy * dy + dz * dz, rinv = rsqrtf(r2);
         float dsw;
@@ -545,11 +558,11 @@ int tiled_coord_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     else if (c->p.want_virial)
         k_coord_force_g<true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
             c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (float)(1.0 / d.r0), d.n, d.m,
-            c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F, va);
+            c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F, va, c->dg);
     else
         k_coord_force_g<false><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(
             c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (float)(1.0 / d.r0), d.n, d.m,
-            c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F, va);
+            c->p.force_scale * d.scale, d_dVds + c->coord_dim, (float *)d_F, va, c->dg);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -559,13 +572,18 @@ int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
     double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
     const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
+#define Q6FG_ARGS                                                                                                          \
+    c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm, ss,  \
+        c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va, c->d_q6 + c->N, c->dg
 #define Q6FG_LAUNCH(SOLID, VIR)                                                                                            \
-    k_q6_force_g<SOLID, VIR><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(                                      \
-        c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm, \
-        ss, c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va, c->d_q6 + c->N)
+    do {                                                                                                                   \
+        if (c->dg) k_q6_force_g<SOLID, VIR, true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(Q6FG_ARGS);      \
+        else k_q6_force_g<SOLID, VIR, false><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(Q6FG_ARGS);           \
+    } while (0)
     if (c->q6_solid_dim >= 0) { if (c->p.want_virial) Q6FG_LAUNCH(true, true); else Q6FG_LAUNCH(true, false); }
     else { if (c->p.want_virial) Q6FG_LAUNCH(false, true); else Q6FG_LAUNCH(false, false); }
 #undef Q6FG_LAUNCH
+#undef Q6FG_ARGS
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -605,10 +623,11 @@ k_mindist_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *
              const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, double rc,
              double *__restrict__ part_r2, long long *__restrict__ part_ij, int *__restrict__ part_s /* [2*nblocks] */,
              unsigned int *__restrict__ ticket, double *__restrict__ rec /* [r, dx, dy, dz, (i, j) as two ints] */,
-             double *__restrict__ cv_out) {
+             double *__restrict__ cv_out, const DevGeom *__restrict__ dg) {
     __shared__ double s_r2[32];
     __shared__ long long s_ij[32];
     __shared__ int s_sj[32], s_si[32];
+    if (dg) pb = dg_pb<T>(dg);
     const int s = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double r2 = 1e300; long long ij = 0x7fffffffffffffffll; int sj = -1, si = -1;
     if (s < N) {
@@ -689,9 +708,10 @@ template <typename T>
 __global__ void __launch_bounds__(CV_THREADS)
 k_mindist_brute(int nA, const int *__restrict__ ga, int nB, const int *__restrict__ gb, const T *__restrict__ pos, BoxD bd,
                 double rc, double *__restrict__ part_r2, long long *__restrict__ part_ij, unsigned int *__restrict__ ticket,
-                double *__restrict__ rec, double *__restrict__ cv_out) {
+                double *__restrict__ rec, double *__restrict__ cv_out, const DevGeom *__restrict__ dg) {
     __shared__ double s_r2[32];
     __shared__ long long s_ij[32];
+    if (dg) bd = dg->bd;
     const int t = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double r2 = 1e300; long long ij = 0x7fffffffffffffffll; int u0 = -1, u1 = -1;     // u0/u1 unused payload of min_warp
     const double rc2 = rc * rc;
@@ -752,7 +772,7 @@ static int mindist_eval_t(metad_ctx *c, double *d_cv) {
     long long *pk = reinterpret_cast<long long *>(c->d_partials + c->nblocks_atoms);
     int *ps = reinterpret_cast<int *>(c->d_partials + 2 * (size_t)c->nblocks_atoms);
     k_mindist_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(c->N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, ctx_pbox<T>(c),
-                                                     c->rc, pr, pk, ps, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim);
+                                                     c->rc, pr, pk, ps, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim, c->dg);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -766,10 +786,10 @@ int mindist_eval(metad_ctx *c, double *d_cv) {
         long long *pk = reinterpret_cast<long long *>(c->d_partials + c->nblocks_atoms);
         if (c->prec == 32)
             k_mindist_brute<float><<<nb, CV_THREADS, 0, c->stream>>>(d.n_ga, d.d_ga, d.n_gb, d.d_gb, (const float *)ctx_last_pos(c), c->boxd,
-                                                                     c->rc, pr, pk, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim);
+                                                                     c->rc, pr, pk, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim, c->dg);
         else
             k_mindist_brute<double><<<nb, CV_THREADS, 0, c->stream>>>(d.n_ga, d.d_ga, d.n_gb, d.d_gb, (const double *)ctx_last_pos(c), c->boxd,
-                                                                      c->rc, pr, pk, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim);
+                                                                      c->rc, pr, pk, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim, c->dg);
         c->launches++;
         CUDA_TRY(cudaGetLastError());
         return METAD_OK;
@@ -804,11 +824,11 @@ static int cv_eval_t(metad_ctx *c, double *d_cv) {
         if (N <= METAD_WARP_PER_ATOM_MAX)
             k_coord_cv_warp<T, 32><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
                 N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials_warp,
-                c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky);
+                c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky, c->dg);
         else
         k_coord_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb,
                                                        (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials,
-                                                       c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky);
+                                                       c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky, c->dg);
         c->launches++;
     }
     if (c->has_q6 && c->tiled) {
@@ -822,7 +842,7 @@ static int cv_eval_t(metad_ctx *c, double *d_cv) {
         k_q6_pass1<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, (T)qt,
                                                        (T)(1.0 / qw), (T *)c->d_rec, sm, ss, c->q6_mean_dim,
                                                        c->q6_solid_dim, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
-                                                       d_cv, c->d_sticky);
+                                                       d_cv, c->d_sticky, c->dg);
         c->launches++;
     }
     return METAD_OK;
@@ -860,19 +880,19 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
         if (c->p.want_virial)                                 // forces and virial in one thread-per-atom pass
             k_coord_force<T, true><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
                                                                     pb, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
-                                                                    d_dVds + c->coord_dim, (T *)d_F, va);
+                                                                    d_dVds + c->coord_dim, (T *)d_F, va, c->dg);
         else if (N <= METAD_WARP_PER_ATOM_MAX)
             k_coord_force_warp<T, 32><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
                 N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, (T)(1.0 / d.r0), d.n, d.m,
-                c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F);
+                c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F, c->dg);
         else if (d.use_groups && N <= 8 * METAD_WARP_PER_ATOM_MAX)
             k_coord_force_warp<T, 8><<<div_up((long long)N * 8, CV_THREADS), CV_THREADS, 0, c->stream>>>(
                 N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, (T)(1.0 / d.r0), d.n, d.m,
-                c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F);
+                c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F, c->dg);
         else
             k_coord_force<T, false><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
                                                                      pb, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
-                                                                     d_dVds + c->coord_dim, (T *)d_F, va);
+                                                                     d_dVds + c->coord_dim, (T *)d_F, va, c->dg);
         c->launches++;
     }
     if (c->has_q6 && c->tiled) {
@@ -885,11 +905,11 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
         if (c->p.want_virial)
             k_q6_force<T, true><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb,
                                                                  (const T *)c->d_rec, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
-                                                                 c->p.force_scale, d_dVds, (T *)d_F, va);
+                                                                 c->p.force_scale, d_dVds, (T *)d_F, va, c->dg);
         else
             k_q6_force<T, false><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb,
                                                                   (const T *)c->d_rec, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
-                                                                  c->p.force_scale, d_dVds, (T *)d_F, va);
+                                                                  c->p.force_scale, d_dVds, (T *)d_F, va, c->dg);
         c->launches++;
     }
     return METAD_OK;

@@ -12,7 +12,8 @@ struct RgScratch { double com[3]; double M; double rg; };   // stored after the 
 template <typename T>
 __global__ void __launch_bounds__(RG_THREADS)
 k_rgyr(int nchain, const int *__restrict__ chain, const double *__restrict__ mass, const T *__restrict__ pos,
-       BoxD bd, double *__restrict__ unwrapped, double *__restrict__ cv_out, unsigned int *__restrict__ sticky) {
+       BoxD bd, double *__restrict__ unwrapped, double *__restrict__ cv_out, unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
+    if (dg) bd = dg->bd;                          // device-resident box (NPT): metad_*_dev
     __shared__ double wsum[3][32];
     __shared__ double carry[3];
     __shared__ double red[4 * 32];
@@ -135,7 +136,8 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_contacts_cv(int npairs, const int *__restrict__ pairs, const double *__restrict__ pair_r0, int n, int m,
               double scale, const T *__restrict__ pos, BoxD bd, double *__restrict__ partials,
-              unsigned int *__restrict__ ticket, double *__restrict__ cv_out, unsigned int *__restrict__ sticky) {
+              unsigned int *__restrict__ ticket, double *__restrict__ cv_out, unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
+    if (dg) bd = dg->bd;                          // device-resident box (NPT): metad_*_dev
     __shared__ double red[32];
     int p = blockIdx.x * blockDim.x + threadIdx.x;
     double v[1] = { 0.0 };
@@ -168,7 +170,8 @@ __global__ void k_contacts_force(int natoms_touched, const int *__restrict__ ato
                                  const int *__restrict__ csr_pair, const int *__restrict__ pairs,
                                  const double *__restrict__ pair_r0, int n, int m, double coef /* fs*scale */,
                                  const T *__restrict__ pos, BoxD bd, const double *__restrict__ dVds,
-                                 T *__restrict__ F) {
+                                 T *__restrict__ F, const DevGeom *__restrict__ dg) {
+    if (dg) bd = dg->bd;                          // device-resident box (NPT): metad_*_dev
     const int t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (t >= natoms_touched) return;
     int a = atoms[t];
@@ -205,12 +208,12 @@ static int chain_eval_t(metad_ctx *c, int dim, double *d_cv) {
     const T *pos = (const T *)ctx_last_pos(c);
     if (d.kind == METAD_CV_RGYR) {
         k_rgyr<T><<<1, RG_THREADS, 0, c->stream>>>(d.nchain, d.d_chain, d.d_mass, pos, c->boxd, d.d_unwrapped, d_cv + dim,
-                                                   c->d_sticky);
+                                                   c->d_sticky, c->dg);
     } else {
         int nb = div_up(d.npairs, 256);
         k_contacts_cv<T><<<nb, 256, 0, c->stream>>>(d.npairs, d.d_pairs, d.d_pair_r0, d.n, d.m, d.scale, pos, c->boxd,
                                                     c->d_partials + 3 * (size_t)c->nblocks_atoms, c->d_tickets + 2 + dim,
-                                                    d_cv + dim, c->d_sticky);
+                                                    d_cv + dim, c->d_sticky, c->dg);
     }
     c->launches++;
     return METAD_OK;
@@ -232,7 +235,7 @@ static int chain_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
         } else if (d.kind == METAD_CV_CONTACTS) {
             k_contacts_force<T><<<div_up((long long)d.ncatoms * 32, 128), 128, 0, c->stream>>>(
                 d.ncatoms, d.d_catoms, d.d_csr_off, d.d_csr_pair, d.d_pairs, d.d_pair_r0, d.n, d.m,
-                c->p.force_scale * d.scale, pos, c->boxd, d_dVds + dim, (T *)d_F);
+                c->p.force_scale * d.scale, pos, c->boxd, d_dVds + dim, (T *)d_F, c->dg);
             c->launches++;
         }
     }
@@ -252,7 +255,8 @@ struct TorsTable { int kind[METAD_MAX_CV]; int idx[METAD_MAX_CV][4]; };
 
 template <typename T>
 __global__ void k_torsions_cv(int D, TorsTable tt, const T *__restrict__ pos, BoxD bd, double *__restrict__ grad,
-                              double *__restrict__ cv_out, unsigned int *__restrict__ sticky) {
+                              double *__restrict__ cv_out, unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
+    if (dg) bd = dg->bd;                          // device-resident box (NPT): metad_*_dev
     const int d = threadIdx.x;
     if (d >= D || tt.kind[d] != METAD_CV_TORSION) return;
     double r[4][3], b[3][3];
@@ -300,9 +304,9 @@ static TorsTable tors_table(const metad_ctx *c) {
 int torsion_eval_all(metad_ctx *c, double *d_cv) {
     if (!c->has_torsion) return METAD_OK;
     if (c->prec == 32)
-        k_torsions_cv<float><<<1, 32, 0, c->stream>>>(c->D, tors_table(c), (const float *)ctx_last_pos(c), c->boxd, c->d_tors_grad, d_cv, c->d_sticky);
+        k_torsions_cv<float><<<1, 32, 0, c->stream>>>(c->D, tors_table(c), (const float *)ctx_last_pos(c), c->boxd, c->d_tors_grad, d_cv, c->d_sticky, c->dg);
     else
-        k_torsions_cv<double><<<1, 32, 0, c->stream>>>(c->D, tors_table(c), (const double *)ctx_last_pos(c), c->boxd, c->d_tors_grad, d_cv, c->d_sticky);
+        k_torsions_cv<double><<<1, 32, 0, c->stream>>>(c->D, tors_table(c), (const double *)ctx_last_pos(c), c->boxd, c->d_tors_grad, d_cv, c->d_sticky, c->dg);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -324,7 +328,8 @@ int torsion_forces(metad_ctx *c, const double *d_dVds, void *d_F) {
 // NEXT-3: lattice-parameter CVs (reading AB): s = |h_k|; the bias force acts on the box rows.
 struct LatTable { int kind[METAD_MAX_CV]; int axis[METAD_MAX_CV]; double h[9]; };
 
-__global__ void k_lattice_cv(int D, LatTable lt, double *__restrict__ cv_out) {
+__global__ void k_lattice_cv(int D, LatTable lt, double *__restrict__ cv_out, const DevGeom *__restrict__ dg) {
+    if (dg) { for (int k = 0; k < 9; ++k) lt.h[k] = dg->box[k]; }   // device-resident box
     const int d = threadIdx.x;
     if (d >= D || lt.kind[d] != METAD_CV_LATTICE) return;
     const double *h = lt.h + 3 * lt.axis[d];
@@ -332,7 +337,8 @@ __global__ void k_lattice_cv(int D, LatTable lt, double *__restrict__ cv_out) {
 }
 
 __global__ void k_lattice_force(int D, LatTable lt, double force_scale, const double *__restrict__ dVds,
-                                double *__restrict__ fbox, double *__restrict__ virial /* NULL: not wanted */) {
+                                double *__restrict__ fbox, double *__restrict__ virial /* NULL: not wanted */, const DevGeom *__restrict__ dg) {
+    if (dg) { for (int k = 0; k < 9; ++k) lt.h[k] = dg->box[k]; }   // device-resident box
     const int e = threadIdx.x;              // box element (row, component)
     if (e >= 9) return;
     const int row = e / 3;
@@ -365,7 +371,7 @@ static LatTable lat_table(const metad_ctx *c) {
 
 int lattice_eval(metad_ctx *c, double *d_cv) {
     if (!c->has_lattice) return METAD_OK;
-    k_lattice_cv<<<1, 32, 0, c->stream>>>(c->D, lat_table(c), d_cv);
+    k_lattice_cv<<<1, 32, 0, c->stream>>>(c->D, lat_table(c), d_cv, c->dg);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -374,7 +380,7 @@ int lattice_eval(metad_ctx *c, double *d_cv) {
 int lattice_forces(metad_ctx *c, const double *d_dVds) {
     if (!c->has_lattice) return METAD_OK;
     k_lattice_force<<<1, 32, 0, c->stream>>>(c->D, lat_table(c), c->p.force_scale, d_dVds, c->d_box_force,
-                                            c->p.want_virial ? c->d_virial : nullptr);
+                                            c->p.want_virial ? c->d_virial : nullptr, c->dg);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -411,7 +417,8 @@ template <typename T>
 __global__ void __launch_bounds__(256)
 k_contacts_virial(int npairs, const int *__restrict__ pairs, const double *__restrict__ pair_r0, int n, int m,
                   double coef /* force_scale * scale */, const T *__restrict__ pos, BoxD bd, const double *__restrict__ dVds,
-                  double *__restrict__ virial) {
+                  double *__restrict__ virial, const DevGeom *__restrict__ dg) {
+    if (dg) bd = dg->bd;                          // device-resident box (NPT): metad_*_dev
     __shared__ double red[9 * 32];
     double w[9];
 #pragma unroll
@@ -440,7 +447,8 @@ k_contacts_virial(int npairs, const int *__restrict__ pairs, const double *__res
 // d phi/d eps = sum_k (d phi/d b_k) b_k^T,  d phi/d b1 = -g_i, d phi/d b2 = -(g_i + g_j), d phi/d b3 = g_l
 template <typename T>
 __global__ void k_torsions_virial(int D, TorsTable tt, const T *__restrict__ pos, BoxD bd, const double *__restrict__ grad,
-                                  double force_scale, const double *__restrict__ dVds, double *__restrict__ virial) {
+                                  double force_scale, const double *__restrict__ dVds, double *__restrict__ virial, const DevGeom *__restrict__ dg) {
+    if (dg) bd = dg->bd;                          // device-resident box (NPT): metad_*_dev
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     for (int d = 0; d < D; ++d) {
         if (tt.kind[d] != METAD_CV_TORSION) continue;
@@ -468,13 +476,13 @@ static int chain_virial_t(metad_ctx *c, const double *d_dVds) {
             c->launches++;
         } else if (d.kind == METAD_CV_CONTACTS) {
             k_contacts_virial<T><<<1, 256, 0, c->stream>>>(d.npairs, d.d_pairs, d.d_pair_r0, d.n, d.m, c->p.force_scale * d.scale,
-                                                           pos, c->boxd, d_dVds + dim, c->d_virial);
+                                                           pos, c->boxd, d_dVds + dim, c->d_virial, c->dg);
             c->launches++;
         }
     }
     if (c->has_torsion) {
         k_torsions_virial<T><<<1, 32, 0, c->stream>>>(c->D, tors_table(c), pos, c->boxd, c->d_tors_grad, c->p.force_scale, d_dVds,
-                                                      c->d_virial);
+                                                      c->d_virial, c->dg);
         c->launches++;
     }
     CUDA_TRY(cudaGetLastError());

@@ -16,9 +16,11 @@
 
 template <typename T>
 __global__ void k_bin(int N, const T *__restrict__ pos, CellGrid g, int *__restrict__ cell_of,
-                      int *__restrict__ slot, int *__restrict__ cell_count, unsigned int *__restrict__ sticky) {
+                      int *__restrict__ slot, int *__restrict__ cell_count, unsigned int *__restrict__ sticky,
+                      const DevGeom *__restrict__ dg) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
+    if (dg) { g.inv[0] = dg->inv[0]; g.inv[1] = dg->inv[1]; g.inv[2] = dg->inv[2]; g.cx = dg->cx; g.cy = dg->cy; g.bx = dg->bx; }
     double x = (double)pos[3 * i], y = (double)pos[3 * i + 1], z = (double)pos[3 * i + 2];
     double sc = z * g.inv[2];
     double sb = (y - sc * g.cy) * g.inv[1];
@@ -187,9 +189,11 @@ template <typename T>
 __global__ void __launch_bounds__(128)
 k_build_list(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ scell,
              const int *__restrict__ cell_start, CellGrid g, PBox<T> pb, BoxD bd, T rc2T, double rc2, int maxn,
-             int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky) {
+             int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
+             const DevGeom *__restrict__ dg) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= N) return;
+    if (dg) { pb = dg_pb<T>(dg); bd = dg->bd; }
     typename Vec4<T>::type pi = spos[s];
     int c = scell[s];
     int ia = c % g.nc[0], t = c / g.nc[0];
@@ -238,11 +242,13 @@ template <typename T, int G>
 __global__ void __launch_bounds__(128)
 k_build_list_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ scell,
                   const int *__restrict__ cell_start, CellGrid g, PBox<T> pb, BoxD bd, T rc2T, double rc2, int maxn,
-                  int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky) {
+                  int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
+                  const DevGeom *__restrict__ dg) {
     // G lanes per atom (G = 32: one warp per atom; G = 8: four atoms per warp, each group votes under its own mask)
     const int gt = blockIdx.x * blockDim.x + threadIdx.x;
     const int s = gt / G, lane = gt % G;
     if (s >= N) return;
+    if (dg) { pb = dg_pb<T>(dg); bd = dg->bd; }
     const unsigned gmask = G == 32 ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
     const int gshift = (threadIdx.x & 31) / G * G;
     const typename Vec4<T>::type pi = spos[s];
@@ -305,9 +311,13 @@ __global__ void __launch_bounds__(128)
 k_build_list_small(int N, const T *__restrict__ pos, const unsigned char *__restrict__ flags,
                    typename Vec4<T>::type *__restrict__ spos, int *__restrict__ perm, int *__restrict__ scell,
                    PBox<T> pb, BoxD bd, T rc2T, double rc2, int maxn, int *__restrict__ nl_count, int *__restrict__ nl,
-                   CellGrid g, unsigned int *__restrict__ sticky) {
+                   CellGrid g, unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
     const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (s >= N) return;
+    if (dg) {
+        pb = dg_pb<T>(dg); bd = dg->bd;
+        g.inv[0] = dg->inv[0]; g.inv[1] = dg->inv[1]; g.inv[2] = dg->inv[2]; g.cx = dg->cx; g.cy = dg->cy; g.bx = dg->bx;
+    }
     typename Vec4<T>::type pi;
     pi.x = pos[3 * s]; pi.y = pos[3 * s + 1]; pi.z = pos[3 * s + 2];
     pi.w = (T)(flags ? (int)flags[s] : 3);
@@ -380,6 +390,57 @@ template <typename T> PBox<T> ctx_pbox(const metad_ctx *c) { return make_pbox<T>
 template PBox<float> ctx_pbox<float>(const metad_ctx *);
 template PBox<double> ctx_pbox<double>(const metad_ctx *);
 
+// Device-resident box (NEXT-3, PAPER.md:51 NPT): derives everything the kernels need from the 9 box doubles in device memory
+// and checks what setup_geometry checks on the host for a host box — here a violation sets the sticky bit METAD_DEV_BOX (the
+// step then runs with defined but meaningless neighbour sets).  nc: cell counts frozen at capture (x in sub-cells).
+__global__ void k_geom_update(const double *__restrict__ box, double rc, int nc0, int nc1, int nc2, int xsub, float band_rel,
+                              DevGeom *__restrict__ out, unsigned int *__restrict__ sticky) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const double ax = box[0], bx = box[3], by = box[4], cx = box[6], cy = box[7], cz = box[8];
+    bool ok = box[1] == 0.0 && box[2] == 0.0 && box[5] == 0.0 && ax > 0.0 && by > 0.0 && cz > 0.0;
+    const double vol = ax * by * cz;
+    const double bxc[3] = { by * cz, -bx * cz, bx * cy - by * cx };
+    const double cxa[3] = { 0.0, cz * ax, -cy * ax };
+    double w[3];
+    w[0] = vol / sqrt(bxc[0] * bxc[0] + bxc[1] * bxc[1] + bxc[2] * bxc[2]);
+    w[1] = vol / sqrt(cxa[1] * cxa[1] + cxa[2] * cxa[2]);
+    w[2] = cz;
+    const int nc[3] = { nc0, nc1, nc2 };
+    for (int d = 0; d < 3; ++d) {
+        if (!(rc < 0.5 * w[d])) ok = false;
+        const int full = d == 0 ? nc[d] / xsub : nc[d];                 // rc-wide cells along this direction
+        if (full > 1 && !(w[d] / full >= rc)) ok = false;               // a cell narrower than rc would miss neighbours
+    }
+    if (!ok) atomicOr(sticky, (unsigned)METAD_DEV_BOX);
+    BoxD b = { ax, bx, by, cx, cy, cz, 0.5 * ax, 0.5 * by, 0.5 * cz };
+    out->bd = b;
+    PBox<double> pd = { ax, bx, by, cx, cy, cz, 0, 0, 0, 0, 0, 0, b.hx, b.hy, b.hz, 0.0 };
+    out->pbd = pd;
+    PBox<float> pf;
+    const double v[6] = { ax, bx, by, cx, cy, cz };
+    float hi[6], lo[6];
+    for (int k = 0; k < 6; ++k) { hi[k] = (float)v[k]; lo[k] = (float)(v[k] - (double)hi[k]); }
+    pf.ax = hi[0]; pf.bx = hi[1]; pf.by = hi[2]; pf.cx = hi[3]; pf.cy = hi[4]; pf.cz = hi[5];
+    pf.lax = lo[0]; pf.lbx = lo[1]; pf.lby = lo[2]; pf.lcx = lo[3]; pf.lcy = lo[4]; pf.lcz = lo[5];
+    pf.hx = (float)b.hx; pf.hy = (float)b.hy; pf.hz = (float)b.hz;
+    const double L = fmax(fabs(ax) + fabs(bx) + fabs(cx), fmax(fabs(by) + fabs(cy), fabs(cz)));
+    const double ulpL = ldexp(1.0, ilogb(fmax(L, 1e-30)) - 23);
+    pf.band = (float)fmax((double)band_rel * rc * rc, 4.0 * rc * ulpL);      // as make_pbox<float>
+    out->pbf = pf;
+    out->inv[0] = 1.0 / ax; out->inv[1] = 1.0 / by; out->inv[2] = 1.0 / cz;
+    out->inv[3] = out->inv[4] = out->inv[5] = 0.0;
+    out->cx = cx; out->cy = cy; out->bx = bx;
+    for (int k = 0; k < 9; ++k) out->box[k] = box[k];
+}
+
+int geom_update(metad_ctx *c, const double *d_box) {
+    k_geom_update<<<1, 32, 0, c->stream>>>(d_box, c->rc, c->grid.nc[0], c->grid.nc[1], c->grid.nc[2], c->tiled ? c->tile_hx : 1,
+                                           1e-5f, c->d_geom, c->d_sticky);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
 template <typename T>
 static int nb_build_t(metad_ctx *c, const void *d_pos) {
     typedef typename Vec4<T>::type V4;
@@ -391,7 +452,7 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
         if (tm) { cudaEventRecord(c->ev[0], st); cudaEventRecord(c->ev[1], st); c->timing_recorded = 1; }
         k_build_list_small<T><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const T *)d_pos, c->d_flags, (V4 *)c->d_spos, c->d_perm,
                                                                              c->d_scell, make_pbox<T>(c->boxd, c->rc), c->boxd, (T)c->rc2, c->rc2,
-                                                                             c->maxn, c->d_nl_count, c->d_nl, c->grid, c->d_sticky);
+                                                                             c->maxn, c->d_nl_count, c->d_nl, c->grid, c->d_sticky, c->dg);
         if (tm) cudaEventRecord(c->ev[2], st);
         c->launches += 1;
         CUDA_TRY(cudaGetLastError());
@@ -399,7 +460,7 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     }
     if (tm) { cudaEventRecord(c->ev[0], st); c->timing_recorded = 1; }
     k_bin<T><<<div_up(N, 256), 256, 0, st>>>(N, (const T *)d_pos, c->grid, c->d_cell_of, c->d_slot, c->d_cell_count,
-                                             c->d_sticky);
+                                             c->d_sticky, c->dg);
     k_scan_sums<<<nsb, SCAN_THREADS, 0, st>>>(ncell, c->d_cell_count, c->d_block_sums);
     k_scan_apply<<<nsb, SCAN_THREADS, 0, st>>>(ncell, N, c->d_cell_count, c->d_block_sums, c->d_cell_start);
     k_scatter<<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_of, c->d_slot, c->d_cell_start, c->d_perm_raw);
@@ -417,15 +478,15 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     if (N <= METAD_WARP_PER_ATOM_MAX)
         k_build_list_warp<T, 32><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start,
                                                                                  c->grid, pb, c->boxd, (T)c->rc2, c->rc2, c->maxn,
-                                                                                 c->d_nl_count, c->d_nl, c->d_sticky);
+                                                                                 c->d_nl_count, c->d_nl, c->d_sticky, c->dg);
     else if (N <= 8 * METAD_WARP_PER_ATOM_MAX)
         k_build_list_warp<T, 8><<<div_up((long long)N * 8, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start,
                                                                                c->grid, pb, c->boxd, (T)c->rc2, c->rc2, c->maxn,
-                                                                               c->d_nl_count, c->d_nl, c->d_sticky);
+                                                                               c->d_nl_count, c->d_nl, c->d_sticky, c->dg);
     else
     k_build_list<T><<<div_up(N, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start, c->grid, pb,
                                                    c->boxd, (T)c->rc2, c->rc2, c->maxn, c->d_nl_count, c->d_nl,
-                                                   c->d_sticky);
+                                                   c->d_sticky, c->dg);
     if (tm) cudaEventRecord(c->ev[2], st);
     c->launches += 6;
     CUDA_TRY(cudaGetLastError());

@@ -32,6 +32,16 @@ struct TileGeom {
     double wa, wb, wc;           // cell edge vectors are a/nc0, b/nc1, c/nc2 (used for the tile's coordinate range)
 };
 
+// lattice rows of the step: from the device-resident geometry when the box lives in device memory (NPT), else the kernel
+// argument (read at the few points of use: the kernel argument itself is never written, it stays in the constant bank)
+struct TileBox { double ax, bx, by, cx, cy, cz; };
+__device__ __forceinline__ TileBox tile_box(const TileGeom &g, const DevGeom *dg) {
+    TileBox b;
+    if (dg) { b.ax = dg->bd.ax; b.bx = dg->bd.bx; b.by = dg->bd.by; b.cx = dg->bd.cx; b.cy = dg->bd.cy; b.cz = dg->bd.cz; }
+    else { b.ax = g.ax; b.bx = g.bx; b.by = g.by; b.cx = g.cx; b.cy = g.cy; b.cz = g.cz; }
+    return b;
+}
+
 struct TileTables {
     int seg_g[TILE_NSEG];        // global (sorted-space) index of the segment's first atom
     int seg_len[TILE_NSEG];
@@ -65,7 +75,8 @@ struct TileScratch {
 #define TILE_SCRATCH_BYTES sizeof(TileScratch)
 __device__ __forceinline__ int tile_cut(int k, int nc, int nt) { return (int)(((unsigned)k * (unsigned)nc) / (unsigned)nt); }
 
-__device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restrict__ cell_start, TileTables &t, TileScratch &w) {
+__device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restrict__ cell_start, TileTables &t, TileScratch &w,
+                                           const DevGeom *dg) {
     const int tid = threadIdx.x;
     int b = blockIdx.x;
     const int tx = b % g.ntx; b /= g.ntx;
@@ -95,7 +106,8 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
         const double fa = (double)(x0 - hx + ((c & 1) ? Txe + 2 * hx : 0)) / g.nc0;
         const double fb = (double)(y0 - 1 + ((c & 2) ? Tye + 2 : 0)) / g.nc1;
         const double fc = (double)(z0 - 1 + ((c & 4) ? Tze + 2 : 0)) / g.nc2;
-        double lo[3] = { fa * g.ax + fb * g.bx + fc * g.cx, fb * g.by + fc * g.cy, fc * g.cz }, hi[3];
+        const TileBox bx = tile_box(g, dg);
+        double lo[3] = { fa * bx.ax + fb * bx.bx + fc * bx.cx, fb * bx.by + fc * bx.cy, fc * bx.cz }, hi[3];
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             hi[a] = lo[a];
@@ -203,14 +215,16 @@ __device__ __forceinline__ int tile_global_of(const TileTables &t, int li) {
 #define NL_CODE_NONE 13
 
 // tile-local position of a halo atom: (x, y, z, as_float(global sorted index | shift code << 27))
-__device__ __forceinline__ float4 tile_transform(const TileGeom &g, const TileTables &t, int seg, float4 p, int gidx) {
+__device__ __forceinline__ float4 tile_transform(const TileGeom &g, const TileTables &t, int seg, float4 p, int gidx,
+                                                 const DevGeom *dg) {
     float4 o;
     if (t.seg_wrapped[seg]) {                  // periodic image: lattice shift - origin added in fp64, rounded once
         const int code = t.seg_code[seg];
         const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
-        o.x = (float)((double)p.x + (wx * g.ax + wy * g.bx + wz * g.cx - (double)t.origin[0]));
-        o.y = (float)((double)p.y + (wy * g.by + wz * g.cy - (double)t.origin[1]));
-        o.z = (float)((double)p.z + (wz * g.cz - (double)t.origin[2]));
+        const TileBox b = tile_box(g, dg);
+        o.x = (float)((double)p.x + (wx * b.ax + wy * b.bx + wz * b.cx - (double)t.origin[0]));
+        o.y = (float)((double)p.y + (wy * b.by + wz * b.cy - (double)t.origin[1]));
+        o.z = (float)((double)p.z + (wz * b.cz - (double)t.origin[2]));
     } else {
         o.x = p.x - t.origin[0]; o.y = p.y - t.origin[1]; o.z = p.z - t.origin[2];
     }
@@ -219,12 +233,13 @@ __device__ __forceinline__ float4 tile_transform(const TileGeom &g, const TileTa
 }
 
 // Stages all halo positions into pos_s (warp per segment, coalesced).  No-op if the halo does not fit.
-__device__ __forceinline__ void tile_stage_pos(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos, float4 *pos_s) {
+__device__ __forceinline__ void tile_stage_pos(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos, float4 *pos_s,
+                                               const DevGeom *dg) {
     if (!t.staged) return;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     for (int s = wid; s < 3 * t.nrows; s += nw) {
         const int len = t.seg_len[s], g0 = t.seg_g[s], l0 = t.seg_off[s];
-        for (int i = lane; i < len; i += 32) pos_s[l0 + i] = tile_transform(g, t, s, spos[g0 + i], g0 + i);
+        for (int i = lane; i < len; i += 32) pos_s[l0 + i] = tile_transform(g, t, s, spos[g0 + i], g0 + i, dg);
     }
 }
 
@@ -261,11 +276,12 @@ __device__ __forceinline__ void tile_stage_pos_tma(const TileTables &t, const fl
 }
 
 // position accessor that also works when the tile was not staged (slow path, global memory)
-__device__ __forceinline__ float4 tile_pos(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos, const float4 *pos_s, int li) {
+__device__ __forceinline__ float4 tile_pos(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos, const float4 *pos_s, int li,
+                                           const DevGeom *dg) {
     if (t.staged) return pos_s[li];
     int s = tile_seg_of(t, li);
     int gi = t.seg_g[s] + (li - t.seg_off[s]);
-    return tile_transform(g, t, s, spos[gi], gi);
+    return tile_transform(g, t, s, spos[gi], gi, dg);
 }
 
 // own atom number a (0..nown-1) -> own-row q

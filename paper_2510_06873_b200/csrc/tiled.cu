@@ -28,11 +28,12 @@ __device__ __forceinline__ f32x2_t mul2(f32x2_t a, f32x2_t b) { f32x2_t r; asm("
 __device__ __forceinline__ f32x2_t fma2(f32x2_t a, f32x2_t b, f32x2_t c) { f32x2_t r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 
 template <bool STAGED>
-__device__ __forceinline__ float4 hpos(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos, const float4 *pos_s, int li) {
+__device__ __forceinline__ float4 hpos(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos, const float4 *pos_s, int li,
+                                       const DevGeom *dg) {
     if (STAGED) return pos_s[li];
     int s = tile_seg_of(t, li);
     int gi = t.seg_g[s] + (li - t.seg_off[s]);
-    return tile_transform(g, t, s, spos[gi], gi);
+    return tile_transform(g, t, s, spos[gi], gi, dg);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -41,11 +42,11 @@ __device__ __forceinline__ float4 hpos(const TileGeom &g, const TileTables &t, c
 template <bool STAGED>
 __device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t, const float4 *__restrict__ spos,
                                          const float4 *pos_s, nl16_t *list_s, const int *__restrict__ scell, int a, int col,
-                                         float rc2_hi, bool &ovf) {
+                                         float rc2_hi, bool &ovf, const DevGeom *dg) {
     const int q = tile_own_row(t, a);
     const int o = a - t.own_off[q];
     const int li = t.own_l[q] + o, s = t.own_g[q] + o;
-    const float4 pi = hpos<STAGED>(g, t, spos, pos_s, li);
+    const float4 pi = hpos<STAGED>(g, t, spos, pos_s, li, dg);
     const int ic = scell[s] % g.nc0 - t.x0 + g.hx;       // halo-cell column of the own atom
     const int r0 = t.own_row[q], rstride = t.Tye + 2;
     // candidate list written through 32-bit shared-memory addresses (generic 64-bit pointer bumps cost 4 extra
@@ -70,7 +71,7 @@ __device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t,
                 const int h2 = min(hi, lo + room);
 #pragma unroll 4
                 for (int lj = lo; lj < h2; ++lj) {
-                    const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj);
+                    const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj, dg);
                     // (dx, dy) and their squares as one packed pair each: 5 issue slots instead of 6 per candidate (the
                     // rounding differs from the exact pass by an ulp: far inside the 1e-5 band of this prefilter)
                     const f32x2_t dxy = add2(pk2(pj.x, pj.y), npi_xy);
@@ -99,14 +100,14 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
                                              int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
                                              float q_thresh, float inv_width, float *__restrict__ rec,
                                              float *__restrict__ q6_out, bool solid, int sw_n, int sw_m,
-                                             const int *__restrict__ perm) {
+                                             const int *__restrict__ perm, const DevGeom *__restrict__ dg) {
     const bool WITH_Q6 = MODE == 1;
     float csum = 0.f;                                      // MODE 2: sum of sw(r / r0) over the neighbours (q_thresh = 1 / r0)
     float cgx = 0.f, cgy = 0.f, cgz = 0.f;                 // MODE 2: sum of 2 sw' d / (r0 r)
     const int q = tile_own_row(t, a);
     const int o = a - t.own_off[q];
     const int li = t.own_l[q] + o, s = t.own_g[q] + o;
-    const float4 pi = hpos<STAGED>(g, t, spos, pos_s, li);
+    const float4 pi = hpos<STAGED>(g, t, spos, pos_s, li, dg);
     const nl16_t *myl = list_s + col;
     if (ovf) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
     int *out = nl + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
@@ -120,13 +121,13 @@ __device__ __forceinline__ float finish_atom(const TileGeom &g, const TileTables
     for (int k = 0; k < cnt; ++k) {
         const int lj = myl[k * TILE_THREADS];
         if (lj == li) continue;
-        const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj);
+        const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj, dg);
         const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         const float r2 = dx * dx + dy * dy + dz * dz;
         bool in = r2 < rc2f;
         if (r2 >= rc2_lo) {                                // borderline: canonical fp64 predicate on the inputs
             const float4 gi = spos[s], gj = spos[__float_as_int(pj.w) & NL_IDX_MASK];
-            in = r2_canonical(bd, (double)gj.x - (double)gi.x, (double)gj.y - (double)gi.y,
+            in = r2_canonical(dg ? dg->bd : bd, (double)gj.x - (double)gi.x, (double)gj.y - (double)gi.y,
                               (double)gj.z - (double)gi.z) < rc2;
         }
         if (!in) continue;
@@ -206,20 +207,23 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
                                            const BoxD &bd, float rc2f, double rc2, int maxn, int *__restrict__ nl_count,
                                            int *__restrict__ nl, unsigned int *__restrict__ sticky, float q_thresh,
                                            float inv_width, float *__restrict__ rec, float *__restrict__ q6_out, bool solid,
-                                           int sw_n, int sw_m, const int *__restrict__ perm, double (&v)[2]) {
+                                           int sw_n, int sw_m, const int *__restrict__ perm, double (&v)[2],
+                                           const DevGeom *__restrict__ dg) {
     const float rc2_hi = rc2f * (1.f + 1e-5f), rc2_lo = rc2f * (1.f - 1e-5f);
     const int tid = threadIdx.x;
     for (int a = tid; a < t.nown; a += blockDim.x) {
         bool ovf = false;
-        const int cnt = scan_atom<STAGED>(g, t, spos, pos_s, list_s, scell, a, tid, rc2_hi, ovf);
+        const int cnt = scan_atom<STAGED>(g, t, spos, pos_s, list_s, scell, a, tid, rc2_hi, ovf, dg);
         const float q6 = finish_atom<STAGED, MODE>(g, t, spos, pos_s, list_s, a, tid, cnt, ovf, bd, rc2f, rc2_lo, rc2, maxn,
-                                                   nl_count, nl, sticky, q_thresh, inv_width, rec, q6_out, solid, sw_n, sw_m, perm);
+                                                   nl_count, nl, sticky, q_thresh, inv_width, rec, q6_out, solid, sw_n, sw_m, perm, dg);
         if (MODE != 0) v[0] += (double)q6;
         if (MODE == 1) v[1] += (double)(1.f / (1.f + expf(-(q6 - q_thresh) * inv_width)));
     }
 }
 
-template <int MODE>   // 0: list only, 1: + Q6 pass 1, 2: + coordination sum (ungrouped COORD, q_thresh = 1 / r0)
+// DEVBOX: the step's box lives in device memory (metad_*_dev, NPT); the host-box instances never touch the pointer, so they
+// keep the registers and the schedule they had without it
+template <int MODE, bool DEVBOX>   // 0: list only, 1: + Q6 pass 1, 2: + coordination sum (ungrouped COORD, q_thresh = 1 / r0)
 __global__ void __launch_bounds__(TILE_THREADS, 5)
 k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict__ scell,
              const int *__restrict__ cell_start, BoxD bd, float rc2f, double rc2, int maxn,
@@ -228,27 +232,30 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
              int sw_n, int sw_m, const int *__restrict__ perm, double *__restrict__ partials, unsigned int *__restrict__ ticket, double scale_mean, double scale_solid,
              double *__restrict__ cv_q6 /* [2]: Q6 mean, solid count */,
              double *__restrict__ cv_out /* the context's CV vector on the run paths (NULL: k_q6_publish hands the sums over) */,
-             int dim0, int dim1) {
+             int dim0, int dim1, const DevGeom *__restrict__ dg_arg) {
+    const DevGeom *dg = DEVBOX ? dg_arg : nullptr;
     extern __shared__ float4 dyn_smem[];
     __shared__ TileTables t;
     __shared__ double red[64];
     float4 *pos_s = dyn_smem;
     nl16_t *list_s = reinterpret_cast<nl16_t *>(dyn_smem + g.cap);
-    tile_setup(g, cell_start, t, *reinterpret_cast<TileScratch *>(dyn_smem));   // scratch = the (still unused) staging area
+    // a device-resident box (NPT, dg != NULL) replaces the lattice rows of the arguments at their few points of use (tile
+    // origin, periodic images, fp64 recheck): the common case costs no registers
+    tile_setup(g, cell_start, t, *reinterpret_cast<TileScratch *>(dyn_smem), dg);   // scratch = the (still unused) staging area
     __shared__ unsigned long long stage_bar;
     if (t.staged && !t.any_wrapped && t.total > 0) tile_stage_pos_tma(t, spos, pos_s, &stage_bar);   // block-uniform choice
     else
-    tile_stage_pos(g, t, spos, pos_s);
+    tile_stage_pos(g, t, spos, pos_s, dg);
     __syncthreads();
     double v[2] = { 0.0, 0.0 };
     if (t.total > 65535) {
         if (threadIdx.x == 0) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
     } else if (t.staged) {
         build_body<true, MODE>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
-                                  inv_width, rec, q6_out, solid != 0, sw_n, sw_m, perm, v);
+                                  inv_width, rec, q6_out, solid != 0, sw_n, sw_m, perm, v, dg);
     } else {
         build_body<false, MODE>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
-                                   inv_width, rec, q6_out, solid != 0, sw_n, sw_m, perm, v);
+                                   inv_width, rec, q6_out, solid != 0, sw_n, sw_m, perm, v, dg);
     }
     if (MODE != 0) {
         block_reduce<2>(v, red);
@@ -299,9 +306,12 @@ static size_t smem_build(const TileGeom &g) {
 int tiled_init() {
     // per (device, function) attribute: set on every metad_create — no process-wide "done" flag, so contexts created from
     // several threads or on several devices need no synchronisation
-    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    CUDA_TRY(cudaFuncSetAttribute(k_tile_build<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
     return METAD_OK;
 }
 
@@ -310,26 +320,31 @@ int tiled_build(metad_ctx *c) {
     int nt = g.ntx * g.nty * g.ntz;
     double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
     double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
+#define TILE_LAUNCH(MODE, ...)                                                                                        \
+    do {                                                                                                              \
+        if (c->dg) k_tile_build<MODE, true><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(__VA_ARGS__);             \
+        else k_tile_build<MODE, false><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(__VA_ARGS__);                  \
+    } while (0)
     if (c->has_q6)
-        k_tile_build<1><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
+        TILE_LAUNCH(1,
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
             c->d_nl_count, c->d_nl, c->d_sticky, (float)qt, (float)(1.0 / qw), (float *)c->d_rec, c->d_q6,
             c->q6_solid_dim >= 0 ? 1 : 0, 0, 0, c->d_perm, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
             c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0, c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0,
-            c->d_cvq6, c->cv_direct, c->q6_mean_dim, c->q6_solid_dim);
+            c->d_cvq6, c->cv_direct, c->q6_mean_dim, c->q6_solid_dim, c->dg);
     else if (c->has_coord) {                                  // ungrouped coordination number: the sum of sw rides on the exact pass
         const CvDev &d = c->cv[c->coord_dim];
         // lazy_neighbors: nothing downstream reads the list (the force stage scales the per-atom gradient; the virial would
         // walk the list) — the pass runs list-free and metad_get_neighbors reports that there is no list
         c->list_skipped = c->p.lazy_neighbors && !c->p.want_virial && c->d_cgrad;
-        k_tile_build<2><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
+        TILE_LAUNCH(2,
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
             c->d_nl_count, c->list_skipped ? nullptr : c->d_nl, c->d_sticky, (float)(1.0 / d.r0), 1.f, c->d_cgrad, nullptr, 0, d.n, d.m, c->d_perm,
-            c->d_partials + c->nblocks_atoms, c->d_tickets + 1, d.scale, 0.0, c->d_cvq6, c->cv_direct, c->coord_dim, -1);
+            c->d_partials + c->nblocks_atoms, c->d_tickets + 1, d.scale, 0.0, c->d_cvq6, c->cv_direct, c->coord_dim, -1, c->dg);
     } else
-        k_tile_build<0><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(
+        TILE_LAUNCH(0,
             g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
-            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, 0, 0, c->d_perm, nullptr, nullptr, 0.0, 0.0, nullptr, nullptr, -1, -1);
+            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, 0, 0, c->d_perm, nullptr, nullptr, 0.0, 0.0, nullptr, nullptr, -1, -1, c->dg);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmetad_b200.so")
 
 MAX_CV = 4
 OK, ERR_ARG, ERR_BOX, ERR_STATE, ERR_CUDA, ERR_NOMEM = range(6)
-DEV_NEIGH_OVERFLOW, DEV_HILL_OVERFLOW, DEV_GRID_RANGE, DEV_NONFINITE, DEV_POS_RANGE, DEV_TRAJ_FULL = 1, 2, 4, 8, 16, 32
+DEV_NEIGH_OVERFLOW, DEV_HILL_OVERFLOW, DEV_GRID_RANGE, DEV_NONFINITE, DEV_POS_RANGE, DEV_TRAJ_FULL, DEV_BOX = 1, 2, 4, 8, 16, 32, 64
 CV_COORD, CV_Q6_MEAN, CV_Q6_SOLID, CV_RGYR, CV_CONTACTS, CV_TORSION, CV_MINDIST, CV_LATTICE = range(8)
 
 _P = ctypes.c_void_p
@@ -36,11 +36,11 @@ class Params(ctypes.Structure):
     _fields_ = [("natoms", _I), ("precision", _I), ("max_neigh", _I), ("ncv", _I),
                 ("cv", CvDesc * MAX_CV), ("sigma", _D * MAX_CV), ("w0", _D), ("kT", _D),
                 ("bias_factor", _D), ("max_hills", _I), ("stride", _I), ("grid_n", _I * 2),
-                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("traj_capacity", _I), ("lazy_neighbors", _I), ("want_virial", _I)]
+                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("traj_capacity", _I), ("lazy_neighbors", _I), ("want_virial", _I), ("box_slack", _D)]
 
 
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
-           "metad_apply_forces", "metad_deposit", "metad_run", "metad_step_host", "metad_host_alloc", "metad_host_free", "metad_status",
+           "metad_apply_forces", "metad_deposit", "metad_run", "metad_build_neighbors_dev", "metad_run_dev", "metad_reset_box", "metad_step_host", "metad_host_alloc", "metad_host_free", "metad_status",
            "metad_get_state", "metad_get_neighbors", "metad_get_q6", "metad_set_hills", "metad_get_hills",
            "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reweight_recorded", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_synchronize", "metad_graph_info", "metad_fma_peak", "metad_version", "metad_last_error"]
 
@@ -65,6 +65,9 @@ def load():
     L.metad_deposit.argtypes = [_P, _P, _P]
     L.metad_run.argtypes = [_P, _P, _P, _D, _P, _I]
     L.metad_step_host.argtypes = [_P, _P, _P, _D, _P, _P, _P]
+    L.metad_build_neighbors_dev.argtypes = [_P, _P, _P, _D]
+    L.metad_run_dev.argtypes = [_P, _P, _P, _D, _P, _I]
+    L.metad_reset_box.argtypes = [_P]
     L.metad_host_alloc.argtypes = [ctypes.POINTER(_P), ctypes.c_size_t]
     L.metad_host_free.argtypes = [_P]
     L.metad_status.argtypes = [_P, _P]
@@ -144,7 +147,8 @@ class MetaD:
     fields); tensors passed to the methods are torch CUDA tensors (float64, or float32 for pos/F when
     precision == 32)."""
 
-    def __init__(self, workload, max_hills=None, precision=None, grid=None, force_scale=1.0, stream=None, want_virial=False, lazy_neighbors=False, traj_capacity=0):
+    def __init__(self, workload, max_hills=None, precision=None, grid=None, force_scale=1.0, stream=None, want_virial=False, lazy_neighbors=False, traj_capacity=0,
+                 box_slack=0.0):
         import torch
         self.torch = torch
         L = load()
@@ -197,6 +201,7 @@ class MetaD:
         p.want_virial = 1 if want_virial else 0
         p.lazy_neighbors = 1 if lazy_neighbors else 0
         p.traj_capacity = int(traj_capacity)
+        p.box_slack = float(box_slack)
         self._params = p
         h = _P()
         _check(L.metad_create(ctypes.byref(h), ctypes.byref(p), _P(self.stream.cuda_stream)))
@@ -249,6 +254,18 @@ class MetaD:
         box = self.box if box is None else np.ascontiguousarray(box, dtype=np.float64)
         _check(load().metad_run(self._h, _ptr(pos), box.ctypes.data, float(self.rc if rc is None else rc), _ptr(F),
                                 int(nsteps)))
+
+    def build_neighbors_dev(self, pos, d_box, rc=None):
+        """Box in device memory (torch float64 CUDA tensor of 9 elements)."""
+        assert pos.dtype == self.dtype and pos.is_cuda and d_box.is_cuda and d_box.dtype == self.torch.float64
+        _check(load().metad_build_neighbors_dev(self._h, _ptr(pos), _ptr(d_box), float(self.rc if rc is None else rc)))
+
+    def run_dev(self, pos, d_box, F, nsteps, rc=None):
+        assert d_box.is_cuda and d_box.dtype == self.torch.float64 and d_box.numel() == 9
+        _check(load().metad_run_dev(self._h, _ptr(pos), _ptr(d_box), float(self.rc if rc is None else rc), _ptr(F), int(nsteps)))
+
+    def reset_box(self):
+        _check(load().metad_reset_box(self._h))
 
     def step_host(self, pos_host, F_host, box=None, rc=None):
         """pos_host / F_host: pinned CPU torch tensors (or numpy arrays) of the context's dtype."""

@@ -111,7 +111,7 @@ def force_bound(F_ref, dV_gpu, dV_ref, grads, tol_f=TOL_F):
 
 
 def chained_run(w, precision=None, nsteps=7, grid=None, lazy=False, hills=None, host=False, n_init_hills=40,
-                pos_of_step=None, box_of_step=None, seed=5):
+                pos_of_step=None, box_of_step=None, seed=5, device_box=False, box_slack=0.0):
     """The library's RUN paths (metad_run = CUDA-graph replay, or metad_step_host with host=True) one step at a time, every
     step checked stage-wise against the oracle fed with the CUDA path's OWN upstream values (reading S, no slack factor):
 
@@ -141,11 +141,12 @@ def chained_run(w, precision=None, nsteps=7, grid=None, lazy=False, hills=None, 
         o.enable_grid(*grid)
         of.enable_grid(*grid)
     of.set_hills(*hills)
-    md = MetaD(w, precision=precision, max_hills=len(hills[1]) + nsteps + 8, grid=grid, lazy_neighbors=lazy)
+    md = MetaD(w, precision=precision, max_hills=len(hills[1]) + nsteps + 8, grid=grid, lazy_neighbors=lazy, box_slack=box_slack)
     md.set_hills(*hills)
     with torch.cuda.stream(md.stream):
         dpos = torch.tensor(pos, device="cuda", dtype=tdt)
         F = torch.zeros((w.natoms, 3), device="cuda", dtype=tdt)
+        dbox = torch.zeros(9, device="cuda", dtype=torch.float64)       # device_box: the library never sees a host box
     md.synchronize()
     if host:
         pos_h = pinned_array(pos.shape, pos.dtype)
@@ -169,8 +170,13 @@ def chained_run(w, precision=None, nsteps=7, grid=None, lazy=False, hills=None, 
             with torch.cuda.stream(md.stream):
                 dpos.copy_(torch.from_numpy(p))
                 F.zero_()
+                if device_box:
+                    dbox.copy_(torch.from_numpy(box))
             md.synchronize()
-            md.run(dpos, F, 1, box=box)
+            if device_box:
+                md.run_dev(dpos, dbox, F, 1)
+            else:
+                md.run(dpos, F, 1, box=box)
             md.synchronize()
             Fg = F.cpu().numpy().astype(np.float64)
         per_step_launches = md.launch_count() - l0
@@ -187,7 +193,8 @@ def chained_run(w, precision=None, nsteps=7, grid=None, lazy=False, hills=None, 
         assert abs(st["V"] - V_ref) <= TOL_CV * max(abs(V_ref), TINY), (k, st["V"], V_ref)
         assert np.abs(st["dVds"] - dV_ref).max() <= TOL_CV * max(np.abs(dV_ref).max(), TINY), (k, st["dVds"], dV_ref)
         F_ref = o.forces(st["dVds"])
-        ulp = 2.0 ** -24 * np.abs(F_ref).max() if precision == 32 else 0.0
+        # fp32 force array: half an ulp of the largest component, and never finer than the smallest fp32 denormal
+        ulp = max(2.0 ** -24 * np.abs(F_ref).max(), 2.0 ** -149) if precision == 32 else 0.0
         assert np.abs(Fg - F_ref).max() <= TOL_F * np.abs(F_ref).max() + ulp, (k, np.abs(Fg - F_ref).max(), np.abs(F_ref).max())
         due = w.stride > 0 and (k + 1) % w.stride == 0
         assert st["step"] == k + 1 and len(ah) == len(hh) + int(due) == st["nhills"]
@@ -200,7 +207,7 @@ def chained_run(w, precision=None, nsteps=7, grid=None, lazy=False, hills=None, 
         Fo = np.zeros((w.natoms, 3))
         s_f, V_f, dV_f = of.run_step(p64, Fo)
         assert rel(st["cv"], s_f) <= TOL_CV
-        bound_acc += force_bound(Fo, st["dVds"], dV_f, of.grads)
+        bound_acc += force_bound(Fo, st["dVds"], dV_f, of.grads) + ulp
         F_acc += Fg
         Fo_acc += Fo
         states.append(dict(st, s_ref=s_ref, V_ref=V_ref, dV_ref=dV_ref, V_free=V_f, dV_free=dV_f))

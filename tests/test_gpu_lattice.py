@@ -157,3 +157,40 @@ def test_changing_box_every_step_updates_the_graph():
                     box_of_step=lambda k: box0 * scales[k], pos_of_step=lambda k: frac @ (box0 * scales[k]).reshape(3, 3))
     assert r["states"][-1]["nhills"] == 30 + 3
     assert np.array_equal(w.box, box0)
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_device_resident_box_one_capture_no_graph_update(precision):
+    """NEXT-3 (PAPER.md:51 NPT; PAPER.md:61 on GPU-CPU transfers): the box lives in device memory and changes every step —
+    metad_run_dev captures its CUDA graph ONCE, never updates it, and every step matches the oracle (gpu_util.chained_run) on
+    the generic fp64 kernels and on the tiled fp32 path; a box that shrinks below the frozen cell grid raises METAD_DEV_BOX,
+    metad_reset_box re-derives the grid."""
+    import torch
+    from paper_2510_06873_b200 import metad
+    w = _workload()
+    w.stride = 2
+    frac = np.linalg.solve(w.box.reshape(3, 3).T, w.pos.T).T
+    box0 = w.box.copy()
+    scales = [1.0, 1.004, 0.985, 1.02, 1.03, 0.975, 1.0]
+    s0 = np.array([5.4, *np.linalg.norm(box0.reshape(3, 3), axis=1)])
+    rng = np.random.default_rng(8)
+    centers = s0 * (1.0 + 0.04 * (rng.random((30, 4)) - 0.5))
+    r = chained_run(w, precision=precision, nsteps=len(scales), hills=(centers, np.full(30, 1.0)), device_box=True, box_slack=0.03,
+                    box_of_step=lambda k: box0 * scales[k], pos_of_step=lambda k: frac @ (box0 * scales[k]).reshape(3, 3))
+    md = r["md"]
+    gi = md.graph_info()
+    assert gi["captures"] == 1 and gi["updates"] == 0
+    assert gi["nodes"] == gi["kernel"] and gi["memcpy"] == 0 and gi["host"] == 0
+    assert md.status() == 0
+    # a box 8 % smaller than the one the grid was frozen for: cells narrower than rc -> sticky bit, no error code
+    tdt = torch.float32 if precision == 32 else torch.float64
+    with torch.cuda.stream(md.stream):
+        dbox = torch.tensor(box0 * 0.92, device="cuda", dtype=torch.float64)
+        dpos = torch.tensor(frac @ (box0 * 0.92).reshape(3, 3), device="cuda", dtype=tdt)
+        F = torch.zeros((w.natoms, 3), device="cuda", dtype=tdt)
+    md.synchronize()
+    md.build_neighbors_dev(dpos, dbox)
+    assert md.status() & metad.DEV_BOX
+    md.reset_box()
+    md.run_dev(dpos, dbox, F, 1)
+    assert md.graph_info()["captures"] == 2
