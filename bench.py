@@ -43,6 +43,12 @@ def parse():
     ap.add_argument("--lazy", action="store_true", help="params.lazy_neighbors: skip the list build when no CV reads it (c1, t0)")
     ap.add_argument("--virial", action="store_true", help="also compute the bias virial every step (NPT; COORD / Q6 / LATTICE CVs)")
     ap.add_argument("--stage-times", action="store_true", default=True)
+    ap.add_argument("--skin", type=float, default=0.0,
+                    help="params.skin: Verlet-skin reuse of the neighbour list (a separately reported mode; the headline rebuilds "
+                         "the list every step)")
+    ap.add_argument("--move", type=float, default=0.0,
+                    help="move every atom by a seeded Gaussian displacement of this width (A) before every timed step (device "
+                         "kernels of the harness, outside the timed events): what an MD integrator does between two calls")
     ap.add_argument("--peaks", action="store_true",
                     help="only measure the scalar-pipe roofline denominators (FP32 / FP32x2 / FP64 FMA microbenchmark, "
                          "metad_fma_peak) and print them as one JSON line")
@@ -326,7 +332,7 @@ def run_ours(args):
         sig = np.asarray(w.sigma)
         grid = (w.grid_n, centers[0] - 120 * sig, centers[0] + 120 * sig)      # reading M
     md = MetaD(w, precision=precision, max_hills=w.n_hills + args.steps + args.warmup + 4096, grid=grid,
-               want_virial=args.virial, lazy_neighbors=(args.config in ("t0", "r0") or args.lazy))
+               want_virial=args.virial, lazy_neighbors=(args.config in ("t0", "r0") or args.lazy), skin=args.skin)
     md.set_hills(centers, heights)
     with torch.cuda.stream(md.stream):
         F = torch.zeros((w.natoms, 3), device="cuda", dtype=tdt)
@@ -339,19 +345,49 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident timed region: K graph replays
-    md.run(dpos, F, args.warmup)
+    moving = args.move > 0.0
+    if moving:
+        # the harness plays the MD integrator: seeded Gaussian displacement + re-wrapping into the (triclinic) box, on the
+        # context's stream, OUTSIDE the timed events; the library sees new coordinates in the same device buffer every step
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(2510068730 + rank)
+        Bm = torch.tensor(w.box.reshape(3, 3), device="cuda", dtype=torch.float64)
+        Binv = torch.linalg.inv(Bm)
+
+        def integrate():
+            with torch.cuda.stream(md.stream):
+                dpos.add_(torch.randn(dpos.shape, device="cuda", dtype=dpos.dtype, generator=gen) * args.move)
+                fr = dpos.double() @ Binv
+                fr -= torch.floor(fr)
+                dpos.copy_((fr @ Bm).to(dpos.dtype))
+    for _ in range(args.warmup):
+        if moving:
+            integrate()
+        md.run(dpos, F, 1)
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
     l0 = md.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(md.stream)
-    md.run(dpos, F, args.steps)
-    e1.record(md.stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
+    b0 = md.rebuilds()
+    if moving:
+        evs_ = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a_, b_ in evs_:
+            integrate()
+            a_.record(md.stream)
+            md.run(dpos, F, 1)
+            b_.record(md.stream)
+        barrier()
+        ms = float(sum(a_.elapsed_time(b_) for a_, b_ in evs_))
+    else:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(md.stream)
+        md.run(dpos, F, args.steps)
+        e1.record(md.stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
     launches = md.launch_count() - l0
+    builds = md.rebuilds() - b0
     # ---- per-stage CUDA-event times (same stream, explicit five calls), inside the same clock-sampled window
     stage_names = ["build_neighbors", "eval_cv", "bias", "apply_forces", "deposit"]
     acc = np.zeros(5)
@@ -512,13 +548,20 @@ def run_ours(args):
                          "algorithmic_flops_per_launch": gfl, "kernel_ms": float(gms), "hills": int(nh_now),
                          "nodes": [int(grid[0][0]), int(grid[0][1])],
                          "gaussian_terms_per_s": grid[0][0] * grid[0][1] * nh_now / (gms * 1e-3)})
+    cfg_ = describe(w, precision)
+    if args.skin > 0.0:
+        cfg_["neighbour_build"] = (f"Verlet skin {args.skin} A (params.skin): the rc + skin list is kept while no atom has moved "
+                                   f"{args.skin / 2} A; {int(builds)} builds in {args.steps} timed steps, decided on the device")
+    cfg_["positions"] = (f"moved before every step by a seeded Gaussian displacement of width {args.move} A and re-wrapped (harness "
+                         "kernels outside the timed events)" if moving else "fixed (BASELINE.json configs: evaluate with fixed positions)")
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32" if precision == 32 else "f64", "data": "synthetic", "config": describe(w, precision),
+            "dtype": "f32" if precision == 32 else "f64", "data": "synthetic", "config": cfg_,
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(pos_h.nbytes + F_h.nbytes),
                     "d2h_bytes_per_step": int(F_h.nbytes + 8 * (w.ncv + 1)), "ms_per_step": e2e_ms_max / ke},
             "roofline": roof, "roofline_kernels": roof_all, "peaks": fpk, "graph": md.graph_info(),
+            "list_builds_in_timed_steps": int(builds),
             "stages_ms": {n: float(v) for n, v in zip(stage_names, stage_ms)},
             "state": {"cv": [float(x) for x in state["cv"]], "V": float(state["V"]), "nhills": state["nhills"],
                       "sticky": status}}

@@ -119,6 +119,14 @@ typedef struct {
                                        returns METAD_ERR_STATE in both cases.  0 (default): always built */
     int want_virial;                /* != 0: metad_apply_forces also computes the bias virial (metad_get_virial) for NPT runs
                                        (reading AD), for every CV kind */
+    double skin;                    /* > 0: Verlet-skin reuse of the neighbour list.  The list is built with
+                                       the cutoff rc + skin and kept while no atom has moved more than skin / 2 from where it was
+                                       at the build (checked on the device every step: no host read, the rebuild decision is taken
+                                       inside the captured graph); every CV / force kernel filters the pairs with the canonical
+                                       predicate r < rc on the current positions, so CVs, forces and metad_get_neighbors are those
+                                       of the exact rc list at every step.  max_neigh must hold the rc + skin list; the box needs
+                                       rc + skin < half of every perpendicular width.  Supported by the list CVs (COORD, Q6_*,
+                                       MINDIST); 0 (default): the list is rebuilt every step */
     double box_slack;               /* metad_*_dev calls: the cell grid is derived ONCE (first call / after metad_reset_box) with
                                        cells at least rc (1 + box_slack) wide, so the device-resident box may shrink by that
                                        fraction before METAD_DEV_BOX is raised; 0 = cells as small as rc allows */
@@ -253,6 +261,10 @@ int metad_get_timing(metad_ctx *ctx, float *h_ms_sort, float *h_ms_list);
 
 /* Number of kernels the library has launched on this context so far (graph replays included). */
 long long metad_launch_count(metad_ctx *ctx);
+
+/* [sync] Number of neighbour-list builds (cell sort + list) the context has executed so far: with params.skin > 0 fewer than
+ * the number of steps.  The count lives on the device; the rebuild decision itself is never read by the host. */
+int metad_get_rebuilds(metad_ctx *ctx, int *h_count);
 
 /* [sync] Waits for everything enqueued on the context's stream (the way to order a context created with cuda_stream ==
  * NULL against the caller's own work). */

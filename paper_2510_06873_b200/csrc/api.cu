@@ -253,7 +253,18 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
     CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
     CUDA_TRY(dev_alloc(&c->d_hill_stage, (size_t)(c->D + 1) * p->max_hills));
     CUDA_TRY(dev_alloc(&c->d_geom, 1));
+    CUDA_TRY(dev_alloc(&c->d_nbuilds, 1));
+    CUDA_TRY(cudaMemset(c->d_nbuilds, 0, sizeof(int)));
     if (!(p->box_slack >= 0.0) || p->box_slack > 1.0) FAIL(METAD_ERR_ARG, "box_slack must be in [0, 1]");
+    if (!(p->skin >= 0.0)) FAIL(METAD_ERR_ARG, "skin must be >= 0");
+    c->skin_on = p->skin > 0.0 && (c->has_q6 || c->has_coord || c->has_mindist);
+    if (c->skin_on) {
+        CUDA_TRY(dev_alloc(&c->d_skin_flag, 2));
+        const int ones[2] = { 1, 1 };                       // the first step builds
+        CUDA_TRY(cudaMemcpy(c->d_skin_flag, ones, sizeof(ones), cudaMemcpyHostToDevice));
+        CUDA_TRY(cudaMalloc(&c->d_ref, 4 * tsz * (size_t)N));
+        if (c->has_q6 && c->prec == 32) CUDA_TRY(dev_alloc(&c->d_keep_mask, N));
+    }
     CUDA_TRY(cudaDeviceSynchronize());
     return METAD_OK;
 }
@@ -269,7 +280,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage, c->d_geom };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage, c->d_geom, c->d_skin_flag, c->d_ref, c->d_nbuilds, c->d_keep_mask };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
@@ -288,6 +299,7 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc, double sla
     if (box[1] != 0.0 || box[2] != 0.0 || box[5] != 0.0) FAIL(METAD_ERR_BOX, "box must be lower-triangular (rows a,b,c)");
     if (!(box[0] > 0.0) || !(box[4] > 0.0) || !(box[8] > 0.0)) FAIL(METAD_ERR_BOX, "box diagonal must be positive");
     if (!(rc > 0.0)) FAIL(METAD_ERR_ARG, "rc must be positive");
+    const double rcl = rc + (c->skin_on ? c->p.skin : 0.0);      // the list (and the cells) reach rc + skin
     const double ax = box[0], bx = box[3], by = box[4], cx = box[6], cy = box[7], cz = box[8];
     const double vol = ax * by * cz;
     // perpendicular widths: V / |b x c|, V / |c x a|, V / |a x b|
@@ -298,13 +310,13 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc, double sla
     w[1] = vol / sqrt(cxa[1] * cxa[1] + cxa[2] * cxa[2]);
     w[2] = cz;
     for (int d = 0; d < 3; ++d)
-        if (!(rc < 0.5 * w[d])) FAIL(METAD_ERR_BOX, "rc must be smaller than half of every perpendicular box width");
+        if (!(rcl < 0.5 * w[d])) FAIL(METAD_ERR_BOX, "rc (+ skin) must be smaller than half of every perpendicular box width");
     CellGrid g;
     double shrink = 1.0;
     for (;;) {
         long long tot = 1;
         for (int d = 0; d < 3; ++d) {
-            int n = (int)floor(w[d] / (rc * 1.000001 * (1.0 + slack) * shrink));
+            int n = (int)floor(w[d] / (rcl * 1.000001 * (1.0 + slack) * shrink));
             g.nc[d] = n < 1 ? 1 : n;
             tot *= g.nc[d];
         }
@@ -314,15 +326,21 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc, double sla
     g.inv[0] = 1.0 / ax; g.inv[1] = 1.0 / by; g.inv[2] = 1.0 / cz;
     g.inv[3] = g.inv[4] = g.inv[5] = 0.0;
     g.cx = cx; g.cy = cy; g.bx = bx;
-    c->grid = g;
     BoxD b = { ax, bx, by, cx, cy, cz, 0.5 * ax, 0.5 * by, 0.5 * cz };
+    // a changed cell grid or cutoff invalidates a kept list: the next step rebuilds (set outside any capture: run_impl calls
+    // this function before it starts one)
+    if (c->skin_on && !c->capturing && (c->rc != rc || c->geom_ncell != g.ncell || memcmp(&c->boxd, &b, sizeof(b)) != 0)) {
+        const int ones[2] = { 1, 1 };
+        cudaMemcpyAsync(c->d_skin_flag, ones, sizeof(ones), cudaMemcpyHostToDevice, c->stream);
+    }
+    c->grid = g; c->geom_ncell = g.ncell;
     c->boxd = b;
-    c->rc = rc; c->rc2 = rc * rc;
+    c->rc = rc; c->rc2 = rc * rc; c->rcl = rcl; c->rcl2 = rcl * rcl;
     // shared-memory tiled fast path: fp32, neighbour-list CVs = Q6 only or an ungrouped coordination number only,
     // >= 3 cells per direction
     c->tiled = 0;
     const bool q6_only = c->has_q6 && !c->has_coord;
-    const bool coord_only = c->has_coord && !c->has_q6 && !c->cv[c->coord_dim].use_groups;
+    const bool coord_only = c->has_coord && !c->has_q6 && !c->cv[c->coord_dim].use_groups && !c->skin_on;
     if (c->prec == 32 && (q6_only || coord_only) && !c->has_mindist && c->N < (1 << NL_IDX_BITS) && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32) {
         // the rc-wide cells are subdivided along x (the direction of the contiguous row runs): an atom then scans
         // 2 xsub + 1 sub-cells per row (2.5 / 2.25 cell widths for xsub = 2 / 4) instead of 3 cells
@@ -721,6 +739,13 @@ extern "C" int metad_get_timing(metad_ctx *c, float *ms_sort, float *ms_list) {
 }
 
 extern "C" long long metad_launch_count(metad_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" int metad_get_rebuilds(metad_ctx *c, int *h_count) {
+    if (!c || !h_count) FAIL(METAD_ERR_ARG, "null argument");
+    CUDA_TRY(cudaMemcpyAsync(h_count, c->d_nbuilds, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return METAD_OK;
+}
 
 extern "C" int metad_synchronize(metad_ctx *c) {
     if (!c) FAIL(METAD_ERR_ARG, "null argument");

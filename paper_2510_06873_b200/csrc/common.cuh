@@ -99,6 +99,34 @@ __device__ __forceinline__ double r2_shifted(const RunShift &w, double dx, doubl
     return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
 }
 
+// Neighbour decision of a pair of cell-sorted atoms in precision T (reading O).  fp64: the canonical predicate.  fp32: fast
+// test; any pair within the recheck band of rc^2 is re-decided with the canonical fp64 arithmetic on the (exactly
+// representable) fp32 coordinates, so the sets are identical to the fp64 definition.
+template <typename T>
+__device__ __forceinline__ bool pair_in_range(const PBox<T> &pb, const BoxD &bd, T rc2T, double rc2,
+                                              const typename Vec4<T>::type &pi, const typename Vec4<T>::type &pj);
+template <>
+__device__ __forceinline__ bool pair_in_range<double>(const PBox<double> &, const BoxD &bd, double, double rc2,
+                                                      const double4 &pi, const double4 &pj) {
+    return r2_canonical(bd, pj.x - pi.x, pj.y - pi.y, pj.z - pi.z) < rc2;
+}
+template <>
+__device__ __forceinline__ bool pair_in_range<float>(const PBox<float> &pb, const BoxD &bd, float rc2T, double rc2,
+                                                     const float4 &pi, const float4 &pj) {
+    float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+    min_image(pb, dx, dy, dz);
+    float r2 = dx * dx + dy * dy + dz * dz;
+    bool in = r2 < rc2T;
+    if (fabsf(r2 - rc2T) <= pb.band)
+        in = r2_canonical(bd, (double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y,
+                          (double)pj.z - (double)pi.z) < rc2;
+    return in;
+}
+
+// Verlet-skin reuse (params.skin): the build kernels of a step do nothing unless the step's rebuild flag is set
+// (k_skin_check, neighbor.cu); flag == NULL: no skin, always build
+#define SKIN_SKIP(flag, step) ((flag) != nullptr && (flag)[*(step) & 1] == 0)
+
 // fp64 minimum image in the order of reading O (chain / torsion CVs, fused small-molecule step)
 __device__ __forceinline__ void min_image_d(const BoxD &b, double &dx, double &dy, double &dz) {
     if (dz > b.hz) { dx -= b.cx; dy -= b.cy; dz -= b.cz; }
@@ -203,7 +231,14 @@ struct metad_ctx {
     // neighbour / cell state
     CellGrid grid;
     BoxD boxd;
-    double rc, rc2;
+    double rc, rc2;                       // CV cutoff
+    double rcl, rcl2;                     // list cutoff rc + skin (== rc without a skin): cells, list build
+    int skin_on;                          // params.skin > 0 and a CV of the context reads the list
+    int geom_ncell;                       // cells of the last setup_geometry before any x-subdivision (skin: detects a new grid)
+    int *d_skin_flag;                     // [2] rebuild flags, indexed by the parity of the device step counter (neighbor.cu)
+    void *d_ref;                          // Vec4<T>[N]: cell-sorted positions at the last build (displacement check)
+    unsigned long long *d_keep_mask;      // skin, tiled Q6 path: per atom, which entries of the kept list lie within rc this step
+    int *d_nbuilds;                       // number of neighbour-list builds so far (metad_get_rebuilds)
     bool have_neighbors, list_built;
     int cell_cap;
     int *d_cell_count, *d_cell_start, *d_block_sums;
@@ -279,6 +314,8 @@ static inline int div_up(long long a, int b) { return (int)((a + b - 1) / b); }
 // stage entry points implemented in the .cu files (host functions that enqueue kernels)
 int nb_build(metad_ctx *c, const void *d_pos);
 int geom_update(metad_ctx *c, const double *d_box);
+int skin_check(metad_ctx *c, const void *d_pos);
+int tiled_q6_pass1_skin(metad_ctx *c, double *d_cv);
 int nb_export(metad_ctx *c, int *d_count, int *d_list);
 int cv_eval_all(metad_ctx *c, double *d_cv);
 int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F);
@@ -304,4 +341,3 @@ int tiled_build(metad_ctx *c);
 int tiled_q6_pass1(metad_ctx *c, double *d_cv);
 int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F);
 int tiled_coord_force(metad_ctx *c, const double *d_dVds, void *d_F);
-int tiled_export(metad_ctx *c, int *d_count, int *d_list);

@@ -14,11 +14,11 @@ template <typename T> PBox<T> ctx_pbox(const metad_ctx *c);
 template <typename T>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-           const int *__restrict__ nl, PBox<T> pb, T inv_r0, int n, int m, double scale,
+           const int *__restrict__ nl, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, T inv_r0, int n, int m, double scale,
            double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
            unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
     __shared__ double red[32];
-    if (dg) pb = dg_pb<T>(dg);
+    if (dg) { pb = dg_pb<T>(dg); bdk = dg->bd; }
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     T acc = T(0);
     if (s < N) {
@@ -29,6 +29,7 @@ k_coord_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
                 int j = nl[(size_t)k * N + s];
                 typename Vec4<T>::type pj = spos[j];
                 if (!(((int)pj.w) & 2)) continue;
+                if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
                 T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
                 min_image(pb, dx, dy, dz);
                 T r = sqrt(dx * dx + dy * dy + dz * dz), dsw;
@@ -56,11 +57,11 @@ k_coord_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
 template <typename T, bool VIRIAL>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-              const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, T inv_r0, int n, int m,
+              const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, T inv_r0, int n, int m,
               double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F, VirArgs va,
               const DevGeom *__restrict__ dg) {
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
-    if (dg) pb = dg_pb<T>(dg);
+    if (dg) { pb = dg_pb<T>(dg); bdk = dg->bd; }
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (!VIRIAL && s >= N) return;
     const bool act = s < N;
@@ -78,6 +79,7 @@ k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int 
         const int fj = (int)pj.w;
         int mult = ((fi & 1) && (fj & 2)) + ((fi & 2) && (fj & 1));
         if (!mult) continue;
+        if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
         T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         min_image(pb, dx, dy, dz);
         T r = sqrt(dx * dx + dy * dy + dz * dz), dsw;
@@ -112,11 +114,11 @@ k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int 
 template <typename T, int G>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-                const int *__restrict__ nl, PBox<T> pb, T inv_r0, int n, int m, double scale,
+                const int *__restrict__ nl, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, T inv_r0, int n, int m, double scale,
                 double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
                 unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
     __shared__ double red[32];
-    if (dg) pb = dg_pb<T>(dg);
+    if (dg) { pb = dg_pb<T>(dg); bdk = dg->bd; }
     const int gt = blockIdx.x * blockDim.x + threadIdx.x;
     const int s = gt / G, lane = gt % G;
     T acc = T(0);
@@ -128,6 +130,7 @@ k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const in
                 const int j = nl[(size_t)k * N + s];
                 typename Vec4<T>::type pj = spos[j];
                 if (!(((int)pj.w) & 2)) continue;
+                if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
                 T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
                 min_image(pb, dx, dy, dz);
                 T r = sqrt(dx * dx + dy * dy + dz * dz), dsw;
@@ -153,13 +156,13 @@ k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const in
 template <typename T, int G>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_force_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-                   const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, T inv_r0, int n, int m,
+                   const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, T inv_r0, int n, int m,
                    double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F,
                    const DevGeom *__restrict__ dg) {
     const int gt = blockIdx.x * blockDim.x + threadIdx.x;
     const int s = gt / G, lane = gt % G;
     if (s >= N) return;
-    if (dg) pb = dg_pb<T>(dg);
+    if (dg) { pb = dg_pb<T>(dg); bdk = dg->bd; }
     const unsigned gmask = G == 32 ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
     typename Vec4<T>::type pi = spos[s];
     const int fi = (int)pi.w;
@@ -171,6 +174,7 @@ k_coord_force_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const
         const int fj = (int)pj.w;
         const int mult = ((fi & 1) && (fj & 2)) + ((fi & 2) && (fj & 1));
         if (!mult) continue;
+        if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
         T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         min_image(pb, dx, dy, dz);
         T r = sqrt(dx * dx + dy * dy + dz * dz), dsw;
@@ -198,12 +202,12 @@ k_coord_force_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const
 template <typename T>
 __global__ void __launch_bounds__(CV_THREADS)
 k_q6_pass1(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-           const int *__restrict__ nl, PBox<T> pb, T q_thresh, T inv_width, T *__restrict__ rec,
+           const int *__restrict__ nl, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, T q_thresh, T inv_width, T *__restrict__ rec,
            double scale_mean, double scale_solid, int dim_mean, int dim_solid,
            double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
            unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
     __shared__ double red[64];
-    if (dg) pb = dg_pb<T>(dg);
+    if (dg) { pb = dg_pb<T>(dg); bdk = dg->bd; }
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     double v[2] = { 0.0, 0.0 };
     if (s < N) {
@@ -211,10 +215,13 @@ k_q6_pass1(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
         T A[13];
 #pragma unroll
         for (int k = 0; k < 13; ++k) A[k] = T(0);
-        int cnt = nl_count[s];
-        for (int k = 0; k < cnt; ++k) {
+        const int nlist = nl_count[s];
+        int cnt = 0;                                     // neighbours within rc (== nlist unless a skin keeps a longer list)
+        for (int k = 0; k < nlist; ++k) {
             int j = nl[(size_t)k * N + s];
             typename Vec4<T>::type pj = spos[j];
+            if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
+            ++cnt;
             T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
             min_image(pb, dx, dy, dz);
             T rinv = T(1) / sqrt(dx * dx + dy * dy + dz * dz);
@@ -276,11 +283,11 @@ k_q6_pass1(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
 template <typename T, bool VIRIAL>
 __global__ void __launch_bounds__(CV_THREADS)
 k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-           const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, const T *__restrict__ rec,
+           const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, const T *__restrict__ rec,
            double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
            const double *__restrict__ dVds, T *__restrict__ F, VirArgs va, const DevGeom *__restrict__ dg) {
     typedef typename Vec4<T>::type V4;
-    if (dg) pb = dg_pb<T>(dg);
+    if (dg) { pb = dg_pb<T>(dg); bdk = dg->bd; }
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (!VIRIAL && s >= N) return;
@@ -307,6 +314,7 @@ k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
     for (int k = 0; k < cnt; ++k) {
         int j = nl[(size_t)k * N + s];
         V4 pj = spos[j];
+        if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
         const V4 *r4 = reinterpret_cast<const V4 *>(rec + (size_t)j * METAD_NREC);
         V4 a = r4[0], b = r4[1], c = r4[2], d = r4[3];
         T gj = alpha + beta * d.y;
@@ -360,14 +368,18 @@ __device__ __forceinline__ void ldg256(const float *p, float4 &a, float4 &b) {
 }
 
 #define Q6F_MINB 9             // resident blocks per SM of k_q6_force_g (56 registers)
-template <bool SOLID, bool VIRIAL, bool DEVBOX>   // DEVBOX: box in device memory (metad_*_dev); the other instances never touch dg
+// SKIN (params.skin): the kept list reaches rc + skin and a neighbour may have crossed a box face since it was built, so the
+// shift codes are ignored: per-pair minimum image on the current positions; pairs beyond rc are skipped by the keep mask that
+// pass 1 (k_q6_pass1_g) wrote for this step, before their records are gathered.
+template <bool SOLID, bool VIRIAL, bool DEVBOX, bool SKIN>   // DEVBOX: box in device memory (metad_*_dev); the other instances never touch dg
 __global__ void __launch_bounds__(CV_THREADS, VIRIAL ? 8 : Q6F_MINB)
 k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
              const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, const float *__restrict__ rec,
              double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
              const double *__restrict__ dVds, float *__restrict__ F, VirArgs va, const float *__restrict__ fprime,
-             const DevGeom *__restrict__ dg_arg) {
+             const DevGeom *__restrict__ dg_arg, PBox<float> pb, const unsigned long long *__restrict__ keep_mask) {
     const DevGeom *dg = DEVBOX ? dg_arg : nullptr;
+    if (SKIN && DEVBOX && dg) pb = dg->pbf;
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (!VIRIAL && s >= N) return;
@@ -397,17 +409,21 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
     // the list entries are fetched two iterations ahead: an entry load (streamed from DRAM) followed by the dependent record
     // gather was 40 % of the stall samples of this kernel (profiles/r1w_ncu.md)
     int e0 = cnt > 0 ? __ldcs(in) : 0, e1 = cnt > 1 ? __ldcs(in + 32) : 0;
+    const unsigned long long km = SKIN && act ? keep_mask[s] : ~0ull;     // skin: which entries of the kept list lie within rc (pass 1)
     for (int k = 0; k < cnt; ++k) {
         const int e = e0;                              // streamed once: do not displace positions / records in L2
         e0 = e1;
         if (k + 2 < cnt) e1 = __ldcs(in + (k + 2) * 32);
+        if (SKIN && !((km >> k) & 1ull)) continue;
         const int j = e & NLG_IDX_MASK, code = (unsigned)e >> 27;
         float4 a4, b4, c4, d4, pj;
         ldg256(rec + (size_t)j * 8, a4, b4);
         ldg256(recB + (size_t)j * 8, c4, d4);
         pj.x = d4.y; pj.y = d4.z; pj.z = d4.w;               // the record carries the position
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-        if (code != 13) {
+        if (SKIN) {
+            min_image(pb, dx, dy, dz);                 // the decision r < rc was taken by pass 1 (keep_mask), on these positions
+        } else if (code != 13) {
             const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
             const BoxD &b = dg ? dg->bd : bd;                  // device-resident box (NPT): read at the rare point of use
             dx = (float)(((double)pj.x - (double)pi.x) + (wx * b.ax + wy * b.bx + wz * b.cx));
@@ -447,6 +463,103 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         for (int q = 0; q < 9; ++q) w[q] = (double)wv[q];
         virial_finish(w, vsm, va, -0.5 * force_scale, nullptr);
     }
+}
+
+// Q6 pass 1 from the KEPT list of the tiled fp32 path (params.skin): thread per atom over the sliced list, one 128-bit
+// position gather per entry, per-pair minimum image (shift codes ignored, see k_q6_force_g), pairs beyond rc skipped with the
+// canonical decision inside the recheck band; writes the same split records, per-atom q6 and f'(q6) as the fused pass of
+// k_tile_build and finishes the global sums in its last block.
+template <bool DEVBOX>
+__global__ void __launch_bounds__(CV_THREADS, 10)
+k_q6_pass1_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count, const int *__restrict__ nl,
+             PBox<float> pb, BoxD bd, float rc2f, double rc2, float q_thresh, float inv_width, float *__restrict__ rec,
+             float *__restrict__ q6_out, int solid, double scale_mean, double scale_solid, double *__restrict__ partials,
+             unsigned int *__restrict__ ticket, double *__restrict__ cv_q6, double *__restrict__ cv_out, int dim0, int dim1,
+             unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg,
+             unsigned long long *__restrict__ keep_mask /* bit k: list entry k of the atom lies within rc (read by the force pass) */) {
+    __shared__ double red[64];
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (DEVBOX) pb = dg->pbf;                      // host-box instance: the box stays in the constant bank
+    double v[2] = { 0.0, 0.0 };
+    if (s < N) {
+        const float4 pi = spos[s];
+        const int *in = nl + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
+        const int cnt = nl_count[s];
+        float A[13];
+#pragma unroll
+        for (int k = 0; k < 13; ++k) A[k] = 0.f;
+        int n = 0;
+        unsigned long long km = 0ull;
+        // entries two iterations ahead, as in k_q6_force_g: the entry load -> position gather chain is the latency to hide
+        int e0 = cnt > 0 ? __ldg(in) : 0, e1 = cnt > 1 ? __ldg(in + 32) : 0;
+        for (int k = 0; k < cnt; ++k) {
+            const int j = e0 & NLG_IDX_MASK;
+            e0 = e1;
+            if (k + 2 < cnt) e1 = __ldg(in + (k + 2) * 32);
+            const float4 pj = spos[j];
+            float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+            min_image(pb, dx, dy, dz);
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            bool keep = r2 < rc2f;
+            if (fabsf(r2 - rc2f) <= pb.band)
+                keep = r2_canonical(DEVBOX ? dg->bd : bd, (double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y,
+                                    (double)pj.z - (double)pi.z) < rc2;
+            if (!keep) continue;
+            ++n;
+            km |= 1ull << k;
+            const float rinv = rsqrtf(r2);
+            Y6<float> y;
+            y6_eval<float>(dx * rinv, dy * rinv, dz * rinv, y);
+            A[0] += y.E[0];
+#pragma unroll
+            for (int m = 1; m <= 6; ++m) { A[2 * m - 1] += y.E[m] * y.c[m]; A[2 * m] += y.E[m] * y.s[m]; }
+        }
+        keep_mask[s] = km;
+        float S = 0.f;
+#pragma unroll
+        for (int k = 0; k < 13; ++k) S += A[k] * A[k];
+        float q6 = 0.f, norm = 0.f;
+        if (n > 0 && S > 0.f) { const float rs = sqrtf(S); q6 = rs / (float)n; norm = 1.f / ((float)n * rs); }
+        float4 *r4 = reinterpret_cast<float4 *>(rec + (size_t)s * 8);                      // split record layout of tiled.cu
+        float4 *r4b = reinterpret_cast<float4 *>(rec + (size_t)N * 8 + (size_t)s * 8) - 2;
+        r4[0] = make_float4(A[0] * norm, A[1] * norm, -A[2] * norm, A[3] * norm);
+        r4[1] = make_float4(-A[4] * norm, A[5] * norm, -A[6] * norm, A[7] * norm);
+        r4b[2] = make_float4(-A[8] * norm, A[9] * norm, -A[10] * norm, A[11] * norm);
+        r4b[3] = make_float4(-A[12] * norm, pi.x, pi.y, pi.z);
+        const float f = 1.f / (1.f + expf(-(q6 - q_thresh) * inv_width));
+        if (solid) q6_out[(size_t)N + s] = f * (1.f - f) * inv_width;
+        q6_out[s] = q6;
+        v[0] = (double)q6; v[1] = (double)f;
+    }
+    block_reduce<2>(v, red);
+    if (threadIdx.x == 0) { partials[2 * blockIdx.x] = v[0]; partials[2 * blockIdx.x + 1] = v[1]; }
+    if (last_block_ticket(ticket)) {
+        double u[2] = { 0.0, 0.0 };
+        for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) { u[0] += partials[2 * b]; u[1] += partials[2 * b + 1]; }
+        block_reduce<2>(u, red);
+        if (threadIdx.x == 0) {
+            cv_q6[0] = scale_mean * u[0]; cv_q6[1] = scale_solid * u[1];
+            if (dim0 >= 0) cv_out[dim0] = cv_q6[0];
+            if (dim1 >= 0) cv_out[dim1] = cv_q6[1];
+            if (!isfinite(cv_q6[0]) || !isfinite(cv_q6[1])) atomicOr(sticky, (unsigned)METAD_DEV_NONFINITE);
+        }
+    }
+}
+
+int tiled_q6_pass1_skin(metad_ctx *c, double *d_cv) {
+    const double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
+    const double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
+#define P1G_ARGS                                                                                                           \
+    c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, ctx_pbox<float>(c), c->boxd, (float)c->rc2, c->rc2,  \
+        (float)qt, (float)(1.0 / qw), (float *)c->d_rec, c->d_q6, c->q6_solid_dim >= 0 ? 1 : 0,                            \
+        c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0, c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0, \
+        c->d_partials + c->nblocks_atoms, c->d_tickets + 1, c->d_cvq6, d_cv, c->q6_mean_dim, c->q6_solid_dim, c->d_sticky, c->dg, c->d_keep_mask
+    if (c->dg) k_q6_pass1_g<true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(P1G_ARGS);
+    else k_q6_pass1_g<false><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(P1G_ARGS);
+#undef P1G_ARGS
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
 }
 
 // Coordination-number forces on the tiled fp32 path (ungrouped: every ordered pair counts, i.e. each pair twice in
@@ -574,15 +687,20 @@ int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
 #define Q6FG_ARGS                                                                                                          \
     c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm, ss,  \
-        c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va, c->d_q6 + c->N, c->dg
+        c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va, c->d_q6 + c->N, c->dg, ctx_pbox<float>(c),    \
+        c->d_keep_mask
+#define Q6FG_GRID <<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>
 #define Q6FG_LAUNCH(SOLID, VIR)                                                                                            \
     do {                                                                                                                   \
-        if (c->dg) k_q6_force_g<SOLID, VIR, true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(Q6FG_ARGS);      \
-        else k_q6_force_g<SOLID, VIR, false><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(Q6FG_ARGS);           \
+        if (c->dg && c->skin_on) k_q6_force_g<SOLID, VIR, true, true> Q6FG_GRID(Q6FG_ARGS);                                \
+        else if (c->dg) k_q6_force_g<SOLID, VIR, true, false> Q6FG_GRID(Q6FG_ARGS);                                        \
+        else if (c->skin_on) k_q6_force_g<SOLID, VIR, false, true> Q6FG_GRID(Q6FG_ARGS);                                   \
+        else k_q6_force_g<SOLID, VIR, false, false> Q6FG_GRID(Q6FG_ARGS);                                                  \
     } while (0)
     if (c->q6_solid_dim >= 0) { if (c->p.want_virial) Q6FG_LAUNCH(true, true); else Q6FG_LAUNCH(true, false); }
     else { if (c->p.want_virial) Q6FG_LAUNCH(false, true); else Q6FG_LAUNCH(false, false); }
 #undef Q6FG_LAUNCH
+#undef Q6FG_GRID
 #undef Q6FG_ARGS
     c->launches++;
     CUDA_TRY(cudaGetLastError());
@@ -620,14 +738,14 @@ __device__ __forceinline__ void min_warp(double &r2, long long &ij, int &sj, int
 template <typename T>
 __global__ void __launch_bounds__(CV_THREADS)
 k_mindist_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-             const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, double rc,
+             const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, double rc,
              double *__restrict__ part_r2, long long *__restrict__ part_ij, int *__restrict__ part_s /* [2*nblocks] */,
              unsigned int *__restrict__ ticket, double *__restrict__ rec /* [r, dx, dy, dz, (i, j) as two ints] */,
              double *__restrict__ cv_out, const DevGeom *__restrict__ dg) {
     __shared__ double s_r2[32];
     __shared__ long long s_ij[32];
     __shared__ int s_sj[32], s_si[32];
-    if (dg) pb = dg_pb<T>(dg);
+    if (dg) { pb = dg_pb<T>(dg); bdk = dg->bd; }
     const int s = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     double r2 = 1e300; long long ij = 0x7fffffffffffffffll; int sj = -1, si = -1;
     if (s < N) {
@@ -639,6 +757,7 @@ k_mindist_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *
                 const int j = nl[(size_t)k * N + s];
                 const typename Vec4<T>::type pj = spos[j];
                 if (!(((int)pj.w) & 2)) continue;
+                if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
                 T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
                 min_image(pb, dx, dy, dz);
                 const double q = (double)(dx * dx + dy * dy + dz * dz);
@@ -771,7 +890,7 @@ static int mindist_eval_t(metad_ctx *c, double *d_cv) {
     double *pr = c->d_partials;
     long long *pk = reinterpret_cast<long long *>(c->d_partials + c->nblocks_atoms);
     int *ps = reinterpret_cast<int *>(c->d_partials + 2 * (size_t)c->nblocks_atoms);
-    k_mindist_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(c->N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, ctx_pbox<T>(c),
+    k_mindist_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(c->N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, ctx_pbox<T>(c), c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0,
                                                      c->rc, pr, pk, ps, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim, c->dg);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
@@ -823,23 +942,23 @@ static int cv_eval_t(metad_ctx *c, double *d_cv) {
         const CvDev &d = c->cv[c->coord_dim];
         if (N <= METAD_WARP_PER_ATOM_MAX)
             k_coord_cv_warp<T, 32><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
-                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials_warp,
+                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials_warp,
                 c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky, c->dg);
         else
-        k_coord_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb,
+        k_coord_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0,
                                                        (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials,
                                                        c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky, c->dg);
         c->launches++;
     }
     if (c->has_q6 && c->tiled) {
-        int r = tiled_q6_pass1(c, d_cv);
+        int r = c->skin_on ? tiled_q6_pass1_skin(c, d_cv) : tiled_q6_pass1(c, d_cv);
         if (r) return r;
     } else if (c->has_q6) {
         double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;
         double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
         double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
         double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
-        k_q6_pass1<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, (T)qt,
+        k_q6_pass1<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)qt,
                                                        (T)(1.0 / qw), (T *)c->d_rec, sm, ss, c->q6_mean_dim,
                                                        c->q6_solid_dim, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
                                                        d_cv, c->d_sticky, c->dg);
@@ -879,19 +998,19 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
         const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
         if (c->p.want_virial)                                 // forces and virial in one thread-per-atom pass
             k_coord_force<T, true><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
-                                                                    pb, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
+                                                                    pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
                                                                     d_dVds + c->coord_dim, (T *)d_F, va, c->dg);
         else if (N <= METAD_WARP_PER_ATOM_MAX)
             k_coord_force_warp<T, 32><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
-                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, (T)(1.0 / d.r0), d.n, d.m,
+                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)(1.0 / d.r0), d.n, d.m,
                 c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F, c->dg);
         else if (d.use_groups && N <= 8 * METAD_WARP_PER_ATOM_MAX)
             k_coord_force_warp<T, 8><<<div_up((long long)N * 8, CV_THREADS), CV_THREADS, 0, c->stream>>>(
-                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, (T)(1.0 / d.r0), d.n, d.m,
+                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)(1.0 / d.r0), d.n, d.m,
                 c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F, c->dg);
         else
             k_coord_force<T, false><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
-                                                                     pb, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
+                                                                     pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
                                                                      d_dVds + c->coord_dim, (T *)d_F, va, c->dg);
         c->launches++;
     }
@@ -903,11 +1022,11 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
         double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
         const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
         if (c->p.want_virial)
-            k_q6_force<T, true><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb,
+            k_q6_force<T, true><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0,
                                                                  (const T *)c->d_rec, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
                                                                  c->p.force_scale, d_dVds, (T *)d_F, va, c->dg);
         else
-            k_q6_force<T, false><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb,
+            k_q6_force<T, false><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0,
                                                                   (const T *)c->d_rec, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
                                                                   c->p.force_scale, d_dVds, (T *)d_F, va, c->dg);
         c->launches++;

@@ -17,9 +17,9 @@
 template <typename T>
 __global__ void k_bin(int N, const T *__restrict__ pos, CellGrid g, int *__restrict__ cell_of,
                       int *__restrict__ slot, int *__restrict__ cell_count, unsigned int *__restrict__ sticky,
-                      const DevGeom *__restrict__ dg) {
+                      const DevGeom *__restrict__ dg, const int *__restrict__ skin_flag, const int *__restrict__ step) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
+    if (i >= N || SKIN_SKIP(skin_flag, step)) return;
     if (dg) { g.inv[0] = dg->inv[0]; g.inv[1] = dg->inv[1]; g.inv[2] = dg->inv[2]; g.cx = dg->cx; g.cy = dg->cy; g.bx = dg->bx; }
     double x = (double)pos[3 * i], y = (double)pos[3 * i + 1], z = (double)pos[3 * i + 2];
     double sc = z * g.inv[2];
@@ -38,8 +38,10 @@ __global__ void k_bin(int N, const T *__restrict__ pos, CellGrid g, int *__restr
     slot[i] = atomicAdd(&cell_count[c], 1);
 }
 
-__global__ void k_scan_sums(int ncell, const int *__restrict__ cell_count, int *__restrict__ block_sums) {
+__global__ void k_scan_sums(int ncell, const int *__restrict__ cell_count, int *__restrict__ block_sums,
+                            const int *__restrict__ skin_flag, const int *__restrict__ step) {
     __shared__ int ws[32];
+    if (SKIN_SKIP(skin_flag, step)) return;
     int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
     int s = 0;
 #pragma unroll
@@ -58,9 +60,10 @@ __global__ void k_scan_sums(int ncell, const int *__restrict__ cell_count, int *
 
 // exclusive scan; also zeroes the histogram for the next step and writes cell_start[ncell] = N
 __global__ void k_scan_apply(int ncell, int N, int *__restrict__ cell_count, const int *__restrict__ block_sums,
-                             int *__restrict__ cell_start) {
+                             int *__restrict__ cell_start, const int *__restrict__ skin_flag, const int *__restrict__ step) {
     __shared__ int ws[32];
     __shared__ int s_prefix;
+    if (SKIN_SKIP(skin_flag, step)) return;
     // prefix of the preceding blocks' sums
     int pre = 0;
     for (int b = threadIdx.x; b < (int)blockIdx.x; b += blockDim.x) pre += block_sums[b];
@@ -117,9 +120,10 @@ __global__ void k_scan_apply(int ncell, int N, int *__restrict__ cell_count, con
 }
 
 __global__ void k_scatter(int N, const int *__restrict__ cell_of, const int *__restrict__ slot,
-                          const int *__restrict__ cell_start, int *__restrict__ perm) {
+                          const int *__restrict__ cell_start, int *__restrict__ perm,
+                          const int *__restrict__ skin_flag, const int *__restrict__ step) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
+    if (i >= N || SKIN_SKIP(skin_flag, step)) return;
     perm[cell_start[cell_of[i]] + slot[i]] = i;
 }
 
@@ -130,9 +134,12 @@ template <typename T>
 __global__ void k_cell_sort_gather(int N, const int *__restrict__ cell_start, const int *__restrict__ cell_of,
                                    const int *__restrict__ perm_in, int *__restrict__ perm,
                                    const T *__restrict__ pos, const unsigned char *__restrict__ flags,
-                                   typename Vec4<T>::type *__restrict__ spos, int *__restrict__ scell, int index_in_w) {
+                                   typename Vec4<T>::type *__restrict__ spos, int *__restrict__ scell, int index_in_w,
+                                   typename Vec4<T>::type *__restrict__ ref /* skin: positions at the build, else NULL */,
+                                   const int *__restrict__ skin_flag, const int *__restrict__ step, int *__restrict__ nbuilds) {
     int a = blockIdx.x * blockDim.x + threadIdx.x;
-    if (a >= N) return;
+    if (a >= N || SKIN_SKIP(skin_flag, step)) return;
+    if (a == 0 && nbuilds) ++*nbuilds;            // list builds so far (metad_get_rebuilds)
     const int i = perm_in[a], c = cell_of[i];
     const int b = cell_start[c], e = cell_start[c + 1];
     int rank = 0;
@@ -146,34 +153,8 @@ __global__ void k_cell_sort_gather(int N, const int *__restrict__ cell_start, co
     if (index_in_w && sizeof(T) == 4) v.w = (T)__int_as_float(d | (13 << 27));
     perm[d] = i;
     spos[d] = v;
+    if (ref) ref[d] = v;
     scell[d] = c;
-}
-
-template <typename T>
-__device__ __forceinline__ bool pair_in_range(const PBox<T> &pb, const BoxD &bd, T rc2T, double rc2,
-                                              const typename Vec4<T>::type &pi,
-                                              const typename Vec4<T>::type &pj);
-
-template <>
-__device__ __forceinline__ bool pair_in_range<double>(const PBox<double> &, const BoxD &bd, double, double rc2,
-                                                      const double4 &pi, const double4 &pj) {
-    return r2_canonical(bd, pj.x - pi.x, pj.y - pi.y, pj.z - pi.z) < rc2;
-}
-
-// fp32: fast test; any pair within a relative band of 1e-5 of rc^2 is re-decided with the canonical
-// fp64 arithmetic on the (exactly representable) fp32 coordinates, so the sets are identical to the
-// fp64 definition (reading O).
-template <>
-__device__ __forceinline__ bool pair_in_range<float>(const PBox<float> &pb, const BoxD &bd, float rc2T, double rc2,
-                                                     const float4 &pi, const float4 &pj) {
-    float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-    min_image(pb, dx, dy, dz);
-    float r2 = dx * dx + dy * dy + dz * dz;
-    bool in = r2 < rc2T;
-    if (fabsf(r2 - rc2T) <= pb.band)
-        in = r2_canonical(bd, (double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y,
-                          (double)pj.z - (double)pi.z) < rc2;
-    return in;
 }
 
 // fp64 contexts on a grid with >= 3 cells per direction take the per-run form of the predicate (common.cuh: r2_shifted)
@@ -190,9 +171,9 @@ __global__ void __launch_bounds__(128)
 k_build_list(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ scell,
              const int *__restrict__ cell_start, CellGrid g, PBox<T> pb, BoxD bd, T rc2T, double rc2, int maxn,
              int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
-             const DevGeom *__restrict__ dg) {
+             const DevGeom *__restrict__ dg, const int *__restrict__ skin_flag, const int *__restrict__ step) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
+    if (s >= N || SKIN_SKIP(skin_flag, step)) return;
     if (dg) { pb = dg_pb<T>(dg); bd = dg->bd; }
     typename Vec4<T>::type pi = spos[s];
     int c = scell[s];
@@ -243,11 +224,11 @@ __global__ void __launch_bounds__(128)
 k_build_list_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ scell,
                   const int *__restrict__ cell_start, CellGrid g, PBox<T> pb, BoxD bd, T rc2T, double rc2, int maxn,
                   int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
-                  const DevGeom *__restrict__ dg) {
+                  const DevGeom *__restrict__ dg, const int *__restrict__ skin_flag, const int *__restrict__ step) {
     // G lanes per atom (G = 32: one warp per atom; G = 8: four atoms per warp, each group votes under its own mask)
     const int gt = blockIdx.x * blockDim.x + threadIdx.x;
     const int s = gt / G, lane = gt % G;
-    if (s >= N) return;
+    if (s >= N || SKIN_SKIP(skin_flag, step)) return;
     if (dg) { pb = dg_pb<T>(dg); bd = dg->bd; }
     const unsigned gmask = G == 32 ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
     const int gshift = (threadIdx.x & 31) / G * G;
@@ -311,9 +292,11 @@ __global__ void __launch_bounds__(128)
 k_build_list_small(int N, const T *__restrict__ pos, const unsigned char *__restrict__ flags,
                    typename Vec4<T>::type *__restrict__ spos, int *__restrict__ perm, int *__restrict__ scell,
                    PBox<T> pb, BoxD bd, T rc2T, double rc2, int maxn, int *__restrict__ nl_count, int *__restrict__ nl,
-                   CellGrid g, unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
+                   CellGrid g, unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg,
+                   typename Vec4<T>::type *__restrict__ ref, const int *__restrict__ skin_flag, const int *__restrict__ step,
+                   int *__restrict__ nbuilds) {
     const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (s >= N) return;
+    if (s >= N || SKIN_SKIP(skin_flag, step)) return;
     if (dg) {
         pb = dg_pb<T>(dg); bd = dg->bd;
         g.inv[0] = dg->inv[0]; g.inv[1] = dg->inv[1]; g.inv[2] = dg->inv[2]; g.cx = dg->cx; g.cy = dg->cy; g.bx = dg->bx;
@@ -323,6 +306,8 @@ k_build_list_small(int N, const T *__restrict__ pos, const unsigned char *__rest
     pi.w = (T)(flags ? (int)flags[s] : 3);
     if (lane == 0) {
         spos[s] = pi; perm[s] = s; scell[s] = 0;
+        if (ref) ref[s] = pi;
+        if (s == 0 && nbuilds) ++*nbuilds;
         // positions must lie in the primary cell (same check as k_bin)
         const double sc = (double)pi.z * g.inv[2], sb = ((double)pi.y - sc * g.cy) * g.inv[1],
                      sa = ((double)pi.x - sb * g.bx - sc * g.cx) * g.inv[0];
@@ -351,13 +336,30 @@ k_build_list_small(int N, const T *__restrict__ pos, const unsigned char *__rest
     }
 }
 
+// metad_get_neighbors: the list in ORIGINAL atom indices.  With a skin the kept list reaches rc + skin; the export applies
+// the canonical fp64 predicate (reading O) on the current cell-sorted coordinates, so the caller sees the exact rc list.
+// sliced: layout of the tiled path ([N/32][maxn][32], entries carry a shift code) or of the generic path (nl[k N + s]).
+template <typename T>
 __global__ void k_export_list(int N, int maxn, const int *__restrict__ perm, const int *__restrict__ nl_count,
-                              const int *__restrict__ nl, int *__restrict__ out_count, int *__restrict__ out_list) {
+                              const int *__restrict__ nl, int *__restrict__ out_count, int *__restrict__ out_list, int sliced,
+                              const typename Vec4<T>::type *__restrict__ spos, BoxD bd, double rc2, int skin,
+                              const DevGeom *__restrict__ dg) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= N) return;
-    int i = perm[s], cnt = nl_count[s];
-    out_count[i] = cnt;
-    for (int k = 0; k < maxn; ++k) out_list[(size_t)i * maxn + k] = k < cnt ? perm[nl[(size_t)k * N + s]] : -1;
+    if (dg) bd = dg->bd;
+    const int i = perm[s], cnt = nl_count[s];
+    const typename Vec4<T>::type pi = spos[s];
+    int n = 0;
+    for (int k = 0; k < cnt; ++k) {
+        const int j = sliced ? (nl[((size_t)(s >> 5) * maxn + k) * 32 + (s & 31)] & ((1 << 27) - 1)) : nl[(size_t)k * N + s];
+        if (skin) {
+            const typename Vec4<T>::type pj = spos[j];
+            if (!(r2_canonical(bd, (double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y, (double)pj.z - (double)pi.z) < rc2)) continue;
+        }
+        out_list[(size_t)i * maxn + n++] = perm[j];
+    }
+    out_count[i] = n;
+    for (int k = n; k < maxn; ++k) out_list[(size_t)i * maxn + k] = -1;
 }
 
 template <typename T>
@@ -441,6 +443,48 @@ int geom_update(metad_ctx *c, const double *d_box) {
     return METAD_OK;
 }
 
+// Verlet-skin reuse (params.skin).  Every step, before the build kernels: has any atom moved more
+// than skin / 2 (minimum-image displacement in fp64) from where it was when the list was built?  Then the step's rebuild flag
+// is raised and the build kernels that follow in the stream (or in the captured graph) do their work; otherwise they return
+// at once and the step works on the kept list, whose cell-sorted positions this kernel refreshes (same slots, current
+// coordinates).  The two flags alternate with the parity of the device step counter: the kernel clears the flag of the NEXT
+// step, so no memset node is needed and the decision never leaves the device.
+template <typename T>
+__global__ void k_skin_check(int N, const T *__restrict__ pos, const int *__restrict__ perm,
+                             const typename Vec4<T>::type *__restrict__ ref, typename Vec4<T>::type *__restrict__ spos, BoxD bd,
+                             double half_skin2, int *__restrict__ skin_flag, const int *__restrict__ step,
+                             const DevGeom *__restrict__ dg) {
+    const int cur = *step & 1;
+    if (blockIdx.x == 0 && threadIdx.x == 0) skin_flag[cur ^ 1] = 0;
+    if (skin_flag[cur]) return;                   // already decided (first step, new geometry): perm / ref are about to be rebuilt
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    bool moved = false;
+    if (s < N) {
+        if (dg) bd = dg->bd;
+        const int i = perm[s];
+        typename Vec4<T>::type r = ref[s], v;
+        v.x = pos[3 * i]; v.y = pos[3 * i + 1]; v.z = pos[3 * i + 2]; v.w = r.w;
+        double dx = (double)v.x - (double)r.x, dy = (double)v.y - (double)r.y, dz = (double)v.z - (double)r.z;
+        min_image_d(bd, dx, dy, dz);
+        moved = !(dx * dx + dy * dy + dz * dz <= half_skin2);       // also catches NaN
+        spos[s] = v;
+    }
+    if (__any_sync(0xffffffffu, moved) && (threadIdx.x & 31) == 0) atomicOr(&skin_flag[cur], 1);
+}
+
+int skin_check(metad_ctx *c, const void *d_pos) {
+    const double h2 = 0.25 * c->p.skin * c->p.skin;
+    if (c->prec == 32)
+        k_skin_check<float><<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, (const float *)d_pos, c->d_perm, (const float4 *)c->d_ref,
+                                                                      (float4 *)c->d_spos, c->boxd, h2, c->d_skin_flag, c->d_step, c->dg);
+    else
+        k_skin_check<double><<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, (const double *)d_pos, c->d_perm, (const double4 *)c->d_ref,
+                                                                       (double4 *)c->d_spos, c->boxd, h2, c->d_skin_flag, c->d_step, c->dg);
+    c->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return METAD_OK;
+}
+
 template <typename T>
 static int nb_build_t(metad_ctx *c, const void *d_pos) {
     typedef typename Vec4<T>::type V4;
@@ -448,25 +492,28 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     cudaStream_t st = c->stream;
     const int nsb = div_up(ncell, SCAN_TILE);
     const bool tm = c->timing && !c->capturing;
+    const int *sf = c->skin_on ? c->d_skin_flag : nullptr, *stp = c->d_step;
+    V4 *ref = c->skin_on ? (V4 *)c->d_ref : nullptr;
+    if (tm) { cudaEventRecord(c->ev[0], st); c->timing_recorded = 1; }
+    if (c->skin_on) { int r = skin_check(c, d_pos); if (r) return r; }
     if (N <= METAD_SMALL_N && !c->tiled) {                     // the whole neighbour stage in one launch
-        if (tm) { cudaEventRecord(c->ev[0], st); cudaEventRecord(c->ev[1], st); c->timing_recorded = 1; }
+        if (tm) cudaEventRecord(c->ev[1], st);
         k_build_list_small<T><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const T *)d_pos, c->d_flags, (V4 *)c->d_spos, c->d_perm,
-                                                                             c->d_scell, make_pbox<T>(c->boxd, c->rc), c->boxd, (T)c->rc2, c->rc2,
-                                                                             c->maxn, c->d_nl_count, c->d_nl, c->grid, c->d_sticky, c->dg);
+                                                                             c->d_scell, make_pbox<T>(c->boxd, c->rcl), c->boxd, (T)c->rcl2, c->rcl2,
+                                                                             c->maxn, c->d_nl_count, c->d_nl, c->grid, c->d_sticky, c->dg, ref, sf, stp, c->d_nbuilds);
         if (tm) cudaEventRecord(c->ev[2], st);
         c->launches += 1;
         CUDA_TRY(cudaGetLastError());
         return METAD_OK;
     }
-    if (tm) { cudaEventRecord(c->ev[0], st); c->timing_recorded = 1; }
     k_bin<T><<<div_up(N, 256), 256, 0, st>>>(N, (const T *)d_pos, c->grid, c->d_cell_of, c->d_slot, c->d_cell_count,
-                                             c->d_sticky, c->dg);
-    k_scan_sums<<<nsb, SCAN_THREADS, 0, st>>>(ncell, c->d_cell_count, c->d_block_sums);
-    k_scan_apply<<<nsb, SCAN_THREADS, 0, st>>>(ncell, N, c->d_cell_count, c->d_block_sums, c->d_cell_start);
-    k_scatter<<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_of, c->d_slot, c->d_cell_start, c->d_perm_raw);
+                                             c->d_sticky, c->dg, sf, stp);
+    k_scan_sums<<<nsb, SCAN_THREADS, 0, st>>>(ncell, c->d_cell_count, c->d_block_sums, sf, stp);
+    k_scan_apply<<<nsb, SCAN_THREADS, 0, st>>>(ncell, N, c->d_cell_count, c->d_block_sums, c->d_cell_start, sf, stp);
+    k_scatter<<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_of, c->d_slot, c->d_cell_start, c->d_perm_raw, sf, stp);
     k_cell_sort_gather<T><<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_start, c->d_cell_of, c->d_perm_raw, c->d_perm, (const T *)d_pos,
                                                              c->d_flags,   /* NULL unless a COORD / MINDIST CV has groups */
-                                                             (V4 *)c->d_spos, c->d_scell, c->tiled ? 1 : 0);
+                                                             (V4 *)c->d_spos, c->d_scell, c->tiled ? 1 : 0, ref, sf, stp, c->d_nbuilds);
     if (tm) cudaEventRecord(c->ev[1], st);
     if (c->tiled && sizeof(T) == 4) {
         c->launches += 5;
@@ -474,19 +521,19 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
         if (tm) cudaEventRecord(c->ev[2], st);
         return r;
     }
-    PBox<T> pb = make_pbox<T>(c->boxd, c->rc);
+    PBox<T> pb = make_pbox<T>(c->boxd, c->rcl);
     if (N <= METAD_WARP_PER_ATOM_MAX)
         k_build_list_warp<T, 32><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start,
-                                                                                 c->grid, pb, c->boxd, (T)c->rc2, c->rc2, c->maxn,
-                                                                                 c->d_nl_count, c->d_nl, c->d_sticky, c->dg);
+                                                                                 c->grid, pb, c->boxd, (T)c->rcl2, c->rcl2, c->maxn,
+                                                                                 c->d_nl_count, c->d_nl, c->d_sticky, c->dg, sf, stp);
     else if (N <= 8 * METAD_WARP_PER_ATOM_MAX)
         k_build_list_warp<T, 8><<<div_up((long long)N * 8, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start,
-                                                                               c->grid, pb, c->boxd, (T)c->rc2, c->rc2, c->maxn,
-                                                                               c->d_nl_count, c->d_nl, c->d_sticky, c->dg);
+                                                                               c->grid, pb, c->boxd, (T)c->rcl2, c->rcl2, c->maxn,
+                                                                               c->d_nl_count, c->d_nl, c->d_sticky, c->dg, sf, stp);
     else
     k_build_list<T><<<div_up(N, 128), 128, 0, st>>>(N, (const V4 *)c->d_spos, c->d_scell, c->d_cell_start, c->grid, pb,
-                                                   c->boxd, (T)c->rc2, c->rc2, c->maxn, c->d_nl_count, c->d_nl,
-                                                   c->d_sticky, c->dg);
+                                                   c->boxd, (T)c->rcl2, c->rcl2, c->maxn, c->d_nl_count, c->d_nl,
+                                                   c->d_sticky, c->dg, sf, stp);
     if (tm) cudaEventRecord(c->ev[2], st);
     c->launches += 6;
     CUDA_TRY(cudaGetLastError());
@@ -498,9 +545,12 @@ int nb_build(metad_ctx *c, const void *d_pos) {
 }
 
 int nb_export(metad_ctx *c, int *d_count, int *d_list) {
-    if (c->tiled) return tiled_export(c, d_count, d_list);
-    k_export_list<<<div_up(c->N, 128), 128, 0, c->stream>>>(c->N, c->maxn, c->d_perm, c->d_nl_count, c->d_nl, d_count,
-                                                            d_list);
+    if (c->prec == 32)
+        k_export_list<float><<<div_up(c->N, 128), 128, 0, c->stream>>>(c->N, c->maxn, c->d_perm, c->d_nl_count, c->d_nl, d_count, d_list,
+                                                                       c->tiled, (const float4 *)c->d_spos, c->boxd, c->rc2, c->skin_on, c->dg);
+    else
+        k_export_list<double><<<div_up(c->N, 128), 128, 0, c->stream>>>(c->N, c->maxn, c->d_perm, c->d_nl_count, c->d_nl, d_count, d_list,
+                                                                        0, (const double4 *)c->d_spos, c->boxd, c->rc2, c->skin_on, c->dg);
     c->launches += 1;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

@@ -232,7 +232,9 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
              int sw_n, int sw_m, const int *__restrict__ perm, double *__restrict__ partials, unsigned int *__restrict__ ticket, double scale_mean, double scale_solid,
              double *__restrict__ cv_q6 /* [2]: Q6 mean, solid count */,
              double *__restrict__ cv_out /* the context's CV vector on the run paths (NULL: k_q6_publish hands the sums over) */,
-             int dim0, int dim1, const DevGeom *__restrict__ dg_arg) {
+             int dim0, int dim1, const DevGeom *__restrict__ dg_arg,
+             const int *__restrict__ skin_flag, const int *__restrict__ step) {
+    if (MODE == 0 && SKIN_SKIP(skin_flag, step)) return;        // Verlet skin: the kept list is still valid (neighbor.cu)
     const DevGeom *dg = DEVBOX ? dg_arg : nullptr;
     extern __shared__ float4 dyn_smem[];
     __shared__ TileTables t;
@@ -285,17 +287,6 @@ __global__ void k_q6_publish(const double *__restrict__ cv_q6, int dim_mean, int
 }
 
 // ------------------------------------------------------------------------------------------------
-__global__ void k_tile_export(int N, int maxn, const int *__restrict__ perm, const int *__restrict__ nl_count,
-                              const int *__restrict__ nl, int *__restrict__ out_count, int *__restrict__ out_list) {
-    int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
-    const int i = perm[s], cnt = nl_count[s];
-    out_count[i] = cnt;
-    for (int k = 0; k < maxn; ++k)
-        out_list[(size_t)i * maxn + k] = k < cnt ? perm[nl[nl_slot(s, k, maxn)] & NL_IDX_MASK] : -1;
-}
-
-// ------------------------------------------------------------------------------------------------
 // host side
 TileGeom tile_geom(const metad_ctx *c);        // api.cu
 
@@ -325,26 +316,27 @@ int tiled_build(metad_ctx *c) {
         if (c->dg) k_tile_build<MODE, true><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(__VA_ARGS__);             \
         else k_tile_build<MODE, false><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(__VA_ARGS__);                  \
     } while (0)
-    if (c->has_q6)
+    const int *sf = c->skin_on ? c->d_skin_flag : nullptr;
+    if (c->has_q6 && !c->skin_on)
         TILE_LAUNCH(1,
-            g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
+            g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rcl2, c->rcl2, c->maxn,
             c->d_nl_count, c->d_nl, c->d_sticky, (float)qt, (float)(1.0 / qw), (float *)c->d_rec, c->d_q6,
             c->q6_solid_dim >= 0 ? 1 : 0, 0, 0, c->d_perm, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
             c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0, c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0,
-            c->d_cvq6, c->cv_direct, c->q6_mean_dim, c->q6_solid_dim, c->dg);
-    else if (c->has_coord) {                                  // ungrouped coordination number: the sum of sw rides on the exact pass
+            c->d_cvq6, c->cv_direct, c->q6_mean_dim, c->q6_solid_dim, c->dg, nullptr, c->d_step);
+    else if (c->has_coord && !c->skin_on) {                   // ungrouped coordination number: the sum of sw rides on the exact pass
         const CvDev &d = c->cv[c->coord_dim];
         // lazy_neighbors: nothing downstream reads the list (the force stage scales the per-atom gradient; the virial would
         // walk the list) — the pass runs list-free and metad_get_neighbors reports that there is no list
         c->list_skipped = c->p.lazy_neighbors && !c->p.want_virial && c->d_cgrad;
         TILE_LAUNCH(2,
-            g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
+            g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rcl2, c->rcl2, c->maxn,
             c->d_nl_count, c->list_skipped ? nullptr : c->d_nl, c->d_sticky, (float)(1.0 / d.r0), 1.f, c->d_cgrad, nullptr, 0, d.n, d.m, c->d_perm,
-            c->d_partials + c->nblocks_atoms, c->d_tickets + 1, d.scale, 0.0, c->d_cvq6, c->cv_direct, c->coord_dim, -1, c->dg);
+            c->d_partials + c->nblocks_atoms, c->d_tickets + 1, d.scale, 0.0, c->d_cvq6, c->cv_direct, c->coord_dim, -1, c->dg, nullptr, c->d_step);
     } else
         TILE_LAUNCH(0,
-            g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rc2, c->rc2, c->maxn,
-            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, 0, 0, c->d_perm, nullptr, nullptr, 0.0, 0.0, nullptr, nullptr, -1, -1, c->dg);
+            g, (const float4 *)c->d_spos, c->d_scell, c->d_cell_start, c->boxd, (float)c->rcl2, c->rcl2, c->maxn,
+            c->d_nl_count, c->d_nl, c->d_sticky, 0.f, 1.f, nullptr, nullptr, 0, 0, 0, c->d_perm, nullptr, nullptr, 0.0, 0.0, nullptr, nullptr, -1, -1, c->dg, sf, c->d_step);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
@@ -355,13 +347,6 @@ int tiled_q6_pass1(metad_ctx *c, double *d_cv) {
     if (c->cv_direct && c->cv_direct == d_cv) return METAD_OK;      // the build kernel wrote these dimensions itself
     if (c->has_q6) k_q6_publish<<<1, 32, 0, c->stream>>>(c->d_cvq6, c->q6_mean_dim, c->q6_solid_dim, d_cv);
     else k_q6_publish<<<1, 32, 0, c->stream>>>(c->d_cvq6, c->coord_dim, -1, d_cv);          // tiled coordination number
-    c->launches++;
-    CUDA_TRY(cudaGetLastError());
-    return METAD_OK;
-}
-
-int tiled_export(metad_ctx *c, int *d_count, int *d_list) {
-    k_tile_export<<<div_up(c->N, 128), 128, 0, c->stream>>>(c->N, c->maxn, c->d_perm, c->d_nl_count, c->d_nl, d_count, d_list);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

@@ -111,7 +111,7 @@ def force_bound(F_ref, dV_gpu, dV_ref, grads, tol_f=TOL_F):
 
 
 def chained_run(w, precision=None, nsteps=7, grid=None, lazy=False, hills=None, host=False, n_init_hills=40,
-                pos_of_step=None, box_of_step=None, seed=5, device_box=False, box_slack=0.0):
+                pos_of_step=None, box_of_step=None, seed=5, device_box=False, box_slack=0.0, skin=0.0, check_neighbors=False):
     """The library's RUN paths (metad_run = CUDA-graph replay, or metad_step_host with host=True) one step at a time, every
     step checked stage-wise against the oracle fed with the CUDA path's OWN upstream values (reading S, no slack factor):
 
@@ -141,7 +141,7 @@ def chained_run(w, precision=None, nsteps=7, grid=None, lazy=False, hills=None, 
         o.enable_grid(*grid)
         of.enable_grid(*grid)
     of.set_hills(*hills)
-    md = MetaD(w, precision=precision, max_hills=len(hills[1]) + nsteps + 8, grid=grid, lazy_neighbors=lazy, box_slack=box_slack)
+    md = MetaD(w, precision=precision, max_hills=len(hills[1]) + nsteps + 8, grid=grid, lazy_neighbors=lazy, box_slack=box_slack, skin=skin)
     md.set_hills(*hills)
     with torch.cuda.stream(md.stream):
         dpos = torch.tensor(pos, device="cuda", dtype=tdt)
@@ -189,6 +189,10 @@ def chained_run(w, precision=None, nsteps=7, grid=None, lazy=False, hills=None, 
         o.build_neighbors(p64)
         s_ref = o.eval_cv()
         assert rel(st["cv"], s_ref) <= TOL_CV, (k, st["cv"], s_ref)
+        if check_neighbors:                          # the exact rc list at every step, also when a kept rc + skin list is reused
+            cnt, lst = md.neighbors()
+            assert np.array_equal(cnt, o.count), k
+            assert np.array_equal(sorted_rows_fast(cnt, lst), sorted_rows_fast(o.count, o.list)), k
         V_ref, dV_ref = o.bias(st["cv"])
         assert abs(st["V"] - V_ref) <= TOL_CV * max(abs(V_ref), TINY), (k, st["V"], V_ref)
         assert np.abs(st["dVds"] - dV_ref).max() <= TOL_CV * max(np.abs(dV_ref).max(), TINY), (k, st["dVds"], dV_ref)
