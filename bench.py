@@ -496,6 +496,16 @@ def run_ours(args):
             roof_all.append(r_build)
             if list_ms > stage_ms[3]:
                 roof = r_build                     # the dominant kernel of the step
+            # what actually binds both kernels is instruction issue (profiles/r2g_ncu.md), so the same launches are also put
+            # against the issue peak 148 SMs x 4 schedulers x 1.965 GHz, with the executed warp instructions ncu counted
+            for key, kms, nm in (("build_warp_instructions", list_ms, "k_tile_build<Q6>"), ("force_warp_instructions", stage_ms[3], "k_q6_force_g")):
+                if traffic.get(key):
+                    gi_ = traffic[key] / (kms * 1e-3) / 1e9
+                    roof_all.append({"kernel": f"{nm}, issue-slot view", "bound": "alu", "achieved": gi_, "peak": ISSUE_PEAK_GINST,
+                                     "unit": "G warp-instructions/s", "frac": gi_ / ISSUE_PEAK_GINST, "traffic": None,
+                                     "peak_source": "148 SMs x 4 schedulers x 1.965 GHz (guide's unit counts); instruction count from "
+                                                    "profiles/ncu_traffic.json (ncu smsp__inst_executed.sum of the same kernel)",
+                                     "warp_instructions_per_launch": traffic[key], "kernel_ms": float(kms)})
     elif (precision == 32 and list_ms is not None and not args.virial and not args.lazy
           and sum(c.kind == 0 and c.group_a is None and c.group_b is None for c in w.cvs) == 1
           and getattr(w, "max_neigh", 64) <= 32):
