@@ -63,7 +63,7 @@ enum metad_cv_kind {
                               nearest pair only (the derivative of a minimum is that of its arg-min, which is what automatic
                               differentiation returns); nobody within rc: s = rc, no force
                               ("distance between a surface oxygen atom and its nearest hydrogen atom"; reading AA).
-                              Groups as for COORD; at most one COORD or MINDIST CV per context                              */
+                              Groups as for COORD.  A context may hold several COORD / MINDIST CVs, each with its own groups    */
     METAD_CV_LATTICE = 7,  /* s = |h_k|, the length of box row k = cv.n in {0, 1, 2} ("the triaxial lattice parameters as
                               CVs"; reading AB).  No atomic forces: the bias acts on the cell, see metad_get_box_force          */
     METAD_CV_TORSION = 5   /* dihedral angle of atoms torsion[0..3] in (-pi, pi], IUPAC sign, minimum-image bonds

@@ -92,25 +92,23 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
         switch (s.kind) {
         case METAD_CV_COORD:
         case METAD_CV_MINDIST: {
-            if (c->coord_dim >= 0 || c->mindist_dim >= 0) FAIL(METAD_ERR_ARG, "only one COORD or MINDIST CV per context");
+            // any number of them (up to METAD_MAX_CV): every list CV owns two bits (in A, in B) of the per-atom flag byte
+            v.fshift = 2 * (c->n_coord + c->n_mindist);
             if (s.kind == METAD_CV_COORD) {
                 if (!(s.r0 > 0.0) || s.n < 1 || s.m <= s.n) FAIL(METAD_ERR_ARG, "COORD needs r0 > 0, 0 < n < m");
-                c->coord_dim = d; c->has_coord = true;
+                if (c->coord_dim < 0) c->coord_dim = d;
+                c->has_coord = true; c->n_coord++;
             } else {
-                c->mindist_dim = d; c->has_mindist = true;
+                if (c->mindist_dim < 0) c->mindist_dim = d;
+                c->has_mindist = true; c->n_mindist++;
                 if (s.group_a && s.group_b && s.n_a > 0 && s.n_b > 0) {      // list-free variant needs explicit groups
                     v.n_ga = s.n_a; v.n_gb = s.n_b;
                     if (upload_ints(&v.d_ga, s.group_a, s.n_a) || upload_ints(&v.d_gb, s.group_b, s.n_b)) return METAD_ERR_CUDA;
                 }
             }
             v.use_groups = s.group_a || s.group_b;
-            if (v.use_groups) {
-                flags.assign(N, 0);
-                if (s.group_a) { for (int k = 0; k < s.n_a; ++k) { int i = s.group_a[k]; if (i < 0 || i >= N) FAIL(METAD_ERR_ARG, "group index"); flags[i] |= 1; } }
-                else for (int i = 0; i < N; ++i) flags[i] |= 1;
-                if (s.group_b) { for (int k = 0; k < s.n_b; ++k) { int i = s.group_b[k]; if (i < 0 || i >= N) FAIL(METAD_ERR_ARG, "group index"); flags[i] |= 2; } }
-                else for (int i = 0; i < N; ++i) flags[i] |= 2;
-            }
+            if (s.group_a) for (int k = 0; k < s.n_a; ++k) if (s.group_a[k] < 0 || s.group_a[k] >= N) FAIL(METAD_ERR_ARG, "group index");
+            if (s.group_b) for (int k = 0; k < s.n_b; ++k) if (s.group_b[k] < 0 || s.group_b[k] >= N) FAIL(METAD_ERR_ARG, "group index");
             break;
         }
         case METAD_CV_Q6_MEAN:
@@ -169,7 +167,25 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
         }
     }
 
-    if (c->has_mindist) CUDA_TRY(dev_alloc(&c->d_mind, 8));
+    // group flags: needed as soon as a list CV has groups or there is more than one list CV (a context with ONE ungrouped
+    // list CV keeps w = 3 in the sorted positions and no flag array)
+    {
+        bool need = c->n_coord + c->n_mindist > 1;
+        for (int d = 0; d < c->D; ++d) need = need || c->cv[d].use_groups;
+        if (need) {
+            flags.assign(N, 0);
+            for (int d = 0; d < c->D; ++d) {
+                const metad_cv_desc &s = p->cv[d];
+                if (s.kind != METAD_CV_COORD && s.kind != METAD_CV_MINDIST) continue;
+                const unsigned char ba = (unsigned char)(1u << c->cv[d].fshift), bb = (unsigned char)(2u << c->cv[d].fshift);
+                if (s.group_a) for (int k = 0; k < s.n_a; ++k) flags[s.group_a[k]] |= ba;
+                else for (int i = 0; i < N; ++i) flags[i] |= ba;
+                if (s.group_b) for (int k = 0; k < s.n_b; ++k) flags[s.group_b[k]] |= bb;
+                else for (int i = 0; i < N; ++i) flags[i] |= bb;
+            }
+        }
+    }
+    if (c->has_mindist) CUDA_TRY(dev_alloc(&c->d_mind, 8 * METAD_MAX_CV));
     if (p->traj_capacity < 0) FAIL(METAD_ERR_ARG, "traj_capacity must be >= 0");
     if (p->traj_capacity > 0) CUDA_TRY(dev_alloc(&c->d_traj, (size_t)p->traj_capacity * c->D));
     if (p->want_virial) {
@@ -212,7 +228,7 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
         CUDA_TRY(dev_alloc(&c->d_flags, N));
         CUDA_TRY(cudaMemcpy(c->d_flags, flags.data(), N, cudaMemcpyHostToDevice));
     }
-    if (c->has_coord && !c->has_q6 && c->prec == 32 && !c->cv[c->coord_dim].use_groups)   // candidates for the tiled path
+    if (c->n_coord == 1 && !c->has_mindist && !c->has_q6 && c->prec == 32 && !c->cv[c->coord_dim].use_groups)   // candidates for the tiled path
         CUDA_TRY(dev_alloc(&c->d_cgrad, 4 * (size_t)N));
     if (c->has_q6) {
         CUDA_TRY(cudaMalloc(&c->d_rec, METAD_NREC * tsz * (size_t)N));
@@ -253,6 +269,7 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
     CUDA_TRY(cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
     CUDA_TRY(dev_alloc(&c->d_hill_stage, (size_t)(c->D + 1) * p->max_hills));
     CUDA_TRY(dev_alloc(&c->d_geom, 1));
+    CUDA_TRY(dev_alloc(&c->d_tile_cuts, (size_t)c->cell_cap / 4 + 64));
     CUDA_TRY(dev_alloc(&c->d_nbuilds, 1));
     CUDA_TRY(cudaMemset(c->d_nbuilds, 0, sizeof(int)));
     if (!(p->box_slack >= 0.0) || p->box_slack > 1.0) FAIL(METAD_ERR_ARG, "box_slack must be in [0, 1]");
@@ -280,7 +297,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage, c->d_geom, c->d_skin_flag, c->d_ref, c->d_nbuilds, c->d_keep_mask };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage, c->d_geom, c->d_skin_flag, c->d_ref, c->d_nbuilds, c->d_keep_mask, c->d_tile_cuts };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
@@ -340,7 +357,7 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc, double sla
     // >= 3 cells per direction
     c->tiled = 0;
     const bool q6_only = c->has_q6 && !c->has_coord;
-    const bool coord_only = c->has_coord && !c->has_q6 && !c->cv[c->coord_dim].use_groups && !c->skin_on;
+    const bool coord_only = c->n_coord == 1 && !c->has_q6 && !c->cv[c->coord_dim].use_groups && !c->skin_on;
     if (c->prec == 32 && (q6_only || coord_only) && !c->has_mindist && c->N < (1 << NL_IDX_BITS) && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32) {
         // the rc-wide cells are subdivided along x (the direction of the contiguous row runs): an atom then scans
         // 2 xsub + 1 sub-cells per row (2.5 / 2.25 cell widths for xsub = 2 / 4) instead of 3 cells
@@ -367,6 +384,19 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc, double sla
         if (bt[0] > 0) {
             c->tiled = 1; c->tile_T[0] = bt[0]; c->tile_T[1] = bt[1]; c->tile_T[2] = bt[2]; c->tile_cap = cap; c->tile_hx = xsub;
             c->grid = gs;
+            // tile boundaries (tile k of a direction covers cells [k nc / nt, (k + 1) nc / nt)): a small device table,
+            // uploaded only when the tiling changes (never inside a capture: run_impl derives the geometry before it starts one)
+            const int ncs[3] = { gs.nc[0], gs.nc[1], gs.nc[2] };
+            int nts[3], key[6];
+            for (int d = 0; d < 3; ++d) { nts[d] = (ncs[d] + bt[d] - 1) / bt[d]; key[d] = ncs[d]; key[3 + d] = nts[d]; }
+            if (memcmp(key, c->tile_cuts_key, sizeof(key)) != 0) {
+                std::vector<int> cuts;
+                for (int d = 0; d < 3; ++d)
+                    for (int k = 0; k <= nts[d]; ++k) cuts.push_back((int)(((long long)k * ncs[d]) / nts[d]));
+                if ((int)cuts.size() > c->cell_cap / 4 + 64) FAIL(METAD_ERR_ARG, "tile table overflow");
+                CUDA_TRY(cudaMemcpyAsync(c->d_tile_cuts, cuts.data(), sizeof(int) * cuts.size(), cudaMemcpyHostToDevice, c->stream));
+                memcpy(c->tile_cuts_key, key, sizeof(key));
+            }
         }
     }
     return METAD_OK;
@@ -378,6 +408,9 @@ TileGeom tile_geom(const metad_ctx *c) {
     t.nc0 = c->grid.nc[0]; t.nc1 = c->grid.nc[1]; t.nc2 = c->grid.nc[2];
     t.ntx = (t.nc0 + t.Tx - 1) / t.Tx; t.nty = (t.nc1 + t.Ty - 1) / t.Ty; t.ntz = (t.nc2 + t.Tz - 1) / t.Tz;
     t.cap = c->tile_cap; t.hx = c->tile_hx; t.natoms = c->N;
+    t.cshift = 0;
+    while ((1 << t.cshift) < t.Tx + 2 * t.hx + 2) ++t.cshift;      // Txe <= Tx + 1 columns + the end-of-row entry
+    t.cuts = c->d_tile_cuts;
     t.ax = c->boxd.ax; t.bx = c->boxd.bx; t.by = c->boxd.by; t.cx = c->boxd.cx; t.cy = c->boxd.cy; t.cz = c->boxd.cz;
     t.wa = t.wb = t.wc = 0.0;
     return t;
@@ -425,8 +458,10 @@ static int build_neighbors_impl(metad_ctx *c, const void *d_pos, const double *h
     if (r) return r;
     c->d_pos_last = d_pos;
     // no CV reads the list; a nearest-distance CV with a few explicit centres is scanned without one (k_mindist_brute)
-    const bool mind_brute = c->has_mindist && c->cv[c->mindist_dim].d_ga && c->cv[c->mindist_dim].n_ga <= 64 &&
-                            div_up(c->cv[c->mindist_dim].n_gb, 128) <= c->nblocks_atoms;
+    bool mind_brute = c->has_mindist;
+    for (int d = 0; d < c->D; ++d)
+        if (c->cv[d].kind == METAD_CV_MINDIST)
+            mind_brute = mind_brute && c->cv[d].d_ga && c->cv[d].n_ga <= 64 && div_up(c->cv[d].n_gb, 128) <= c->nblocks_atoms;
     if (c->p.lazy_neighbors && !c->has_q6 && !c->has_coord && (!c->has_mindist || mind_brute)) {
         c->have_neighbors = true; c->list_built = false;
         return METAD_OK;
@@ -521,7 +556,7 @@ extern "C" int metad_run_dev(metad_ctx *c, const void *d_pos, const double *d_bo
 static int run_impl(metad_ctx *c, const void *d_pos, const double *h_box, const double *d_box, double rc, void *d_F, int nsteps) {
     bool same = c->graph_exec && c->graph_pos == d_pos && c->graph_F == d_F && c->graph_rc == rc &&
                 (d_box ? (c->graph_devbox && c->graph_dbox == d_box && c->dev_geom_ready)
-                       : (!c->graph_devbox && memcmp(c->graph_box, h_box, sizeof(double) * 9) == 0));
+                       : (!c->graph_devbox && h_box && memcmp(c->graph_box, h_box, sizeof(double) * 9) == 0));
     if (!same) {
         // argument errors surface before the capture starts; a device box is read ONCE here to derive the frozen cell grid
         int r = d_box ? dev_geometry(c, d_box, rc) : setup_geometry(c, h_box, rc);

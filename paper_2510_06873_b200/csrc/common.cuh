@@ -173,7 +173,7 @@ __device__ __forceinline__ bool last_block_ticket(unsigned int *ticket) {
     __syncthreads();
     if (threadIdx.x == 0) {
         unsigned int t = atomicAdd(ticket, 1u);
-        is_last = (t == gridDim.x - 1);
+        is_last = (t == gridDim.x * gridDim.y * gridDim.z - 1);
         if (is_last) *ticket = 0u;  // re-arm for the next launch
     }
     __syncthreads();
@@ -220,6 +220,7 @@ struct CvDev {                      // device copies of one CV descriptor
     int *d_chain; double *d_mass;         // RGYR
     double *d_unwrapped;                  // RGYR scratch: [nchain*3] + com[3] + rg
     bool use_groups;
+    int fshift;                           // COORD, MINDIST: bit offset of this CV's (in A, in B) pair in the per-atom group flags
     int tors[4];                          // TORSION
     int *d_ga, *d_gb; int n_ga, n_gb;     // MINDIST: device copies of the group index lists (list-free variant)
 };
@@ -252,8 +253,9 @@ struct metad_ctx {
     double *d_traj;                       // traj_capacity > 0: [capacity][D] CV frames, frame k = step k + 1 since the last reset
     double *d_virial, *d_vir_partials;    // want_virial: [9] bias virial of the last apply_forces; per-block partials
     double *d_box_force;                  // LATTICE: [9] bias force on the box rows, written by apply_forces
-    int mindist_dim;
-    double *d_mind;                       // MINDIST: [r, dx, dy, dz] of the nearest pair + its two original indices (as int pair)
+    int mindist_dim;                      // first MINDIST dimension (-1: none); n_mindist of them, n_coord COORD dimensions
+    int n_coord, n_mindist;
+    double *d_mind;                       // MINDIST: per CV dimension d, at + 8 d: [r, dx, dy, dz] of the nearest pair + its two original indices
     double *d_tors_grad;                  // TORSION: [D][12] d phi / d r of the four atoms, written by the CV kernel
     int *d_tors_atoms; int ntors_atoms;   //          unique touched atoms (gather-form force kernel: thread per atom)
     int q6_mean_dim, q6_solid_dim, coord_dim;
@@ -292,6 +294,7 @@ struct metad_ctx {
     int *d_aux;                           // device scalars: grid-miss flag, index of the hill deposited this step
     // shared-memory tiled fast path (fp32, Q6): tile.cuh / tiled.cu
     int tiled; int tile_T[3]; int tile_cap; int tile_hx;
+    int *d_tile_cuts; int tile_cuts_key[6];    // tile boundaries per direction (device) and the (nc, nt) they were computed for
     int timing; int capturing; int timing_recorded; cudaEvent_t ev[3];
     cudaStream_t copy_stream; cudaEvent_t ev_copy;   // metad_step_host: the force upload overlaps the first three stages
     float *d_q6;                          // tiled path: per-atom q6 (sorted order) [N], then f'(q6) [N]

@@ -14,7 +14,7 @@ template <typename T> PBox<T> ctx_pbox(const metad_ctx *c);
 template <typename T>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-           const int *__restrict__ nl, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, T inv_r0, int n, int m, double scale,
+           const int *__restrict__ nl, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, int fshift /* this CV's bits of the group flags */, T inv_r0, int n, int m, double scale,
            double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
            unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
     __shared__ double red[32];
@@ -23,12 +23,12 @@ k_coord_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
     T acc = T(0);
     if (s < N) {
         typename Vec4<T>::type pi = spos[s];
-        if (((int)pi.w) & 1) {
+        if ((((int)pi.w) >> fshift) & 1) {
             int cnt = nl_count[s];
             for (int k = 0; k < cnt; ++k) {
                 int j = nl[(size_t)k * N + s];
                 typename Vec4<T>::type pj = spos[j];
-                if (!(((int)pj.w) & 2)) continue;
+                if (!((((int)pj.w) >> fshift) & 2)) continue;
                 if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
                 T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
                 min_image(pb, dx, dy, dz);
@@ -57,7 +57,7 @@ k_coord_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
 template <typename T, bool VIRIAL>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-              const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, T inv_r0, int n, int m,
+              const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, int fshift /* this CV's bits of the group flags */, T inv_r0, int n, int m,
               double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F, VirArgs va,
               const DevGeom *__restrict__ dg) {
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
@@ -70,13 +70,13 @@ k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int 
 #pragma unroll
     for (int q = 0; q < 9; ++q) wv[q] = T(0);
     typename Vec4<T>::type pi = spos[s];
-    const int fi = (int)pi.w;
+    const int fi = ((int)pi.w) >> fshift;
     T ax = T(0), ay = T(0), az = T(0);
     int cnt = act ? nl_count[s] : 0;
     for (int k = 0; k < cnt; ++k) {
         int j = nl[(size_t)k * N + s];
         typename Vec4<T>::type pj = spos[j];
-        const int fj = (int)pj.w;
+        const int fj = ((int)pj.w) >> fshift;
         int mult = ((fi & 1) && (fj & 2)) + ((fi & 2) && (fj & 1));
         if (!mult) continue;
         if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
@@ -114,7 +114,7 @@ k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int 
 template <typename T, int G>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-                const int *__restrict__ nl, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, T inv_r0, int n, int m, double scale,
+                const int *__restrict__ nl, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, int fshift /* this CV's bits of the group flags */, T inv_r0, int n, int m, double scale,
                 double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
                 unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
     __shared__ double red[32];
@@ -124,12 +124,12 @@ k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const in
     T acc = T(0);
     if (s < N) {
         typename Vec4<T>::type pi = spos[s];
-        if (((int)pi.w) & 1) {
+        if ((((int)pi.w) >> fshift) & 1) {
             const int cnt = nl_count[s];
             for (int k = lane; k < cnt; k += G) {
                 const int j = nl[(size_t)k * N + s];
                 typename Vec4<T>::type pj = spos[j];
-                if (!(((int)pj.w) & 2)) continue;
+                if (!((((int)pj.w) >> fshift) & 2)) continue;
                 if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
                 T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
                 min_image(pb, dx, dy, dz);
@@ -156,7 +156,7 @@ k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const in
 template <typename T, int G>
 __global__ void __launch_bounds__(CV_THREADS)
 k_coord_force_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-                   const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, T inv_r0, int n, int m,
+                   const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, int fshift /* this CV's bits of the group flags */, T inv_r0, int n, int m,
                    double coef /* force_scale*scale */, const double *__restrict__ dVds, T *__restrict__ F,
                    const DevGeom *__restrict__ dg) {
     const int gt = blockIdx.x * blockDim.x + threadIdx.x;
@@ -165,13 +165,13 @@ k_coord_force_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const
     if (dg) { pb = dg_pb<T>(dg); bdk = dg->bd; }
     const unsigned gmask = G == 32 ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
     typename Vec4<T>::type pi = spos[s];
-    const int fi = (int)pi.w;
+    const int fi = ((int)pi.w) >> fshift;
     T ax = T(0), ay = T(0), az = T(0);
     const int cnt = (fi & 3) ? nl_count[s] : 0;             // an atom in neither group takes no force
     for (int k = lane; k < cnt; k += G) {
         const int j = nl[(size_t)k * N + s];
         typename Vec4<T>::type pj = spos[j];
-        const int fj = (int)pj.w;
+        const int fj = ((int)pj.w) >> fshift;
         const int mult = ((fi & 1) && (fj & 2)) + ((fi & 2) && (fj & 1));
         if (!mult) continue;
         if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
@@ -738,7 +738,7 @@ __device__ __forceinline__ void min_warp(double &r2, long long &ij, int &sj, int
 template <typename T>
 __global__ void __launch_bounds__(CV_THREADS)
 k_mindist_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
-             const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, double rc,
+             const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, int fshift /* this CV's bits of the group flags */, double rc,
              double *__restrict__ part_r2, long long *__restrict__ part_ij, int *__restrict__ part_s /* [2*nblocks] */,
              unsigned int *__restrict__ ticket, double *__restrict__ rec /* [r, dx, dy, dz, (i, j) as two ints] */,
              double *__restrict__ cv_out, const DevGeom *__restrict__ dg) {
@@ -750,13 +750,13 @@ k_mindist_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *
     double r2 = 1e300; long long ij = 0x7fffffffffffffffll; int sj = -1, si = -1;
     if (s < N) {
         const typename Vec4<T>::type pi = spos[s];
-        if (((int)pi.w) & 1) {
+        if ((((int)pi.w) >> fshift) & 1) {
             const int cnt = nl_count[s];
             const long long io = perm[s];
             for (int k = 0; k < cnt; ++k) {
                 const int j = nl[(size_t)k * N + s];
                 const typename Vec4<T>::type pj = spos[j];
-                if (!(((int)pj.w) & 2)) continue;
+                if (!((((int)pj.w) >> fshift) & 2)) continue;
                 if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
                 T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
                 min_image(pb, dx, dy, dz);
@@ -884,44 +884,53 @@ k_mindist_brute(int nA, const int *__restrict__ ga, int nB, const int *__restric
 }
 
 template <typename T>
-static int mindist_eval_t(metad_ctx *c, double *d_cv) {
+static int mindist_eval_t(metad_ctx *c, double *d_cv, int md) {
     typedef typename Vec4<T>::type V4;
+    const CvDev &d = c->cv[md];
     const int nb = div_up(c->N, CV_THREADS);
     double *pr = c->d_partials;
     long long *pk = reinterpret_cast<long long *>(c->d_partials + c->nblocks_atoms);
     int *ps = reinterpret_cast<int *>(c->d_partials + 2 * (size_t)c->nblocks_atoms);
-    k_mindist_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(c->N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, ctx_pbox<T>(c), c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0,
-                                                     c->rc, pr, pk, ps, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim, c->dg);
+    k_mindist_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(c->N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, ctx_pbox<T>(c), c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, d.fshift,
+                                                     c->rc, pr, pk, ps, c->d_tickets + 0, c->d_mind + 8 * md, d_cv + md, c->dg);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
 }
 int mindist_eval(metad_ctx *c, double *d_cv) {
     if (!c->has_mindist) return METAD_OK;
+    for (int md = 0; md < c->D; ++md) {
+    if (c->cv[md].kind != METAD_CV_MINDIST) continue;
     if (!c->list_built) {                                       // lazy_neighbors: list-free scan of the few centres
-        const CvDev &d = c->cv[c->mindist_dim];
+        const CvDev &d = c->cv[md];
         const int nb = div_up(d.n_gb, CV_THREADS);
         double *pr = c->d_partials;
         long long *pk = reinterpret_cast<long long *>(c->d_partials + c->nblocks_atoms);
         if (c->prec == 32)
             k_mindist_brute<float><<<nb, CV_THREADS, 0, c->stream>>>(d.n_ga, d.d_ga, d.n_gb, d.d_gb, (const float *)ctx_last_pos(c), c->boxd,
-                                                                     c->rc, pr, pk, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim, c->dg);
+                                                                     c->rc, pr, pk, c->d_tickets + 0, c->d_mind + 8 * md, d_cv + md, c->dg);
         else
             k_mindist_brute<double><<<nb, CV_THREADS, 0, c->stream>>>(d.n_ga, d.d_ga, d.n_gb, d.d_gb, (const double *)ctx_last_pos(c), c->boxd,
-                                                                      c->rc, pr, pk, c->d_tickets + 0, c->d_mind, d_cv + c->mindist_dim, c->dg);
+                                                                      c->rc, pr, pk, c->d_tickets + 0, c->d_mind + 8 * md, d_cv + md, c->dg);
         c->launches++;
         CUDA_TRY(cudaGetLastError());
-        return METAD_OK;
+        continue;
     }
-    return c->prec == 32 ? mindist_eval_t<float>(c, d_cv) : mindist_eval_t<double>(c, d_cv);
+    const int r = c->prec == 32 ? mindist_eval_t<float>(c, d_cv, md) : mindist_eval_t<double>(c, d_cv, md);
+    if (r) return r;
+    }
+    return METAD_OK;
 }
 int mindist_forces(metad_ctx *c, const double *d_dVds, void *d_F) {
     if (!c->has_mindist) return METAD_OK;
-    if (c->prec == 32) k_mindist_force<float><<<1, 32, 0, c->stream>>>(c->d_mind, c->p.force_scale, d_dVds + c->mindist_dim, (float *)d_F,
-                                                                   c->p.want_virial ? c->d_virial : nullptr);
-    else k_mindist_force<double><<<1, 32, 0, c->stream>>>(c->d_mind, c->p.force_scale, d_dVds + c->mindist_dim, (double *)d_F,
-                                                         c->p.want_virial ? c->d_virial : nullptr);
-    c->launches++;
+    for (int md = 0; md < c->D; ++md) {
+        if (c->cv[md].kind != METAD_CV_MINDIST) continue;
+        if (c->prec == 32) k_mindist_force<float><<<1, 32, 0, c->stream>>>(c->d_mind + 8 * md, c->p.force_scale, d_dVds + md, (float *)d_F,
+                                                                       c->p.want_virial ? c->d_virial : nullptr);
+        else k_mindist_force<double><<<1, 32, 0, c->stream>>>(c->d_mind + 8 * md, c->p.force_scale, d_dVds + md, (double *)d_F,
+                                                             c->p.want_virial ? c->d_virial : nullptr);
+        c->launches++;
+    }
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
 }
@@ -938,16 +947,17 @@ static int cv_eval_t(metad_ctx *c, double *d_cv) {
     if (c->has_coord && c->tiled) {                          // the sum ran inside k_tile_build<2>
         int r = tiled_q6_pass1(c, d_cv);
         if (r) return r;
-    } else if (c->has_coord) {
-        const CvDev &d = c->cv[c->coord_dim];
+    } else for (int cd = 0; cd < c->D; ++cd) {               // every COORD dimension: its own pass over the list
+        if (c->cv[cd].kind != METAD_CV_COORD) continue;
+        const CvDev &d = c->cv[cd];
         if (N <= METAD_WARP_PER_ATOM_MAX)
             k_coord_cv_warp<T, 32><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
-                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials_warp,
-                c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky, c->dg);
+                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, d.fshift, (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials_warp,
+                c->d_tickets + 0, d_cv + cd, c->d_sticky, c->dg);
         else
-        k_coord_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0,
+        k_coord_cv<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, d.fshift,
                                                        (T)(1.0 / d.r0), d.n, d.m, d.scale, c->d_partials,
-                                                       c->d_tickets + 0, d_cv + c->coord_dim, c->d_sticky, c->dg);
+                                                       c->d_tickets + 0, d_cv + cd, c->d_sticky, c->dg);
         c->launches++;
     }
     if (c->has_q6 && c->tiled) {
@@ -993,25 +1003,26 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
     if (c->has_coord && c->tiled) {
         int r = tiled_coord_force(c, d_dVds, d_F);
         if (r) return r;
-    } else if (c->has_coord) {
-        const CvDev &d = c->cv[c->coord_dim];
+    } else for (int cd = 0; cd < c->D; ++cd) {               // every COORD dimension adds its forces in turn (fixed order)
+        if (c->cv[cd].kind != METAD_CV_COORD) continue;
+        const CvDev &d = c->cv[cd];
         const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
         if (c->p.want_virial)                                 // forces and virial in one thread-per-atom pass
             k_coord_force<T, true><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
-                                                                    pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
-                                                                    d_dVds + c->coord_dim, (T *)d_F, va, c->dg);
+                                                                    pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, d.fshift, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
+                                                                    d_dVds + cd, (T *)d_F, va, c->dg);
         else if (N <= METAD_WARP_PER_ATOM_MAX)
             k_coord_force_warp<T, 32><<<div_up((long long)N * 32, CV_THREADS), CV_THREADS, 0, c->stream>>>(
-                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)(1.0 / d.r0), d.n, d.m,
-                c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F, c->dg);
+                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, d.fshift, (T)(1.0 / d.r0), d.n, d.m,
+                c->p.force_scale * d.scale, d_dVds + cd, (T *)d_F, c->dg);
         else if (d.use_groups && N <= 8 * METAD_WARP_PER_ATOM_MAX)
             k_coord_force_warp<T, 8><<<div_up((long long)N * 8, CV_THREADS), CV_THREADS, 0, c->stream>>>(
-                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)(1.0 / d.r0), d.n, d.m,
-                c->p.force_scale * d.scale, d_dVds + c->coord_dim, (T *)d_F, c->dg);
+                N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, d.fshift, (T)(1.0 / d.r0), d.n, d.m,
+                c->p.force_scale * d.scale, d_dVds + cd, (T *)d_F, c->dg);
         else
             k_coord_force<T, false><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm,
-                                                                     pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
-                                                                     d_dVds + c->coord_dim, (T *)d_F, va, c->dg);
+                                                                     pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, d.fshift, (T)(1.0 / d.r0), d.n, d.m, c->p.force_scale * d.scale,
+                                                                     d_dVds + cd, (T *)d_F, va, c->dg);
         c->launches++;
     }
     if (c->has_q6 && c->tiled) {

@@ -27,6 +27,8 @@ struct TileGeom {
     int ntx, nty, ntz;           // tiles per direction
     int nc0, nc1, nc2;           // cells per direction
     int cap;                     // halo capacity (atoms) of the shared-memory staging area
+    int cshift;                  // log2 of the power of two >= Tx + 2 hx + 1: a halo cell is (row, column) = (i >> cshift, i & mask)
+    const int *cuts;             // device: tile boundaries along x [ntx + 1], y [nty + 1], z [ntz + 1] (api.cu: no division in the kernel)
     int natoms;                  // N (the second halves of the q6 records start at rec + 8 N)
     double ax, bx, by, cx, cy, cz;   // lattice rows
     double wa, wb, wc;           // cell edge vectors are a/nc0, b/nc1, c/nc2 (used for the tile's coordinate range)
@@ -73,24 +75,30 @@ struct TileScratch {
     int hrel[TILE_MAXROWS][TILE_TXMAX + 2 * TILE_HXMAX + 1];    // start of the halo cell relative to its segment | piece << 28
 };
 #define TILE_SCRATCH_BYTES sizeof(TileScratch)
-__device__ __forceinline__ int tile_cut(int k, int nc, int nt) { return (int)(((unsigned)k * (unsigned)nc) / (unsigned)nt); }
+// r / d and r % d for 0 <= r < 64, 3 <= d <= 6 (rows of a halo: d = Ty + 2) by a reciprocal multiplication instead of the
+// ~20-instruction integer division
+__device__ __forceinline__ int small_div(int r, int d) {
+    const int magic = d == 3 ? 21846 : (d == 4 ? 16384 : (d == 5 ? 13108 : 10923));      // ceil(65536 / d)
+    return (r * magic) >> 16;
+}
 
 __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restrict__ cell_start, TileTables &t, TileScratch &w,
                                            const DevGeom *dg) {
     const int tid = threadIdx.x;
-    int b = blockIdx.x;
-    const int tx = b % g.ntx; b /= g.ntx;
-    const int ty = b % g.nty, tz = b / g.nty;
-    const int x0 = tile_cut(tx, g.nc0, g.ntx), y0 = tile_cut(ty, g.nc1, g.nty), z0 = tile_cut(tz, g.nc2, g.ntz);
-    const int Txe = tile_cut(tx + 1, g.nc0, g.ntx) - x0, Tye = tile_cut(ty + 1, g.nc1, g.nty) - y0,
-              Tze = tile_cut(tz + 1, g.nc2, g.ntz) - z0;
+    // the launch grid is (ntx, nty, ntz) and the tile boundaries come from a table: no integer division on the way in
+    const int tx = blockIdx.x, ty = blockIdx.y, tz = blockIdx.z;
+    const int *cy = g.cuts + g.ntx + 1, *cz = cy + g.nty + 1;
+    const int x0 = g.cuts[tx], y0 = cy[ty], z0 = cz[tz];
+    const int Txe = g.cuts[tx + 1] - x0, Tye = cy[ty + 1] - y0, Tze = cz[tz + 1] - z0;
     const int hx = g.hx;
     const int nrows = (Tye + 2) * (Tze + 2), ncol = Txe + 2 * hx;
     const int xa = x0 - hx, xb = x0 + Txe + hx - 1;
+    const int cmask = (1 << g.cshift) - 1, nslot = nrows << g.cshift;
     // ---- phase 1: cell_start of every halo cell (both ends); warp 7 fixes the tile origin
-    for (int i = tid; i < nrows * ncol; i += blockDim.x) {
-        const int r = i / ncol, c = i - r * ncol;
-        const int hy = r % (Tye + 2) - 1, hz = r / (Tye + 2) - 1;
+    for (int i = tid; i < nslot; i += blockDim.x) {
+        const int r = i >> g.cshift, c = i & cmask;
+        if (c >= ncol) continue;
+        const int hz = small_div(r, Tye + 2) - 1, hy = r - (hz + 1) * (Tye + 2) - 1;
         const int ly = y0 + hy, lz = z0 + hz, lx = xa + c;
         const int jy = ly < 0 ? ly + g.nc1 : (ly >= g.nc1 ? ly - g.nc1 : ly);
         const int jz = lz < 0 ? lz + g.nc2 : (lz >= g.nc2 ? lz - g.nc2 : lz);
@@ -127,7 +135,7 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
     //      p = 1 inside the box, p = 2 right of x = nc0 - 1 (shift +a).
     if (tid < 3 * nrows) {
         const int r = tid / 3, p = tid - 3 * r;
-        const int hy = r % (Tye + 2) - 1, hz = r / (Tye + 2) - 1;
+        const int hz = small_div(r, Tye + 2) - 1, hy = r - (hz + 1) * (Tye + 2) - 1;
         const int ly = y0 + hy, lz = z0 + hz;
         const int wy = ly < 0 ? -1 : (ly >= g.nc1 ? 1 : 0), wz = lz < 0 ? -1 : (lz >= g.nc2 ? 1 : 0), wx = p - 1;
         const int ls = p == 0 ? xa : (p == 1 ? max(xa, 0) : max(xa, g.nc0));
@@ -138,8 +146,9 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
         if ((wx | wy | wz) != 0 && ls <= le && t.seg_len[tid] > 0) t.any_wrapped = 1;      // benign race: every writer stores 1
         t.seg_code[tid] = (unsigned char)((wx + 1) + 3 * (wy + 1) + 9 * (wz + 1));
     }
-    for (int i = tid; i < nrows * ncol; i += blockDim.x) {
-        const int r = i / ncol, c = i - r * ncol;
+    for (int i = tid; i < nslot; i += blockDim.x) {
+        const int r = i >> g.cshift, c = i & cmask;
+        if (c >= ncol) continue;
         const int lx = xa + c, p = lx < 0 ? 0 : (lx >= g.nc0 ? 2 : 1);
         const int ls = p == 0 ? xa : (p == 1 ? max(xa, 0) : max(xa, g.nc0));
         w.hrel[r][c] = (w.hbeg[r][c] - w.hbeg[r][ls - xa]) | (p << 28);
@@ -160,8 +169,9 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
     }
     __syncthreads();
     // ---- phase 4: local halo-cell starts (thread per halo cell); own rows (last warp, lane per own row)
-    for (int i = tid; i < nrows * (ncol + 1); i += blockDim.x) {
-        const int r = i / (ncol + 1), c = i - r * (ncol + 1);
+    for (int i = tid; i < nslot; i += blockDim.x) {
+        const int r = i >> g.cshift, c = i & cmask;
+        if (c > ncol) continue;
         if (c < ncol) {
             const int v = w.hrel[r][c];
             t.hcell[r][c] = (unsigned short)((v & 0xfffffff) + t.seg_off[3 * r + (v >> 28)]);
@@ -173,7 +183,7 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
         const int q = tid & 31, nq = Tye * Tze;
         int len = 0, l0 = 0, r = 0;
         if (q < nq) {
-            const int oz = q / Tye, oy = q - oz * Tye;
+            const int oz = Tye == 1 ? q : (Tye == 2 ? q >> 1 : (Tye == 4 ? q >> 2 : small_div(q, 3))), oy = q - oz * Tye;
             r = (oz + 1) * (Tye + 2) + (oy + 1);
             // column hx (cell x0) always lies in piece 1; column Txe + hx (cell x0 + Txe) in piece 1 or, at the box end, 2
             const int v1 = w.hrel[r][Txe + hx];

@@ -261,10 +261,11 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
     }
     if (MODE != 0) {
         block_reduce<2>(v, red);
-        if (threadIdx.x == 0) { partials[2 * blockIdx.x] = v[0]; partials[2 * blockIdx.x + 1] = v[1]; }
+        const int bid = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x, nblk = gridDim.x * gridDim.y * gridDim.z;
+        if (threadIdx.x == 0) { partials[2 * bid] = v[0]; partials[2 * bid + 1] = v[1]; }
         if (last_block_ticket(ticket)) {                      // fixed-order sum of the per-tile partials
             double u[2] = { 0.0, 0.0 };
-            for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) { u[0] += partials[2 * b]; u[1] += partials[2 * b + 1]; }
+            for (int b = threadIdx.x; b < nblk; b += blockDim.x) { u[0] += partials[2 * b]; u[1] += partials[2 * b + 1]; }
             block_reduce<2>(u, red);
             if (threadIdx.x == 0) {
                 cv_q6[0] = scale_mean * u[0]; cv_q6[1] = scale_solid * u[1];
@@ -308,13 +309,13 @@ int tiled_init() {
 
 int tiled_build(metad_ctx *c) {
     TileGeom g = tile_geom(c);
-    int nt = g.ntx * g.nty * g.ntz;
+    const dim3 grid3(g.ntx, g.nty, g.ntz);         // tile (tx, ty, tz) = blockIdx: no division in the kernel
     double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
     double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
 #define TILE_LAUNCH(MODE, ...)                                                                                        \
     do {                                                                                                              \
-        if (c->dg) k_tile_build<MODE, true><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(__VA_ARGS__);             \
-        else k_tile_build<MODE, false><<<nt, TILE_THREADS, smem_build(g), c->stream>>>(__VA_ARGS__);                  \
+        if (c->dg) k_tile_build<MODE, true><<<grid3, TILE_THREADS, smem_build(g), c->stream>>>(__VA_ARGS__);          \
+        else k_tile_build<MODE, false><<<grid3, TILE_THREADS, smem_build(g), c->stream>>>(__VA_ARGS__);               \
     } while (0)
     const int *sf = c->skin_on ? c->d_skin_flag : nullptr;
     if (c->has_q6 && !c->skin_on)

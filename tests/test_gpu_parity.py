@@ -421,3 +421,31 @@ def test_fp32_borderline_pairs_across_the_faces_of_a_large_box():
         assert md.status() == 0
         assert np.array_equal(cnt, cref)
         assert np.array_equal(sorted_rows_fast(cnt, lst), sorted_rows_fast(cref, lref))
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_several_list_cvs_in_one_context(precision):
+    """Two coordination numbers with different groups, exponents and r0, an ungrouped one, and a nearest-distance CV in ONE
+    context (each list CV owns two bits of the per-atom group flags): every CV, V, dV/ds, the forces and the bias virial against
+    the oracle, stage-wise."""
+    from paper_2510_06873_b200.inputs import CV_COORD, CV_MINDIST
+    w = _small("c2")
+    cv = w.cvs[0]
+    A, B = np.asarray(cv.group_a), np.asarray(cv.group_b)
+    w.cvs = [CVSpec(kind=CV_COORD, r0=1.2, n=6, m=12, scale=1.0, group_a=A, group_b=B),
+             CVSpec(kind=CV_COORD, r0=1.6, n=8, m=16, scale=1.0 / len(B), group_a=B[::2], group_b=B[1::2]),
+             CVSpec(kind=CV_MINDIST, group_a=A[11:12], group_b=B),
+             CVSpec(kind=CV_COORD, r0=2.0, n=6, m=10, scale=1.0 / w.natoms)]
+    w.sigma = [0.5, 0.05, 0.05, 0.02]
+    w.n_hills = 120
+    r = stagewise(w, precision=precision, want_virial=True)
+    assert_stagewise(r)
+    assert np.all(np.abs(r["dV_ref"]) > 0)
+    W, W_ref = r["md"].virial(), r["o"].virial(r["dV_ref"])
+    assert np.abs(W - W_ref).max() <= (1e-9 if precision == 64 else 1e-5) * np.abs(W_ref).max()
+    # and through the run path with a skin (every list CV filters the kept list on its own)
+    w.stride = 2
+    frames = [wrap(w.pos + np.random.default_rng(3 + k).standard_normal(w.pos.shape) * 0.01 * k, w.box) for k in range(5)]
+    w.max_neigh = 96
+    rr = chained_run(w, precision=precision, nsteps=5, skin=0.3, check_neighbors=True, pos_of_step=lambda k: frames[k])
+    assert rr["md"].rebuilds() < 5
