@@ -69,7 +69,7 @@ __device__ __forceinline__ int scan_atom(const TileGeom &g, const TileTables &t,
                 const int room = (int)((wend - wp) / STRIDE);
                 if (room <= 0) { ovf = true; break; }
                 const int h2 = min(hi, lo + room);
-#pragma unroll 4
+#pragma unroll 2
                 for (int lj = lo; lj < h2; ++lj) {
                     const float4 pj = hpos<STAGED>(g, t, spos, pos_s, lj, dg);
                     // (dx, dy) and their squares as one packed pair each: 5 issue slots instead of 6 per candidate (the
