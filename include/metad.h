@@ -126,7 +126,9 @@ typedef struct {
                                        predicate r < rc on the current positions, so CVs, forces and metad_get_neighbors are those
                                        of the exact rc list at every step.  max_neigh must hold the rc + skin list; the box needs
                                        rc + skin < half of every perpendicular width.  Supported by the list CVs (COORD, Q6_*,
-                                       MINDIST); 0 (default): the list is rebuilt every step */
+                                       MINDIST).  The two rebuild flags alternate with the step counter that metad_deposit
+                                       advances: a caller of the stage calls who never calls metad_deposit gets a rebuild in every
+                                       step after the first one that needed it.  0 (default): the list is rebuilt every step */
     double box_slack;               /* metad_*_dev calls: the cell grid is derived ONCE (first call / after metad_reset_box) with
                                        cells at least rc (1 + box_slack) wide, so the device-resident box may shrink by that
                                        fraction before METAD_DEV_BOX is raised; 0 = cells as small as rc allows */
@@ -272,8 +274,10 @@ int metad_synchronize(metad_ctx *ctx);
 
 /* Proof of the zero-host-copy step (BASELINE.json north_star: "a multi-step loop makes zero host round-trips"; PAPER.md:61 on
  * GPU-CPU transfer overhead): node counts of the CUDA graph metad_run captured last.
- * h_counts: int[8] = { nodes, kernel nodes, memcpy nodes, memset nodes, host nodes, other nodes,
- *                      captures so far, in-place graph updates so far }.
+ * h_counts: int[9] = { nodes, kernel nodes, memcpy nodes, memset nodes, host nodes, other nodes,
+ *                      captures so far, in-place graph updates so far, conditional nodes }.
+ * With params.skin > 0 the graph holds ONE conditional IF node whose body (the list-build kernels) runs only in the steps
+ * whose displacement check asks for a rebuild; the condition is set on the device (cudaGraphSetConditional).
  * Errors: METAD_ERR_STATE before the first metad_run. */
 int metad_graph_info(metad_ctx *ctx, int *h_counts);
 

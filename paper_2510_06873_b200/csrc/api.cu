@@ -280,7 +280,10 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
         const int ones[2] = { 1, 1 };                       // the first step builds
         CUDA_TRY(cudaMemcpy(c->d_skin_flag, ones, sizeof(ones), cudaMemcpyHostToDevice));
         CUDA_TRY(cudaMalloc(&c->d_ref, 4 * tsz * (size_t)N));
-        if (c->has_q6 && c->prec == 32) CUDA_TRY(dev_alloc(&c->d_keep_mask, N));
+        if (c->has_q6 && c->prec == 32 && c->maxn <= 32) {            // the tiled Q6 path may run: its per-step rc list
+            CUDA_TRY(dev_alloc(&c->d_rc_count, N));
+            CUDA_TRY(dev_alloc(&c->d_rc_list, (size_t)c->maxn * (((size_t)N + 31) / 32 * 32)));
+        }
     }
     CUDA_TRY(cudaDeviceSynchronize());
     return METAD_OK;
@@ -290,14 +293,13 @@ extern "C" int metad_destroy(metad_ctx *c) {
     if (!c) return METAD_OK;
     if (c->stream) cudaStreamSynchronize(c->stream);
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
-    if (c->graph) cudaGraphDestroy(c->graph);
     for (int k = 0; k < 3; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     if (c->ev_copy) cudaEventDestroy(c->ev_copy);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage, c->d_geom, c->d_skin_flag, c->d_ref, c->d_nbuilds, c->d_keep_mask, c->d_tile_cuts };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage, c->d_geom, c->d_skin_flag, c->d_ref, c->d_nbuilds, c->d_rc_count, c->d_rc_list, c->d_tile_cuts };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
@@ -542,6 +544,7 @@ static int enqueue_step(metad_ctx *c, const void *d_pos, const double *box, doub
 }
 
 static int run_impl(metad_ctx *c, const void *d_pos, const double *h_box, const double *d_box, double rc, void *d_F, int nsteps);
+static int count_graph_nodes(cudaGraph_t graph, int *k);
 
 extern "C" int metad_run(metad_ctx *c, const void *d_pos, const double *h_box, double rc, void *d_F, int nsteps) {
     if (!c || !d_pos || !d_F || !h_box || nsteps < 0) FAIL(METAD_ERR_ARG, "bad argument");
@@ -578,9 +581,10 @@ static int run_impl(metad_ctx *c, const void *d_pos, const double *h_box, const 
             if (cudaGraphExecUpdate(c->graph_exec, graph, &info) == cudaSuccess) updated = true;
             else { cudaGetLastError(); cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         }
-        if (!updated) CUDA_TRY(cudaGraphInstantiate(&c->graph_exec, graph, 0));
-        if (c->graph) cudaGraphDestroy(c->graph);
-        c->graph = graph;                           // kept for metad_graph_info
+        int cr = count_graph_nodes(graph, c->graph_counts);      // for metad_graph_info (the zero-host-copy proof)
+        if (!updated) { cudaError_t ei = cudaGraphInstantiate(&c->graph_exec, graph, 0); if (ei != cudaSuccess) { cudaGraphDestroy(graph); CUDA_TRY(ei); } }
+        cudaGraphDestroy(graph);
+        if (cr) return cr;
         c->graph_captures++;
         c->graph_updates += updated ? 1 : 0;
         c->launches_per_step = (int)(c->launches - before);
@@ -788,24 +792,37 @@ extern "C" int metad_synchronize(metad_ctx *c) {
     return METAD_OK;
 }
 
-extern "C" int metad_graph_info(metad_ctx *c, int *h_counts) {
-    if (!c || !h_counts) FAIL(METAD_ERR_ARG, "null argument");
-    if (!c->graph) FAIL(METAD_ERR_STATE, "metad_run has not captured a step yet");
+// node counts of a freshly captured step graph (taken before instantiation and cached in the context)
+static int count_graph_nodes(cudaGraph_t graph, int *k /* [9] */) {
     size_t n = 0;
-    CUDA_TRY(cudaGraphGetNodes(c->graph, nullptr, &n));
+    CUDA_TRY(cudaGraphGetNodes(graph, nullptr, &n));
     std::vector<cudaGraphNode_t> nodes(n);
-    if (n) CUDA_TRY(cudaGraphGetNodes(c->graph, nodes.data(), &n));
-    int k[6] = { (int)n, 0, 0, 0, 0, 0 };
+    if (n) CUDA_TRY(cudaGraphGetNodes(graph, nodes.data(), &n));
+    for (int q = 0; q < 9; ++q) k[q] = 0;
+    k[0] = (int)n;
     for (size_t i = 0; i < n; ++i) {
         cudaGraphNodeType t;
-        CUDA_TRY(cudaGraphNodeGetType(nodes[i], &t));
+        if (cudaGraphNodeGetType(nodes[i], &t) != cudaSuccess) {
+            // CUDA 12.9 / driver 580 answers cudaErrorUnknown for a conditional node (the only node kind this library adds by
+            // hand: the skin's IF node); every node a stream capture records has a type the call knows
+            (void)cudaGetLastError();
+            k[8]++;
+            continue;
+        }
         if (t == cudaGraphNodeTypeKernel) k[1]++;
         else if (t == cudaGraphNodeTypeMemcpy) k[2]++;
         else if (t == cudaGraphNodeTypeMemset) k[3]++;
         else if (t == cudaGraphNodeTypeHost) k[4]++;
+        else if (t == cudaGraphNodeTypeConditional) k[8]++;
         else k[5]++;
     }
-    memcpy(h_counts, k, sizeof(k));
+    return METAD_OK;
+}
+
+extern "C" int metad_graph_info(metad_ctx *c, int *h_counts) {
+    if (!c || !h_counts) FAIL(METAD_ERR_ARG, "null argument");
+    if (!c->graph_exec) FAIL(METAD_ERR_STATE, "metad_run has not captured a step yet");
+    memcpy(h_counts, c->graph_counts, sizeof(int) * 9);
     h_counts[6] = c->graph_captures;
     h_counts[7] = c->graph_updates;
     return METAD_OK;

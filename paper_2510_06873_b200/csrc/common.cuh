@@ -238,7 +238,7 @@ struct metad_ctx {
     int geom_ncell;                       // cells of the last setup_geometry before any x-subdivision (skin: detects a new grid)
     int *d_skin_flag;                     // [2] rebuild flags, indexed by the parity of the device step counter (neighbor.cu)
     void *d_ref;                          // Vec4<T>[N]: cell-sorted positions at the last build (displacement check)
-    unsigned long long *d_keep_mask;      // skin, tiled Q6 path: per atom, which entries of the kept list lie within rc this step
+    int *d_rc_count, *d_rc_list;          // skin, tiled Q6 path: the entries of the kept list that lie within rc THIS step (pass 1 -> force pass)
     int *d_nbuilds;                       // number of neighbour-list builds so far (metad_get_rebuilds)
     bool have_neighbors, list_built;
     int cell_cap;
@@ -284,7 +284,7 @@ struct metad_ctx {
     int graph_devbox;                     // the captured graph reads the box from device memory
     const double *graph_dbox;             //   ... from this pointer
     cudaGraphExec_t graph_exec;
-    cudaGraph_t graph;                    // the captured step (kept for metad_graph_info)
+    int graph_counts[9];                  // node counts of the captured step (metad_graph_info)
     int graph_captures, graph_updates;    // how often metad_run captured a step / updated the instantiated graph in place
     int owns_stream;                      // metad_create made the stream (cuda_stream == NULL): destroyed with the context
     double *d_hill_stage;                 // [(D + 1) * max_hills] staging of metad_set_hills / metad_get_hills with host pointers
@@ -317,7 +317,6 @@ static inline int div_up(long long a, int b) { return (int)((a + b - 1) / b); }
 // stage entry points implemented in the .cu files (host functions that enqueue kernels)
 int nb_build(metad_ctx *c, const void *d_pos);
 int geom_update(metad_ctx *c, const double *d_box);
-int skin_check(metad_ctx *c, const void *d_pos);
 int tiled_q6_pass1_skin(metad_ctx *c, double *d_cv);
 int nb_export(metad_ctx *c, int *d_count, int *d_list);
 int cv_eval_all(metad_ctx *c, double *d_cv);

@@ -369,15 +369,15 @@ __device__ __forceinline__ void ldg256(const float *p, float4 &a, float4 &b) {
 
 #define Q6F_MINB 9             // resident blocks per SM of k_q6_force_g (56 registers)
 // SKIN (params.skin): the kept list reaches rc + skin and a neighbour may have crossed a box face since it was built, so the
-// shift codes are ignored: per-pair minimum image on the current positions; pairs beyond rc are skipped by the keep mask that
-// pass 1 (k_q6_pass1_g) wrote for this step, before their records are gathered.
+// shift codes are ignored: per-pair minimum image on the current positions; the kernel walks the compacted rc list that pass 1
+// (k_q6_pass1_g) wrote for this step, so no record of a pair beyond rc is gathered.
 template <bool SOLID, bool VIRIAL, bool DEVBOX, bool SKIN>   // DEVBOX: box in device memory (metad_*_dev); the other instances never touch dg
 __global__ void __launch_bounds__(CV_THREADS, VIRIAL ? 8 : Q6F_MINB)
 k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
              const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, const float *__restrict__ rec,
              double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
              const double *__restrict__ dVds, float *__restrict__ F, VirArgs va, const float *__restrict__ fprime,
-             const DevGeom *__restrict__ dg_arg, PBox<float> pb, const unsigned long long *__restrict__ keep_mask) {
+             const DevGeom *__restrict__ dg_arg, PBox<float> pb) {
     const DevGeom *dg = DEVBOX ? dg_arg : nullptr;
     if (SKIN && DEVBOX && dg) pb = dg->pbf;
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
@@ -409,12 +409,10 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
     // the list entries are fetched two iterations ahead: an entry load (streamed from DRAM) followed by the dependent record
     // gather was 40 % of the stall samples of this kernel (profiles/r1w_ncu.md)
     int e0 = cnt > 0 ? __ldcs(in) : 0, e1 = cnt > 1 ? __ldcs(in + 32) : 0;
-    const unsigned long long km = SKIN && act ? keep_mask[s] : ~0ull;     // skin: which entries of the kept list lie within rc (pass 1)
     for (int k = 0; k < cnt; ++k) {
         const int e = e0;                              // streamed once: do not displace positions / records in L2
         e0 = e1;
         if (k + 2 < cnt) e1 = __ldcs(in + (k + 2) * 32);
-        if (SKIN && !((km >> k) & 1ull)) continue;
         const int j = e & NLG_IDX_MASK, code = (unsigned)e >> 27;
         float4 a4, b4, c4, d4, pj;
         ldg256(rec + (size_t)j * 8, a4, b4);
@@ -422,7 +420,7 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         pj.x = d4.y; pj.y = d4.z; pj.z = d4.w;               // the record carries the position
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         if (SKIN) {
-            min_image(pb, dx, dy, dz);                 // the decision r < rc was taken by pass 1 (keep_mask), on these positions
+            min_image(pb, dx, dy, dz);                 // the decision r < rc was taken by pass 1, on these positions
         } else if (code != 13) {
             const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
             const BoxD &b = dg ? dg->bd : bd;                  // device-resident box (NPT): read at the rare point of use
@@ -476,7 +474,7 @@ k_q6_pass1_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
              float *__restrict__ q6_out, int solid, double scale_mean, double scale_solid, double *__restrict__ partials,
              unsigned int *__restrict__ ticket, double *__restrict__ cv_q6, double *__restrict__ cv_out, int dim0, int dim1,
              unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg,
-             unsigned long long *__restrict__ keep_mask /* bit k: list entry k of the atom lies within rc (read by the force pass) */) {
+             int *__restrict__ rc_count, int *__restrict__ rc_list /* the entries within rc, same sliced layout: read by the force pass */) {
     __shared__ double red[64];
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (DEVBOX) pb = dg->pbf;                      // host-box instance: the box stays in the constant bank
@@ -489,11 +487,11 @@ k_q6_pass1_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
 #pragma unroll
         for (int k = 0; k < 13; ++k) A[k] = 0.f;
         int n = 0;
-        unsigned long long km = 0ull;
+        int *out = rc_list + ((size_t)(s >> 5) * maxn) * 32 + (s & 31);
         // entries two iterations ahead, as in k_q6_force_g: the entry load -> position gather chain is the latency to hide
         int e0 = cnt > 0 ? __ldg(in) : 0, e1 = cnt > 1 ? __ldg(in + 32) : 0;
         for (int k = 0; k < cnt; ++k) {
-            const int j = e0 & NLG_IDX_MASK;
+            const int e = e0, j = e0 & NLG_IDX_MASK;
             e0 = e1;
             if (k + 2 < cnt) e1 = __ldg(in + (k + 2) * 32);
             const float4 pj = spos[j];
@@ -505,8 +503,8 @@ k_q6_pass1_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
                 keep = r2_canonical(DEVBOX ? dg->bd : bd, (double)pj.x - (double)pi.x, (double)pj.y - (double)pi.y,
                                     (double)pj.z - (double)pi.z) < rc2;
             if (!keep) continue;
+            __stcs(out + n * 32, e);                   // read once, by the force pass of this step
             ++n;
-            km |= 1ull << k;
             const float rinv = rsqrtf(r2);
             Y6<float> y;
             y6_eval<float>(dx * rinv, dy * rinv, dz * rinv, y);
@@ -514,7 +512,7 @@ k_q6_pass1_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
 #pragma unroll
             for (int m = 1; m <= 6; ++m) { A[2 * m - 1] += y.E[m] * y.c[m]; A[2 * m] += y.E[m] * y.s[m]; }
         }
-        keep_mask[s] = km;
+        rc_count[s] = n;
         float S = 0.f;
 #pragma unroll
         for (int k = 0; k < 13; ++k) S += A[k] * A[k];
@@ -553,7 +551,7 @@ int tiled_q6_pass1_skin(metad_ctx *c, double *d_cv) {
     c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, ctx_pbox<float>(c), c->boxd, (float)c->rc2, c->rc2,  \
         (float)qt, (float)(1.0 / qw), (float *)c->d_rec, c->d_q6, c->q6_solid_dim >= 0 ? 1 : 0,                            \
         c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0, c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0, \
-        c->d_partials + c->nblocks_atoms, c->d_tickets + 1, c->d_cvq6, d_cv, c->q6_mean_dim, c->q6_solid_dim, c->d_sticky, c->dg, c->d_keep_mask
+        c->d_partials + c->nblocks_atoms, c->d_tickets + 1, c->d_cvq6, d_cv, c->q6_mean_dim, c->q6_solid_dim, c->d_sticky, c->dg, c->d_rc_count, c->d_rc_list
     if (c->dg) k_q6_pass1_g<true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(P1G_ARGS);
     else k_q6_pass1_g<false><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(P1G_ARGS);
 #undef P1G_ARGS
@@ -686,9 +684,8 @@ int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
     const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
 #define Q6FG_ARGS                                                                                                          \
-    c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm, ss,  \
-        c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va, c->d_q6 + c->N, c->dg, ctx_pbox<float>(c),    \
-        c->d_keep_mask
+    c->N, c->maxn, (const float4 *)c->d_spos, c->skin_on ? c->d_rc_count : c->d_nl_count, c->skin_on ? c->d_rc_list : c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm, ss,  \
+        c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va, c->d_q6 + c->N, c->dg, ctx_pbox<float>(c)
 #define Q6FG_GRID <<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>
 #define Q6FG_LAUNCH(SOLID, VIR)                                                                                            \
     do {                                                                                                                   \

@@ -453,10 +453,13 @@ template <typename T>
 __global__ void k_skin_check(int N, const T *__restrict__ pos, const int *__restrict__ perm,
                              const typename Vec4<T>::type *__restrict__ ref, typename Vec4<T>::type *__restrict__ spos, BoxD bd,
                              double half_skin2, int *__restrict__ skin_flag, const int *__restrict__ step,
-                             const DevGeom *__restrict__ dg) {
+                             const DevGeom *__restrict__ dg, cudaGraphConditionalHandle cond, int use_cond) {
     const int cur = *step & 1;
     if (blockIdx.x == 0 && threadIdx.x == 0) skin_flag[cur ^ 1] = 0;
-    if (skin_flag[cur]) return;                   // already decided (first step, new geometry): perm / ref are about to be rebuilt
+    if (skin_flag[cur]) {                         // already decided (first step, new geometry): perm / ref are about to be rebuilt
+        if (use_cond && blockIdx.x == 0 && threadIdx.x == 0) cudaGraphSetConditional(cond, 1);
+        return;
+    }
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
     if (s < N) {
@@ -469,24 +472,74 @@ __global__ void k_skin_check(int N, const T *__restrict__ pos, const int *__rest
         moved = !(dx * dx + dy * dy + dz * dz <= half_skin2);       // also catches NaN
         spos[s] = v;
     }
-    if (__any_sync(0xffffffffu, moved) && (threadIdx.x & 31) == 0) atomicOr(&skin_flag[cur], 1);
+    if (__any_sync(0xffffffffu, moved) && (threadIdx.x & 31) == 0) {
+        atomicOr(&skin_flag[cur], 1);
+        // inside a captured graph the build kernels are the body of a conditional IF node (default: skipped): switch it on
+        if (use_cond) cudaGraphSetConditional(cond, 1);
+    }
 }
 
-int skin_check(metad_ctx *c, const void *d_pos) {
+static int skin_check_launch(metad_ctx *c, const void *d_pos, cudaGraphConditionalHandle cond, int use_cond) {
     const double h2 = 0.25 * c->p.skin * c->p.skin;
     if (c->prec == 32)
         k_skin_check<float><<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, (const float *)d_pos, c->d_perm, (const float4 *)c->d_ref,
-                                                                      (float4 *)c->d_spos, c->boxd, h2, c->d_skin_flag, c->d_step, c->dg);
+                                                                      (float4 *)c->d_spos, c->boxd, h2, c->d_skin_flag, c->d_step, c->dg,
+                                                                      cond, use_cond);
     else
         k_skin_check<double><<<div_up(c->N, 256), 256, 0, c->stream>>>(c->N, (const double *)d_pos, c->d_perm, (const double4 *)c->d_ref,
-                                                                       (double4 *)c->d_spos, c->boxd, h2, c->d_skin_flag, c->d_step, c->dg);
+                                                                       (double4 *)c->d_spos, c->boxd, h2, c->d_skin_flag, c->d_step, c->dg,
+                                                                       cond, use_cond);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
 }
 
+template <typename T> static int nb_build_kernels(metad_ctx *c, const void *d_pos);
+
+// With a skin, inside a stream capture (metad_run), the build kernels become the body of a conditional IF node that
+// k_skin_check switches on from the device (cudaGraphSetConditional): a step that keeps its list launches none of them.
+// Outside a capture (stage calls) the kernels are launched and return at once when the flag is clear.
 template <typename T>
 static int nb_build_t(metad_ctx *c, const void *d_pos) {
+    const bool tm = c->timing && !c->capturing;
+    if (tm) { cudaEventRecord(c->ev[0], c->stream); c->timing_recorded = 1; }
+    if (!c->skin_on) return nb_build_kernels<T>(c, d_pos);
+    if (!c->capturing) {
+        int r = skin_check_launch(c, d_pos, 0, 0);
+        return r ? r : nb_build_kernels<T>(c, d_pos);
+    }
+    cudaStream_t st = c->stream;
+    cudaStreamCaptureStatus status;
+    unsigned long long id;
+    cudaGraph_t graph;
+    const cudaGraphNode_t *deps;
+    size_t ndeps;
+    CUDA_TRY(cudaStreamGetCaptureInfo(st, &status, &id, &graph, &deps, &ndeps));
+    cudaGraphConditionalHandle cond;
+    CUDA_TRY(cudaGraphConditionalHandleCreate(&cond, graph, 0, cudaGraphCondAssignDefault));
+    int r = skin_check_launch(c, d_pos, cond, 1);
+    if (r) return r;
+    CUDA_TRY(cudaStreamGetCaptureInfo(st, &status, &id, &graph, &deps, &ndeps));      // now: the check kernel
+    cudaGraphNodeParams np = {};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = cond;
+    np.conditional.type = cudaGraphCondTypeIf;
+    np.conditional.size = 1;
+    cudaGraphNode_t cnode;
+    CUDA_TRY(cudaGraphAddNode(&cnode, graph, deps, ndeps, &np));
+    CUDA_TRY(cudaStreamBeginCaptureToGraph(c->copy_stream, np.conditional.phGraph_out[0], nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+    c->stream = c->copy_stream;                   // the build kernels are captured into the body graph
+    r = nb_build_kernels<T>(c, d_pos);
+    c->stream = st;
+    cudaError_t e = cudaStreamEndCapture(c->copy_stream, nullptr);
+    if (r) return r;
+    CUDA_TRY(e);
+    CUDA_TRY(cudaStreamUpdateCaptureDependencies(st, &cnode, 1, cudaStreamSetCaptureDependencies));
+    return METAD_OK;
+}
+
+template <typename T>
+static int nb_build_kernels(metad_ctx *c, const void *d_pos) {
     typedef typename Vec4<T>::type V4;
     const int N = c->N, ncell = c->grid.ncell;
     cudaStream_t st = c->stream;
@@ -494,8 +547,6 @@ static int nb_build_t(metad_ctx *c, const void *d_pos) {
     const bool tm = c->timing && !c->capturing;
     const int *sf = c->skin_on ? c->d_skin_flag : nullptr, *stp = c->d_step;
     V4 *ref = c->skin_on ? (V4 *)c->d_ref : nullptr;
-    if (tm) { cudaEventRecord(c->ev[0], st); c->timing_recorded = 1; }
-    if (c->skin_on) { int r = skin_check(c, d_pos); if (r) return r; }
     if (N <= METAD_SMALL_N && !c->tiled) {                     // the whole neighbour stage in one launch
         if (tm) cudaEventRecord(c->ev[1], st);
         k_build_list_small<T><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const T *)d_pos, c->d_flags, (V4 *)c->d_spos, c->d_perm,

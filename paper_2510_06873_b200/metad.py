@@ -400,7 +400,7 @@ class MetaD:
 
     def graph_info(self):
         """Node counts of the captured step graph (metad_graph_info)."""
-        k = (ctypes.c_int * 8)()
+        k = (ctypes.c_int * 9)()
         _check(load().metad_graph_info(self._h, k))
-        names = ("nodes", "kernel", "memcpy", "memset", "host", "other", "captures", "updates")
+        names = ("nodes", "kernel", "memcpy", "memset", "host", "other", "captures", "updates", "conditional")
         return dict(zip(names, (int(x) for x in k)))

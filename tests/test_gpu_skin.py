@@ -47,7 +47,9 @@ def test_skin_reuse_matches_the_exact_list_every_step(name, precision):
     nb = md.rebuilds()
     assert 1 <= nb < nsteps, nb                   # the list was kept over most steps ...
     gi = md.graph_info()
-    assert gi["captures"] == 1 and gi["nodes"] == gi["kernel"] and gi["memcpy"] == 0 and gi["memset"] == 0   # ... decided on the device
+    # ... decided on the device: kernel nodes + ONE conditional node (the build kernels are its body), nothing that touches the host
+    assert gi["captures"] == 1 and gi["conditional"] == 1 and gi["nodes"] == gi["kernel"] + 1
+    assert gi["memcpy"] == gi["memset"] == gi["host"] == gi["other"] == 0
     # the same walk without a skin: same physics, a build every step
     r0 = chained_run(w, precision=precision, nsteps=nsteps, skin=0.0, hills=r["hills0"], pos_of_step=lambda k: frames[k])
     assert r0["md"].rebuilds() == nsteps
