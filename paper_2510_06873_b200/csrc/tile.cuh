@@ -1,11 +1,11 @@
-// tile.cuh — shared-memory tiling of the cell grid (fp32 fast path; DESIGN.md §5.2).
+// tile.cuh — shared-memory tiling of the cell grid (fp32 fast path; DESIGN.md §6).
 //
-// A thread block owns a tile of Tx x Ty x Tz cells.  Its halo = the tile grown by one cell in
-// every direction = (Ty+2)(Tz+2) "rows", each row a run of Tx+2 cells that is contiguous in the
-// cell-sorted atom order (up to a periodic split into <= 3 pieces A|B|C with lattice shift -a|0|+a).
-// The halo atoms are numbered 0..total-1 in (row, piece, atom) order: the LOCAL index.  Neighbour
-// lists of the tiled path store local indices (uint16), so that the CV and force kernels gather
-// positions and q6 records straight from shared memory.
+// A thread block owns a tile of Tx x Ty x Tz cells (x counted in sub-cells: the rc-wide cells are split hx-fold along x).
+// Its halo = the tile grown by hx sub-cells in x and one cell in y and z = (Ty+2)(Tz+2) "rows", each row a run of Tx+2hx
+// sub-cells that is contiguous in the cell-sorted atom order (up to a periodic split into <= 3 pieces A|B|C with lattice
+// shift -a|0|+a).  The halo atoms are numbered 0..total-1 in (row, piece, atom) order: the LOCAL index, used by the
+// per-thread candidate lists in shared memory (uint16); the neighbour list written to global memory holds global sorted
+// indices | lattice-shift code << 27.
 //
 // Positions are staged in tile-local coordinates  p - origin (+ lattice shift for periodic images):
 // for atoms of the primary cell the subtraction is exact in fp32 (origin is the point of the tile's
