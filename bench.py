@@ -485,7 +485,24 @@ def run_ours(args):
                              "achieved": p1 / (stage_ms[1] * 1e-3) / 1e12, "peak": f64_peak, "unit": "TFLOP/s",
                              "frac": p1 / (stage_ms[1] * 1e-3) / 1e12 / f64_peak, "traffic": None, "peak_source": f64_src,
                              "algorithmic_flops_per_launch": p1, "kernel_ms": float(stage_ms[1])})
-        if precision == 32 and list_ms is not None:
+        if precision == 32 and args.skin > 0.0:
+            # skin mode: the stage calls above found the list still valid, so eval_cv timed k_q6_pass1_g (Q6 pass 1 over the stored
+            # rc + skin list).  Algorithmic bytes: the list entries (4 B each, mean rc + skin count), the sorted positions once,
+            # the 64-byte record and q6 / f' written per atom; flops: the same Y6m accumulation as the fused build (85 per pair)
+            nbl = nb * ((w.rc + args.skin) / w.rc) ** 3
+            by1 = (4.0 * nbl + 16 + 64 + 8 + 4.0 * nb) * w.natoms
+            a1 = by1 / (stage_ms[1] * 1e-3) / 1e9
+            roof_all.append({"kernel": "k_q6_pass1_g (stage eval_cv, list kept)", "bound": "hbm", "achieved": a1, "peak": hbm_peak,
+                             "unit": "GB/s", "frac": a1 / hbm_peak, "traffic": None, "peak_source": peak_src,
+                             "algorithmic_bytes_per_launch": by1, "kernel_ms": float(stage_ms[1]), "mean_list_entries": nbl})
+            if stage_ms[1] > stage_ms[3]:
+                roof = roof_all[-1]                # the dominant kernel of a step that keeps its list
+            fl1 = (12.0 * nbl + 85.0 * nb) * w.natoms
+            roof_all.append({"kernel": "k_q6_pass1_g, scalar-pipe view", "bound": "alu", "achieved": fl1 / (stage_ms[1] * 1e-3) / 1e12,
+                             "peak": f32_peak, "unit": "TFLOP/s", "frac": fl1 / (stage_ms[1] * 1e-3) / 1e12 / f32_peak,
+                             "traffic": None, "peak_source": f32_src, "algorithmic_flops_per_launch": fl1,
+                             "kernel_ms": float(stage_ms[1])})
+        elif precision == 32 and list_ms is not None:
             # a1+a3: candidate scan fused with Q6 pass 1 — plain FP32 ALU / issue bound (no tensor-core work on this path)
             fl = algo_build_flops(nb) * w.natoms
             ach_tf = fl / (list_ms * 1e-3) / 1e12
@@ -496,7 +513,7 @@ def run_ours(args):
             roof_all.append(r_build)
             if list_ms > stage_ms[3]:
                 roof = r_build                     # the dominant kernel of the step
-            # what actually binds both kernels is instruction issue (profiles/r2g_ncu.md), so the same launches are also put
+            # what actually binds both kernels is instruction issue (profiles/r2h_ncu.md), so the same launches are also put
             # against the issue peak 148 SMs x 4 schedulers x 1.965 GHz, with the executed warp instructions ncu counted
             for key, kms, nm in (("build_warp_instructions", list_ms, "k_tile_build<Q6>"), ("force_warp_instructions", stage_ms[3], "k_q6_force_g")):
                 if traffic.get(key):
