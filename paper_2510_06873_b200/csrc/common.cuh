@@ -125,6 +125,28 @@ __device__ __forceinline__ bool pair_in_range<float>(const PBox<float> &pb, cons
 
 // Verlet-skin reuse (params.skin): the build kernels of a step do nothing unless the step's rebuild flag is set
 // (k_skin_check, neighbor.cu); flag == NULL: no skin, always build
+// Programmatic dependent launch (sort phase and tile build): a kernel launched with klaunch_pdl(true, ...) may be scheduled while its
+// predecessor in the stream still drains; pdl_enter() at its top (1) lets ITS successor be scheduled likewise and (2) waits until the
+// predecessor grid has completed and its writes are visible.  Nothing is read or written before it, so the chain is as ordered as
+// plain stream order; what is gained is the launch latency at every kernel boundary: 10 us per build on the stream paths (stage
+// calls, metad_step_host), nothing inside the captured graph, whose node-to-node latency is already small.  The hill sum and the
+// force kernel are NOT launched this way: their early-resident blocks cost the tail of k_tile_build 0.11 ms (measured,
+// profiles/r2_experiments.md).  A kernel launched without the attribute passes through both instructions at once.
+__device__ __forceinline__ void pdl_enter() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+template <typename... P, typename... A>
+static inline void klaunch_pdl(bool pdl, void (*kernel)(P...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, A &&...args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    (void)cudaLaunchKernelEx(&cfg, kernel, static_cast<P>(args)...);          // errors surface through cudaGetLastError at the call sites
+}
+
 #define SKIN_SKIP(flag, step) ((flag) != nullptr && (flag)[*(step) & 1] == 0)
 
 // fp64 minimum image in the order of reading O (chain / torsion CVs, fused small-molecule step)

@@ -18,6 +18,7 @@ template <typename T>
 __global__ void k_bin(int N, const T *__restrict__ pos, CellGrid g, int *__restrict__ cell_of,
                       int *__restrict__ slot, int *__restrict__ cell_count, unsigned int *__restrict__ sticky,
                       const DevGeom *__restrict__ dg, const int *__restrict__ skin_flag, const int *__restrict__ step) {
+    pdl_enter();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N || SKIN_SKIP(skin_flag, step)) return;
     if (dg) { g.inv[0] = dg->inv[0]; g.inv[1] = dg->inv[1]; g.inv[2] = dg->inv[2]; g.cx = dg->cx; g.cy = dg->cy; g.bx = dg->bx; }
@@ -41,6 +42,7 @@ __global__ void k_bin(int N, const T *__restrict__ pos, CellGrid g, int *__restr
 __global__ void k_scan_sums(int ncell, const int *__restrict__ cell_count, int *__restrict__ block_sums,
                             const int *__restrict__ skin_flag, const int *__restrict__ step) {
     __shared__ int ws[32];
+    pdl_enter();
     if (SKIN_SKIP(skin_flag, step)) return;
     int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
     int s = 0;
@@ -63,6 +65,7 @@ __global__ void k_scan_apply(int ncell, int N, int *__restrict__ cell_count, con
                              int *__restrict__ cell_start, const int *__restrict__ skin_flag, const int *__restrict__ step) {
     __shared__ int ws[32];
     __shared__ int s_prefix;
+    pdl_enter();
     if (SKIN_SKIP(skin_flag, step)) return;
     // prefix of the preceding blocks' sums
     int pre = 0;
@@ -122,6 +125,7 @@ __global__ void k_scan_apply(int ncell, int N, int *__restrict__ cell_count, con
 __global__ void k_scatter(int N, const int *__restrict__ cell_of, const int *__restrict__ slot,
                           const int *__restrict__ cell_start, int *__restrict__ perm,
                           const int *__restrict__ skin_flag, const int *__restrict__ step) {
+    pdl_enter();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N || SKIN_SKIP(skin_flag, step)) return;
     perm[cell_start[cell_of[i]] + slot[i]] = i;
@@ -137,6 +141,7 @@ __global__ void k_cell_sort_gather(int N, const int *__restrict__ cell_start, co
                                    typename Vec4<T>::type *__restrict__ spos, int *__restrict__ scell, int index_in_w,
                                    typename Vec4<T>::type *__restrict__ ref /* skin: positions at the build, else NULL */,
                                    const int *__restrict__ skin_flag, const int *__restrict__ step, int *__restrict__ nbuilds) {
+    pdl_enter();
     int a = blockIdx.x * blockDim.x + threadIdx.x;
     if (a >= N || SKIN_SKIP(skin_flag, step)) return;
     if (a == 0 && nbuilds) ++*nbuilds;            // list builds so far (metad_get_rebuilds)
@@ -557,14 +562,19 @@ static int nb_build_kernels(metad_ctx *c, const void *d_pos) {
         CUDA_TRY(cudaGetLastError());
         return METAD_OK;
     }
-    k_bin<T><<<div_up(N, 256), 256, 0, st>>>(N, (const T *)d_pos, c->grid, c->d_cell_of, c->d_slot, c->d_cell_count,
-                                             c->d_sticky, c->dg, sf, stp);
-    k_scan_sums<<<nsb, SCAN_THREADS, 0, st>>>(ncell, c->d_cell_count, c->d_block_sums, sf, stp);
-    k_scan_apply<<<nsb, SCAN_THREADS, 0, st>>>(ncell, N, c->d_cell_count, c->d_block_sums, c->d_cell_start, sf, stp);
-    k_scatter<<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_of, c->d_slot, c->d_cell_start, c->d_perm_raw, sf, stp);
-    k_cell_sort_gather<T><<<div_up(N, 256), 256, 0, st>>>(N, c->d_cell_start, c->d_cell_of, c->d_perm_raw, c->d_perm, (const T *)d_pos,
-                                                             c->d_flags,   /* NULL unless a COORD / MINDIST CV has groups */
-                                                             (V4 *)c->d_spos, c->d_scell, c->tiled ? 1 : 0, ref, sf, stp, c->d_nbuilds);
+    // the kernels of the step chain are launched as programmatic dependents of one another (common.cuh: pdl_enter); not in skin
+    // mode, where the build sits in the body of a conditional graph node
+    const bool pdl = !c->skin_on;
+    klaunch_pdl(pdl, k_bin<T>, div_up(N, 256), 256, 0, st, N, (const T *)d_pos, c->grid, c->d_cell_of, c->d_slot, c->d_cell_count,
+                c->d_sticky, (const DevGeom *)c->dg, sf, stp);
+    klaunch_pdl(pdl, k_scan_sums, nsb, SCAN_THREADS, 0, st, ncell, (const int *)c->d_cell_count, c->d_block_sums, sf, stp);
+    klaunch_pdl(pdl, k_scan_apply, nsb, SCAN_THREADS, 0, st, ncell, N, c->d_cell_count, (const int *)c->d_block_sums, c->d_cell_start, sf, stp);
+    klaunch_pdl(pdl, k_scatter, div_up(N, 256), 256, 0, st, N, (const int *)c->d_cell_of, (const int *)c->d_slot, (const int *)c->d_cell_start,
+                c->d_perm_raw, sf, stp);
+    klaunch_pdl(pdl, k_cell_sort_gather<T>, div_up(N, 256), 256, 0, st, N, (const int *)c->d_cell_start, (const int *)c->d_cell_of,
+                (const int *)c->d_perm_raw, c->d_perm, (const T *)d_pos,
+                (const unsigned char *)c->d_flags,   /* NULL unless a COORD / MINDIST CV has groups */
+                (V4 *)c->d_spos, c->d_scell, c->tiled ? 1 : 0, ref, sf, stp, c->d_nbuilds);
     if (tm) cudaEventRecord(c->ev[1], st);
     if (c->tiled && sizeof(T) == 4) {
         c->launches += 5;

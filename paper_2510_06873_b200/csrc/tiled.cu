@@ -234,6 +234,7 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
              double *__restrict__ cv_out /* the context's CV vector on the run paths (NULL: k_q6_publish hands the sums over) */,
              int dim0, int dim1, const DevGeom *__restrict__ dg_arg,
              const int *__restrict__ skin_flag, const int *__restrict__ step) {
+    pdl_enter();
     if (MODE == 0 && SKIN_SKIP(skin_flag, step)) return;        // Verlet skin: the kept list is still valid (neighbor.cu)
     const DevGeom *dg = DEVBOX ? dg_arg : nullptr;
     extern __shared__ float4 dyn_smem[];
@@ -314,8 +315,8 @@ int tiled_build(metad_ctx *c) {
     double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
 #define TILE_LAUNCH(MODE, ...)                                                                                        \
     do {                                                                                                              \
-        if (c->dg) k_tile_build<MODE, true><<<grid3, TILE_THREADS, smem_build(g), c->stream>>>(__VA_ARGS__);          \
-        else k_tile_build<MODE, false><<<grid3, TILE_THREADS, smem_build(g), c->stream>>>(__VA_ARGS__);               \
+        if (c->dg) klaunch_pdl(!c->skin_on, k_tile_build<MODE, true>, grid3, TILE_THREADS, smem_build(g), c->stream, __VA_ARGS__);   \
+        else klaunch_pdl(!c->skin_on, k_tile_build<MODE, false>, grid3, TILE_THREADS, smem_build(g), c->stream, __VA_ARGS__);        \
     } while (0)
     const int *sf = c->skin_on ? c->d_skin_flag : nullptr;
     if (c->has_q6 && !c->skin_on)
