@@ -293,6 +293,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     if (!c) return METAD_OK;
     if (c->stream) cudaStreamSynchronize(c->stream);
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->graph_exec_h) cudaGraphExecDestroy(c->graph_exec_h);
     for (int k = 0; k < 3; ++k) if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     if (c->ev_copy) cudaEventDestroy(c->ev_copy);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
@@ -522,6 +523,7 @@ static int enqueue_step(metad_ctx *c, const void *d_pos, const double *box, doub
         if (d_box) { c->dg = c->d_geom; c->d_box_last = d_box; if ((r = geom_update(c, d_box))) return r; }
         else { c->dg = nullptr; if ((r = setup_geometry(c, box, rc))) return r; }
         c->d_pos_last = d_pos; c->have_neighbors = true; c->list_built = false;
+        if (c->wait_copy) CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_copy, cudaEventWaitExternal));
         return bias_fused_torsion_step(c, d_pos, d_F);
     }
     // without a grid the deposition rides on the hill sum (one launch less; same V, same order of effects: the forces of
@@ -539,8 +541,41 @@ static int enqueue_step(metad_ctx *c, const void *d_pos, const double *box, doub
     c->cv_direct = nullptr;
     if (r) return r;
     if ((r = bias_eval(c, c->d_cv, c->d_V, c->d_dVds, fuse))) return r;
+    // metad_step_host: the caller's forces travel on the copy stream while the build, the CVs and the bias run; the force
+    // kernel waits for them (an external event-wait node of the captured step)
+    if (c->wait_copy) CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_copy, cudaEventWaitExternal));
     if ((r = metad_apply_forces(c, c->d_dVds, d_F))) return r;
     return fuse ? METAD_OK : metad_deposit(c, c->d_cv, c->d_V);
+}
+
+// One step captured into a graph (the caller instantiates it or updates its instantiated graph).  Argument errors must have
+// surfaced before: the geometry is derived outside the capture.
+static int capture_step(metad_ctx *c, const void *d_pos, const double *h_box, const double *d_box, double rc, void *d_F,
+                        bool wait_copy, cudaGraph_t *graph, int *launches_per_step) {
+    const long long before = c->launches;
+    CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+    c->capturing = 1; c->wait_copy = wait_copy ? 1 : 0;
+    int r = enqueue_step(c, d_pos, h_box, rc, d_F, d_box);
+    c->capturing = 0; c->wait_copy = 0;
+    cudaError_t e = cudaStreamEndCapture(c->stream, graph);
+    *launches_per_step = (int)(c->launches - before);
+    c->launches = before;                          // capture enqueued nothing
+    if (r) { if (e == cudaSuccess) cudaGraphDestroy(*graph); return r; }
+    CUDA_TRY(e);
+    return METAD_OK;
+}
+
+// a changed box (NPT) or pointer changes kernel arguments and grid sizes, not the topology: update the
+// instantiated graph in place when the driver allows it, re-instantiate otherwise
+static int instantiate_or_update(cudaGraphExec_t *exec, cudaGraph_t graph, bool *updated) {
+    *updated = false;
+    if (*exec) {
+        cudaGraphExecUpdateResultInfo info;
+        if (cudaGraphExecUpdate(*exec, graph, &info) == cudaSuccess) *updated = true;
+        else { cudaGetLastError(); cudaGraphExecDestroy(*exec); *exec = nullptr; }
+    }
+    if (!*updated) CUDA_TRY(cudaGraphInstantiate(exec, graph, 0));
+    return METAD_OK;
 }
 
 static int run_impl(metad_ctx *c, const void *d_pos, const double *h_box, const double *d_box, double rc, void *d_F, int nsteps);
@@ -564,31 +599,18 @@ static int run_impl(metad_ctx *c, const void *d_pos, const double *h_box, const 
         // argument errors surface before the capture starts; a device box is read ONCE here to derive the frozen cell grid
         int r = d_box ? dev_geometry(c, d_box, rc) : setup_geometry(c, h_box, rc);
         if (r) return r;
-        long long before = c->launches;
         cudaGraph_t graph;
-        CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
-        c->capturing = 1;
-        r = enqueue_step(c, d_pos, h_box, rc, d_F, d_box);
-        c->capturing = 0;
-        cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
-        if (r) { if (e == cudaSuccess) cudaGraphDestroy(graph); return r; }
-        CUDA_TRY(e);
-        // a changed box (NPT) or pointer changes kernel arguments and grid sizes, not the topology: update the
-        // instantiated graph in place when the driver allows it, re-instantiate otherwise
-        bool updated = false;
-        if (c->graph_exec) {
-            cudaGraphExecUpdateResultInfo info;
-            if (cudaGraphExecUpdate(c->graph_exec, graph, &info) == cudaSuccess) updated = true;
-            else { cudaGetLastError(); cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
-        }
+        int lps = 0;
+        if ((r = capture_step(c, d_pos, h_box, d_box, rc, d_F, false, &graph, &lps))) return r;
         int cr = count_graph_nodes(graph, c->graph_counts);      // for metad_graph_info (the zero-host-copy proof)
-        if (!updated) { cudaError_t ei = cudaGraphInstantiate(&c->graph_exec, graph, 0); if (ei != cudaSuccess) { cudaGraphDestroy(graph); CUDA_TRY(ei); } }
+        bool updated = false;
+        r = instantiate_or_update(&c->graph_exec, graph, &updated);
         cudaGraphDestroy(graph);
+        if (r) return r;
         if (cr) return cr;
         c->graph_captures++;
         c->graph_updates += updated ? 1 : 0;
-        c->launches_per_step = (int)(c->launches - before);
-        c->launches = before;                      // capture enqueued nothing
+        c->launches_per_step = lps;
         c->graph_pos = d_pos; c->graph_F = d_F; c->graph_rc = rc;
         c->graph_devbox = d_box != nullptr; c->graph_dbox = d_box;
         if (h_box) memcpy(c->graph_box, h_box, sizeof(double) * 9);
@@ -602,27 +624,29 @@ extern "C" int metad_step_host(metad_ctx *c, const void *h_pos, const double *h_
                                double *h_cv, double *h_V) {
     if (!c || !h_pos || !h_F || !h_box) FAIL(METAD_ERR_ARG, "null argument");
     const size_t bytes = 3 * (size_t)c->N * (c->prec == 32 ? sizeof(float) : sizeof(double));
+    // the kernels of the step are a captured graph on the staging buffers (lower node-to-node latency than eight stream
+    // launches), re-captured only when the box or the cutoff changes
+    int r;
+    const bool same = c->graph_exec_h && c->graph_h_rc == rc && memcmp(c->graph_h_box, h_box, sizeof(double) * 9) == 0;
+    if (!same) {
+        if ((r = setup_geometry(c, h_box, rc))) return r;
+        cudaGraph_t graph;
+        int lps = 0;
+        if ((r = capture_step(c, c->d_pos_stage, h_box, nullptr, rc, c->d_F_stage, true, &graph, &lps))) return r;
+        bool updated = false;
+        r = instantiate_or_update(&c->graph_exec_h, graph, &updated);
+        cudaGraphDestroy(graph);
+        if (r) return r;
+        c->launches_per_step_h = lps;
+        c->graph_h_rc = rc; memcpy(c->graph_h_box, h_box, sizeof(double) * 9);
+    }
     // positions first; the caller's forces travel on a second stream while the neighbour build, the CVs and the bias
     // run (they are not needed before apply_forces)
     CUDA_TRY(cudaMemcpyAsync(c->d_pos_stage, h_pos, bytes, cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(cudaMemcpyAsync(c->d_F_stage, h_F, bytes, cudaMemcpyHostToDevice, c->copy_stream));
     CUDA_TRY(cudaEventRecord(c->ev_copy, c->copy_stream));
-    int r;
-    if (fused_torsion_ok(c)) {
-        CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_copy, 0));
-        if ((r = enqueue_step(c, c->d_pos_stage, h_box, rc, c->d_F_stage))) return r;
-    } else {
-        const bool fuse = !c->grid_on;            // as in enqueue_step
-        c->cv_direct = c->d_cv;
-        r = metad_build_neighbors(c, c->d_pos_stage, h_box, rc);
-        if (!r) r = metad_eval_cv(c, c->d_cv);
-        c->cv_direct = nullptr;
-        if (r) return r;
-        if ((r = bias_eval(c, c->d_cv, c->d_V, c->d_dVds, fuse))) return r;
-        CUDA_TRY(cudaStreamWaitEvent(c->stream, c->ev_copy, 0));
-        if ((r = metad_apply_forces(c, c->d_dVds, c->d_F_stage))) return r;
-        if (!fuse && (r = metad_deposit(c, c->d_cv, c->d_V))) return r;
-    }
+    CUDA_TRY(cudaGraphLaunch(c->graph_exec_h, c->stream));
+    c->launches += c->launches_per_step_h;
     CUDA_TRY(cudaMemcpyAsync(h_F, c->d_F_stage, bytes, cudaMemcpyDeviceToHost, c->stream));
     if (h_cv) CUDA_TRY(cudaMemcpyAsync(h_cv, c->d_cv, sizeof(double) * c->D, cudaMemcpyDeviceToHost, c->stream));
     if (h_V) CUDA_TRY(cudaMemcpyAsync(h_V, c->d_V, sizeof(double), cudaMemcpyDeviceToHost, c->stream));

@@ -306,6 +306,8 @@ struct metad_ctx {
     int graph_devbox;                     // the captured graph reads the box from device memory
     const double *graph_dbox;             //   ... from this pointer
     cudaGraphExec_t graph_exec;
+    cudaGraphExec_t graph_exec_h;         // metad_step_host: the step on the staging buffers (waits for the F upload before the forces)
+    double graph_h_rc, graph_h_box[9]; int launches_per_step_h, wait_copy;
     int graph_counts[9];                  // node counts of the captured step (metad_graph_info)
     int graph_captures, graph_updates;    // how often metad_run captured a step / updated the instantiated graph in place
     int owns_stream;                      // metad_create made the stream (cuda_stream == NULL): destroyed with the context
