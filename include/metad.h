@@ -186,8 +186,9 @@ int metad_run_dev(metad_ctx *ctx, const void *d_pos, const double *d_box, double
 /* Forget the frozen cell grid (and the captured graph): the next *_dev call derives it again from the then current box. */
 int metad_reset_box(metad_ctx *ctx);
 
-/* One step with HOST buffers (end-to-end path): copies h_pos -> device, h_F -> device, runs the
- * five stages, copies F, cv[ncv] and V back.  [sync] */
+/* One step with HOST buffers (end-to-end path): copies h_pos -> device, h_F -> device (on a second stream, while the
+ * neighbour build, the CVs and the bias run), runs the five stages as one captured graph on the library's staging buffers
+ * (re-captured only when h_box or rc changes), copies F, cv[ncv] and V back.  [sync] */
 int metad_step_host(metad_ctx *ctx, const void *h_pos, const double *h_box, double rc, void *h_F,
                     double *h_cv, double *h_V);
 
