@@ -125,6 +125,8 @@ __device__ __forceinline__ bool pair_in_range<float>(const PBox<float> &pb, cons
 
 // Verlet-skin reuse (params.skin): the build kernels of a step do nothing unless the step's rebuild flag is set
 // (k_skin_check, neighbor.cu); flag == NULL: no skin, always build
+#define SKIN_SKIP(flag, step) ((flag) != nullptr && (flag)[*(step) & 1] == 0)
+
 // Programmatic dependent launch (sort phase and tile build): a kernel launched with klaunch_pdl(true, ...) may be scheduled while its
 // predecessor in the stream still drains; pdl_enter() at its top (1) lets ITS successor be scheduled likewise and (2) waits until the
 // predecessor grid has completed and its writes are visible.  Nothing is read or written before it, so the chain is as ordered as
@@ -146,8 +148,6 @@ static inline void klaunch_pdl(bool pdl, void (*kernel)(P...), dim3 grid, dim3 b
     cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
     (void)cudaLaunchKernelEx(&cfg, kernel, static_cast<P>(args)...);          // errors surface through cudaGetLastError at the call sites
 }
-
-#define SKIN_SKIP(flag, step) ((flag) != nullptr && (flag)[*(step) & 1] == 0)
 
 // fp64 minimum image in the order of reading O (chain / torsion CVs, fused small-molecule step)
 __device__ __forceinline__ void min_image_d(const BoxD &b, double &dx, double &dy, double &dz) {
