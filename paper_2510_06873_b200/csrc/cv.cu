@@ -375,18 +375,30 @@ __device__ __forceinline__ void ldg256(const float *p, float4 &a, float4 &b) {
 }
 
 #define Q6F_MINB 9             // resident blocks per SM of k_q6_force_g (56 registers)
-// SKIN (params.skin): the kept list reaches rc + skin and a neighbour may have crossed a box face since it was built, so the
-// shift codes are ignored: per-pair minimum image on the current positions; the kernel walks the compacted rc list that pass 1
-// (k_q6_pass1_g) wrote for this step, so no record of a pair beyond rc is gathered.
+// SKIN (params.skin): the kept list reaches rc + skin and a neighbour may have crossed a box face since it was built (the caller
+// re-wraps), so the shift codes are ignored and the image is found from the current positions.  The raw difference d = pj - pi
+// settles almost every pair: with perpendicular box widths W >= 2 (rc + skin) (the box check of this mode) any other image lies
+// at |d - t| >= W - |d|, so for |d|^2 <= far2 = (rc + 2 skin)^2 (1 - 1e-4) no other image is within rc — d is the minimum
+// image if |d| < rc and the pair is out of range otherwise.  Only pairs beyond far2 (across a periodic face, a few %) take the
+// minimum image, in fp64 on the exact fp32 inputs (the fp32 form is not accurate enough for the forces in a 255 A box,
+// profiles/r2_experiments.md).  Pass 1 and the force pass share this function, so both see the same displacement.
+__device__ __forceinline__ void skin_displacement(const BoxD &b, float far2, const float4 &pi, const float4 &pj,
+                                                  float &dx, float &dy, float &dz) {
+    if (dx * dx + dy * dy + dz * dz > far2) {
+        double ex = (double)pj.x - (double)pi.x, ey = (double)pj.y - (double)pi.y, ez = (double)pj.z - (double)pi.z;
+        min_image_d(b, ex, ey, ez);
+        dx = (float)ex; dy = (float)ey; dz = (float)ez;
+    }
+}
+// The kernel walks the compacted rc list that pass 1 (k_q6_pass1_g) wrote for this step, so no record of a pair beyond rc is gathered.
 template <bool SOLID, bool VIRIAL, bool DEVBOX, bool SKIN>   // DEVBOX: box in device memory (metad_*_dev); the other instances never touch dg
 __global__ void __launch_bounds__(CV_THREADS, VIRIAL ? 8 : Q6F_MINB)
 k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__restrict__ nl_count,
              const int *__restrict__ nl, const int *__restrict__ perm, BoxD bd, const float *__restrict__ rec,
              double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
              const double *__restrict__ dVds, float *__restrict__ F, VirArgs va, const float *__restrict__ fprime,
-             const DevGeom *__restrict__ dg_arg, PBox<float> pb) {
+             const DevGeom *__restrict__ dg_arg, float far2 /* SKIN: see skin_displacement */) {
     const DevGeom *dg = DEVBOX ? dg_arg : nullptr;
-    if (SKIN && DEVBOX && dg) pb = dg->pbf;
     __shared__ double vsm[VIRIAL ? 9 * 32 : 1];
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (!VIRIAL && s >= N) return;
@@ -427,7 +439,7 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         pj.x = d4.y; pj.y = d4.z; pj.z = d4.w;               // the record carries the position
         float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         if (SKIN) {
-            min_image(pb, dx, dy, dz);                 // the decision r < rc was taken by pass 1, on these positions
+            skin_displacement(dg ? dg->bd : bd, far2, pi, pj, dx, dy, dz);   // the image pass 1 decided r < rc on
         } else if (code != 13) {
             const int wx = code % 3 - 1, wy = (code / 3) % 3 - 1, wz = code / 9 - 1;
             const BoxD &b = dg ? dg->bd : bd;                  // device-resident box (NPT): read at the rare point of use
@@ -471,7 +483,7 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
 }
 
 // Q6 pass 1 from the KEPT list of the tiled fp32 path (params.skin): thread per atom over the sliced list, one 128-bit
-// position gather per entry, per-pair minimum image (shift codes ignored, see k_q6_force_g), pairs beyond rc skipped with the
+// position gather per entry, image from the current positions (skin_displacement), pairs beyond rc skipped with the
 // canonical decision inside the recheck band; writes the same split records, per-atom q6 and f'(q6) as the fused pass of
 // k_tile_build and finishes the global sums in its last block.
 template <bool DEVBOX>
@@ -481,7 +493,8 @@ k_q6_pass1_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
              float *__restrict__ q6_out, int solid, double scale_mean, double scale_solid, double *__restrict__ partials,
              unsigned int *__restrict__ ticket, double *__restrict__ cv_q6, double *__restrict__ cv_out, int dim0, int dim1,
              unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg,
-             int *__restrict__ rc_count, int *__restrict__ rc_list /* the entries within rc, same sliced layout: read by the force pass */) {
+             int *__restrict__ rc_count, int *__restrict__ rc_list /* the entries within rc, same sliced layout: read by the force pass */,
+             float far2) {
     __shared__ double red[64];
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (DEVBOX) pb = dg->pbf;                      // host-box instance: the box stays in the constant bank
@@ -503,7 +516,7 @@ k_q6_pass1_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
             if (k + 2 < cnt) e1 = __ldg(in + (k + 2) * 32);
             const float4 pj = spos[j];
             float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-            min_image(pb, dx, dy, dz);
+            skin_displacement(DEVBOX ? dg->bd : bd, far2, pi, pj, dx, dy, dz);
             const float r2 = dx * dx + dy * dy + dz * dz;
             bool keep = r2 < rc2f;
             if (fabsf(r2 - rc2f) <= pb.band)
@@ -551,6 +564,12 @@ k_q6_pass1_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
     }
 }
 
+// threshold of skin_displacement: (rc + 2 skin)^2, a little inside
+static float skin_far2(const metad_ctx *c) {
+    const double r = c->rc + 2.0 * (c->rcl - c->rc);
+    return (float)(r * r * (1.0 - 1e-4));
+}
+
 int tiled_q6_pass1_skin(metad_ctx *c, double *d_cv) {
     const double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
     const double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
@@ -558,7 +577,7 @@ int tiled_q6_pass1_skin(metad_ctx *c, double *d_cv) {
     c->N, c->maxn, (const float4 *)c->d_spos, c->d_nl_count, c->d_nl, ctx_pbox<float>(c), c->boxd, (float)c->rc2, c->rc2,  \
         (float)qt, (float)(1.0 / qw), (float *)c->d_rec, c->d_q6, c->q6_solid_dim >= 0 ? 1 : 0,                            \
         c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0, c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0, \
-        c->d_partials + c->nblocks_atoms, c->d_tickets + 1, c->d_cvq6, d_cv, c->q6_mean_dim, c->q6_solid_dim, c->d_sticky, c->dg, c->d_rc_count, c->d_rc_list
+        c->d_partials + c->nblocks_atoms, c->d_tickets + 1, c->d_cvq6, d_cv, c->q6_mean_dim, c->q6_solid_dim, c->d_sticky, c->dg, c->d_rc_count, c->d_rc_list, skin_far2(c)
     if (c->dg) k_q6_pass1_g<true><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(P1G_ARGS);
     else k_q6_pass1_g<false><<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>(P1G_ARGS);
 #undef P1G_ARGS
@@ -692,7 +711,7 @@ int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
 #define Q6FG_ARGS                                                                                                          \
     c->N, c->maxn, (const float4 *)c->d_spos, c->skin_on ? c->d_rc_count : c->d_nl_count, c->skin_on ? c->d_rc_list : c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm, ss,  \
-        c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va, c->d_q6 + c->N, c->dg, ctx_pbox<float>(c)
+        c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va, c->d_q6 + c->N, c->dg, skin_far2(c)
 #define Q6FG_GRID <<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>
 #define Q6FG_LAUNCH(SOLID, VIR)                                                                                            \
     do {                                                                                                                   \

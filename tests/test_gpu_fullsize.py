@@ -145,3 +145,23 @@ def test_config3_full_size_is_bit_identical_from_run_to_run():
     assert np.abs(out[0][0]).max() > 0
     for a, b in zip(out[0], out[1]):
         assert np.array_equal(np.asarray(a), np.asarray(b))
+
+
+def test_config3_full_size_with_a_verlet_skin():
+    """params.skin at the size bench.py --skin times (1,024,000 atoms, fp32 pair math): every atom takes a seeded Gaussian step
+    of width 0.012 A per step and is re-wrapped into the 255 A box, so pairs across a face and freshly re-wrapped atoms occur
+    in the kept list; every step is compared with the oracle, which builds its list from scratch (gpu_util.chained_run: CV,
+    V, dV/ds, every force component, the deposited hill)."""
+    from paper_2510_06873_b200.inputs import wrap
+    from gpu_util import chained_run
+    w = configs.config3()
+    w.stride = 2
+    rng = np.random.default_rng(77)
+    frames, p = [], w.pos.copy()
+    for k in range(3):
+        if k:
+            p = wrap(p + rng.standard_normal(p.shape) * 0.012, w.box)
+        frames.append(p.copy())
+    r = chained_run(w, precision=32, nsteps=3, skin=0.3, pos_of_step=lambda k: frames[k], n_init_hills=30)
+    assert r["md"].rebuilds() == 1                # one build, then the list is kept
+    assert r["md"].status() == 0
