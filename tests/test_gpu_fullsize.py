@@ -165,3 +165,26 @@ def test_config3_full_size_with_a_verlet_skin():
     r = chained_run(w, precision=32, nsteps=3, skin=0.3, pos_of_step=lambda k: frames[k], n_init_hills=30)
     assert r["md"].rebuilds() == 1                # one build, then the list is kept
     assert r["md"].status() == 0
+
+
+@pytest.mark.parametrize("mode", ["host box", "device box, rescaled every step", "device box + skin"])
+def test_config3_full_size_run_paths(mode):
+    """The run paths at the size bench.py times (1,024,000 atoms, fp32 pair math, CUDA-graph replay with deposition), every step
+    against the oracle (gpu_util.chained_run): metad_run with a host box; metad_run_dev with the box in device memory, rescaled
+    with the positions every step as a barostat would (one capture, no graph update); and the same with a Verlet
+    skin on top."""
+    from gpu_util import chained_run
+    w = configs.config3()
+    w.stride = 2
+    if mode == "host box":
+        r = chained_run(w, precision=32, nsteps=2, n_init_hills=30)
+    else:
+        box0 = w.box.copy()
+        frac = np.linalg.solve(box0.reshape(3, 3).T, w.pos.T).T
+        scales = [1.0, 1.0006, 0.9996]
+        r = chained_run(w, precision=32, nsteps=3, n_init_hills=30, device_box=True, box_slack=0.01,
+                        skin=0.3 if "skin" in mode else 0.0,
+                        box_of_step=lambda k: box0 * scales[k], pos_of_step=lambda k: frac @ (box0 * scales[k]).reshape(3, 3))
+        gi = r["md"].graph_info()
+        assert gi["captures"] == 1 and gi["updates"] == 0
+    assert r["md"].status() == 0
