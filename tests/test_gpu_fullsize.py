@@ -188,3 +188,34 @@ def test_config3_full_size_run_paths(mode):
         gi = r["md"].graph_info()
         assert gi["captures"] == 1 and gi["updates"] == 0
     assert r["md"].status() == 0
+
+
+@pytest.mark.parametrize("case", ["c4 grid", "c4 skin", "g0 lazy", "c3 fp64", "c2 skin", "c1"])
+def test_other_workloads_full_size_run_paths(case):
+    """metad_run at BASELINE size for the other workloads and modes, every step against the oracle (gpu_util.chained_run):
+    c4 (4,096,000 atoms, Q6 mean + solid-like count) through the 512 x 512 grid and, separately, with a Verlet skin over
+    moving atoms; the paper's GaN CV set list-free (`lazy_neighbors`); c3 on the generic fp64 kernels; the grouped
+    coordination number of c2 with a skin; the chain CVs of c1."""
+    from paper_2510_06873_b200.inputs import wrap
+    from gpu_util import chained_run
+    name = case.split()[0]
+    w = {"c4": configs.config4, "g0": configs.config_g0, "c3": configs.config3, "c2": configs.config2, "c1": configs.config1}[name]()
+    w.stride = 2
+    kw = dict(nsteps=2, n_init_hills=30)
+    if "skin" in case:
+        rng = np.random.default_rng(3)
+        frames, p = [], w.pos.copy()
+        for k in range(3):
+            if k:
+                p = wrap(p + rng.standard_normal(p.shape) * 0.012, w.box)
+            frames.append(p.copy())
+        kw.update(nsteps=3, skin=0.3, pos_of_step=lambda k: frames[k])
+    if case == "c4 grid":
+        s0 = np.array([0.2315, 4.7e5])                       # the structure's own CV values (test_config4_grid_leg_full_size)
+        sig = np.asarray(w.sigma, dtype=np.float64)
+        kw.update(grid=((512, 512), s0 - 120 * sig, s0 + 120 * sig))
+    precision = {"c4": 32, "g0": 32, "c3": 64, "c2": 64, "c1": 64}[name]
+    r = chained_run(w, precision=precision, lazy=(case == "g0 lazy"), **kw)
+    assert r["md"].status() == 0
+    if "skin" in case:
+        assert r["md"].rebuilds() == 1
