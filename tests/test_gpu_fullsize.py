@@ -209,13 +209,13 @@ def test_other_workloads_full_size_run_paths(case):
             if k:
                 p = wrap(p + rng.standard_normal(p.shape) * 0.012, w.box)
             frames.append(p.copy())
-        kw.update(nsteps=3, skin=0.3, pos_of_step=lambda k: frames[k])
+        kw.update(nsteps=2 if name == "c4" else 3, skin=0.3, pos_of_step=lambda k: frames[k])
     if case == "c4 grid":
         s0 = np.array([0.2315, 4.7e5])                       # the structure's own CV values (test_config4_grid_leg_full_size)
         sig = np.asarray(w.sigma, dtype=np.float64)
         kw.update(grid=((512, 512), s0 - 120 * sig, s0 + 120 * sig))
     precision = {"c4": 32, "g0": 32, "c3": 64, "c2": 64, "c1": 64}[name]
-    r = chained_run(w, precision=precision, lazy=(case == "g0 lazy"), **kw)
+    r = chained_run(w, precision=precision, lazy=(case == "g0 lazy"), free_run=(name != "c4"), **kw)
     assert r["md"].status() == 0
     if "skin" in case:
         assert r["md"].rebuilds() == 1

@@ -79,11 +79,11 @@ def test_virial_needs_the_flag():
         md.virial()
 
 
-@pytest.mark.parametrize("name", ["c3", "g0"])
+@pytest.mark.parametrize("name", ["c3", "g0", "c4"])
 def test_virial_full_size_tiled_fp32(name):
-    """The bias virial at the sizes bench.py times (1,024,000 atoms, fp32 pair math on the tiled path): Q6 (traceless) and the
-    paper's GaN CV set (coordination number + a, b, c)."""
-    w = configs.config3() if name == "c3" else configs.config_g0()
+    """The bias virial at the sizes bench.py times (fp32 pair math on the tiled path): Q6 at 1,024,000 atoms (traceless), the
+    paper's GaN CV set (coordination number + a, b, c), and Q6 + solid-like count at 4,096,000 atoms."""
+    w = {"c3": configs.config3, "g0": configs.config_g0, "c4": configs.config4}[name]()
     r, W = _check(w, 32, 1e-5, from_force_bar=True)
     if name == "c3":
         assert abs(np.trace(W)) <= 1e-5 * np.abs(W).max()     # Q6 is scale-invariant: traceless (no coherent radial residue)
