@@ -218,7 +218,7 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
     CUDA_TRY(dev_alloc(&c->d_cell_of, N));
     CUDA_TRY(dev_alloc(&c->d_slot, N));
     CUDA_TRY(dev_alloc(&c->d_perm, N));
-    CUDA_TRY(dev_alloc(&c->d_perm_raw, N));
+    CUDA_TRY(dev_alloc(&c->d_perm_raw, 2 * (size_t)N));      // (atom, cell) pairs in raw counting-sort order
     CUDA_TRY(dev_alloc(&c->d_scell, N));
     CUDA_TRY(cudaMalloc(&c->d_spos, 4 * tsz * (size_t)N));
     CUDA_TRY(dev_alloc(&c->d_nl_count, N));

@@ -122,21 +122,24 @@ __global__ void k_scan_apply(int ncell, int N, int *__restrict__ cell_count, con
     if (blockIdx.x == 0 && threadIdx.x == 0) cell_start[ncell] = N;
 }
 
+// counting-sort scatter: slot a of the raw order receives (atom index, cell) in ONE 8-byte store, so that the ordering pass
+// reads its cell from contiguous memory instead of gathering cell_of[i]
 __global__ void k_scatter(int N, const int *__restrict__ cell_of, const int *__restrict__ slot,
-                          const int *__restrict__ cell_start, int *__restrict__ perm,
+                          const int *__restrict__ cell_start, int2 *__restrict__ perm,
                           const int *__restrict__ skin_flag, const int *__restrict__ step) {
     pdl_enter();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N || SKIN_SKIP(skin_flag, step)) return;
-    perm[cell_start[cell_of[i]] + slot[i]] = i;
+    const int c = cell_of[i];
+    perm[cell_start[c] + slot[i]] = make_int2(i, c);
 }
 
 // Thread per sorted slot: the atom in slot a finds its rank by original index among the atoms of its cell (a handful,
 // read from the unsorted permutation through L1) and moves itself to that place: in-cell order = original index, so the
 // float summation order downstream is run-to-run deterministic (reading P) no matter how the atomics of k_bin fell.
 template <typename T>
-__global__ void k_cell_sort_gather(int N, const int *__restrict__ cell_start, const int *__restrict__ cell_of,
-                                   const int *__restrict__ perm_in, int *__restrict__ perm,
+__global__ void k_cell_sort_gather(int N, const int *__restrict__ cell_start,
+                                   const int2 *__restrict__ perm_in /* (atom, cell) in raw order */, int *__restrict__ perm,
                                    const T *__restrict__ pos, const unsigned char *__restrict__ flags,
                                    typename Vec4<T>::type *__restrict__ spos, int *__restrict__ scell, int index_in_w,
                                    typename Vec4<T>::type *__restrict__ ref /* skin: positions at the build, else NULL */,
@@ -145,10 +148,11 @@ __global__ void k_cell_sort_gather(int N, const int *__restrict__ cell_start, co
     int a = blockIdx.x * blockDim.x + threadIdx.x;
     if (a >= N || SKIN_SKIP(skin_flag, step)) return;
     if (a == 0 && nbuilds) ++*nbuilds;            // list builds so far (metad_get_rebuilds)
-    const int i = perm_in[a], c = cell_of[i];
+    const int2 ic = perm_in[a];
+    const int i = ic.x, c = ic.y;
     const int b = cell_start[c], e = cell_start[c + 1];
     int rank = 0;
-    for (int q = b; q < e; ++q) rank += perm_in[q] < i;
+    for (int q = b; q < e; ++q) rank += perm_in[q].x < i;
     typename Vec4<T>::type v;
     v.x = pos[3 * i]; v.y = pos[3 * i + 1]; v.z = pos[3 * i + 2];
     v.w = (T)(flags ? (int)flags[i] : 3);
@@ -570,9 +574,9 @@ static int nb_build_kernels(metad_ctx *c, const void *d_pos) {
     klaunch_pdl(pdl, k_scan_sums, nsb, SCAN_THREADS, 0, st, ncell, (const int *)c->d_cell_count, c->d_block_sums, sf, stp);
     klaunch_pdl(pdl, k_scan_apply, nsb, SCAN_THREADS, 0, st, ncell, N, c->d_cell_count, (const int *)c->d_block_sums, c->d_cell_start, sf, stp);
     klaunch_pdl(pdl, k_scatter, div_up(N, 256), 256, 0, st, N, (const int *)c->d_cell_of, (const int *)c->d_slot, (const int *)c->d_cell_start,
-                c->d_perm_raw, sf, stp);
-    klaunch_pdl(pdl, k_cell_sort_gather<T>, div_up(N, 256), 256, 0, st, N, (const int *)c->d_cell_start, (const int *)c->d_cell_of,
-                (const int *)c->d_perm_raw, c->d_perm, (const T *)d_pos,
+                (int2 *)c->d_perm_raw, sf, stp);
+    klaunch_pdl(pdl, k_cell_sort_gather<T>, div_up(N, 256), 256, 0, st, N, (const int *)c->d_cell_start,
+                (const int2 *)c->d_perm_raw, c->d_perm, (const T *)d_pos,
                 (const unsigned char *)c->d_flags,   /* NULL unless a COORD / MINDIST CV has groups */
                 (V4 *)c->d_spos, c->d_scell, c->tiled ? 1 : 0, ref, sf, stp, c->d_nbuilds);
     if (tm) cudaEventRecord(c->ev[1], st);
