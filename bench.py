@@ -513,7 +513,7 @@ def run_ours(args):
             roof_all.append(r_build)
             if list_ms > stage_ms[3]:
                 roof = r_build                     # the dominant kernel of the step
-            # what actually binds both kernels is instruction issue (profiles/r2h_ncu.md), so the same launches are also put
+            # what actually binds both kernels is instruction issue (profiles/r2i_ncu.md), so the same launches are also put
             # against the issue peak 148 SMs x 4 schedulers x 1.965 GHz, with the executed warp instructions ncu counted
             for key, kms, nm in (("build_warp_instructions", list_ms, "k_tile_build<Q6>"), ("force_warp_instructions", stage_ms[3], "k_q6_force_g")):
                 if traffic.get(key):
