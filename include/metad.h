@@ -288,6 +288,28 @@ int metad_graph_info(metad_ctx *ctx, int *h_counts);
  * Needs no context.  [sync] */
 int metad_fma_peak(int kind, double *h_tflops, double *h_ms);
 
+/* The hill sum V(s), dV/ds (reading W for periodic dimensions) WITHOUT a context and WITHOUT any allocation: for
+ * callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid it).  The call
+ * makes no cudaMalloc / cudaFree and uses no allocating library routine; its scratch (one row of partial sums per 2,048 hills +
+ * the ticket of the fixed-order reduction) is a file-scope __device__ array of METAD_NOALLOC_SCRATCH_BYTES that every GPU
+ * loading this library holds until the process exits.
+ *   d_centers  device, [ncv][ld_centers] doubles: centre of hill k in dimension d at d_centers[d * ld_centers + k]
+ *   d_heights  device, [nhills] doubles;   nhills  0..METAD_NOALLOC_MAX_HILLS (more: METAD_ERR_ARG, the message names the limit)
+ *   h_sigma    host, [ncv] Gaussian widths (> 0);   h_period  host, [ncv] periods (0: not periodic) or NULL
+ *   d_cv       device, [ncv] the point s;   d_V  device, 1 double (out);   d_dVds  device, [ncv] doubles (out)
+ *   cuda_stream  the cudaStream_t to enqueue on (NULL: the default stream).  [async]: a memset of the ticket and one kernel;
+ *                all device arrays stay owned by the caller and must stay valid until the work has completed.
+ * Every call shares the one scratch array, which keeps the last call's contents (the call clears what must start at zero):
+ * calls that OVERLAP on the GPU — different streams with no ordering between them, or several host threads — race on it.
+ * The result equals metad_bias's up to the order of the fp64 sum (another fixed order: run-to-run identical).
+ * Errors: METAD_ERR_ARG (null pointer, ncv outside 1..METAD_MAX_CV, nhills beyond the limit, ld_centers < nhills,
+ * sigma <= 0), METAD_ERR_CUDA. */
+#define METAD_NOALLOC_MAX_HILLS 1048576
+#define METAD_NOALLOC_SCRATCH_BYTES 20736
+int metad_bias_noalloc(const double *d_centers, int ld_centers, const double *d_heights, int nhills, int ncv,
+                       const double *h_sigma, const double *h_period, const double *d_cv, double *d_V, double *d_dVds,
+                       void *cuda_stream);
+
 const char *metad_version(void);
 const char *metad_last_error(void);
 

@@ -42,7 +42,7 @@ class Params(ctypes.Structure):
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
            "metad_apply_forces", "metad_deposit", "metad_run", "metad_build_neighbors_dev", "metad_run_dev", "metad_reset_box", "metad_step_host", "metad_host_alloc", "metad_host_free", "metad_status",
            "metad_get_state", "metad_get_neighbors", "metad_get_q6", "metad_set_hills", "metad_get_hills",
-           "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reweight_recorded", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_synchronize", "metad_get_rebuilds", "metad_graph_info", "metad_fma_peak", "metad_version", "metad_last_error"]
+           "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reweight_recorded", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_synchronize", "metad_get_rebuilds", "metad_graph_info", "metad_fma_peak", "metad_bias_noalloc", "metad_version", "metad_last_error"]
 
 _lib = None
 
@@ -91,6 +91,7 @@ def load():
     L.metad_get_rebuilds.argtypes = [_P, _P]
     L.metad_graph_info.argtypes = [_P, _P]
     L.metad_fma_peak.argtypes = [_I, _P, _P]
+    L.metad_bias_noalloc.argtypes = [_P, _I, _P, _I, _I, _P, _P, _P, _P, _P, _P]
     L.metad_version.restype = ctypes.c_char_p
     L.metad_last_error.restype = ctypes.c_char_p
     _lib = L
@@ -102,6 +103,27 @@ def fma_peak(kind):
     t, ms = ctypes.c_double(0), ctypes.c_double(0)
     _check(load().metad_fma_peak({"f32": 0, "f32x2": 1, "f64": 2}[kind], ctypes.byref(t), ctypes.byref(ms)))
     return t.value, ms.value
+
+
+NOALLOC_MAX_HILLS = 1048576       # include/metad.h: METAD_NOALLOC_MAX_HILLS
+
+
+def bias_noalloc(centers, heights, cv, sigma, V, dVds, period=None, nhills=None, stream=None):
+    """metad_bias_noalloc: V(s), dV/ds of the caller's own hill arrays with no context and no allocation (argument
+    marshalling only).  centers: CUDA float64 tensor [ncv, ld]; heights: CUDA float64 [>= nhills]; cv: CUDA float64 [ncv];
+    V (1) and dVds (ncv): CUDA float64 outputs owned by the caller; stream: a torch.cuda.Stream or None (default stream)."""
+    ncv = int(cv.numel())
+    for t in (centers, heights, cv, V, dVds):
+        assert t.is_cuda and t.is_contiguous() and t.element_size() == 8
+    ld = int(centers.shape[1]) if centers.dim() == 2 else int(centers.numel())
+    n = int(heights.numel()) if nhills is None else int(nhills)
+    sg = np.ascontiguousarray(sigma, dtype=np.float64)
+    assert len(sg) == ncv
+    pr = None if period is None else np.ascontiguousarray(period, dtype=np.float64)
+    _check(load().metad_bias_noalloc(_ptr(centers), ld, _ptr(heights), n, ncv, sg.ctypes.data,
+                                     None if pr is None else pr.ctypes.data, _ptr(cv), _ptr(V), _ptr(dVds),
+                                     None if stream is None else ctypes.c_void_p(stream.cuda_stream)))
+    return V, dVds
 
 
 class MetadError(RuntimeError):
