@@ -132,6 +132,9 @@ typedef struct {
     double box_slack;               /* metad_*_dev calls: the cell grid is derived ONCE (first call / after metad_reset_box) with
                                        cells at least rc (1 + box_slack) wide, so the device-resident box may shrink by that
                                        fraction before METAD_DEV_BOX is raised; 0 = cells as small as rc allows */
+    double fill_fraction;           /* fraction of the box volume the atoms occupy, in (0, 1]; 0 (default) = 1.  A rank of a slab
+                                       decomposition holds its slab + halo in the GLOBAL box: the shared-memory
+                                       tiles are sized for natoms / (fill_fraction * cells) atoms per cell instead of the box average */
 } metad_params;
 
 /* Creates a context on the current CUDA device; `cuda_stream` is the cudaStream_t on which every later call is enqueued.
@@ -309,6 +312,13 @@ int metad_fma_peak(int kind, double *h_tflops, double *h_ms);
 int metad_bias_noalloc(const double *d_centers, int ld_centers, const double *d_heights, int nhills, int ncv,
                        const double *h_sigma, const double *h_period, const double *d_cv, double *d_V, double *d_dVds,
                        void *cuda_stream);
+
+/* Slab decomposition over several GPUs: after metad_eval_cv, replaces the Q6 CVs in
+ * d_cv (device, [ncv]) by their sums over the atoms this rank OWNS — d_owned: device, natoms bytes, != 0 for an owned atom,
+ * indexed like d_pos.  The ranks then add their d_cv (one all-reduce of ncv doubles) and go on with metad_bias /
+ * metad_apply_forces / metad_deposit on the same global s.  Fixed-order sum (run-to-run identical).  [async]
+ * Errors: METAD_ERR_STATE unless every CV dimension of the context is a Q6 CV and the CVs have been evaluated. */
+int metad_cv_owned_sum(metad_ctx *ctx, const unsigned char *d_owned, double *d_cv);
 
 const char *metad_version(void);
 const char *metad_last_error(void);

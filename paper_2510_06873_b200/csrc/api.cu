@@ -273,6 +273,7 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
     CUDA_TRY(dev_alloc(&c->d_nbuilds, 1));
     CUDA_TRY(cudaMemset(c->d_nbuilds, 0, sizeof(int)));
     if (!(p->box_slack >= 0.0) || p->box_slack > 1.0) FAIL(METAD_ERR_ARG, "box_slack must be in [0, 1]");
+    if (!(p->fill_fraction >= 0.0) || p->fill_fraction > 1.0) FAIL(METAD_ERR_ARG, "fill_fraction must be in [0, 1] (0 = 1)");
     if (!(p->skin >= 0.0)) FAIL(METAD_ERR_ARG, "skin must be >= 0");
     c->skin_on = p->skin > 0.0 && (c->has_q6 || c->has_coord || c->has_mindist);
     if (c->skin_on) {
@@ -368,7 +369,8 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc, double sla
         while (xsub > 1 && (long long)g.ncell * xsub > c->cell_cap) --xsub;
         CellGrid gs = g;
         gs.nc[0] *= xsub; gs.ncell *= xsub;
-        const double rho = (double)c->N / gs.ncell, margin = 1.3;
+        // atoms per cell where there are atoms (a slab-decomposition rank fills only part of the global box)
+        const double rho = (double)c->N / (gs.ncell * (c->p.fill_fraction > 0.0 ? c->p.fill_fraction : 1.0)), margin = 1.3;
         int cap = 1216;
         double best = 1e30; int bt[3] = { 0, 0, 0 };
         // two passes: the smallest halo ratio, then among the shapes within 2 % of it the longest along x (rows are the

@@ -36,13 +36,13 @@ class Params(ctypes.Structure):
     _fields_ = [("natoms", _I), ("precision", _I), ("max_neigh", _I), ("ncv", _I),
                 ("cv", CvDesc * MAX_CV), ("sigma", _D * MAX_CV), ("w0", _D), ("kT", _D),
                 ("bias_factor", _D), ("max_hills", _I), ("stride", _I), ("grid_n", _I * 2),
-                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("traj_capacity", _I), ("lazy_neighbors", _I), ("want_virial", _I), ("skin", _D), ("box_slack", _D)]
+                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("traj_capacity", _I), ("lazy_neighbors", _I), ("want_virial", _I), ("skin", _D), ("box_slack", _D), ("fill_fraction", _D)]
 
 
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
            "metad_apply_forces", "metad_deposit", "metad_run", "metad_build_neighbors_dev", "metad_run_dev", "metad_reset_box", "metad_step_host", "metad_host_alloc", "metad_host_free", "metad_status",
            "metad_get_state", "metad_get_neighbors", "metad_get_q6", "metad_set_hills", "metad_get_hills",
-           "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reweight_recorded", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_synchronize", "metad_get_rebuilds", "metad_graph_info", "metad_fma_peak", "metad_bias_noalloc", "metad_version", "metad_last_error"]
+           "metad_get_grid", "metad_get_box_force", "metad_get_virial", "metad_bias_batch", "metad_reweight", "metad_reweight_recorded", "metad_reset_steps", "metad_set_timing", "metad_get_timing", "metad_launch_count", "metad_synchronize", "metad_get_rebuilds", "metad_graph_info", "metad_fma_peak", "metad_bias_noalloc", "metad_cv_owned_sum", "metad_version", "metad_last_error"]
 
 _lib = None
 
@@ -91,6 +91,7 @@ def load():
     L.metad_get_rebuilds.argtypes = [_P, _P]
     L.metad_graph_info.argtypes = [_P, _P]
     L.metad_fma_peak.argtypes = [_I, _P, _P]
+    L.metad_cv_owned_sum.argtypes = [_P, _P, _P]
     L.metad_bias_noalloc.argtypes = [_P, _I, _P, _I, _I, _P, _P, _P, _P, _P, _P]
     L.metad_version.restype = ctypes.c_char_p
     L.metad_last_error.restype = ctypes.c_char_p
@@ -171,7 +172,7 @@ class MetaD:
     precision == 32)."""
 
     def __init__(self, workload, max_hills=None, precision=None, grid=None, force_scale=1.0, stream=None, want_virial=False, lazy_neighbors=False, traj_capacity=0,
-                 box_slack=0.0, skin=0.0):
+                 box_slack=0.0, skin=0.0, fill_fraction=0.0):
         import torch
         self.torch = torch
         L = load()
@@ -225,6 +226,7 @@ class MetaD:
         p.lazy_neighbors = 1 if lazy_neighbors else 0
         p.traj_capacity = int(traj_capacity)
         p.box_slack = float(box_slack)
+        p.fill_fraction = float(fill_fraction)
         p.skin = float(skin)
         self._params = p
         h = _P()
@@ -263,6 +265,13 @@ class MetaD:
         dVds = self.dVds if dVds is None else dVds
         _check(load().metad_bias(self._h, _ptr(cv), _ptr(V), _ptr(dVds)))
         return V, dVds
+
+    def cv_owned_sum(self, owned, cv=None):
+        """metad_cv_owned_sum: the Q6 CVs summed over the atoms flagged in `owned` (CUDA uint8 tensor, natoms)."""
+        assert owned.is_cuda and owned.is_contiguous() and owned.element_size() == 1 and owned.numel() == self.N
+        cv = self.cv if cv is None else cv
+        _check(load().metad_cv_owned_sum(self._h, _ptr(owned), _ptr(cv)))
+        return cv
 
     def apply_forces(self, F, dVds=None):
         assert F.dtype == self.dtype and F.is_cuda and F.is_contiguous()
