@@ -49,6 +49,12 @@ def parse():
     ap.add_argument("--move", type=float, default=0.0,
                     help="move every atom by a seeded Gaussian displacement of this width (A) before every timed step (device "
                          "kernels of the harness, outside the timed events): what an MD integrator does between two calls")
+    ap.add_argument("--decompose", action="store_true",
+                    help="slab decomposition of ONE c3 / c4 system over the ranks (strong scaling; DESIGN.md section 8): halo of "
+                         "2 (rc + skin), one all-reduce of ncv doubles per step.  Default without it: N independent replicas")
+    ap.add_argument("--as-rank", type=int, default=-1,
+                    help="with --decompose on ONE GPU: time the share of this rank of a world of --of ranks alone (no all-reduce)")
+    ap.add_argument("--of", type=int, default=1)
     ap.add_argument("--peaks", action="store_true",
                     help="only measure the scalar-pipe roofline denominators (FP32 / FP32x2 / FP64 FMA microbenchmark, "
                          "metad_fma_peak) and print them as one JSON line")
@@ -624,6 +630,141 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_decomposed(args):
+    """--decompose: ONE system cut into slabs along c, one rank per GPU (paper_2510_06873_b200/domain.py).  Stage calls +
+    metad_cv_owned_sum + an all-reduce of ncv doubles per step; value = atoms of the WHOLE system x steps / slowest rank."""
+    import torch
+    import torch.distributed as dist
+    from paper_2510_06873_b200 import domain
+    from paper_2510_06873_b200.inputs import hill_walk, seeded_heights
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.config not in ("c3", "c4"):
+        raise SystemExit("--decompose: the Q6 workloads c3 and c4 (DESIGN.md section 8)")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl ours needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    solo = args.as_rank >= 0                       # one rank's share, alone on this GPU
+    dworld, drank = (args.of, args.as_rank) if solo else (world, rank)
+    w = workload(args.config)                      # every rank builds the same seeded system
+    precision = args.precision or 32
+    tdt = torch.float32 if precision == 32 else torch.float64
+    centers, heights = hill_walk(5, np.full(w.ncv, 0.23), w.sigma, w.n_hills), seeded_heights(5, w.n_hills, w.w0)
+    rk = domain.SlabMetaD(w, dworld, drank, precision=precision, skin=args.skin, max_hills=w.n_hills + args.steps + args.warmup + 64)
+    md = rk.md
+    md.set_hills(centers, heights)
+    nloc = len(rk.local)
+    pos_h = torch.tensor(w.pos[rk.local].astype(np.float32 if precision == 32 else np.float64)).pin_memory()
+    F_h = torch.zeros((nloc, 3), dtype=tdt).pin_memory()
+    with torch.cuda.stream(md.stream):
+        dpos = pos_h.to("cuda", non_blocking=True)
+        F = torch.zeros((nloc, 3), device="cuda", dtype=tdt)
+    md.synchronize()
+
+    def step():
+        rk.phase1(dpos)
+        if not solo:
+            rk.all_reduce()
+        rk.phase2(F)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = md.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(md.stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(md.stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = md.launch_count() - l0
+    # stage times of this rank
+    names = ["build_neighbors", "eval_cv", "cv_owned_sum", "all_reduce", "bias", "apply_forces", "deposit"]
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(8)]
+    acc = np.zeros(7)
+    for it in range(7):
+        evs[0].record(md.stream)
+        md.build_neighbors(dpos); evs[1].record(md.stream)
+        md.eval_cv(); evs[2].record(md.stream)
+        md.cv_owned_sum(rk.d_owned); evs[3].record(md.stream)
+        if not solo:
+            rk.all_reduce()
+        evs[4].record(md.stream)
+        md.bias(); evs[5].record(md.stream)
+        md.apply_forces(F); evs[6].record(md.stream)
+        md.deposit(); evs[7].record(md.stream)
+        barrier()
+        if it >= 2:
+            acc += np.array([evs[k].elapsed_time(evs[k + 1]) for k in range(7)])
+    stage_ms = acc / 5
+    clocks = sampler.stop() if rank == 0 else None
+    # end to end: this rank's positions and forces from / to page-locked host memory inside the timed region
+    ke = max(3, min(args.steps, 20))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(ke):
+        with torch.cuda.stream(md.stream):
+            dpos.copy_(pos_h, non_blocking=True)
+            F.copy_(F_h, non_blocking=True)
+        step()
+        with torch.cuda.stream(md.stream):
+            F_h.copy_(F, non_blocking=True)
+            cv_h = md.cv.cpu()
+        md.synchronize()
+    e2e_s = time.perf_counter() - t0
+    ms_max, e2e_ms_max = max_over_ranks([ms, e2e_s * 1e3])
+    status = md.status()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    natoms_job = w.natoms                           # strong scaling: the whole system, whatever the number of ranks
+    value = natoms_job * args.steps / (ms_max * 1e-3)
+    tb = 4 if precision == 32 else 8
+    peaks = {}
+    pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(pk):
+        peaks = json.load(open(pk))
+    hbm_peak, peak_src = (peaks["hbm_gbs"], "measured (MEASURED_PEAKS.json hbm_gbs)") if "hbm_gbs" in peaks else (6650.0, "fallback (B200_PROFILING.md)")
+    cnt, _ = md.neighbors()
+    nb = float(cnt[rk.owned_local].mean())
+    by = algo_q6_force_bytes(nb, tb) * nloc
+    ach = by / (stage_ms[5] * 1e-3) / 1e9
+    roof = {"kernel": "k_q6_force_g (stage apply_forces of this rank: held atoms = owned + halo)", "bound": "hbm", "achieved": ach,
+            "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "traffic": None, "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": by, "kernel_ms": float(stage_ms[5]), "mean_neighbours": nb}
+    cfg_ = describe(w, precision)
+    cfg_["parallelism"] = (f"slab decomposition along c over {dworld} rank(s): rank {drank} owns {int(rk.owned_local.sum())} atoms and holds "
+                           f"{nloc} (halo 2 (rc + skin) = {rk.reach:.2f} A on either side, global coordinates, global box); one all-reduce "
+                           f"of {w.ncv} double(s) per step" + ("; THIS LINE: that rank's share alone on one GPU, no all-reduce (--as-rank)" if solo else ""))
+    cfg_["hills"] = f"{w.n_hills} seeded hills (no well-tempered replay in this mode)"
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f32" if precision == 32 else "f64", "data": "synthetic", "config": cfg_, "clocks": clocks,
+            "gpu_launches": int(launches),
+            "e2e": {"value": natoms_job * ke / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(pos_h.nbytes + F_h.nbytes),
+                    "d2h_bytes_per_step": int(F_h.nbytes + 8 * w.ncv), "ms_per_step": e2e_ms_max / ke},
+            "roofline": roof, "stages_ms": {n: float(v) for n, v in zip(names, stage_ms)},
+            "decomposition": {"world": dworld, "rank": drank, "owned": int(rk.owned_local.sum()), "held": int(nloc),
+                              "fill_fraction": domain.fill_fraction(w.box, rk.reach, dworld), "solo": bool(solo)},
+            "state": {"cv": [float(x) for x in cv_h], "sticky": status}}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_peaks(args):
     import torch
     if not torch.cuda.is_available():
@@ -643,6 +784,8 @@ def main():
         return
     if args.impl == "reference":
         run_reference(args)
+    elif args.decompose:
+        run_decomposed(args)
     else:
         run_ours(args)
 

@@ -135,6 +135,9 @@ typedef struct {
     double fill_fraction;           /* fraction of the box volume the atoms occupy, in (0, 1]; 0 (default) = 1.  A rank of a slab
                                        decomposition holds its slab + halo in the GLOBAL box: the shared-memory
                                        tiles are sized for natoms / (fill_fraction * cells) atoms per cell instead of the box average */
+    double c_window_lo;             /* read when fill_fraction < 1: every atom has its fractional c-coordinate in the window
+                                       [c_window_lo, c_window_lo + fill_fraction) modulo 1 (the slab + halo of the rank); only the
+                                       tiles of that window are launched.  An atom outside it raises METAD_DEV_POS_RANGE */
 } metad_params;
 
 /* Creates a context on the current CUDA device; `cuda_stream` is the cudaStream_t on which every later call is enqueued.

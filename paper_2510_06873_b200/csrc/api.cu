@@ -207,8 +207,13 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
         CUDA_TRY(dev_alloc(&c->d_tors_grad, 12 * METAD_MAX_CV));
     }
     // ---- buffers (everything the hot path needs; nothing is allocated later)
-    c->cell_cap = std::max(4 * N, 4096);
-    c->nblocks_atoms = div_up(N, 128) + 1;
+    // fill_fraction < 1 (a rank of a slab decomposition: N atoms in that fraction of the GLOBAL box): cells and tiles cover the
+    // whole box, so their tables are sized for the N / fill_fraction atoms a full box of this density would hold
+    const double fill = p->fill_fraction > 0.0 ? p->fill_fraction : 1.0;
+    const long long n_full = (long long)ceil((double)N / fill);
+    if (n_full > (1ll << 29)) FAIL(METAD_ERR_ARG, "natoms / fill_fraction too large");
+    c->cell_cap = (int)std::max(4 * n_full, 4096ll);
+    c->nblocks_atoms = div_up((int)n_full, 128) + 1;
     int max_pair_blocks = 1;
     for (int d = 0; d < c->D; ++d) max_pair_blocks = std::max(max_pair_blocks, div_up(c->cv[d].npairs, 256) + 1);
     CUDA_TRY(dev_alloc(&c->d_cell_count, (size_t)c->cell_cap + 1));
@@ -274,6 +279,7 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
     CUDA_TRY(cudaMemset(c->d_nbuilds, 0, sizeof(int)));
     if (!(p->box_slack >= 0.0) || p->box_slack > 1.0) FAIL(METAD_ERR_ARG, "box_slack must be in [0, 1]");
     if (!(p->fill_fraction >= 0.0) || p->fill_fraction > 1.0) FAIL(METAD_ERR_ARG, "fill_fraction must be in [0, 1] (0 = 1)");
+    if (!(p->c_window_lo >= 0.0) || !(p->c_window_lo < 1.0)) FAIL(METAD_ERR_ARG, "c_window_lo must be in [0, 1)");
     if (!(p->skin >= 0.0)) FAIL(METAD_ERR_ARG, "skin must be >= 0");
     c->skin_on = p->skin > 0.0 && (c->has_q6 || c->has_coord || c->has_mindist);
     if (c->skin_on) {
@@ -347,6 +353,7 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc, double sla
     g.inv[0] = 1.0 / ax; g.inv[1] = 1.0 / by; g.inv[2] = 1.0 / cz;
     g.inv[3] = g.inv[4] = g.inv[5] = 0.0;
     g.cx = cx; g.cy = cy; g.bx = bx;
+    g.wlo = c->p.c_window_lo; g.wlen = (c->p.fill_fraction > 0.0 && c->p.fill_fraction < 1.0) ? c->p.fill_fraction : 2.0;
     BoxD b = { ax, bx, by, cx, cy, cz, 0.5 * ax, 0.5 * by, 0.5 * cz };
     // a changed cell grid or cutoff invalidates a kept list: the next step rebuilds (set outside any capture: run_impl calls
     // this function before it starts one)
@@ -413,6 +420,22 @@ TileGeom tile_geom(const metad_ctx *c) {
     t.nc0 = c->grid.nc[0]; t.nc1 = c->grid.nc[1]; t.nc2 = c->grid.nc[2];
     t.ntx = (t.nc0 + t.Tx - 1) / t.Tx; t.nty = (t.nc1 + t.Ty - 1) / t.Ty; t.ntz = (t.nc2 + t.Tz - 1) / t.Tz;
     t.cap = c->tile_cap; t.hx = c->tile_hx; t.natoms = c->N;
+    t.sparse = (c->p.fill_fraction > 0.0 && c->p.fill_fraction < 1.0) ? 1 : 0;
+    t.tz0 = 0; t.ntz_launch = t.ntz;
+    if (t.sparse) {
+        // the z-tiles that overlap the window of occupied cells [c0, c1] along c (periodic); tile k covers cells
+        // [k nc / nt, (k + 1) nc / nt), so the tile of cell j is the largest k with k nc / nt <= j
+        const int c0 = std::min((int)floor(c->p.c_window_lo * t.nc2), t.nc2 - 1);
+        const int ncw = std::min((int)ceil((c->p.c_window_lo + c->p.fill_fraction) * t.nc2) - c0, t.nc2);   // cells in the window
+        auto tile_of = [&](int j) { int k = (int)(((long long)(j + 1) * t.ntz - 1) / t.nc2); while ((long long)k * t.nc2 / t.ntz > j) --k;
+                                    while ((long long)(k + 1) * t.nc2 / t.ntz <= j) ++k; return k; };
+        if (ncw < t.nc2) {
+            const int k0 = tile_of(c0), k1 = tile_of((c0 + ncw - 1) % t.nc2);
+            const int n = ((k1 - k0) % t.ntz + t.ntz) % t.ntz + 1;
+            // a window that wraps onto its own first tile would launch that tile twice: then launch everything
+            if (!(c0 + ncw - 1 >= t.nc2 && k1 == k0)) { t.tz0 = k0; t.ntz_launch = n; }
+        }
+    }
     t.cshift = 0;
     while ((1 << t.cshift) < t.Tx + 2 * t.hx + 2) ++t.cshift;      // Txe <= Tx + 1 columns + the end-of-row entry
     t.cuts = c->d_tile_cuts;

@@ -34,6 +34,7 @@ struct CellGrid {
     int ncell;
     double inv[6];                   // fractional transform: s_c = z*i0; s_b = (y - s_c*cy)*i1; ...
     double cx, cy, bx;               // tilt terms for cartesian -> fractional
+    double wlo, wlen;                // window of fractional c-coordinates that holds every atom (params.fill_fraction < 1); wlen >= 1: none
 };
 
 // Device-resident geometry of the current step (metad_build_neighbors_dev / metad_run_dev: the box lives in device memory and

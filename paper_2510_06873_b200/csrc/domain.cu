@@ -8,23 +8,26 @@
 // the ranks add these partial sums (ONE all-reduce of ncv doubles per step, NCCL), and every rank goes on with the same
 // s: metad_bias, metad_apply_forces (the forces of the owned atoms are complete: they need the records of their neighbours,
 // which need THEIR neighbours — hence the 2 (rc + skin) halo), metad_deposit (identical hills on every rank).
+#include <algorithm>
 #include "common.cuh"
 
-#define OWN_THREADS 128
+#define OWN_THREADS 256
+#define OWN_MAX_BLOCKS 592                                  // 4 x 148 SMs: a few atoms per thread, ONE block reduction per block
 
-// q6 of sorted atom s: tiled fp32 contexts keep a dense per-atom array, the generic kernels the record entry [14]
+// q6 of sorted atom s: tiled fp32 contexts keep a dense per-atom array, the generic kernels the record entry [14].
+// Fixed assignment of atoms to threads and blocks, fixed-order reductions: run-to-run identical.
 template <typename T>
 __global__ void __launch_bounds__(OWN_THREADS)
 k_cv_owned_sum(int N, const int *__restrict__ perm, const unsigned char *__restrict__ owned, const T *__restrict__ q6,
                int q6_stride, T q_thresh, T inv_width, double scale_mean, double scale_solid, int dim_mean, int dim_solid,
                double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out) {
     __shared__ double red[64];
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
     double v[2] = { 0.0, 0.0 };
-    if (s < N && owned[perm[s]]) {
+    for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < N; s += gridDim.x * blockDim.x) {
+        if (!owned[perm[s]]) continue;
         const T q = q6[(size_t)s * q6_stride];
-        v[0] = (double)q;
-        v[1] = (double)(T(1) / (T(1) + exp(-(q - q_thresh) * inv_width)));     // the expression of the pass-1 kernels
+        v[0] += (double)q;
+        if (dim_solid >= 0) v[1] += (double)(T(1) / (T(1) + exp(-(q - q_thresh) * inv_width)));     // the expression of the pass-1 kernels
     }
     block_reduce<2>(v, red);
     if (threadIdx.x == 0) { partials[2 * blockIdx.x] = v[0]; partials[2 * blockIdx.x + 1] = v[1]; }
@@ -47,7 +50,7 @@ extern "C" int metad_cv_owned_sum(metad_ctx *c, const unsigned char *d_owned, do
         if (d != c->q6_mean_dim && d != c->q6_solid_dim) {
             metad_set_error("metad_cv_owned_sum: every CV dimension of the context must be a Q6 CV"); return METAD_ERR_STATE;
         }
-    const int N = c->N, nb = div_up(N, OWN_THREADS);           // nb <= nblocks_atoms: the Q6 region of the per-block scratch
+    const int N = c->N, nb = std::min(std::min(div_up(N, OWN_THREADS), OWN_MAX_BLOCKS), c->nblocks_atoms);   // the Q6 region of the per-block scratch
     const double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
     const double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
     const double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;

@@ -31,6 +31,11 @@ __global__ void k_bin(int N, const T *__restrict__ pos, CellGrid g, int *__restr
     // next to that cell's atoms, which is what the lattice-shift logic of the tiled path relies on.
     if (!(fabs(sa - 0.5) <= 0.5001) || !(fabs(sb - 0.5) <= 0.5001) || !(fabs(sc - 0.5) <= 0.5001))   // also catches NaN
         atomicOr(sticky, (unsigned)METAD_DEV_POS_RANGE);
+    if (g.wlen < 1.0) {              // slab-decomposition rank: only the tiles of its window are launched (params.c_window_lo)
+        double u = sc - g.wlo;
+        u -= floor(u);
+        if (!(u < g.wlen)) atomicOr(sticky, (unsigned)METAD_DEV_POS_RANGE);
+    }
     int ia = min(max((int)floor(sa * g.nc[0]), 0), g.nc[0] - 1);
     int ib = min(max((int)floor(sb * g.nc[1]), 0), g.nc[1] - 1);
     int ic = min(max((int)floor(sc * g.nc[2]), 0), g.nc[2] - 1);

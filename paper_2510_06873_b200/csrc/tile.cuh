@@ -30,6 +30,8 @@ struct TileGeom {
     int cshift;                  // log2 of the power of two >= Tx + 2 hx + 1: a halo cell is (row, column) = (i >> cshift, i & mask)
     const int *cuts;             // device: tile boundaries along x [ntx + 1], y [nty + 1], z [ntz + 1] (api.cu: no division in the kernel)
     int natoms;                  // N (the second halves of the q6 records start at rec + 8 N)
+    int sparse;                  // params.fill_fraction < 1: most tiles of the box hold no atom (tile_is_empty)
+    int tz0, ntz_launch;         // z-tiles launched: tz0, tz0 + 1, ... (mod ntz), ntz_launch of them (all unless sparse)
     double ax, bx, by, cx, cy, cz;   // lattice rows
     double wa, wb, wc;           // cell edge vectors are a/nc0, b/nc1, c/nc2 (used for the tile's coordinate range)
 };
@@ -42,6 +44,23 @@ __device__ __forceinline__ TileBox tile_box(const TileGeom &g, const DevGeom *dg
     if (dg) { b.ax = dg->bd.ax; b.bx = dg->bd.bx; b.by = dg->bd.by; b.cx = dg->bd.cx; b.cy = dg->bd.cy; b.cz = dg->bd.cz; }
     else { b.ax = g.ax; b.bx = g.bx; b.by = g.by; b.cx = g.cx; b.cy = g.cy; b.cz = g.cz; }
     return b;
+}
+
+// A rank of a slab decomposition holds atoms in part of the GLOBAL box only (params.fill_fraction < 1):
+// a tile none of whose own rows holds an atom skips set-up, staging and scan.  All threads of the block must call it.
+__device__ __forceinline__ bool tile_is_empty(const TileGeom &g, const int *__restrict__ cell_start) {
+    const int *cy = g.cuts + g.ntx + 1, *cz = cy + g.nty + 1;
+    const int x0 = g.cuts[blockIdx.x], x1 = g.cuts[blockIdx.x + 1];
+    int tz = blockIdx.z + g.tz0;
+    if (tz >= g.ntz) tz -= g.ntz;
+    const int y0 = cy[blockIdx.y], ny = cy[blockIdx.y + 1] - y0, z0 = cz[tz], nz = cz[tz + 1] - z0;
+    int n = 0;
+    if ((int)threadIdx.x < ny * nz) {                         // an own row = cells [x0, x1) of one (y, z): contiguous in the sort
+        const int oz = (int)threadIdx.x / ny, oy = (int)threadIdx.x - oz * ny;
+        const int base = ((z0 + oz) * g.nc1 + (y0 + oy)) * g.nc0;
+        n = cell_start[base + x1] - cell_start[base + x0];
+    }
+    return __syncthreads_or(n) == 0;
 }
 
 struct TileTables {
@@ -86,7 +105,9 @@ __device__ __forceinline__ void tile_setup(const TileGeom &g, const int *__restr
                                            const DevGeom *dg) {
     const int tid = threadIdx.x;
     // the launch grid is (ntx, nty, ntz) and the tile boundaries come from a table: no integer division on the way in
-    const int tx = blockIdx.x, ty = blockIdx.y, tz = blockIdx.z;
+    const int tx = blockIdx.x, ty = blockIdx.y;
+    int tz = blockIdx.z + g.tz0;                  // tz0 != 0 only on a slab-decomposition rank (its window of z-tiles)
+    if (tz >= g.ntz) tz -= g.ntz;
     const int *cy = g.cuts + g.ntx + 1, *cz = cy + g.nty + 1;
     const int x0 = g.cuts[tx], y0 = cy[ty], z0 = cz[tz];
     const int Txe = g.cuts[tx + 1] - x0, Tye = cy[ty + 1] - y0, Tze = cz[tz + 1] - z0;

@@ -242,15 +242,18 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
     __shared__ double red[64];
     float4 *pos_s = dyn_smem;
     nl16_t *list_s = reinterpret_cast<nl16_t *>(dyn_smem + g.cap);
+    __shared__ unsigned long long stage_bar;
+    double v[2] = { 0.0, 0.0 };
+    if (g.sparse && tile_is_empty(g, cell_start)) {
+        // nothing to build here (block-uniform): the block only takes part in the reduction below
+    } else {
     // a device-resident box (NPT, dg != NULL) replaces the lattice rows of the arguments at their few points of use (tile
     // origin, periodic images, fp64 recheck): the common case costs no registers
     tile_setup(g, cell_start, t, *reinterpret_cast<TileScratch *>(dyn_smem), dg);   // scratch = the (still unused) staging area
-    __shared__ unsigned long long stage_bar;
     if (t.staged && !t.any_wrapped && t.total > 0) tile_stage_pos_tma(t, spos, pos_s, &stage_bar);   // block-uniform choice
     else
     tile_stage_pos(g, t, spos, pos_s, dg);
     __syncthreads();
-    double v[2] = { 0.0, 0.0 };
     if (t.total > 65535) {
         if (threadIdx.x == 0) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
     } else if (t.staged) {
@@ -259,6 +262,7 @@ k_tile_build(TileGeom g, const float4 *__restrict__ spos, const int *__restrict_
     } else {
         build_body<false, MODE>(g, t, spos, pos_s, list_s, scell, bd, rc2f, rc2, maxn, nl_count, nl, sticky, q_thresh,
                                    inv_width, rec, q6_out, solid != 0, sw_n, sw_m, perm, v, dg);
+    }
     }
     if (MODE != 0) {
         block_reduce<2>(v, red);
@@ -310,7 +314,7 @@ int tiled_init() {
 
 int tiled_build(metad_ctx *c) {
     TileGeom g = tile_geom(c);
-    const dim3 grid3(g.ntx, g.nty, g.ntz);         // tile (tx, ty, tz) = blockIdx: no division in the kernel
+    const dim3 grid3(g.ntx, g.nty, g.ntz_launch);  // tile (tx, ty, tz) = blockIdx (+ the window offset tz0): no division in the kernel
     double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
     double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
 #define TILE_LAUNCH(MODE, ...)                                                                                        \

@@ -4,7 +4,8 @@ One process per GPU.  Rank r OWNS the atoms whose fractional c-coordinate lies i
 every atom within `reach` = 2 (rc + skin) of that slab (a and b span the x-y plane of the lower-triangular box, so the distance
 to a slab face is |dz|).  The held atoms keep their GLOBAL coordinates and the GLOBAL box: every pair a rank sees is computed
 with the very arithmetic of the undivided system, so the neighbour sets, per-atom q6 and forces of the owned atoms are those of
-the whole system — the rest of the box is simply empty for that rank (`params.fill_fraction` sizes the tiles for it).
+the whole system — the rest of the box is simply empty for that rank (`params.fill_fraction` sizes the tiles for it, `params.c_window_lo` says
+where the occupied window starts, so that only its tiles are launched).
 
 Per step and rank (all kernels; argument marshalling only here):
     metad_build_neighbors -> metad_eval_cv -> metad_cv_owned_sum          (Q6 CVs summed over the OWNED atoms)
@@ -55,9 +56,15 @@ def slab_partition(pos, box, reach, world, rank):
 
 
 def fill_fraction(box, reach, world):
-    """Fraction of the box volume a rank's atoms occupy: (slab + 2 reach) / c_z, at most 1."""
+    """Fraction of the box volume a rank's atoms occupy: (slab + 2 reach) / c_z (a hair more), at most 1."""
     cz = float(np.asarray(box, dtype=np.float64).reshape(3, 3)[2, 2])
-    return float(min(1.0, (cz / world + 2.0 * reach) / cz))
+    return float(min(1.0, (cz / world + 2.0 * reach) / cz + 2e-9))
+
+
+def c_window_lo(box, reach, world, rank):
+    """Fractional c-coordinate at which the rank's window (slab + halo) starts, in [0, 1)."""
+    cz = float(np.asarray(box, dtype=np.float64).reshape(3, 3)[2, 2])
+    return float((rank / world - reach / cz - 1e-9) % 1.0)
 
 
 def sub_workload(w, local):
@@ -86,7 +93,8 @@ class SlabMetaD:
         self.owned_global = self.local[owned]
         self.sub = sub_workload(w, self.local)
         self.md = MetaD(self.sub, precision=precision, skin=skin, max_hills=max_hills,
-                        fill_fraction=fill_fraction(w.box, self.reach, world), **kw)
+                        fill_fraction=fill_fraction(w.box, self.reach, world),
+                        c_window_lo=c_window_lo(w.box, self.reach, world, rank), **kw)
         self.torch = torch
         with torch.cuda.stream(self.md.stream):
             self.d_owned = torch.tensor(owned.astype(np.uint8), device="cuda")

@@ -36,7 +36,7 @@ class Params(ctypes.Structure):
     _fields_ = [("natoms", _I), ("precision", _I), ("max_neigh", _I), ("ncv", _I),
                 ("cv", CvDesc * MAX_CV), ("sigma", _D * MAX_CV), ("w0", _D), ("kT", _D),
                 ("bias_factor", _D), ("max_hills", _I), ("stride", _I), ("grid_n", _I * 2),
-                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("traj_capacity", _I), ("lazy_neighbors", _I), ("want_virial", _I), ("skin", _D), ("box_slack", _D), ("fill_fraction", _D)]
+                ("grid_lo", _D * 2), ("grid_hi", _D * 2), ("force_scale", _D), ("period", _D * MAX_CV), ("traj_capacity", _I), ("lazy_neighbors", _I), ("want_virial", _I), ("skin", _D), ("box_slack", _D), ("fill_fraction", _D), ("c_window_lo", _D)]
 
 
 EXPORTS = ["metad_create", "metad_destroy", "metad_build_neighbors", "metad_eval_cv", "metad_bias",
@@ -172,7 +172,7 @@ class MetaD:
     precision == 32)."""
 
     def __init__(self, workload, max_hills=None, precision=None, grid=None, force_scale=1.0, stream=None, want_virial=False, lazy_neighbors=False, traj_capacity=0,
-                 box_slack=0.0, skin=0.0, fill_fraction=0.0):
+                 box_slack=0.0, skin=0.0, fill_fraction=0.0, c_window_lo=0.0):
         import torch
         self.torch = torch
         L = load()
@@ -227,6 +227,7 @@ class MetaD:
         p.traj_capacity = int(traj_capacity)
         p.box_slack = float(box_slack)
         p.fill_fraction = float(fill_fraction)
+        p.c_window_lo = float(c_window_lo)
         p.skin = float(skin)
         self._params = p
         h = _P()

@@ -65,7 +65,7 @@ def _run_ranks(w, world, precision, pos, hills, skin=0.0, frames=None):
     return out, ranks
 
 
-@pytest.mark.parametrize("name,precision,world", [("c3", 32, 2), ("c3", 32, 3), ("c4", 32, 2), ("c3", 64, 2)])
+@pytest.mark.parametrize("name,precision,world", [("c3", 32, 2), ("c3", 32, 3), ("c3", 32, 5), ("c4", 32, 2), ("c3", 64, 2)])
 def test_decomposed_step_matches_the_oracle_and_the_single_context(name, precision, world):
     import torch
     from paper_2510_06873_b200.metad import MetaD
@@ -163,3 +163,24 @@ def test_owned_sum_rejects_contexts_without_per_atom_values():
     with pytest.raises(MetadError) as e:
         md.cv_owned_sum(ow)
     assert e.value.code == metad.ERR_STATE
+
+
+def test_an_atom_outside_the_window_of_the_rank_is_flagged():
+    """Only the tiles of the rank's window [c_window_lo, c_window_lo + fill_fraction) are launched: an atom that has left it
+    would silently get no neighbours, so the binning raises METAD_DEV_POS_RANGE."""
+    import torch
+    from paper_2510_06873_b200 import metad
+    w = _workload("c3")
+    rk = domain.SlabMetaD(w, 4, 1, precision=32, max_hills=8)
+    p = w.pos[rk.local].astype(np.float32)
+    with torch.cuda.stream(rk.md.stream):
+        dp = torch.tensor(p, device="cuda")
+    rk.md.synchronize()
+    rk.phase1(dp)
+    assert rk.md.status() == 0
+    cz = w.box.reshape(3, 3)[2, 2]
+    p[7, 2] = np.float32((p[7, 2] + 0.5 * cz) % cz)            # half a box away along c: outside the window of rank 1 of 4
+    with torch.cuda.stream(rk.md.stream):
+        dp.copy_(torch.tensor(p))
+    rk.phase1(dp)
+    assert rk.md.status() & metad.DEV_POS_RANGE
