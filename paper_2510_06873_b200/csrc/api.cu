@@ -287,6 +287,10 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
         const int ones[2] = { 1, 1 };                       // the first step builds
         CUDA_TRY(cudaMemcpy(c->d_skin_flag, ones, sizeof(ones), cudaMemcpyHostToDevice));
         CUDA_TRY(cudaMalloc(&c->d_ref, 4 * tsz * (size_t)N));
+    }
+    if (p->fill_fraction > 0.0 && p->fill_fraction < 1.0 && c->has_q6 && c->prec == 32 && c->maxn <= 32)
+        CUDA_TRY(dev_alloc(&c->d_own_count, N));             // slab-decomposition rank on the tiled Q6 path (domain.cu)
+    if (c->skin_on) {
         if (c->has_q6 && c->prec == 32 && c->maxn <= 32) {            // the tiled Q6 path may run: its per-step rc list
             CUDA_TRY(dev_alloc(&c->d_rc_count, N));
             CUDA_TRY(dev_alloc(&c->d_rc_list, (size_t)c->maxn * (((size_t)N + 31) / 32 * 32)));
@@ -307,7 +311,7 @@ extern "C" int metad_destroy(metad_ctx *c) {
     void *ptrs[] = { c->d_cell_count, c->d_cell_start, c->d_block_sums, c->d_cell_of, c->d_slot, c->d_perm, c->d_scell,
                      c->d_spos, c->d_nl_count, c->d_nl, c->d_flags, c->d_rec, c->d_partials, c->d_tickets, c->d_centers,
                      c->d_heights, c->d_nhills, c->d_step, c->d_sticky, c->d_cv, c->d_V, c->d_dVds, c->d_bias_partials,
-                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage, c->d_geom, c->d_skin_flag, c->d_ref, c->d_nbuilds, c->d_rc_count, c->d_rc_list, c->d_tile_cuts };
+                     c->d_table, c->d_pos_stage, c->d_F_stage, c->d_aux, c->d_q6, c->d_cgrad, c->d_cvq6, c->d_perm_raw, c->d_tors_grad, c->d_tors_atoms, c->d_partials_warp, c->d_mind, c->d_box_force, c->d_virial, c->d_vir_partials, c->d_traj, c->d_hill_stage, c->d_geom, c->d_skin_flag, c->d_ref, c->d_nbuilds, c->d_rc_count, c->d_rc_list, c->d_tile_cuts, c->d_own_count };
     for (void *q : ptrs) if (q) cudaFree(q);
     for (int d = 0; d < c->D; ++d) {
         CvDev &v = c->cv[d];
@@ -485,6 +489,7 @@ static int build_neighbors_impl(metad_ctx *c, const void *d_pos, const double *h
     int r = c->dg ? METAD_OK : setup_geometry(c, h_box, rc);     // device box: geometry frozen by metad_build_neighbors_dev
     if (r) return r;
     c->d_pos_last = d_pos;
+    c->own_count_valid = 0;                         // masked counts of the last step (metad_cv_owned_sum) are stale now
     // no CV reads the list; a nearest-distance CV with a few explicit centres is scanned without one (k_mindist_brute)
     bool mind_brute = c->has_mindist;
     for (int d = 0; d < c->D; ++d)

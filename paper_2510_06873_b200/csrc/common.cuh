@@ -261,6 +261,8 @@ struct metad_ctx {
     int geom_ncell;                       // cells of the last setup_geometry before any x-subdivision (skin: detects a new grid)
     int *d_skin_flag;                     // [2] rebuild flags, indexed by the parity of the device step counter (neighbor.cu)
     void *d_ref;                          // Vec4<T>[N]: cell-sorted positions at the last build (displacement check)
+    int *d_own_count; int own_count_valid; // slab-decomposition rank (fill_fraction < 1), tiled Q6 path: neighbour counts with the atoms the
+                                          // rank does not own set to 0 (metad_cv_owned_sum), read by the force pass of the same step
     int *d_rc_count, *d_rc_list;          // skin, tiled Q6 path: the entries of the kept list that lie within rc THIS step (pass 1 -> force pass)
     int *d_nbuilds;                       // number of neighbour-list builds so far (metad_get_rebuilds)
     bool have_neighbors, list_built;

@@ -716,7 +716,7 @@ int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
     double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
     const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
 #define Q6FG_ARGS                                                                                                          \
-    c->N, c->maxn, (const float4 *)c->d_spos, c->skin_on ? c->d_rc_count : c->d_nl_count, c->skin_on ? c->d_rc_list : c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm, ss,  \
+    c->N, c->maxn, (const float4 *)c->d_spos, c->own_count_valid ? c->d_own_count : (c->skin_on ? c->d_rc_count : c->d_nl_count), c->skin_on ? c->d_rc_list : c->d_nl, c->d_perm, c->boxd, (const float *)c->d_rec, sm, ss,  \
         c->q6_mean_dim, c->q6_solid_dim, c->p.force_scale, d_dVds, (float *)d_F, va, c->d_q6 + c->N, c->dg, skin_far2(c)
 #define Q6FG_GRID <<<div_up(c->N, CV_THREADS), CV_THREADS, 0, c->stream>>>
 #define Q6FG_LAUNCH(SOLID, VIR)                                                                                            \

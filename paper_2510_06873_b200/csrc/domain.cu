@@ -20,11 +20,14 @@ template <typename T>
 __global__ void __launch_bounds__(OWN_THREADS)
 k_cv_owned_sum(int N, const int *__restrict__ perm, const unsigned char *__restrict__ owned, const T *__restrict__ q6,
                int q6_stride, T q_thresh, T inv_width, double scale_mean, double scale_solid, int dim_mean, int dim_solid,
-               double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out) {
+               double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
+               const int *__restrict__ count_in, int *__restrict__ count_out /* tiled path: neighbour counts, 0 for atoms not owned */) {
     __shared__ double red[64];
     double v[2] = { 0.0, 0.0 };
     for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < N; s += gridDim.x * blockDim.x) {
-        if (!owned[perm[s]]) continue;
+        const bool mine = owned[perm[s]] != 0;
+        if (count_out) count_out[s] = mine ? count_in[s] : 0;
+        if (!mine) continue;
         const T q = q6[(size_t)s * q6_stride];
         v[0] += (double)q;
         if (dim_solid >= 0) v[1] += (double)(T(1) / (T(1) + exp(-(q - q_thresh) * inv_width)));     // the expression of the pass-1 kernels
@@ -57,15 +60,20 @@ extern "C" int metad_cv_owned_sum(metad_ctx *c, const unsigned char *d_owned, do
     const double ss = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0;
     double *partials = c->d_partials + c->nblocks_atoms;       // free again once eval_cv's kernel has finished (stream order)
     unsigned int *ticket = c->d_tickets + 14;
-    if (c->tiled)
+    if (c->tiled) {
+        // the force pass of this step skips the atoms the rank does not own (their rows of F belong to other ranks): it walks
+        // the neighbour counts written here, which are 0 for them
+        const int *cin = c->skin_on ? c->d_rc_count : c->d_nl_count;
         k_cv_owned_sum<float><<<nb, OWN_THREADS, 0, c->stream>>>(N, c->d_perm, d_owned, c->d_q6, 1, (float)qt, (float)(1.0 / qw), sm, ss,
-                                                                 c->q6_mean_dim, c->q6_solid_dim, partials, ticket, d_cv);
+                                                                 c->q6_mean_dim, c->q6_solid_dim, partials, ticket, d_cv, cin, c->d_own_count);
+        c->own_count_valid = c->d_own_count != nullptr;
+    }
     else if (c->prec == 32)
         k_cv_owned_sum<float><<<nb, OWN_THREADS, 0, c->stream>>>(N, c->d_perm, d_owned, (const float *)c->d_rec + 14, METAD_NREC, (float)qt,
-                                                                 (float)(1.0 / qw), sm, ss, c->q6_mean_dim, c->q6_solid_dim, partials, ticket, d_cv);
+                                                                 (float)(1.0 / qw), sm, ss, c->q6_mean_dim, c->q6_solid_dim, partials, ticket, d_cv, nullptr, nullptr);
     else
         k_cv_owned_sum<double><<<nb, OWN_THREADS, 0, c->stream>>>(N, c->d_perm, d_owned, (const double *)c->d_rec + 14, METAD_NREC, qt, 1.0 / qw,
-                                                                  sm, ss, c->q6_mean_dim, c->q6_solid_dim, partials, ticket, d_cv);
+                                                                  sm, ss, c->q6_mean_dim, c->q6_solid_dim, partials, ticket, d_cv, nullptr, nullptr);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;
