@@ -319,7 +319,9 @@ int metad_bias_noalloc(const double *d_centers, int ld_centers, const double *d_
 /* Slab decomposition over several GPUs: after metad_eval_cv, replaces the Q6 CVs in
  * d_cv (device, [ncv]) by their sums over the atoms this rank OWNS — d_owned: device, natoms bytes, != 0 for an owned atom,
  * indexed like d_pos.  The ranks then add their d_cv (one all-reduce of ncv doubles) and go on with metad_bias /
- * metad_apply_forces / metad_deposit on the same global s.  Fixed-order sum (run-to-run identical).  [async]
+ * metad_apply_forces / metad_deposit on the same global s.  Fixed-order sum (run-to-run identical).  On the tiled fp32 path
+ * (fill_fraction < 1) the metad_apply_forces of the SAME step then skips the atoms that are not owned: their rows of d_F
+ * belong to other ranks and get nothing added.  [async]
  * Errors: METAD_ERR_STATE unless every CV dimension of the context is a Q6 CV and the CVs have been evaluated. */
 int metad_cv_owned_sum(metad_ctx *ctx, const unsigned char *d_owned, double *d_cv);
 
