@@ -52,7 +52,7 @@ extern "C" int metad_create(metad_ctx **out, const metad_params *p, void *cuda_s
     if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0)
         FAIL(METAD_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
 
-    if (tiled_init()) return METAD_ERR_CUDA;
+    if (tiled_init() || tiled64_init()) return METAD_ERR_CUDA;
     metad_ctx *c = new metad_ctx();
     memset(c, 0, sizeof(*c));
     // every failure below leaves through ONE path that frees whatever was allocated so far (metad_destroy works on a
@@ -239,7 +239,9 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
         CUDA_TRY(cudaMalloc(&c->d_rec, METAD_NREC * tsz * (size_t)N));
         CUDA_TRY(dev_alloc(&c->d_q6, 2 * (size_t)N));       // q6 per atom, then f'(q6) per atom (tiled path, solid-like count)
     }
-    CUDA_TRY(dev_alloc(&c->d_partials, 3 * (size_t)c->nblocks_atoms + max_pair_blocks));
+    // (+ 2 x 4096: per-tile partials of the fp64 tiled build on systems too small for one tile per 128 atoms; partials never
+    // outlive the kernel that writes them, so the regions of different kernels may overlap)
+    CUDA_TRY(dev_alloc(&c->d_partials, 3 * (size_t)c->nblocks_atoms + max_pair_blocks + 2 * 4096));
     if (c->has_coord && N <= METAD_WARP_PER_ATOM_MAX) CUDA_TRY(dev_alloc(&c->d_partials_warp, (size_t)N / 4 + 2));
     CUDA_TRY(dev_alloc(&c->d_tickets, 16));
     CUDA_TRY(cudaMemset(c->d_tickets, 0, sizeof(unsigned) * 16));
@@ -370,10 +372,12 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc, double sla
     c->rc = rc; c->rc2 = rc * rc; c->rcl = rcl; c->rcl2 = rcl * rcl;
     // shared-memory tiled fast path: fp32, neighbour-list CVs = Q6 only or an ungrouped coordination number only,
     // >= 3 cells per direction
-    c->tiled = 0;
+    c->tiled = 0; c->tiled64 = 0;
     const bool q6_only = c->has_q6 && !c->has_coord;
     const bool coord_only = c->n_coord == 1 && !c->has_q6 && !c->cv[c->coord_dim].use_groups && !c->skin_on;
-    if (c->prec == 32 && (q6_only || coord_only) && !c->has_mindist && c->N < (1 << NL_IDX_BITS) && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32) {
+    // fp64 pair math: the same tiles for Q6 contexts without a skin (tiled64.cu; 32 bytes per staged atom)
+    const bool tile32 = c->prec == 32 && (q6_only || coord_only), tile64 = c->prec == 64 && q6_only && !c->skin_on;
+    if ((tile32 || tile64) && !c->has_mindist && c->N < (1 << NL_IDX_BITS) && g.nc[0] >= 3 && g.nc[1] >= 3 && g.nc[2] >= 3 && c->maxn <= 32) {
         // the rc-wide cells are subdivided along x (the direction of the contiguous row runs): an atom then scans
         // 2 xsub + 1 sub-cells per row (2.5 / 2.25 cell widths for xsub = 2 / 4) instead of 3 cells
         int xsub = 2;
@@ -392,13 +396,13 @@ static int setup_geometry(metad_ctx *c, const double *box, double rc, double sla
             double own = rho * tx * ty * tz, halo = rho * (tx + 2 * xsub) * (ty + 2) * (tz + 2);
             if (halo * margin > cap || own > TILE_THREADS) continue;
             long long ntl = (long long)((gs.nc[0] + tx - 1) / tx) * ((gs.nc[1] + ty - 1) / ty) * ((gs.nc[2] + tz - 1) / tz);
-            if (ntl > c->nblocks_atoms) continue;     // per-tile partials live in the per-block scratch
+            if (ntl > c->nblocks_atoms + (tile64 ? 4096 : 0)) continue;     // per-tile partials live in the per-block scratch
             double score = halo / own + (own < 128 ? 2.0 : 0.0);   // halo ratio; keep the block busy
             if (pass == 0) { if (score < best) best = score; }
             else if (score <= 1.02 * best && tx > bt[0]) { bt[0] = tx; bt[1] = ty; bt[2] = tz; }
         }
         if (bt[0] > 0) {
-            c->tiled = 1; c->tile_T[0] = bt[0]; c->tile_T[1] = bt[1]; c->tile_T[2] = bt[2]; c->tile_cap = cap; c->tile_hx = xsub;
+            c->tiled = tile32; c->tiled64 = tile64; c->tile_T[0] = bt[0]; c->tile_T[1] = bt[1]; c->tile_T[2] = bt[2]; c->tile_cap = cap; c->tile_hx = xsub;
             c->grid = gs;
             // tile boundaries (tile k of a direction covers cells [k nc / nt, (k + 1) nc / nt)): a small device table,
             // uploaded only when the tiling changes (never inside a capture: run_impl derives the geometry before it starts one)

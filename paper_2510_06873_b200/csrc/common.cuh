@@ -321,6 +321,7 @@ struct metad_ctx {
     int *d_aux;                           // device scalars: grid-miss flag, index of the hill deposited this step
     // shared-memory tiled fast path (fp32, Q6): tile.cuh / tiled.cu
     int tiled; int tile_T[3]; int tile_cap; int tile_hx;
+    int tiled64;                          // the same tiling with fp64 pair math (tiled64.cu: Q6 contexts; output in the generic formats)
     int *d_tile_cuts; int tile_cuts_key[6];    // tile boundaries per direction (device) and the (nc, nt) they were computed for
     int timing; int capturing; int timing_recorded; cudaEvent_t ev[3];
     cudaStream_t copy_stream; cudaEvent_t ev_copy;   // metad_step_host: the force upload overlaps the first three stages
@@ -370,3 +371,5 @@ int tiled_build(metad_ctx *c);
 int tiled_q6_pass1(metad_ctx *c, double *d_cv);
 int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F);
 int tiled_coord_force(metad_ctx *c, const double *d_dVds, void *d_F);
+int tiled64_init();
+int tiled64_build(metad_ctx *c);

@@ -989,8 +989,8 @@ static int cv_eval_t(metad_ctx *c, double *d_cv) {
                                                        c->d_tickets + 0, d_cv + cd, c->d_sticky, c->dg);
         c->launches++;
     }
-    if (c->has_q6 && c->tiled) {
-        int r = c->skin_on ? tiled_q6_pass1_skin(c, d_cv) : tiled_q6_pass1(c, d_cv);
+    if (c->has_q6 && (c->tiled || c->tiled64)) {              // tiled64: the fp64 sums ran inside k_tile_build64
+        int r = (c->tiled && c->skin_on) ? tiled_q6_pass1_skin(c, d_cv) : tiled_q6_pass1(c, d_cv);
         if (r) return r;
     } else if (c->has_q6) {
         double sm = c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0;

@@ -450,7 +450,7 @@ __global__ void k_geom_update(const double *__restrict__ box, double rc, int nc0
 }
 
 int geom_update(metad_ctx *c, const double *d_box) {
-    k_geom_update<<<1, 32, 0, c->stream>>>(d_box, c->rc, c->grid.nc[0], c->grid.nc[1], c->grid.nc[2], c->tiled ? c->tile_hx : 1,
+    k_geom_update<<<1, 32, 0, c->stream>>>(d_box, c->rc, c->grid.nc[0], c->grid.nc[1], c->grid.nc[2], (c->tiled || c->tiled64) ? c->tile_hx : 1,
                                            1e-5f, c->d_geom, c->d_sticky);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
@@ -561,7 +561,7 @@ static int nb_build_kernels(metad_ctx *c, const void *d_pos) {
     const bool tm = c->timing && !c->capturing;
     const int *sf = c->skin_on ? c->d_skin_flag : nullptr, *stp = c->d_step;
     V4 *ref = c->skin_on ? (V4 *)c->d_ref : nullptr;
-    if (N <= METAD_SMALL_N && !c->tiled) {                     // the whole neighbour stage in one launch
+    if (N <= METAD_SMALL_N && !c->tiled && !c->tiled64) {                     // the whole neighbour stage in one launch
         if (tm) cudaEventRecord(c->ev[1], st);
         k_build_list_small<T><<<div_up((long long)N * 32, 128), 128, 0, st>>>(N, (const T *)d_pos, c->d_flags, (V4 *)c->d_spos, c->d_perm,
                                                                              c->d_scell, make_pbox<T>(c->boxd, c->rcl), c->boxd, (T)c->rcl2, c->rcl2,
@@ -585,9 +585,9 @@ static int nb_build_kernels(metad_ctx *c, const void *d_pos) {
                 (const unsigned char *)c->d_flags,   /* NULL unless a COORD / MINDIST CV has groups */
                 (V4 *)c->d_spos, c->d_scell, c->tiled ? 1 : 0, ref, sf, stp, c->d_nbuilds);
     if (tm) cudaEventRecord(c->ev[1], st);
-    if (c->tiled && sizeof(T) == 4) {
+    if ((c->tiled && sizeof(T) == 4) || (c->tiled64 && sizeof(T) == 8)) {
         c->launches += 5;
-        int r = tiled_build(c);
+        int r = sizeof(T) == 4 ? tiled_build(c) : tiled64_build(c);
         if (tm) cudaEventRecord(c->ev[2], st);
         return r;
     }
