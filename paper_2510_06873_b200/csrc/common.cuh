@@ -60,6 +60,19 @@ template <> struct Vec4<double> { typedef double4 type; };
 template <typename T>
 __device__ __forceinline__ typename Vec4<T>::type ld4(const typename Vec4<T>::type *p) { return *p; }
 
+// Read-only gather of one Vec4: a double4 is 32 bytes but only 16-byte aligned for the compiler, which splits it into two
+// 128-bit loads; the arrays gathered here (cell-sorted positions, q6 records) have 32-byte element strides on 256-byte
+// aligned allocations, so the fp64 kernels fetch an element with ONE 256-bit load (sm_100 LDG.E.256: half the L1 requests
+// of a gather-bound kernel).  Only for arrays the kernel does not write.
+template <typename T>
+__device__ __forceinline__ typename Vec4<T>::type ldg4(const typename Vec4<T>::type *p);
+template <> __device__ __forceinline__ float4 ldg4<float>(const float4 *p) { return *p; }
+template <> __device__ __forceinline__ double4 ldg4<double>(const double4 *p) {
+    double4 v;
+    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+    return v;
+}
+
 // Minimum-image displacement (reading O order: z against c, y against b, x against a).
 template <typename T>
 __device__ __forceinline__ void min_image(const PBox<T> &b, T &dx, T &dy, T &dz) {

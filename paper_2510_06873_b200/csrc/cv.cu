@@ -27,7 +27,7 @@ k_coord_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
             int cnt = nl_count[s];
             for (int k = 0; k < cnt; ++k) {
                 int j = nl[(size_t)k * N + s];
-                typename Vec4<T>::type pj = spos[j];
+                typename Vec4<T>::type pj = ldg4<T>(spos + j);
                 if (!((((int)pj.w) >> fshift) & 2)) continue;
                 if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
                 T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
@@ -75,7 +75,7 @@ k_coord_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int 
     int cnt = act ? nl_count[s] : 0;
     for (int k = 0; k < cnt; ++k) {
         int j = nl[(size_t)k * N + s];
-        typename Vec4<T>::type pj = spos[j];
+        typename Vec4<T>::type pj = ldg4<T>(spos + j);
         const int fj = ((int)pj.w) >> fshift;
         int mult = ((fi & 1) && (fj & 2)) + ((fi & 2) && (fj & 1));
         if (!mult) continue;
@@ -128,7 +128,7 @@ k_coord_cv_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const in
             const int cnt = nl_count[s];
             for (int k = lane; k < cnt; k += G) {
                 const int j = nl[(size_t)k * N + s];
-                typename Vec4<T>::type pj = spos[j];
+                typename Vec4<T>::type pj = ldg4<T>(spos + j);
                 if (!((((int)pj.w) >> fshift) & 2)) continue;
                 if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
                 T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
@@ -170,7 +170,7 @@ k_coord_force_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const
     const int cnt = (fi & 3) ? nl_count[s] : 0;             // an atom in neither group takes no force
     for (int k = lane; k < cnt; k += G) {
         const int j = nl[(size_t)k * N + s];
-        typename Vec4<T>::type pj = spos[j];
+        typename Vec4<T>::type pj = ldg4<T>(spos + j);
         const int fj = ((int)pj.w) >> fshift;
         const int mult = ((fi & 1) && (fj & 2)) + ((fi & 2) && (fj & 1));
         if (!mult) continue;
@@ -223,7 +223,7 @@ k_q6_pass1(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
             const int j = e0;
             e0 = e1;
             if (k + 2 < nlist) e1 = nl[(size_t)(k + 2) * N + s];
-            typename Vec4<T>::type pj = spos[j];
+            typename Vec4<T>::type pj = ldg4<T>(spos + j);
             if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
             ++cnt;
             T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
@@ -306,7 +306,7 @@ k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
     T Bk[13];
     {
         const V4 *r4 = reinterpret_cast<const V4 *>(rec + (size_t)s * METAD_NREC);
-        V4 a = r4[0], b = r4[1], c = r4[2], d = r4[3];
+        V4 a = ldg4<T>(r4), b = ldg4<T>(r4 + 1), c = ldg4<T>(r4 + 2), d = ldg4<T>(r4 + 3);
         T gk = alpha + beta * d.y;
         Bk[0] = gk * a.x; Bk[1] = gk * a.y; Bk[2] = gk * a.z; Bk[3] = gk * a.w;
         Bk[4] = gk * b.x; Bk[5] = gk * b.y; Bk[6] = gk * b.z; Bk[7] = gk * b.w;
@@ -320,10 +320,10 @@ k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
         const int j = e0;
         e0 = e1;
         if (k + 2 < cnt) e1 = nl[(size_t)(k + 2) * N + s];
-        V4 pj = spos[j];
+        V4 pj = ldg4<T>(spos + j);
         if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
         const V4 *r4 = reinterpret_cast<const V4 *>(rec + (size_t)j * METAD_NREC);
-        V4 a = r4[0], b = r4[1], c = r4[2], d = r4[3];
+        V4 a = ldg4<T>(r4), b = ldg4<T>(r4 + 1), c = ldg4<T>(r4 + 2), d = ldg4<T>(r4 + 3);
         T gj = alpha + beta * d.y;
         T bb[13];
         bb[0] = Bk[0] + gj * a.x; bb[1] = Bk[1] + gj * a.y; bb[2] = Bk[2] + gj * a.z; bb[3] = Bk[3] + gj * a.w;
@@ -784,7 +784,7 @@ k_mindist_cv(int N, const typename Vec4<T>::type *__restrict__ spos, const int *
             const long long io = perm[s];
             for (int k = 0; k < cnt; ++k) {
                 const int j = nl[(size_t)k * N + s];
-                const typename Vec4<T>::type pj = spos[j];
+                const typename Vec4<T>::type pj = ldg4<T>(spos + j);
                 if (!((((int)pj.w) >> fshift) & 2)) continue;
                 if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
                 T dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;

@@ -217,7 +217,7 @@ k_build_list(int N, const typename Vec4<T>::type *__restrict__ spos, const int *
                 ja += ja < 0 ? g.nc[0] : 0; ja -= ja >= g.nc[0] ? g.nc[0] : 0;
                 int cb = cell_start[rowbase + ja], ce = cell_start[rowbase + ja + 1];
                 for (int j = cb; j < ce; ++j) {
-                    typename Vec4<T>::type pj = spos[j];
+                    typename Vec4<T>::type pj = ldg4<T>(spos + j);
                     if (j != s && pair_in_run<T>(shifted, w, pb, bd, rc2T, rc2, pi, pj)) {
                         if (cnt < maxn) nl[(size_t)cnt * N + s] = j;
                         ++cnt;
@@ -281,7 +281,7 @@ k_build_list_warp(int N, const typename Vec4<T>::type *__restrict__ spos, const 
                 for (int j0 = cb; j0 < ce; j0 += G) {
                     const int j = j0 + lane;
                     bool hit = false;
-                    if (j < ce && j != s) hit = pair_in_run<T>(shifted, w, pb, bd, rc2T, rc2, pi, spos[j]);
+                    if (j < ce && j != s) hit = pair_in_run<T>(shifted, w, pb, bd, rc2T, rc2, pi, ldg4<T>(spos + j));
                     const unsigned m = (__ballot_sync(gmask, hit) & gmask) >> gshift;
                     if (hit) {
                         const int k = cnt + __popc(m & ((1u << lane) - 1u));

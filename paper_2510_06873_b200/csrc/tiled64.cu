@@ -84,8 +84,16 @@ __device__ __forceinline__ int scan_atom64(const TileGeom &g, const TileTables &
                 const int h2 = min(hi, lo + room);
 #pragma unroll 2
                 for (int lj = lo; lj < h2; ++lj) {
-                    const double4 pj = hpos64<STAGED>(g, t, spos, pos_s, lj, dg);
-                    const double ex = pj.x - pi.x, ey = pj.y - pi.y, ez = pj.z - pi.z;
+                    // staged: 24 of the 32 bytes (one 128-bit + one 64-bit shared-memory load: the scan is bound by
+                    // shared-memory wavefronts, profiles/r2l_fp64.md); the index in .w is read by the exact pass only
+                    double ex, ey, ez;
+                    if (STAGED) {
+                        const double2 xy = *reinterpret_cast<const double2 *>(pos_s + lj);
+                        ex = xy.x - pi.x; ey = xy.y - pi.y; ez = reinterpret_cast<const double *>(pos_s + lj)[2] - pi.z;
+                    } else {
+                        const double4 pj = hpos64<STAGED>(g, t, spos, pos_s, lj, dg);
+                        ex = pj.x - pi.x; ey = pj.y - pi.y; ez = pj.z - pi.z;
+                    }
                     const double r2 = fma(ez, ez, fma(ey, ey, ex * ex));
                     asm volatile("st.shared.u16 [%0], %1;" ::"r"(wp), "h"((unsigned short)lj));
                     asm volatile("{ .reg .pred p; setp.lt.f64 p, %1, %2; @p add.u32 %0, %0, %3; }"
