@@ -237,7 +237,7 @@ static int create_impl(metad_ctx *c, const metad_params *p, void *cuda_stream) {
         CUDA_TRY(dev_alloc(&c->d_cgrad, 4 * (size_t)N));
     if (c->has_q6) {
         CUDA_TRY(cudaMalloc(&c->d_rec, METAD_NREC * tsz * (size_t)N));
-        CUDA_TRY(dev_alloc(&c->d_q6, 2 * (size_t)N));       // q6 per atom, then f'(q6) per atom (tiled path, solid-like count)
+        CUDA_TRY(cudaMalloc((void **)&c->d_q6, 2 * tsz * (size_t)N));   // q6 per atom, then f'(q6) per atom, in the pair precision
     }
     // (+ 2 x 4096: per-tile partials of the fp64 tiled build on systems too small for one tile per 128 atoms; partials never
     // outlive the kernel that writes them, so the regions of different kernels may overlap)

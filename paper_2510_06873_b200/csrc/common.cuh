@@ -11,7 +11,8 @@
 // below this size the neighbour stage is one brute-force kernel without cells (k_build_list_small)
 #define METAD_SMALL_N 1024
 
-#define METAD_NREC 16  // per-atom Q6 record: 13 normalised q6m components + f'(q6) + q6 + pad
+#define METAD_NREC 16  // per-atom Q6 record: 13 normalised q6m components + the atom's position (the force pass gathers ONE array);
+                       // q6 and f'(q6) live in the dense per-atom arrays d_q6 [N] | [N]
 
 // ------------------------------------------------------------------------------------------------
 // Periodic box for the pair arithmetic in precision T.  Lattice rows a=(ax,0,0), b=(bx,by,0),
@@ -338,7 +339,7 @@ struct metad_ctx {
     int *d_tile_cuts; int tile_cuts_key[6];    // tile boundaries per direction (device) and the (nc, nt) they were computed for
     int timing; int capturing; int timing_recorded; cudaEvent_t ev[3];
     cudaStream_t copy_stream; cudaEvent_t ev_copy;   // metad_step_host: the force upload overlaps the first three stages
-    float *d_q6;                          // tiled path: per-atom q6 (sorted order) [N], then f'(q6) [N]
+    float *d_q6;                          // per-atom q6 (sorted order) [N], then f'(q6) [N], in the pair precision (double on fp64 contexts)
     float *d_cgrad;                       // tiled coordination path: per-atom sum_j 2 sw' d / (r0 r) as float4, ORIGINAL atom
                                           // order (k_tile_build<2>), scaled and added to F by k_force_add
     double *d_cvq6;                       // tiled path: [Q6 mean, solid count] finished by k_tile_build

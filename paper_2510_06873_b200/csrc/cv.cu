@@ -203,6 +203,7 @@ template <typename T>
 __global__ void __launch_bounds__(CV_THREADS, 5)        // fp64: 96 registers instead of 120, five blocks per SM: 0.305 -> 0.262 ms at c3
 k_q6_pass1(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
            const int *__restrict__ nl, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, T q_thresh, T inv_width, T *__restrict__ rec,
+           T *__restrict__ q6arr /* [N] q6, then [N] f'(q6) */,
            double scale_mean, double scale_solid, int dim_mean, int dim_solid,
            double *__restrict__ partials, unsigned int *__restrict__ ticket, double *__restrict__ cv_out,
            unsigned int *__restrict__ sticky, const DevGeom *__restrict__ dg) {
@@ -252,12 +253,13 @@ k_q6_pass1(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
             fsw = f;
             dfsw = f * (T(1) - f) * inv_width;
         }
-        // record: B_m = conj(A_m)/(n sqrt(S)); [13] = f'(q6); [14] = q6
+        // record: B_m = conj(A_m)/(n sqrt(S)); [13..15] = the atom's position (one gather per pair in the force pass)
         T out[METAD_NREC];
         out[0] = A[0] * norm;
 #pragma unroll
         for (int m = 1; m <= 6; ++m) { out[2 * m - 1] = A[2 * m - 1] * norm; out[2 * m] = -A[2 * m] * norm; }
-        out[13] = dfsw; out[14] = q6; out[15] = T(0);
+        out[13] = pi.x; out[14] = pi.y; out[15] = pi.z;
+        q6arr[s] = q6; q6arr[(size_t)N + s] = dfsw;
         typename Vec4<T>::type *r4 = reinterpret_cast<typename Vec4<T>::type *>(rec + (size_t)s * METAD_NREC);
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
@@ -288,7 +290,7 @@ template <typename T, bool VIRIAL>
 __global__ void __launch_bounds__(CV_THREADS)
 k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__restrict__ nl_count,
            const int *__restrict__ nl, const int *__restrict__ perm, PBox<T> pb, BoxD bdk, T rc2T, double rc2k /* Verlet skin: keep pairs with r < rc only; 0 = the list is exact */, const T *__restrict__ rec,
-           double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
+           const T *__restrict__ fprime /* [N] f'(q6) */, double scale_mean, double scale_solid, int dim_mean, int dim_solid, double force_scale,
            const double *__restrict__ dVds, T *__restrict__ F, VirArgs va, const DevGeom *__restrict__ dg) {
     typedef typename Vec4<T>::type V4;
     if (dg) { pb = dg_pb<T>(dg); bdk = dg->bd; }
@@ -307,7 +309,7 @@ k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
     {
         const V4 *r4 = reinterpret_cast<const V4 *>(rec + (size_t)s * METAD_NREC);
         V4 a = ldg4<T>(r4), b = ldg4<T>(r4 + 1), c = ldg4<T>(r4 + 2), d = ldg4<T>(r4 + 3);
-        T gk = alpha + beta * d.y;
+        T gk = beta != T(0) ? alpha + beta * fprime[s] : alpha;
         Bk[0] = gk * a.x; Bk[1] = gk * a.y; Bk[2] = gk * a.z; Bk[3] = gk * a.w;
         Bk[4] = gk * b.x; Bk[5] = gk * b.y; Bk[6] = gk * b.z; Bk[7] = gk * b.w;
         Bk[8] = gk * c.x; Bk[9] = gk * c.y; Bk[10] = gk * c.z; Bk[11] = gk * c.w;
@@ -320,11 +322,13 @@ k_q6_force(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
         const int j = e0;
         e0 = e1;
         if (k + 2 < cnt) e1 = nl[(size_t)(k + 2) * N + s];
-        V4 pj = ldg4<T>(spos + j);
-        if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
+        // the record carries the neighbour's position: four gathers of one array per pair instead of five of two
         const V4 *r4 = reinterpret_cast<const V4 *>(rec + (size_t)j * METAD_NREC);
-        V4 a = ldg4<T>(r4), b = ldg4<T>(r4 + 1), c = ldg4<T>(r4 + 2), d = ldg4<T>(r4 + 3);
-        T gj = alpha + beta * d.y;
+        V4 d = ldg4<T>(r4 + 3), pj;
+        pj.x = d.y; pj.y = d.z; pj.z = d.w; pj.w = T(0);
+        if (rc2k > 0.0 && !pair_in_range<T>(pb, bdk, rc2T, rc2k, pi, pj)) continue;
+        V4 a = ldg4<T>(r4), b = ldg4<T>(r4 + 1), c = ldg4<T>(r4 + 2);
+        T gj = beta != T(0) ? alpha + beta * fprime[j] : alpha;
         T bb[13];
         bb[0] = Bk[0] + gj * a.x; bb[1] = Bk[1] + gj * a.y; bb[2] = Bk[2] + gj * a.z; bb[3] = Bk[3] + gj * a.w;
         bb[4] = Bk[4] + gj * b.x; bb[5] = Bk[5] + gj * b.y; bb[6] = Bk[6] + gj * b.z; bb[7] = Bk[7] + gj * b.w;
@@ -737,12 +741,7 @@ int tiled_q6_force(metad_ctx *c, const double *d_dVds, void *d_F) {
 }
 
 template <typename T>
-__global__ void k_q6_export(int N, const int *__restrict__ perm, const T *__restrict__ rec, T *__restrict__ q6) {
-    int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s < N) q6[perm[s]] = rec[(size_t)s * METAD_NREC + 14];
-}
-
-__global__ void k_q6_export_arr(int N, const int *__restrict__ perm, const float *__restrict__ q6s, float *__restrict__ q6) {
+__global__ void k_q6_export_arr(int N, const int *__restrict__ perm, const T *__restrict__ q6s, T *__restrict__ q6) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s < N) q6[perm[s]] = q6s[s];
 }
@@ -998,7 +997,7 @@ static int cv_eval_t(metad_ctx *c, double *d_cv) {
         double qt = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_thresh : 0.0;
         double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
         k_q6_pass1<T><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0, (T)qt,
-                                                       (T)(1.0 / qw), (T *)c->d_rec, sm, ss, c->q6_mean_dim,
+                                                       (T)(1.0 / qw), (T *)c->d_rec, (T *)c->d_q6, sm, ss, c->q6_mean_dim,
                                                        c->q6_solid_dim, c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
                                                        d_cv, c->d_sticky, c->dg);
         c->launches++;
@@ -1063,11 +1062,11 @@ static int cv_forces_t(metad_ctx *c, const double *d_dVds, void *d_F) {
         const VirArgs va = { c->d_vir_partials, c->d_tickets + 12, c->d_virial };
         if (c->p.want_virial)
             k_q6_force<T, true><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0,
-                                                                 (const T *)c->d_rec, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
+                                                                 (const T *)c->d_rec, (const T *)c->d_q6 + c->N, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
                                                                  c->p.force_scale, d_dVds, (T *)d_F, va, c->dg);
         else
             k_q6_force<T, false><<<nb, CV_THREADS, 0, c->stream>>>(N, (const V4 *)c->d_spos, c->d_nl_count, c->d_nl, c->d_perm, pb, c->boxd, (T)c->rc2, c->skin_on ? c->rc2 : 0.0,
-                                                                  (const T *)c->d_rec, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
+                                                                  (const T *)c->d_rec, (const T *)c->d_q6 + c->N, sm, ss, c->q6_mean_dim, c->q6_solid_dim,
                                                                   c->p.force_scale, d_dVds, (T *)d_F, va, c->dg);
         c->launches++;
     }
@@ -1095,14 +1094,8 @@ int cv_forces_all(metad_ctx *c, const double *d_dVds, void *d_F) {
 int q6_export(metad_ctx *c, void *d_q6) {
     if (!c->has_q6) return METAD_ERR_STATE;
     int nb = div_up(c->N, 256);
-    if (c->tiled) {
-        k_q6_export_arr<<<nb, 256, 0, c->stream>>>(c->N, c->d_perm, c->d_q6, (float *)d_q6);
-        c->launches++;
-        CUDA_TRY(cudaGetLastError());
-        return METAD_OK;
-    }
-    if (c->prec == 32) k_q6_export<float><<<nb, 256, 0, c->stream>>>(c->N, c->d_perm, (const float *)c->d_rec, (float *)d_q6);
-    else k_q6_export<double><<<nb, 256, 0, c->stream>>>(c->N, c->d_perm, (const double *)c->d_rec, (double *)d_q6);
+    if (c->prec == 32) k_q6_export_arr<float><<<nb, 256, 0, c->stream>>>(c->N, c->d_perm, (const float *)c->d_q6, (float *)d_q6);
+    else k_q6_export_arr<double><<<nb, 256, 0, c->stream>>>(c->N, c->d_perm, (const double *)c->d_q6, (double *)d_q6);
     c->launches++;
     CUDA_TRY(cudaGetLastError());
     return METAD_OK;

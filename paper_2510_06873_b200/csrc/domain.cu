@@ -14,7 +14,7 @@
 #define OWN_THREADS 256
 #define OWN_MAX_BLOCKS 592                                  // 4 x 148 SMs: a few atoms per thread, ONE block reduction per block
 
-// q6 of sorted atom s: tiled fp32 contexts keep a dense per-atom array, the generic kernels the record entry [14].
+// q6 of sorted atom s: the dense per-atom array d_q6 of every Q6 path (q6_stride = 1).
 // Fixed assignment of atoms to threads and blocks, fixed-order reductions: run-to-run identical.
 template <typename T>
 __global__ void __launch_bounds__(OWN_THREADS)
@@ -69,10 +69,10 @@ extern "C" int metad_cv_owned_sum(metad_ctx *c, const unsigned char *d_owned, do
         c->own_count_valid = c->d_own_count != nullptr;
     }
     else if (c->prec == 32)
-        k_cv_owned_sum<float><<<nb, OWN_THREADS, 0, c->stream>>>(N, c->d_perm, d_owned, (const float *)c->d_rec + 14, METAD_NREC, (float)qt,
+        k_cv_owned_sum<float><<<nb, OWN_THREADS, 0, c->stream>>>(N, c->d_perm, d_owned, (const float *)c->d_q6, 1, (float)qt,
                                                                  (float)(1.0 / qw), sm, ss, c->q6_mean_dim, c->q6_solid_dim, partials, ticket, d_cv, nullptr, nullptr);
     else
-        k_cv_owned_sum<double><<<nb, OWN_THREADS, 0, c->stream>>>(N, c->d_perm, d_owned, (const double *)c->d_rec + 14, METAD_NREC, qt, 1.0 / qw,
+        k_cv_owned_sum<double><<<nb, OWN_THREADS, 0, c->stream>>>(N, c->d_perm, d_owned, (const double *)c->d_q6, 1, qt, 1.0 / qw,
                                                                   sm, ss, c->q6_mean_dim, c->q6_solid_dim, partials, ticket, d_cv, nullptr, nullptr);
     c->launches++;
     CUDA_TRY(cudaGetLastError());

@@ -9,7 +9,7 @@
 // What differs from the fp32 kernel: the halo is staged as RAW coordinates (plus the lattice shift of a periodic image,
 // added once): in fp64 there is no exactness to gain from tile-local coordinates, and for a pair inside the primary cell
 // pj - pi is then the very difference the canonical predicate forms.  The OUTPUT keeps the formats of the generic fp64
-// kernels — list nl[k N + s] of plain sorted indices, records [N][16] = 13 components, f'(q6), q6, pad — so that every
+// kernels — list nl[k N + s] of plain sorted indices, records [N][16] = 13 components + position, q6 | f'(q6) arrays — so that every
 // downstream kernel (k_q6_force<double>, the virial instance, the exports, metad_cv_owned_sum) runs unchanged: this
 // kernel replaces k_build_list<double> + k_q6_pass1<double> (0.35 + 0.26 ms at 1,024,000 atoms) and nothing else.
 #include <algorithm>
@@ -112,7 +112,8 @@ __device__ __forceinline__ void finish_atom64(const TileGeom &g, const TileTable
                                               const double4 *pos_s, const nl16_t *list_s, int a, int col, int cnt, bool ovf,
                                               const BoxD &bd, double rc2, double rc2_lo, int maxn, int *__restrict__ nl_count,
                                               int *__restrict__ nl, unsigned int *__restrict__ sticky, double q_thresh,
-                                              double inv_width, double *__restrict__ rec, const DevGeom *__restrict__ dg,
+                                              double inv_width, double *__restrict__ rec, double *__restrict__ q6arr,
+                                              const DevGeom *__restrict__ dg,
                                               double &q6_out, double &f_out) {
     const int q = tile_own_row(t, a);
     const int o = a - t.own_off[q];
@@ -160,12 +161,14 @@ __device__ __forceinline__ void finish_atom64(const TileGeom &g, const TileTable
     double q6 = 0.0, norm = 0.0;
     if (n > 0 && S > 0.0) { const double rs = sqrt(S); q6 = rs / (double)n; norm = 1.0 / ((double)n * rs); }
     const double f = 1.0 / (1.0 + exp(-(q6 - q_thresh) * inv_width));
-    // record of the generic fp64 kernels (cv.cu: k_q6_pass1): B_m = conj(A_m) / (n sqrt(S)); [13] = f'(q6); [14] = q6
+    // record of the generic fp64 kernels (cv.cu: k_q6_pass1): B_m = conj(A_m) / (n sqrt(S)); [13..15] = the atom's position;
+    // q6 and f'(q6) go to the dense per-atom arrays
     double4 *r4 = reinterpret_cast<double4 *>(rec + (size_t)s * METAD_NREC);
     r4[0] = make_double4(A[0] * norm, A[1] * norm, -A[2] * norm, A[3] * norm);
     r4[1] = make_double4(-A[4] * norm, A[5] * norm, -A[6] * norm, A[7] * norm);
     r4[2] = make_double4(-A[8] * norm, A[9] * norm, -A[10] * norm, A[11] * norm);
-    r4[3] = make_double4(-A[12] * norm, f * (1.0 - f) * inv_width, q6, 0.0);
+    r4[3] = make_double4(-A[12] * norm, pi.x, pi.y, pi.z);             // own atoms are never periodic images: pi is the raw position
+    q6arr[s] = q6; q6arr[N + s] = f * (1.0 - f) * inv_width;
     q6_out = q6; f_out = f;
 }
 
@@ -174,7 +177,7 @@ __device__ __forceinline__ void build_body64(const TileGeom &g, const TileTables
                                              const double4 *pos_s, nl16_t *list_s, const int *__restrict__ scell,
                                              const BoxD &bd, double rc2, int maxn, int *__restrict__ nl_count,
                                              int *__restrict__ nl, unsigned int *__restrict__ sticky, double q_thresh,
-                                             double inv_width, double *__restrict__ rec, double (&v)[2],
+                                             double inv_width, double *__restrict__ rec, double *__restrict__ q6arr, double (&v)[2],
                                              const DevGeom *__restrict__ dg) {
     const double rc2_hi = rc2 * (1.0 + 1e-9), rc2_lo = rc2 * (1.0 - 1e-9);
     const int tid = threadIdx.x;
@@ -183,7 +186,7 @@ __device__ __forceinline__ void build_body64(const TileGeom &g, const TileTables
         const int cnt = scan_atom64<STAGED>(g, t, spos, pos_s, list_s, scell, a, tid, rc2_hi, ovf, dg);
         double q6, f;
         finish_atom64<STAGED>(g, t, spos, pos_s, list_s, a, tid, cnt, ovf, bd, rc2, rc2_lo, maxn, nl_count, nl, sticky,
-                              q_thresh, inv_width, rec, dg, q6, f);
+                              q_thresh, inv_width, rec, q6arr, dg, q6, f);
         v[0] += q6; v[1] += f;
     }
 }
@@ -192,7 +195,7 @@ __global__ void __launch_bounds__(TILE_THREADS, TILE64_MINB)
 k_tile_build64(TileGeom g, const double4 *__restrict__ spos, const int *__restrict__ scell,
                const int *__restrict__ cell_start, BoxD bd, double rc2, int maxn,
                int *__restrict__ nl_count, int *__restrict__ nl, unsigned int *__restrict__ sticky,
-               double q_thresh, double inv_width, double *__restrict__ rec,
+               double q_thresh, double inv_width, double *__restrict__ rec, double *__restrict__ q6arr /* [N] q6 | [N] f'(q6) */,
                double *__restrict__ partials, unsigned int *__restrict__ ticket, double scale_mean, double scale_solid,
                double *__restrict__ cv_q6 /* [2]: Q6 mean, solid count */,
                double *__restrict__ cv_out /* the context's CV vector on the run paths, else NULL (k_q6_publish) */,
@@ -213,9 +216,9 @@ k_tile_build64(TileGeom g, const double4 *__restrict__ spos, const int *__restri
         if (t.total > 65535) {
             if (threadIdx.x == 0) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
         } else if (t.staged) {
-            build_body64<true>(g, t, spos, pos_s, list_s, scell, bd, rc2, maxn, nl_count, nl, sticky, q_thresh, inv_width, rec, v, dg);
+            build_body64<true>(g, t, spos, pos_s, list_s, scell, bd, rc2, maxn, nl_count, nl, sticky, q_thresh, inv_width, rec, q6arr, v, dg);
         } else {
-            build_body64<false>(g, t, spos, pos_s, list_s, scell, bd, rc2, maxn, nl_count, nl, sticky, q_thresh, inv_width, rec, v, dg);
+            build_body64<false>(g, t, spos, pos_s, list_s, scell, bd, rc2, maxn, nl_count, nl, sticky, q_thresh, inv_width, rec, q6arr, v, dg);
         }
     }
     block_reduce<2>(v, red);
@@ -256,7 +259,7 @@ int tiled64_build(metad_ctx *c) {
     const double qw = c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].q_width : 1.0;
     klaunch_pdl(true, k_tile_build64, grid3, TILE_THREADS, smem_build64(g), c->stream,
                 g, (const double4 *)c->d_spos, (const int *)c->d_scell, (const int *)c->d_cell_start, c->boxd, c->rcl2, c->maxn,
-                c->d_nl_count, c->d_nl, c->d_sticky, qt, 1.0 / qw, (double *)c->d_rec,
+                c->d_nl_count, c->d_nl, c->d_sticky, qt, 1.0 / qw, (double *)c->d_rec, (double *)c->d_q6,
                 c->d_partials + c->nblocks_atoms, c->d_tickets + 1,
                 c->q6_mean_dim >= 0 ? c->cv[c->q6_mean_dim].scale : 0.0, c->q6_solid_dim >= 0 ? c->cv[c->q6_solid_dim].scale : 0.0,
                 c->d_cvq6, c->cv_direct, c->q6_mean_dim, c->q6_solid_dim, (const DevGeom *)c->dg);
