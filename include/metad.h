@@ -263,7 +263,7 @@ int metad_reset_steps(metad_ctx *ctx);
 
 /* Kernel-level timing for bench.py: when enabled, metad_build_neighbors records CUDA events around its
  * sort phase (binning, scan, scatter, in-cell sort + gather) and its list phase (candidate scan; on the tiled
- * fp32 path fused with Q6 pass 1).  metad_get_timing [sync] returns the last two durations in ms.
+ * paths, fp32 and fp64, fused with Q6 pass 1).  metad_get_timing [sync] returns the last two durations in ms.
  * Not usable inside metad_run (events are not recorded during graph capture). */
 int metad_set_timing(metad_ctx *ctx, int enabled);
 int metad_get_timing(metad_ctx *ctx, float *h_ms_sort, float *h_ms_list);
