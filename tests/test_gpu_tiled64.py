@@ -146,3 +146,36 @@ def test_tiled_fp64_dense_blob_unstaged_tiles_and_overflow(rc_over_a, overflow):
     md.close()
     wg = Workload(name="blob", pos=pos, box=box, rc=rc, max_neigh=33, cvs=w.cvs, sigma=[0.1], n_hills=4, precision=64)
     assert _kernel_nodes(w) == _kernel_nodes(wg) - 1                  # the tiled path did run
+
+
+def test_tiled_fp64_device_resident_box_changing_every_step():
+    """NEXT-3 on the tiled fp64 path: the box lives in device memory and is rescaled every step (metad_run_dev: one capture, no
+    update); k_tile_build64 takes the lattice rows of its periodic images and of the recheck from the device geometry.  Every step
+    against the oracle."""
+    w = configs.small("c4")
+    w.stride = 2
+    frac = np.linalg.solve(w.box.reshape(3, 3).T, w.pos.T).T
+    box0 = w.box.copy()
+    scales = [1.0, 1.003, 0.99, 1.012, 1.02, 0.985, 1.0]
+    r = chained_run(w, precision=64, nsteps=len(scales), device_box=True, box_slack=0.03,
+                    box_of_step=lambda k: box0 * scales[k], pos_of_step=lambda k: frac @ (box0 * scales[k]).reshape(3, 3),
+                    check_neighbors=True)
+    gi = r["md"].graph_info()
+    assert gi["captures"] == 1 and gi["updates"] == 0
+    assert gi["nodes"] == gi["kernel"] == 9          # k_geom_update + five sort kernels + k_tile_build64 + hill sum + forces
+    assert r["md"].status() == 0
+
+
+@pytest.mark.parametrize("name", ["c3", "c4"])
+def test_tiled_fp64_virial(name):
+    """Bias virial of the Q6 CVs with the list and the records written by k_tile_build64 (k_q6_force<double, VIRIAL>) against the
+    oracle's strain derivatives (reading AD) at the fp64 bar of tests/test_gpu_virial.py."""
+    w = configs.small(name)
+    r = stagewise(w, precision=64, want_virial=True)
+    assert_stagewise(r, tol_cv=1e-12, tol_f=1e-11)
+    W = r["md"].virial()
+    W_ref = r["o"].virial(r["dV_ref"])
+    assert np.abs(W_ref).max() > 0
+    assert np.abs(W - W_ref).max() <= 1e-9 * np.abs(W_ref).max(), (W, W_ref)
+    if name == "c3":
+        assert abs(np.trace(W)) <= 1e-9 * np.abs(W).max()      # Q6 is scale-invariant: traceless virial
