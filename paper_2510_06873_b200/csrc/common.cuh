@@ -68,6 +68,13 @@ __device__ __forceinline__ typename Vec4<T>::type ld4(const typename Vec4<T>::ty
 template <typename T>
 __device__ __forceinline__ typename Vec4<T>::type ldg4(const typename Vec4<T>::type *p);
 template <> __device__ __forceinline__ float4 ldg4<float>(const float4 *p) { return *p; }
+// one 256-bit store of a double4 (st.global.v4.f64; 32-byte aligned address)
+__device__ __forceinline__ void stg4(double4 *p, const double4 &v) {
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(v.x), "d"(v.y), "d"(v.z), "d"(v.w) : "memory");
+}
+template <typename T> __device__ __forceinline__ void st4(typename Vec4<T>::type *p, const typename Vec4<T>::type &v);
+template <> __device__ __forceinline__ void st4<float>(float4 *p, const float4 &v) { *p = v; }
+template <> __device__ __forceinline__ void st4<double>(double4 *p, const double4 &v) { stg4(p, v); }
 template <> __device__ __forceinline__ double4 ldg4<double>(const double4 *p) {
     double4 v;
     asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));

@@ -265,7 +265,7 @@ k_q6_pass1(int N, const typename Vec4<T>::type *__restrict__ spos, const int *__
         for (int q = 0; q < 4; ++q) {
             typename Vec4<T>::type w;
             w.x = out[4 * q]; w.y = out[4 * q + 1]; w.z = out[4 * q + 2]; w.w = out[4 * q + 3];
-            r4[q] = w;
+            st4<T>(r4 + q, w);
         }
         v[0] = (double)q6; v[1] = (double)fsw;
     }

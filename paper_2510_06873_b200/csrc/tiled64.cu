@@ -6,7 +6,7 @@
 //   finish  the exact decision on that short list — pairs within the 1e-9 band of rc^2 are re-decided with the canonical
 //           predicate of reading O on the original coordinates, so the sets are bit-exact —, the neighbour-list write and
 //           the atom's 13 q6m components by the Y6m recurrence, all in fp64.
-// What differs from the fp32 kernel: the halo is staged as RAW coordinates (plus the lattice shift of a periodic image,
+// What differs from the fp32 kernel: the halo is staged (as a structure of arrays) in RAW coordinates (plus the lattice shift of a periodic image,
 // added once): in fp64 there is no exactness to gain from tile-local coordinates, and for a pair inside the primary cell
 // pj - pi is then the very difference the canonical predicate forms.  The OUTPUT keeps the formats of the generic fp64
 // kernels — list nl[k N + s] of plain sorted indices, records [N][16] = 13 components + position, q6 | f'(q6) arrays — so that every
@@ -19,7 +19,15 @@
 
 typedef unsigned short nl16_t;   // local halo index (shared-memory candidate list only)
 #define LIST_CAP64 40            // per-thread candidate slots (maxn <= 32 on this path + band + self)
-#define TILE64_MINB 3            // resident blocks per SM: 38.9 KB of staged positions + 20 KB of candidate lists + tables
+#define TILE64_MINB 3            // resident blocks per SM: 34 KB of staged positions + 20 KB of candidate lists + tables
+
+// Shared-memory staging area, structure of arrays: (x, y) pairs, z and the global sorted index of every halo atom.  An array of
+// double4 would put the 16 bytes a lane reads at a 32-byte stride: two-way bank conflicts on the 128-bit load and four-way on
+// the 64-bit one (profiles/r2l_fp64.md: the scan sat at 77 % of the shared-memory wavefronts); with 16- and 8-byte strides both
+// loads are conflict-free.
+struct Stage64 { double2 *xy; double *z; int *idx; };
+#define STAGE64_BYTES 28         // per staged atom
+struct P64 { double x, y, z; int j; };
 
 // staged position of a halo atom: (x, y, z) of the image this tile sees, .w = its global sorted index
 __device__ __forceinline__ double4 tile_transform64(const TileGeom &g, const TileTables &t, int seg, double4 p, int gidx,
@@ -37,33 +45,45 @@ __device__ __forceinline__ double4 tile_transform64(const TileGeom &g, const Til
 }
 
 __device__ __forceinline__ void tile_stage_pos64(const TileGeom &g, const TileTables &t, const double4 *__restrict__ spos,
-                                                 double4 *pos_s, const DevGeom *dg) {
+                                                 const Stage64 &pos_s, const DevGeom *dg) {
     if (!t.staged) return;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     for (int s = wid; s < 3 * t.nrows; s += nw) {
         const int len = t.seg_len[s], g0 = t.seg_g[s], l0 = t.seg_off[s];
-        for (int i = lane; i < len; i += 32) pos_s[l0 + i] = tile_transform64(g, t, s, spos[g0 + i], g0 + i, dg);
+        for (int i = lane; i < len; i += 32) {
+            const double4 p = tile_transform64(g, t, s, ldg4<double>(spos + g0 + i), g0 + i, dg);
+            pos_s.xy[l0 + i] = make_double2(p.x, p.y);
+            pos_s.z[l0 + i] = p.z;
+            pos_s.idx[l0 + i] = g0 + i;
+        }
     }
 }
 
 template <bool STAGED>
-__device__ __forceinline__ double4 hpos64(const TileGeom &g, const TileTables &t, const double4 *__restrict__ spos,
-                                          const double4 *pos_s, int li, const DevGeom *dg) {
-    if (STAGED) return pos_s[li];
+__device__ __forceinline__ P64 hpos64(const TileGeom &g, const TileTables &t, const double4 *__restrict__ spos,
+                                      const Stage64 &pos_s, int li, const DevGeom *dg) {
+    P64 o;
+    if (STAGED) {
+        const double2 xy = pos_s.xy[li];
+        o.x = xy.x; o.y = xy.y; o.z = pos_s.z[li]; o.j = pos_s.idx[li];
+        return o;
+    }
     const int s = tile_seg_of(t, li);          // halo larger than the staging area: global memory, segment by binary search
     const int gi = t.seg_g[s] + (li - t.seg_off[s]);
-    return tile_transform64(g, t, s, spos[gi], gi, dg);
+    const double4 p = tile_transform64(g, t, s, spos[gi], gi, dg);
+    o.x = p.x; o.y = p.y; o.z = p.z; o.j = gi;
+    return o;
 }
 
 // candidate scan of own atom a into list column `col`; returns the number of candidates kept
 template <bool STAGED>
 __device__ __forceinline__ int scan_atom64(const TileGeom &g, const TileTables &t, const double4 *__restrict__ spos,
-                                           const double4 *pos_s, nl16_t *list_s, const int *__restrict__ scell, int a, int col,
+                                           const Stage64 &pos_s, nl16_t *list_s, const int *__restrict__ scell, int a, int col,
                                            double rc2_hi, bool &ovf, const DevGeom *dg) {
     const int q = tile_own_row(t, a);
     const int o = a - t.own_off[q];
     const int li = t.own_l[q] + o, s = t.own_g[q] + o;
-    const double4 pi = hpos64<STAGED>(g, t, spos, pos_s, li, dg);
+    const P64 pi = hpos64<STAGED>(g, t, spos, pos_s, li, dg);
     const int ic = scell[s] % g.nc0 - t.x0 + g.hx;       // halo-cell column of the own atom
     const int r0 = t.own_row[q], rstride = t.Tye + 2;
     const unsigned STRIDE = TILE_THREADS * (unsigned)sizeof(nl16_t);
@@ -84,14 +104,13 @@ __device__ __forceinline__ int scan_atom64(const TileGeom &g, const TileTables &
                 const int h2 = min(hi, lo + room);
 #pragma unroll 2
                 for (int lj = lo; lj < h2; ++lj) {
-                    // staged: 24 of the 32 bytes (one 128-bit + one 64-bit shared-memory load: the scan is bound by
-                    // shared-memory wavefronts, profiles/r2l_fp64.md); the index in .w is read by the exact pass only
+                    // staged: one 128-bit and one 64-bit conflict-free shared-memory load; the index is read by the exact pass only
                     double ex, ey, ez;
                     if (STAGED) {
-                        const double2 xy = *reinterpret_cast<const double2 *>(pos_s + lj);
-                        ex = xy.x - pi.x; ey = xy.y - pi.y; ez = reinterpret_cast<const double *>(pos_s + lj)[2] - pi.z;
+                        const double2 xy = pos_s.xy[lj];
+                        ex = xy.x - pi.x; ey = xy.y - pi.y; ez = pos_s.z[lj] - pi.z;
                     } else {
-                        const double4 pj = hpos64<STAGED>(g, t, spos, pos_s, lj, dg);
+                        const P64 pj = hpos64<STAGED>(g, t, spos, pos_s, lj, dg);
                         ex = pj.x - pi.x; ey = pj.y - pi.y; ez = pj.z - pi.z;
                     }
                     const double r2 = fma(ez, ez, fma(ey, ey, ex * ex));
@@ -109,7 +128,7 @@ __device__ __forceinline__ int scan_atom64(const TileGeom &g, const TileTables &
 // exact decision on the short list, neighbour-list write (generic layout), q6m accumulation, record; returns q6 and f(q6)
 template <bool STAGED>
 __device__ __forceinline__ void finish_atom64(const TileGeom &g, const TileTables &t, const double4 *__restrict__ spos,
-                                              const double4 *pos_s, const nl16_t *list_s, int a, int col, int cnt, bool ovf,
+                                              const Stage64 &pos_s, const nl16_t *list_s, int a, int col, int cnt, bool ovf,
                                               const BoxD &bd, double rc2, double rc2_lo, int maxn, int *__restrict__ nl_count,
                                               int *__restrict__ nl, unsigned int *__restrict__ sticky, double q_thresh,
                                               double inv_width, double *__restrict__ rec, double *__restrict__ q6arr,
@@ -119,7 +138,7 @@ __device__ __forceinline__ void finish_atom64(const TileGeom &g, const TileTable
     const int o = a - t.own_off[q];
     const int li = t.own_l[q] + o, s = t.own_g[q] + o;
     const size_t N = (size_t)g.natoms;
-    const double4 pi = hpos64<STAGED>(g, t, spos, pos_s, li, dg);
+    const P64 pi = hpos64<STAGED>(g, t, spos, pos_s, li, dg);
     const nl16_t *myl = list_s + col;
     if (ovf) atomicOr(sticky, (unsigned)METAD_DEV_NEIGH_OVERFLOW);
     double A[13];
@@ -129,10 +148,10 @@ __device__ __forceinline__ void finish_atom64(const TileGeom &g, const TileTable
     for (int k = 0; k < cnt; ++k) {
         const int lj = myl[k * TILE_THREADS];
         if (lj == li) continue;
-        const double4 pj = hpos64<STAGED>(g, t, spos, pos_s, lj, dg);
+        const P64 pj = hpos64<STAGED>(g, t, spos, pos_s, lj, dg);
         const double dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
         const double r2 = dx * dx + dy * dy + dz * dz;
-        const int j = (int)pj.w;
+        const int j = pj.j;
         bool in = r2 < rc2;
         if (r2 >= rc2_lo) {                                // borderline: canonical predicate on the original coordinates
             const double4 gi = spos[s], gj = spos[j];
@@ -164,17 +183,17 @@ __device__ __forceinline__ void finish_atom64(const TileGeom &g, const TileTable
     // record of the generic fp64 kernels (cv.cu: k_q6_pass1): B_m = conj(A_m) / (n sqrt(S)); [13..15] = the atom's position;
     // q6 and f'(q6) go to the dense per-atom arrays
     double4 *r4 = reinterpret_cast<double4 *>(rec + (size_t)s * METAD_NREC);
-    r4[0] = make_double4(A[0] * norm, A[1] * norm, -A[2] * norm, A[3] * norm);
-    r4[1] = make_double4(-A[4] * norm, A[5] * norm, -A[6] * norm, A[7] * norm);
-    r4[2] = make_double4(-A[8] * norm, A[9] * norm, -A[10] * norm, A[11] * norm);
-    r4[3] = make_double4(-A[12] * norm, pi.x, pi.y, pi.z);             // own atoms are never periodic images: pi is the raw position
+    stg4(r4, make_double4(A[0] * norm, A[1] * norm, -A[2] * norm, A[3] * norm));
+    stg4(r4 + 1, make_double4(-A[4] * norm, A[5] * norm, -A[6] * norm, A[7] * norm));
+    stg4(r4 + 2, make_double4(-A[8] * norm, A[9] * norm, -A[10] * norm, A[11] * norm));
+    stg4(r4 + 3, make_double4(-A[12] * norm, pi.x, pi.y, pi.z));       // own atoms are never periodic images: pi is the raw position
     q6arr[s] = q6; q6arr[N + s] = f * (1.0 - f) * inv_width;
     q6_out = q6; f_out = f;
 }
 
 template <bool STAGED>
 __device__ __forceinline__ void build_body64(const TileGeom &g, const TileTables &t, const double4 *__restrict__ spos,
-                                             const double4 *pos_s, nl16_t *list_s, const int *__restrict__ scell,
+                                             const Stage64 &pos_s, nl16_t *list_s, const int *__restrict__ scell,
                                              const BoxD &bd, double rc2, int maxn, int *__restrict__ nl_count,
                                              int *__restrict__ nl, unsigned int *__restrict__ sticky, double q_thresh,
                                              double inv_width, double *__restrict__ rec, double *__restrict__ q6arr, double (&v)[2],
@@ -204,8 +223,11 @@ k_tile_build64(TileGeom g, const double4 *__restrict__ spos, const int *__restri
     extern __shared__ double4 dyn_smem64[];
     __shared__ TileTables t;
     __shared__ double red[64];
-    double4 *pos_s = dyn_smem64;
-    nl16_t *list_s = reinterpret_cast<nl16_t *>(dyn_smem64 + g.cap);
+    Stage64 pos_s;
+    pos_s.xy = reinterpret_cast<double2 *>(dyn_smem64);
+    pos_s.z = reinterpret_cast<double *>(pos_s.xy + g.cap);
+    pos_s.idx = reinterpret_cast<int *>(pos_s.z + g.cap);
+    nl16_t *list_s = reinterpret_cast<nl16_t *>(pos_s.idx + g.cap);
     double v[2] = { 0.0, 0.0 };
     if (g.sparse && tile_is_empty(g, cell_start)) {
         // nothing to build here (block-uniform): the block only takes part in the reduction below
@@ -244,7 +266,7 @@ k_tile_build64(TileGeom g, const double4 *__restrict__ spos, const int *__restri
 TileGeom tile_geom(const metad_ctx *c);        // api.cu
 
 static size_t smem_build64(const TileGeom &g) {
-    return std::max(sizeof(double4) * (size_t)g.cap, (size_t)TILE_SCRATCH_BYTES) + sizeof(nl16_t) * LIST_CAP64 * TILE_THREADS;
+    return std::max((size_t)STAGE64_BYTES * (size_t)g.cap, (size_t)TILE_SCRATCH_BYTES) + sizeof(nl16_t) * LIST_CAP64 * TILE_THREADS;
 }
 
 int tiled64_init() {
