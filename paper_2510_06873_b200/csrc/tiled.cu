@@ -211,10 +211,14 @@ __device__ __forceinline__ void build_body(const TileGeom &g, const TileTables &
                                            const DevGeom *__restrict__ dg) {
     const float rc2_hi = rc2f * (1.f + 1e-5f), rc2_lo = rc2f * (1.f - 1e-5f);
     const int tid = threadIdx.x;
+    // list column of this thread: the two 16-bit halves of a 32-bit shared-memory word belong to the SAME lane of two
+    // neighbouring warps, so the lanes of a warp store to 32 different banks whatever slot each of them is at (with column =
+    // thread index, lanes 2i and 2i + 1 shared a bank and conflicted whenever their candidate counts differed)
+    const int col = ((((tid >> 6) << 5) + (tid & 31)) << 1) + ((tid >> 5) & 1);
     for (int a = tid; a < t.nown; a += blockDim.x) {
         bool ovf = false;
-        const int cnt = scan_atom<STAGED>(g, t, spos, pos_s, list_s, scell, a, tid, rc2_hi, ovf, dg);
-        const float q6 = finish_atom<STAGED, MODE>(g, t, spos, pos_s, list_s, a, tid, cnt, ovf, bd, rc2f, rc2_lo, rc2, maxn,
+        const int cnt = scan_atom<STAGED>(g, t, spos, pos_s, list_s, scell, a, col, rc2_hi, ovf, dg);
+        const float q6 = finish_atom<STAGED, MODE>(g, t, spos, pos_s, list_s, a, col, cnt, ovf, bd, rc2f, rc2_lo, rc2, maxn,
                                                    nl_count, nl, sticky, q_thresh, inv_width, rec, q6_out, solid, sw_n, sw_m, perm, dg);
         if (MODE != 0) v[0] += (double)q6;
         if (MODE == 1) v[1] += (double)(1.f / (1.f + expf(-(q6 - q_thresh) * inv_width)));

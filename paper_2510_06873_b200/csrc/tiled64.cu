@@ -200,11 +200,15 @@ __device__ __forceinline__ void build_body64(const TileGeom &g, const TileTables
                                              const DevGeom *__restrict__ dg) {
     const double rc2_hi = rc2 * (1.0 + 1e-9), rc2_lo = rc2 * (1.0 - 1e-9);
     const int tid = threadIdx.x;
+    // list column of this thread: the two 16-bit halves of a 32-bit shared-memory word belong to the SAME lane of two
+    // neighbouring warps, so the lanes of a warp store to 32 different banks whatever slot each of them is at (with column =
+    // thread index, lanes 2i and 2i + 1 shared a bank and conflicted whenever their candidate counts differed)
+    const int col = ((((tid >> 6) << 5) + (tid & 31)) << 1) + ((tid >> 5) & 1);
     for (int a = tid; a < t.nown; a += blockDim.x) {
         bool ovf = false;
-        const int cnt = scan_atom64<STAGED>(g, t, spos, pos_s, list_s, scell, a, tid, rc2_hi, ovf, dg);
+        const int cnt = scan_atom64<STAGED>(g, t, spos, pos_s, list_s, scell, a, col, rc2_hi, ovf, dg);
         double q6, f;
-        finish_atom64<STAGED>(g, t, spos, pos_s, list_s, a, tid, cnt, ovf, bd, rc2, rc2_lo, maxn, nl_count, nl, sticky,
+        finish_atom64<STAGED>(g, t, spos, pos_s, list_s, a, col, cnt, ovf, bd, rc2, rc2_lo, maxn, nl_count, nl, sticky,
                               q_thresh, inv_width, rec, q6arr, dg, q6, f);
         v[0] += q6; v[1] += f;
     }
